@@ -1,0 +1,350 @@
+/*
+ * tl_oracle.c -- FP64 CPU ORACLE for the batched lens-model likelihood.
+ *
+ * THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke() and
+ * bench.py's cpu_baseline / --impl reference legs may build, load or call it.  It shares no
+ * code, header, table or constant with the CUDA path under paper_2503_08586_b200/csrc/.
+ *
+ * What it is: the plain definition of the forward model of arxiv 2503.08586 (TinyLensGpu),
+ * written out with pixel loops in double precision, in the paper's order and notation.  There
+ * is no blocking, fusion or reordering.  Citations are PAPER.md:<line> (+ equation); where
+ * the paper is silent the reading is SURVEY.md 8(c) G<k>, repeated in DESIGN.md "Readings".
+ *
+ * Pinned (tests/test_oracle_pins.py, -m "not gpu") against closed forms, invariants, library
+ * routines and brute force: every exported function below has at least one pin, so nothing
+ * here is "parity unpinned".  The conventions G4, G5, G10, G13 are choices, not facts; the
+ * pins check the code implements the choice.
+ *
+ * Parameter row (float, widened exactly to double), P = 7 + 7*n_lens_light + 7*n_source:
+ *   theta_E, e1, e2, cx, cy, gamma1, gamma2,
+ *   then per Sersic (lens light first, then sources): I_e, r_e, n, e1, e2, cx, cy.
+ *
+ * Build: gcc -O2 -fopenmp -shared -fPIC -o liboracle.so tl_oracle.c -lm   (no -ffast-math)
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define ORC_EDGE_EXTEND 0
+#define ORC_EDGE_ZERO 1
+
+typedef struct {
+    int32_t ny, nx;
+    double pix_scale;
+    int32_t supersample;
+    int32_t n_lens_light;
+    int32_t n_source;
+    int32_t edge_mode;
+} orc_config;
+
+/* ------------------------------------------------------------------ Eq. 9: b_n
+ * PAPER.md:137-141 Eq. 9:  Gamma(2n) = 2 gamma(2n, b_n), i.e. P(2n, b_n) = 1/2 with P the
+ * regularised lower incomplete gamma function.  gamma(a,x) by its power series
+ *   gamma(a,x) = x^a e^{-x} sum_{k>=0} x^k / (a (a+1) ... (a+k)),
+ * always in its fast regime here because the root lies below a = 2n.  Root by bisection.
+ */
+double orc_gammainc_p(double a, double x)
+{
+    if (x <= 0.0) return 0.0;
+    double term = 1.0 / a, sum = term;
+    for (int k = 1; k < 100000; ++k) {
+        term *= x / (a + k);
+        sum += term;
+        if (term < sum * 1e-17) break;
+    }
+    return sum * exp(a * log(x) - x - lgamma(a));
+}
+
+double orc_bn(double n)
+{
+    double a = 2.0 * n;
+    double lo = 0.0, hi = a > 1.0 ? a : 1.0;     /* the median of Gamma(a,1) is below max(a,1)... */
+    while (orc_gammainc_p(a, hi) < 0.5) hi *= 2.0; /* ...and this loop makes the bracket unconditional */
+    for (int it = 0; it < 200; ++it) {
+        double mid = 0.5 * (lo + hi);
+        if (orc_gammainc_p(a, mid) < 0.5) lo = mid; else hi = mid;
+        if (hi - lo <= 1e-16 * hi) break;
+    }
+    return 0.5 * (lo + hi);
+}
+
+/* ------------------------------------------------------------------ Eq. 11 inverse
+ * PAPER.md:150-154 Eq. 11: (e1,e2) = (1-q)/(1+q) (cos 2phi, sin 2phi).  Inverse (G3):
+ * e = hypot(e1,e2), q = (1-e)/(1+e), phi = atan2(e2,e1)/2.  phi is the major-axis direction,
+ * counter-clockwise from +x (G2).
+ */
+void orc_shape(double e1, double e2, double *q, double *phi)
+{
+    double e = hypot(e1, e2);
+    *q = (1.0 - e) / (1.0 + e);
+    *phi = 0.5 * atan2(e2, e1);
+}
+
+/* ------------------------------------------------------------------ Eq. 12 (gamma = 2): SIE
+ * PAPER.md:156-160 Eq. 12 with gamma = 2 and R -> R_p of Eq. 10 ("extended to a two-
+ * dimensional elliptical distribution ... similar to the light profile"), Kormann et al.
+ * 1994 cited, no formula printed (G1):
+ *   kappa = theta_E / (2 sqrt(q x'^2 + y'^2 / q))        in the frame rotated by phi,
+ *   psi = sqrt(q^2 x'^2 + y'^2),  q' = sqrt((1-q)(1+q)),
+ *   alpha_x' = theta_E sqrt(q) (x'/psi) A(q' x'/psi),  A(z) = atan(z)/z,
+ *   alpha_y' = theta_E sqrt(q) (y'/psi) H(q' y'/psi),  H(z) = atanh(z)/z,
+ * A, H -> 1 as z -> 0 (series below |z| < 1e-4), alpha = 0 at psi = 0 (G6).
+ */
+static double fn_A(double z)
+{
+    if (fabs(z) < 1e-4) { double z2 = z * z; return 1.0 - z2 / 3.0 + z2 * z2 / 5.0; }
+    return atan(z) / z;
+}
+static double fn_H(double z)
+{
+    if (fabs(z) < 1e-4) { double z2 = z * z; return 1.0 + z2 / 3.0 + z2 * z2 / 5.0; }
+    return atanh(z) / z;
+}
+
+void orc_sie_deflection(double theta_e, double q, double phi, double cx, double cy,
+                        double x, double y, double *ax, double *ay)
+{
+    double c = cos(phi), s = sin(phi);
+    double dx = x - cx, dy = y - cy;
+    double xp = dx * c + dy * s;
+    double yp = -dx * s + dy * c;
+    double psi = sqrt(q * q * xp * xp + yp * yp);
+    if (psi == 0.0) { *ax = 0.0; *ay = 0.0; return; }
+    double qp = sqrt((1.0 - q) * (1.0 + q));
+    double axp = theta_e * sqrt(q) * (xp / psi) * fn_A(qp * xp / psi);
+    double ayp = theta_e * sqrt(q) * (yp / psi) * fn_H(qp * yp / psi);
+    *ax = axp * c - ayp * s;
+    *ay = axp * s + ayp * c;
+}
+
+/* PAPER.md:160-162 Eq. 13, :187-190 Eq. 14: psi_ext = -1/2 gamma theta^2 cos 2(phi - phi_ext)
+ * = -1/2 [gamma1 (x^2 - y^2) + 2 gamma2 x y] about the image origin (G4, G5);
+ * alpha = grad psi_ext.                                                                   */
+void orc_shear_deflection(double g1, double g2, double x, double y, double *ax, double *ay)
+{
+    *ax = -(g1 * x + g2 * y);
+    *ay = -(g2 * x - g1 * y);
+}
+
+/* PAPER.md:133-137 Eq. 8 with R -> R_p of PAPER.md:141-150 Eq. 10. */
+double orc_sersic(double i_e, double r_e, double n, double bn, double q, double phi,
+                  double cx, double cy, double x, double y)
+{
+    double c = cos(phi), s = sin(phi);
+    double x1 = (x - cx) * c + (y - cy) * s;
+    double x2 = -(x - cx) * s + (y - cy) * c;
+    double rp = sqrt(x1 * x1 * q + x2 * x2 / q);
+    return i_e * exp(-bn * (pow(rp / r_e, 1.0 / n) - 1.0));
+}
+
+/* ------------------------------------------------------------------ validity (boundary rule)
+ * include/tinylens.h: hypot(e1,e2) >= 1, theta_E < 0, r_e <= 0, n <= 0 or any non-finite
+ * value makes the row physically invalid: logL = -inf, image = NaN.                        */
+int orc_row_valid(const orc_config *cfg, const float *row)
+{
+    int ncomp = cfg->n_lens_light + cfg->n_source;
+    int P = 7 + 7 * ncomp;
+    for (int i = 0; i < P; ++i) if (!isfinite((double)row[i])) return 0;
+    if (row[0] < 0.0f) return 0;
+    if (hypot((double)row[1], (double)row[2]) >= 1.0) return 0;
+    for (int k = 0; k < ncomp; ++k) {
+        const float *s = row + 7 + 7 * k;
+        if (!(s[1] > 0.0f) || !(s[2] > 0.0f)) return 0;
+        if (hypot((double)s[3], (double)s[4]) >= 1.0) return 0;
+    }
+    return 1;
+}
+
+static int halo_of(const orc_config *cfg, int K) { return cfg->edge_mode == ORC_EDGE_EXTEND ? (K - 1) / 2 : 0; }
+
+/* ------------------------------------------------------------------ Eq. 1, 2 + supersample + bin
+ * Ideal (unblurred) image on the extended native grid (ny+2g) x (nx+2g), g = halo in EXTEND
+ * mode, 0 in ZERO mode (G10).  Grid (G13): native pixel (i,j), i = row, centre
+ *   x_j = (j - g - (nx-1)/2) s,  y_i = (i - g - (ny-1)/2) s,   s = pix_scale,
+ * sub-sample (a,b): x = x_j + ((b+1/2)/S - 1/2) s, y = y_i + ((a+1/2)/S - 1/2) s.
+ * Sample value (Eq. 2): sum of lens-light Sersics at theta plus source Sersics
+ * at beta = theta - alpha (Eq. 1).  Native pixel = mean of S^2 samples
+ * (G9).
+ */
+void orc_ideal_image(const orc_config *cfg, int g, const float *row, double *img)
+{
+    int S = cfg->supersample, ny = cfg->ny, nx = cfg->nx;
+    int hy = ny + 2 * g, wx = nx + 2 * g;
+    double s = cfg->pix_scale;
+    double theta_e = row[0], q, phi;
+    orc_shape(row[1], row[2], &q, &phi);
+    double lcx = row[3], lcy = row[4], g1 = row[5], g2 = row[6];
+    int ncomp = cfg->n_lens_light + cfg->n_source;
+    double cq[8], cphi[8], cbn[8];
+    for (int k = 0; k < ncomp && k < 8; ++k) {
+        const float *c = row + 7 + 7 * k;
+        orc_shape(c[3], c[4], &cq[k], &cphi[k]);
+        cbn[k] = orc_bn(c[2]);
+    }
+    for (int i = 0; i < hy; ++i) {
+        double yi = (i - g - (ny - 1) / 2.0) * s;
+        for (int j = 0; j < wx; ++j) {
+            double xj = (j - g - (nx - 1) / 2.0) * s;
+            double acc = 0.0;
+            for (int a = 0; a < S; ++a) {
+                double y = yi + ((a + 0.5) / S - 0.5) * s;
+                for (int b = 0; b < S; ++b) {
+                    double x = xj + ((b + 0.5) / S - 0.5) * s;
+                    double ax, ay, sx, sy;
+                    orc_sie_deflection(theta_e, q, phi, lcx, lcy, x, y, &ax, &ay);
+                    orc_shear_deflection(g1, g2, x, y, &sx, &sy);
+                    double bx = x - (ax + sx), by = y - (ay + sy);          /* Eq. 1 */
+                    double v = 0.0;
+                    for (int k = 0; k < ncomp; ++k) {
+                        const float *c = row + 7 + 7 * k;
+                        int is_lens = k < cfg->n_lens_light;
+                        v += orc_sersic(c[0], c[1], c[2], cbn[k], cq[k], cphi[k], c[5], c[6],
+                                        is_lens ? x : bx, is_lens ? y : by);  /* Eq. 2 */
+                    }
+                    acc += v;
+                }
+            }
+            img[(size_t)i * wx + j] = acc / (double)(S * S);
+        }
+    }
+}
+
+/* ------------------------------------------------------------------ Eq. 3: PSF convolution
+ * PAPER.md:67-71 Eq. 3, true convolution, kernel used as given (G11):
+ *   Im[i,j] = sum_{a,b} K[a,b] I[i-(a-h), j-(b-h)],  h = (K-1)/2,
+ * I indexed in native pixels; img holds native index -g..n-1+g (g = h for EXTEND, so every
+ * tap is inside; g = 0 for ZERO, taps outside the cutout read 0) (G10).
+ */
+void orc_convolve(int ny, int nx, int g, const double *img, const float *psf, int K, double *out)
+{
+    int h = (K - 1) / 2, wx = nx + 2 * g, hy = ny + 2 * g;
+    for (int i = 0; i < ny; ++i)
+        for (int j = 0; j < nx; ++j) {
+            double acc = 0.0;
+            for (int a = 0; a < K; ++a)
+                for (int b = 0; b < K; ++b) {
+                    int ii = i - (a - h) + g, jj = j - (b - h) + g;
+                    if (ii < 0 || ii >= hy || jj < 0 || jj >= wx) continue;
+                    acc += (double)psf[a * K + b] * img[(size_t)ii * wx + jj];
+                }
+            out[(size_t)i * nx + j] = acc;
+        }
+}
+
+/* Whole forward model for one row: I^m [ny][nx].  Returns 0 for an invalid row
+ * (image filled with NaN), 1 otherwise.                                                    */
+int orc_render(const orc_config *cfg, const float *psf, int K, const float *row, double *image)
+{
+    size_t n = (size_t)cfg->ny * cfg->nx;
+    if (!orc_row_valid(cfg, row)) { for (size_t i = 0; i < n; ++i) image[i] = NAN; return 0; }
+    int g = halo_of(cfg, K);
+    double *ext = (double *)malloc(sizeof(double) * (size_t)(cfg->ny + 2 * g) * (cfg->nx + 2 * g));
+    orc_ideal_image(cfg, g, row, ext);
+    orc_convolve(cfg->ny, cfg->nx, g, ext, psf, K, image);
+    free(ext);
+    return 1;
+}
+
+/* ------------------------------------------------------------------ Eq. 5: Gaussian likelihood
+ * PAPER.md:80-84 Eq. 5: logL = -1/2 sum_i [ (d_i - Im_i)^2 / sigma_i^2 + ln(2 pi sigma_i^2) ]
+ * (normalisation included, G12), Kahan-summed.                                             */
+double orc_loglike_from_image(const double *image, const float *data, const float *noise, size_t n)
+{
+    double sum = 0.0, comp = 0.0;
+    for (size_t i = 0; i < n; ++i) {
+        double sg = noise[i], r = ((double)data[i] - image[i]) / sg;
+        double t = r * r + log(2.0 * M_PI * sg * sg);
+        double yk = t - comp, tk = sum + yk;
+        comp = (tk - sum) - yk;
+        sum = tk;
+    }
+    return -0.5 * sum;
+}
+
+double orc_chi2_from_image(const double *image, const float *data, const float *noise, size_t n)
+{
+    double sum = 0.0, comp = 0.0;
+    for (size_t i = 0; i < n; ++i) {
+        double r = ((double)data[i] - image[i]) / (double)noise[i];
+        double yk = r * r - comp, tk = sum + yk;
+        comp = (tk - sum) - yk;
+        sum = tk;
+    }
+    return sum;
+}
+
+double orc_loglike(const orc_config *cfg, const float *psf, int K, const float *data,
+                   const float *noise, const float *row)
+{
+    size_t n = (size_t)cfg->ny * cfg->nx;
+    double *image = (double *)malloc(sizeof(double) * n);
+    double r;
+    if (!orc_render(cfg, psf, K, row, image)) r = -INFINITY;
+    else r = orc_loglike_from_image(image, data, noise, n);
+    free(image);
+    return r;
+}
+
+/* ------------------------------------------------------------------ batches (rows independent)
+ * n_lens > 1: psf/data/noise hold n_lens blocks, row r belongs to lens r / (B / n_lens).
+ * OpenMP over rows; `threads` <= 0 means the OpenMP default.  Returns threads used.        */
+int orc_loglike_batch(const orc_config *cfg, int n_lens, const float *psf, int K, const float *data,
+                      const float *noise, const float *rows, int64_t B, double *logl, int threads)
+{
+    int P = 7 + 7 * (cfg->n_lens_light + cfg->n_source);
+    size_t n = (size_t)cfg->ny * cfg->nx;
+    int64_t per = B / (n_lens > 0 ? n_lens : 1);
+    int used = 1;
+#ifdef _OPENMP
+    if (threads > 0) omp_set_num_threads(threads);
+#pragma omp parallel
+    {
+#pragma omp single
+        used = omp_get_num_threads();
+#pragma omp for schedule(dynamic, 1)
+        for (int64_t r = 0; r < B; ++r) {
+            int64_t l = n_lens > 1 ? r / per : 0;
+            logl[r] = orc_loglike(cfg, psf + (size_t)l * K * K, K, data + l * n, noise + l * n,
+                                  rows + r * P);
+        }
+    }
+#else
+    for (int64_t r = 0; r < B; ++r) {
+        int64_t l = n_lens > 1 ? r / per : 0;
+        logl[r] = orc_loglike(cfg, psf + (size_t)l * K * K, K, data + l * n, noise + l * n, rows + r * P);
+    }
+#endif
+    return used;
+}
+
+int orc_render_batch(const orc_config *cfg, int n_lens, const float *psf, int K, const float *rows,
+                     int64_t B, double *images, int threads)
+{
+    int P = 7 + 7 * (cfg->n_lens_light + cfg->n_source);
+    size_t n = (size_t)cfg->ny * cfg->nx;
+    int64_t per = B / (n_lens > 0 ? n_lens : 1);
+    int used = 1;
+#ifdef _OPENMP
+    if (threads > 0) omp_set_num_threads(threads);
+#pragma omp parallel
+    {
+#pragma omp single
+        used = omp_get_num_threads();
+#pragma omp for schedule(dynamic, 1)
+        for (int64_t r = 0; r < B; ++r) {
+            int64_t l = n_lens > 1 ? r / per : 0;
+            orc_render(cfg, psf + (size_t)l * K * K, K, rows + r * P, images + r * n);
+        }
+    }
+#else
+    for (int64_t r = 0; r < B; ++r) {
+        int64_t l = n_lens > 1 ? r / per : 0;
+        orc_render(cfg, psf + (size_t)l * K * K, K, rows + r * P, images + r * n);
+    }
+#endif
+    return used;
+}
