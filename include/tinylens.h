@@ -1,0 +1,156 @@
+/*
+ * tinylens.h -- C ABI of the B200-native batched lens-model likelihood.
+ *
+ * The library evaluates, for a batch of B parameter vectors, the forward model of
+ * arxiv 2503.08586 (TinyLensGpu) and its Gaussian log-likelihood, entirely in hand-written
+ * sm_100a CUDA kernels.  There is NO CPU fallback: every compute entry point returns
+ * TL_ECUDA when no CUDA device is usable.
+ *
+ * Citations are PAPER.md:<line> (+ equation) of the paper text; "G<k>" are the readings of
+ * points the paper leaves open, listed in DESIGN.md "Readings of the paper".
+ *
+ * The operation (per parameter row; PAPER.md:52-71 section 2.1, :80-84 Eq. 5, :133-162 section 2.4):
+ *   1. every S x S sub-sample theta of every native pixel ("4x4 supersampling")
+ *      is ray-traced, beta = theta - alpha(theta)                       (Eq. 1),
+ *      alpha = SIE (EPL with gamma = 2, Eq. 12) + external shear
+ *      (PAPER.md:162 Eq. 13, :187-190 Eq. 14);
+ *   2. I(theta) = sum_lens-light Sersic(theta) + sum_sources Sersic(beta)  (Eq. 2)
+ *      with the elliptical Sersic profile of PAPER.md:135 Eq. 8, :139 Eq. 9 (b_n), :143-148 Eq. 10;
+ *   3. the S*S samples of a native pixel are averaged ("binning");
+ *   4. the binned image is convolved with the PSF kernel K               (Eq. 3);
+ *   5. logL = -1/2 sum_i [ (d_i - Im_i)^2 / sigma_i^2 + ln(2 pi sigma_i^2) ]  (Eq. 5).
+ *
+ * Conventions (G2, G4, G5, G10, G11, G13): angles in arcsec, origin at the image
+ * centre, native pixel (i, j) (i = row) centred at x = (j - (nx-1)/2) s, y = (i - (ny-1)/2) s,
+ * row index increases with +y; phi is the major-axis direction counter-clockwise from +x;
+ * shear taken about the image origin with the sign of Eq. 13; true convolution with the PSF
+ * used as given (not renormalised, odd sizes only).
+ *
+ * Parameter row layout, P = 7 + 7*n_lens_light + 7*n_source floats:
+ *   [0] theta_E  [1] e1  [2] e2  [3] cx  [4] cy          SIE (ellipticities: Eq. 11)
+ *   [5] gamma1   [6] gamma2                               external shear
+ *   then per Sersic component, lens light first, then sources:
+ *   [+0] I_e  [+1] r_e  [+2] n  [+3] e1  [+4] e2  [+5] cx  [+6] cy
+ *
+ * Invalid rows are not errors: hypot(e1,e2) >= 1, theta_E < 0, r_e <= 0, n <= 0 or any
+ * non-finite entry gives logL = -INFINITY and a NaN-filled image for that row.
+ *
+ * Threading: a context is immutable after tl_create and may be used from several host
+ * threads / streams concurrently; per-call scratch comes from the stream-ordered allocator.
+ */
+#ifndef TINYLENS_H
+#define TINYLENS_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TL_OK       0
+#define TL_EINVAL  -1   /* bad shape, even PSF size, null pointer, noise not finite/positive  */
+#define TL_ENOMEM  -2   /* host or device allocation failed                                   */
+#define TL_ECUDA   -3   /* no usable CUDA device, or a CUDA runtime call failed               */
+#define TL_ESIZE   -4   /* configuration exceeds what the kernels support (see tl_create)     */
+
+#define TL_EDGE_EXTEND 0 /* evaluate the analytic model on a border of h = (K-1)/2 pixels so   */
+                         /* every output pixel sees its full PSF support (Eq. 3 with only the  */
+                         /* kernel truncated; G10)                                   */
+#define TL_EDGE_ZERO   1 /* model taken as zero outside the cutout ('same' zero-padded conv)   */
+
+typedef struct tl_ctx tl_ctx;     /* opaque; owned by the library */
+
+typedef struct {
+    int32_t ny, nx;          /* native image size (rows, columns)                              */
+    double  pix_scale;       /* arcsec per native pixel, > 0                                   */
+    int32_t supersample;     /* S >= 1: S x S samples per native pixel, S <= 16  */
+    int32_t n_lens_light;    /* 0 or 1 Sersic components evaluated at theta                    */
+    int32_t n_source;        /* 1 or 2 Sersic components evaluated at beta                     */
+    int32_t edge_mode;       /* TL_EDGE_EXTEND or TL_EDGE_ZERO                                 */
+    int32_t n_lens;          /* 1, or L for a heterogeneous batch of L lenses (own psf, data,  */
+                             /* noise per lens; row r of a B-row call belongs to lens          */
+                             /* r / (B / L), B must be a multiple of L)                        */
+} tl_config;
+
+/* What a context will launch; filled by tl_get_info (for benchmarks and reports).             */
+typedef struct {
+    int32_t n_params;          /* P                                                            */
+    int32_t path;              /* 0 = fused (binned image in shared memory), 1 = split (binned  */
+                               /*     image staged through global memory, for large images)    */
+    int32_t block_threads;     /* threads per CTA of the dominant kernel                       */
+    int32_t ctas_per_sm;       /* resident CTAs per SM of the dominant kernel                  */
+    int32_t grid;              /* CTAs launched (persistent: n_sm * ctas_per_sm)                */
+    int32_t smem_bytes;        /* dynamic shared memory per CTA                                */
+    int32_t n_sm;              /* SMs of the device                                            */
+    int32_t launches_per_call; /* kernels launched by one tl_loglike_batch                     */
+    int64_t samples_per_row;   /* ray-traced sub-samples per likelihood                        */
+    int64_t conv_fma_per_row;  /* K*K*ny*nx                                                    */
+    double  logl_const;        /* lens 0:  sum_i ln(2 pi sigma_i^2)                            */
+    double  sigma_min;         /* lens 0:  min_i sigma_i                                       */
+} tl_info;
+
+/*
+ * tl_create -- build an immutable context (image d, noise sigma,
+ * PSF kernel K are fixed per lens; only the parameter vector varies between evaluations).
+ *   out        receives the handle (set to NULL on failure)
+ *   cfg        see tl_config
+ *   psf        HOST pointer, float [n_lens][psf_ny][psf_nx], psf_ny == psf_nx odd, row-major,
+ *              K[a][b] with a the row (y) index.  Used as given.
+ *   data       HOST pointer, float [n_lens][ny][nx], row-major (d_i of Eq. 5)
+ *   noise      HOST pointer, float [n_lens][ny][nx], every value finite and > 0 (sigma_i)
+ *   cuda_stream  a cudaStream_t (NULL = default stream) on which uploads are enqueued;
+ *              the call synchronises that stream before returning, so the host arrays may
+ *              be freed immediately.
+ * The arrays are copied; the caller keeps ownership of its buffers.  The context is bound to
+ * the CUDA device current at the time of the call.
+ * Returns TL_OK, TL_EINVAL, TL_ENOMEM, TL_ECUDA or TL_ESIZE (PSF larger than the image plus
+ * halo allows, or a tile that cannot fit in 227 KB of shared memory).
+ */
+int tl_create(tl_ctx **out, const tl_config *cfg,
+              const float *psf, int32_t psf_ny, int32_t psf_nx,
+              const float *data, const float *noise, void *cuda_stream);
+
+/* Number of floats per parameter row, P = 7 + 7*n_lens_light + 7*n_source; < 0 on NULL.       */
+int tl_param_count(const tl_ctx *ctx);
+
+/* Launch geometry and sizes of this context.  Returns TL_OK or TL_EINVAL.                     */
+int tl_get_info(const tl_ctx *ctx, tl_info *info);
+
+/*
+ * tl_loglike_batch -- logL[r] (Eq. 5, normalisation included) for r = 0..B-1.
+ *   params     DEVICE pointer, float [B][P] row-major, caller-owned, read only
+ *   B          rows (>= 0; multiple of n_lens)
+ *   logL       DEVICE pointer, float [B], caller-owned, written
+ *   cuda_stream  stream the kernels are enqueued on.  The call does NOT synchronise.
+ * The result is bitwise reproducible (fixed-shape FP64 reduction, no atomics).
+ */
+int tl_loglike_batch(tl_ctx *ctx, const float *params, int64_t B, float *logL, void *cuda_stream);
+
+/*
+ * tl_render_batch -- the blurred model images Im for every row.
+ *   images     DEVICE pointer, float [B][ny][nx], caller-owned, written (NaN for invalid rows)
+ * Same arithmetic as tl_loglike_batch up to and including the PSF convolution.
+ */
+int tl_render_batch(tl_ctx *ctx, const float *params, int64_t B, float *images, void *cuda_stream);
+
+/*
+ * tl_loglike_batch_host -- end-to-end convenience for a host-side sampler (PAPER.md:250 names
+ * the CPU<->GPU transfers as part of the cost): copies params (HOST, float [B][P], ideally
+ * pinned) to the device, runs tl_loglike_batch, copies logL back to logL (HOST, float [B]),
+ * and synchronises the stream before returning.
+ */
+int tl_loglike_batch_host(tl_ctx *ctx, const float *params, int64_t B, float *logL, void *cuda_stream);
+
+/* Release a context and its device memory (NULL is allowed).                                  */
+void tl_destroy(tl_ctx *ctx);
+
+/* Static, never-NULL description of a return code.                                            */
+const char *tl_strerror(int code);
+
+/* Library version string, e.g. "tinylens-b200 0.1 (sm_100a)".                                 */
+const char *tl_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TINYLENS_H */

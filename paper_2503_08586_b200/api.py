@@ -1,0 +1,236 @@
+"""Thin Python binding of the C ABI in include/tinylens.h (argument marshalling only).
+
+Every step of the path runs in the CUDA kernels of csrc/; PyTorch supplies device memory and
+streams.  There is no CPU fallback: if the shared library is missing or no CUDA device is
+usable, the calls raise ``TinyLensError``.
+
+The functions carry the C names (``tl_create`` ...); ``LensContext`` is a small RAII wrapper.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libtinylens.so")
+
+TL_OK, TL_EINVAL, TL_ENOMEM, TL_ECUDA, TL_ESIZE = 0, -1, -2, -3, -4
+TL_EDGE_EXTEND, TL_EDGE_ZERO = 0, 1
+
+
+class TinyLensError(RuntimeError):
+    def __init__(self, code: int, what: str = ""):
+        self.code = code
+        msg = tl_strerror(code) if _lib is not None else "library not loaded"
+        super().__init__("%s: %s (code %d)" % (what, msg, code))
+
+
+class tl_config(C.Structure):
+    _fields_ = [("ny", C.c_int32), ("nx", C.c_int32), ("pix_scale", C.c_double),
+                ("supersample", C.c_int32), ("n_lens_light", C.c_int32), ("n_source", C.c_int32),
+                ("edge_mode", C.c_int32), ("n_lens", C.c_int32)]
+
+
+class tl_info(C.Structure):
+    _fields_ = [("n_params", C.c_int32), ("path", C.c_int32), ("block_threads", C.c_int32),
+                ("ctas_per_sm", C.c_int32), ("grid", C.c_int32), ("smem_bytes", C.c_int32),
+                ("n_sm", C.c_int32), ("launches_per_call", C.c_int32),
+                ("samples_per_row", C.c_int64), ("conv_fma_per_row", C.c_int64),
+                ("logl_const", C.c_double), ("sigma_min", C.c_double)]
+
+
+_lib = None
+
+
+def load(build_if_missing: bool = True):
+    """dlopen libtinylens.so (building it in-tree with nvcc when it is missing or stale)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if build_if_missing:
+        from . import build as _build
+        try:
+            _build.build()
+        except Exception:
+            if not os.path.exists(LIB_PATH):
+                raise
+    if not os.path.exists(LIB_PATH):
+        raise OSError("libtinylens.so not found at %s: run `python -m paper_2503_08586_b200.build`" % LIB_PATH)
+    L = C.CDLL(LIB_PATH)
+    vp, i32, i64, fp = C.c_void_p, C.c_int32, C.c_int64, C.POINTER(C.c_float)
+    L.tl_create.restype = C.c_int
+    L.tl_create.argtypes = [C.POINTER(vp), C.POINTER(tl_config), fp, i32, i32, fp, fp, vp]
+    L.tl_param_count.restype = C.c_int; L.tl_param_count.argtypes = [vp]
+    L.tl_get_info.restype = C.c_int; L.tl_get_info.argtypes = [vp, C.POINTER(tl_info)]
+    L.tl_loglike_batch.restype = C.c_int; L.tl_loglike_batch.argtypes = [vp, vp, i64, vp, vp]
+    L.tl_render_batch.restype = C.c_int; L.tl_render_batch.argtypes = [vp, vp, i64, vp, vp]
+    L.tl_loglike_batch_host.restype = C.c_int; L.tl_loglike_batch_host.argtypes = [vp, vp, i64, vp, vp]
+    L.tl_destroy.restype = None; L.tl_destroy.argtypes = [vp]
+    L.tl_strerror.restype = C.c_char_p; L.tl_strerror.argtypes = [C.c_int]
+    L.tl_version.restype = C.c_char_p; L.tl_version.argtypes = []
+    _lib = L
+    return L
+
+
+def tl_strerror(code: int) -> str:
+    return load().tl_strerror(int(code)).decode()
+
+
+def tl_version() -> str:
+    return load().tl_version().decode()
+
+
+def _check(code: int, what: str):
+    if code != TL_OK:
+        raise TinyLensError(code, what)
+
+
+def _stream_handle(stream) -> int:
+    """cudaStream_t of a torch stream (None = torch's current stream)."""
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream)
+
+
+def _f32c(a) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=np.float32)
+
+
+def tl_create(ny, nx, pix_scale, supersample, n_lens_light, n_source, psf, data, noise,
+              edge_mode=TL_EDGE_EXTEND, n_lens=1, stream=None) -> int:
+    """-> opaque handle (int).  psf [n_lens,K,K], data/noise [n_lens,ny,nx]: host float32 arrays."""
+    L = load()
+    p, d, s = _f32c(psf), _f32c(data), _f32c(noise)
+    K = p.shape[-1]
+    if p.size != n_lens * K * K or p.shape[-2] != K:
+        raise TinyLensError(TL_EINVAL, "tl_create (psf shape)")
+    if d.size != n_lens * ny * nx or s.size != n_lens * ny * nx:
+        raise TinyLensError(TL_EINVAL, "tl_create (data/noise shape)")
+    cfg = tl_config(int(ny), int(nx), float(pix_scale), int(supersample), int(n_lens_light),
+                    int(n_source), int(edge_mode), int(n_lens))
+    h = C.c_void_p()
+    fp = C.POINTER(C.c_float)
+    sh = 0
+    try:
+        import torch
+        if torch.cuda.is_available():
+            sh = _stream_handle(stream)
+    except ImportError:
+        pass
+    _check(L.tl_create(C.byref(h), C.byref(cfg), p.ctypes.data_as(fp), K, K,
+                       d.ctypes.data_as(fp), s.ctypes.data_as(fp), sh), "tl_create")
+    return h.value
+
+
+def tl_param_count(handle: int) -> int:
+    return load().tl_param_count(handle)
+
+
+def tl_get_info(handle: int) -> dict:
+    info = tl_info()
+    _check(load().tl_get_info(handle, C.byref(info)), "tl_get_info")
+    return {k: getattr(info, k) for k, _ in tl_info._fields_}
+
+
+def _dev_rows(handle, params):
+    import torch
+    P = tl_param_count(handle)
+    if not (isinstance(params, torch.Tensor) and params.is_cuda and params.dtype == torch.float32
+            and params.is_contiguous() and params.dim() == 2 and params.shape[1] == P):
+        raise TinyLensError(TL_EINVAL, "params must be a contiguous CUDA float32 tensor [B, %d]" % P)
+    return params.shape[0]
+
+
+def tl_loglike_batch(handle: int, params, out=None, stream=None):
+    """params: CUDA float32 [B,P] -> logL CUDA float32 [B] (enqueued on `stream`, no sync)."""
+    import torch
+    B = _dev_rows(handle, params)
+    if out is None:
+        out = torch.empty(B, dtype=torch.float32, device=params.device)
+    _check(load().tl_loglike_batch(handle, params.data_ptr(), B, out.data_ptr(), _stream_handle(stream)),
+           "tl_loglike_batch")
+    return out
+
+
+def tl_render_batch(handle: int, params, ny: int, nx: int, out=None, stream=None):
+    """params: CUDA float32 [B,P] -> images CUDA float32 [B,ny,nx]."""
+    import torch
+    B = _dev_rows(handle, params)
+    if out is None:
+        out = torch.empty((B, ny, nx), dtype=torch.float32, device=params.device)
+    _check(load().tl_render_batch(handle, params.data_ptr(), B, out.data_ptr(), _stream_handle(stream)),
+           "tl_render_batch")
+    return out
+
+
+def tl_loglike_batch_host(handle: int, params_host, out_host=None, stream=None):
+    """params_host: host float32 [B,P] (torch CPU tensor, ideally pinned, or numpy) -> host logL [B].
+    Host->device copy, kernels, device->host copy and a stream synchronise, all inside the call."""
+    import torch
+    P = tl_param_count(handle)
+    if isinstance(params_host, np.ndarray):
+        params_host = torch.from_numpy(_f32c(params_host))
+    if params_host.is_cuda or params_host.dtype != torch.float32 or not params_host.is_contiguous() \
+            or params_host.dim() != 2 or params_host.shape[1] != P:
+        raise TinyLensError(TL_EINVAL, "params_host must be a contiguous host float32 tensor [B, %d]" % P)
+    B = params_host.shape[0]
+    if out_host is None:
+        out_host = torch.empty(B, dtype=torch.float32, pin_memory=True)
+    _check(load().tl_loglike_batch_host(handle, params_host.data_ptr(), B, out_host.data_ptr(),
+                                        _stream_handle(stream)), "tl_loglike_batch_host")
+    return out_host
+
+
+def tl_destroy(handle: Optional[int]):
+    if handle:
+        load().tl_destroy(handle)
+
+
+class LensContext:
+    """RAII wrapper: ``ctx = LensContext.from_problem(problem); ctx.loglike(params)``."""
+
+    def __init__(self, ny, nx, pix_scale, supersample, n_lens_light, n_source, psf, data, noise,
+                 edge_mode=TL_EDGE_EXTEND, n_lens=1, stream=None):
+        self.ny, self.nx, self.n_lens = int(ny), int(nx), int(n_lens)
+        self.handle = tl_create(ny, nx, pix_scale, supersample, n_lens_light, n_source, psf, data,
+                                noise, edge_mode, n_lens, stream)
+        self.n_params = tl_param_count(self.handle)
+
+    @classmethod
+    def from_problem(cls, prob, stream=None):
+        w = prob.workload
+        return cls(w.ny, w.nx, w.pix_scale, w.supersample, w.n_lens_light, w.n_source,
+                   prob.psf, prob.data, prob.noise, w.edge_mode, w.n_lens, stream)
+
+    def info(self) -> dict:
+        return tl_get_info(self.handle)
+
+    def loglike(self, params, out=None, stream=None):
+        return tl_loglike_batch(self.handle, params, out, stream)
+
+    def render(self, params, out=None, stream=None):
+        return tl_render_batch(self.handle, params, self.ny, self.nx, out, stream)
+
+    def loglike_host(self, params_host, out_host=None, stream=None):
+        return tl_loglike_batch_host(self.handle, params_host, out_host, stream)
+
+    def close(self):
+        if getattr(self, "handle", None):
+            tl_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()

@@ -1,0 +1,309 @@
+// tinylens.cu -- C ABI (include/tinylens.h) and host-side launch logic.
+//
+// No CPU fallback lives here: every compute entry point either enqueues the CUDA kernels of
+// tl_kernels.cuh or returns an error code.
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include <cuda_runtime.h>
+
+#include "../../include/tinylens.h"
+#include "tl_kernels.cuh"
+
+#define TL_VERSION_STRING "tinylens-b200 0.1 (sm_100a)"
+
+struct tl_ctx {
+    tl_config cfg;
+    int device = 0;
+    int n_sm = 0;
+    int P = 0, K = 0, Kp = 0, h = 0, He = 0, We = 0, pitch = 0, n_comp = 0;
+    // device arrays (library-owned)
+    float *psf = nullptr, *data = nullptr, *wgt = nullptr, *sigma_min = nullptr;
+    double *lconst = nullptr;
+    double lconst0 = 0.0, sigma_min0 = 0.0;
+    // launch geometry
+    int path = 0;                 // 0 fused, 1 split
+    int threads = 256, ctas_per_sm = 1, grid = 1;
+    size_t smem = 0;
+    int tile_rows = 0, n_tiles = 0;
+    size_t conv_smem = 0;
+    int64_t chunk_rows = 0;       // rows per scratch chunk
+    double refine_tau = 3e-4;
+};
+
+namespace {
+
+constexpr size_t SMEM_LIMIT = 227 * 1024;
+constexpr int64_t CONST_CHUNK = 1 << 17;        // rows of RowC scratch per chunk (fused path)
+constexpr size_t EXT_SCRATCH_BYTES = 512u << 20; // split path: binned-image scratch per chunk
+
+inline bool cuda_ok(cudaError_t e) { return e == cudaSuccess; }
+
+size_t fused_smem_bytes(const tl_ctx *c)
+{
+    return sizeof(tl::RowC) + 32 * sizeof(double) + sizeof(float) * ((size_t)c->K * c->Kp + (size_t)c->He * c->pitch + c->Kp + 8);
+}
+
+size_t conv_smem_bytes(const tl_ctx *c, int tile_rows)
+{
+    return 32 * sizeof(double) + sizeof(float) * ((size_t)c->K * c->Kp + (size_t)(tile_rows + 2 * c->h) * c->pitch + c->Kp + 8);
+}
+
+tl::KArgs base_args(const tl_ctx *c)
+{
+    tl::KArgs a;
+    memset(&a, 0, sizeof(a));
+    a.psf = c->psf; a.data = c->data; a.wgt = c->wgt; a.lconst = c->lconst;
+    a.ny = c->cfg.ny; a.nx = c->cfg.nx; a.K = c->K; a.Kp = c->Kp; a.h = c->h;
+    a.He = c->He; a.We = c->We; a.pitch = c->pitch; a.S = c->cfg.supersample;
+    a.n_lens_light = c->cfg.n_lens_light; a.n_comp = c->n_comp;
+    a.edge_zero = c->cfg.edge_mode == TL_EDGE_ZERO;
+    a.tile_rows = c->tile_rows; a.n_tiles = c->n_tiles;
+    return a;
+}
+
+int run_batch(tl_ctx *c, const float *params, int64_t B, float *logL, float *images, cudaStream_t st)
+{
+    if (!c || B < 0) return TL_EINVAL;
+    if (B == 0) return TL_OK;
+    if (!params || (!logL && !images)) return TL_EINVAL;
+    if (B % c->cfg.n_lens) return TL_EINVAL;
+    int dev = -1;
+    if (!cuda_ok(cudaGetDevice(&dev))) return TL_ECUDA;
+    if (dev != c->device && !cuda_ok(cudaSetDevice(c->device))) return TL_ECUDA;
+
+    const int64_t rows_per_lens = B / c->cfg.n_lens;
+    const int64_t chunk = c->chunk_rows < B ? c->chunk_rows : B;
+    tl::RowC *rows = nullptr;
+    float *ext = nullptr;
+    double *partial = nullptr;
+    if (!cuda_ok(cudaMallocAsync(&rows, sizeof(tl::RowC) * (size_t)chunk, st))) return TL_ENOMEM;
+    if (c->path == 1) {
+        const size_t ext_bytes = sizeof(float) * (size_t)chunk * c->He * c->pitch;
+        if (!cuda_ok(cudaMallocAsync(&ext, ext_bytes, st)) ||
+            !cuda_ok(cudaMallocAsync(&partial, sizeof(double) * (size_t)chunk * c->n_tiles, st))) {
+            cudaFreeAsync(rows, st);
+            if (ext) cudaFreeAsync(ext, st);
+            return TL_ENOMEM;
+        }
+        cudaMemsetAsync(ext, 0, ext_bytes, st);      // pitch padding must read as finite zeros
+    }
+
+    int rc = TL_OK;
+    for (int64_t r0 = 0; r0 < B && rc == TL_OK; r0 += chunk) {
+        const int64_t nb = (B - r0 < chunk) ? (B - r0) : chunk;
+        tl::PrologueArgs pa;
+        pa.params = params + r0 * c->P; pa.rows = rows; pa.sigma_min = c->sigma_min;
+        pa.B = nb; pa.row0 = r0; pa.rows_per_lens = rows_per_lens;
+        pa.P = c->P; pa.n_lens_light = c->cfg.n_lens_light; pa.n_source = c->cfg.n_source;
+        pa.S = c->cfg.supersample;
+        pa.inv_u = 2.0 * c->cfg.supersample / c->cfg.pix_scale;
+        pa.fov_half = 0.5 * c->cfg.pix_scale * (c->He > c->We ? c->He : c->We);
+        pa.refine_tau = c->refine_tau;
+        const int64_t nthr = nb * (1 + c->n_comp);
+        tl::prologue_kernel<<<(unsigned)((nthr + 127) / 128), 128, 0, st>>>(pa);
+
+        tl::KArgs a = base_args(c);
+        a.rows = rows; a.B = nb; a.rows_per_lens = rows_per_lens; a.row0 = r0;
+        a.logL = logL; a.images = images;
+        if (c->path == 0) {
+            int grid = c->grid;
+            if ((int64_t)grid > nb) grid = (int)nb;
+            tl::fused_kernel<<<grid, c->threads, c->smem, st>>>(a);
+        } else {
+            a.ext = ext; a.partial = logL ? partial : nullptr;
+            const int slabs = 8;
+            dim3 tg((unsigned)(nb < 65535 ? nb : 65535), slabs);
+            tl::trace_kernel<<<tg, 256, 0, st>>>(a, (int)nb);
+            dim3 cg((unsigned)nb, (unsigned)c->n_tiles);
+            tl::conv_kernel<<<cg, 256, c->conv_smem, st>>>(a, (int)nb);
+            if (logL) tl::finalize_kernel<<<(unsigned)((nb + 127) / 128), 128, 0, st>>>(a, (int)nb);
+        }
+        if (!cuda_ok(cudaGetLastError())) rc = TL_ECUDA;
+    }
+    cudaFreeAsync(rows, st);
+    if (ext) cudaFreeAsync(ext, st);
+    if (partial) cudaFreeAsync(partial, st);
+    return rc;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *tl_version(void) { return TL_VERSION_STRING; }
+
+const char *tl_strerror(int code)
+{
+    switch (code) {
+    case TL_OK: return "success";
+    case TL_EINVAL: return "invalid argument (shape, even PSF size, null pointer, or noise not finite and positive)";
+    case TL_ENOMEM: return "out of host or device memory";
+    case TL_ECUDA: return "no usable CUDA device or a CUDA runtime call failed (there is no CPU fallback)";
+    case TL_ESIZE: return "configuration exceeds what the kernels support";
+    default: return "unknown tinylens error code";
+    }
+}
+
+int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_ny, int32_t psf_nx,
+              const float *data, const float *noise, void *cuda_stream)
+{
+    if (out) *out = nullptr;
+    if (!out || !cfg || !psf || !data || !noise) return TL_EINVAL;
+    if (cfg->ny < 1 || cfg->nx < 1 || !(cfg->pix_scale > 0.0) || !std::isfinite(cfg->pix_scale)) return TL_EINVAL;
+    if (cfg->supersample < 1 || cfg->supersample > 16) return TL_EINVAL;
+    if (cfg->n_lens_light < 0 || cfg->n_lens_light > 1 || cfg->n_source < 1 || cfg->n_source > 2) return TL_EINVAL;
+    if (cfg->edge_mode != TL_EDGE_EXTEND && cfg->edge_mode != TL_EDGE_ZERO) return TL_EINVAL;
+    if (cfg->n_lens < 1) return TL_EINVAL;
+    if (psf_ny != psf_nx || psf_ny < 1 || (psf_ny & 1) == 0) return TL_EINVAL;
+    // exact sub-sample coordinates need 2 S (n + K) < 2^24
+    if ((int64_t)2 * cfg->supersample * ((int64_t)(cfg->ny > cfg->nx ? cfg->ny : cfg->nx) + psf_ny) >= (1 << 24)) return TL_ESIZE;
+
+    const size_t npix = (size_t)cfg->ny * cfg->nx, L = (size_t)cfg->n_lens;
+    for (size_t i = 0; i < npix * L; ++i)
+        if (!(noise[i] > 0.f) || !std::isfinite(noise[i])) return TL_EINVAL;
+
+    int ndev = 0;
+    if (!cuda_ok(cudaGetDeviceCount(&ndev)) || ndev < 1) return TL_ECUDA;
+
+    tl_ctx *c = new (std::nothrow) tl_ctx;
+    if (!c) return TL_ENOMEM;
+    c->cfg = *cfg;
+    if (!cuda_ok(cudaGetDevice(&c->device))) { delete c; return TL_ECUDA; }
+    cudaDeviceProp prop;
+    if (!cuda_ok(cudaGetDeviceProperties(&prop, c->device))) { delete c; return TL_ECUDA; }
+    c->n_sm = prop.multiProcessorCount;
+    c->n_comp = cfg->n_lens_light + cfg->n_source;
+    c->P = 7 + 7 * c->n_comp;
+    c->K = psf_ny; c->Kp = (c->K + 3) & ~3; c->h = (c->K - 1) / 2;
+    c->He = cfg->ny + 2 * c->h; c->We = cfg->nx + 2 * c->h;
+    c->pitch = (c->We + 3) & ~3;
+
+    // host-side preparation in FP64: flipped + padded PSF, inverse variance, Eq. 5 constant
+    std::vector<float> psf_f((size_t)L * c->K * c->Kp, 0.f), wgt(npix * L), smin(L);
+    std::vector<double> lconst(L);
+    for (size_t l = 0; l < L; ++l) {
+        // true convolution (Eq. 3, G11) == correlation with the flipped kernel
+        for (int a = 0; a < c->K; ++a)
+            for (int b = 0; b < c->K; ++b)
+                psf_f[(l * c->K + a) * c->Kp + b] = psf[(l * c->K + (c->K - 1 - a)) * c->K + (c->K - 1 - b)];
+        double s = 0.0, comp = 0.0, mn = INFINITY;
+        for (size_t i = 0; i < npix; ++i) {
+            const double sg = noise[l * npix + i];
+            wgt[l * npix + i] = (float)(1.0 / (sg * sg));
+            const double t = std::log(2.0 * M_PI * sg * sg) - comp, u = s + t;   // Kahan
+            comp = (u - s) - t; s = u;
+            if (sg < mn) mn = sg;
+        }
+        lconst[l] = s; smin[l] = (float)mn;
+    }
+    c->lconst0 = lconst[0]; c->sigma_min0 = smin[0];
+    if (const char *e = std::getenv("TL_REFINE_TAU")) {   // tuning knob
+        const double v = std::atof(e);
+        if (v > 0.0 && std::isfinite(v)) c->refine_tau = v;
+    }
+
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    bool ok = cuda_ok(cudaMalloc(&c->psf, psf_f.size() * sizeof(float))) &&
+              cuda_ok(cudaMalloc(&c->data, npix * L * sizeof(float))) &&
+              cuda_ok(cudaMalloc(&c->wgt, npix * L * sizeof(float))) &&
+              cuda_ok(cudaMalloc(&c->sigma_min, L * sizeof(float))) &&
+              cuda_ok(cudaMalloc(&c->lconst, L * sizeof(double)));
+    if (!ok) { tl_destroy(c); return TL_ENOMEM; }
+    ok = cuda_ok(cudaMemcpyAsync(c->psf, psf_f.data(), psf_f.size() * sizeof(float), cudaMemcpyHostToDevice, st)) &&
+         cuda_ok(cudaMemcpyAsync(c->data, data, npix * L * sizeof(float), cudaMemcpyHostToDevice, st)) &&
+         cuda_ok(cudaMemcpyAsync(c->wgt, wgt.data(), npix * L * sizeof(float), cudaMemcpyHostToDevice, st)) &&
+         cuda_ok(cudaMemcpyAsync(c->sigma_min, smin.data(), L * sizeof(float), cudaMemcpyHostToDevice, st)) &&
+         cuda_ok(cudaMemcpyAsync(c->lconst, lconst.data(), L * sizeof(double), cudaMemcpyHostToDevice, st)) &&
+         cuda_ok(cudaStreamSynchronize(st));
+    if (!ok) { tl_destroy(c); return TL_ECUDA; }
+
+    // launch geometry
+    const size_t fs = fused_smem_bytes(c);
+    if (fs <= SMEM_LIMIT) {
+        c->path = 0; c->smem = fs;
+        c->threads = fs > SMEM_LIMIT / 2 ? 512 : 256;
+        if (!cuda_ok(cudaFuncSetAttribute(tl::fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT))) { tl_destroy(c); return TL_ECUDA; }
+        int occ = 0;
+        if (!cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, tl::fused_kernel, c->threads, fs)) || occ < 1) { tl_destroy(c); return TL_ECUDA; }
+        c->ctas_per_sm = occ; c->grid = occ * c->n_sm;
+        c->chunk_rows = CONST_CHUNK;
+    } else {
+        c->path = 1;
+        // tile rows: as many as fit in ~100 KB so two CTAs share an SM
+        int tr = (int)((100 * 1024 / sizeof(float) - (size_t)c->K * c->Kp - c->Kp - 8) / c->pitch) - 2 * c->h;
+        if (tr < 4) tr = (int)((SMEM_LIMIT / sizeof(float) - 64 - (size_t)c->K * c->Kp - c->Kp - 8) / c->pitch) - 2 * c->h;
+        if (tr < 1) { tl_destroy(c); return TL_ESIZE; }
+        if (tr > cfg->ny) tr = cfg->ny;
+        c->tile_rows = tr; c->n_tiles = (cfg->ny + tr - 1) / tr;
+        c->conv_smem = conv_smem_bytes(c, tr);
+        if (!cuda_ok(cudaFuncSetAttribute(tl::conv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT))) { tl_destroy(c); return TL_ECUDA; }
+        c->threads = 256; c->smem = c->conv_smem;
+        int occ = 0;
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, tl::trace_kernel, 256, 0);
+        c->ctas_per_sm = occ > 0 ? occ : 1; c->grid = 0;
+        int64_t cr = (int64_t)(EXT_SCRATCH_BYTES / (sizeof(float) * (size_t)c->He * c->pitch));
+        if (cr < 1) cr = 1;
+        if (cr > 65535) cr = 65535;
+        c->chunk_rows = cr;
+    }
+    *out = c;
+    return TL_OK;
+}
+
+int tl_param_count(const tl_ctx *ctx) { return ctx ? ctx->P : TL_EINVAL; }
+
+int tl_get_info(const tl_ctx *c, tl_info *info)
+{
+    if (!c || !info) return TL_EINVAL;
+    info->n_params = c->P; info->path = c->path; info->block_threads = c->threads;
+    info->ctas_per_sm = c->ctas_per_sm; info->grid = c->grid; info->smem_bytes = (int32_t)c->smem;
+    info->n_sm = c->n_sm; info->launches_per_call = c->path == 0 ? 2 : 4;
+    const bool ext = c->cfg.edge_mode == TL_EDGE_EXTEND;
+    const int64_t hy = ext ? c->He : c->cfg.ny, wx = ext ? c->We : c->cfg.nx;
+    info->samples_per_row = hy * wx * c->cfg.supersample * c->cfg.supersample;
+    info->conv_fma_per_row = (int64_t)c->K * c->K * c->cfg.ny * c->cfg.nx;
+    info->logl_const = c->lconst0; info->sigma_min = c->sigma_min0;
+    return TL_OK;
+}
+
+int tl_loglike_batch(tl_ctx *ctx, const float *params, int64_t B, float *logL, void *cuda_stream)
+{
+    return run_batch(ctx, params, B, logL, nullptr, (cudaStream_t)cuda_stream);
+}
+
+int tl_render_batch(tl_ctx *ctx, const float *params, int64_t B, float *images, void *cuda_stream)
+{
+    return run_batch(ctx, params, B, nullptr, images, (cudaStream_t)cuda_stream);
+}
+
+int tl_loglike_batch_host(tl_ctx *ctx, const float *params, int64_t B, float *logL, void *cuda_stream)
+{
+    if (!ctx || B < 0 || (B > 0 && (!params || !logL))) return TL_EINVAL;
+    if (B == 0) return TL_OK;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    float *dp = nullptr, *dl = nullptr;
+    if (!cuda_ok(cudaMallocAsync(&dp, sizeof(float) * (size_t)B * ctx->P, st))) return TL_ENOMEM;
+    if (!cuda_ok(cudaMallocAsync(&dl, sizeof(float) * (size_t)B, st))) { cudaFreeAsync(dp, st); return TL_ENOMEM; }
+    int rc = TL_OK;
+    if (!cuda_ok(cudaMemcpyAsync(dp, params, sizeof(float) * (size_t)B * ctx->P, cudaMemcpyHostToDevice, st))) rc = TL_ECUDA;
+    if (rc == TL_OK) rc = run_batch(ctx, dp, B, dl, nullptr, st);
+    if (rc == TL_OK && !cuda_ok(cudaMemcpyAsync(logL, dl, sizeof(float) * (size_t)B, cudaMemcpyDeviceToHost, st))) rc = TL_ECUDA;
+    cudaFreeAsync(dp, st);
+    cudaFreeAsync(dl, st);
+    if (!cuda_ok(cudaStreamSynchronize(st)) && rc == TL_OK) rc = TL_ECUDA;
+    return rc;
+}
+
+void tl_destroy(tl_ctx *c)
+{
+    if (!c) return;
+    cudaFree(c->psf); cudaFree(c->data); cudaFree(c->wgt); cudaFree(c->sigma_min); cudaFree(c->lconst);
+    delete c;
+}
+
+}  // extern "C"

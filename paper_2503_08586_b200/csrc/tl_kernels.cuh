@@ -1,0 +1,267 @@
+// tl_kernels.cuh -- the hot-path kernels (steps a1..a8 of DESIGN.md).
+//
+// fused_kernel: persistent CTAs, one parameter row at a time per CTA.
+//   phase 1  every thread ray-traces whole native pixels (S*S sub-samples accumulated in a
+//            register = step a5) and stores the binned value into the extended image held
+//            in shared memory;
+//   phase 2  register-blocked direct PSF convolution (1 x 4 output strip per thread, LDS.128
+//            for both the image window and the taps) straight from shared memory, followed
+//            by the chi^2 terms against data / inverse-variance read through L2;
+//   phase 3  deterministic FP64 reduction: per-thread partial -> warp shuffle tree -> fixed
+//            order over warps.  No atomics, so logL is bitwise reproducible.
+// The split path (large images) runs phase 1 into global memory (trace_kernel) and phases
+// 2-3 from shared-memory tiles of it (conv_kernel + finalize_kernel).
+#pragma once
+#include "tl_sample.cuh"
+
+namespace tl {
+
+constexpr int CONV_R = 4;            // outputs per thread strip (along x)
+
+struct KArgs {
+    const RowC *rows;        // [B] derived constants
+    const float *psf;        // [n_lens][K][Kp]  flipped, rows zero-padded to Kp (multiple of 4)
+    const float *data;       // [n_lens][ny][nx]
+    const float *wgt;        // [n_lens][ny][nx]  1 / sigma^2
+    const double *lconst;    // [n_lens]          sum ln(2 pi sigma^2)
+    float *logL;             // [B] or null
+    float *images;           // [B][ny][nx] or null
+    float *ext;              // split path: [chunk][He][pitch] binned extended images
+    double *partial;         // split path: [chunk][n_tiles] chi^2 partials
+    int64_t B, rows_per_lens, row0;
+    int ny, nx, K, Kp, h, He, We, pitch, S, n_lens_light, n_comp, edge_zero;
+    int tile_rows, n_tiles;  // split path
+};
+
+__device__ __forceinline__ bool row_is_valid(const RowC &rc, int n_comp)
+{
+    bool ok = rc.lens.valid != 0;
+    for (int k = 0; k < n_comp; ++k) ok = ok && (rc.comp[k].valid != 0);
+    return ok;
+}
+
+// steps a1-a5 for one extended native pixel (i, j)
+__device__ __forceinline__ float trace_pixel(const RowC &rc, const KArgs &a, int i, int j)
+{
+    const int S = a.S;
+    if (a.edge_zero && (i < a.h || i >= a.He - a.h || j < a.h || j >= a.We - a.h)) return 0.f;
+    // u-units: X = 2 (j S + b) + 1 - S We is the exact sub-sample abscissa (DESIGN.md a1)
+    const float X0 = (float)(2 * j * S + 1 - S * a.We);
+    const float Y0 = (float)(2 * i * S + 1 - S * a.He);
+    float acc = 0.f;
+    for (int sa = 0; sa < S; ++sa) {
+        const float Y = Y0 + (float)(2 * sa);
+        for (int sb = 0; sb < S; ++sb) {
+            const float X = X0 + (float)(2 * sb);
+            acc += sample_value<true>(rc, a.n_lens_light, a.n_comp, X, Y);
+        }
+    }
+    return acc;
+}
+
+// step a6 for a 1 x CONV_R strip whose window starts at `win` (16-byte aligned) in an image of
+// row pitch `pitch`; `taps` = flipped PSF [K][Kp] in shared memory.
+__device__ __forceinline__ void conv_strip(const float *win, int pitch, const float *taps,
+                                           int K, int Kp, float acc[CONV_R])
+{
+#pragma unroll
+    for (int r = 0; r < CONV_R; ++r) acc[r] = 0.f;
+    for (int ka = 0; ka < K; ++ka) {
+        const float *rp = win + ka * pitch;
+        const float *kp = taps + ka * Kp;
+        float4 lo = *reinterpret_cast<const float4 *>(rp);
+        for (int kb = 0; kb < Kp; kb += 4) {
+            const float4 hi = *reinterpret_cast<const float4 *>(rp + kb + 4);
+            const float4 t = *reinterpret_cast<const float4 *>(kp + kb);
+            acc[0] = fmaf(t.x, lo.x, fmaf(t.y, lo.y, fmaf(t.z, lo.z, fmaf(t.w, lo.w, acc[0]))));
+            acc[1] = fmaf(t.x, lo.y, fmaf(t.y, lo.z, fmaf(t.z, lo.w, fmaf(t.w, hi.x, acc[1]))));
+            acc[2] = fmaf(t.x, lo.z, fmaf(t.y, lo.w, fmaf(t.z, hi.x, fmaf(t.w, hi.y, acc[2]))));
+            acc[3] = fmaf(t.x, lo.w, fmaf(t.y, hi.x, fmaf(t.z, hi.y, fmaf(t.w, hi.z, acc[3]))));
+            lo = hi;
+        }
+    }
+}
+
+// step a7 reduction: fixed-shape FP64 tree; result valid in thread 0.
+__device__ __forceinline__ double block_sum(double v, double *red)
+{
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    if (lane == 0) red[wid] = v;
+    __syncthreads();
+    double s = 0.0;
+    if (threadIdx.x == 0)
+        for (int w = 0; w < nw; ++w) s += red[w];
+    __syncthreads();
+    return s;
+}
+
+__device__ __forceinline__ void load_row_consts(RowC *dst, const RowC *src)
+{
+    const int n16 = sizeof(RowC) / 16;
+    const uint4 *s = reinterpret_cast<const uint4 *>(src);
+    uint4 *d = reinterpret_cast<uint4 *>(dst);
+    for (int i = threadIdx.x; i < n16; i += blockDim.x) d[i] = s[i];
+}
+
+__device__ __forceinline__ void load_psf(float *dst, const float *src, int n)
+{
+    for (int i = threadIdx.x; i < n; i += blockDim.x) dst[i] = src[i];
+}
+
+// convolve + chi^2 over output rows [i0, i1) of one image; `img` is a shared-memory image
+// whose row 0 corresponds to extended row `e0`.  Returns this thread's chi^2 partial.
+__device__ __forceinline__ double conv_chi2_rows(const KArgs &a, const float *img, int e0,
+                                                 const float *taps, int i0, int i1,
+                                                 const float *data, const float *wgt, float *image_out)
+{
+    const int nsx = (a.nx + CONV_R - 1) / CONV_R;
+    const int total = (i1 - i0) * nsx;
+    double part = 0.0;
+    for (int s = threadIdx.x; s < total; s += blockDim.x) {
+        const int ir = s / nsx, i = i0 + ir, x0 = (s - ir * nsx) * CONV_R;
+        float acc[CONV_R];
+        conv_strip(img + (i - e0) * a.pitch + x0, a.pitch, taps, a.K, a.Kp, acc);
+        float c = 0.f;
+#pragma unroll
+        for (int r = 0; r < CONV_R; ++r) {
+            const int x = x0 + r;
+            if (x < a.nx) {
+                const int o = i * a.nx + x;
+                if (image_out) image_out[o] = acc[r];
+                if (data) {
+                    const float d = __ldg(data + o) - acc[r];
+                    c = fmaf(d * d, __ldg(wgt + o), c);
+                }
+            }
+        }
+        part += (double)c;
+    }
+    return part;
+}
+
+// ------------------------------------------------------------------------------ fused path
+__global__ void __launch_bounds__(512) fused_kernel(const KArgs a)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    RowC *rc = reinterpret_cast<RowC *>(smem_raw);
+    double *red = reinterpret_cast<double *>(smem_raw + sizeof(RowC));
+    float *taps = reinterpret_cast<float *>(smem_raw + sizeof(RowC) + 32 * sizeof(double));
+    float *img = taps + a.K * a.Kp;
+    const int n_img = a.He * a.pitch;
+    // pitch padding and the slack after the image are read by zero-padded taps only (and by
+    // discarded strip lanes); phase 1 never writes them, so zero them once
+    for (int i = threadIdx.x; i < n_img + a.Kp + 8; i += blockDim.x) img[i] = 0.f;
+
+    int64_t cur_lens = -1;
+    for (int64_t r = blockIdx.x; r < a.B; r += gridDim.x) {
+        const int64_t row = a.row0 + r;                // global row; a.rows is chunk-local
+        const int64_t lens = row / a.rows_per_lens;
+        __syncthreads();                               // previous row fully consumed
+        load_row_consts(rc, a.rows + r);
+        if (lens != cur_lens) { load_psf(taps, a.psf + lens * a.K * a.Kp, a.K * a.Kp); cur_lens = lens; }
+        __syncthreads();
+        const size_t npix = (size_t)a.ny * a.nx;
+        if (!row_is_valid(*rc, a.n_comp)) {            // uniform over the CTA
+            if (a.logL && threadIdx.x == 0) a.logL[row] = -INFINITY;
+            if (a.images)
+                for (size_t i = threadIdx.x; i < npix; i += blockDim.x) a.images[row * npix + i] = NAN;
+            continue;
+        }
+        // phase 1: ray-trace + light + bin into shared memory
+        const int next = a.He * a.We;
+        for (int pix = threadIdx.x; pix < next; pix += blockDim.x) {
+            const int i = pix / a.We, j = pix - i * a.We;
+            img[i * a.pitch + j] = trace_pixel(*rc, a, i, j);
+        }
+        __syncthreads();
+        // phase 2: PSF convolution from shared memory + chi^2
+        const double part = conv_chi2_rows(a, img, 0, taps, 0, a.ny,
+                                           a.logL ? a.data + lens * npix : nullptr,
+                                           a.wgt + lens * npix,
+                                           a.images ? a.images + row * npix : nullptr);
+        // phase 3: deterministic reduction (Eq. 5)
+        if (a.logL) {
+            const double chi2 = block_sum(part, red);
+            if (threadIdx.x == 0) a.logL[row] = (float)(-0.5 * (chi2 + a.lconst[lens]));
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------ split path
+// trace_kernel: grid-stride over (row, extended pixel) of the current chunk.
+__global__ void __launch_bounds__(256) trace_kernel(const KArgs a, int chunk_rows)
+{
+    __shared__ RowC rc_s;
+    // one row per CTA-iteration keeps the constants in shared memory; the row's pixels are
+    // spread over `n_tiles`-independent CTAs: blockIdx = (row_in_chunk, slab)
+    const int slabs = gridDim.y;
+    for (int r = blockIdx.x; r < chunk_rows; r += gridDim.x) {
+        __syncthreads();
+        load_row_consts(&rc_s, a.rows + r);
+        __syncthreads();
+        if (!row_is_valid(rc_s, a.n_comp)) continue;
+        float *dst = a.ext + (size_t)r * a.He * a.pitch;
+        const int next = a.He * a.We;
+        for (int pix = blockIdx.y * blockDim.x + threadIdx.x; pix < next; pix += slabs * blockDim.x) {
+            const int i = pix / a.We, j = pix - i * a.We;
+            dst[i * a.pitch + j] = trace_pixel(rc_s, a, i, j);
+        }
+    }
+}
+
+// conv_kernel: one CTA per (row_in_chunk, tile of `tile_rows` output rows).
+__global__ void __launch_bounds__(256) conv_kernel(const KArgs a, int chunk_rows)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    double *red = reinterpret_cast<double *>(smem_raw);
+    float *taps = reinterpret_cast<float *>(smem_raw + 32 * sizeof(double));
+    float *img = taps + a.K * a.Kp;
+    const int r = blockIdx.x, tile = blockIdx.y;
+    const int64_t row = a.row0 + r;
+    const int64_t lens = row / a.rows_per_lens;
+    const size_t npix = (size_t)a.ny * a.nx;
+    const RowC *rcg = a.rows + r;
+    bool ok = rcg->lens.valid != 0;
+    for (int k = 0; k < a.n_comp; ++k) ok = ok && (rcg->comp[k].valid != 0);
+    const int i0 = tile * a.tile_rows, i1 = min(a.ny, i0 + a.tile_rows);
+    if (!ok) {
+        if (a.images)
+            for (size_t i = (size_t)i0 * a.nx + threadIdx.x; i < (size_t)i1 * a.nx; i += blockDim.x)
+                a.images[row * npix + i] = NAN;
+        if (a.partial && threadIdx.x == 0) a.partial[(size_t)r * a.n_tiles + tile] = INFINITY;
+        return;
+    }
+    load_psf(taps, a.psf + lens * a.K * a.Kp, a.K * a.Kp);
+    // extended rows i0 .. i1 + 2h - 1 of this row's binned image, plus slack
+    const int erows = (i1 - i0) + 2 * a.h;
+    const float4 *src = reinterpret_cast<const float4 *>(a.ext + ((size_t)r * a.He + i0) * a.pitch);
+    float4 *dst = reinterpret_cast<float4 *>(img);
+    const int n4 = erows * a.pitch / 4;
+    for (int i = threadIdx.x; i < n4; i += blockDim.x) dst[i] = src[i];
+    for (int i = threadIdx.x; i < a.Kp + 8; i += blockDim.x) img[erows * a.pitch + i] = 0.f;
+    __syncthreads();
+    const double part = conv_chi2_rows(a, img, i0, taps, i0, i1,
+                                       a.partial ? a.data + lens * npix : nullptr,
+                                       a.wgt + lens * npix,
+                                       a.images ? a.images + row * npix : nullptr);
+    if (a.partial) {
+        const double s = block_sum(part, red);
+        if (threadIdx.x == 0) a.partial[(size_t)r * a.n_tiles + tile] = s;
+    }
+}
+
+// finalize_kernel: fixed-order sum of the tile partials -> logL.
+__global__ void finalize_kernel(const KArgs a, int chunk_rows)
+{
+    const int r = blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= chunk_rows) return;
+    const int64_t row = a.row0 + r;
+    double s = 0.0;
+    for (int t = 0; t < a.n_tiles; ++t) s += a.partial[(size_t)r * a.n_tiles + t];
+    const double ll = -0.5 * (s + a.lconst[row / a.rows_per_lens]);
+    a.logL[row] = isfinite(s) ? (float)ll : -INFINITY;
+}
+
+}  // namespace tl
