@@ -1,0 +1,326 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the batched lens-model likelihood (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config i]
+
+A "step" is one pass of the whole hot path (DESIGN.md steps a0-a7: prologue, ray-trace, light,
+bin, PSF convolution, chi^2 -> logL) over one batch of B synthetic parameter rows.  At N = 1 the
+workload is BASELINE.json configs[1] (CSST-like 100x100, 4x4 supersampling, 21x21 PSF, B = 4096).
+For N > 1 (torchrun, one process per GPU) every rank evaluates its own B rows: the path shards
+over independent rows with no data-path collective ("scaling": "weak").
+
+Prints ONE JSON line on rank 0.  --impl reference times the FP64 CPU oracle instead (the
+deliberately slow checker).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2503_08586_b200 import workloads as W  # noqa: E402
+
+METRIC = "likelihood evals/s"
+UNIT = "likelihoods/s"
+
+# ---- frozen algorithmic op model (BASELINE.md section 3 / SURVEY.md 8(d), op model v0) ----------
+# FP32-pipe instruction slots (FMA = MUL = ADD = 1) and MUFU operations the METHOD needs per
+# sub-sample; precision overhead (hi/lo constants, FP64 refinement, accurate-function
+# polynomials) is not algorithmic work and is not counted.
+OP_POS_FP32 = 2
+OP_SIE_FP32, OP_SIE_MUFU = 46, 4
+OP_SERSIC_FP32, OP_SERSIC_MUFU = 11, 3
+OP_CHI2_FP32 = 4
+SM_FP32_LANES = 128          # thread-instruction issue slots per SM per clock (4 warps x 32), measured 122-128
+SM_MUFU_LANES = 16           # measured 15.96 (profiles/r1_pipe_peaks.md)
+
+# dram bytes of the dominant kernel per launch from the committed `ncu --set full` capture
+# (profiles/): filled in by hand after each capture; None until one exists.
+NCU_DRAM_BYTES_PER_LAUNCH = None
+
+
+def op_model(w: W.Workload) -> dict:
+    ncomp = w.n_lens_light + w.n_source
+    samples = w.samples_per_likelihood
+    fp32 = samples * (OP_POS_FP32 + OP_SIE_FP32 + ncomp * OP_SERSIC_FP32) \
+        + w.ny * w.nx * (w.psf_size ** 2 + OP_CHI2_FP32)
+    mufu = samples * (OP_SIE_MUFU + ncomp * OP_SERSIC_MUFU)
+    return {"fp32_slots": fp32, "mufu_ops": mufu, "issue_slots": fp32 + mufu, "samples": samples}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.idx, self.rows, self.stop, self.t = gpu_index, [], False, None
+
+    def _run(self):
+        while not self.stop:
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.idx), "--query-gpu=" + self.Q,
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True,
+                                     timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([x.strip() for x in out.split(",")])
+            except Exception:
+                pass
+            time.sleep(0.1)
+
+    def __enter__(self):
+        self.t = threading.Thread(target=self._run, daemon=True)
+        self.t.start()
+        return self
+
+    def __exit__(self, *exc):
+        self.stop = True
+        self.t.join(timeout=10)
+
+    def summary(self) -> dict:
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except Exception:
+                continue
+            for n, v in zip(names, r[4:8]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None,
+                "sm_max_mhz": float(max(mx)) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def measured_peaks() -> dict:
+    try:
+        return json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        return {}
+
+
+def oracle_time(w: W.Workload, prob, rows: np.ndarray, threads: int = 0):
+    from oracle import oracle as O
+    cfg = O.config_of(w)
+    t0 = time.perf_counter()
+    _, used = O.loglike_batch(cfg, prob.psf, prob.data, prob.noise, rows, n_lens=w.n_lens, threads=threads)
+    return time.perf_counter() - t0, used
+
+
+def reference_problem(w: W.Workload):
+    """Inputs for the reference arm: data from the oracle's own renderer."""
+    from oracle import oracle as O
+    return W.make_problem(w, O.render_for_workloads)
+
+
+def run_reference(args, w: W.Workload):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import oracle as O
+    O.lib()
+    prob = reference_problem(w)
+    rows_all = W.batch_rows(w)
+    n = args.ref_rows
+    # bounded sample per step: the first n rows of each step's window of the workload
+    times, used = [], 1
+    for s in range(args.warmup + args.steps):
+        lo = (s * n) % max(1, len(rows_all) - n)
+        dt, used = oracle_time(w, prob, rows_all[lo:lo + n])
+        if s >= args.warmup:
+            times.append(dt)
+    tot = float(np.sum(times))
+    value = n * len(times) / tot
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / len(times),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": config_dict(w, "none (CPU)"),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": used, "kind": "oracle",
+                         "sample": "%d of the %d rows per step" % (n, w.batch)},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "pixel_evals_per_s": value * w.ny * w.nx, "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def config_dict(w: W.Workload, l2: str) -> dict:
+    return {"workload": "BASELINE.json configs[%d] %s: %dx%d px, %.3g\"/px, %dx%d supersampling, %dx%d %s PSF, "
+                        "SIE+shear, %d lens-light + %d source Sersic, B=%d rows/GPU%s"
+                        % (w.index, w.name, w.ny, w.nx, w.pix_scale, w.supersample, w.supersample, w.psf_size,
+                           w.psf_size, w.psf_kind, w.n_lens_light, w.n_source, w.batch,
+                           (", %d lenses" % w.n_lens) if w.n_lens > 1 else ""),
+            "batch_per_gpu": w.batch, "n_params": w.n_params, "l2": l2, "parallelism": "rows sharded, no collective"}
+
+
+def run_ours(args, w: W.Workload):
+    import torch
+    import torch.distributed as dist
+    from paper_2503_08586_b200 import api
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    dev = torch.device("cuda", local)
+
+    # mock data = model(truth) + noise, the model coming from the library's own renderer
+    def gpu_render(w1, psf, row):
+        ctx = api.LensContext(w1.ny, w1.nx, w1.pix_scale, w1.supersample, w1.n_lens_light, w1.n_source,
+                              psf[None], np.zeros((1, w1.ny, w1.nx), np.float32),
+                              np.ones((1, w1.ny, w1.nx), np.float32), w1.edge_mode)
+        im = ctx.render(torch.from_numpy(np.ascontiguousarray(row[None])).to(dev)).cpu().numpy()[0]
+        ctx.close()
+        return im
+
+    prob = W.make_problem(w, gpu_render)
+    ctx = api.LensContext.from_problem(prob)
+    info = ctx.info()
+    # each rank draws its own rows (weak scaling): stream id offset by rank
+    rows = W.batch_rows(w) if rank == 0 else \
+        np.concatenate([W.draw_params(w, W.rng_for(w.index, W.STREAM_BATCH + 16 * rank, l), w.rows_per_lens)
+                        for l in range(w.n_lens)], axis=0)
+    B = rows.shape[0]
+    d_rows = torch.from_numpy(rows).to(dev)
+    d_out = torch.empty(B, dtype=torch.float32, device=dev)
+    h_rows = torch.from_numpy(rows).pin_memory()
+    h_out = torch.empty(B, dtype=torch.float32).pin_memory()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    stream = torch.cuda.current_stream()
+    ctx.set_profiling(True)
+    for _ in range(max(args.warmup, 3)):
+        ctx.loglike(d_rows, d_out)
+    torch.cuda.synchronize()
+
+    # ---- device-resident timing: K steps, L2 flushed between steps, CUDA events per step -------
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    kern_ms = []
+    with ClockSampler(local) as clk:
+        barrier()
+        for s in range(args.steps):
+            flush.fill_(s & 0xff)
+            ev[s][0].record(stream)
+            ctx.loglike(d_rows, d_out)
+            ev[s][1].record(stream)
+            kern_ms.append(ctx.last_kernel_ms())      # waits for the kernel; keeps steps separate
+        barrier()
+        step_ms = [a.elapsed_time(b) for a, b in ev]
+        # ---- end to end through the host entry point (H2D + kernels + D2H + sync per step) ----
+        for _ in range(2):
+            ctx.loglike_host(h_rows, h_out)
+        barrier()
+        t0 = time.perf_counter()
+        for s in range(args.steps):
+            ctx.loglike_host(h_rows, h_out)
+        torch.cuda.synchronize()
+        e2e_s = time.perf_counter() - t0
+        barrier()
+    clocks = clk.summary()
+    total_ms = float(np.sum(step_ms))
+    logl_sum = float(h_out.double().sum())
+
+    if world > 1:
+        t = torch.tensor([total_ms, e2e_s], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms, e2e_s = float(t[0]), float(t[1])
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    value = world * B * args.steps / (total_ms * 1e-3)
+    e2e_value = world * B * args.steps / e2e_s
+    om = op_model(w)
+    peaks = measured_peaks()
+    sm_max = float(peaks.get("sm_max_mhz", 1965.0))
+    k_ms = float(np.mean(kern_ms))
+    achieved = om["issue_slots"] * B / (k_ms * 1e-3) / 1e12          # algorithmic Tinst/s
+    peak = info["n_sm"] * SM_FP32_LANES * sm_max * 1e6 / 1e12
+    mufu_frac = om["mufu_ops"] * B / (k_ms * 1e-3) / (info["n_sm"] * SM_MUFU_LANES * sm_max * 1e6)
+    fp32_frac = om["fp32_slots"] * B / (k_ms * 1e-3) / (info["n_sm"] * SM_FP32_LANES * sm_max * 1e6)
+    hbm_bytes = B * (w.n_params + 1) * 4 + (2 * w.ny * w.nx + w.psf_size ** 2) * 4 * w.n_lens
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": config_dict(w, "flushed between steps (256 MiB fill)"),
+        "pixel_evals_per_s": value * w.ny * w.nx,
+        "sample_evals_per_s": value * om["samples"],
+        "clocks": clocks,
+        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": B * w.n_params * 4,
+                "d2h_bytes_per_step": B * 4, "api": "tl_loglike_batch_host (pinned host buffers)"},
+        "gpu_launches": info["launches_per_call"] * args.steps,
+        "roofline": {
+            "bound": "alu", "kernel": "fused_kernel" if info["path"] == 0 else "trace_kernel",
+            "achieved": achieved, "peak": peak, "unit": "Tinst/s", "frac": achieved / peak,
+            "traffic": NCU_DRAM_BYTES_PER_LAUNCH,
+            "peak_source": "derived: %d SMs x %d issue slots/clk x %.0f MHz (MEASURED_PEAKS.json sm_max_mhz; "
+                           "slots/clk measured, profiles/r1_pipe_peaks.md)" % (info["n_sm"], SM_FP32_LANES, sm_max),
+            "kernel_ms": k_ms, "fp32_pipe_frac": fp32_frac, "mufu_pipe_frac": mufu_frac,
+            "algorithmic_issue_slots_per_likelihood": om["issue_slots"],
+            "hbm": {"algorithmic_bytes_per_step": hbm_bytes,
+                    "achieved_GBs": hbm_bytes / (k_ms * 1e-3) / 1e9,
+                    "peak_GBs": peaks.get("hbm_gbs"), "note": "compute-bound by design; HBM traffic is negligible"},
+        },
+        "launch": {k: info[k] for k in ("path", "block_threads", "ctas_per_sm", "grid", "smem_bytes")},
+        "checksum_logL": logl_sum,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        from oracle import oracle as O
+        O.lib()
+        n = args.ref_rows
+        dt, used = oracle_time(w, prob, rows[:n])
+        line["cpu_baseline"] = {"value": n / dt, "unit": UNIT, "cores": used, "kind": "oracle",
+                                "sample": "first %d of the %d rows of the step, %.1f s" % (n, B, dt)}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=1, help="BASELINE.json config index (default 1, the metric's)")
+    ap.add_argument("--batch", type=int, default=0, help="override rows per GPU (parity/debug only)")
+    ap.add_argument("--ref-rows", type=int, default=256, help="oracle sample size per step")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    w = W.workload(args.config)
+    if args.batch:
+        w = w.scaled(batch=args.batch)
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if world != args.gpus and world > 1:
+        raise SystemExit("--gpus %d does not match WORLD_SIZE %d" % (args.gpus, world))
+    if args.impl == "reference":
+        run_reference(args, w)
+    else:
+        run_ours(args, w)
+
+
+if __name__ == "__main__":
+    main()

@@ -141,6 +141,17 @@ int tl_render_batch(tl_ctx *ctx, const float *params, int64_t B, float *images, 
  */
 int tl_loglike_batch_host(tl_ctx *ctx, const float *params, int64_t B, float *logL, void *cuda_stream);
 
+/*
+ * Benchmark facility.  tl_set_profiling(ctx, 1) makes every later batch call record a pair of
+ * CUDA events, on the call's stream, around its dominant kernel (fused path: the fused kernel;
+ * split path: the ray-trace kernel) -- for a call that is split into several chunks, around the
+ * last chunk's.  tl_last_kernel_ms waits for the second event and returns the elapsed device
+ * time of that launch in milliseconds.  Not thread-safe: use one context per measuring thread.
+ * Returns TL_OK, TL_EINVAL (no profiled call pending) or TL_ECUDA.
+ */
+int tl_set_profiling(tl_ctx *ctx, int enable);
+int tl_last_kernel_ms(tl_ctx *ctx, float *ms);
+
 /* Release a context and its device memory (NULL is allowed).                                  */
 void tl_destroy(tl_ctx *ctx);
 

@@ -68,6 +68,8 @@ def load(build_if_missing: bool = True):
     L.tl_loglike_batch.restype = C.c_int; L.tl_loglike_batch.argtypes = [vp, vp, i64, vp, vp]
     L.tl_render_batch.restype = C.c_int; L.tl_render_batch.argtypes = [vp, vp, i64, vp, vp]
     L.tl_loglike_batch_host.restype = C.c_int; L.tl_loglike_batch_host.argtypes = [vp, vp, i64, vp, vp]
+    L.tl_set_profiling.restype = C.c_int; L.tl_set_profiling.argtypes = [vp, C.c_int]
+    L.tl_last_kernel_ms.restype = C.c_int; L.tl_last_kernel_ms.argtypes = [vp, C.POINTER(C.c_float)]
     L.tl_destroy.restype = None; L.tl_destroy.argtypes = [vp]
     L.tl_strerror.restype = C.c_char_p; L.tl_strerror.argtypes = [C.c_int]
     L.tl_version.restype = C.c_char_p; L.tl_version.argtypes = []
@@ -185,6 +187,16 @@ def tl_loglike_batch_host(handle: int, params_host, out_host=None, stream=None):
     return out_host
 
 
+def tl_set_profiling(handle: int, enable: bool):
+    _check(load().tl_set_profiling(handle, 1 if enable else 0), "tl_set_profiling")
+
+
+def tl_last_kernel_ms(handle: int) -> float:
+    ms = C.c_float()
+    _check(load().tl_last_kernel_ms(handle, C.byref(ms)), "tl_last_kernel_ms")
+    return float(ms.value)
+
+
 def tl_destroy(handle: Optional[int]):
     if handle:
         load().tl_destroy(handle)
@@ -217,6 +229,12 @@ class LensContext:
 
     def loglike_host(self, params_host, out_host=None, stream=None):
         return tl_loglike_batch_host(self.handle, params_host, out_host, stream)
+
+    def set_profiling(self, enable: bool = True):
+        tl_set_profiling(self.handle, enable)
+
+    def last_kernel_ms(self) -> float:
+        return tl_last_kernel_ms(self.handle)
 
     def close(self):
         if getattr(self, "handle", None):

@@ -29,13 +29,69 @@ struct tl_ctx {
     int path = 0;                 // 0 fused, 1 split
     int threads = 256, ctas_per_sm = 1, grid = 1;
     size_t smem = 0;
-    int tile_rows = 0, n_tiles = 0;
+    int tile_rows = 0, n_tiles = 0, G = 1, trace_slabs = 1;
+    void (*fused)(const tl::KArgs) = nullptr;
+    void (*trace)(const tl::KArgs, int) = nullptr;
     size_t conv_smem = 0;
     int64_t chunk_rows = 0;       // rows per scratch chunk
     double refine_tau = 3e-4;
+    // benchmark facility (tl_set_profiling): events around the dominant kernel of the last call
+    int profile = 0;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr;
+    float prof_ms = 0.f;          // accumulated over the chunks of the last call
+    int prof_pending = 0;
 };
 
 namespace {
+
+typedef void (*fused_fn)(const tl::KArgs);
+typedef void (*trace_fn)(const tl::KArgs, int);
+
+template <int S_T>
+fused_fn pick_fused(int nll, int nsrc)
+{
+    if (nll == 0) return nsrc == 1 ? tl::fused_kernel<S_T, 0, 1> : tl::fused_kernel<S_T, 0, 2>;
+    return nsrc == 1 ? tl::fused_kernel<S_T, 1, 1> : tl::fused_kernel<S_T, 1, 2>;
+}
+template <int S_T>
+trace_fn pick_trace(int nll, int nsrc)
+{
+    if (nll == 0) return nsrc == 1 ? tl::trace_kernel<S_T, 0, 1> : tl::trace_kernel<S_T, 0, 2>;
+    return nsrc == 1 ? tl::trace_kernel<S_T, 1, 1> : tl::trace_kernel<S_T, 1, 2>;
+}
+fused_fn fused_for(int S, int nll, int nsrc)
+{
+    switch (S) {
+    case 1: return pick_fused<1>(nll, nsrc);
+    case 2: return pick_fused<2>(nll, nsrc);
+    case 4: return pick_fused<4>(nll, nsrc);
+    case 8: return pick_fused<8>(nll, nsrc);
+    default: return pick_fused<0>(nll, nsrc);
+    }
+}
+trace_fn trace_for(int S, int nll, int nsrc)
+{
+    switch (S) {
+    case 1: return pick_trace<1>(nll, nsrc);
+    case 2: return pick_trace<2>(nll, nsrc);
+    case 4: return pick_trace<4>(nll, nsrc);
+    case 8: return pick_trace<8>(nll, nsrc);
+    default: return pick_trace<0>(nll, nsrc);
+    }
+}
+
+// phase-1 work split: G row groups per column; pick the G whose slowest thread does the least
+int best_row_groups(int He, int We, int threads)
+{
+    int best = 1; double best_cost = 1e300;
+    for (int G = 1; G <= 32 && G <= He; ++G) {
+        const int items = G * We;
+        const int rounds = (items + threads - 1) / threads;
+        const double cost = (double)rounds * ((He + G - 1) / G);      // pixels of the slowest thread
+        if (cost < best_cost - 1e-9) { best_cost = cost; best = G; }
+    }
+    return best;
+}
 
 constexpr size_t SMEM_LIMIT = 227 * 1024;
 constexpr int64_t CONST_CHUNK = 1 << 17;        // rows of RowC scratch per chunk (fused path)
@@ -62,7 +118,7 @@ tl::KArgs base_args(const tl_ctx *c)
     a.He = c->He; a.We = c->We; a.pitch = c->pitch; a.S = c->cfg.supersample;
     a.n_lens_light = c->cfg.n_lens_light; a.n_comp = c->n_comp;
     a.edge_zero = c->cfg.edge_mode == TL_EDGE_ZERO;
-    a.tile_rows = c->tile_rows; a.n_tiles = c->n_tiles;
+    a.tile_rows = c->tile_rows; a.n_tiles = c->n_tiles; a.G = c->G;
     return a;
 }
 
@@ -113,12 +169,15 @@ int run_batch(tl_ctx *c, const float *params, int64_t B, float *logL, float *ima
         if (c->path == 0) {
             int grid = c->grid;
             if ((int64_t)grid > nb) grid = (int)nb;
-            tl::fused_kernel<<<grid, c->threads, c->smem, st>>>(a);
+            if (c->profile) cudaEventRecord(c->ev0, st);
+            c->fused<<<grid, c->threads, c->smem, st>>>(a);
+            if (c->profile) { cudaEventRecord(c->ev1, st); c->prof_pending = 1; }
         } else {
             a.ext = ext; a.partial = logL ? partial : nullptr;
-            const int slabs = 8;
-            dim3 tg((unsigned)(nb < 65535 ? nb : 65535), slabs);
-            tl::trace_kernel<<<tg, 256, 0, st>>>(a, (int)nb);
+            dim3 tg((unsigned)(nb < 65535 ? nb : 65535), (unsigned)c->trace_slabs);
+            if (c->profile) cudaEventRecord(c->ev0, st);
+            c->trace<<<tg, 256, 0, st>>>(a, (int)nb);
+            if (c->profile) { cudaEventRecord(c->ev1, st); c->prof_pending = 1; }
             dim3 cg((unsigned)nb, (unsigned)c->n_tiles);
             tl::conv_kernel<<<cg, 256, c->conv_smem, st>>>(a, (int)nb);
             if (logL) tl::finalize_kernel<<<(unsigned)((nb + 127) / 128), 128, 0, st>>>(a, (int)nb);
@@ -227,9 +286,12 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
     if (fs <= SMEM_LIMIT) {
         c->path = 0; c->smem = fs;
         c->threads = fs > SMEM_LIMIT / 2 ? 512 : 256;
-        if (!cuda_ok(cudaFuncSetAttribute(tl::fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT))) { tl_destroy(c); return TL_ECUDA; }
+        if (const char *e = std::getenv("TL_THREADS")) { const int v = std::atoi(e); if (v >= 32 && v <= 512 && v % 32 == 0) c->threads = v; }
+        c->fused = fused_for(cfg->supersample, cfg->n_lens_light, cfg->n_source);
+        c->G = best_row_groups(c->He, c->We, c->threads);
+        if (!cuda_ok(cudaFuncSetAttribute(c->fused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT))) { tl_destroy(c); return TL_ECUDA; }
         int occ = 0;
-        if (!cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, tl::fused_kernel, c->threads, fs)) || occ < 1) { tl_destroy(c); return TL_ECUDA; }
+        if (!cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, c->fused, c->threads, fs)) || occ < 1) { tl_destroy(c); return TL_ECUDA; }
         c->ctas_per_sm = occ; c->grid = occ * c->n_sm;
         c->chunk_rows = CONST_CHUNK;
     } else {
@@ -243,8 +305,12 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
         c->conv_smem = conv_smem_bytes(c, tr);
         if (!cuda_ok(cudaFuncSetAttribute(tl::conv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT))) { tl_destroy(c); return TL_ECUDA; }
         c->threads = 256; c->smem = c->conv_smem;
+        c->trace = trace_for(cfg->supersample, cfg->n_lens_light, cfg->n_source);
+        // one CTA slab = 256 columns-items; G row groups so that a row of the batch fills >= 8 CTAs
+        c->trace_slabs = 8;
+        c->G = best_row_groups(c->He, c->We, 256 * c->trace_slabs);
         int occ = 0;
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, tl::trace_kernel, 256, 0);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, c->trace, 256, 0);
         c->ctas_per_sm = occ > 0 ? occ : 1; c->grid = 0;
         int64_t cr = (int64_t)(EXT_SCRATCH_BYTES / (sizeof(float) * (size_t)c->He * c->pitch));
         if (cr < 1) cr = 1;
@@ -299,9 +365,29 @@ int tl_loglike_batch_host(tl_ctx *ctx, const float *params, int64_t B, float *lo
     return rc;
 }
 
+int tl_set_profiling(tl_ctx *c, int enable)
+{
+    if (!c) return TL_EINVAL;
+    if (enable && !c->ev0) {
+        if (!cuda_ok(cudaEventCreate(&c->ev0)) || !cuda_ok(cudaEventCreate(&c->ev1))) return TL_ECUDA;
+    }
+    c->profile = enable ? 1 : 0;
+    c->prof_pending = 0;
+    return TL_OK;
+}
+
+int tl_last_kernel_ms(tl_ctx *c, float *ms)
+{
+    if (!c || !ms || !c->profile || !c->prof_pending) return TL_EINVAL;
+    if (!cuda_ok(cudaEventSynchronize(c->ev1)) || !cuda_ok(cudaEventElapsedTime(ms, c->ev0, c->ev1))) return TL_ECUDA;
+    return TL_OK;
+}
+
 void tl_destroy(tl_ctx *c)
 {
     if (!c) return;
+    if (c->ev0) cudaEventDestroy(c->ev0);
+    if (c->ev1) cudaEventDestroy(c->ev1);
     cudaFree(c->psf); cudaFree(c->data); cudaFree(c->wgt); cudaFree(c->sigma_min); cudaFree(c->lconst);
     delete c;
 }

@@ -9,6 +9,13 @@
 // Units: positions are carried in "u-units", u = pix_scale / (2 S) arcsec, in which every
 // sub-sample coordinate is an odd integer (exact in FP32).  The SIE deflection is homogeneous
 // of degree 0 in position and the shear is linear, so only the constants change.
+//
+// Frames: the ray-trace works in the LENS frame (rotated by phi about the lens centre),
+//     (x', y') = R^T (theta - c),   R = [[cos phi, -sin phi], [sin phi, cos phi]],
+// and never rotates back: with Gamma = [[g1, g2], [g2, -g1]] (alpha_shear = -Gamma theta),
+//     R^T beta = N (theta - c) + D0 - alpha',   N = R^T (I + Gamma),  D0 = N c,
+// where alpha' = (alpha_x', alpha_y') is the SIE deflection in its own frame.  Every source
+// Sersic is expressed as a quadratic form in the lens-frame offset R^T (beta - s).
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
@@ -20,26 +27,35 @@ constexpr int MAX_COMP = 3;          // n_lens_light (<= 1) + n_source (<= 2)
 struct LensC {                       // SIE + external shear
     float cXh, cXl, cYh, cYl;        // centre, u-units
     float ch, cl, sh, sl;            // cos(phi), sin(phi)
-    float q2h, q2l, qph, qpl;        // q^2, q' = sqrt(1 - q^2)
-    float fh, fl;                    // theta_E sqrt(q) / q', u-units
-    float g1, g2;                    // shear
-    double dcX, dcY, dc, ds, dq2, dqp, df;   // FP64 copies for the selective refinement
-    int32_t valid, pad;
+    float n11h, n11l, n12h, n12l;    // N = R^T (I + Gamma)
+    float n21h, n21l, n22h, n22l;
+    float d1h, d1l, d2h, d2l;        // D0 = N c
+    float q2h, q2l;                  // q^2
+    float qph, qpl;                  // q' = sqrt(1 - q^2)  (clamped at 1e-6)
+    float c0, s0, qc0, qs0;          // cos/sin(theta0), q' cos/sin(theta0), theta0 = atan(q'/q)/2
+    float z0, z0qp;                  // z0 = tanh(atanh(q')/2),  z0 q'
+    float fh, fl;                    // f = theta_E sqrt(q) / q', u-units
+    float ft0h, ft0l;                // f theta0
+    float fT2h, fT2l;                // f atanh(q') / 2
+    int32_t mode;                    // 0: polynomial path (q >= 0.5), 1: libdevice path
+    int32_t valid;
+    double dcX, dcY, dc, ds, dq2, dqp, df, dg1, dg2;   // FP64 copies for the selective refinement
 };
 
 struct SersicC {                     // one elliptical Sersic component
-    float cXh, cXl, cYh, cYl;        // centre, u-units
-    float c, s;                      // cos, sin of the position angle
-    float A, B;                      // q u^2 / r_e^2,  u^2 / (q r_e^2):  t = A x1^2 + B x2^2 = (R_p/r_e)^2
+    // lens light: centre in the image frame (u-units); source: R^T s in the lens frame
+    float cXh, cXl, cYh, cYl;
+    // quadratic form t = (R_p / r_e)^2 = a x^2 + b2 x y + cc y^2 in the frame of the offsets
+    float ah, al, b2h, b2l, cch, ccl;
     float ph, pl;                    // 1 / (2 n)
     float kh, kl;                    // b_n log2(e)
     float amp;                       // I_e / S^2
-    float cflag;                     // refinement criterion constant (sources only, else 0)
+    float lcf;                       // log2 of the refinement criterion constant (sources), else -1e30
     int32_t valid, pad;
-    double dcX, dcY;                 // FP64 centre for the refinement
+    double dcX, dcY;                 // image-frame centre (u-units), FP64, for the refinement
 };
 
-struct RowC {
+struct alignas(16) RowC {
     LensC lens;
     SersicC comp[MAX_COMP];
 };
@@ -125,66 +141,90 @@ __global__ void __launch_bounds__(128) prologue_kernel(PrologueArgs a)
     const float *p = a.params + row * a.P;
     RowC *rc = a.rows + row;
 
+    // lens shape is needed by every slot (sources live in the lens frame)
+    bool lens_ok = true;
+    for (int i = 0; i < 7; ++i) lens_ok = lens_ok && isfinite(p[i]);
+    double thE = p[0], q = 1.0, c = 1.0, s = 0.0;
+    lens_ok = lens_ok && (thE >= 0.0);
+    lens_ok = lens_ok && shape_from_e(p[1], p[2], &q, &c, &s);
+    if (!lens_ok) { thE = 0.0; q = 1.0; c = 1.0; s = 0.0; }
+
     if (slot == 0) {
         LensC L;
-        bool ok = true;
-        for (int i = 0; i < 7; ++i) ok = ok && isfinite(p[i]);
-        double thE = p[0], q = 1.0, c = 1.0, s = 0.0;
-        ok = ok && (thE >= 0.0);
-        ok = ok && shape_from_e(p[1], p[2], &q, &c, &s);
-        if (!ok) { thE = 0.0; q = 1.0; c = 1.0; s = 0.0; }
         // q' = sqrt((1-q)(1+q)); clamped away from 0 so that f = theta_E sqrt(q)/q' stays
         // finite: for q' <= 1e-6 the exact deflection differs from the clamped one by a
-        // relative O(q'^2) < 1e-12 (A(z), H(z) -> 1).
+        // relative O(q'^2) < 1e-12 (atan(z)/z, atanh(z)/z -> 1).
         double qp = fmax(sqrt((1.0 - q) * (1.0 + q)), 1e-6);
         double f = thE * sqrt(q) / qp * a.inv_u;
-        double cX = (double)p[3] * a.inv_u, cY = (double)p[4] * a.inv_u;
+        double g1 = lens_ok ? (double)p[5] : 0.0, g2 = lens_ok ? (double)p[6] : 0.0;
+        double cX = (lens_ok ? (double)p[3] : 0.0) * a.inv_u, cY = (lens_ok ? (double)p[4] : 0.0) * a.inv_u;
+        double n11 = c * (1.0 + g1) + s * g2, n12 = c * g2 + s * (1.0 - g1);
+        double n21 = -s * (1.0 + g1) + c * g2, n22 = -s * g2 + c * (1.0 - g1);
+        double d1 = n11 * cX + n12 * cY, d2 = n21 * cX + n22 * cY;
+        double th0 = 0.5 * atan2(qp, q), c0 = cos(th0), s0 = sin(th0);
+        double T = atanh(fmin(qp, 1.0 - 1e-16)), z0 = tanh(0.5 * T);
         split2(cX, &L.cXh, &L.cXl); split2(cY, &L.cYh, &L.cYl);
         split2(c, &L.ch, &L.cl);    split2(s, &L.sh, &L.sl);
+        split2(n11, &L.n11h, &L.n11l); split2(n12, &L.n12h, &L.n12l);
+        split2(n21, &L.n21h, &L.n21l); split2(n22, &L.n22h, &L.n22l);
+        split2(d1, &L.d1h, &L.d1l); split2(d2, &L.d2h, &L.d2l);
         split2(q * q, &L.q2h, &L.q2l); split2(qp, &L.qph, &L.qpl);
+        L.c0 = (float)c0; L.s0 = (float)s0; L.qc0 = (float)(qp * c0); L.qs0 = (float)(qp * s0);
+        L.z0 = (float)z0; L.z0qp = (float)(z0 * qp);
         split2(f, &L.fh, &L.fl);
-        L.g1 = ok ? p[5] : 0.f; L.g2 = ok ? p[6] : 0.f;
+        split2(f * th0, &L.ft0h, &L.ft0l);
+        split2(f * 0.5 * T, &L.fT2h, &L.fT2l);
+        L.mode = (q >= 0.5) ? 0 : 1;
+        L.valid = lens_ok ? 1 : 0;
         L.dcX = cX; L.dcY = cY; L.dc = c; L.ds = s; L.dq2 = q * q; L.dqp = qp; L.df = f;
-        L.valid = ok ? 1 : 0; L.pad = 0;
+        L.dg1 = g1; L.dg2 = g2;
         rc->lens = L;
         return;
     }
 
     const int k = slot - 1;
+    const bool is_lens_light = k < a.n_lens_light;
     const float *sp = p + 7 + 7 * k;
     SersicC C;
     bool ok = true;
     for (int i = 0; i < 7; ++i) ok = ok && isfinite(sp[i]);
-    double Ie = sp[0], re = sp[1], n = sp[2], q = 1.0, c = 1.0, s = 0.0;
+    double Ie = sp[0], re = sp[1], n = sp[2], qs = 1.0, cs = 1.0, ss = 0.0;
     ok = ok && (re > 0.0) && (n > 0.0);
-    ok = ok && shape_from_e(sp[3], sp[4], &q, &c, &s);
-    if (!ok) { Ie = 0.0; re = 1.0; n = 1.0; q = 1.0; c = 1.0; s = 0.0; }
-    double bn = sersic_bn(n);
-    double u_arc = 1.0 / a.inv_u;                     // arcsec per u-unit
-    double cX = (ok ? (double)sp[5] : 0.0) * a.inv_u, cY = (ok ? (double)sp[6] : 0.0) * a.inv_u;
-    split2(cX, &C.cXh, &C.cXl); split2(cY, &C.cYh, &C.cYl);
-    C.c = (float)c; C.s = (float)s;
-    C.A = (float)(q * u_arc * u_arc / (re * re));
-    C.B = (float)(u_arc * u_arc / (q * re * re));
+    ok = ok && shape_from_e(sp[3], sp[4], &qs, &cs, &ss);
+    if (!ok) { Ie = 0.0; re = 1.0; n = 1.0; qs = 1.0; cs = 1.0; ss = 0.0; }
+    const double bn = sersic_bn(n);
+    const double u_arc = 1.0 / a.inv_u;                     // arcsec per u-unit
+    const double cX = (ok ? (double)sp[5] : 0.0) * a.inv_u, cY = (ok ? (double)sp[6] : 0.0) * a.inv_u;
+    C.dcX = cX; C.dcY = cY;
+    // Eq. 10: t = (R_p/r_e)^2 = A x1^2 + B x2^2 in the component's own frame
+    const double A = qs * u_arc * u_arc / (re * re), Bq = u_arc * u_arc / (qs * re * re);
+    // rotation from the frame the offsets are given in to the component frame
+    double cd, sd, oX, oY;
+    if (is_lens_light) { cd = cs; sd = ss; oX = cX; oY = cY; }                 // image frame
+    else {                                                                      // lens frame
+        cd = cs * c + ss * s; sd = ss * c - cs * s;                             // cos, sin(phi_s - phi)
+        oX = c * cX + s * cY; oY = -s * cX + c * cY;                            // R^T s
+    }
+    split2(oX, &C.cXh, &C.cXl); split2(oY, &C.cYh, &C.cYl);
+    split2(A * cd * cd + Bq * sd * sd, &C.ah, &C.al);
+    split2(2.0 * (A - Bq) * cd * sd, &C.b2h, &C.b2l);
+    split2(A * sd * sd + Bq * cd * cd, &C.cch, &C.ccl);
     split2(0.5 / n, &C.ph, &C.pl);
     split2(bn * 1.4426950408889634074, &C.kh, &C.kl);
-    double amp = Ie / (double)(a.S * a.S);
+    const double amp = Ie / (double)(a.S * a.S);
     C.amp = (float)amp;
     // Selective FP64 refinement of beta:
     // the FP32 ray-trace carries an absolute error delta_beta ~ 2^-22 (theta_E + |theta|);
     // the induced brightness error of a sample is  I (b_n/n) u delta_beta / R.  It is refined
-    // when that exceeds tau * sigma_min:   (cflag * e * u)^2 > t,  t = (R/r_e)^2.
-    C.cflag = 0.f;
-    if (k >= a.n_lens_light && ok) {
-        double thE = fmax((double)p[0], 0.0);
-        double dbeta = 2.4e-7 * (thE + a.fov_half);               // arcsec
+    // when that exceeds tau * sigma_min:  (cf e u)^2 > t, i.e. in log2:  lcf + arg + vp > v/2.
+    C.lcf = -1e30f;
+    if (!is_lens_light && ok && amp != 0.0) {
+        double dbeta = 2.4e-7 * (fmax((double)p[0], 0.0) + a.fov_half);               // arcsec
         double smin = a.sigma_min[(a.row0 + row) / a.rows_per_lens];
-        double thr = a.refine_tau * smin;
-        double cf = fabs(amp) * (bn / n) * dbeta / (re * thr);
-        C.cflag = (float)fmin(cf, 1e30);
+        double cf = fabs(amp) * (bn / n) * dbeta / (re * a.refine_tau * smin);
+        C.lcf = (float)fmin(fmax(log2(cf), -1e30), 1e30);
     }
     C.valid = ok ? 1 : 0; C.pad = 0;
-    C.dcX = cX; C.dcY = cY;
     rc->comp[k] = C;
 }
 

@@ -31,6 +31,7 @@ struct KArgs {
     int64_t B, rows_per_lens, row0;
     int ny, nx, K, Kp, h, He, We, pitch, S, n_lens_light, n_comp, edge_zero;
     int tile_rows, n_tiles;  // split path
+    int G;                   // phase-1 row groups per column (see trace_image)
 };
 
 __device__ __forceinline__ bool row_is_valid(const RowC &rc, int n_comp)
@@ -40,23 +41,133 @@ __device__ __forceinline__ bool row_is_valid(const RowC &rc, int n_comp)
     return ok;
 }
 
-// steps a1-a5 for one extended native pixel (i, j)
-__device__ __forceinline__ float trace_pixel(const RowC &rc, const KArgs &a, int i, int j)
+// Values that depend only on the sub-sample column (abscissa X) / only on the sub-sample row
+// (ordinate Y).  x' = Pc + Qs, y' = Qc - Ps, N (theta - c) + D0 = (U + V, U2 + V2); the
+// lens-light quadratic form is  t = LA + LC + LB * dyl.
+struct ColV { float Pc, Ps, U, U2, LA, LB; };
+struct RowV { float Qc, Qs, V, V2, LC, dyl; };
+
+template <int NLL>
+__device__ __forceinline__ ColV col_values(const RowC &rc, float X)
 {
-    const int S = a.S;
-    if (a.edge_zero && (i < a.h || i >= a.He - a.h || j < a.h || j >= a.We - a.h)) return 0.f;
-    // u-units: X = 2 (j S + b) + 1 - S We is the exact sub-sample abscissa (DESIGN.md a1)
-    const float X0 = (float)(2 * j * S + 1 - S * a.We);
-    const float Y0 = (float)(2 * i * S + 1 - S * a.He);
+    const LensC &L = rc.lens;
+    ColV c;
+    const float dx = (X - L.cXh) - L.cXl;
+    c.Pc = fmaf(dx, L.cl, dx * L.ch);
+    c.Ps = fmaf(dx, L.sl, dx * L.sh);
+    c.U = fmaf(dx, L.n11l, dx * L.n11h);
+    c.U2 = fmaf(dx, L.n21l, dx * L.n21h);
+    if (NLL) {
+        const SersicC &C = rc.comp[0];
+        const float dxl = (X - C.cXh) - C.cXl;
+        c.LA = fmaf(C.al * dxl, dxl, (C.ah * dxl) * dxl);
+        c.LB = fmaf(dxl, C.b2l, dxl * C.b2h);
+    } else { c.LA = 0.f; c.LB = 0.f; }
+    return c;
+}
+
+template <int NLL>
+__device__ __forceinline__ RowV row_values(const RowC &rc, float Y)
+{
+    const LensC &L = rc.lens;
+    RowV r;
+    const float dy = (Y - L.cYh) - L.cYl;
+    r.Qc = fmaf(dy, L.cl, dy * L.ch);
+    r.Qs = fmaf(dy, L.sl, dy * L.sh);
+    r.V = fmaf(dy, L.n12h, L.d1h) + fmaf(dy, L.n12l, L.d1l);
+    r.V2 = fmaf(dy, L.n22h, L.d2h) + fmaf(dy, L.n22l, L.d2l);
+    if (NLL) {
+        const SersicC &C = rc.comp[0];
+        r.dyl = (Y - C.cYh) - C.cYl;
+        r.LC = fmaf(C.ccl * r.dyl, r.dyl, (C.cch * r.dyl) * r.dyl);
+    } else { r.dyl = 0.f; r.LC = 0.f; }
+    return r;
+}
+
+// One sub-sample (steps a2-a4, Eq. 2): lens light at theta + sources at beta,
+// already scaled by 1/S^2 so that the caller only adds (step a5, bin = mean).
+template <int NLL, int NSRC>
+__device__ __forceinline__ float sample_value(const RowC &rc, const ColV &c, const RowV &r, float X, float Y)
+{
     float acc = 0.f;
-    for (int sa = 0; sa < S; ++sa) {
-        const float Y = Y0 + (float)(2 * sa);
-        for (int sb = 0; sb < S; ++sb) {
-            const float X = X0 + (float)(2 * sb);
-            acc += sample_value<true>(rc, a.n_lens_light, a.n_comp, X, Y);
+    bool flag = false, fl;
+    if (NLL) acc = sersic_from_t(rc.comp[0], fmaf(c.LB, r.dyl, c.LA + r.LC), fl);
+    const float xp = c.Pc + r.Qs, yp = r.Qc - c.Ps;
+    float axp, ayp;
+    sie_alpha(rc.lens, xp, yp, axp, ayp);
+    const float bx = (c.U + r.V) - axp, by = (c.U2 + r.V2) - ayp;      // R^T beta
+    float src = 0.f;
+#pragma unroll
+    for (int k = NLL; k < NLL + NSRC; ++k) {
+        const SersicC &C = rc.comp[k];
+        src += sersic_from_t(C, quad_form(C, (bx - C.cXh) - C.cXl, (by - C.cYh) - C.cYl), fl);
+        flag = flag || fl;
+    }
+    if (flag) {                                     // rare: FP64 ray-trace for this sample
+        src = 0.f;
+#pragma unroll
+        for (int k = NLL; k < NLL + NSRC; ++k) {
+            const SersicC &C = rc.comp[k];
+            float xi, eta;
+            refine_offsets(rc.lens, C, X, Y, xi, eta);
+            src += sersic_from_t(C, quad_form(C, xi, eta), fl);
         }
     }
-    return acc;
+    return acc + src;
+}
+
+// steps a1-a5 for the extended native pixels of column j, rows i = i_first, i_first + i_step, ...
+// S_T > 0: compile-time supersampling (column values live in registers); S_T = 0: any S.
+template <int S_T, int NLL, int NSRC, class Store>
+__device__ __forceinline__ void trace_column(const RowC &rc, const KArgs &a, int j, int i_first, int i_step, Store store)
+{
+    const int S = S_T > 0 ? S_T : a.S;
+    const bool edge_col = a.edge_zero && (j < a.h || j >= a.We - a.h);
+    // u-units: X = 2 (j S + b) + 1 - S We is the exact sub-sample abscissa (DESIGN.md a1)
+    const float X0 = (float)(2 * j * S + 1 - S * a.We);
+    ColV cv[S_T > 0 ? S_T : 1];
+    if (S_T > 0) {
+#pragma unroll
+        for (int b = 0; b < S_T; ++b) cv[b] = col_values<NLL>(rc, X0 + (float)(2 * b));
+    }
+    for (int i = i_first; i < a.He; i += i_step) {
+        float acc = 0.f;
+        if (!(edge_col || (a.edge_zero && (i < a.h || i >= a.He - a.h)))) {
+            const float Y0 = (float)(2 * i * S + 1 - S * a.He);
+            if (S_T > 0) {
+#pragma unroll
+                for (int sa = 0; sa < S_T; ++sa) {
+                    const float Y = Y0 + (float)(2 * sa);
+                    const RowV rv = row_values<NLL>(rc, Y);
+#pragma unroll
+                    for (int sb = 0; sb < S_T; ++sb)
+                        acc += sample_value<NLL, NSRC>(rc, cv[sb], rv, X0 + (float)(2 * sb), Y);
+                }
+            } else {
+                for (int sa = 0; sa < S; ++sa) {
+                    const float Y = Y0 + (float)(2 * sa);
+                    const RowV rv = row_values<NLL>(rc, Y);
+                    for (int sb = 0; sb < S; ++sb) {
+                        const float X = X0 + (float)(2 * sb);
+                        acc += sample_value<NLL, NSRC>(rc, col_values<NLL>(rc, X), rv, X, Y);
+                    }
+                }
+            }
+        }
+        store(i, j, acc);
+    }
+}
+
+// Work distribution of phase 1: items (g, j), g < G row groups; item (g, j) owns the pixels of
+// column j in rows g, g + G, ...   Threads take items tid, tid + blockDim, ...
+template <int S_T, int NLL, int NSRC, class Store>
+__device__ __forceinline__ void trace_image(const RowC &rc, const KArgs &a, int item0, int item_step, Store store)
+{
+    const int items = a.G * a.We;
+    for (int it = item0; it < items; it += item_step) {
+        const int g = it / a.We, j = it - g * a.We;
+        trace_column<S_T, NLL, NSRC>(rc, a, j, g, a.G, store);
+    }
 }
 
 // step a6 for a 1 x CONV_R strip whose window starts at `win` (16-byte aligned) in an image of
@@ -142,6 +253,7 @@ __device__ __forceinline__ double conv_chi2_rows(const KArgs &a, const float *im
 }
 
 // ------------------------------------------------------------------------------ fused path
+template <int S_T, int NLL, int NSRC>
 __global__ void __launch_bounds__(512) fused_kernel(const KArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -170,11 +282,8 @@ __global__ void __launch_bounds__(512) fused_kernel(const KArgs a)
             continue;
         }
         // phase 1: ray-trace + light + bin into shared memory
-        const int next = a.He * a.We;
-        for (int pix = threadIdx.x; pix < next; pix += blockDim.x) {
-            const int i = pix / a.We, j = pix - i * a.We;
-            img[i * a.pitch + j] = trace_pixel(*rc, a, i, j);
-        }
+        trace_image<S_T, NLL, NSRC>(*rc, a, threadIdx.x, blockDim.x,
+                                    [&](int i, int j, float v) { img[i * a.pitch + j] = v; });
         __syncthreads();
         // phase 2: PSF convolution from shared memory + chi^2
         const double part = conv_chi2_rows(a, img, 0, taps, 0, a.ny,
@@ -190,24 +299,20 @@ __global__ void __launch_bounds__(512) fused_kernel(const KArgs a)
 }
 
 // ------------------------------------------------------------------------------ split path
-// trace_kernel: grid-stride over (row, extended pixel) of the current chunk.
+// trace_kernel: one parameter row per blockIdx.x iteration, the row's items spread over
+// gridDim.y CTAs (slabs); binned extended image -> global memory.
+template <int S_T, int NLL, int NSRC>
 __global__ void __launch_bounds__(256) trace_kernel(const KArgs a, int chunk_rows)
 {
     __shared__ RowC rc_s;
-    // one row per CTA-iteration keeps the constants in shared memory; the row's pixels are
-    // spread over `n_tiles`-independent CTAs: blockIdx = (row_in_chunk, slab)
-    const int slabs = gridDim.y;
     for (int r = blockIdx.x; r < chunk_rows; r += gridDim.x) {
         __syncthreads();
         load_row_consts(&rc_s, a.rows + r);
         __syncthreads();
         if (!row_is_valid(rc_s, a.n_comp)) continue;
         float *dst = a.ext + (size_t)r * a.He * a.pitch;
-        const int next = a.He * a.We;
-        for (int pix = blockIdx.y * blockDim.x + threadIdx.x; pix < next; pix += slabs * blockDim.x) {
-            const int i = pix / a.We, j = pix - i * a.We;
-            dst[i * a.pitch + j] = trace_pixel(rc_s, a, i, j);
-        }
+        trace_image<S_T, NLL, NSRC>(rc_s, a, blockIdx.y * blockDim.x + threadIdx.x, gridDim.y * blockDim.x,
+                                    [&](int i, int j, float v) { dst[i * a.pitch + j] = v; });
     }
 }
 

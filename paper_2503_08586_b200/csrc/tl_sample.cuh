@@ -1,114 +1,128 @@
 // tl_sample.cuh -- per-sub-sample arithmetic: steps a2 (deflection), a3 (source light),
-// a4 (lens light) of DESIGN.md.  FP32 with hi/lo constants; FP64 only in refine_beta().
+// a4 (lens light) of DESIGN.md.  FP32 with hi/lo constants; FP64 only in refine_offsets().
 //
 // SIE deflection (Eq. 12 with gamma = 2 made elliptical through R_p of
-// PAPER.md:143-148 Eq. 10; Kormann et al. 1994 closed form, G1), in the frame
-// rotated by phi about the lens centre:
+// PAPER.md:143-148 Eq. 10; Kormann et al. 1994 closed form, G1), in the lens frame:
 //     psi = sqrt(q^2 x'^2 + y'^2),  f = theta_E sqrt(q) / q',
 //     alpha_x' = f atan(q' x' / psi),   alpha_y' = f atanh(q' y' / psi).
-// External shear (PAPER.md:162 Eq. 13, :187-190 Eq. 14; G4, G5):
-//     alpha_shear = -(g1 x + g2 y, g2 x - g1 y)   about the image origin.
-// Ray-trace (Eq. 1): beta = theta - alpha.
-// Sersic (Eq. 8): I = I_e exp(-b_n (u - 1)),  u = (R_p/r_e)^(1/n) = t^(1/2n).
+// Both inverse functions are evaluated without range tests:
+//   atan:  the angle of (psi, q'|x'|) lies in [0, thmax], thmax = atan(q'/q); rotating the
+//          vector by -theta0 = -thmax/2 leaves an angle in [-theta0, theta0], |tan| <= 0.58 for
+//          q >= 0.5, where a degree-5 odd minimax polynomial is exact to 5e-9;
+//   atanh: z = q'|y'|/psi lies in [0, q']; the hyperbolic shift by T/2, T = atanh(q'),
+//          r = (z - z0)/(1 - z z0), z0 = tanh(T/2), leaves |r| <= z0 <= 0.58 (degree-6, 4e-9).
+// One MUFU.RSQ and two MUFU.RCP per sample; rows with q < 0.5 take the libdevice path.
+// External shear (PAPER.md:162 Eq. 13, :187-190 Eq. 14; G4, G5) and the identity are the
+// linear map N of tl_consts.cuh.  Ray-trace (Eq. 1): beta = theta - alpha.
+// Sersic (Eq. 8): I = I_e exp(-b_n (u - 1)),  u = (R_p/r_e)^(1/n) = t^(1/2n),
+// evaluated as amp * ex2(k (1 - ex2(p lg2 t))) with three MUFU ops.
 #pragma once
 #include "tl_consts.cuh"
 
 namespace tl {
 
-// ---- step a2, FP32 ---------------------------------------------------------------------
-__device__ __forceinline__ void deflect_f32(const LensC &L, float X, float Y, float &bx, float &by)
+__device__ __forceinline__ float mufu_ex2(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float mufu_lg2(float x) { float y; asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float mufu_rsq(float x) { float y; asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float mufu_rcp(float x) { float y; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+
+// atan(r) for |r| <= 0.58 (max relative error 4.6e-9 before rounding)
+__device__ __forceinline__ float atan_small(float r)
 {
-    float dx = (X - L.cXh) - L.cXl;
-    float dy = (Y - L.cYh) - L.cYl;
-    // rotate into the lens frame with hi/lo cos, sin
-    float xp = fmaf(dx, L.ch, fmaf(dy, L.sh, fmaf(dx, L.cl, dy * L.sl)));
-    float yp = fmaf(dy, L.ch, fmaf(-dx, L.sh, fmaf(dy, L.cl, -dx * L.sl)));
-    float xx = xp * xp;
-    float psi2 = fmaf(L.q2h, xx, fmaf(L.q2l, xx, yp * yp));
-    float psi = sqrtf(psi2);
-    float nx = fmaf(L.qpl, xp, L.qph * xp);         // q' x'
-    float ny = fmaf(L.qpl, yp, L.qph * yp);         // q' y'
-    float at = atan2f(nx, psi);                     // psi >= 0: angle in [-pi/2, pi/2]
-    float zy = psi2 > 0.f ? ny / psi : 0.f;         // |zy| <= q' < 1; alpha = 0 at psi = 0 (G6)
-    float ah = atanhf(zy);
-    float axp = fmaf(L.fl, at, L.fh * at);
-    float ayp = fmaf(L.fl, ah, L.fh * ah);
-    // rotate back
-    float ax = fmaf(axp, L.ch, fmaf(-ayp, L.sh, fmaf(axp, L.cl, -ayp * L.sl)));
-    float ay = fmaf(axp, L.sh, fmaf(ayp, L.ch, fmaf(axp, L.sl, ayp * L.cl)));
-    // beta = theta - alpha_SIE - alpha_shear
-    bx = fmaf(L.g1, X, fmaf(L.g2, Y, X - ax));
-    by = fmaf(L.g2, X, fmaf(-L.g1, Y, Y - ay));
+    const float s = r * r;
+    float p = 3.199305013e-02f;
+    p = fmaf(p, s, -7.467620820e-02f);
+    p = fmaf(p, s, 1.079487726e-01f);
+    p = fmaf(p, s, -1.425360143e-01f);
+    p = fmaf(p, s, 1.999849826e-01f);
+    p = fmaf(p, s, -3.333331048e-01f);
+    return fmaf(r * s, p, r);
 }
 
-// ---- step a2, FP64 (selective refinement only) --------------------------------------------
-__device__ __noinline__ void refine_beta(const LensC &L, float Xf, float Yf, double &bx, double &by)
+// atanh(r) for |r| <= 0.58 (max relative error 4.3e-9 before rounding)
+__device__ __forceinline__ float atanh_small(float r)
 {
-    double X = Xf, Y = Yf;
-    double dx = X - L.dcX, dy = Y - L.dcY;
-    double xp = dx * L.dc + dy * L.ds;
-    double yp = dy * L.dc - dx * L.ds;
-    double psi = sqrt(L.dq2 * xp * xp + yp * yp);
+    const float s = r * r;
+    float p = 2.593644857e-01f;
+    p = fmaf(p, s, -5.470913649e-02f);
+    p = fmaf(p, s, 1.322188675e-01f);
+    p = fmaf(p, s, 1.043291166e-01f);
+    p = fmaf(p, s, 1.434355527e-01f);
+    p = fmaf(p, s, 1.999771595e-01f);
+    p = fmaf(p, s, 3.333336413e-01f);
+    return fmaf(r * s, p, r);
+}
+
+// ---- step a2: SIE deflection in the lens frame ---------------------------------------------
+__device__ __forceinline__ void sie_alpha(const LensC &L, float xp, float yp, float &axp, float &ayp)
+{
+    const float xx = xp * xp;
+    const float psi2 = fmaf(L.q2h, xx, fmaf(L.q2l, xx, yp * yp));
+    const float rpsi = mufu_rsq(fmaxf(psi2, 1e-30f));          // alpha = 0 at psi = 0 (G6)
+    const float psi = psi2 * rpsi;
+    const float ax = fabsf(xp), ay = fabsf(yp);
+    if (L.mode == 0) {
+        // atan: rotate (psi, q'|x'|) by -theta0
+        const float d2 = fmaf(ax, L.qs0, psi * L.c0);
+        const float n2 = fmaf(ax, L.qc0, -psi * L.s0);
+        const float pa = atan_small(n2 * mufu_rcp(d2));
+        const float a1 = fmaf(L.fh, pa, L.ft0h) + fmaf(L.fl, pa, L.ft0l);
+        // atanh: hyperbolic shift of z = q'|y'|/psi by z0
+        const float num = fmaf(ay, L.qph, -L.z0 * psi);
+        const float den = fmaf(-ay, L.z0qp, psi);
+        const float ph = atanh_small(num * mufu_rcp(den));
+        const float a2 = fmaf(L.fh, ph, L.fT2h) + fmaf(L.fl, ph, L.fT2l);
+        axp = psi2 > 0.f ? copysignf(a1, xp) : 0.f;
+        ayp = psi2 > 0.f ? copysignf(a2, yp) : 0.f;
+    } else {
+        // strongly flattened lenses (q < 0.5): libdevice inverse functions
+        const float nx = fmaf(L.qpl, xp, L.qph * xp), ny = fmaf(L.qpl, yp, L.qph * yp);
+        const float at = atan2f(nx, psi);
+        const float ah = atanhf(psi2 > 0.f ? ny / psi : 0.f);
+        axp = fmaf(L.fl, at, L.fh * at);
+        ayp = fmaf(L.fl, ah, L.fh * ah);
+    }
+}
+
+// ---- step a2 in FP64 (selective refinement only): lens-frame offset R^T (beta - s) ----------
+__device__ __noinline__ void refine_offsets(const LensC &L, const SersicC &C, float Xf, float Yf,
+                                            float &xi, float &eta)
+{
+    const double X = Xf, Y = Yf;
+    const double dx = X - L.dcX, dy = Y - L.dcY;
+    const double xp = dx * L.dc + dy * L.ds;
+    const double yp = dy * L.dc - dx * L.ds;
+    const double psi = sqrt(L.dq2 * xp * xp + yp * yp);
     double axp = 0.0, ayp = 0.0;
     if (psi > 0.0) {
         axp = L.df * atan(L.dqp * xp / psi);
         ayp = L.df * atanh(L.dqp * yp / psi);
     }
-    double ax = axp * L.dc - ayp * L.ds;
-    double ay = axp * L.ds + ayp * L.dc;
-    double g1 = L.g1, g2 = L.g2;
-    bx = X - ax + (g1 * X + g2 * Y);
-    by = Y - ay + (g2 * X - g1 * Y);
+    const double ax = axp * L.dc - ayp * L.ds;
+    const double ay = axp * L.ds + ayp * L.dc;
+    const double bx = X - ax + (L.dg1 * X + L.dg2 * Y) - C.dcX;      // beta - s, image frame
+    const double by = Y - ay + (L.dg2 * X - L.dg1 * Y) - C.dcY;
+    xi = (float)(bx * L.dc + by * L.ds);
+    eta = (float)(by * L.dc - bx * L.ds);
 }
 
-// ---- steps a3 / a4: one elliptical Sersic at offset (dx, dy) from its centre ----------------
-// Returns amp * exp2(k (1 - u)); `u_out`, `t_out`, `e_out` feed the refinement test.
-__device__ __forceinline__ float sersic_eval(const SersicC &C, float dx, float dy,
-                                             float &t_out, float &u_out, float &e_out)
+// ---- steps a3 / a4: Sersic value from t = (R_p/r_e)^2 -----------------------------------------
+// Returns amp * 2^(k (1 - u)), u = t^(1/2n).  `flag` is set when the sample needs the FP64
+// refinement (sources only; see tl_consts.cuh).
+__device__ __forceinline__ float sersic_from_t(const SersicC &C, float t, bool &flag)
 {
-    float x1 = fmaf(dx, C.c, dy * C.s);
-    float x2 = fmaf(dy, C.c, -dx * C.s);
-    float t = fmaf(C.A * x1, x1, (C.B * x2) * x2);   // (R_p / r_e)^2
-    float v = log2f(t);                              // t = 0 -> -inf -> u = 0 -> I_e e^{b_n}
-    float vp = fmaf(v, C.pl, v * C.ph);
-    float u = exp2f(vp);
-    float arg = fmaf(-C.kh, u, C.kh) + fmaf(-C.kl, u, C.kl);
-    float e = exp2f(arg);
-    t_out = t; u_out = u; e_out = e;
-    return C.amp * e;
+    const float v = mufu_lg2(t);                     // t = 0 -> -inf -> u = 0 -> I_e e^{b_n}
+    const float vp = fmaf(v, C.pl, v * C.ph);
+    const float u = mufu_ex2(vp);
+    const float arg = fmaf(-C.kh, u, C.kh) + fmaf(-C.kl, u, C.kl);
+    flag = (arg + vp + C.lcf) > 0.5f * v;
+    return C.amp * mufu_ex2(arg);
 }
 
-// One sub-sample: lens light at theta, sources at beta (Eq. 2).  Already scaled
-// by 1/S^2, so the caller only adds (step a5, bin = mean).
-template <bool REFINE>
-__device__ __forceinline__ float sample_value(const RowC &rc, int n_lens_light, int n_comp,
-                                              float X, float Y)
+__device__ __forceinline__ float quad_form(const SersicC &C, float x, float y)
 {
-    float acc = 0.f, t, u, e;
-    for (int k = 0; k < n_lens_light; ++k) {
-        const SersicC &C = rc.comp[k];
-        acc += sersic_eval(C, (X - C.cXh) - C.cXl, (Y - C.cYh) - C.cYl, t, u, e);
-    }
-    float bx, by;
-    deflect_f32(rc.lens, X, Y, bx, by);
-    float src = 0.f;
-    bool flag = false;
-    for (int k = n_lens_light; k < n_comp; ++k) {
-        const SersicC &C = rc.comp[k];
-        src += sersic_eval(C, (bx - C.cXh) - C.cXl, (by - C.cYh) - C.cYl, t, u, e);
-        float w = C.cflag * e * u;
-        flag = flag || (w * w > t);
-    }
-    if (REFINE && flag) {
-        double dbx, dby;
-        refine_beta(rc.lens, X, Y, dbx, dby);
-        src = 0.f;
-        for (int k = n_lens_light; k < n_comp; ++k) {
-            const SersicC &C = rc.comp[k];
-            src += sersic_eval(C, (float)(dbx - C.dcX), (float)(dby - C.dcY), t, u, e);
-        }
-    }
-    return acc + src;
+    const float w = fmaf(C.ah, x, fmaf(C.b2h, y, fmaf(C.al, x, C.b2l * y)));
+    return fmaf(x, w, fmaf(C.cch * y, y, (C.ccl * y) * y));
 }
 
 }  // namespace tl
