@@ -15,7 +15,7 @@ from typing import Optional
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libtinylens.so")
+LIB_PATH = os.environ.get("TL_LIB") or os.path.join(_HERE, "libtinylens.so")   # TL_LIB: experiments only
 
 TL_OK, TL_EINVAL, TL_ENOMEM, TL_ECUDA, TL_ESIZE = 0, -1, -2, -3, -4
 TL_EDGE_EXTEND, TL_EDGE_ZERO = 0, 1
@@ -50,7 +50,7 @@ def load(build_if_missing: bool = True):
     global _lib
     if _lib is not None:
         return _lib
-    if build_if_missing:
+    if build_if_missing and not os.environ.get("TL_LIB"):
         from . import build as _build
         try:
             _build.build()

@@ -29,12 +29,12 @@ struct tl_ctx {
     int path = 0;                 // 0 fused, 1 split
     int threads = 256, ctas_per_sm = 1, grid = 1;
     size_t smem = 0;
-    int tile_rows = 0, n_tiles = 0, G = 1, trace_slabs = 1;
+    int tile_rows = 0, n_tiles = 0, CW = 32, CH = 1, trace_slabs = 1;
     void (*fused)(const tl::KArgs) = nullptr;
     void (*trace)(const tl::KArgs, int) = nullptr;
     size_t conv_smem = 0;
     int64_t chunk_rows = 0;       // rows per scratch chunk
-    double refine_tau = 3e-4;
+    double refine_tau = 7.5e-4;   // x S at create: a pixel averages S^2 samples
     // benchmark facility (tl_set_profiling): events around the dominant kernel of the last call
     int profile = 0;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
@@ -80,17 +80,16 @@ trace_fn trace_for(int S, int nll, int nsrc)
     }
 }
 
-// phase-1 work split: G row groups per column; pick the G whose slowest thread does the least
-int best_row_groups(int He, int We, int threads)
+// phase-1 warp tile CW x CH = 32 lanes: the shape that wastes the fewest lanes on the ragged
+// right / bottom edge of the extended image
+void best_warp_tile(int He, int We, int *CW, int *CH)
 {
-    int best = 1; double best_cost = 1e300;
-    for (int G = 1; G <= 32 && G <= He; ++G) {
-        const int items = G * We;
-        const int rounds = (items + threads - 1) / threads;
-        const double cost = (double)rounds * ((He + G - 1) / G);      // pixels of the slowest thread
-        if (cost < best_cost - 1e-9) { best_cost = cost; best = G; }
+    double best = -1.0;
+    for (int cw = 32; cw >= 1; cw >>= 1) {
+        const int ch = 32 / cw;
+        const double eff = (double)He * We / ((double)((We + cw - 1) / cw * cw) * ((He + ch - 1) / ch * ch));
+        if (eff > best + 1e-12) { best = eff; *CW = cw; *CH = ch; }
     }
-    return best;
 }
 
 constexpr size_t SMEM_LIMIT = 227 * 1024;
@@ -118,7 +117,8 @@ tl::KArgs base_args(const tl_ctx *c)
     a.He = c->He; a.We = c->We; a.pitch = c->pitch; a.S = c->cfg.supersample;
     a.n_lens_light = c->cfg.n_lens_light; a.n_comp = c->n_comp;
     a.edge_zero = c->cfg.edge_mode == TL_EDGE_ZERO;
-    a.tile_rows = c->tile_rows; a.n_tiles = c->n_tiles; a.G = c->G;
+    a.tile_rows = c->tile_rows; a.n_tiles = c->n_tiles;
+    a.CW = c->CW; a.CH = c->CH; a.tiles_x = (c->We + c->CW - 1) / c->CW; a.tiles_y = (c->He + c->CH - 1) / c->CH;
     return a;
 }
 
@@ -261,6 +261,7 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
         lconst[l] = s; smin[l] = (float)mn;
     }
     c->lconst0 = lconst[0]; c->sigma_min0 = smin[0];
+    c->refine_tau *= cfg->supersample;
     if (const char *e = std::getenv("TL_REFINE_TAU")) {   // tuning knob
         const double v = std::atof(e);
         if (v > 0.0 && std::isfinite(v)) c->refine_tau = v;
@@ -282,13 +283,13 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
     if (!ok) { tl_destroy(c); return TL_ECUDA; }
 
     // launch geometry
+    best_warp_tile(c->He, c->We, &c->CW, &c->CH);
     const size_t fs = fused_smem_bytes(c);
     if (fs <= SMEM_LIMIT) {
         c->path = 0; c->smem = fs;
         c->threads = fs > SMEM_LIMIT / 2 ? 512 : 256;
         if (const char *e = std::getenv("TL_THREADS")) { const int v = std::atoi(e); if (v >= 32 && v <= 512 && v % 32 == 0) c->threads = v; }
         c->fused = fused_for(cfg->supersample, cfg->n_lens_light, cfg->n_source);
-        c->G = best_row_groups(c->He, c->We, c->threads);
         if (!cuda_ok(cudaFuncSetAttribute(c->fused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT))) { tl_destroy(c); return TL_ECUDA; }
         int occ = 0;
         if (!cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, c->fused, c->threads, fs)) || occ < 1) { tl_destroy(c); return TL_ECUDA; }
@@ -308,7 +309,6 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
         c->trace = trace_for(cfg->supersample, cfg->n_lens_light, cfg->n_source);
         // one CTA slab = 256 columns-items; G row groups so that a row of the batch fills >= 8 CTAs
         c->trace_slabs = 8;
-        c->G = best_row_groups(c->He, c->We, 256 * c->trace_slabs);
         int occ = 0;
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, c->trace, 256, 0);
         c->ctas_per_sm = occ > 0 ? occ : 1; c->grid = 0;

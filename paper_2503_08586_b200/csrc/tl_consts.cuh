@@ -43,15 +43,16 @@ struct LensC {                       // SIE + external shear
 };
 
 struct SersicC {                     // one elliptical Sersic component
-    // lens light: centre in the image frame (u-units); source: R^T s in the lens frame
+    // lens light: centre in the image frame (u-units); source: R^T (s - s_first) in the lens frame
     float cXh, cXl, cYh, cYl;
     // quadratic form t = (R_p / r_e)^2 = a x^2 + b2 x y + cc y^2 in the frame of the offsets
     float ah, al, b2h, b2l, cch, ccl;
     float ph, pl;                    // 1 / (2 n)
     float kh, kl;                    // b_n log2(e)
     float amp;                       // I_e / S^2
-    float lcf;                       // log2 of the refinement criterion constant (sources), else -1e30
-    int32_t valid, pad;
+    float nlcf;                      // -log2 of the refinement criterion constant (sources), else +1e30
+    float pm;                        // 1/(2n) - 1/2
+    int32_t valid;
     double dcX, dcY;                 // image-frame centre (u-units), FP64, for the refinement
 };
 
@@ -160,7 +161,12 @@ __global__ void __launch_bounds__(128) prologue_kernel(PrologueArgs a)
         double cX = (lens_ok ? (double)p[3] : 0.0) * a.inv_u, cY = (lens_ok ? (double)p[4] : 0.0) * a.inv_u;
         double n11 = c * (1.0 + g1) + s * g2, n12 = c * g2 + s * (1.0 - g1);
         double n21 = -s * (1.0 + g1) + c * g2, n22 = -s * g2 + c * (1.0 - g1);
-        double d1 = n11 * cX + n12 * cY, d2 = n21 * cX + n22 * cY;
+        // D0 = N c - R^T s_1: the first source's centre is folded into the linear map, so
+        // (U + V, U2 + V2) - alpha' is directly the lens-frame offset R^T (beta - s_1)
+        const float *s1 = p + 7 + 7 * a.n_lens_light;
+        const bool s1ok = isfinite(s1[5]) && isfinite(s1[6]);
+        double s1X = (s1ok ? (double)s1[5] : 0.0) * a.inv_u, s1Y = (s1ok ? (double)s1[6] : 0.0) * a.inv_u;
+        double d1 = n11 * cX + n12 * cY - (c * s1X + s * s1Y), d2 = n21 * cX + n22 * cY - (-s * s1X + c * s1Y);
         double th0 = 0.5 * atan2(qp, q), c0 = cos(th0), s0 = sin(th0);
         double T = atanh(fmin(qp, 1.0 - 1e-16)), z0 = tanh(0.5 * T);
         split2(cX, &L.cXh, &L.cXl); split2(cY, &L.cYh, &L.cYl);
@@ -203,7 +209,11 @@ __global__ void __launch_bounds__(128) prologue_kernel(PrologueArgs a)
     if (is_lens_light) { cd = cs; sd = ss; oX = cX; oY = cY; }                 // image frame
     else {                                                                      // lens frame
         cd = cs * c + ss * s; sd = ss * c - cs * s;                             // cos, sin(phi_s - phi)
-        oX = c * cX + s * cY; oY = -s * cX + c * cY;                            // R^T s
+        // R^T (s_k - s_1): offsets are measured from the first source (folded into D0)
+        const float *s1 = p + 7 + 7 * a.n_lens_light;
+        const bool s1ok = isfinite(s1[5]) && isfinite(s1[6]);
+        const double rX = cX - (s1ok ? (double)s1[5] : 0.0) * a.inv_u, rY = cY - (s1ok ? (double)s1[6] : 0.0) * a.inv_u;
+        oX = c * rX + s * rY; oY = -s * rX + c * rY;
     }
     split2(oX, &C.cXh, &C.cXl); split2(oY, &C.cYh, &C.cYl);
     split2(A * cd * cd + Bq * sd * sd, &C.ah, &C.al);
@@ -216,15 +226,17 @@ __global__ void __launch_bounds__(128) prologue_kernel(PrologueArgs a)
     // Selective FP64 refinement of beta:
     // the FP32 ray-trace carries an absolute error delta_beta ~ 2^-22 (theta_E + |theta|);
     // the induced brightness error of a sample is  I (b_n/n) u delta_beta / R.  It is refined
-    // when that exceeds tau * sigma_min:  (cf e u)^2 > t, i.e. in log2:  lcf + arg + vp > v/2.
-    C.lcf = -1e30f;
+    // when that exceeds tau * sigma_min:  (cf e u)^2 > t, i.e. in log2 (v = lg2 t, vp = v/2n,
+    // arg = lg2 e):  arg + v (1/2n - 1/2) > -lg2 cf.
+    C.nlcf = 1e30f;
+    C.pm = (float)(0.5 / n - 0.5);
     if (!is_lens_light && ok && amp != 0.0) {
         double dbeta = 2.4e-7 * (fmax((double)p[0], 0.0) + a.fov_half);               // arcsec
         double smin = a.sigma_min[(a.row0 + row) / a.rows_per_lens];
         double cf = fabs(amp) * (bn / n) * dbeta / (re * a.refine_tau * smin);
-        C.lcf = (float)fmin(fmax(log2(cf), -1e30), 1e30);
+        C.nlcf = (float)fmin(fmax(-log2(cf), -1e30), 1e30);
     }
-    C.valid = ok ? 1 : 0; C.pad = 0;
+    C.valid = ok ? 1 : 0;
     rc->comp[k] = C;
 }
 

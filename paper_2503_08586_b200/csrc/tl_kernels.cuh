@@ -31,7 +31,7 @@ struct KArgs {
     int64_t B, rows_per_lens, row0;
     int ny, nx, K, Kp, h, He, We, pitch, S, n_lens_light, n_comp, edge_zero;
     int tile_rows, n_tiles;  // split path
-    int G;                   // phase-1 row groups per column (see trace_image)
+    int CW, CH, tiles_x, tiles_y;   // phase-1 warp tiles (see trace_tiles)
 };
 
 __device__ __forceinline__ bool row_is_valid(const RowC &rc, int n_comp)
@@ -84,90 +84,133 @@ __device__ __forceinline__ RowV row_values(const RowC &rc, float Y)
     return r;
 }
 
-// One sub-sample (steps a2-a4, Eq. 2): lens light at theta + sources at beta,
-// already scaled by 1/S^2 so that the caller only adds (step a5, bin = mean).
+// Register-resident constants of one row for the sample loop.
 template <int NLL, int NSRC>
-__device__ __forceinline__ float sample_value(const RowC &rc, const ColV &c, const RowV &r, float X, float Y)
+struct HotC {
+    SieHot sie;
+    SersicHot ll;                 // lens light (NLL = 1)
+    SersicHot src[NSRC];
+    QuadHot q[NSRC];
+    __device__ __forceinline__ explicit HotC(const RowC &rc) : sie(rc.lens)
+    {
+        if (NLL) ll = SersicHot(rc.comp[0]);
+#pragma unroll
+        for (int k = 0; k < NSRC; ++k) { src[k] = SersicHot(rc.comp[NLL + k]); q[k] = QuadHot(rc.comp[NLL + k]); }
+    }
+};
+
+// One sub-sample (steps a2-a4, Eq. 2): lens light at theta (added to `acc`) and
+// sources at beta (returned), both already scaled by 1/S^2 so that the caller only adds
+// (step a5, bin = mean).  FAST = polynomial SIE path (q >= 0.5).
+template <int NLL, int NSRC, bool FAST>
+__device__ __forceinline__ float sample_value(const RowC &rc, const HotC<NLL, NSRC> &h, const ColV &c, const RowV &r,
+                                              float &acc, bool &flag)
 {
-    float acc = 0.f;
-    bool flag = false, fl;
-    if (NLL) acc = sersic_from_t(rc.comp[0], fmaf(c.LB, r.dyl, c.LA + r.LC), fl);
+    bool fl;
+    if (NLL) acc = fmaf(h.ll.amp, sersic_from_t(h.ll, fmaf(c.LB, r.dyl, c.LA + r.LC), fl), acc);
     const float xp = c.Pc + r.Qs, yp = r.Qc - c.Ps;
     float axp, ayp;
-    sie_alpha(rc.lens, xp, yp, axp, ayp);
-    const float bx = (c.U + r.V) - axp, by = (c.U2 + r.V2) - ayp;      // R^T beta
-    float src = 0.f;
-#pragma unroll
-    for (int k = NLL; k < NLL + NSRC; ++k) {
-        const SersicC &C = rc.comp[k];
-        src += sersic_from_t(C, quad_form(C, (bx - C.cXh) - C.cXl, (by - C.cYh) - C.cYl), fl);
+    if (FAST) sie_alpha(h.sie, xp, yp, axp, ayp);
+    else sie_alpha_slow(rc.lens, xp, yp, axp, ayp);
+    const float bx = (c.U + r.V) - axp, by = (c.U2 + r.V2) - ayp;      // R^T (beta - s_1)
+    float src = h.src[0].amp * sersic_from_t(h.src[0], quad_form(h.q[0], bx, by), fl);
+    flag = fl;
+    if (NSRC > 1) {
+        const float t2 = quad_form(h.q[1], (bx - h.q[1].oxh) - h.q[1].oxl, (by - h.q[1].oyh) - h.q[1].oyl);
+        src = fmaf(h.src[1].amp, sersic_from_t(h.src[1], t2, fl), src);
         flag = flag || fl;
     }
-    if (flag) {                                     // rare: FP64 ray-trace for this sample
-        src = 0.f;
-#pragma unroll
-        for (int k = NLL; k < NLL + NSRC; ++k) {
-            const SersicC &C = rc.comp[k];
-            float xi, eta;
-            refine_offsets(rc.lens, C, X, Y, xi, eta);
-            src += sersic_from_t(C, quad_form(C, xi, eta), fl);
-        }
-    }
-    return acc + src;
+    return src;
 }
 
-// steps a1-a5 for the extended native pixels of column j, rows i = i_first, i_first + i_step, ...
-// S_T > 0: compile-time supersampling (column values live in registers); S_T = 0: any S.
-template <int S_T, int NLL, int NSRC, class Store>
-__device__ __forceinline__ void trace_column(const RowC &rc, const KArgs &a, int j, int i_first, int i_step, Store store)
+// steps a1-a5 for a run of `count` warp tiles.  A warp tile is CW x CH = 32 extended native
+// pixels (lane -> column lane % CW, row lane / CW), so the samples a warp works on are
+// neighbours in the image (coherent refinement branches) and all lanes are busy; tiles are
+// numbered column-major (t = c * tiles_y + r), so a thread's column -- and the column values it
+// keeps in registers -- changes only when the whole warp moves to the next tile column.
+// S_T > 0: compile-time supersampling; S_T = 0: any S (column values recomputed per sample).
+template <int S_T, int NLL, int NSRC, bool FAST, class Store>
+__device__ __forceinline__ void trace_tiles(const RowC &rc, const HotC<NLL, NSRC> &h, const KArgs &a,
+                                            int tile, int count, Store store)
 {
     const int S = S_T > 0 ? S_T : a.S;
-    const bool edge_col = a.edge_zero && (j < a.h || j >= a.We - a.h);
+    const int lane = threadIdx.x & 31;
+    const int lj = lane % a.CW, li = lane / a.CW;
+    int c = tile / a.tiles_y, r = tile - c * a.tiles_y;
+    int j = c * a.CW + lj;
     // u-units: X = 2 (j S + b) + 1 - S We is the exact sub-sample abscissa (DESIGN.md a1)
-    const float X0 = (float)(2 * j * S + 1 - S * a.We);
+    float X0 = (float)(2 * j * S + 1 - S * a.We);
     ColV cv[S_T > 0 ? S_T : 1];
     if (S_T > 0) {
 #pragma unroll
         for (int b = 0; b < S_T; ++b) cv[b] = col_values<NLL>(rc, X0 + (float)(2 * b));
     }
-    for (int i = i_first; i < a.He; i += i_step) {
-        float acc = 0.f;
-        if (!(edge_col || (a.edge_zero && (i < a.h || i >= a.He - a.h)))) {
-            const float Y0 = (float)(2 * i * S + 1 - S * a.He);
-            if (S_T > 0) {
-#pragma unroll
-                for (int sa = 0; sa < S_T; ++sa) {
-                    const float Y = Y0 + (float)(2 * sa);
-                    const RowV rv = row_values<NLL>(rc, Y);
-#pragma unroll
-                    for (int sb = 0; sb < S_T; ++sb)
-                        acc += sample_value<NLL, NSRC>(rc, cv[sb], rv, X0 + (float)(2 * sb), Y);
-                }
-            } else {
+#pragma unroll 1
+    for (int k = 0; k < count; ++k) {
+        const int i = r * a.CH + li;
+        if (i < a.He && j < a.We) {
+            float acc = 0.f;
+            const bool edge = a.edge_zero && (j < a.h || j >= a.We - a.h || i < a.h || i >= a.He - a.h);
+            if (!edge) {
+                const float Y0 = (float)(2 * i * S + 1 - S * a.He);
+#pragma unroll 1
                 for (int sa = 0; sa < S; ++sa) {
                     const float Y = Y0 + (float)(2 * sa);
                     const RowV rv = row_values<NLL>(rc, Y);
-                    for (int sb = 0; sb < S; ++sb) {
-                        const float X = X0 + (float)(2 * sb);
-                        acc += sample_value<NLL, NSRC>(rc, col_values<NLL>(rc, X), rv, X, Y);
+                    if (S_T > 0) {
+                        float src[S_T > 0 ? S_T : 1];
+                        bool any = false;
+#pragma unroll
+                        for (int sb = 0; sb < S_T; ++sb) {
+                            bool fl;
+                            src[sb] = sample_value<NLL, NSRC, FAST>(rc, h, cv[sb], rv, acc, fl);
+                            any = any || fl;
+                            if (fl) src[sb] = __int_as_float(0x7fc00000);      // NaN marks "refine me"
+                        }
+                        if (any) {                                  // rare: FP64 ray-trace, out of line
+#pragma unroll
+                            for (int sb = 0; sb < S_T; ++sb)
+                                if (src[sb] != src[sb])
+                                    src[sb] = refined_source_light(rc, NLL, NLL + NSRC, X0 + (float)(2 * sb), Y);
+                        }
+#pragma unroll
+                        for (int sb = 0; sb < S_T; ++sb) acc += src[sb];
+                    } else {
+                        for (int sb = 0; sb < S; ++sb) {
+                            const float X = X0 + (float)(2 * sb);
+                            bool fl;
+                            float sv = sample_value<NLL, NSRC, FAST>(rc, h, col_values<NLL>(rc, X), rv, acc, fl);
+                            if (fl) sv = refined_source_light(rc, NLL, NLL + NSRC, X, Y);
+                            acc += sv;
+                        }
                     }
                 }
             }
+            store(i, j, acc);
         }
-        store(i, j, acc);
+        if (++r == a.tiles_y) {                        // next tile column (uniform over the warp)
+            r = 0; ++c;
+            j = c * a.CW + lj;
+            X0 = (float)(2 * j * S + 1 - S * a.We);
+            if (S_T > 0) {
+#pragma unroll
+                for (int b = 0; b < S_T; ++b) cv[b] = col_values<NLL>(rc, X0 + (float)(2 * b));
+            }
+        }
     }
 }
 
-// Work distribution of phase 1: items (g, j), g < G row groups; item (g, j) owns the pixels of
-// column j in rows g, g + G, ...   Threads take items tid, tid + blockDim, ...
+// Work distribution of phase 1: warp w of W takes the contiguous tile range
+// [w n / W, (w + 1) n / W), n = tiles_x * tiles_y: floor(n/W) or ceil(n/W) tiles each.
 template <int S_T, int NLL, int NSRC, class Store>
-__device__ __forceinline__ void trace_image(const RowC &rc, const KArgs &a, int item0, int item_step, Store store)
+__device__ __forceinline__ void trace_image(const RowC &rc, const KArgs &a, int warp, int n_warps, Store store)
 {
-    const int items = a.G * a.We;
-    for (int it = item0; it < items; it += item_step) {
-        const int g = it / a.We, j = it - g * a.We;
-        trace_column<S_T, NLL, NSRC>(rc, a, j, g, a.G, store);
-    }
+    const long long n = (long long)a.tiles_x * a.tiles_y;
+    const int t0 = (int)(n * warp / n_warps);
+    const int count = (int)(n * (warp + 1) / n_warps) - t0;
+    const HotC<NLL, NSRC> h(rc);
+    if (rc.lens.mode == 0) trace_tiles<S_T, NLL, NSRC, true>(rc, h, a, t0, count, store);     // uniform over the CTA
+    else trace_tiles<S_T, NLL, NSRC, false>(rc, h, a, t0, count, store);
 }
 
 // step a6 for a 1 x CONV_R strip whose window starts at `win` (16-byte aligned) in an image of
@@ -253,8 +296,12 @@ __device__ __forceinline__ double conv_chi2_rows(const KArgs &a, const float *im
 }
 
 // ------------------------------------------------------------------------------ fused path
+#ifndef TL_LB_T
+#define TL_LB_T 512
+#define TL_LB_B 1
+#endif
 template <int S_T, int NLL, int NSRC>
-__global__ void __launch_bounds__(512) fused_kernel(const KArgs a)
+__global__ void __launch_bounds__(TL_LB_T, TL_LB_B) fused_kernel(const KArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     RowC *rc = reinterpret_cast<RowC *>(smem_raw);
@@ -282,7 +329,7 @@ __global__ void __launch_bounds__(512) fused_kernel(const KArgs a)
             continue;
         }
         // phase 1: ray-trace + light + bin into shared memory
-        trace_image<S_T, NLL, NSRC>(*rc, a, threadIdx.x, blockDim.x,
+        trace_image<S_T, NLL, NSRC>(*rc, a, threadIdx.x >> 5, blockDim.x >> 5,
                                     [&](int i, int j, float v) { img[i * a.pitch + j] = v; });
         __syncthreads();
         // phase 2: PSF convolution from shared memory + chi^2
@@ -311,7 +358,7 @@ __global__ void __launch_bounds__(256) trace_kernel(const KArgs a, int chunk_row
         __syncthreads();
         if (!row_is_valid(rc_s, a.n_comp)) continue;
         float *dst = a.ext + (size_t)r * a.He * a.pitch;
-        trace_image<S_T, NLL, NSRC>(rc_s, a, blockIdx.y * blockDim.x + threadIdx.x, gridDim.y * blockDim.x,
+        trace_image<S_T, NLL, NSRC>(rc_s, a, (blockIdx.y * blockDim.x + threadIdx.x) >> 5, (gridDim.y * blockDim.x) >> 5,
                                     [&](int i, int j, float v) { dst[i * a.pitch + j] = v; });
     }
 }

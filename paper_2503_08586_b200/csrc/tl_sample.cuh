@@ -53,40 +53,85 @@ __device__ __forceinline__ float atanh_small(float r)
     return fmaf(r * s, p, r);
 }
 
-// ---- step a2: SIE deflection in the lens frame ---------------------------------------------
-__device__ __forceinline__ void sie_alpha(const LensC &L, float xp, float yp, float &axp, float &ayp)
+// Per-row constants of the pixel loop, copied from shared memory into registers once per row
+// (a by-value copy also tells the compiler they cannot alias the image stores).
+struct SieHot {
+    float q2h, q2l, c0, s0, qc0, qs0, z0, z0qp, qph, qpl, fh, fl, ft0h, ft0l, fT2h, fT2l;
+    __device__ __forceinline__ explicit SieHot(const LensC &L)
+        : q2h(L.q2h), q2l(L.q2l), c0(L.c0), s0(L.s0), qc0(L.qc0), qs0(L.qs0), z0(L.z0), z0qp(L.z0qp),
+          qph(L.qph), qpl(L.qpl), fh(L.fh), fl(L.fl), ft0h(L.ft0h), ft0l(L.ft0l), fT2h(L.fT2h), fT2l(L.fT2l) {}
+};
+struct SersicHot {
+    float ph, pl, kh, kl, amp, pm, nlcf;
+    __device__ __forceinline__ SersicHot() {}
+    __device__ __forceinline__ explicit SersicHot(const SersicC &C)
+        : ph(C.ph), pl(C.pl), kh(C.kh), kl(C.kl), amp(C.amp), pm(C.pm), nlcf(C.nlcf) {}
+};
+struct QuadHot {
+    float ah, al, b2h, b2l, cch, ccl, oxh, oxl, oyh, oyl;
+    __device__ __forceinline__ QuadHot() {}
+    __device__ __forceinline__ explicit QuadHot(const SersicC &C)
+        : ah(C.ah), al(C.al), b2h(C.b2h), b2l(C.b2l), cch(C.cch), ccl(C.ccl),
+          oxh(C.cXh), oxl(C.cXl), oyh(C.cYh), oyl(C.cYl) {}
+};
+
+// ---- step a2: SIE deflection in the lens frame (q >= 0.5) ------------------------------------
+__device__ __forceinline__ void sie_alpha(const SieHot &L, float xp, float yp, float &axp, float &ayp)
+{
+    const float xx = xp * xp;
+    // the 1e-30 keeps psi > 0: at the lens centre both angles come out as 0 +- rounding (G6)
+    const float psi2 = fmaf(L.q2h, xx, fmaf(L.q2l, xx, fmaf(yp, yp, 1e-30f)));
+    const float psi = psi2 * mufu_rsq(psi2);
+    const float ax = fabsf(xp), ay = fabsf(yp);
+    // atan: rotate (psi, q'|x'|) by -theta0
+    const float d2 = fmaf(ax, L.qs0, psi * L.c0);
+    const float n2 = fmaf(ax, L.qc0, -psi * L.s0);
+    const float pa = atan_small(n2 * mufu_rcp(d2));
+    const float a1 = fmaf(L.fh, pa, L.ft0h) + fmaf(L.fl, pa, L.ft0l);
+    // atanh: hyperbolic shift of z = q'|y'|/psi by z0
+    const float num = fmaf(ay, L.qph, -L.z0 * psi);
+    const float den = fmaf(-ay, L.z0qp, psi);
+    const float ph = atanh_small(num * mufu_rcp(den));
+    const float a2 = fmaf(L.fh, ph, L.fT2h) + fmaf(L.fl, ph, L.fT2l);
+    axp = copysignf(a1, xp);
+    ayp = copysignf(a2, yp);
+}
+
+// strongly flattened lenses (q < 0.5): libdevice inverse functions, out of line
+__device__ __noinline__ void sie_alpha_slow(const LensC &L, float xp, float yp, float &axp, float &ayp)
 {
     const float xx = xp * xp;
     const float psi2 = fmaf(L.q2h, xx, fmaf(L.q2l, xx, yp * yp));
-    const float rpsi = mufu_rsq(fmaxf(psi2, 1e-30f));          // alpha = 0 at psi = 0 (G6)
-    const float psi = psi2 * rpsi;
-    const float ax = fabsf(xp), ay = fabsf(yp);
-    if (L.mode == 0) {
-        // atan: rotate (psi, q'|x'|) by -theta0
-        const float d2 = fmaf(ax, L.qs0, psi * L.c0);
-        const float n2 = fmaf(ax, L.qc0, -psi * L.s0);
-        const float pa = atan_small(n2 * mufu_rcp(d2));
-        const float a1 = fmaf(L.fh, pa, L.ft0h) + fmaf(L.fl, pa, L.ft0l);
-        // atanh: hyperbolic shift of z = q'|y'|/psi by z0
-        const float num = fmaf(ay, L.qph, -L.z0 * psi);
-        const float den = fmaf(-ay, L.z0qp, psi);
-        const float ph = atanh_small(num * mufu_rcp(den));
-        const float a2 = fmaf(L.fh, ph, L.fT2h) + fmaf(L.fl, ph, L.fT2l);
-        axp = psi2 > 0.f ? copysignf(a1, xp) : 0.f;
-        ayp = psi2 > 0.f ? copysignf(a2, yp) : 0.f;
-    } else {
-        // strongly flattened lenses (q < 0.5): libdevice inverse functions
-        const float nx = fmaf(L.qpl, xp, L.qph * xp), ny = fmaf(L.qpl, yp, L.qph * yp);
-        const float at = atan2f(nx, psi);
-        const float ah = atanhf(psi2 > 0.f ? ny / psi : 0.f);
-        axp = fmaf(L.fl, at, L.fh * at);
-        ayp = fmaf(L.fl, ah, L.fh * ah);
-    }
+    const float psi = sqrtf(psi2);
+    const float nx = fmaf(L.qpl, xp, L.qph * xp), ny = fmaf(L.qpl, yp, L.qph * yp);
+    const float at = atan2f(nx, psi);
+    const float ah = atanhf(psi2 > 0.f ? ny / psi : 0.f);
+    axp = fmaf(L.fl, at, L.fh * at);
+    ayp = fmaf(L.fl, ah, L.fh * ah);
+}
+
+// ---- steps a3 / a4: Sersic value from t = (R_p/r_e)^2 -----------------------------------------
+// Returns 2^(k (1 - u)), u = t^(1/2n) (the caller multiplies by amp).  `flag` is set when the
+// sample needs the FP64 refinement (meaningful for sources only; see tl_consts.cuh).
+__device__ __forceinline__ float sersic_from_t(const SersicHot &C, float t, bool &flag)
+{
+    const float v = mufu_lg2(t);                     // t = 0 -> -inf -> u = 0 -> I_e e^{b_n}
+    const float vp = fmaf(v, C.pl, v * C.ph);
+    const float u = mufu_ex2(vp);
+    const float arg = fmaf(-C.kh, u, C.kh) + fmaf(-C.kl, u, C.kl);
+    flag = fmaf(v, C.pm, arg) > C.nlcf;
+    return mufu_ex2(arg);
+}
+
+__device__ __forceinline__ float quad_form(const QuadHot &C, float x, float y)
+{
+    const float w = fmaf(C.ah, x, fmaf(C.b2h, y, fmaf(C.al, x, C.b2l * y)));
+    return fmaf(x, w, fmaf(C.cch * y, y, (C.ccl * y) * y));
 }
 
 // ---- step a2 in FP64 (selective refinement only): lens-frame offset R^T (beta - s) ----------
-__device__ __noinline__ void refine_offsets(const LensC &L, const SersicC &C, float Xf, float Yf,
-                                            float &xi, float &eta)
+__device__ __forceinline__ void refine_offsets(const LensC &L, const SersicC &C, float Xf, float Yf,
+                                               float &xi, float &eta)
 {
     const double X = Xf, Y = Yf;
     const double dx = X - L.dcX, dy = Y - L.dcY;
@@ -106,23 +151,20 @@ __device__ __noinline__ void refine_offsets(const LensC &L, const SersicC &C, fl
     eta = (float)(by * L.dc - bx * L.ds);
 }
 
-// ---- steps a3 / a4: Sersic value from t = (R_p/r_e)^2 -----------------------------------------
-// Returns amp * 2^(k (1 - u)), u = t^(1/2n).  `flag` is set when the sample needs the FP64
-// refinement (sources only; see tl_consts.cuh).
-__device__ __forceinline__ float sersic_from_t(const SersicC &C, float t, bool &flag)
+// Source light of one sub-sample with the ray-trace redone in FP64 (rare, out of line).
+__device__ __noinline__ float refined_source_light(const RowC &rc, int k0, int k1, float X, float Y)
 {
-    const float v = mufu_lg2(t);                     // t = 0 -> -inf -> u = 0 -> I_e e^{b_n}
-    const float vp = fmaf(v, C.pl, v * C.ph);
-    const float u = mufu_ex2(vp);
-    const float arg = fmaf(-C.kh, u, C.kh) + fmaf(-C.kl, u, C.kl);
-    flag = (arg + vp + C.lcf) > 0.5f * v;
-    return C.amp * mufu_ex2(arg);
-}
-
-__device__ __forceinline__ float quad_form(const SersicC &C, float x, float y)
-{
-    const float w = fmaf(C.ah, x, fmaf(C.b2h, y, fmaf(C.al, x, C.b2l * y)));
-    return fmaf(x, w, fmaf(C.cch * y, y, (C.ccl * y) * y));
+    float src = 0.f;
+    for (int k = k0; k < k1; ++k) {
+        const SersicC &C = rc.comp[k];
+        float xi, eta;
+        refine_offsets(rc.lens, C, X, Y, xi, eta);
+        QuadHot Q(C);
+        Q.oxh = Q.oxl = Q.oyh = Q.oyl = 0.f;
+        bool fl;
+        src = fmaf(C.amp, sersic_from_t(SersicHot(C), quad_form(Q, xi, eta), fl), src);
+    }
+    return src;
 }
 
 }  // namespace tl
