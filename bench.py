@@ -42,7 +42,7 @@ OP_SIE_FP32, OP_SIE_MUFU = 46, 4
 OP_SERSIC_FP32, OP_SERSIC_MUFU = 11, 3
 OP_CHI2_FP32 = 4
 SM_FP32_LANES = 128          # thread-instruction issue slots per SM per clock (4 warps x 32), measured 122-128
-SM_MUFU_LANES = 16           # measured 15.96 (profiles/r1_pipe_peaks.md)
+SM_MUFU_LANES = 16           # measured 15.96 (profiles/r1_mufu_accuracy.md)
 
 # dram bytes of the dominant kernel per launch from the committed `ncu --set full` capture
 # (profiles/): filled in by hand after each capture; None until one exists.
@@ -277,7 +277,7 @@ def run_ours(args, w: W.Workload):
             "achieved": achieved, "peak": peak, "unit": "Tinst/s", "frac": achieved / peak,
             "traffic": NCU_DRAM_BYTES_PER_LAUNCH,
             "peak_source": "derived: %d SMs x %d issue slots/clk x %.0f MHz (MEASURED_PEAKS.json sm_max_mhz; "
-                           "slots/clk measured, profiles/r1_pipe_peaks.md)" % (info["n_sm"], SM_FP32_LANES, sm_max),
+                           "slots/clk measured, profiles/r1_mufu_accuracy.md)" % (info["n_sm"], SM_FP32_LANES, sm_max),
             "kernel_ms": k_ms, "fp32_pipe_frac": fp32_frac, "mufu_pipe_frac": mufu_frac,
             "algorithmic_issue_slots_per_likelihood": om["issue_slots"],
             "hbm": {"algorithmic_bytes_per_step": hbm_bytes,

