@@ -46,7 +46,7 @@ SM_MUFU_LANES = 16           # measured 15.96 (profiles/r1_mufu_accuracy.md)
 
 # dram bytes of the dominant kernel per launch from the committed `ncu --set full` capture
 # (profiles/): filled in by hand after each capture; None until one exists.
-NCU_DRAM_BYTES_PER_LAUNCH = None
+NCU_DRAM_BYTES_PER_LAUNCH = 2182656       # profiles/r1_fused_kernel.md: 2.179328 MB read + 3.328 KB written
 
 
 def op_model(w: W.Workload) -> dict:
@@ -307,7 +307,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=1, help="BASELINE.json config index (default 1, the metric's)")
     ap.add_argument("--batch", type=int, default=0, help="override rows per GPU (parity/debug only)")
-    ap.add_argument("--ref-rows", type=int, default=256, help="oracle sample size per step")
+    ap.add_argument("--ref-rows", type=int, default=512, help="oracle sample size per step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     w = W.workload(args.config)

@@ -102,21 +102,26 @@ __device__ inline double gamma_p_series(double a, double x, double *prefactor)
 __device__ inline double sersic_bn(double n)
 {
     const double a = 2.0 * n;
-    double lo = 0.0, hi = fmax(a, 1.0);
-    double pf;
-    for (int it = 0; it < 64 && gamma_p_series(a, hi, &pf) < 0.5; ++it) hi *= 2.0;
-    // asymptotic start (Ciotti & Bertin 1999) where it is inside the bracket
-    double b = a - 1.0 / 3.0 + 4.0 / (405.0 * n);
-    if (!(b > lo && b < hi)) b = 0.5 * (lo + hi);
-    for (int it = 0; it < 100; ++it) {
-        double P = gamma_p_series(a, b, &pf);
+    double lo = 0.0, hi = INFINITY, pf;
+    // start: asymptotic series (Ciotti & Bertin 1999, relative error < 1e-5 for n >= 0.36);
+    // for smaller n the small-x limit P(a,x) ~ x^a / Gamma(a+1)
+    double b;
+    if (n >= 0.36) {
+        const double r = 1.0 / n;
+        b = a - 1.0 / 3.0 + r * (4.0 / 405.0 + r * (46.0 / 25515.0 + r * (131.0 / 1148175.0 - r * (2194697.0 / 30690717750.0))));
+    } else {
+        b = exp((lgamma(a + 1.0) + log(0.5)) / a);
+    }
+    for (int it = 0; it < 60; ++it) {
+        const double P = gamma_p_series(a, b, &pf);
         if (P < 0.5) lo = b; else hi = b;
-        double dPdb = pf * a / b;                 // x^(a-1) e^-x / Gamma(a)
+        const double dPdb = pf * a / b;           // x^(a-1) e^-x / Gamma(a)
         double nb = b - (P - 0.5) / dPdb;
-        if (!(nb > lo && nb < hi)) nb = 0.5 * (lo + hi);
-        double step = fabs(nb - b);
+        if (!(nb > lo && nb < hi)) nb = isinf(hi) ? 2.0 * b : 0.5 * (lo + hi);
+        const double step = fabs(nb - b);
         b = nb;
-        if (step <= 4e-16 * b) break;
+        // Newton converges quadratically: a step below 1e-8 b leaves an error below 1e-15 b
+        if (step <= 1e-8 * b) break;
     }
     return b;
 }
