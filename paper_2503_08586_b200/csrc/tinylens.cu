@@ -25,6 +25,8 @@ struct tl_ctx {
     float *psf = nullptr, *data = nullptr, *wgt = nullptr, *sigma_min = nullptr;
     double *lconst = nullptr;
     double lconst0 = 0.0, sigma_min0 = 0.0;
+    std::vector<float> psf_host;   // lens 0: flipped, padded taps (kernel-parameter copy)
+    int ctaps = 0;
     // launch geometry
     int path = 0;                 // 0 fused, 1 split
     int threads = 256, ctas_per_sm = 1, grid = 1;
@@ -100,12 +102,12 @@ inline bool cuda_ok(cudaError_t e) { return e == cudaSuccess; }
 
 size_t fused_smem_bytes(const tl_ctx *c)
 {
-    return sizeof(tl::RowC) + 32 * sizeof(double) + sizeof(float) * ((size_t)c->K * c->Kp + (size_t)c->He * c->pitch + c->Kp + 8);
+    return sizeof(tl::RowC) + 32 * sizeof(double) + sizeof(float) * ((size_t)c->K * c->Kp + (size_t)(c->He + 1) * c->pitch + c->Kp + 8);
 }
 
 size_t conv_smem_bytes(const tl_ctx *c, int tile_rows)
 {
-    return 32 * sizeof(double) + sizeof(float) * ((size_t)c->K * c->Kp + (size_t)(tile_rows + 2 * c->h) * c->pitch + c->Kp + 8);
+    return 32 * sizeof(double) + sizeof(float) * ((size_t)c->K * c->Kp + (size_t)(tile_rows + 2 * c->h + 1) * c->pitch + c->Kp + 8);
 }
 
 tl::KArgs base_args(const tl_ctx *c)
@@ -118,6 +120,8 @@ tl::KArgs base_args(const tl_ctx *c)
     a.n_lens_light = c->cfg.n_lens_light; a.n_comp = c->n_comp;
     a.edge_zero = c->cfg.edge_mode == TL_EDGE_ZERO;
     a.tile_rows = c->tile_rows; a.n_tiles = c->n_tiles;
+    a.ctaps = c->ctaps;
+    if (c->ctaps) memcpy(a.taps_c, c->psf_host.data(), sizeof(float) * (size_t)c->K * c->Kp);
     a.CW = c->CW; a.CH = c->CH; a.tiles_x = (c->We + c->CW - 1) / c->CW; a.tiles_y = (c->He + c->CH - 1) / c->CH;
     return a;
 }
@@ -261,6 +265,8 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
         lconst[l] = s; smin[l] = (float)mn;
     }
     c->lconst0 = lconst[0]; c->sigma_min0 = smin[0];
+    c->ctaps = (L == 1 && c->K <= tl::CTAPS_MAX_K) ? 1 : 0;
+    if (c->ctaps) c->psf_host.assign(psf_f.begin(), psf_f.begin() + (size_t)c->K * c->Kp);
     c->refine_tau *= cfg->supersample;
     if (const char *e = std::getenv("TL_REFINE_TAU")) {   // tuning knob
         const double v = std::atof(e);
@@ -298,8 +304,8 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
     } else {
         c->path = 1;
         // tile rows: as many as fit in ~100 KB so two CTAs share an SM
-        int tr = (int)((100 * 1024 / sizeof(float) - (size_t)c->K * c->Kp - c->Kp - 8) / c->pitch) - 2 * c->h;
-        if (tr < 4) tr = (int)((SMEM_LIMIT / sizeof(float) - 64 - (size_t)c->K * c->Kp - c->Kp - 8) / c->pitch) - 2 * c->h;
+        int tr = (int)((100 * 1024 / sizeof(float) - (size_t)c->K * c->Kp - c->Kp - 8) / c->pitch) - 2 * c->h - 1;
+        if (tr < 4) tr = (int)((SMEM_LIMIT / sizeof(float) - 64 - (size_t)c->K * c->Kp - c->Kp - 8) / c->pitch) - 2 * c->h - 1;
         if (tr < 1) { tl_destroy(c); return TL_ESIZE; }
         if (tr > cfg->ny) tr = cfg->ny;
         c->tile_rows = tr; c->n_tiles = (cfg->ny + tr - 1) / tr;

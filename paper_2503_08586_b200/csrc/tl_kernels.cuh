@@ -17,6 +17,8 @@
 namespace tl {
 
 constexpr int CONV_R = 4;            // outputs per thread strip (along x)
+constexpr int CTAPS_MAX_K = 41;      // largest PSF whose taps travel as kernel parameters
+constexpr int CTAPS_FLOATS = CTAPS_MAX_K * ((CTAPS_MAX_K + 3) & ~3);
 
 struct KArgs {
     const RowC *rows;        // [B] derived constants
@@ -32,6 +34,11 @@ struct KArgs {
     int ny, nx, K, Kp, h, He, We, pitch, S, n_lens_light, n_comp, edge_zero;
     int tile_rows, n_tiles;  // split path
     int CW, CH, tiles_x, tiles_y;   // phase-1 warp tiles (see trace_tiles)
+    // Single-lens contexts: the flipped, padded PSF also travels in the kernel parameters, i.e.
+    // in the constant bank, so that the convolution reads its taps through uniform loads
+    // (LDCU -> uniform registers -> FFMA operand) instead of the shared-memory pipe.
+    int ctaps;
+    float taps_c[CTAPS_FLOATS];
 };
 
 __device__ __forceinline__ bool row_is_valid(const RowC &rc, int n_comp)
@@ -284,12 +291,128 @@ __device__ __forceinline__ void load_psf(float *dst, const float *src, int n)
     for (int i = threadIdx.x; i < n; i += blockDim.x) dst[i] = src[i];
 }
 
+// step a6 for a 2 x 4 output block, PSF size known at compile time.  Per kernel row `ka` the
+// thread holds the windows of image rows i+ka and i+ka+1 (NW float4 each) in registers: the
+// second one is loaded (NW LDS.128) and becomes the first one of the next kernel row, so every
+// window float is read from shared memory once and used for up to 2 x 4 FMAs per tap.  With the
+// taps coming from the constant bank (CT) the shared-memory pipe carries NW wavefront-quads per
+// 8 K FMAs (57 % of its bandwidth at K = 21) instead of being the limiter.
+template <int K, bool CT>
+struct ConvBlock {
+    static constexpr int KG = (K + 3) / 4;           // tap groups of 4 per kernel row
+    static constexpr int Kp = KG * 4;
+    static constexpr int NW = (K + 3 + 3) / 4;       // float4 per window: columns 0 .. K + 2
+
+    static __device__ __forceinline__ void load_window(float4 (&w)[NW], const float *rp)
+    {
+#pragma unroll
+        for (int g = 0; g < NW; ++g) w[g] = *reinterpret_cast<const float4 *>(rp + 4 * g);
+    }
+
+    // one kernel row applied to one image-row window -> 4 outputs, summed into a fresh partial
+    static __device__ __forceinline__ void row(const float4 (&w)[NW], const float *kp, float (&acc)[4])
+    {
+        float p0 = 0.f, p1 = 0.f, p2 = 0.f, p3 = 0.f;
+#pragma unroll
+        for (int g = 0; g < KG; ++g) {
+            const float4 t = *reinterpret_cast<const float4 *>(kp + 4 * g);
+            const float4 lo = w[g];
+            const float4 hi = (g + 1 < NW) ? w[g + 1] : make_float4(0.f, 0.f, 0.f, 0.f);
+            const int nt = (K - 4 * g) >= 4 ? 4 : (K - 4 * g);     // real taps in this group
+            p0 = fmaf(t.x, lo.x, p0); p1 = fmaf(t.x, lo.y, p1); p2 = fmaf(t.x, lo.z, p2); p3 = fmaf(t.x, lo.w, p3);
+            if (nt > 1) { p0 = fmaf(t.y, lo.y, p0); p1 = fmaf(t.y, lo.z, p1); p2 = fmaf(t.y, lo.w, p2); p3 = fmaf(t.y, hi.x, p3); }
+            if (nt > 2) { p0 = fmaf(t.z, lo.z, p0); p1 = fmaf(t.z, lo.w, p1); p2 = fmaf(t.z, hi.x, p2); p3 = fmaf(t.z, hi.y, p3); }
+            if (nt > 3) { p0 = fmaf(t.w, lo.w, p0); p1 = fmaf(t.w, hi.x, p1); p2 = fmaf(t.w, hi.y, p2); p3 = fmaf(t.w, hi.z, p3); }
+        }
+        acc[0] += p0; acc[1] += p1; acc[2] += p2; acc[3] += p3;
+    }
+
+    // `win` = image row i, column x0 (16-byte aligned); taps = flipped PSF [K][Kp]
+    static __device__ __forceinline__ void run(const float *win, int pitch, const float *taps,
+                                               float (&a0)[4], float (&a1)[4])
+    {
+#pragma unroll
+        for (int r = 0; r < 4; ++r) { a0[r] = 0.f; a1[r] = 0.f; }
+        float4 wa[NW], wb[NW];
+        load_window(wa, win);
+        // kernel rows two at a time so that the windows ping-pong without register moves
+#pragma unroll 1
+        for (int ka = 0; ka + 1 < K; ka += 2) {
+            load_window(wb, win + (ka + 1) * pitch);
+            row(wa, taps + ka * Kp, a0);
+            row(wb, taps + ka * Kp, a1);
+            load_window(wa, win + (ka + 2) * pitch);
+            row(wb, taps + (ka + 1) * Kp, a0);
+            row(wa, taps + (ka + 1) * Kp, a1);
+        }
+        if (K & 1) {                                  // K is odd: last kernel row
+            load_window(wb, win + K * pitch);
+            row(wa, taps + (K - 1) * Kp, a0);
+            row(wb, taps + (K - 1) * Kp, a1);
+        }
+    }
+};
+
+// chi^2 terms of up to 4 outputs of row i starting at column x0 (and the optional image store)
+__device__ __forceinline__ float chi2_strip(const KArgs &a, const float acc[4], int i, int x0,
+                                            const float *data, const float *wgt, float *image_out)
+{
+    float c = 0.f;
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {
+        const int x = x0 + r;
+        if (x < a.nx) {
+            const int o = i * a.nx + x;
+            if (image_out) image_out[o] = acc[r];
+            if (data) {
+                const float d = __ldg(data + o) - acc[r];
+                c = fmaf(d * d, __ldg(wgt + o), c);
+            }
+        }
+    }
+    return c;
+}
+
+template <int K, bool CT>
+__device__ __forceinline__ double conv_chi2_blocks(const KArgs &a, const float *img, int e0, const float *taps,
+                                                   int i0, int i1, const float *data, const float *wgt, float *image_out)
+{
+    const int nsx = (a.nx + 3) / 4, npair = (i1 - i0 + 1) / 2;
+    const int total = npair * nsx;
+    const float *tp = CT ? a.taps_c : taps;
+    double part = 0.0;
+    for (int s = threadIdx.x; s < total; s += blockDim.x) {
+        const int ip = s / nsx, i = i0 + 2 * ip, x0 = (s - ip * nsx) * 4;
+        float a0[4], a1[4];
+        ConvBlock<K, CT>::run(img + (i - e0) * a.pitch + x0, a.pitch, tp, a0, a1);
+        float c = chi2_strip(a, a0, i, x0, data, wgt, image_out);
+        if (i + 1 < i1) c += chi2_strip(a, a1, i + 1, x0, data, wgt, image_out);
+        part += (double)c;
+    }
+    return part;
+}
+
 // convolve + chi^2 over output rows [i0, i1) of one image; `img` is a shared-memory image
-// whose row 0 corresponds to extended row `e0`.  Returns this thread's chi^2 partial.
+// whose row 0 corresponds to extended row `e0` (one spare row after the last one must be
+// readable).  Returns this thread's chi^2 partial.  The common PSF sizes get the register-
+// blocked 2 x 4 kernel, any other odd size the generic 1 x 4 strip.
 __device__ __forceinline__ double conv_chi2_rows(const KArgs &a, const float *img, int e0,
                                                  const float *taps, int i0, int i1,
                                                  const float *data, const float *wgt, float *image_out)
 {
+#define TL_CONV_CASE(KK)                                                                                  \
+    case KK:                                                                                              \
+        return a.ctaps ? conv_chi2_blocks<KK, true>(a, img, e0, taps, i0, i1, data, wgt, image_out)       \
+                       : conv_chi2_blocks<KK, false>(a, img, e0, taps, i0, i1, data, wgt, image_out);
+    switch (a.K) {
+        TL_CONV_CASE(5)
+        TL_CONV_CASE(15)
+        TL_CONV_CASE(21)
+        TL_CONV_CASE(31)
+        TL_CONV_CASE(41)
+    default: break;
+    }
+#undef TL_CONV_CASE
     const int nsx = (a.nx + CONV_R - 1) / CONV_R;
     const int total = (i1 - i0) * nsx;
     double part = 0.0;
@@ -297,20 +420,7 @@ __device__ __forceinline__ double conv_chi2_rows(const KArgs &a, const float *im
         const int ir = s / nsx, i = i0 + ir, x0 = (s - ir * nsx) * CONV_R;
         float acc[CONV_R];
         conv_strip(img + (i - e0) * a.pitch + x0, a.pitch, taps, a.K, a.Kp, acc);
-        float c = 0.f;
-#pragma unroll
-        for (int r = 0; r < CONV_R; ++r) {
-            const int x = x0 + r;
-            if (x < a.nx) {
-                const int o = i * a.nx + x;
-                if (image_out) image_out[o] = acc[r];
-                if (data) {
-                    const float d = __ldg(data + o) - acc[r];
-                    c = fmaf(d * d, __ldg(wgt + o), c);
-                }
-            }
-        }
-        part += (double)c;
+        part += (double)chi2_strip(a, acc, i, x0, data, wgt, image_out);
     }
     return part;
 }
@@ -331,7 +441,7 @@ __global__ void __launch_bounds__(TL_LB_T, TL_LB_B) fused_kernel(const KArgs a)
     const int n_img = a.He * a.pitch;
     // pitch padding and the slack after the image are read by zero-padded taps only (and by
     // discarded strip lanes); phase 1 never writes them, so zero them once
-    for (int i = threadIdx.x; i < n_img + a.Kp + 8; i += blockDim.x) img[i] = 0.f;
+    for (int i = threadIdx.x; i < n_img + a.pitch + a.Kp + 8; i += blockDim.x) img[i] = 0.f;
 
     int64_t cur_lens = -1;
     for (int64_t r = blockIdx.x; r < a.B; r += gridDim.x) {
@@ -349,9 +459,15 @@ __global__ void __launch_bounds__(TL_LB_T, TL_LB_B) fused_kernel(const KArgs a)
             continue;
         }
         // phase 1: ray-trace + light + bin into shared memory
+#ifndef TL_EXP_SKIP_TRACE
         trace_image<S_T, NLL, NSRC>(*rc, a, threadIdx.x >> 5, blockDim.x >> 5,
                                     [&](int i, int j, float v) { img[i * a.pitch + j] = v; });
+#endif
         __syncthreads();
+#ifdef TL_EXP_SKIP_CONV
+        if (a.logL && threadIdx.x == 0) a.logL[row] = img[(a.He / 2) * a.pitch + a.We / 2];
+        continue;
+#endif
         // phase 2: PSF convolution from shared memory + chi^2
         const double part = conv_chi2_rows(a, img, 0, taps, 0, a.ny,
                                            a.logL ? a.data + lens * npix : nullptr,
@@ -412,7 +528,7 @@ __global__ void __launch_bounds__(256) conv_kernel(const KArgs a, int chunk_rows
     float4 *dst = reinterpret_cast<float4 *>(img);
     const int n4 = erows * a.pitch / 4;
     for (int i = threadIdx.x; i < n4; i += blockDim.x) dst[i] = src[i];
-    for (int i = threadIdx.x; i < a.Kp + 8; i += blockDim.x) img[erows * a.pitch + i] = 0.f;
+    for (int i = threadIdx.x; i < a.pitch + a.Kp + 8; i += blockDim.x) img[erows * a.pitch + i] = 0.f;
     __syncthreads();
     const double part = conv_chi2_rows(a, img, i0, taps, i0, i1,
                                        a.partial ? a.data + lens * npix : nullptr,
