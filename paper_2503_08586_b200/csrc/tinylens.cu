@@ -240,6 +240,15 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
     cudaDeviceProp prop;
     if (!cuda_ok(cudaGetDeviceProperties(&prop, c->device))) { delete c; return TL_ECUDA; }
     c->n_sm = prop.multiProcessorCount;
+    {   // per-call scratch comes from the stream-ordered allocator: keep freed blocks cached in
+        // the pool across synchronisations instead of returning them to the driver every call
+        cudaMemPool_t pool;
+        if (cuda_ok(cudaDeviceGetDefaultMemPool(&pool, c->device))) {
+            unsigned long long keep = ~0ull;
+            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        }
+        cudaGetLastError();
+    }
     c->n_comp = cfg->n_lens_light + cfg->n_source;
     c->P = 7 + 7 * c->n_comp;
     c->K = psf_ny; c->Kp = (c->K + 3) & ~3; c->h = (c->K - 1) / 2;
