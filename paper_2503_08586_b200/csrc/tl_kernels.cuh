@@ -138,13 +138,16 @@ __device__ __forceinline__ float sample_value(const RowC &rc, const HotC<NLL, NS
 // numbered column-major (t = c * tiles_y + r), so a thread's column -- and the column values it
 // keeps in registers -- changes only when the whole warp moves to the next tile column.
 // S_T > 0: compile-time supersampling; S_T = 0: any S (column values recomputed per sample).
-template <int S_T, int NLL, int NSRC, bool FAST, class Store>
+// `next()` yields the warp's next tile index (uniform over the warp) or -1.
+template <int S_T, int NLL, int NSRC, bool FAST, class Next, class Store>
 __device__ __forceinline__ void trace_tiles(const RowC &rc, const HotC<NLL, NSRC> &h, const KArgs &a,
-                                            int tile, int count, Store store)
+                                            Next next, Store store)
 {
     const int S = S_T > 0 ? S_T : a.S;
     const int lane = threadIdx.x & 31;
     const int lj = lane % a.CW, li = lane / a.CW;
+    int tile = next();
+    if (tile < 0) return;
     int c = tile / a.tiles_y, r = tile - c * a.tiles_y;
     int j = c * a.CW + lj;
     // u-units: X = 2 (j S + b) + 1 - S We is the exact sub-sample abscissa (DESIGN.md a1)
@@ -155,7 +158,7 @@ __device__ __forceinline__ void trace_tiles(const RowC &rc, const HotC<NLL, NSRC
         for (int b = 0; b < S_T; ++b) cv[b] = col_values<NLL>(rc, X0 + (float)(2 * b));
     }
 #pragma unroll 1
-    for (int k = 0; k < count; ++k) {
+    for (;;) {
         const int i = r * a.CH + li;
         if (i < a.He && j < a.We) {
             float acc = 0.f;
@@ -197,8 +200,12 @@ __device__ __forceinline__ void trace_tiles(const RowC &rc, const HotC<NLL, NSRC
             }
             store(i, j, acc);
         }
-        if (++r == a.tiles_y) {                        // next tile column (uniform over the warp)
-            r = 0; ++c;
+        tile = next();
+        if (tile < 0) break;
+        const int c2 = tile / a.tiles_y;
+        r = tile - c2 * a.tiles_y;
+        if (c2 != c) {                                 // another tile column (uniform over the warp)
+            c = c2;
             j = c * a.CW + lj;
             X0 = (float)(2 * j * S + 1 - S * a.We);
             if (S_T > 0) {
@@ -209,17 +216,33 @@ __device__ __forceinline__ void trace_tiles(const RowC &rc, const HotC<NLL, NSRC
     }
 }
 
-// Work distribution of phase 1: warp w of W takes the contiguous tile range
-// [w n / W, (w + 1) n / W), n = tiles_x * tiles_y: floor(n/W) or ceil(n/W) tiles each.
+// Work distribution of phase 1.  Static (split path): warp w of W takes the contiguous tile
+// range [w n / W, (w + 1) n / W), n = tiles_x * tiles_y.  Dynamic (fused path): the warps of the
+// CTA draw tiles from a shared-memory counter, so they all reach the barrier that ends the
+// phase within one tile of each other whatever the refinement branches cost; the value of a
+// pixel does not depend on which warp computes it, so logL stays bitwise reproducible.
 template <int S_T, int NLL, int NSRC, class Store>
-__device__ __forceinline__ void trace_image(const RowC &rc, const KArgs &a, int warp, int n_warps, Store store)
+__device__ __forceinline__ void trace_image(const RowC &rc, const KArgs &a, int warp, int n_warps, int *counter, Store store)
 {
-    const long long n = (long long)a.tiles_x * a.tiles_y;
-    const int t0 = (int)(n * warp / n_warps);
-    const int count = (int)(n * (warp + 1) / n_warps) - t0;
+    const int n = a.tiles_x * a.tiles_y;
     const HotC<NLL, NSRC> h(rc);
-    if (rc.lens.mode == 0) trace_tiles<S_T, NLL, NSRC, true>(rc, h, a, t0, count, store);     // uniform over the CTA
-    else trace_tiles<S_T, NLL, NSRC, false>(rc, h, a, t0, count, store);
+    const bool fast = rc.lens.mode == 0;               // uniform over the CTA
+    if (counter) {
+        auto next = [&]() -> int {
+            int t = 0;
+            if ((threadIdx.x & 31) == 0) t = atomicAdd(counter, 1);
+            t = __shfl_sync(0xffffffffu, t, 0);
+            return t < n ? t : -1;
+        };
+        if (fast) trace_tiles<S_T, NLL, NSRC, true>(rc, h, a, next, store);
+        else trace_tiles<S_T, NLL, NSRC, false>(rc, h, a, next, store);
+    } else {
+        int t = (int)((long long)n * warp / n_warps);
+        const int t_end = (int)((long long)n * (warp + 1) / n_warps);
+        auto next = [&]() -> int { return t < t_end ? t++ : -1; };
+        if (fast) trace_tiles<S_T, NLL, NSRC, true>(rc, h, a, next, store);
+        else trace_tiles<S_T, NLL, NSRC, false>(rc, h, a, next, store);
+    }
 }
 
 // step a6 for a 1 x CONV_R strip whose window starts at `win` (16-byte aligned) in an image of
@@ -435,7 +458,8 @@ __global__ void __launch_bounds__(TL_LB_T, TL_LB_B) fused_kernel(const KArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     RowC *rc = reinterpret_cast<RowC *>(smem_raw);
-    double *red = reinterpret_cast<double *>(smem_raw + sizeof(RowC));
+    double *red = reinterpret_cast<double *>(smem_raw + sizeof(RowC));            // [0, 16): block_sum
+    int *tile_counter = reinterpret_cast<int *>(red + 24);                          // phase-1 work queue
     float *taps = reinterpret_cast<float *>(smem_raw + sizeof(RowC) + 32 * sizeof(double));
     float *img = taps + a.K * a.Kp;
     const int n_img = a.He * a.pitch;
@@ -449,6 +473,7 @@ __global__ void __launch_bounds__(TL_LB_T, TL_LB_B) fused_kernel(const KArgs a)
         const int64_t lens = row / a.rows_per_lens;
         __syncthreads();                               // previous row fully consumed
         load_row_consts(rc, a.rows + r);
+        if (threadIdx.x == 0) *tile_counter = 0;
         if (lens != cur_lens) { load_psf(taps, a.psf + lens * a.K * a.Kp, a.K * a.Kp); cur_lens = lens; }
         __syncthreads();
         const size_t npix = (size_t)a.ny * a.nx;
@@ -460,7 +485,7 @@ __global__ void __launch_bounds__(TL_LB_T, TL_LB_B) fused_kernel(const KArgs a)
         }
         // phase 1: ray-trace + light + bin into shared memory
 #ifndef TL_EXP_SKIP_TRACE
-        trace_image<S_T, NLL, NSRC>(*rc, a, threadIdx.x >> 5, blockDim.x >> 5,
+        trace_image<S_T, NLL, NSRC>(*rc, a, threadIdx.x >> 5, blockDim.x >> 5, tile_counter,
                                     [&](int i, int j, float v) { img[i * a.pitch + j] = v; });
 #endif
         __syncthreads();
@@ -494,7 +519,7 @@ __global__ void __launch_bounds__(256) trace_kernel(const KArgs a, int chunk_row
         __syncthreads();
         if (!row_is_valid(rc_s, a.n_comp)) continue;
         float *dst = a.ext + (size_t)r * a.He * a.pitch;
-        trace_image<S_T, NLL, NSRC>(rc_s, a, (blockIdx.y * blockDim.x + threadIdx.x) >> 5, (gridDim.y * blockDim.x) >> 5,
+        trace_image<S_T, NLL, NSRC>(rc_s, a, (blockIdx.y * blockDim.x + threadIdx.x) >> 5, (gridDim.y * blockDim.x) >> 5, nullptr,
                                     [&](int i, int j, float v) { dst[i * a.pitch + j] = v; });
     }
 }
