@@ -25,13 +25,13 @@ struct tl_ctx {
     float *psf = nullptr, *data = nullptr, *wgt = nullptr, *sigma_min = nullptr;
     double *lconst = nullptr;
     double lconst0 = 0.0, sigma_min0 = 0.0;
-    std::vector<float> psf_host;   // lens 0: flipped, padded taps (kernel-parameter copy)
-    int ctaps = 0;
     // launch geometry
     int path = 0;                 // 0 fused, 1 split
     int threads = 256, ctas_per_sm = 1, grid = 1;
     size_t smem = 0;
     int tile_rows = 0, n_tiles = 0, CW = 32, CH = 1, trace_slabs = 1;
+    int rowtab = 0;               // RowV table in shared memory (fused: after the image; split: trace_kernel)
+    size_t trace_smem = 0;
     void (*fused)(const tl::KArgs) = nullptr;
     void (*trace)(const tl::KArgs, int) = nullptr;
     size_t conv_smem = 0;
@@ -120,8 +120,7 @@ tl::KArgs base_args(const tl_ctx *c)
     a.n_lens_light = c->cfg.n_lens_light; a.n_comp = c->n_comp;
     a.edge_zero = c->cfg.edge_mode == TL_EDGE_ZERO;
     a.tile_rows = c->tile_rows; a.n_tiles = c->n_tiles;
-    a.ctaps = c->ctaps;
-    if (c->ctaps) memcpy(a.taps_c, c->psf_host.data(), sizeof(float) * (size_t)c->K * c->Kp);
+    a.rowtab = c->rowtab;
     a.CW = c->CW; a.CH = c->CH; a.tiles_x = (c->We + c->CW - 1) / c->CW; a.tiles_y = (c->He + c->CH - 1) / c->CH;
     return a;
 }
@@ -180,7 +179,7 @@ int run_batch(tl_ctx *c, const float *params, int64_t B, float *logL, float *ima
             a.ext = ext; a.partial = logL ? partial : nullptr;
             dim3 tg((unsigned)(nb < 65535 ? nb : 65535), (unsigned)c->trace_slabs);
             if (c->profile) cudaEventRecord(c->ev0, st);
-            c->trace<<<tg, 256, 0, st>>>(a, (int)nb);
+            c->trace<<<tg, 256, c->trace_smem, st>>>(a, (int)nb);
             if (c->profile) { cudaEventRecord(c->ev1, st); c->prof_pending = 1; }
             dim3 cg((unsigned)nb, (unsigned)c->n_tiles);
             tl::conv_kernel<<<cg, 256, c->conv_smem, st>>>(a, (int)nb);
@@ -274,8 +273,6 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
         lconst[l] = s; smin[l] = (float)mn;
     }
     c->lconst0 = lconst[0]; c->sigma_min0 = smin[0];
-    c->ctaps = (L == 1 && c->K <= tl::CTAPS_MAX_K) ? 1 : 0;
-    if (c->ctaps) c->psf_host.assign(psf_f.begin(), psf_f.begin() + (size_t)c->K * c->Kp);
     c->refine_tau *= cfg->supersample;
     if (const char *e = std::getenv("TL_REFINE_TAU")) {   // tuning knob
         const double v = std::atof(e);
@@ -299,8 +296,13 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
 
     // launch geometry
     best_warp_tile(c->He, c->We, &c->CW, &c->CH);
-    const size_t fs = fused_smem_bytes(c);
+    size_t fs = fused_smem_bytes(c);
+    const size_t rowtab_bytes = sizeof(tl::RowV) * (size_t)c->He * cfg->supersample;
     if (fs <= SMEM_LIMIT) {
+        // the row-value table is worth its shared memory unless it costs a resident CTA
+        const size_t fs2 = ((fs + 15) & ~(size_t)15) + rowtab_bytes;
+        const int per_sm_1 = (int)(SMEM_LIMIT / (fs + 1024)), per_sm_2 = (int)(SMEM_LIMIT / (fs2 + 1024));
+        if (fs2 <= SMEM_LIMIT && (per_sm_2 >= per_sm_1 || per_sm_2 >= 2)) { c->rowtab = 1; fs = fs2; }
         c->path = 0; c->smem = fs;
         c->threads = fs > SMEM_LIMIT / 2 ? 512 : 256;
         if (const char *e = std::getenv("TL_THREADS")) { const int v = std::atoi(e); if (v >= 32 && v <= 512 && v % 32 == 0) c->threads = v; }
@@ -322,10 +324,14 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
         if (!cuda_ok(cudaFuncSetAttribute(tl::conv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT))) { tl_destroy(c); return TL_ECUDA; }
         c->threads = 256; c->smem = c->conv_smem;
         c->trace = trace_for(cfg->supersample, cfg->n_lens_light, cfg->n_source);
+        if (rowtab_bytes <= 48 * 1024 && cfg->supersample <= 4) {   // S = 8 amortises row values over 8 samples already
+            c->rowtab = 1; c->trace_smem = rowtab_bytes;
+            if (!cuda_ok(cudaFuncSetAttribute(c->trace, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rowtab_bytes))) { tl_destroy(c); return TL_ECUDA; }
+        }
         // one CTA slab = 256 columns-items; G row groups so that a row of the batch fills >= 8 CTAs
         c->trace_slabs = 8;
         int occ = 0;
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, c->trace, 256, 0);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, c->trace, 256, c->trace_smem);
         c->ctas_per_sm = occ > 0 ? occ : 1; c->grid = 0;
         int64_t cr = (int64_t)(EXT_SCRATCH_BYTES / (sizeof(float) * (size_t)c->He * c->pitch));
         if (cr < 1) cr = 1;

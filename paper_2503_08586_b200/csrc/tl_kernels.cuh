@@ -17,8 +17,6 @@
 namespace tl {
 
 constexpr int CONV_R = 4;            // outputs per thread strip (along x)
-constexpr int CTAPS_MAX_K = 41;      // largest PSF whose taps travel as kernel parameters
-constexpr int CTAPS_FLOATS = CTAPS_MAX_K * ((CTAPS_MAX_K + 3) & ~3);
 
 struct KArgs {
     const RowC *rows;        // [B] derived constants
@@ -34,11 +32,7 @@ struct KArgs {
     int ny, nx, K, Kp, h, He, We, pitch, S, n_lens_light, n_comp, edge_zero;
     int tile_rows, n_tiles;  // split path
     int CW, CH, tiles_x, tiles_y;   // phase-1 warp tiles (see trace_tiles)
-    // Single-lens contexts: the flipped, padded PSF also travels in the kernel parameters, i.e.
-    // in the constant bank, so that the convolution reads its taps through uniform loads
-    // (LDCU -> uniform registers -> FFMA operand) instead of the shared-memory pipe.
-    int ctaps;
-    float taps_c[CTAPS_FLOATS];
+    int rowtab;              // 1: the kernel's shared memory holds a RowV table (He * S entries)
 };
 
 __device__ __forceinline__ bool row_is_valid(const RowC &rc, int n_comp)
@@ -52,7 +46,7 @@ __device__ __forceinline__ bool row_is_valid(const RowC &rc, int n_comp)
 // (ordinate Y).  x' = Pc + Qs, y' = Qc - Ps, N (theta - c) + D0 = (U + V, U2 + V2); the
 // lens-light quadratic form is  t = LA + LC + LB * dyl.
 struct ColV { float Pc, Ps, U, U2, LA, LB; };
-struct RowV { float Qc, Qs, V, V2, LC, dyl; };
+struct alignas(16) RowV { float Qc, Qs, V, V2, LC, dyl, pad0, pad1; };      // 32 bytes: two LDS.128
 
 template <int NLL>
 __device__ __forceinline__ ColV col_values(const RowC &rc, float X)
@@ -90,6 +84,7 @@ __device__ __forceinline__ RowV row_values(const RowC &rc, float Y)
         const float y2 = r.dyl * r.dyl;
         r.LC = fmaf(C.cch, y2, C.ccl * y2);
     } else { r.dyl = 0.f; r.LC = 0.f; }
+    r.pad0 = r.pad1 = 0.f;
     return r;
 }
 
@@ -139,9 +134,12 @@ __device__ __forceinline__ float sample_value(const RowC &rc, const HotC<NLL, NS
 // keeps in registers -- changes only when the whole warp moves to the next tile column.
 // S_T > 0: compile-time supersampling; S_T = 0: any S (column values recomputed per sample).
 // `next()` yields the warp's next tile index (uniform over the warp) or -1.
+// `rowtab` (optional, shared memory): the RowV of every sub-sample row of the image, filled once
+// per parameter row by fill_rowtab(); without it each thread recomputes them (18 instructions
+// per sub-row instead of two LDS.128).
 template <int S_T, int NLL, int NSRC, bool FAST, class Next, class Store>
 __device__ __forceinline__ void trace_tiles(const RowC &rc, const HotC<NLL, NSRC> &h, const KArgs &a,
-                                            Next next, Store store)
+                                            const RowV *rowtab, Next next, Store store)
 {
     const int S = S_T > 0 ? S_T : a.S;
     const int lane = threadIdx.x & 31;
@@ -168,7 +166,7 @@ __device__ __forceinline__ void trace_tiles(const RowC &rc, const HotC<NLL, NSRC
 #pragma unroll 1
                 for (int sa = 0; sa < S; ++sa) {
                     const float Y = Y0 + (float)(2 * sa);
-                    const RowV rv = row_values<NLL>(rc, Y);
+                    const RowV rv = rowtab ? rowtab[i * S + sa] : row_values<NLL>(rc, Y);
                     if (S_T > 0) {
                         float src[S_T > 0 ? S_T : 1];
                         bool any = false;
@@ -216,13 +214,24 @@ __device__ __forceinline__ void trace_tiles(const RowC &rc, const HotC<NLL, NSRC
     }
 }
 
+// RowV of all He * S sub-sample rows -> shared memory (all threads of the CTA; caller syncs).
+template <int NLL>
+__device__ __forceinline__ void fill_rowtab(const RowC &rc, const KArgs &a, RowV *rowtab)
+{
+    const int S = a.S, n = a.He * S;
+    for (int k = threadIdx.x; k < n; k += blockDim.x) {
+        const int i = k / S, sa = k - i * S;
+        rowtab[k] = row_values<NLL>(rc, (float)(2 * i * S + 1 - S * a.He + 2 * sa));
+    }
+}
+
 // Work distribution of phase 1.  Static (split path): warp w of W takes the contiguous tile
 // range [w n / W, (w + 1) n / W), n = tiles_x * tiles_y.  Dynamic (fused path): the warps of the
 // CTA draw tiles from a shared-memory counter, so they all reach the barrier that ends the
 // phase within one tile of each other whatever the refinement branches cost; the value of a
 // pixel does not depend on which warp computes it, so logL stays bitwise reproducible.
 template <int S_T, int NLL, int NSRC, class Store>
-__device__ __forceinline__ void trace_image(const RowC &rc, const KArgs &a, int warp, int n_warps, int *counter, Store store)
+__device__ __forceinline__ void trace_image(const RowC &rc, const KArgs &a, const RowV *rowtab, int warp, int n_warps, int *counter, Store store)
 {
     const int n = a.tiles_x * a.tiles_y;
     const HotC<NLL, NSRC> h(rc);
@@ -234,14 +243,14 @@ __device__ __forceinline__ void trace_image(const RowC &rc, const KArgs &a, int 
             t = __shfl_sync(0xffffffffu, t, 0);
             return t < n ? t : -1;
         };
-        if (fast) trace_tiles<S_T, NLL, NSRC, true>(rc, h, a, next, store);
-        else trace_tiles<S_T, NLL, NSRC, false>(rc, h, a, next, store);
+        if (fast) trace_tiles<S_T, NLL, NSRC, true>(rc, h, a, rowtab, next, store);
+        else trace_tiles<S_T, NLL, NSRC, false>(rc, h, a, rowtab, next, store);
     } else {
         int t = (int)((long long)n * warp / n_warps);
         const int t_end = (int)((long long)n * (warp + 1) / n_warps);
         auto next = [&]() -> int { return t < t_end ? t++ : -1; };
-        if (fast) trace_tiles<S_T, NLL, NSRC, true>(rc, h, a, next, store);
-        else trace_tiles<S_T, NLL, NSRC, false>(rc, h, a, next, store);
+        if (fast) trace_tiles<S_T, NLL, NSRC, true>(rc, h, a, rowtab, next, store);
+        else trace_tiles<S_T, NLL, NSRC, false>(rc, h, a, rowtab, next, store);
     }
 }
 
@@ -317,10 +326,11 @@ __device__ __forceinline__ void load_psf(float *dst, const float *src, int n)
 // step a6 for a 2 x 4 output block, PSF size known at compile time.  Per kernel row `ka` the
 // thread holds the windows of image rows i+ka and i+ka+1 (NW float4 each) in registers: the
 // second one is loaded (NW LDS.128) and becomes the first one of the next kernel row, so every
-// window float is read from shared memory once and used for up to 2 x 4 FMAs per tap.  With the
-// taps coming from the constant bank (CT) the shared-memory pipe carries NW wavefront-quads per
-// 8 K FMAs (57 % of its bandwidth at K = 21) instead of being the limiter.
-template <int K, bool CT>
+// window float is read from shared memory once and used for up to 2 x 4 FMAs per tap: the
+// shared-memory pipe carries NW window loads + KG (broadcast) tap loads per 8 K FMAs, about 70 %
+// of its bandwidth at K = 21, instead of being the limiter as with 1 x 4 strips.  (Feeding the
+// taps through the constant bank instead was measured: no faster, LDC is the slower path.)
+template <int K>
 struct ConvBlock {
     static constexpr int KG = (K + 3) / 4;           // tap groups of 4 per kernel row
     static constexpr int Kp = KG * 4;
@@ -396,18 +406,17 @@ __device__ __forceinline__ float chi2_strip(const KArgs &a, const float acc[4], 
     return c;
 }
 
-template <int K, bool CT>
+template <int K>
 __device__ __forceinline__ double conv_chi2_blocks(const KArgs &a, const float *img, int e0, const float *taps,
                                                    int i0, int i1, const float *data, const float *wgt, float *image_out)
 {
     const int nsx = (a.nx + 3) / 4, npair = (i1 - i0 + 1) / 2;
     const int total = npair * nsx;
-    const float *tp = CT ? a.taps_c : taps;
     double part = 0.0;
     for (int s = threadIdx.x; s < total; s += blockDim.x) {
         const int ip = s / nsx, i = i0 + 2 * ip, x0 = (s - ip * nsx) * 4;
         float a0[4], a1[4];
-        ConvBlock<K, CT>::run(img + (i - e0) * a.pitch + x0, a.pitch, tp, a0, a1);
+        ConvBlock<K>::run(img + (i - e0) * a.pitch + x0, a.pitch, taps, a0, a1);
         float c = chi2_strip(a, a0, i, x0, data, wgt, image_out);
         if (i + 1 < i1) c += chi2_strip(a, a1, i + 1, x0, data, wgt, image_out);
         part += (double)c;
@@ -423,10 +432,8 @@ __device__ __forceinline__ double conv_chi2_rows(const KArgs &a, const float *im
                                                  const float *taps, int i0, int i1,
                                                  const float *data, const float *wgt, float *image_out)
 {
-#define TL_CONV_CASE(KK)                                                                                  \
-    case KK:                                                                                              \
-        return a.ctaps ? conv_chi2_blocks<KK, true>(a, img, e0, taps, i0, i1, data, wgt, image_out)       \
-                       : conv_chi2_blocks<KK, false>(a, img, e0, taps, i0, i1, data, wgt, image_out);
+#define TL_CONV_CASE(KK) \
+    case KK: return conv_chi2_blocks<KK>(a, img, e0, taps, i0, i1, data, wgt, image_out);
     switch (a.K) {
         TL_CONV_CASE(5)
         TL_CONV_CASE(15)
@@ -463,6 +470,7 @@ __global__ void __launch_bounds__(TL_LB_T, TL_LB_B) fused_kernel(const KArgs a)
     float *taps = reinterpret_cast<float *>(smem_raw + sizeof(RowC) + 32 * sizeof(double));
     float *img = taps + a.K * a.Kp;
     const int n_img = a.He * a.pitch;
+    RowV *rowtab = a.rowtab ? reinterpret_cast<RowV *>(img + ((n_img + a.pitch + a.Kp + 8 + 3) & ~3)) : nullptr;
     // pitch padding and the slack after the image are read by zero-padded taps only (and by
     // discarded strip lanes); phase 1 never writes them, so zero them once
     for (int i = threadIdx.x; i < n_img + a.pitch + a.Kp + 8; i += blockDim.x) img[i] = 0.f;
@@ -484,8 +492,9 @@ __global__ void __launch_bounds__(TL_LB_T, TL_LB_B) fused_kernel(const KArgs a)
             continue;
         }
         // phase 1: ray-trace + light + bin into shared memory
+        if (rowtab) { fill_rowtab<NLL>(*rc, a, rowtab); __syncthreads(); }
 #ifndef TL_EXP_SKIP_TRACE
-        trace_image<S_T, NLL, NSRC>(*rc, a, threadIdx.x >> 5, blockDim.x >> 5, tile_counter,
+        trace_image<S_T, NLL, NSRC>(*rc, a, rowtab, threadIdx.x >> 5, blockDim.x >> 5, tile_counter,
                                     [&](int i, int j, float v) { img[i * a.pitch + j] = v; });
 #endif
         __syncthreads();
@@ -513,13 +522,16 @@ template <int S_T, int NLL, int NSRC>
 __global__ void __launch_bounds__(256) trace_kernel(const KArgs a, int chunk_rows)
 {
     __shared__ RowC rc_s;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    RowV *rowtab = a.rowtab ? reinterpret_cast<RowV *>(smem_raw) : nullptr;
     for (int r = blockIdx.x; r < chunk_rows; r += gridDim.x) {
         __syncthreads();
         load_row_consts(&rc_s, a.rows + r);
         __syncthreads();
         if (!row_is_valid(rc_s, a.n_comp)) continue;
+        if (rowtab) { fill_rowtab<NLL>(rc_s, a, rowtab); __syncthreads(); }
         float *dst = a.ext + (size_t)r * a.He * a.pitch;
-        trace_image<S_T, NLL, NSRC>(rc_s, a, (blockIdx.y * blockDim.x + threadIdx.x) >> 5, (gridDim.y * blockDim.x) >> 5, nullptr,
+        trace_image<S_T, NLL, NSRC>(rc_s, a, rowtab, (blockIdx.y * blockDim.x + threadIdx.x) >> 5, (gridDim.y * blockDim.x) >> 5, nullptr,
                                     [&](int i, int j, float v) { dst[i * a.pitch + j] = v; });
     }
 }
