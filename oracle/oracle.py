@@ -59,6 +59,11 @@ def lib():
         L.orc_loglike_batch.argtypes = [cp, i32, fp, i32, fp, fp, fp, i64, dp, i32]
         L.orc_render_batch.restype = i32
         L.orc_render_batch.argtypes = [cp, i32, fp, i32, fp, i64, dp, i32]
+        L.orc_nnls_small.restype = None; L.orc_nnls_small.argtypes = [i32, dp, dp, dp]
+        L.orc_component_images.restype = i32; L.orc_component_images.argtypes = [cp, fp, i32, fp, dp]
+        L.orc_loglike_linear.restype = d; L.orc_loglike_linear.argtypes = [cp, fp, i32, fp, fp, fp, dp]
+        L.orc_loglike_linear_batch.restype = i32
+        L.orc_loglike_linear_batch.argtypes = [cp, i32, fp, i32, fp, fp, fp, i64, dp, dp, i32]
         _lib = L
     return _lib
 
@@ -196,3 +201,39 @@ def render_batch(cfg: OrcConfig, psf, rows, n_lens: int = 1, threads: int = 0) -
 def render_for_workloads(w, psf, row) -> np.ndarray:
     """`render` callable for workloads.make_problem (tests / cpu_baseline leg only)."""
     return render(config_of(w), psf, row)
+
+
+# ---- NEXT-1: linear amplitudes (PAPER.md:86-129) ------------------------------------------
+
+def nnls_small(G, b) -> np.ndarray:
+    G = np.ascontiguousarray(G, dtype=np.float64); b = np.ascontiguousarray(b, dtype=np.float64)
+    n = b.size
+    s = np.zeros(n, np.float64)
+    lib().orc_nnls_small(int(n), _dp(G), _dp(b), _dp(s))
+    return s
+
+
+def component_images(cfg: OrcConfig, psf, row) -> np.ndarray:
+    p, r = _f32(psf), _f32(row)
+    C_ = cfg.n_lens_light + cfg.n_source
+    out = np.empty((C_, cfg.ny, cfg.nx), np.float64)
+    lib().orc_component_images(C.byref(cfg), _fp(p), int(p.shape[-1]), _fp(r), _dp(out))
+    return out
+
+
+def loglike_linear(cfg: OrcConfig, psf, data, noise, row):
+    """(logL at the NNLS amplitudes, amplitudes [C])."""
+    p, d, s, r = _f32(psf), _f32(data), _f32(noise), _f32(row)
+    amps = np.empty(cfg.n_lens_light + cfg.n_source, np.float64)
+    ll = lib().orc_loglike_linear(C.byref(cfg), _fp(p), int(p.shape[-1]), _fp(d), _fp(s), _fp(r), _dp(amps))
+    return ll, amps
+
+
+def loglike_linear_batch(cfg: OrcConfig, psf, data, noise, rows, n_lens: int = 1, threads: int = 0):
+    p, d, s, r = _f32(psf), _f32(data), _f32(noise), _f32(rows)
+    B = r.shape[0]
+    out = np.empty(B, np.float64)
+    amps = np.empty((B, cfg.n_lens_light + cfg.n_source), np.float64)
+    lib().orc_loglike_linear_batch(C.byref(cfg), int(n_lens), _fp(p), int(p.shape[-1]), _fp(d), _fp(s), _fp(r),
+                                   B, _dp(out), _dp(amps), int(threads))
+    return out, amps

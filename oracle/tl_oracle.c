@@ -348,3 +348,136 @@ int orc_render_batch(const orc_config *cfg, int n_lens, const float *psf, int K,
 #endif
     return used;
 }
+
+/* ================================================================== NEXT-1: linear amplitudes
+ * PAPER.md:86-93 Eq. 6 and :97-129 Eq. 7 (section 2.3): for given non-linear parameters the
+ * amplitudes s of the N_l + N_s light profiles enter linearly, d = M s + n with M = B [L_l | L_s]
+ * (column k = blurred image of component k at unit amplitude), and the likelihood is evaluated
+ * at the s >= 0 that minimises || (M s - d) / n ||^2 (squared 2-norm).  The
+ * paper solves this NNLS problem with the Bro & De Jong iteration; its result is the unique
+ * minimiser of a convex problem, so the oracle writes the definition out: with at most three
+ * components, every support set (which amplitudes are > 0) is tried, the normal equations are
+ * solved on it, and the feasible candidate with the smallest penalty wins.  The I_e entries of
+ * the row are ignored.
+ */
+int orc_component_images(const orc_config *cfg, const float *psf, int K, const float *row, double *M)
+{
+    int C = cfg->n_lens_light + cfg->n_source, P = 7 + 7 * C;
+    size_t n = (size_t)cfg->ny * cfg->nx;
+    float tmp[7 + 7 * 8];
+    for (int k = 0; k < C; ++k) {
+        memcpy(tmp, row, sizeof(float) * (size_t)P);
+        for (int j = 0; j < C; ++j) tmp[7 + 7 * j] = (j == k) ? 1.0f : 0.0f;     /* unit amplitude */
+        if (!orc_render(cfg, psf, K, tmp, M + (size_t)k * n)) return 0;
+    }
+    return 1;
+}
+
+/* minimise s'G s - 2 b's over s >= 0 (n <= 4) by enumeration of the supports */
+void orc_nnls_small(int n, const double *G, const double *b, double *s_out)
+{
+    double best = 0.0;                                   /* empty support: s = 0, penalty change 0 */
+    for (int i = 0; i < n; ++i) s_out[i] = 0.0;
+    for (int mask = 1; mask < (1 << n); ++mask) {
+        int idx[4], m = 0;
+        for (int i = 0; i < n; ++i) if (mask & (1 << i)) idx[m++] = i;
+        double A[4][5];
+        for (int r = 0; r < m; ++r) {
+            for (int c = 0; c < m; ++c) A[r][c] = G[idx[r] * n + idx[c]];
+            A[r][m] = b[idx[r]];
+        }
+        int singular = 0;
+        for (int c = 0; c < m && !singular; ++c) {       /* Gaussian elimination, partial pivoting */
+            int p = c;
+            for (int r = c + 1; r < m; ++r) if (fabs(A[r][c]) > fabs(A[p][c])) p = r;
+            if (!(fabs(A[p][c]) > 1e-300)) { singular = 1; break; }
+            if (p != c) for (int k = 0; k <= m; ++k) { double t = A[c][k]; A[c][k] = A[p][k]; A[p][k] = t; }
+            for (int r = c + 1; r < m; ++r) {
+                double f = A[r][c] / A[c][c];
+                for (int k = c; k <= m; ++k) A[r][k] -= f * A[c][k];
+            }
+        }
+        if (singular) continue;
+        double x[4];
+        for (int r = m - 1; r >= 0; --r) {
+            double t = A[r][m];
+            for (int k = r + 1; k < m; ++k) t -= A[r][k] * x[k];
+            x[r] = t / A[r][r];
+        }
+        int feasible = 1;
+        double f = 0.0;
+        for (int r = 0; r < m; ++r) { if (!(x[r] >= 0.0)) feasible = 0; f -= b[idx[r]] * x[r]; }
+        if (feasible && f < best) {                      /* at a stationary point s'Gs - 2b's = -b's */
+            best = f;
+            for (int i = 0; i < n; ++i) s_out[i] = 0.0;
+            for (int r = 0; r < m; ++r) s_out[idx[r]] = x[r];
+        }
+    }
+}
+
+double orc_loglike_linear(const orc_config *cfg, const float *psf, int K, const float *data,
+                          const float *noise, const float *row, double *amps)
+{
+    int C = cfg->n_lens_light + cfg->n_source;
+    size_t n = (size_t)cfg->ny * cfg->nx;
+    for (int k = 0; k < C; ++k) if (amps) amps[k] = NAN;
+    /* the amplitudes are not parameters here: validity is judged with them set to one */
+    float tmp[7 + 7 * 8];
+    memcpy(tmp, row, sizeof(float) * (size_t)(7 + 7 * C));
+    for (int j = 0; j < C; ++j) tmp[7 + 7 * j] = 1.0f;
+    if (!orc_row_valid(cfg, tmp)) return -INFINITY;
+    double *M = (double *)malloc(sizeof(double) * n * (size_t)C);
+    double *model = (double *)malloc(sizeof(double) * n);
+    orc_component_images(cfg, psf, K, tmp, M);
+    double G[16], b[4], s[4];
+    for (int k = 0; k < C; ++k) {
+        double bk = 0.0;
+        for (size_t i = 0; i < n; ++i) bk += M[k * n + i] * (double)data[i] / ((double)noise[i] * noise[i]);
+        b[k] = bk;
+        for (int l = 0; l < C; ++l) {
+            double g = 0.0;
+            for (size_t i = 0; i < n; ++i) g += M[k * n + i] * M[l * n + i] / ((double)noise[i] * noise[i]);
+            G[k * C + l] = g;
+        }
+    }
+    orc_nnls_small(C, G, b, s);
+    for (size_t i = 0; i < n; ++i) {
+        double m = 0.0;
+        for (int k = 0; k < C; ++k) m += s[k] * M[k * n + i];
+        model[i] = m;
+    }
+    double ll = orc_loglike_from_image(model, data, noise, n);     /* Eq. 5 at the optimal amplitudes (Eq. 6) */
+    if (amps) for (int k = 0; k < C; ++k) amps[k] = s[k];
+    free(M); free(model);
+    return ll;
+}
+
+int orc_loglike_linear_batch(const orc_config *cfg, int n_lens, const float *psf, int K, const float *data,
+                             const float *noise, const float *rows, int64_t B, double *logl, double *amps, int threads)
+{
+    int C = cfg->n_lens_light + cfg->n_source, P = 7 + 7 * C;
+    size_t n = (size_t)cfg->ny * cfg->nx;
+    int64_t per = B / (n_lens > 0 ? n_lens : 1);
+    int used = 1;
+#ifdef _OPENMP
+    if (threads > 0) omp_set_num_threads(threads);
+#pragma omp parallel
+    {
+#pragma omp single
+        used = omp_get_num_threads();
+#pragma omp for schedule(dynamic, 1)
+        for (int64_t r = 0; r < B; ++r) {
+            int64_t l = n_lens > 1 ? r / per : 0;
+            logl[r] = orc_loglike_linear(cfg, psf + (size_t)l * K * K, K, data + l * n, noise + l * n,
+                                         rows + r * P, amps ? amps + r * C : NULL);
+        }
+    }
+#else
+    for (int64_t r = 0; r < B; ++r) {
+        int64_t l = n_lens > 1 ? r / per : 0;
+        logl[r] = orc_loglike_linear(cfg, psf + (size_t)l * K * K, K, data + l * n, noise + l * n,
+                                     rows + r * P, amps ? amps + r * C : NULL);
+    }
+#endif
+    return used;
+}
