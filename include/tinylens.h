@@ -134,6 +134,25 @@ int tl_loglike_batch(tl_ctx *ctx, const float *params, int64_t B, float *logL, v
 int tl_render_batch(tl_ctx *ctx, const float *params, int64_t B, float *images, void *cuda_stream);
 
 /*
+ * tl_loglike_linear_batch -- the paper's linear/non-linear split (Eq. 6,
+ * :97-129 Eq. 7): for every row the amplitudes s of the N_l + N_s light components are not
+ * parameters but are solved as the non-negative least-squares minimiser of
+ * || (M s - d) / sigma ||^2, M = B [L_l | L_s] (column k = blurred unit-amplitude image of
+ * component k), and logL[r] is Eq. 5 at that optimum.  The I_e entries of the rows are ignored
+ * (they may hold anything; a finite |I_e| > 1 is used only as a magnitude hint for the
+ * precision refinement).
+ *   params   DEVICE pointer, float [B][P], same layout as tl_loglike_batch
+ *   logL     DEVICE pointer, float [B], written (-INFINITY for invalid rows)
+ *   amps     DEVICE pointer, float [B][N_l + N_s] (lens light first, then sources), written
+ *            (NaN for invalid rows), or NULL
+ * Asynchronous on cuda_stream; bitwise reproducible.  Always uses the staged pipeline
+ * (component images through global memory).  Returns TL_OK, TL_EINVAL, TL_ENOMEM, TL_ECUDA,
+ * or TL_ESIZE when the PSF tile does not fit in shared memory.
+ */
+int tl_loglike_linear_batch(tl_ctx *ctx, const float *params, int64_t B, float *logL, float *amps,
+                            void *cuda_stream);
+
+/*
  * tl_loglike_batch_host -- end-to-end convenience for a host-side sampler (PAPER.md:250 names
  * the CPU<->GPU transfers as part of the cost): copies params (HOST, float [B][P], ideally
  * pinned) to the device, runs tl_loglike_batch, copies logL back to logL (HOST, float [B]),

@@ -68,6 +68,7 @@ def load(build_if_missing: bool = True):
     L.tl_loglike_batch.restype = C.c_int; L.tl_loglike_batch.argtypes = [vp, vp, i64, vp, vp]
     L.tl_render_batch.restype = C.c_int; L.tl_render_batch.argtypes = [vp, vp, i64, vp, vp]
     L.tl_loglike_batch_host.restype = C.c_int; L.tl_loglike_batch_host.argtypes = [vp, vp, i64, vp, vp]
+    L.tl_loglike_linear_batch.restype = C.c_int; L.tl_loglike_linear_batch.argtypes = [vp, vp, i64, vp, vp, vp]
     L.tl_set_profiling.restype = C.c_int; L.tl_set_profiling.argtypes = [vp, C.c_int]
     L.tl_last_kernel_ms.restype = C.c_int; L.tl_last_kernel_ms.argtypes = [vp, C.POINTER(C.c_float)]
     L.tl_destroy.restype = None; L.tl_destroy.argtypes = [vp]
@@ -169,6 +170,20 @@ def tl_render_batch(handle: int, params, ny: int, nx: int, out=None, stream=None
     return out
 
 
+def tl_loglike_linear_batch(handle: int, params, n_comp: int, out=None, amps=None, want_amps=True, stream=None):
+    """params: CUDA float32 [B,P] -> (logL CUDA float32 [B], amplitudes CUDA float32 [B,n_comp] or None)."""
+    import torch
+    B = _dev_rows(handle, params)
+    if out is None:
+        out = torch.empty(B, dtype=torch.float32, device=params.device)
+    if amps is None and want_amps:
+        amps = torch.empty((B, n_comp), dtype=torch.float32, device=params.device)
+    _check(load().tl_loglike_linear_batch(handle, params.data_ptr(), B, out.data_ptr(),
+                                          amps.data_ptr() if amps is not None else None, _stream_handle(stream)),
+           "tl_loglike_linear_batch")
+    return out, amps
+
+
 def tl_loglike_batch_host(handle: int, params_host, out_host=None, stream=None):
     """params_host: host float32 [B,P] (torch CPU tensor, ideally pinned, or numpy) -> host logL [B].
     Host->device copy, kernels, device->host copy and a stream synchronise, all inside the call."""
@@ -226,6 +241,9 @@ class LensContext:
 
     def render(self, params, out=None, stream=None):
         return tl_render_batch(self.handle, params, self.ny, self.nx, out, stream)
+
+    def loglike_linear(self, params, out=None, amps=None, want_amps=True, stream=None):
+        return tl_loglike_linear_batch(self.handle, params, (self.n_params - 7) // 7, out, amps, want_amps, stream)
 
     def loglike_host(self, params_host, out_host=None, stream=None):
         return tl_loglike_batch_host(self.handle, params_host, out_host, stream)

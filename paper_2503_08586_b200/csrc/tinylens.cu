@@ -30,6 +30,10 @@ struct tl_ctx {
     int threads = 256, ctas_per_sm = 1, grid = 1;
     size_t smem = 0;
     int tile_rows = 0, n_tiles = 0, CW = 32, CH = 1, trace_slabs = 1;
+    // linear-amplitude mode (tl_loglike_linear_batch): always the staged pipeline
+    void (*trace_lin)(const tl::KArgs, int) = nullptr;
+    int lin_tile_rows = 0, lin_n_tiles = 0, lin_rowtab = 0;
+    size_t lin_conv_smem = 0, lin_trace_smem = 0;
     int rowtab = 0;               // RowV table in shared memory (fused: after the image; split: trace_kernel)
     size_t trace_smem = 0;
     void (*fused)(const tl::KArgs) = nullptr;
@@ -80,6 +84,12 @@ trace_fn trace_for(int S, int nll, int nsrc)
     case 8: return pick_trace<8>(nll, nsrc);
     default: return pick_trace<0>(nll, nsrc);
     }
+}
+
+trace_fn trace_lin_for(int nll, int nsrc)
+{
+    if (nll == 0) return nsrc == 1 ? tl::trace_lin_kernel<0, 1> : tl::trace_lin_kernel<0, 2>;
+    return nsrc == 1 ? tl::trace_lin_kernel<1, 1> : tl::trace_lin_kernel<1, 2>;
 }
 
 // phase-1 warp tile CW x CH = 32 lanes: the shape that wastes the fewest lanes on the ragged
@@ -163,6 +173,7 @@ int run_batch(tl_ctx *c, const float *params, int64_t B, float *logL, float *ima
         pa.inv_u = 2.0 * c->cfg.supersample / c->cfg.pix_scale;
         pa.fov_half = 0.5 * c->cfg.pix_scale * (c->He > c->We ? c->He : c->We);
         pa.refine_tau = c->refine_tau;
+        pa.unit_amp = 0;
         const int64_t nthr = nb * (1 + c->n_comp);
         tl::prologue_kernel<<<(unsigned)((nthr + 127) / 128), 128, 0, st>>>(pa);
 
@@ -338,6 +349,22 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
         if (cr > 65535) cr = 65535;
         c->chunk_rows = cr;
     }
+    {   // linear-amplitude pipeline: conv tiles of ~100 KB, row-value table when small
+        int tr = (int)((100 * 1024 / sizeof(float) - (size_t)c->K * c->Kp - c->Kp - 8) / c->pitch) - 2 * c->h - 1;
+        if (tr < 4) tr = (int)((SMEM_LIMIT / sizeof(float) - 64 - (size_t)c->K * c->Kp - c->Kp - 8) / c->pitch) - 2 * c->h - 1;
+        if (tr >= 1) {
+            if (tr > cfg->ny) tr = cfg->ny;
+            c->lin_tile_rows = tr; c->lin_n_tiles = (cfg->ny + tr - 1) / tr;
+            c->lin_conv_smem = sizeof(float) * ((size_t)c->K * c->Kp + (size_t)(tr + 2 * c->h + 1) * c->pitch + c->Kp + 8);
+            c->trace_lin = trace_lin_for(cfg->n_lens_light, cfg->n_source);
+            bool okl = cuda_ok(cudaFuncSetAttribute(tl::conv_lin_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT));
+            if (rowtab_bytes <= 48 * 1024) {
+                c->lin_rowtab = 1; c->lin_trace_smem = rowtab_bytes;
+                okl = okl && cuda_ok(cudaFuncSetAttribute(c->trace_lin, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rowtab_bytes));
+            }
+            if (!okl) { tl_destroy(c); return TL_ECUDA; }
+        }
+    }
     *out = c;
     return TL_OK;
 }
@@ -366,6 +393,63 @@ int tl_loglike_batch(tl_ctx *ctx, const float *params, int64_t B, float *logL, v
 int tl_render_batch(tl_ctx *ctx, const float *params, int64_t B, float *images, void *cuda_stream)
 {
     return run_batch(ctx, params, B, nullptr, images, (cudaStream_t)cuda_stream);
+}
+
+int tl_loglike_linear_batch(tl_ctx *c, const float *params, int64_t B, float *logL, float *amps, void *cuda_stream)
+{
+    if (!c || B < 0) return TL_EINVAL;
+    if (B == 0) return TL_OK;
+    if (!params || !logL || (B % c->cfg.n_lens)) return TL_EINVAL;
+    if (!c->trace_lin) return TL_ESIZE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = -1;
+    if (!cuda_ok(cudaGetDevice(&dev))) return TL_ECUDA;
+    if (dev != c->device && !cuda_ok(cudaSetDevice(c->device))) return TL_ECUDA;
+    const int NC = c->n_comp;
+    const size_t npix = (size_t)c->cfg.ny * c->cfg.nx;
+    const size_t ext_row = sizeof(float) * (size_t)NC * c->He * c->pitch, m_row = sizeof(float) * NC * npix;
+    int64_t chunk = (int64_t)(EXT_SCRATCH_BYTES / (ext_row + m_row));
+    if (chunk < 1) chunk = 1;
+    if (chunk > 65535) chunk = 65535;
+    if (chunk > B) chunk = B;
+    tl::RowC *rows = nullptr;
+    float *ext = nullptr, *mimg = nullptr;
+    if (!cuda_ok(cudaMallocAsync(&rows, sizeof(tl::RowC) * (size_t)chunk, st))) return TL_ENOMEM;
+    if (!cuda_ok(cudaMallocAsync(&ext, ext_row * (size_t)chunk, st)) ||
+        !cuda_ok(cudaMallocAsync(&mimg, m_row * (size_t)chunk, st))) {
+        cudaFreeAsync(rows, st);
+        if (ext) cudaFreeAsync(ext, st);
+        return TL_ENOMEM;
+    }
+    cudaMemsetAsync(ext, 0, ext_row * (size_t)chunk, st);      // pitch padding must read as finite zeros
+    const int64_t rows_per_lens = B / c->cfg.n_lens;
+    int rc = TL_OK;
+    for (int64_t r0 = 0; r0 < B && rc == TL_OK; r0 += chunk) {
+        const int64_t nb = (B - r0 < chunk) ? (B - r0) : chunk;
+        tl::PrologueArgs pa;
+        pa.params = params + r0 * c->P; pa.rows = rows; pa.sigma_min = c->sigma_min;
+        pa.B = nb; pa.row0 = r0; pa.rows_per_lens = rows_per_lens;
+        pa.P = c->P; pa.n_lens_light = c->cfg.n_lens_light; pa.n_source = c->cfg.n_source;
+        pa.S = c->cfg.supersample;
+        pa.inv_u = 2.0 * c->cfg.supersample / c->cfg.pix_scale;
+        pa.fov_half = 0.5 * c->cfg.pix_scale * (c->He > c->We ? c->He : c->We);
+        pa.refine_tau = c->refine_tau;
+        pa.unit_amp = 1;
+        const int64_t nthr = nb * (1 + c->n_comp);
+        tl::prologue_kernel<<<(unsigned)((nthr + 127) / 128), 128, 0, st>>>(pa);
+        tl::KArgs a = base_args(c);
+        a.rows = rows; a.B = nb; a.rows_per_lens = rows_per_lens; a.row0 = r0;
+        a.logL = logL; a.amps = amps; a.ext = ext; a.mimg = mimg;
+        a.tile_rows = c->lin_tile_rows; a.n_tiles = c->lin_n_tiles; a.rowtab = c->lin_rowtab;
+        dim3 tg((unsigned)nb, 8);
+        c->trace_lin<<<tg, 256, c->lin_trace_smem, st>>>(a, (int)nb);
+        dim3 cg((unsigned)nb, (unsigned)c->lin_n_tiles, (unsigned)NC);
+        tl::conv_lin_kernel<<<cg, 256, c->lin_conv_smem, st>>>(a, (int)nb);
+        tl::solve_lin_kernel<<<(unsigned)nb, 256, 0, st>>>(a, (int)nb);
+        if (!cuda_ok(cudaGetLastError())) rc = TL_ECUDA;
+    }
+    cudaFreeAsync(rows, st); cudaFreeAsync(ext, st); cudaFreeAsync(mimg, st);
+    return rc;
 }
 
 int tl_loglike_batch_host(tl_ctx *ctx, const float *params, int64_t B, float *logL, void *cuda_stream)

@@ -80,6 +80,7 @@ struct PrologueArgs {
     double inv_u;                    // 2 S / pix_scale   (u-units per arcsec)
     double fov_half;                 // arcsec, half the extended field of view
     double refine_tau;               // refinement threshold in units of sigma_min
+    int unit_amp;                    // linear-amplitude mode: every I_e is taken as 1
 };
 
 // ---- b_n of PAPER.md:139 Eq. 9:  P(2n, b_n) = 1/2 ---------------------------------------
@@ -216,8 +217,11 @@ __global__ void __launch_bounds__(128) prologue_kernel(PrologueArgs a)
     const float *sp = p + 7 + 7 * k;
     SersicC C;
     bool ok = true;
-    for (int i = 0; i < 7; ++i) ok = ok && isfinite(sp[i]);
-    double Ie = sp[0], re = sp[1], n = sp[2], qs = 1.0, cs = 1.0, ss = 0.0;
+    for (int i = a.unit_amp ? 1 : 0; i < 7; ++i) ok = ok && isfinite(sp[i]);
+    // linear mode: unit amplitude; the row's own I_e (when usable) only scales the refinement
+    // criterion, as a hint of the magnitude the solved amplitude will have
+    const double Ie_hint = (isfinite(sp[0]) && fabsf(sp[0]) > 1.f) ? fabs((double)sp[0]) : 1.0;
+    double Ie = a.unit_amp ? 1.0 : (double)sp[0], re = sp[1], n = sp[2], qs = 1.0, cs = 1.0, ss = 0.0;
     ok = ok && (re > 0.0) && (n > 0.0);
     ok = ok && shape_from_e(sp[3], sp[4], &qs, &cs, &ss);
     if (!ok) { Ie = 0.0; re = 1.0; n = 1.0; qs = 1.0; cs = 1.0; ss = 0.0; }
@@ -261,7 +265,7 @@ __global__ void __launch_bounds__(128) prologue_kernel(PrologueArgs a)
     if (!is_lens_light && ok && amp != 0.0) {
         double dbeta = 2.4e-7 * (fmax((double)p[0], 0.0) + a.fov_half);               // arcsec
         double smin = a.sigma_min[(a.row0 + row) / a.rows_per_lens];
-        double cf = fabs(amp) * (bn / n) * dbeta / (re * a.refine_tau * smin);
+        double cf = fabs(amp) * (a.unit_amp ? Ie_hint : 1.0) * (bn / n) * dbeta / (re * a.refine_tau * smin);
         C.nlcf = (float)fmin(fmax(-log2(cf), -1e30), 1e30);
     }
     C.valid = ok ? 1 : 0;

@@ -28,6 +28,8 @@ struct KArgs {
     float *images;           // [B][ny][nx] or null
     float *ext;              // split path: [chunk][He][pitch] binned extended images
     double *partial;         // split path: [chunk][n_tiles] chi^2 partials
+    float *mimg;             // linear mode: [chunk][C][ny][nx] blurred unit-amplitude component images
+    float *amps;             // linear mode: [B][C] solved amplitudes or null
     int64_t B, rows_per_lens, row0;
     int ny, nx, K, Kp, h, He, We, pitch, S, n_lens_light, n_comp, edge_zero;
     int tile_rows, n_tiles;  // split path
@@ -214,6 +216,65 @@ __device__ __forceinline__ void trace_tiles(const RowC &rc, const HotC<NLL, NSRC
     }
 }
 
+// ---- linear-amplitude mode (NEXT-1, Eq. 7): the same ray-trace, but every
+// light component is accumulated on its own (at the amplitude the prologue put in `amp`, 1/S^2)
+// and stored as its own binned image: column k of L = [L_l | L_s] before blurring.
+template <int NLL, int NSRC, bool FAST>
+__device__ __forceinline__ void sample_components(const RowC &rc, const HotC<NLL, NSRC> &h, const ColV &c, const RowV &r,
+                                                  float X, float Y, float (&acc)[NLL + NSRC])
+{
+    bool fl;
+    if (NLL) acc[0] = fmaf(h.ll.amp, sersic_from_t(h.ll, fmaf(c.LB, r.dyl, c.LA + r.LC), fl), acc[0]);
+    const float xp = c.Pc + r.Qs, yp = r.Qc - c.Ps;
+    float axp, ayp;
+    if (FAST) sie_alpha(h.sie, xp, yp, axp, ayp);
+    else sie_alpha_slow(rc.lens, xp, yp, axp, ayp);
+    const float bx = (c.U + r.V) - axp, by = (c.U2 + r.V2) - ayp;      // R^T (beta - s_1)
+    float v0 = h.src[0].amp * sersic_from_t(h.src[0], quad_form(h.q[0], bx, by), fl);
+    if (fl) v0 = refined_source_light_k(rc, NLL, X, Y);
+    acc[NLL] += v0;
+    if (NSRC > 1) {
+        const float t2 = quad_form(h.q[1], (bx - h.q[1].oxh) - h.q[1].oxl, (by - h.q[1].oyh) - h.q[1].oyl);
+        float v1 = h.src[1].amp * sersic_from_t(h.src[1], t2, fl);
+        if (fl) v1 = refined_source_light_k(rc, NLL + 1, X, Y);
+        acc[NLL + NSRC - 1] += v1;
+    }
+}
+
+template <int S_T, int NLL, int NSRC, bool FAST, class Next, class Store>
+__device__ __forceinline__ void trace_tiles_lin(const RowC &rc, const HotC<NLL, NSRC> &h, const KArgs &a,
+                                                const RowV *rowtab, Next next, Store store)
+{
+    constexpr int NC = NLL + NSRC;
+    const int S = S_T > 0 ? S_T : a.S;
+    const int lane = threadIdx.x & 31;
+    const int lj = lane % a.CW, li = lane / a.CW;
+    for (int tile = next(); tile >= 0; tile = next()) {
+        const int c = tile / a.tiles_y, r = tile - c * a.tiles_y;
+        const int j = c * a.CW + lj, i = r * a.CH + li;
+        if (i >= a.He || j >= a.We) continue;
+        float acc[NC];
+#pragma unroll
+        for (int k = 0; k < NC; ++k) acc[k] = 0.f;
+        const bool edge = a.edge_zero && (j < a.h || j >= a.We - a.h || i < a.h || i >= a.He - a.h);
+        if (!edge) {
+            const float X0 = (float)(2 * j * S + 1 - S * a.We), Y0 = (float)(2 * i * S + 1 - S * a.He);
+#pragma unroll 1
+            for (int sa = 0; sa < S; ++sa) {
+                const float Y = Y0 + (float)(2 * sa);
+                const RowV rv = rowtab ? rowtab[i * S + sa] : row_values<NLL>(rc, Y);
+#pragma unroll 1
+                for (int sb = 0; sb < S; ++sb) {
+                    const float X = X0 + (float)(2 * sb);
+                    sample_components<NLL, NSRC, FAST>(rc, h, col_values<NLL>(rc, X), rv, X, Y, acc);
+                }
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < NC; ++k) store(i, j, k, acc[k]);
+    }
+}
+
 // RowV of all He * S sub-sample rows -> shared memory (all threads of the CTA; caller syncs).
 template <int NLL>
 __device__ __forceinline__ void fill_rowtab(const RowC &rc, const KArgs &a, RowV *rowtab)
@@ -230,6 +291,18 @@ __device__ __forceinline__ void fill_rowtab(const RowC &rc, const KArgs &a, RowV
 // CTA draw tiles from a shared-memory counter, so they all reach the barrier that ends the
 // phase within one tile of each other whatever the refinement branches cost; the value of a
 // pixel does not depend on which warp computes it, so logL stays bitwise reproducible.
+template <int S_T, int NLL, int NSRC, class Store>
+__device__ __forceinline__ void trace_image_lin(const RowC &rc, const KArgs &a, const RowV *rowtab, int warp, int n_warps, Store store)
+{
+    const int n = a.tiles_x * a.tiles_y;
+    const HotC<NLL, NSRC> h(rc);
+    int t = (int)((long long)n * warp / n_warps);
+    const int t_end = (int)((long long)n * (warp + 1) / n_warps);
+    auto next = [&]() -> int { return t < t_end ? t++ : -1; };
+    if (rc.lens.mode == 0) trace_tiles_lin<S_T, NLL, NSRC, true>(rc, h, a, rowtab, next, store);
+    else trace_tiles_lin<S_T, NLL, NSRC, false>(rc, h, a, rowtab, next, store);
+}
+
 template <int S_T, int NLL, int NSRC, class Store>
 __device__ __forceinline__ void trace_image(const RowC &rc, const KArgs &a, const RowV *rowtab, int warp, int n_warps, int *counter, Store store)
 {
@@ -587,6 +660,140 @@ __global__ void finalize_kernel(const KArgs a, int chunk_rows)
     for (int t = 0; t < a.n_tiles; ++t) s += a.partial[(size_t)r * a.n_tiles + t];
     const double ll = -0.5 * (s + a.lconst[row / a.rows_per_lens]);
     a.logL[row] = isfinite(s) ? (float)ll : -INFINITY;
+}
+
+// ------------------------------------------------------------------------------ linear mode
+// (NEXT-1, Eq. 6-7)  trace_lin_kernel -> conv_lin_kernel -> solve_lin_kernel.
+template <int NLL, int NSRC>
+__global__ void __launch_bounds__(256) trace_lin_kernel(const KArgs a, int chunk_rows)
+{
+    __shared__ RowC rc_s;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    RowV *rowtab = a.rowtab ? reinterpret_cast<RowV *>(smem_raw) : nullptr;
+    constexpr int NC = NLL + NSRC;
+    for (int r = blockIdx.x; r < chunk_rows; r += gridDim.x) {
+        __syncthreads();
+        load_row_consts(&rc_s, a.rows + r);
+        __syncthreads();
+        if (!row_is_valid(rc_s, a.n_comp)) continue;
+        if (rowtab) { fill_rowtab<NLL>(rc_s, a, rowtab); __syncthreads(); }
+        float *dst = a.ext + (size_t)r * NC * a.He * a.pitch;
+        const size_t comp_stride = (size_t)a.He * a.pitch;
+        trace_image_lin<0, NLL, NSRC>(rc_s, a, rowtab, (blockIdx.y * blockDim.x + threadIdx.x) >> 5, (gridDim.y * blockDim.x) >> 5,
+                                      [&](int i, int j, int k, float v) { dst[k * comp_stride + i * a.pitch + j] = v; });
+    }
+}
+
+// one CTA per (row_in_chunk, tile of output rows, component): M_k = K (*) L_k  (blurring matrix B)
+__global__ void __launch_bounds__(256) conv_lin_kernel(const KArgs a, int chunk_rows)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float *taps = reinterpret_cast<float *>(smem_raw);
+    float *img = taps + a.K * a.Kp;
+    const int r = blockIdx.x, tile = blockIdx.y, k = blockIdx.z, NC = gridDim.z;
+    const int64_t row = a.row0 + r;
+    const int64_t lens = row / a.rows_per_lens;
+    const size_t npix = (size_t)a.ny * a.nx;
+    if (!row_is_valid(a.rows[r], a.n_comp)) return;
+    const int i0 = tile * a.tile_rows, i1 = min(a.ny, i0 + a.tile_rows);
+    load_psf(taps, a.psf + lens * a.K * a.Kp, a.K * a.Kp);
+    const int erows = (i1 - i0) + 2 * a.h;
+    const float4 *src = reinterpret_cast<const float4 *>(a.ext + (((size_t)r * NC + k) * a.He + i0) * a.pitch);
+    float4 *dst = reinterpret_cast<float4 *>(img);
+    const int n4 = erows * a.pitch / 4;
+    for (int i = threadIdx.x; i < n4; i += blockDim.x) dst[i] = src[i];
+    for (int i = threadIdx.x; i < a.pitch + a.Kp + 8; i += blockDim.x) img[erows * a.pitch + i] = 0.f;
+    __syncthreads();
+    conv_chi2_rows(a, img, i0, taps, i0, i1, nullptr, nullptr, a.mimg + ((size_t)r * NC + k) * npix);
+}
+
+// minimise s'G s - 2 b's over s >= 0 for n <= 3: every support, normal equations by Cramer's rule
+__device__ inline void nnls_small(int n, const double G[3][3], const double b[3], double s[3])
+{
+    double best = 0.0;
+    s[0] = s[1] = s[2] = 0.0;
+    for (int m = 1; m < (1 << n); ++m) {
+        double x[3] = {0.0, 0.0, 0.0};
+        const bool u0 = m & 1, u1 = m & 2, u2 = m & 4;
+        const int cnt = (int)u0 + (int)u1 + (int)u2;
+        if (cnt == 1) {
+            const int i = u0 ? 0 : (u1 ? 1 : 2);
+            if (!(G[i][i] > 0.0)) continue;
+            x[i] = b[i] / G[i][i];
+        } else if (cnt == 2) {
+            const int i = u0 ? 0 : 1, j = u2 ? 2 : 1;
+            const double det = G[i][i] * G[j][j] - G[i][j] * G[i][j];
+            if (!(fabs(det) > 1e-300)) continue;
+            x[i] = (b[i] * G[j][j] - b[j] * G[i][j]) / det;
+            x[j] = (b[j] * G[i][i] - b[i] * G[i][j]) / det;
+        } else {
+            const double c00 = G[1][1] * G[2][2] - G[1][2] * G[1][2], c01 = G[0][2] * G[1][2] - G[0][1] * G[2][2],
+                         c02 = G[0][1] * G[1][2] - G[0][2] * G[1][1], c11 = G[0][0] * G[2][2] - G[0][2] * G[0][2],
+                         c12 = G[0][1] * G[0][2] - G[0][0] * G[1][2], c22 = G[0][0] * G[1][1] - G[0][1] * G[0][1];
+            const double det = G[0][0] * c00 + G[0][1] * c01 + G[0][2] * c02;
+            if (!(fabs(det) > 1e-300)) continue;
+            x[0] = (c00 * b[0] + c01 * b[1] + c02 * b[2]) / det;
+            x[1] = (c01 * b[0] + c11 * b[1] + c12 * b[2]) / det;
+            x[2] = (c02 * b[0] + c12 * b[1] + c22 * b[2]) / det;
+        }
+        if (!(x[0] >= 0.0 && x[1] >= 0.0 && x[2] >= 0.0)) continue;
+        const double f = -(b[0] * x[0] + b[1] * x[1] + b[2] * x[2]);       // penalty change at a stationary point
+        if (f < best) { best = f; s[0] = x[0]; s[1] = x[1]; s[2] = x[2]; }
+    }
+}
+
+// one CTA per row: G = M'WM, b = M'Wd (fixed-shape FP64 reductions), NNLS, chi^2 of the residual
+__global__ void __launch_bounds__(256) solve_lin_kernel(const KArgs a, int chunk_rows)
+{
+    __shared__ double red[32];
+    __shared__ double s_sh[3];
+    const int r = blockIdx.x, NC = a.n_comp;
+    const int64_t row = a.row0 + r;
+    const int64_t lens = row / a.rows_per_lens;
+    const int npix = a.ny * a.nx;
+    if (!row_is_valid(a.rows[r], a.n_comp)) {
+        if (threadIdx.x == 0) {
+            a.logL[row] = -INFINITY;
+            if (a.amps) for (int k = 0; k < NC; ++k) a.amps[row * NC + k] = NAN;
+        }
+        return;
+    }
+    const float *M = a.mimg + (size_t)r * NC * npix;
+    const float *d = a.data + lens * (size_t)npix, *w = a.wgt + lens * (size_t)npix;
+    double g[6] = {0, 0, 0, 0, 0, 0}, bb[3] = {0, 0, 0};             // G00 G01 G02 G11 G12 G22
+    for (int i = threadIdx.x; i < npix; i += blockDim.x) {
+        const double wi = w[i], di = d[i];
+        double m[3] = {0.0, 0.0, 0.0};
+        for (int k = 0; k < NC; ++k) m[k] = M[(size_t)k * npix + i];
+        g[0] += wi * m[0] * m[0]; g[1] += wi * m[0] * m[1]; g[2] += wi * m[0] * m[2];
+        g[3] += wi * m[1] * m[1]; g[4] += wi * m[1] * m[2]; g[5] += wi * m[2] * m[2];
+        bb[0] += wi * m[0] * di; bb[1] += wi * m[1] * di; bb[2] += wi * m[2] * di;
+    }
+    double G[3][3], b[3];
+    const double g0 = block_sum(g[0], red), g1 = block_sum(g[1], red), g2 = block_sum(g[2], red),
+                 g3 = block_sum(g[3], red), g4 = block_sum(g[4], red), g5 = block_sum(g[5], red);
+    b[0] = block_sum(bb[0], red); b[1] = block_sum(bb[1], red); b[2] = block_sum(bb[2], red);
+    if (threadIdx.x == 0) {
+        G[0][0] = g0; G[0][1] = G[1][0] = g1; G[0][2] = G[2][0] = g2; G[1][1] = g3; G[1][2] = G[2][1] = g4; G[2][2] = g5;
+        double s[3];
+        nnls_small(NC, G, b, s);
+        s_sh[0] = s[0]; s_sh[1] = s[1]; s_sh[2] = s[2];
+    }
+    __syncthreads();
+    const double s0 = s_sh[0], s1 = s_sh[1], s2 = s_sh[2];
+    double part = 0.0;
+    for (int i = threadIdx.x; i < npix; i += blockDim.x) {
+        double m = s0 * M[i];
+        if (NC > 1) m += s1 * M[(size_t)npix + i];
+        if (NC > 2) m += s2 * M[2 * (size_t)npix + i];
+        const double res = (double)d[i] - m;
+        part += res * res * (double)w[i];
+    }
+    const double chi2 = block_sum(part, red);
+    if (threadIdx.x == 0) {
+        a.logL[row] = (float)(-0.5 * (chi2 + a.lconst[lens]));
+        if (a.amps) { a.amps[row * NC] = (float)s0; if (NC > 1) a.amps[row * NC + 1] = (float)s1; if (NC > 2) a.amps[row * NC + 2] = (float)s2; }
+    }
 }
 
 }  // namespace tl

@@ -169,4 +169,10 @@ __device__ __noinline__ float refined_source_light(const RowC &rc, int k0, int k
     return src;
 }
 
+// Same for one source component k only (linear-amplitude mode keeps the components apart).
+__device__ __noinline__ float refined_source_light_k(const RowC &rc, int k, float X, float Y)
+{
+    return refined_source_light(rc, k, k + 1, X, Y);
+}
+
 }  // namespace tl

@@ -1,0 +1,85 @@
+"""GPU parity of tl_loglike_linear_batch (NEXT-1: Eq. 6-7) against the oracle."""
+import numpy as np
+import pytest
+
+from paper_2503_08586_b200 import workloads as W
+from tests import parity as PT
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def api():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_2503_08586_b200 import api as _api
+    _api.load()
+    return _api
+
+
+def _run(api, orc, w, prob, rows):
+    import torch
+    ctx = api.LensContext.from_problem(prob)
+    d = torch.from_numpy(rows).cuda()
+    ll, amps = ctx.loglike_linear(d)
+    ll2, _ = ctx.loglike_linear(d, want_amps=False)
+    torch.cuda.synchronize()
+    assert torch.equal(ll, ll2)                      # bitwise reproducible
+    fixed = ctx.loglike(d)
+    ctx.close()
+    oll, oamps = orc.loglike_linear_batch(orc.config_of(w), prob.psf, prob.data, prob.noise, rows, n_lens=w.n_lens)
+    return ll.cpu().numpy().astype(np.float64), amps.cpu().numpy().astype(np.float64), oll, oamps, \
+        fixed.cpu().numpy().astype(np.float64)
+
+
+@pytest.mark.parametrize("idx,n_prior,n_near,n_lens", [(0, 32, 32, 1), (1, 12, 12, 1), (3, 6, 6, 3), (4, 1, 1, 1)])
+def test_linear_likelihood_matches_oracle(api, orc, idx, n_prior, n_near, n_lens):
+    w = W.workload(idx).scaled(batch=n_lens * n_prior, n_lens=n_lens)
+    prob = W.make_problem(w, orc.render_for_workloads)
+    rows, isnear = PT.rows_with_near(W, w, prob, n_prior, n_near)
+    rows[::3, 7] = np.nan                     # the I_e entries are ignored, whatever they hold
+    ll, amps, oll, oamps, fixed = _run(api, orc, w, prob, rows)
+    assert np.all(np.isfinite(ll))
+    # amplitudes: relative to the largest amplitude of the row
+    scale = np.maximum(np.abs(oamps).max(axis=1, keepdims=True), 1e-30)
+    assert np.all(np.abs(amps - oamps) <= 2e-5 * scale), np.abs((amps - oamps) / scale).max()
+    tol = PT.logl_tol(oll)
+    dl = np.abs(ll - oll)
+    # With the amplitudes solved every row is "near its best fit": |logL| is small while chi^2
+    # terms are large, so the FP32 floor of tests/parity.py applies to all rows;
+    # the oracle's own optimal model image provides z and SNR.
+    per = len(rows) // w.n_lens
+    lens = np.arange(len(rows)) // per
+    cfg = orc.config_of(w)
+    oimg = np.stack([np.tensordot(oamps[r], orc.component_images(cfg, prob.psf[lens[r]], np.where(np.isnan(rows[r]), 1.0, rows[r]).astype(np.float32)), axes=1)
+                     for r in range(len(rows))])
+    floor = PT.fp32_floor(oimg, prob.data[lens], prob.noise[lens], w.supersample)
+    tn = np.maximum(tol, floor)
+    assert np.all(dl <= tn), "linear logL parity: worst %.3g x derived tol (%.3g x north-star)" % ((dl / tn).max(), (dl / tol).max())
+    print("config %d linear: logL %.3g x north-star tol, %.3g x derived; amps rel %.2e"
+          % (idx, (dl / tol).max(), (dl / tn).max(), np.abs((amps - oamps) / scale).max()))
+    # Eq. 6: the solved likelihood is at least the fixed-amplitude one of the same row
+    ok = np.isfinite(fixed)
+    assert np.all(ll[ok] >= fixed[ok] - 1e-3 - 1e-6 * np.abs(fixed[ok]))
+
+
+def test_linear_invalid_rows_and_clamp(api, orc):
+    import torch
+    w = W.workload(0).scaled(batch=8)
+    prob = W.make_problem(w, orc.render_for_workloads)
+    rows = W.batch_rows(w, 8)
+    rows[1, 0] = -1.0                          # theta_E < 0
+    rows[2, 9] = 0.0                           # n = 0
+    rows[3, 1] = np.inf
+    # a source far outside the field: its image is ~0 everywhere, amplitude stays finite and >= 0
+    rows[4, 12] = 50.0; rows[4, 13] = 50.0
+    ctx = api.LensContext.from_problem(prob)
+    ll, amps = ctx.loglike_linear(torch.from_numpy(rows).cuda())
+    ll = ll.cpu().numpy(); amps = amps.cpu().numpy()
+    ctx.close()
+    for r in (1, 2, 3):
+        assert ll[r] == -np.inf and np.all(np.isnan(amps[r]))
+    for r in (0, 4, 5, 6, 7):
+        assert np.isfinite(ll[r]) and np.all(amps[r] >= 0.0)
+    oll, oamps = orc.loglike_linear_batch(orc.config_of(w), prob.psf, prob.data, prob.noise, rows)
+    assert np.all(np.isinf(oll[[1, 2, 3]]))
