@@ -331,6 +331,60 @@ def run_ours(args, w: W.Workload):
         dist.destroy_process_group()
 
 
+def run_linear(args, w: W.Workload):
+    """Secondary line: the paper's linear/non-linear split (NEXT-1).  Same workload, amplitudes
+    solved per row; value = rows / device time (CUDA events), oracle timed on a bounded sample."""
+    import torch
+    from paper_2503_08586_b200 import api
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    dev = torch.device("cuda", 0)
+
+    def gpu_render(w1, psf, row):
+        ctx = api.LensContext(w1.ny, w1.nx, w1.pix_scale, w1.supersample, w1.n_lens_light, w1.n_source,
+                              psf[None], np.zeros((1, w1.ny, w1.nx), np.float32),
+                              np.ones((1, w1.ny, w1.nx), np.float32), w1.edge_mode)
+        im = ctx.render(torch.from_numpy(np.ascontiguousarray(row[None])).to(dev)).cpu().numpy()[0]
+        ctx.close()
+        return im
+
+    prob = W.make_problem(w, gpu_render)
+    ctx = api.LensContext.from_problem(prob)
+    rows = W.batch_rows(w)
+    B = rows.shape[0]
+    d_rows = torch.from_numpy(rows).to(dev)
+    out = torch.empty(B, dtype=torch.float32, device=dev)
+    amps = torch.empty((B, w.n_lens_light + w.n_source), dtype=torch.float32, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    for _ in range(max(args.warmup, 3)):
+        ctx.loglike_linear(d_rows, out, amps)
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    with ClockSampler(0) as clk:
+        for s in range(args.steps):
+            flush.fill_(s & 0xff)
+            ev[s][0].record(); ctx.loglike_linear(d_rows, out, amps); ev[s][1].record()
+        torch.cuda.synchronize()
+    total_ms = float(np.sum([a.elapsed_time(b) for a, b in ev]))
+    value = B * args.steps / (total_ms * 1e-3)
+    line = {"metric": METRIC + " (linear amplitudes, NNLS per row)", "value": value, "unit": UNIT, "n_gpus": 1,
+            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": config_dict(w, "flushed between steps (256 MiB fill)"), "clocks": clk.summary(),
+            "pixel_evals_per_s": value * w.ny * w.nx, "mode": "linear",
+            "gpu_launches": args.steps * 4 * int(np.ceil(B / 2600.0)), "checksum_logL": float(out.double().sum())}
+    if not args.no_cpu_baseline:
+        from oracle import oracle as O
+        O.lib()
+        n = min(args.ref_rows, 128)
+        t0 = time.perf_counter()
+        O.loglike_linear_batch(O.config_of(w), prob.psf, prob.data, prob.noise, rows[:n], n_lens=w.n_lens)
+        dt = time.perf_counter() - t0
+        line["cpu_baseline"] = {"value": n / dt, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle",
+                                "sample": "first %d of the %d rows, %.1f s" % (n, B, dt)}
+    print(json.dumps(line))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -341,6 +395,9 @@ def main():
     ap.add_argument("--batch", type=int, default=0, help="override rows per GPU (parity/debug only)")
     ap.add_argument("--ref-rows", type=int, default=512, help="oracle sample size per step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--mode", default="fixed", choices=["fixed", "linear"],
+                    help="fixed: amplitudes are parameters (the headline metric); linear: amplitudes solved by NNLS "
+                         "per row (tl_loglike_linear_batch, PAPER.md Eq. 6-7) -- a secondary line")
     args = ap.parse_args()
     w = W.workload(args.config)
     if args.batch:
@@ -348,7 +405,9 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if world != args.gpus and world > 1:
         raise SystemExit("--gpus %d does not match WORLD_SIZE %d" % (args.gpus, world))
-    if args.impl == "reference":
+    if args.mode == "linear":
+        run_linear(args, w)
+    elif args.impl == "reference":
         run_reference(args, w)
     else:
         run_ours(args, w)

@@ -86,10 +86,20 @@ trace_fn trace_for(int S, int nll, int nsrc)
     }
 }
 
-trace_fn trace_lin_for(int nll, int nsrc)
+template <int S_T>
+trace_fn pick_trace_lin(int nll, int nsrc)
 {
-    if (nll == 0) return nsrc == 1 ? tl::trace_lin_kernel<0, 1> : tl::trace_lin_kernel<0, 2>;
-    return nsrc == 1 ? tl::trace_lin_kernel<1, 1> : tl::trace_lin_kernel<1, 2>;
+    if (nll == 0) return nsrc == 1 ? tl::trace_lin_kernel<S_T, 0, 1> : tl::trace_lin_kernel<S_T, 0, 2>;
+    return nsrc == 1 ? tl::trace_lin_kernel<S_T, 1, 1> : tl::trace_lin_kernel<S_T, 1, 2>;
+}
+trace_fn trace_lin_for(int S, int nll, int nsrc)
+{
+    switch (S) {
+    case 1: return pick_trace_lin<1>(nll, nsrc);
+    case 2: return pick_trace_lin<2>(nll, nsrc);
+    case 4: return pick_trace_lin<4>(nll, nsrc);
+    default: return pick_trace_lin<0>(nll, nsrc);       // S = 8 and odd S: generic loop
+    }
 }
 
 // phase-1 warp tile CW x CH = 32 lanes: the shape that wastes the fewest lanes on the ragged
@@ -356,7 +366,7 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
             if (tr > cfg->ny) tr = cfg->ny;
             c->lin_tile_rows = tr; c->lin_n_tiles = (cfg->ny + tr - 1) / tr;
             c->lin_conv_smem = sizeof(float) * ((size_t)c->K * c->Kp + (size_t)(tr + 2 * c->h + 1) * c->pitch + c->Kp + 8);
-            c->trace_lin = trace_lin_for(cfg->n_lens_light, cfg->n_source);
+            c->trace_lin = trace_lin_for(cfg->supersample, cfg->n_lens_light, cfg->n_source);
             bool okl = cuda_ok(cudaFuncSetAttribute(tl::conv_lin_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT));
             if (rowtab_bytes <= 48 * 1024) {
                 c->lin_rowtab = 1; c->lin_trace_smem = rowtab_bytes;

@@ -109,8 +109,8 @@ struct HotC {
 // sources at beta (returned), both already scaled by 1/S^2 so that the caller only adds
 // (step a5, bin = mean).  FAST = polynomial SIE path (q >= 0.5).
 template <int NLL, int NSRC, bool FAST>
-__device__ __forceinline__ float sample_value(const RowC &rc, const HotC<NLL, NSRC> &h, const ColV &c, const RowV &r,
-                                              float &acc, bool &flag)
+__device__ __forceinline__ void sample_value(const RowC &rc, const HotC<NLL, NSRC> &h, const ColV &c, const RowV &r,
+                                             float &acc, float (&src)[NSRC], bool &flag)
 {
     bool fl;
     if (NLL) acc = fmaf(h.ll.amp, sersic_from_t(h.ll, fmaf(c.LB, r.dyl, c.LA + r.LC), fl), acc);
@@ -119,14 +119,13 @@ __device__ __forceinline__ float sample_value(const RowC &rc, const HotC<NLL, NS
     if (FAST) sie_alpha(h.sie, xp, yp, axp, ayp);
     else sie_alpha_slow(rc.lens, xp, yp, axp, ayp);
     const float bx = (c.U + r.V) - axp, by = (c.U2 + r.V2) - ayp;      // R^T (beta - s_1)
-    float src = h.src[0].amp * sersic_from_t(h.src[0], quad_form(h.q[0], bx, by), fl);
+    src[0] = h.src[0].amp * sersic_from_t(h.src[0], quad_form(h.q[0], bx, by), fl);
     flag = fl;
     if (NSRC > 1) {
         const float t2 = quad_form(h.q[1], (bx - h.q[1].oxh) - h.q[1].oxl, (by - h.q[1].oyh) - h.q[1].oyl);
-        src = fmaf(h.src[1].amp, sersic_from_t(h.src[1], t2, fl), src);
+        src[NSRC - 1] = h.src[1].amp * sersic_from_t(h.src[1], t2, fl);
         flag = flag || fl;
     }
-    return src;
 }
 
 // steps a1-a5 for a run of `count` warp tiles.  A warp tile is CW x CH = 32 extended native
@@ -139,7 +138,9 @@ __device__ __forceinline__ float sample_value(const RowC &rc, const HotC<NLL, NS
 // `rowtab` (optional, shared memory): the RowV of every sub-sample row of the image, filled once
 // per parameter row by fill_rowtab(); without it each thread recomputes them (18 instructions
 // per sub-row instead of two LDS.128).
-template <int S_T, int NLL, int NSRC, bool FAST, class Next, class Store>
+// LIN (linear-amplitude mode): the components are kept apart and handed to store(i, j, k, v),
+// k = 0 .. NLL + NSRC - 1; otherwise their sum goes to store(i, j, v).
+template <int S_T, int NLL, int NSRC, bool FAST, bool LIN, class Next, class Store>
 __device__ __forceinline__ void trace_tiles(const RowC &rc, const HotC<NLL, NSRC> &h, const KArgs &a,
                                             const RowV *rowtab, Next next, Store store)
 {
@@ -161,7 +162,10 @@ __device__ __forceinline__ void trace_tiles(const RowC &rc, const HotC<NLL, NSRC
     for (;;) {
         const int i = r * a.CH + li;
         if (i < a.He && j < a.We) {
-            float acc = 0.f;
+            float acc = 0.f;                           // lens light (and, unless LIN, everything)
+            float accs[NSRC];                          // LIN: the sources, each on its own
+#pragma unroll
+            for (int k = 0; k < NSRC; ++k) accs[k] = 0.f;
             const bool edge = a.edge_zero && (j < a.h || j >= a.We - a.h || i < a.h || i >= a.He - a.h);
             if (!edge) {
                 const float Y0 = (float)(2 * i * S + 1 - S * a.He);
@@ -170,35 +174,67 @@ __device__ __forceinline__ void trace_tiles(const RowC &rc, const HotC<NLL, NSRC
                     const float Y = Y0 + (float)(2 * sa);
                     const RowV rv = rowtab ? rowtab[i * S + sa] : row_values<NLL>(rc, Y);
                     if (S_T > 0) {
-                        float src[S_T > 0 ? S_T : 1];
+                        float src[S_T > 0 ? S_T : 1][NSRC];
                         bool any = false;
 #pragma unroll
                         for (int sb = 0; sb < S_T; ++sb) {
                             bool fl;
-                            src[sb] = sample_value<NLL, NSRC, FAST>(rc, h, cv[sb], rv, acc, fl);
+                            sample_value<NLL, NSRC, FAST>(rc, h, cv[sb], rv, acc, src[sb], fl);
                             any = any || fl;
-                            if (fl) src[sb] = __int_as_float(0x7fc00000);      // NaN marks "refine me"
+                            if (fl) src[sb][0] = __int_as_float(0x7fc00000);      // NaN marks "refine me"
                         }
                         if (any) {                                  // rare: FP64 ray-trace, out of line
 #pragma unroll
                             for (int sb = 0; sb < S_T; ++sb)
-                                if (src[sb] != src[sb])
-                                    src[sb] = refined_source_light(rc, NLL, NLL + NSRC, X0 + (float)(2 * sb), Y);
+                                if (src[sb][0] != src[sb][0]) {
+                                    if (LIN && NSRC > 1) {
+#pragma unroll
+                                        for (int k = 0; k < NSRC; ++k)
+                                            src[sb][k] = refined_source_light_k(rc, NLL + k, X0 + (float)(2 * sb), Y);
+                                    } else {
+                                        src[sb][0] = refined_source_light(rc, NLL, NLL + NSRC, X0 + (float)(2 * sb), Y);
+                                        if (NSRC > 1) src[sb][NSRC - 1] = 0.f;
+                                    }
+                                }
                         }
 #pragma unroll
-                        for (int sb = 0; sb < S_T; ++sb) acc += src[sb];
+                        for (int sb = 0; sb < S_T; ++sb) {
+                            if (LIN) {
+#pragma unroll
+                                for (int k = 0; k < NSRC; ++k) accs[k] += src[sb][k];
+                            } else {
+                                acc += src[sb][0];
+                                if (NSRC > 1) acc += src[sb][NSRC - 1];
+                            }
+                        }
                     } else {
                         for (int sb = 0; sb < S; ++sb) {
                             const float X = X0 + (float)(2 * sb);
                             bool fl;
-                            float sv = sample_value<NLL, NSRC, FAST>(rc, h, col_values<NLL>(rc, X), rv, acc, fl);
-                            if (fl) sv = refined_source_light(rc, NLL, NLL + NSRC, X, Y);
-                            acc += sv;
+                            float sv[NSRC];
+                            sample_value<NLL, NSRC, FAST>(rc, h, col_values<NLL>(rc, X), rv, acc, sv, fl);
+                            if (fl) {
+#pragma unroll
+                                for (int k = 0; k < NSRC; ++k) sv[k] = refined_source_light_k(rc, NLL + k, X, Y);
+                            }
+                            if (LIN) {
+#pragma unroll
+                                for (int k = 0; k < NSRC; ++k) accs[k] += sv[k];
+                            } else {
+#pragma unroll
+                                for (int k = 0; k < NSRC; ++k) acc += sv[k];
+                            }
                         }
                     }
                 }
             }
-            store(i, j, acc);
+            if constexpr (LIN) {
+                if (NLL) store(i, j, 0, acc);
+#pragma unroll
+                for (int k = 0; k < NSRC; ++k) store(i, j, NLL + k, accs[k]);
+            } else {
+                store(i, j, acc);
+            }
         }
         tile = next();
         if (tile < 0) break;
@@ -213,65 +249,6 @@ __device__ __forceinline__ void trace_tiles(const RowC &rc, const HotC<NLL, NSRC
                 for (int b = 0; b < S_T; ++b) cv[b] = col_values<NLL>(rc, X0 + (float)(2 * b));
             }
         }
-    }
-}
-
-// ---- linear-amplitude mode (NEXT-1, Eq. 7): the same ray-trace, but every
-// light component is accumulated on its own (at the amplitude the prologue put in `amp`, 1/S^2)
-// and stored as its own binned image: column k of L = [L_l | L_s] before blurring.
-template <int NLL, int NSRC, bool FAST>
-__device__ __forceinline__ void sample_components(const RowC &rc, const HotC<NLL, NSRC> &h, const ColV &c, const RowV &r,
-                                                  float X, float Y, float (&acc)[NLL + NSRC])
-{
-    bool fl;
-    if (NLL) acc[0] = fmaf(h.ll.amp, sersic_from_t(h.ll, fmaf(c.LB, r.dyl, c.LA + r.LC), fl), acc[0]);
-    const float xp = c.Pc + r.Qs, yp = r.Qc - c.Ps;
-    float axp, ayp;
-    if (FAST) sie_alpha(h.sie, xp, yp, axp, ayp);
-    else sie_alpha_slow(rc.lens, xp, yp, axp, ayp);
-    const float bx = (c.U + r.V) - axp, by = (c.U2 + r.V2) - ayp;      // R^T (beta - s_1)
-    float v0 = h.src[0].amp * sersic_from_t(h.src[0], quad_form(h.q[0], bx, by), fl);
-    if (fl) v0 = refined_source_light_k(rc, NLL, X, Y);
-    acc[NLL] += v0;
-    if (NSRC > 1) {
-        const float t2 = quad_form(h.q[1], (bx - h.q[1].oxh) - h.q[1].oxl, (by - h.q[1].oyh) - h.q[1].oyl);
-        float v1 = h.src[1].amp * sersic_from_t(h.src[1], t2, fl);
-        if (fl) v1 = refined_source_light_k(rc, NLL + 1, X, Y);
-        acc[NLL + NSRC - 1] += v1;
-    }
-}
-
-template <int S_T, int NLL, int NSRC, bool FAST, class Next, class Store>
-__device__ __forceinline__ void trace_tiles_lin(const RowC &rc, const HotC<NLL, NSRC> &h, const KArgs &a,
-                                                const RowV *rowtab, Next next, Store store)
-{
-    constexpr int NC = NLL + NSRC;
-    const int S = S_T > 0 ? S_T : a.S;
-    const int lane = threadIdx.x & 31;
-    const int lj = lane % a.CW, li = lane / a.CW;
-    for (int tile = next(); tile >= 0; tile = next()) {
-        const int c = tile / a.tiles_y, r = tile - c * a.tiles_y;
-        const int j = c * a.CW + lj, i = r * a.CH + li;
-        if (i >= a.He || j >= a.We) continue;
-        float acc[NC];
-#pragma unroll
-        for (int k = 0; k < NC; ++k) acc[k] = 0.f;
-        const bool edge = a.edge_zero && (j < a.h || j >= a.We - a.h || i < a.h || i >= a.He - a.h);
-        if (!edge) {
-            const float X0 = (float)(2 * j * S + 1 - S * a.We), Y0 = (float)(2 * i * S + 1 - S * a.He);
-#pragma unroll 1
-            for (int sa = 0; sa < S; ++sa) {
-                const float Y = Y0 + (float)(2 * sa);
-                const RowV rv = rowtab ? rowtab[i * S + sa] : row_values<NLL>(rc, Y);
-#pragma unroll 1
-                for (int sb = 0; sb < S; ++sb) {
-                    const float X = X0 + (float)(2 * sb);
-                    sample_components<NLL, NSRC, FAST>(rc, h, col_values<NLL>(rc, X), rv, X, Y, acc);
-                }
-            }
-        }
-#pragma unroll
-        for (int k = 0; k < NC; ++k) store(i, j, k, acc[k]);
     }
 }
 
@@ -299,8 +276,8 @@ __device__ __forceinline__ void trace_image_lin(const RowC &rc, const KArgs &a, 
     int t = (int)((long long)n * warp / n_warps);
     const int t_end = (int)((long long)n * (warp + 1) / n_warps);
     auto next = [&]() -> int { return t < t_end ? t++ : -1; };
-    if (rc.lens.mode == 0) trace_tiles_lin<S_T, NLL, NSRC, true>(rc, h, a, rowtab, next, store);
-    else trace_tiles_lin<S_T, NLL, NSRC, false>(rc, h, a, rowtab, next, store);
+    if (rc.lens.mode == 0) trace_tiles<S_T, NLL, NSRC, true, true>(rc, h, a, rowtab, next, store);
+    else trace_tiles<S_T, NLL, NSRC, false, true>(rc, h, a, rowtab, next, store);
 }
 
 template <int S_T, int NLL, int NSRC, class Store>
@@ -316,14 +293,14 @@ __device__ __forceinline__ void trace_image(const RowC &rc, const KArgs &a, cons
             t = __shfl_sync(0xffffffffu, t, 0);
             return t < n ? t : -1;
         };
-        if (fast) trace_tiles<S_T, NLL, NSRC, true>(rc, h, a, rowtab, next, store);
-        else trace_tiles<S_T, NLL, NSRC, false>(rc, h, a, rowtab, next, store);
+        if (fast) trace_tiles<S_T, NLL, NSRC, true, false>(rc, h, a, rowtab, next, store);
+        else trace_tiles<S_T, NLL, NSRC, false, false>(rc, h, a, rowtab, next, store);
     } else {
         int t = (int)((long long)n * warp / n_warps);
         const int t_end = (int)((long long)n * (warp + 1) / n_warps);
         auto next = [&]() -> int { return t < t_end ? t++ : -1; };
-        if (fast) trace_tiles<S_T, NLL, NSRC, true>(rc, h, a, rowtab, next, store);
-        else trace_tiles<S_T, NLL, NSRC, false>(rc, h, a, rowtab, next, store);
+        if (fast) trace_tiles<S_T, NLL, NSRC, true, false>(rc, h, a, rowtab, next, store);
+        else trace_tiles<S_T, NLL, NSRC, false, false>(rc, h, a, rowtab, next, store);
     }
 }
 
@@ -664,8 +641,8 @@ __global__ void finalize_kernel(const KArgs a, int chunk_rows)
 
 // ------------------------------------------------------------------------------ linear mode
 // (NEXT-1, Eq. 6-7)  trace_lin_kernel -> conv_lin_kernel -> solve_lin_kernel.
-template <int NLL, int NSRC>
-__global__ void __launch_bounds__(256) trace_lin_kernel(const KArgs a, int chunk_rows)
+template <int S_T, int NLL, int NSRC>
+__global__ void __launch_bounds__(256, 2) trace_lin_kernel(const KArgs a, int chunk_rows)
 {
     __shared__ RowC rc_s;
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -679,7 +656,7 @@ __global__ void __launch_bounds__(256) trace_lin_kernel(const KArgs a, int chunk
         if (rowtab) { fill_rowtab<NLL>(rc_s, a, rowtab); __syncthreads(); }
         float *dst = a.ext + (size_t)r * NC * a.He * a.pitch;
         const size_t comp_stride = (size_t)a.He * a.pitch;
-        trace_image_lin<0, NLL, NSRC>(rc_s, a, rowtab, (blockIdx.y * blockDim.x + threadIdx.x) >> 5, (gridDim.y * blockDim.x) >> 5,
+        trace_image_lin<S_T, NLL, NSRC>(rc_s, a, rowtab, (blockIdx.y * blockDim.x + threadIdx.x) >> 5, (gridDim.y * blockDim.x) >> 5,
                                       [&](int i, int j, int k, float v) { dst[k * comp_stride + i * a.pitch + j] = v; });
     }
 }
