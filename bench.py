@@ -205,7 +205,8 @@ def run_ours(args, w: W.Workload):
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
     torch.cuda.set_device(local)
-    if world > 1:
+    use_dist = world > 1 or "TORCHELASTIC_RUN_ID" in os.environ      # under torchrun, even with one rank
+    if use_dist:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     dev = torch.device("cuda", local)
 
@@ -233,7 +234,7 @@ def run_ours(args, w: W.Workload):
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
 
     def barrier():
-        if world > 1:
+        if use_dist:
             dist.barrier()
         torch.cuda.synchronize()
 
@@ -273,12 +274,12 @@ def run_ours(args, w: W.Workload):
     total_ms = float(np.sum(step_ms))
     logl_sum = float(h_out.double().sum())
 
-    if world > 1:
+    if use_dist:
         t = torch.tensor([total_ms, e2e_s], dtype=torch.float64, device=dev)
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         total_ms, e2e_s = float(t[0]), float(t[1])
     if rank != 0:
-        if world > 1:
+        if use_dist:
             dist.destroy_process_group()
         return
 
@@ -327,7 +328,7 @@ def run_ours(args, w: W.Workload):
         line["cpu_baseline"] = {"value": n / dt, "unit": UNIT, "cores": used, "kind": "oracle",
                                 "sample": "first %d of the %d rows of the step, %.1f s" % (n, B, dt)}
     print(json.dumps(line))
-    if world > 1:
+    if use_dist:
         dist.destroy_process_group()
 
 
