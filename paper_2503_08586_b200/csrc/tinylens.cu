@@ -44,7 +44,6 @@ struct tl_ctx {
     // benchmark facility (tl_set_profiling): events around the dominant kernel of the last call
     int profile = 0;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
-    float prof_ms = 0.f;          // accumulated over the chunks of the last call
     int prof_pending = 0;
 };
 

@@ -543,15 +543,9 @@ __global__ void __launch_bounds__(TL_LB_T, TL_LB_B) fused_kernel(const KArgs a)
         }
         // phase 1: ray-trace + light + bin into shared memory
         if (rowtab) { fill_rowtab<NLL>(*rc, a, rowtab); __syncthreads(); }
-#ifndef TL_EXP_SKIP_TRACE
         trace_image<S_T, NLL, NSRC>(*rc, a, rowtab, threadIdx.x >> 5, blockDim.x >> 5, tile_counter,
                                     [&](int i, int j, float v) { img[i * a.pitch + j] = v; });
-#endif
         __syncthreads();
-#ifdef TL_EXP_SKIP_CONV
-        if (a.logL && threadIdx.x == 0) a.logL[row] = img[(a.He / 2) * a.pitch + a.We / 2];
-        continue;
-#endif
         // phase 2: PSF convolution from shared memory + chi^2
         const double part = conv_chi2_rows(a, img, 0, taps, 0, a.ny,
                                            a.logL ? a.data + lens * npix : nullptr,
