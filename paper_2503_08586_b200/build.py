@@ -14,17 +14,17 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtinylens.so")
-SOURCES = [os.path.join(CSRC, "tinylens.cu")]
-HEADERS = [os.path.join(CSRC, f) for f in ("tl_consts.cuh", "tl_sample.cuh", "tl_kernels.cuh")] + \
+SOURCES = [os.path.join(CSRC, f) for f in ("tinylens.cu", "tl_inst_fused.cu", "tl_inst_split.cu", "tl_inst_lin.cu")]
+HEADERS = [os.path.join(CSRC, f) for f in ("tl_consts.cuh", "tl_sample.cuh", "tl_kernels.cuh", "tl_dispatch.h")] + \
           [os.path.join(os.path.dirname(HERE), "include", "tinylens.h")]
 
-NVCC_FLAGS = [
+NVCC_COMPILE = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-lineinfo", "-std=c++17",
-    "--shared", "-Xcompiler", "-fPIC",
-    "-cudart", "static",
+    "-Xcompiler", "-fPIC",
     "-Xptxas", "-v",
 ]
+NVCC_LINK = ["-gencode", "arch=compute_100a,code=sm_100a", "--shared", "-Xcompiler", "-fPIC", "-cudart", "static"]
 
 
 def nvcc_path() -> str:
@@ -44,18 +44,41 @@ def needs_build() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not needs_build():
         return LIB
+    # the translation units are independent (no relocatable device code): compile them in
+    # parallel, then link one shared library
+    bdir = os.path.join(HERE, "build")
+    os.makedirs(bdir, exist_ok=True)
+    procs, objs, log = [], [], []
+    for src in SOURCES:
+        obj = os.path.join(bdir, os.path.basename(src)[:-3] + ".%d.o" % os.getpid())
+        cmd = [nvcc_path()] + NVCC_COMPILE + ["-c", "-o", obj, src]
+        procs.append((cmd, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
+        objs.append(obj)
+    failed = None
+    for cmd, p in procs:
+        out, _ = p.communicate()
+        log.append(" ".join(cmd) + "\n" + out)
+        if p.returncode != 0 and failed is None:
+            failed = (cmd, out)
     tmp = LIB + ".tmp.%d" % os.getpid()
-    cmd = [nvcc_path()] + NVCC_FLAGS + ["-o", tmp] + SOURCES
-    proc = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
-    if proc.returncode != 0:
+    if failed is None:
+        cmd = [nvcc_path()] + NVCC_LINK + ["-o", tmp] + objs
+        proc = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
+        log.append(" ".join(cmd) + "\n" + proc.stdout)
+        if proc.returncode != 0:
+            failed = (cmd, proc.stdout)
+    for o in objs:
+        if os.path.exists(o):
+            os.remove(o)
+    if failed is not None:
         if os.path.exists(tmp):
             os.remove(tmp)
-        raise RuntimeError("nvcc failed:\n%s\n%s" % (" ".join(cmd), proc.stdout))
+        raise RuntimeError("nvcc failed:\n%s\n%s" % (" ".join(failed[0]), failed[1]))
     os.replace(tmp, LIB)
     with open(os.path.join(HERE, "build.log"), "w") as f:
-        f.write(" ".join(cmd) + "\n" + proc.stdout)
+        f.write("\n".join(log))
     if verbose:
-        print(proc.stdout)
+        print("\n".join(log))
     return LIB
 
 

@@ -12,7 +12,9 @@
 #include <cuda_runtime.h>
 
 #include "../../include/tinylens.h"
+#define TL_MAIN_TU            /* this unit owns the non-template kernels */
 #include "tl_kernels.cuh"
+#include "tl_dispatch.h"
 
 #define TL_VERSION_STRING "tinylens-b200 0.1 (sm_100a)"
 
@@ -33,6 +35,9 @@ struct tl_ctx {
     // linear-amplitude mode (tl_loglike_linear_batch): always the staged pipeline
     void (*trace_lin)(const tl::KArgs, int) = nullptr;
     int lin_tile_rows = 0, lin_n_tiles = 0, lin_rowtab = 0;
+    void (*fused_lin)(const tl::KArgs) = nullptr;     // component images in shared memory, when they fit
+    size_t lin_fused_smem = 0;
+    int lin_fused_rowtab = 0, lin_fused_grid = 0;
     size_t lin_conv_smem = 0, lin_trace_smem = 0;
     int rowtab = 0;               // RowV table in shared memory (fused: after the image; split: trace_kernel)
     size_t trace_smem = 0;
@@ -48,58 +53,6 @@ struct tl_ctx {
 };
 
 namespace {
-
-typedef void (*fused_fn)(const tl::KArgs);
-typedef void (*trace_fn)(const tl::KArgs, int);
-
-template <int S_T>
-fused_fn pick_fused(int nll, int nsrc)
-{
-    if (nll == 0) return nsrc == 1 ? tl::fused_kernel<S_T, 0, 1> : tl::fused_kernel<S_T, 0, 2>;
-    return nsrc == 1 ? tl::fused_kernel<S_T, 1, 1> : tl::fused_kernel<S_T, 1, 2>;
-}
-template <int S_T>
-trace_fn pick_trace(int nll, int nsrc)
-{
-    if (nll == 0) return nsrc == 1 ? tl::trace_kernel<S_T, 0, 1> : tl::trace_kernel<S_T, 0, 2>;
-    return nsrc == 1 ? tl::trace_kernel<S_T, 1, 1> : tl::trace_kernel<S_T, 1, 2>;
-}
-fused_fn fused_for(int S, int nll, int nsrc)
-{
-    switch (S) {
-    case 1: return pick_fused<1>(nll, nsrc);
-    case 2: return pick_fused<2>(nll, nsrc);
-    case 4: return pick_fused<4>(nll, nsrc);
-    case 8: return pick_fused<8>(nll, nsrc);
-    default: return pick_fused<0>(nll, nsrc);
-    }
-}
-trace_fn trace_for(int S, int nll, int nsrc)
-{
-    switch (S) {
-    case 1: return pick_trace<1>(nll, nsrc);
-    case 2: return pick_trace<2>(nll, nsrc);
-    case 4: return pick_trace<4>(nll, nsrc);
-    case 8: return pick_trace<8>(nll, nsrc);
-    default: return pick_trace<0>(nll, nsrc);
-    }
-}
-
-template <int S_T>
-trace_fn pick_trace_lin(int nll, int nsrc)
-{
-    if (nll == 0) return nsrc == 1 ? tl::trace_lin_kernel<S_T, 0, 1> : tl::trace_lin_kernel<S_T, 0, 2>;
-    return nsrc == 1 ? tl::trace_lin_kernel<S_T, 1, 1> : tl::trace_lin_kernel<S_T, 1, 2>;
-}
-trace_fn trace_lin_for(int S, int nll, int nsrc)
-{
-    switch (S) {
-    case 1: return pick_trace_lin<1>(nll, nsrc);
-    case 2: return pick_trace_lin<2>(nll, nsrc);
-    case 4: return pick_trace_lin<4>(nll, nsrc);
-    default: return pick_trace_lin<0>(nll, nsrc);       // S = 8 and odd S: generic loop
-    }
-}
 
 // phase-1 warp tile CW x CH = 32 lanes: the shape that wastes the fewest lanes on the ragged
 // right / bottom edge of the extended image
@@ -326,7 +279,7 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
         c->path = 0; c->smem = fs;
         c->threads = fs > SMEM_LIMIT / 2 ? 512 : 256;
         if (const char *e = std::getenv("TL_THREADS")) { const int v = std::atoi(e); if (v >= 32 && v <= 512 && v % 32 == 0) c->threads = v; }
-        c->fused = fused_for(cfg->supersample, cfg->n_lens_light, cfg->n_source);
+        c->fused = tl_fused_for(cfg->supersample, cfg->n_lens_light, cfg->n_source);
         if (!cuda_ok(cudaFuncSetAttribute(c->fused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT))) { tl_destroy(c); return TL_ECUDA; }
         int occ = 0;
         if (!cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, c->fused, c->threads, fs)) || occ < 1) { tl_destroy(c); return TL_ECUDA; }
@@ -343,7 +296,7 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
         c->conv_smem = conv_smem_bytes(c, tr);
         if (!cuda_ok(cudaFuncSetAttribute(tl::conv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT))) { tl_destroy(c); return TL_ECUDA; }
         c->threads = 256; c->smem = c->conv_smem;
-        c->trace = trace_for(cfg->supersample, cfg->n_lens_light, cfg->n_source);
+        c->trace = tl_trace_for(cfg->supersample, cfg->n_lens_light, cfg->n_source);
         if (rowtab_bytes <= 48 * 1024 && cfg->supersample <= 4) {   // S = 8 amortises row values over 8 samples already
             c->rowtab = 1; c->trace_smem = rowtab_bytes;
             if (!cuda_ok(cudaFuncSetAttribute(c->trace, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rowtab_bytes))) { tl_destroy(c); return TL_ECUDA; }
@@ -365,13 +318,27 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
             if (tr > cfg->ny) tr = cfg->ny;
             c->lin_tile_rows = tr; c->lin_n_tiles = (cfg->ny + tr - 1) / tr;
             c->lin_conv_smem = sizeof(float) * ((size_t)c->K * c->Kp + (size_t)(tr + 2 * c->h + 1) * c->pitch + c->Kp + 8);
-            c->trace_lin = trace_lin_for(cfg->supersample, cfg->n_lens_light, cfg->n_source);
+            c->trace_lin = tl_trace_lin_for(cfg->supersample, cfg->n_lens_light, cfg->n_source);
             bool okl = cuda_ok(cudaFuncSetAttribute(tl::conv_lin_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT));
             if (rowtab_bytes <= 48 * 1024) {
                 c->lin_rowtab = 1; c->lin_trace_smem = rowtab_bytes;
                 okl = okl && cuda_ok(cudaFuncSetAttribute(c->trace_lin, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rowtab_bytes));
             }
             if (!okl) { tl_destroy(c); return TL_ECUDA; }
+        }
+        // fused variant: C binned component images (+ the row-value table) in shared memory
+        const size_t img_floats = ((size_t)c->He * c->pitch + c->pitch + c->Kp + 8 + 3) & ~(size_t)3;
+        size_t fl = sizeof(tl::RowC) + 32 * sizeof(double) + sizeof(float) * ((size_t)c->K * c->Kp + (size_t)c->n_comp * img_floats);
+        int rt = 0;
+        if (fl + rowtab_bytes <= SMEM_LIMIT) { fl += rowtab_bytes; rt = 1; }
+        if (fl <= SMEM_LIMIT) {
+            fused_fn fn = tl_fused_lin_for(cfg->supersample, cfg->n_lens_light, cfg->n_source);
+            int occ = 0;
+            if (cuda_ok(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT)) &&
+                cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, 512, fl)) && occ >= 1) {
+                c->fused_lin = fn; c->lin_fused_smem = fl; c->lin_fused_rowtab = rt; c->lin_fused_grid = occ * c->n_sm;
+            }
+            cudaGetLastError();
         }
     }
     *out = c;
@@ -416,6 +383,38 @@ int tl_loglike_linear_batch(tl_ctx *c, const float *params, int64_t B, float *lo
     if (dev != c->device && !cuda_ok(cudaSetDevice(c->device))) return TL_ECUDA;
     const int NC = c->n_comp;
     const size_t npix = (size_t)c->cfg.ny * c->cfg.nx;
+    if (c->fused_lin && !std::getenv("TL_LINEAR_STAGED")) {
+        const int64_t chunkf = CONST_CHUNK < B ? CONST_CHUNK : B;
+        tl::RowC *rowsf = nullptr;
+        float *mscr = nullptr;
+        if (!cuda_ok(cudaMallocAsync(&rowsf, sizeof(tl::RowC) * (size_t)chunkf, st))) return TL_ENOMEM;
+        if (!cuda_ok(cudaMallocAsync(&mscr, sizeof(float) * (size_t)c->lin_fused_grid * NC * npix, st))) { cudaFreeAsync(rowsf, st); return TL_ENOMEM; }
+        const int64_t rpl = B / c->cfg.n_lens;
+        int rcf = TL_OK;
+        for (int64_t r0 = 0; r0 < B && rcf == TL_OK; r0 += chunkf) {
+            const int64_t nb = (B - r0 < chunkf) ? (B - r0) : chunkf;
+            tl::PrologueArgs pa;
+            pa.params = params + r0 * c->P; pa.rows = rowsf; pa.sigma_min = c->sigma_min;
+            pa.B = nb; pa.row0 = r0; pa.rows_per_lens = rpl;
+            pa.P = c->P; pa.n_lens_light = c->cfg.n_lens_light; pa.n_source = c->cfg.n_source;
+            pa.S = c->cfg.supersample;
+            pa.inv_u = 2.0 * c->cfg.supersample / c->cfg.pix_scale;
+            pa.fov_half = 0.5 * c->cfg.pix_scale * (c->He > c->We ? c->He : c->We);
+            pa.refine_tau = c->refine_tau;
+            pa.unit_amp = 1;
+            const int64_t nthr = nb * (1 + c->n_comp);
+            tl::prologue_kernel<<<(unsigned)((nthr + 127) / 128), 128, 0, st>>>(pa);
+            tl::KArgs a = base_args(c);
+            a.rows = rowsf; a.B = nb; a.rows_per_lens = rpl; a.row0 = r0;
+            a.logL = logL; a.amps = amps; a.mimg = mscr; a.rowtab = c->lin_fused_rowtab;
+            int grid = c->lin_fused_grid;
+            if ((int64_t)grid > nb) grid = (int)nb;
+            c->fused_lin<<<grid, 512, c->lin_fused_smem, st>>>(a);
+            if (!cuda_ok(cudaGetLastError())) rcf = TL_ECUDA;
+        }
+        cudaFreeAsync(rowsf, st); cudaFreeAsync(mscr, st);
+        return rcf;
+    }
     const size_t ext_row = sizeof(float) * (size_t)NC * c->He * c->pitch, m_row = sizeof(float) * NC * npix;
     int64_t chunk = (int64_t)(EXT_SCRATCH_BYTES / (ext_row + m_row));
     if (chunk < 1) chunk = 1;

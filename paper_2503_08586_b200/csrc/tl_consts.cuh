@@ -145,6 +145,7 @@ __device__ inline bool shape_from_e(double e1, double e2, double *q, double *c, 
     return true;
 }
 
+#ifdef TL_MAIN_TU
 __global__ void __launch_bounds__(128) prologue_kernel(PrologueArgs a)
 {
     const int nslot = 1 + a.n_lens_light + a.n_source;
@@ -271,5 +272,7 @@ __global__ void __launch_bounds__(128) prologue_kernel(PrologueArgs a)
     C.valid = ok ? 1 : 0;
     rc->comp[k] = C;
 }
+
+#endif  // TL_MAIN_TU
 
 }  // namespace tl

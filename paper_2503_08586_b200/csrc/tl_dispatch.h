@@ -1,0 +1,13 @@
+// tl_dispatch.h -- kernel tables.  The template kernels are instantiated in three translation
+// units of their own (tl_inst_fused.cu, tl_inst_split.cu, tl_inst_lin.cu) so that nvcc can compile
+// them in parallel; tinylens.cu only asks for the function pointer that matches a context.
+#pragma once
+#include "tl_kernels.cuh"
+
+typedef void (*fused_fn)(const tl::KArgs);
+typedef void (*trace_fn)(const tl::KArgs, int);
+
+fused_fn tl_fused_for(int S, int n_lens_light, int n_source);          // fused_kernel<S, NLL, NSRC>
+trace_fn tl_trace_for(int S, int n_lens_light, int n_source);          // trace_kernel<S, NLL, NSRC>
+fused_fn tl_fused_lin_for(int S, int n_lens_light, int n_source);      // fused_lin_kernel<...>
+trace_fn tl_trace_lin_for(int S, int n_lens_light, int n_source);      // trace_lin_kernel<...>

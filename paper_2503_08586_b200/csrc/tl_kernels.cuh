@@ -269,15 +269,27 @@ __device__ __forceinline__ void fill_rowtab(const RowC &rc, const KArgs &a, RowV
 // phase within one tile of each other whatever the refinement branches cost; the value of a
 // pixel does not depend on which warp computes it, so logL stays bitwise reproducible.
 template <int S_T, int NLL, int NSRC, class Store>
-__device__ __forceinline__ void trace_image_lin(const RowC &rc, const KArgs &a, const RowV *rowtab, int warp, int n_warps, Store store)
+__device__ __forceinline__ void trace_image_lin(const RowC &rc, const KArgs &a, const RowV *rowtab, int warp, int n_warps, int *counter, Store store)
 {
     const int n = a.tiles_x * a.tiles_y;
     const HotC<NLL, NSRC> h(rc);
-    int t = (int)((long long)n * warp / n_warps);
-    const int t_end = (int)((long long)n * (warp + 1) / n_warps);
-    auto next = [&]() -> int { return t < t_end ? t++ : -1; };
-    if (rc.lens.mode == 0) trace_tiles<S_T, NLL, NSRC, true, true>(rc, h, a, rowtab, next, store);
-    else trace_tiles<S_T, NLL, NSRC, false, true>(rc, h, a, rowtab, next, store);
+    const bool fast = rc.lens.mode == 0;
+    if (counter) {
+        auto next = [&]() -> int {
+            int t = 0;
+            if ((threadIdx.x & 31) == 0) t = atomicAdd(counter, 1);
+            t = __shfl_sync(0xffffffffu, t, 0);
+            return t < n ? t : -1;
+        };
+        if (fast) trace_tiles<S_T, NLL, NSRC, true, true>(rc, h, a, rowtab, next, store);
+        else trace_tiles<S_T, NLL, NSRC, false, true>(rc, h, a, rowtab, next, store);
+    } else {
+        int t = (int)((long long)n * warp / n_warps);
+        const int t_end = (int)((long long)n * (warp + 1) / n_warps);
+        auto next = [&]() -> int { return t < t_end ? t++ : -1; };
+        if (fast) trace_tiles<S_T, NLL, NSRC, true, true>(rc, h, a, rowtab, next, store);
+        else trace_tiles<S_T, NLL, NSRC, false, true>(rc, h, a, rowtab, next, store);
+    }
 }
 
 template <int S_T, int NLL, int NSRC, class Store>
@@ -580,6 +592,7 @@ __global__ void __launch_bounds__(256) trace_kernel(const KArgs a, int chunk_row
     }
 }
 
+#ifdef TL_MAIN_TU
 // conv_kernel: one CTA per (row_in_chunk, tile of `tile_rows` output rows).
 __global__ void __launch_bounds__(256) conv_kernel(const KArgs a, int chunk_rows)
 {
@@ -633,6 +646,8 @@ __global__ void finalize_kernel(const KArgs a, int chunk_rows)
     a.logL[row] = isfinite(s) ? (float)ll : -INFINITY;
 }
 
+#endif  // TL_MAIN_TU
+
 // ------------------------------------------------------------------------------ linear mode
 // (NEXT-1, Eq. 6-7)  trace_lin_kernel -> conv_lin_kernel -> solve_lin_kernel.
 template <int S_T, int NLL, int NSRC>
@@ -650,11 +665,12 @@ __global__ void __launch_bounds__(256, 2) trace_lin_kernel(const KArgs a, int ch
         if (rowtab) { fill_rowtab<NLL>(rc_s, a, rowtab); __syncthreads(); }
         float *dst = a.ext + (size_t)r * NC * a.He * a.pitch;
         const size_t comp_stride = (size_t)a.He * a.pitch;
-        trace_image_lin<S_T, NLL, NSRC>(rc_s, a, rowtab, (blockIdx.y * blockDim.x + threadIdx.x) >> 5, (gridDim.y * blockDim.x) >> 5,
+        trace_image_lin<S_T, NLL, NSRC>(rc_s, a, rowtab, (blockIdx.y * blockDim.x + threadIdx.x) >> 5, (gridDim.y * blockDim.x) >> 5, nullptr,
                                       [&](int i, int j, int k, float v) { dst[k * comp_stride + i * a.pitch + j] = v; });
     }
 }
 
+#ifdef TL_MAIN_TU
 // one CTA per (row_in_chunk, tile of output rows, component): M_k = K (*) L_k  (blurring matrix B)
 __global__ void __launch_bounds__(256) conv_lin_kernel(const KArgs a, int chunk_rows)
 {
@@ -677,6 +693,8 @@ __global__ void __launch_bounds__(256) conv_lin_kernel(const KArgs a, int chunk_
     __syncthreads();
     conv_chi2_rows(a, img, i0, taps, i0, i1, nullptr, nullptr, a.mimg + ((size_t)r * NC + k) * npix);
 }
+
+#endif  // TL_MAIN_TU
 
 // minimise s'G s - 2 b's over s >= 0 for n <= 3: every support, normal equations by Cramer's rule
 __device__ inline void nnls_small(int n, const double G[3][3], const double b[3], double s[3])
@@ -713,23 +731,12 @@ __device__ inline void nnls_small(int n, const double G[3][3], const double b[3]
     }
 }
 
-// one CTA per row: G = M'WM, b = M'Wd (fixed-shape FP64 reductions), NNLS, chi^2 of the residual
-__global__ void __launch_bounds__(256) solve_lin_kernel(const KArgs a, int chunk_rows)
+// G = M'WM, b = M'Wd (fixed-shape FP64 reductions), NNLS, chi^2 of the residual d - M s -> logL.
+// All threads of the CTA; M = the row's blurred unit-amplitude component images [C][npix].
+__device__ __forceinline__ void solve_row(const KArgs &a, const float *M, int64_t row, int64_t lens,
+                                          double *red, double *s_sh)
 {
-    __shared__ double red[32];
-    __shared__ double s_sh[3];
-    const int r = blockIdx.x, NC = a.n_comp;
-    const int64_t row = a.row0 + r;
-    const int64_t lens = row / a.rows_per_lens;
-    const int npix = a.ny * a.nx;
-    if (!row_is_valid(a.rows[r], a.n_comp)) {
-        if (threadIdx.x == 0) {
-            a.logL[row] = -INFINITY;
-            if (a.amps) for (int k = 0; k < NC; ++k) a.amps[row * NC + k] = NAN;
-        }
-        return;
-    }
-    const float *M = a.mimg + (size_t)r * NC * npix;
+    const int NC = a.n_comp, npix = a.ny * a.nx;
     const float *d = a.data + lens * (size_t)npix, *w = a.wgt + lens * (size_t)npix;
     double g[6] = {0, 0, 0, 0, 0, 0}, bb[3] = {0, 0, 0};             // G00 G01 G02 G11 G12 G22
     for (int i = threadIdx.x; i < npix; i += blockDim.x) {
@@ -764,6 +771,70 @@ __global__ void __launch_bounds__(256) solve_lin_kernel(const KArgs a, int chunk
     if (threadIdx.x == 0) {
         a.logL[row] = (float)(-0.5 * (chi2 + a.lconst[lens]));
         if (a.amps) { a.amps[row * NC] = (float)s0; if (NC > 1) a.amps[row * NC + 1] = (float)s1; if (NC > 2) a.amps[row * NC + 2] = (float)s2; }
+    }
+}
+
+__device__ __forceinline__ void invalid_row_lin(const KArgs &a, int64_t row)
+{
+    if (threadIdx.x == 0) {
+        a.logL[row] = -INFINITY;
+        if (a.amps) for (int k = 0; k < a.n_comp; ++k) a.amps[row * a.n_comp + k] = NAN;
+    }
+}
+
+#ifdef TL_MAIN_TU
+// staged pipeline: one CTA per row
+__global__ void __launch_bounds__(256) solve_lin_kernel(const KArgs a, int chunk_rows)
+{
+    __shared__ double red[32];
+    __shared__ double s_sh[3];
+    const int r = blockIdx.x;
+    const int64_t row = a.row0 + r;
+    if (!row_is_valid(a.rows[r], a.n_comp)) { invalid_row_lin(a, row); return; }
+    solve_row(a, a.mimg + (size_t)r * a.n_comp * a.ny * a.nx, row, row / a.rows_per_lens, red, s_sh);
+}
+
+#endif  // TL_MAIN_TU
+
+// fused pipeline (when the C binned component images fit in shared memory): persistent CTAs,
+// per row  trace (components apart, dynamic tile queue) -> C convolutions from shared memory,
+// blurred columns of M to a per-CTA global scratch (L2-resident) -> solve_row.
+template <int S_T, int NLL, int NSRC>
+__global__ void __launch_bounds__(512, 1) fused_lin_kernel(const KArgs a)
+{
+    constexpr int NC = NLL + NSRC;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    RowC *rc = reinterpret_cast<RowC *>(smem_raw);
+    double *red = reinterpret_cast<double *>(smem_raw + sizeof(RowC));            // [0, 16): block_sum
+    double *s_sh = red + 20;
+    int *tile_counter = reinterpret_cast<int *>(red + 24);
+    float *taps = reinterpret_cast<float *>(smem_raw + sizeof(RowC) + 32 * sizeof(double));
+    float *img = taps + a.K * a.Kp;
+    const int img_stride = (a.He * a.pitch + a.pitch + a.Kp + 8 + 3) & ~3;         // floats per component image
+    RowV *rowtab = a.rowtab ? reinterpret_cast<RowV *>(img + NC * img_stride) : nullptr;
+    for (int i = threadIdx.x; i < NC * img_stride; i += blockDim.x) img[i] = 0.f;
+    const size_t npix = (size_t)a.ny * a.nx;
+    float *M = a.mimg + (size_t)blockIdx.x * NC * npix;                            // this CTA's scratch
+
+    int64_t cur_lens = -1;
+    for (int64_t r = blockIdx.x; r < a.B; r += gridDim.x) {
+        const int64_t row = a.row0 + r;
+        const int64_t lens = row / a.rows_per_lens;
+        __syncthreads();
+        load_row_consts(rc, a.rows + r);
+        if (threadIdx.x == 0) *tile_counter = 0;
+        if (lens != cur_lens) { load_psf(taps, a.psf + lens * a.K * a.Kp, a.K * a.Kp); cur_lens = lens; }
+        __syncthreads();
+        if (!row_is_valid(*rc, a.n_comp)) { invalid_row_lin(a, row); continue; }
+        if (rowtab) { fill_rowtab<NLL>(*rc, a, rowtab); __syncthreads(); }
+        trace_image_lin<S_T, NLL, NSRC>(*rc, a, rowtab, threadIdx.x >> 5, blockDim.x >> 5, tile_counter,
+                                        [&](int i, int j, int k, float v) { img[k * img_stride + i * a.pitch + j] = v; });
+        __syncthreads();
+#pragma unroll 1
+        for (int k = 0; k < NC; ++k)
+            conv_chi2_rows(a, img + k * img_stride, 0, taps, 0, a.ny, nullptr, nullptr, M + k * npix);
+        __syncthreads();                               // M (global) visible to the whole CTA
+        solve_row(a, M, row, lens, red, s_sh);
     }
 }
 

@@ -100,7 +100,7 @@ __device__ __forceinline__ void sie_alpha(const SieHot &L, float xp, float yp, f
 }
 
 // strongly flattened lenses (q < 0.5): libdevice inverse functions, out of line
-__device__ __noinline__ void sie_alpha_slow(const LensC &L, float xp, float yp, float &axp, float &ayp)
+static __device__ __noinline__ void sie_alpha_slow(const LensC &L, float xp, float yp, float &axp, float &ayp)
 {
     const float xx = xp * xp;
     const float psi2 = fmaf(L.q2h, xx, fmaf(L.q2l, xx, yp * yp));
@@ -154,7 +154,7 @@ __device__ __forceinline__ void refine_offsets(const LensC &L, const SersicC &C,
 }
 
 // Source light of one sub-sample with the ray-trace redone in FP64 (rare, out of line).
-__device__ __noinline__ float refined_source_light(const RowC &rc, int k0, int k1, float X, float Y)
+static __device__ __noinline__ float refined_source_light(const RowC &rc, int k0, int k1, float X, float Y)
 {
     float src = 0.f;
     for (int k = k0; k < k1; ++k) {
@@ -170,7 +170,7 @@ __device__ __noinline__ float refined_source_light(const RowC &rc, int k0, int k
 }
 
 // Same for one source component k only (linear-amplitude mode keeps the components apart).
-__device__ __noinline__ float refined_source_light_k(const RowC &rc, int k, float X, float Y)
+static __device__ __noinline__ float refined_source_light_k(const RowC &rc, int k, float X, float Y)
 {
     return refined_source_light(rc, k, k + 1, X, Y);
 }

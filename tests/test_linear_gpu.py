@@ -83,3 +83,21 @@ def test_linear_invalid_rows_and_clamp(api, orc):
         assert np.isfinite(ll[r]) and np.all(amps[r] >= 0.0)
     oll, oamps = orc.loglike_linear_batch(orc.config_of(w), prob.psf, prob.data, prob.noise, rows)
     assert np.all(np.isinf(oll[[1, 2, 3]]))
+
+
+def test_fused_and_staged_pipelines_agree(api, orc, monkeypatch):
+    """configs[1] fits the fused linear kernel; TL_LINEAR_STAGED forces the staged pipeline that
+    larger images use.  Same arithmetic per pixel -> identical bits."""
+    import torch
+    w = W.workload(1).scaled(batch=40)
+    prob = W.make_problem(w, orc.render_for_workloads)
+    rows = W.batch_rows(w, 40)
+    ctx = api.LensContext.from_problem(prob)
+    d = torch.from_numpy(rows).cuda()
+    ll_f, am_f = ctx.loglike_linear(d)
+    torch.cuda.synchronize()
+    monkeypatch.setenv("TL_LINEAR_STAGED", "1")
+    ll_s, am_s = ctx.loglike_linear(d)
+    torch.cuda.synchronize()
+    ctx.close()
+    assert torch.equal(ll_f, ll_s) and torch.equal(am_f, am_s)
