@@ -18,7 +18,7 @@ LOGL_ABS, LOGL_REL = 1e-3, 1e-6
 #   * a systematic relative error |eps_coh| <= 2^-22 (measured <= 1.5e-7; MUFU.LG2 / MUFU.EX2
 #     biases amplified by b_n u), coherent over the image,
 # hence the bound that FP32 arithmetic can meet on such rows,
-#   tol = max(north_star, eps_coh |sum_i z_i SNR_i| + 4 eps_rnd sqrt(sum_i z_i^2 SNR_i^2)).
+#   tol = max(north_star, eps_coh |sum_i z_i SNR_i| + 5 eps_rnd sqrt(sum_i z_i^2 SNR_i^2))   (5 sigma: several hundred rows are tested).
 EPS_RND = 2.0 ** -21
 EPS_COH = 2.0 ** -22
 EPS_ACC = 2.0 ** -22
@@ -29,12 +29,12 @@ def logl_tol(oll):
 
 
 def fp32_floor(oimg, data, noise, S):
-    """eps_coh |sum z SNR| + 4 (eps_rnd/S + eps_acc) sqrt(sum z^2 SNR^2) per row; oimg [B,ny,nx] float64 oracle images."""
+    """eps_coh |sum z SNR| + 5 (eps_rnd/S + eps_acc) sqrt(sum z^2 SNR^2) per row; oimg [B,ny,nx] float64 oracle images."""
     sig = np.asarray(noise, np.float64)
     z = (np.asarray(data, np.float64) - oimg) / sig
     snr = oimg / sig
     coh = EPS_COH * np.abs(np.sum(z * snr, axis=(1, 2)))
-    rnd = 4.0 * (EPS_RND / S + EPS_ACC) * np.sqrt(np.sum((z * snr) ** 2, axis=(1, 2)))
+    rnd = 5.0 * (EPS_RND / S + EPS_ACC) * np.sqrt(np.sum((z * snr) ** 2, axis=(1, 2)))
     return coh + rnd
 
 

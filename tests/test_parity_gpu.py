@@ -304,3 +304,55 @@ def test_full_size_batches_sampled_against_oracle(api, torch, orc, idx, batch, n
         l = r // per
         want = orc.loglike(cfg, prob.psf[l], prob.data[l], prob.noise[l], rows[r])
         assert abs(ll[r] - want) <= max(PT.LOGL_ABS, PT.LOGL_REL * abs(want)), (r, ll[r], want)
+
+
+def test_call_is_cuda_graph_capturable(api, torch, orc):
+    """NEXT-4 (caller-side overheads): tl_loglike_batch makes no host sync and takes
+    its scratch from the stream-ordered allocator, so a sampler can capture it in a CUDA graph."""
+    w = W.workload(0)
+    prob = W.make_problem(w, orc.render_for_workloads)
+    rows = W.batch_rows(w)
+    ctx = api.LensContext.from_problem(prob)
+    d = torch.from_numpy(rows).cuda()
+    ref = ctx.loglike(d).clone()
+    out = torch.empty_like(ref)
+    s = torch.cuda.Stream()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(s):
+        ctx.loglike(d, out, stream=s)
+        s.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            ctx.loglike(d, out, stream=s)
+    out.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(out, ref)
+    d.copy_(torch.from_numpy(rows[::-1].copy()).cuda())       # new parameters, same buffers
+    g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(out, ref.flip(0))
+    del g
+    ctx.close()
+
+
+def _random_case(rng):
+    ny, nx = int(rng.integers(3, 40)), int(rng.integers(3, 40))
+    S = int(rng.integers(1, 7))
+    K = int(rng.choice([1, 3, 5, 7, 9, 13, 15, 21]))
+    return dict(ny=ny, nx=nx, supersample=S, psf_size=K, pix_scale=float(rng.uniform(0.03, 0.3)),
+                n_lens_light=int(rng.integers(0, 2)), n_source=int(rng.integers(1, 3)),
+                edge_mode=int(rng.integers(0, 2)), psf_kind=str(rng.choice(["gaussian", "moffat"])),
+                psf_fwhm=float(rng.uniform(0.1, 0.4)))
+
+
+@pytest.mark.parametrize("seed", range(12))
+def test_random_shapes(api, torch, orc, seed):
+    """Seeded random geometry (odd / tiny sizes, every S in 1..6, PSF sizes on both convolution
+    paths, both edge modes, 1-3 components): indexing errors anywhere show up as pixel errors."""
+    rng = np.random.default_rng(1000 + seed)
+    w, prob = _small_problem(orc, index=20 + seed, **_random_case(rng))
+    rows, isnear = PT.rows_with_near(W, w, prob, 6, 2)
+    ll, im, _ = _gpu_eval(api, torch, w, prob, rows)
+    oll, oim = PT.oracle_reference(orc, w, prob, rows)
+    _check(w, prob, rows, isnear, ll, im, oll, oim, floor_all=True)
