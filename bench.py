@@ -357,14 +357,17 @@ def run_linear(args, w: W.Workload):
     out = torch.empty(B, dtype=torch.float32, device=dev)
     amps = torch.empty((B, w.n_lens_light + w.n_source), dtype=torch.float32, device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    ctx.set_profiling(True)
     for _ in range(max(args.warmup, 3)):
         ctx.loglike_linear(d_rows, out, amps)
     torch.cuda.synchronize()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    kern_ms = []
     with ClockSampler(0) as clk:
         for s in range(args.steps):
             flush.fill_(s & 0xff)
             ev[s][0].record(); ctx.loglike_linear(d_rows, out, amps); ev[s][1].record()
+            kern_ms.append(ctx.last_kernel_ms())
         torch.cuda.synchronize()
     total_ms = float(np.sum([a.elapsed_time(b) for a, b in ev]))
     value = B * args.steps / (total_ms * 1e-3)
@@ -373,7 +376,21 @@ def run_linear(args, w: W.Workload):
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": config_dict(w, "flushed between steps (256 MiB fill)"), "clocks": clk.summary(),
             "pixel_evals_per_s": value * w.ny * w.nx, "mode": "linear",
-            "gpu_launches": args.steps * 4 * int(np.ceil(B / 2600.0)), "checksum_logL": float(out.double().sum())}
+            "gpu_launches": args.steps * 2, "checksum_logL": float(out.double().sum())}
+    # roofline of the fused linear kernel: op model v0 per sample (unchanged) + per native pixel
+    # C convolutions, the Gram matrix / right-hand side (C (C + 3)) and the residual (C + 3)
+    C_ = w.n_lens_light + w.n_source
+    om = op_model(w)
+    slots = om["issue_slots"] + w.ny * w.nx * ((C_ - 1) * w.psf_size ** 2 + C_ * (C_ + 3) + C_ + 3 - OP_CHI2_FP32)
+    info = ctx.info()
+    sm_max = float(measured_peaks().get("sm_max_mhz", 1965.0))
+    k_ms = float(np.mean(kern_ms))
+    ach = slots * B / (k_ms * 1e-3) / 1e12
+    peak = info["n_sm"] * SM_FP32_LANES * sm_max * 1e6 / 1e12
+    line["roofline"] = {"bound": "alu", "kernel": "fused_lin_kernel", "achieved": ach, "peak": peak, "unit": "Tinst/s",
+                        "frac": ach / peak, "traffic": None, "kernel_ms": k_ms,
+                        "algorithmic_issue_slots_per_likelihood": slots,
+                        "peak_source": "as in the default mode"}
     if not args.no_cpu_baseline:
         from oracle import oracle as O
         O.lib()

@@ -409,7 +409,9 @@ int tl_loglike_linear_batch(tl_ctx *c, const float *params, int64_t B, float *lo
             a.logL = logL; a.amps = amps; a.mimg = mscr; a.rowtab = c->lin_fused_rowtab;
             int grid = c->lin_fused_grid;
             if ((int64_t)grid > nb) grid = (int)nb;
+            if (c->profile) cudaEventRecord(c->ev0, st);
             c->fused_lin<<<grid, 512, c->lin_fused_smem, st>>>(a);
+            if (c->profile) { cudaEventRecord(c->ev1, st); c->prof_pending = 1; }
             if (!cuda_ok(cudaGetLastError())) rcf = TL_ECUDA;
         }
         cudaFreeAsync(rowsf, st); cudaFreeAsync(mscr, st);
@@ -450,7 +452,9 @@ int tl_loglike_linear_batch(tl_ctx *c, const float *params, int64_t B, float *lo
         a.logL = logL; a.amps = amps; a.ext = ext; a.mimg = mimg;
         a.tile_rows = c->lin_tile_rows; a.n_tiles = c->lin_n_tiles; a.rowtab = c->lin_rowtab;
         dim3 tg((unsigned)nb, 8);
+        if (c->profile) cudaEventRecord(c->ev0, st);
         c->trace_lin<<<tg, 256, c->lin_trace_smem, st>>>(a, (int)nb);
+        if (c->profile) { cudaEventRecord(c->ev1, st); c->prof_pending = 1; }
         dim3 cg((unsigned)nb, (unsigned)c->lin_n_tiles, (unsigned)NC);
         tl::conv_lin_kernel<<<cg, 256, c->lin_conv_smem, st>>>(a, (int)nb);
         tl::solve_lin_kernel<<<(unsigned)nb, 256, 0, st>>>(a, (int)nb);
