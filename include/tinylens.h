@@ -53,6 +53,9 @@ extern "C" {
 #define TL_ECUDA   -3   /* no usable CUDA device, or a CUDA runtime call failed               */
 #define TL_ESIZE   -4   /* configuration exceeds what the kernels support (see tl_create)     */
 
+#define TL_PRECISION_FP32 0 /* default: the FP32 / MUFU kernels      */
+#define TL_PRECISION_FP64 1 /* validation mode: the same model in double precision on the device   */
+
 #define TL_EDGE_EXTEND 0 /* evaluate the analytic model on a border of h = (K-1)/2 pixels so   */
                          /* every output pixel sees its full PSF support (Eq. 3 with only the  */
                          /* kernel truncated; G10)                                   */
@@ -159,6 +162,18 @@ int tl_loglike_linear_batch(tl_ctx *ctx, const float *params, int64_t B, float *
  * and synchronises the stream before returning.
  */
 int tl_loglike_batch_host(tl_ctx *ctx, const float *params, int64_t B, float *logL, void *cuda_stream);
+
+/*
+ * tl_set_precision -- choose the arithmetic of later tl_loglike_batch / tl_render_batch /
+ * tl_loglike_batch_host calls on this context (not of tl_loglike_linear_batch).
+ *   TL_PRECISION_FP32 (default)  the FP32 kernels: meet the tolerances of DESIGN.md "Tolerances"
+ *   TL_PRECISION_FP64            the same forward model in double precision on the device, about
+ *                                ten times slower; agrees with an FP64 CPU evaluation to ~1e-9
+ *                                relative, i.e. |delta logL| <= 1e-3 also where FP32 cannot
+ *                                (rows near the best fit).  Results are still returned as float.
+ * Not thread-safe with respect to calls in flight on the same context.  TL_OK or TL_EINVAL.
+ */
+int tl_set_precision(tl_ctx *ctx, int precision);
 
 /*
  * Benchmark facility.  tl_set_profiling(ctx, 1) makes every later batch call record a pair of

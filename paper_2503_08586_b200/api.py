@@ -19,6 +19,7 @@ LIB_PATH = os.environ.get("TL_LIB") or os.path.join(_HERE, "libtinylens.so")   #
 
 TL_OK, TL_EINVAL, TL_ENOMEM, TL_ECUDA, TL_ESIZE = 0, -1, -2, -3, -4
 TL_EDGE_EXTEND, TL_EDGE_ZERO = 0, 1
+TL_PRECISION_FP32, TL_PRECISION_FP64 = 0, 1
 
 
 class TinyLensError(RuntimeError):
@@ -69,6 +70,7 @@ def load(build_if_missing: bool = True):
     L.tl_render_batch.restype = C.c_int; L.tl_render_batch.argtypes = [vp, vp, i64, vp, vp]
     L.tl_loglike_batch_host.restype = C.c_int; L.tl_loglike_batch_host.argtypes = [vp, vp, i64, vp, vp]
     L.tl_loglike_linear_batch.restype = C.c_int; L.tl_loglike_linear_batch.argtypes = [vp, vp, i64, vp, vp, vp]
+    L.tl_set_precision.restype = C.c_int; L.tl_set_precision.argtypes = [vp, C.c_int]
     L.tl_set_profiling.restype = C.c_int; L.tl_set_profiling.argtypes = [vp, C.c_int]
     L.tl_last_kernel_ms.restype = C.c_int; L.tl_last_kernel_ms.argtypes = [vp, C.POINTER(C.c_float)]
     L.tl_destroy.restype = None; L.tl_destroy.argtypes = [vp]
@@ -202,6 +204,10 @@ def tl_loglike_batch_host(handle: int, params_host, out_host=None, stream=None):
     return out_host
 
 
+def tl_set_precision(handle: int, precision: int):
+    _check(load().tl_set_precision(handle, int(precision)), "tl_set_precision")
+
+
 def tl_set_profiling(handle: int, enable: bool):
     _check(load().tl_set_profiling(handle, 1 if enable else 0), "tl_set_profiling")
 
@@ -247,6 +253,9 @@ class LensContext:
 
     def loglike_host(self, params_host, out_host=None, stream=None):
         return tl_loglike_batch_host(self.handle, params_host, out_host, stream)
+
+    def set_precision(self, precision: int):
+        tl_set_precision(self.handle, precision)
 
     def set_profiling(self, enable: bool = True):
         tl_set_profiling(self.handle, enable)

@@ -15,6 +15,7 @@
 #define TL_MAIN_TU            /* this unit owns the non-template kernels */
 #include "tl_kernels.cuh"
 #include "tl_dispatch.h"
+#include "tl_precise.cuh"
 
 #define TL_VERSION_STRING "tinylens-b200 0.1 (sm_100a)"
 
@@ -24,7 +25,8 @@ struct tl_ctx {
     int n_sm = 0;
     int P = 0, K = 0, Kp = 0, h = 0, He = 0, We = 0, pitch = 0, n_comp = 0;
     // device arrays (library-owned)
-    float *psf = nullptr, *data = nullptr, *wgt = nullptr, *sigma_min = nullptr;
+    float *psf = nullptr, *data = nullptr, *wgt = nullptr, *sigma_min = nullptr, *noise = nullptr;
+    int precision = 0;            // TL_PRECISION_FP32 / TL_PRECISION_FP64
     double *lconst = nullptr;
     double lconst0 = 0.0, sigma_min0 = 0.0;
     // launch geometry
@@ -108,6 +110,36 @@ int run_batch(tl_ctx *c, const float *params, int64_t B, float *logL, float *ima
     if (dev != c->device && !cuda_ok(cudaSetDevice(c->device))) return TL_ECUDA;
 
     const int64_t rows_per_lens = B / c->cfg.n_lens;
+    if (c->precision == TL_PRECISION_FP64) {
+        const size_t ext_row = sizeof(double) * (size_t)c->He * c->We;
+        int64_t pch = (int64_t)(EXT_SCRATCH_BYTES / ext_row);
+        if (pch < 1) pch = 1;
+        if (pch > 65535) pch = 65535;
+        if (pch > B) pch = B;
+        double *pext = nullptr;
+        if (!cuda_ok(cudaMallocAsync(&pext, ext_row * (size_t)pch, st))) return TL_ENOMEM;
+        int prc = TL_OK;
+        for (int64_t r0 = 0; r0 < B && prc == TL_OK; r0 += pch) {
+            const int64_t nb = (B - r0 < pch) ? (B - r0) : pch;
+            tl::PreciseArgs pa;
+            pa.params = params + r0 * c->P; pa.psf = c->psf; pa.data = c->data; pa.noise = c->noise;
+            pa.lconst = c->lconst; pa.ext = pext; pa.logL = logL; pa.images = images;
+            pa.row0 = r0; pa.rows_per_lens = rows_per_lens;
+            pa.P = c->P; pa.ny = c->cfg.ny; pa.nx = c->cfg.nx; pa.K = c->K; pa.Kp = c->Kp; pa.h = c->h;
+            pa.He = c->He; pa.We = c->We; pa.S = c->cfg.supersample;
+            pa.n_lens_light = c->cfg.n_lens_light; pa.n_comp = c->n_comp;
+            pa.edge_zero = c->cfg.edge_mode == TL_EDGE_ZERO; pa.pix_scale = c->cfg.pix_scale;
+            int slabs = (int)((2 * (int64_t)c->n_sm * 8 + nb - 1) / nb);          // enough CTAs for small batches
+            const int max_slabs = (c->He * c->We + 255) / 256;
+            if (slabs > max_slabs) slabs = max_slabs;
+            if (slabs < 1) slabs = 1;
+            tl::precise_trace_kernel<<<dim3((unsigned)nb, (unsigned)slabs), 256, 0, st>>>(pa);
+            tl::precise_conv_kernel<<<(unsigned)nb, 256, 0, st>>>(pa);
+            if (!cuda_ok(cudaGetLastError())) prc = TL_ECUDA;
+        }
+        cudaFreeAsync(pext, st);
+        return prc;
+    }
     const int64_t chunk = c->chunk_rows < B ? c->chunk_rows : B;
     tl::RowC *rows = nullptr;
     float *ext = nullptr;
@@ -256,12 +288,14 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
     bool ok = cuda_ok(cudaMalloc(&c->psf, psf_f.size() * sizeof(float))) &&
               cuda_ok(cudaMalloc(&c->data, npix * L * sizeof(float))) &&
               cuda_ok(cudaMalloc(&c->wgt, npix * L * sizeof(float))) &&
+              cuda_ok(cudaMalloc(&c->noise, npix * L * sizeof(float))) &&
               cuda_ok(cudaMalloc(&c->sigma_min, L * sizeof(float))) &&
               cuda_ok(cudaMalloc(&c->lconst, L * sizeof(double)));
     if (!ok) { tl_destroy(c); return TL_ENOMEM; }
     ok = cuda_ok(cudaMemcpyAsync(c->psf, psf_f.data(), psf_f.size() * sizeof(float), cudaMemcpyHostToDevice, st)) &&
          cuda_ok(cudaMemcpyAsync(c->data, data, npix * L * sizeof(float), cudaMemcpyHostToDevice, st)) &&
          cuda_ok(cudaMemcpyAsync(c->wgt, wgt.data(), npix * L * sizeof(float), cudaMemcpyHostToDevice, st)) &&
+         cuda_ok(cudaMemcpyAsync(c->noise, noise, npix * L * sizeof(float), cudaMemcpyHostToDevice, st)) &&
          cuda_ok(cudaMemcpyAsync(c->sigma_min, smin.data(), L * sizeof(float), cudaMemcpyHostToDevice, st)) &&
          cuda_ok(cudaMemcpyAsync(c->lconst, lconst.data(), L * sizeof(double), cudaMemcpyHostToDevice, st)) &&
          cuda_ok(cudaStreamSynchronize(st));
@@ -485,6 +519,13 @@ int tl_loglike_batch_host(tl_ctx *ctx, const float *params, int64_t B, float *lo
     return rc;
 }
 
+int tl_set_precision(tl_ctx *c, int precision)
+{
+    if (!c || (precision != TL_PRECISION_FP32 && precision != TL_PRECISION_FP64)) return TL_EINVAL;
+    c->precision = precision;
+    return TL_OK;
+}
+
 int tl_set_profiling(tl_ctx *c, int enable)
 {
     if (!c) return TL_EINVAL;
@@ -508,7 +549,7 @@ void tl_destroy(tl_ctx *c)
     if (!c) return;
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
-    cudaFree(c->psf); cudaFree(c->data); cudaFree(c->wgt); cudaFree(c->sigma_min); cudaFree(c->lconst);
+    cudaFree(c->psf); cudaFree(c->data); cudaFree(c->wgt); cudaFree(c->noise); cudaFree(c->sigma_min); cudaFree(c->lconst);
     delete c;
 }
 
