@@ -575,7 +575,7 @@ __global__ void __launch_bounds__(TL_LB_T, TL_LB_B) fused_kernel(const KArgs a)
 // trace_kernel: one parameter row per blockIdx.x iteration, the row's items spread over
 // gridDim.y CTAs (slabs); binned extended image -> global memory.
 template <int S_T, int NLL, int NSRC>
-__global__ void __launch_bounds__(256) trace_kernel(const KArgs a, int chunk_rows)
+__global__ void __launch_bounds__(256, 2) trace_kernel(const KArgs a, int chunk_rows)
 {
     __shared__ RowC rc_s;
     extern __shared__ __align__(16) unsigned char smem_raw[];
