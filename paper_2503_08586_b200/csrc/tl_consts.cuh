@@ -116,13 +116,17 @@ __device__ inline double sersic_bn(double n)
     for (int it = 0; it < 60; ++it) {
         const double P = gamma_p_series(a, b, &pf);
         if (P < 0.5) lo = b; else hi = b;
-        const double dPdb = pf * a / b;           // x^(a-1) e^-x / Gamma(a)
-        double nb = b - (P - 0.5) / dPdb;
+        const double f = P - 0.5;
+        const double d1 = pf * a / b;             // dP/db   = b^(a-1) e^-b / Gamma(a)
+        const double d2 = d1 * ((a - 1.0) / b - 1.0);   // d2P/db2
+        // Halley step (cubic convergence: from the 1e-5 start one evaluation reaches 1e-15)
+        const double newton = f / d1;
+        double nb = b - newton / (1.0 - 0.5 * newton * d2 / d1);
         if (!(nb > lo && nb < hi)) nb = isinf(hi) ? 2.0 * b : 0.5 * (lo + hi);
         const double step = fabs(nb - b);
         b = nb;
-        // Newton converges quadratically: a step below 1e-8 b leaves an error below 1e-15 b
-        if (step <= 1e-8 * b) break;
+        // a step below 2e-5 b leaves an error of order step^3: below 1e-14 b
+        if (step <= 2e-5 * b) break;
     }
     return b;
 }
