@@ -46,7 +46,7 @@ SM_MUFU_LANES = 16           # measured 15.96 (profiles/r1_mufu_accuracy.md)
 
 # dram bytes of the dominant kernel per launch from the committed `ncu --set full` capture
 # (profiles/): filled in by hand after each capture; None until one exists.
-NCU_DRAM_BYTES_PER_LAUNCH = 2205184       # profiles/r1_fused_kernel.md: dram__bytes_read.sum 2.205184 MB + 0 B written
+NCU_DRAM_BYTES_PER_LAUNCH = 2363136       # profiles/r1_fused_kernel.md: dram__bytes_read.sum 2.363136 MB + 0 B written
 
 
 def op_model(w: W.Workload) -> dict:
