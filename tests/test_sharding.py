@@ -39,12 +39,11 @@ def _worker(rank, world, port, n_lens, rows_per_lens, out_path):
     w = W.Workload(**{**w.__dict__, "ny": 16, "nx": 16, "psf_size": 5})
     prob = W.make_problem(w, O.render_for_workloads)
     rows = W.batch_rows(w, rows_per_lens)
-    r0, r1 = sharding.shard_bounds(len(rows), n_lens, rank, world)
-    l0, l1 = sharding.lens_bounds(n_lens, rank, world)
+    sub, my_rows = sharding.shard_problem(prob, rows, rank, world)
     ll = np.zeros(0)
-    if r1 > r0:
-        ll, _ = O.loglike_batch(O.config_of(w), prob.psf[l0:l1], prob.data[l0:l1], prob.noise[l0:l1],
-                                rows[r0:r1], n_lens=l1 - l0, threads=1)
+    if sub is not None and len(my_rows):
+        ll, _ = O.loglike_batch(O.config_of(sub.workload), sub.psf, sub.data, sub.noise,
+                                my_rows, n_lens=sub.workload.n_lens, threads=1)
     mine = torch.from_numpy(np.asarray(ll, np.float64))
     sizes = [torch.zeros(1, dtype=torch.int64) for _ in range(world)]
     dist.all_gather(sizes, torch.tensor([mine.numel()], dtype=torch.int64))
