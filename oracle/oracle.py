@@ -21,7 +21,7 @@ _LIB = os.path.join(_HERE, "liboracle.so")
 class OrcConfig(C.Structure):
     _fields_ = [("ny", C.c_int32), ("nx", C.c_int32), ("pix_scale", C.c_double),
                 ("supersample", C.c_int32), ("n_lens_light", C.c_int32),
-                ("n_source", C.c_int32), ("edge_mode", C.c_int32)]
+                ("n_source", C.c_int32), ("edge_mode", C.c_int32), ("mass_model", C.c_int32)]
 
 
 def build(force: bool = False) -> str:
@@ -46,6 +46,7 @@ def lib():
         L.orc_bn.restype = d; L.orc_bn.argtypes = [d]
         L.orc_shape.restype = None; L.orc_shape.argtypes = [d, d, dp, dp]
         L.orc_sie_deflection.restype = None; L.orc_sie_deflection.argtypes = [d] * 7 + [dp, dp]
+        L.orc_epl_deflection.restype = None; L.orc_epl_deflection.argtypes = [d] * 8 + [dp, dp]
         L.orc_shear_deflection.restype = None; L.orc_shear_deflection.argtypes = [d] * 4 + [dp, dp]
         L.orc_sersic.restype = d; L.orc_sersic.argtypes = [d] * 10
         L.orc_row_valid.restype = i32; L.orc_row_valid.argtypes = [cp, fp]
@@ -80,14 +81,15 @@ def _dp(a):
     return a.ctypes.data_as(C.POINTER(C.c_double))
 
 
-def config(ny, nx, pix_scale, supersample, n_lens_light, n_source, edge_mode=0) -> OrcConfig:
+def config(ny, nx, pix_scale, supersample, n_lens_light, n_source, edge_mode=0, mass_model=0) -> OrcConfig:
     return OrcConfig(int(ny), int(nx), float(pix_scale), int(supersample), int(n_lens_light),
-                     int(n_source), int(edge_mode))
+                     int(n_source), int(edge_mode), int(mass_model))
 
 
 def config_of(w) -> OrcConfig:
     """OrcConfig from a workloads.Workload-like record."""
-    return config(w.ny, w.nx, w.pix_scale, w.supersample, w.n_lens_light, w.n_source, w.edge_mode)
+    return config(w.ny, w.nx, w.pix_scale, w.supersample, w.n_lens_light, w.n_source, w.edge_mode,
+                  getattr(w, "mass_model", 0))
 
 
 # ---- scalar pieces (each cites the passage in tl_oracle.c) -------------------------------
@@ -109,6 +111,13 @@ def shape(e1, e2):
 def sie_deflection(theta_e, q, phi, cx, cy, x, y):
     ax, ay = C.c_double(), C.c_double()
     lib().orc_sie_deflection(float(theta_e), float(q), float(phi), float(cx), float(cy),
+                             float(x), float(y), C.byref(ax), C.byref(ay))
+    return ax.value, ay.value
+
+
+def epl_deflection(theta_e, gamma, q, phi, cx, cy, x, y):
+    ax, ay = C.c_double(), C.c_double()
+    lib().orc_epl_deflection(float(theta_e), float(gamma), float(q), float(phi), float(cx), float(cy),
                              float(x), float(y), C.byref(ax), C.byref(ay))
     return ax.value, ay.value
 

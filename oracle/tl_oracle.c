@@ -17,6 +17,7 @@
  *
  * Parameter row (float, widened exactly to double), P = 7 + 7*n_lens_light + 7*n_source:
  *   theta_E, e1, e2, cx, cy, gamma1, gamma2,
+ *   [mass_model = EPL only: the slope gamma of Eq. 12, making P one larger,]
  *   then per Sersic (lens light first, then sources): I_e, r_e, n, e1, e2, cx, cy.
  *
  * Build: gcc -O2 -fopenmp -shared -fPIC -o liboracle.so tl_oracle.c -lm   (no -ffast-math)
@@ -39,7 +40,13 @@ typedef struct {
     int32_t n_lens_light;
     int32_t n_source;
     int32_t edge_mode;
+    int32_t mass_model;      /* 0 = SIE (gamma = 2), 1 = EPL: the row carries the slope gamma at index 7 */
 } orc_config;
+
+#define ORC_MASS_SIE 0
+#define ORC_MASS_EPL 1
+/* parameters of the lens block: theta_E, e1, e2, cx, cy, gamma1, gamma2 [, gamma (EPL)] */
+static int lens_np(const orc_config *cfg) { return 7 + (cfg->mass_model == ORC_MASS_EPL ? 1 : 0); }
 
 /* ------------------------------------------------------------------ Eq. 9: b_n
  * PAPER.md:137-141 Eq. 9:  Gamma(2n) = 2 gamma(2n, b_n), i.e. P(2n, b_n) = 1/2 with P the
@@ -121,6 +128,43 @@ void orc_sie_deflection(double theta_e, double q, double phi, double cx, double 
     *ay = axp * s + ayp * c;
 }
 
+/* ------------------------------------------------------------------ Eq. 12 (general gamma): EPL
+ * PAPER.md:156-160 Eq. 12, kappa(R) = (3-gamma)/2 (theta_E/R)^(gamma-1), made elliptical as the
+ * SIE above (R -> R_p of Eq. 10; reading G19), deflection after Tessore & Metcalf
+ * (2015), which the paper cites and does not print.  With t = gamma - 1, the elliptical radius
+ * and angle  R = sqrt(q^2 x'^2 + y'^2),  R cos(phi) = q x',  R sin(phi) = y',  b = theta_E sqrt(q)
+ * (so that kappa = (2-t)/2 (b/R)^t), and f = (1-q)/(1+q), the complex deflection is
+ *   alpha_x' + i alpha_y' = 2b/(1+q) (b/R)^(t-1) Omega,
+ *   Omega = sum_{n>=0} Omega_n,  Omega_0 = e^{i phi},
+ *   Omega_n = -f (2n - (2-t)) / (2n + (2-t)) e^{2 i phi} Omega_{n-1}
+ * (their angular series of 2F1(1, t/2; 2 - t/2; -f e^{2 i phi})), summed in their order until a
+ * term falls below 1e-18 of the sum.  alpha = 0 at R = 0.  Valid for 0 < t < 2.             */
+void orc_epl_deflection(double theta_e, double gamma, double q, double phi, double cx, double cy,
+                        double x, double y, double *ax, double *ay)
+{
+    double c = cos(phi), s = sin(phi);
+    double dx = x - cx, dy = y - cy;
+    double xp = dx * c + dy * s;
+    double yp = -dx * s + dy * c;
+    double R = sqrt(q * q * xp * xp + yp * yp);
+    if (R == 0.0 || theta_e == 0.0) { *ax = 0.0; *ay = 0.0; return; }
+    double t = gamma - 1.0, b = theta_e * sqrt(q), f = (1.0 - q) / (1.0 + q);
+    double cph = q * xp / R, sph = yp / R;                    /* e^{i phi} */
+    double c2 = cph * cph - sph * sph, s2 = 2.0 * cph * sph;  /* e^{2 i phi} */
+    double on_re = cph, on_im = sph, sum_re = on_re, sum_im = on_im;
+    for (int n = 1; n < 100000; ++n) {
+        double fac = -f * (2.0 * n - (2.0 - t)) / (2.0 * n + (2.0 - t));
+        double re = fac * (c2 * on_re - s2 * on_im), im = fac * (c2 * on_im + s2 * on_re);
+        on_re = re; on_im = im;
+        sum_re += re; sum_im += im;
+        if (hypot(re, im) < 1e-18 * hypot(sum_re, sum_im)) break;
+    }
+    double pre = 2.0 * b / (1.0 + q) * pow(b / R, t - 1.0);
+    double axp = pre * sum_re, ayp = pre * sum_im;
+    *ax = axp * c - ayp * s;
+    *ay = axp * s + ayp * c;
+}
+
 /* PAPER.md:160-162 Eq. 13, :187-190 Eq. 14: psi_ext = -1/2 gamma theta^2 cos 2(phi - phi_ext)
  * = -1/2 [gamma1 (x^2 - y^2) + 2 gamma2 x y] about the image origin (G4, G5);
  * alpha = grad psi_ext.                                                                   */
@@ -143,16 +187,18 @@ double orc_sersic(double i_e, double r_e, double n, double bn, double q, double 
 
 /* ------------------------------------------------------------------ validity (boundary rule)
  * include/tinylens.h: hypot(e1,e2) >= 1, theta_E < 0, r_e <= 0, n <= 0 or any non-finite
- * value makes the row physically invalid: logL = -inf, image = NaN.                        */
+ * value makes the row physically invalid: logL = -inf, image = NaN.  EPL: also a slope outside
+ * 1 < gamma < 3, where the deflection of Eq. 12 does not exist.                             */
 int orc_row_valid(const orc_config *cfg, const float *row)
 {
     int ncomp = cfg->n_lens_light + cfg->n_source;
-    int P = 7 + 7 * ncomp;
+    int LP = lens_np(cfg), P = LP + 7 * ncomp;
     for (int i = 0; i < P; ++i) if (!isfinite((double)row[i])) return 0;
     if (row[0] < 0.0f) return 0;
     if (hypot((double)row[1], (double)row[2]) >= 1.0) return 0;
+    if (cfg->mass_model == ORC_MASS_EPL && !(row[7] > 1.0f && row[7] < 3.0f)) return 0;   /* 0 < t < 2 */
     for (int k = 0; k < ncomp; ++k) {
-        const float *s = row + 7 + 7 * k;
+        const float *s = row + LP + 7 * k;
         if (!(s[1] > 0.0f) || !(s[2] > 0.0f)) return 0;
         if (hypot((double)s[3], (double)s[4]) >= 1.0) return 0;
     }
@@ -178,10 +224,12 @@ void orc_ideal_image(const orc_config *cfg, int g, const float *row, double *img
     double theta_e = row[0], q, phi;
     orc_shape(row[1], row[2], &q, &phi);
     double lcx = row[3], lcy = row[4], g1 = row[5], g2 = row[6];
-    int ncomp = cfg->n_lens_light + cfg->n_source;
+    int ncomp = cfg->n_lens_light + cfg->n_source, LP = lens_np(cfg);
+    int epl = cfg->mass_model == ORC_MASS_EPL;
+    double slope = epl ? (double)row[7] : 2.0;
     double cq[8], cphi[8], cbn[8];
     for (int k = 0; k < ncomp && k < 8; ++k) {
-        const float *c = row + 7 + 7 * k;
+        const float *c = row + LP + 7 * k;
         orc_shape(c[3], c[4], &cq[k], &cphi[k]);
         cbn[k] = orc_bn(c[2]);
     }
@@ -195,12 +243,13 @@ void orc_ideal_image(const orc_config *cfg, int g, const float *row, double *img
                 for (int b = 0; b < S; ++b) {
                     double x = xj + ((b + 0.5) / S - 0.5) * s;
                     double ax, ay, sx, sy;
-                    orc_sie_deflection(theta_e, q, phi, lcx, lcy, x, y, &ax, &ay);
+                    if (epl) orc_epl_deflection(theta_e, slope, q, phi, lcx, lcy, x, y, &ax, &ay);
+                    else orc_sie_deflection(theta_e, q, phi, lcx, lcy, x, y, &ax, &ay);
                     orc_shear_deflection(g1, g2, x, y, &sx, &sy);
                     double bx = x - (ax + sx), by = y - (ay + sy);          /* Eq. 1 */
                     double v = 0.0;
                     for (int k = 0; k < ncomp; ++k) {
-                        const float *c = row + 7 + 7 * k;
+                        const float *c = row + LP + 7 * k;
                         int is_lens = k < cfg->n_lens_light;
                         v += orc_sersic(c[0], c[1], c[2], cbn[k], cq[k], cphi[k], c[5], c[6],
                                         is_lens ? x : bx, is_lens ? y : by);  /* Eq. 2 */
@@ -295,7 +344,7 @@ double orc_loglike(const orc_config *cfg, const float *psf, int K, const float *
 int orc_loglike_batch(const orc_config *cfg, int n_lens, const float *psf, int K, const float *data,
                       const float *noise, const float *rows, int64_t B, double *logl, int threads)
 {
-    int P = 7 + 7 * (cfg->n_lens_light + cfg->n_source);
+    int P = lens_np(cfg) + 7 * (cfg->n_lens_light + cfg->n_source);
     size_t n = (size_t)cfg->ny * cfg->nx;
     int64_t per = B / (n_lens > 0 ? n_lens : 1);
     int used = 1;
@@ -324,7 +373,7 @@ int orc_loglike_batch(const orc_config *cfg, int n_lens, const float *psf, int K
 int orc_render_batch(const orc_config *cfg, int n_lens, const float *psf, int K, const float *rows,
                      int64_t B, double *images, int threads)
 {
-    int P = 7 + 7 * (cfg->n_lens_light + cfg->n_source);
+    int P = lens_np(cfg) + 7 * (cfg->n_lens_light + cfg->n_source);
     size_t n = (size_t)cfg->ny * cfg->nx;
     int64_t per = B / (n_lens > 0 ? n_lens : 1);
     int used = 1;
@@ -362,12 +411,12 @@ int orc_render_batch(const orc_config *cfg, int n_lens, const float *psf, int K,
  */
 int orc_component_images(const orc_config *cfg, const float *psf, int K, const float *row, double *M)
 {
-    int C = cfg->n_lens_light + cfg->n_source, P = 7 + 7 * C;
+    int C = cfg->n_lens_light + cfg->n_source, LP = lens_np(cfg), P = LP + 7 * C;
     size_t n = (size_t)cfg->ny * cfg->nx;
-    float tmp[7 + 7 * 8];
+    float tmp[8 + 7 * 8];
     for (int k = 0; k < C; ++k) {
         memcpy(tmp, row, sizeof(float) * (size_t)P);
-        for (int j = 0; j < C; ++j) tmp[7 + 7 * j] = (j == k) ? 1.0f : 0.0f;     /* unit amplitude */
+        for (int j = 0; j < C; ++j) tmp[LP + 7 * j] = (j == k) ? 1.0f : 0.0f;     /* unit amplitude */
         if (!orc_render(cfg, psf, K, tmp, M + (size_t)k * n)) return 0;
     }
     return 1;
@@ -422,9 +471,9 @@ double orc_loglike_linear(const orc_config *cfg, const float *psf, int K, const 
     size_t n = (size_t)cfg->ny * cfg->nx;
     for (int k = 0; k < C; ++k) if (amps) amps[k] = NAN;
     /* the amplitudes are not parameters here: validity is judged with them set to one */
-    float tmp[7 + 7 * 8];
-    memcpy(tmp, row, sizeof(float) * (size_t)(7 + 7 * C));
-    for (int j = 0; j < C; ++j) tmp[7 + 7 * j] = 1.0f;
+    float tmp[8 + 7 * 8];
+    memcpy(tmp, row, sizeof(float) * (size_t)(lens_np(cfg) + 7 * C));
+    for (int j = 0; j < C; ++j) tmp[lens_np(cfg) + 7 * j] = 1.0f;
     if (!orc_row_valid(cfg, tmp)) return -INFINITY;
     double *M = (double *)malloc(sizeof(double) * n * (size_t)C);
     double *model = (double *)malloc(sizeof(double) * n);
@@ -455,7 +504,7 @@ double orc_loglike_linear(const orc_config *cfg, const float *psf, int K, const 
 int orc_loglike_linear_batch(const orc_config *cfg, int n_lens, const float *psf, int K, const float *data,
                              const float *noise, const float *rows, int64_t B, double *logl, double *amps, int threads)
 {
-    int C = cfg->n_lens_light + cfg->n_source, P = 7 + 7 * C;
+    int C = cfg->n_lens_light + cfg->n_source, LP = lens_np(cfg), P = LP + 7 * C;
     size_t n = (size_t)cfg->ny * cfg->nx;
     int64_t per = B / (n_lens > 0 ? n_lens : 1);
     int used = 1;

@@ -12,7 +12,7 @@ What is here:
     supersampling, PSF and noise recipes, priors)                     [DESIGN.md "Inputs"]
   * a counter-based RNG (numpy Philox) keyed by  250308586 + 1000*config + stream
   * prior draws -> parameter rows in the boundary's layout (include/tinylens.h):
-        theta_E, e1, e2, cx, cy, gamma1, gamma2,
+        theta_E, e1, e2, cx, cy, gamma1, gamma2, [slope gamma when mass_model = MASS_EPL,]
         then per Sersic (lens light first, then sources): I_e, r_e, n, e1, e2, cx, cy
     Drawn (q, phi) are encoded as (e1, e2) with the forward map of PAPER.md:152 Eq. 11.
   * PSF builders sampled at pixel centres, normalised to sum 1 (Gaussian / Moffat)
@@ -35,6 +35,7 @@ SEED_BASE = 250308586
 STREAM_TRUTH, STREAM_NOISE, STREAM_BATCH, STREAM_NEAR, STREAM_PSF = 0, 1, 2, 3, 4
 
 EDGE_EXTEND, EDGE_ZERO = 0, 1
+MASS_SIE, MASS_EPL = 0, 1
 
 
 @dataclass(frozen=True)
@@ -59,10 +60,15 @@ class Workload:
     n_lens: int = 1
     psf_fwhm_range: Optional[tuple] = None
     edge_mode: int = EDGE_EXTEND
+    mass_model: int = MASS_SIE  # MASS_EPL: the row carries the power-law slope (Eq. 12)
+
+    @property
+    def n_lens_params(self) -> int:
+        return 7 + (1 if self.mass_model == MASS_EPL else 0)
 
     @property
     def n_params(self) -> int:
-        return 7 + 7 * self.n_lens_light + 7 * self.n_source
+        return self.n_lens_params + 7 * self.n_lens_light + 7 * self.n_source
 
     @property
     def rows_per_lens(self) -> int:
@@ -76,6 +82,10 @@ class Workload:
     def samples_per_likelihood(self) -> int:
         h = self.halo if self.edge_mode == EDGE_EXTEND else 0
         return (self.ny + 2 * h) * (self.nx + 2 * h) * self.supersample ** 2
+
+    def with_epl(self) -> "Workload":
+        """Same workload with the elliptical power-law mass model (free slope)."""
+        return replace(self, mass_model=MASS_EPL)
 
     def scaled(self, batch: Optional[int] = None, n_lens: Optional[int] = None) -> "Workload":
         """Same workload with a smaller batch / fewer lenses (parity-test sizes)."""
@@ -152,6 +162,9 @@ def draw_params(w: Workload, rng: np.random.Generator, n: int) -> np.ndarray:
         sx = rng.uniform(-0.2, 0.2, n)
         sy = rng.uniform(-0.2, 0.2, n)
         cols += [amp, re, ns, s1, s2, sx, sy]
+    if w.mass_model == MASS_EPL:
+        # drawn last, so that every other parameter equals the SIE workload's draw
+        cols.insert(7, rng.uniform(1.6, 2.4, n))
     return np.ascontiguousarray(np.stack(cols, axis=1).astype(np.float32))
 
 
