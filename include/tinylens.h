@@ -29,11 +29,13 @@
  * Parameter row layout, P = 7 + 7*n_lens_light + 7*n_source floats:
  *   [0] theta_E  [1] e1  [2] e2  [3] cx  [4] cy          SIE (ellipticities: Eq. 11)
  *   [5] gamma1   [6] gamma2                               external shear
+ *   [7] gamma                                             mass_model = TL_MASS_EPL only: the slope
+ *                                                         of PAPER.md:158 Eq. 12 (then P is 8 + ...)
  *   then per Sersic component, lens light first, then sources:
  *   [+0] I_e  [+1] r_e  [+2] n  [+3] e1  [+4] e2  [+5] cx  [+6] cy
  *
- * Invalid rows are not errors: hypot(e1,e2) >= 1, theta_E < 0, r_e <= 0, n <= 0 or any
- * non-finite entry gives logL = -INFINITY and a NaN-filled image for that row.
+ * Invalid rows are not errors: hypot(e1,e2) >= 1, theta_E < 0, r_e <= 0, n <= 0, a slope outside
+ * 1 < gamma < 3, or any non-finite entry gives logL = -INFINITY and a NaN-filled image for that row.
  *
  * Threading: a context is immutable after tl_create and may be used from several host
  * threads / streams concurrently; per-call scratch comes from the stream-ordered allocator.
@@ -61,6 +63,12 @@ extern "C" {
                          /* kernel truncated; G10)                                   */
 #define TL_EDGE_ZERO   1 /* model taken as zero outside the cutout ('same' zero-padded conv)   */
 
+#define TL_MASS_SIE 0 /* singular isothermal ellipsoid: Eq. 12 with gamma = 2        */
+#define TL_MASS_EPL 1 /* elliptical power law, Eq. 12 with the slope gamma a parameter  */
+                      /* of every row: kappa = (3-gamma)/2 (theta_E/R_p)^(gamma-1) on the ellipses   */
+                      /* R_p of Eq. 10, deflection by the angular series of Tessore & Metcalf 2015   */
+                      /* (G19).  gamma = 2 reproduces TL_MASS_SIE.                          */
+
 typedef struct tl_ctx tl_ctx;     /* opaque; owned by the library */
 
 typedef struct {
@@ -73,6 +81,7 @@ typedef struct {
     int32_t n_lens;          /* 1, or L for a heterogeneous batch of L lenses (own psf, data,  */
                              /* noise per lens; row r of a B-row call belongs to lens          */
                              /* r / (B / L), B must be a multiple of L)                        */
+    int32_t mass_model;      /* TL_MASS_SIE or TL_MASS_EPL                                     */
 } tl_config;
 
 /* What a context will launch; filled by tl_get_info (for benchmarks and reports).             */
@@ -113,7 +122,8 @@ int tl_create(tl_ctx **out, const tl_config *cfg,
               const float *psf, int32_t psf_ny, int32_t psf_nx,
               const float *data, const float *noise, void *cuda_stream);
 
-/* Number of floats per parameter row, P = 7 + 7*n_lens_light + 7*n_source; < 0 on NULL.       */
+/* Number of floats per parameter row, P = 7 (8 for TL_MASS_EPL) + 7*n_lens_light + 7*n_source;
+ * < 0 on NULL.                                                                                */
 int tl_param_count(const tl_ctx *ctx);
 
 /* Launch geometry and sizes of this context.  Returns TL_OK or TL_EINVAL.                     */

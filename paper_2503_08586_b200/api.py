@@ -20,6 +20,7 @@ LIB_PATH = os.environ.get("TL_LIB") or os.path.join(_HERE, "libtinylens.so")   #
 TL_OK, TL_EINVAL, TL_ENOMEM, TL_ECUDA, TL_ESIZE = 0, -1, -2, -3, -4
 TL_EDGE_EXTEND, TL_EDGE_ZERO = 0, 1
 TL_PRECISION_FP32, TL_PRECISION_FP64 = 0, 1
+TL_MASS_SIE, TL_MASS_EPL = 0, 1
 
 
 class TinyLensError(RuntimeError):
@@ -32,7 +33,7 @@ class TinyLensError(RuntimeError):
 class tl_config(C.Structure):
     _fields_ = [("ny", C.c_int32), ("nx", C.c_int32), ("pix_scale", C.c_double),
                 ("supersample", C.c_int32), ("n_lens_light", C.c_int32), ("n_source", C.c_int32),
-                ("edge_mode", C.c_int32), ("n_lens", C.c_int32)]
+                ("edge_mode", C.c_int32), ("n_lens", C.c_int32), ("mass_model", C.c_int32)]
 
 
 class tl_info(C.Structure):
@@ -106,7 +107,7 @@ def _f32c(a) -> np.ndarray:
 
 
 def tl_create(ny, nx, pix_scale, supersample, n_lens_light, n_source, psf, data, noise,
-              edge_mode=TL_EDGE_EXTEND, n_lens=1, stream=None) -> int:
+              edge_mode=TL_EDGE_EXTEND, n_lens=1, stream=None, mass_model=TL_MASS_SIE) -> int:
     """-> opaque handle (int).  psf [n_lens,K,K], data/noise [n_lens,ny,nx]: host float32 arrays."""
     L = load()
     p, d, s = _f32c(psf), _f32c(data), _f32c(noise)
@@ -116,7 +117,7 @@ def tl_create(ny, nx, pix_scale, supersample, n_lens_light, n_source, psf, data,
     if d.size != n_lens * ny * nx or s.size != n_lens * ny * nx:
         raise TinyLensError(TL_EINVAL, "tl_create (data/noise shape)")
     cfg = tl_config(int(ny), int(nx), float(pix_scale), int(supersample), int(n_lens_light),
-                    int(n_source), int(edge_mode), int(n_lens))
+                    int(n_source), int(edge_mode), int(n_lens), int(mass_model))
     h = C.c_void_p()
     fp = C.POINTER(C.c_float)
     sh = 0
@@ -227,17 +228,19 @@ class LensContext:
     """RAII wrapper: ``ctx = LensContext.from_problem(problem); ctx.loglike(params)``."""
 
     def __init__(self, ny, nx, pix_scale, supersample, n_lens_light, n_source, psf, data, noise,
-                 edge_mode=TL_EDGE_EXTEND, n_lens=1, stream=None):
+                 edge_mode=TL_EDGE_EXTEND, n_lens=1, stream=None, mass_model=TL_MASS_SIE):
         self.ny, self.nx, self.n_lens = int(ny), int(nx), int(n_lens)
+        self.n_comp = int(n_lens_light) + int(n_source)
         self.handle = tl_create(ny, nx, pix_scale, supersample, n_lens_light, n_source, psf, data,
-                                noise, edge_mode, n_lens, stream)
+                                noise, edge_mode, n_lens, stream, mass_model)
         self.n_params = tl_param_count(self.handle)
 
     @classmethod
     def from_problem(cls, prob, stream=None):
         w = prob.workload
         return cls(w.ny, w.nx, w.pix_scale, w.supersample, w.n_lens_light, w.n_source,
-                   prob.psf, prob.data, prob.noise, w.edge_mode, w.n_lens, stream)
+                   prob.psf, prob.data, prob.noise, w.edge_mode, w.n_lens, stream,
+                   getattr(w, "mass_model", TL_MASS_SIE))
 
     def info(self) -> dict:
         return tl_get_info(self.handle)
@@ -249,7 +252,7 @@ class LensContext:
         return tl_render_batch(self.handle, params, self.ny, self.nx, out, stream)
 
     def loglike_linear(self, params, out=None, amps=None, want_amps=True, stream=None):
-        return tl_loglike_linear_batch(self.handle, params, (self.n_params - 7) // 7, out, amps, want_amps, stream)
+        return tl_loglike_linear_batch(self.handle, params, self.n_comp, out, amps, want_amps, stream)
 
     def loglike_host(self, params_host, out_host=None, stream=None):
         return tl_loglike_batch_host(self.handle, params_host, out_host, stream)

@@ -17,13 +17,13 @@
 #include "tl_dispatch.h"
 #include "tl_precise.cuh"
 
-#define TL_VERSION_STRING "tinylens-b200 0.1 (sm_100a)"
+#define TL_VERSION_STRING "tinylens-b200 0.2 (sm_100a)"
 
 struct tl_ctx {
     tl_config cfg;
     int device = 0;
     int n_sm = 0;
-    int P = 0, K = 0, Kp = 0, h = 0, He = 0, We = 0, pitch = 0, n_comp = 0;
+    int P = 0, lens_np = 7, K = 0, Kp = 0, h = 0, He = 0, We = 0, pitch = 0, n_comp = 0;
     // device arrays (library-owned)
     float *psf = nullptr, *data = nullptr, *wgt = nullptr, *sigma_min = nullptr, *noise = nullptr;
     int precision = 0;            // TL_PRECISION_FP32 / TL_PRECISION_FP64
@@ -129,6 +129,7 @@ int run_batch(tl_ctx *c, const float *params, int64_t B, float *logL, float *ima
             pa.He = c->He; pa.We = c->We; pa.S = c->cfg.supersample;
             pa.n_lens_light = c->cfg.n_lens_light; pa.n_comp = c->n_comp;
             pa.edge_zero = c->cfg.edge_mode == TL_EDGE_ZERO; pa.pix_scale = c->cfg.pix_scale;
+            pa.mass_model = c->cfg.mass_model;
             int slabs = (int)((2 * (int64_t)c->n_sm * 8 + nb - 1) / nb);          // enough CTAs for small batches
             const int max_slabs = (c->He * c->We + 255) / 256;
             if (slabs > max_slabs) slabs = max_slabs;
@@ -164,6 +165,7 @@ int run_batch(tl_ctx *c, const float *params, int64_t B, float *logL, float *ima
         pa.B = nb; pa.row0 = r0; pa.rows_per_lens = rows_per_lens;
         pa.P = c->P; pa.n_lens_light = c->cfg.n_lens_light; pa.n_source = c->cfg.n_source;
         pa.S = c->cfg.supersample;
+        pa.mass_model = c->cfg.mass_model; pa.lens_np = c->lens_np;
         pa.inv_u = 2.0 * c->cfg.supersample / c->cfg.pix_scale;
         pa.fov_half = 0.5 * c->cfg.pix_scale * (c->He > c->We ? c->He : c->We);
         pa.refine_tau = c->refine_tau;
@@ -226,6 +228,7 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
     if (cfg->n_lens_light < 0 || cfg->n_lens_light > 1 || cfg->n_source < 1 || cfg->n_source > 2) return TL_EINVAL;
     if (cfg->edge_mode != TL_EDGE_EXTEND && cfg->edge_mode != TL_EDGE_ZERO) return TL_EINVAL;
     if (cfg->n_lens < 1) return TL_EINVAL;
+    if (cfg->mass_model != TL_MASS_SIE && cfg->mass_model != TL_MASS_EPL) return TL_EINVAL;
     if (psf_ny != psf_nx || psf_ny < 1 || (psf_ny & 1) == 0) return TL_EINVAL;
     // exact sub-sample coordinates need 2 S (n + K) < 2^24
     if ((int64_t)2 * cfg->supersample * ((int64_t)(cfg->ny > cfg->nx ? cfg->ny : cfg->nx) + psf_ny) >= (1 << 24)) return TL_ESIZE;
@@ -254,7 +257,8 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
         cudaGetLastError();
     }
     c->n_comp = cfg->n_lens_light + cfg->n_source;
-    c->P = 7 + 7 * c->n_comp;
+    c->lens_np = 7 + (cfg->mass_model == TL_MASS_EPL ? 1 : 0);
+    c->P = c->lens_np + 7 * c->n_comp;
     c->K = psf_ny; c->Kp = (c->K + 3) & ~3; c->h = (c->K - 1) / 2;
     c->He = cfg->ny + 2 * c->h; c->We = cfg->nx + 2 * c->h;
     c->pitch = (c->We + 3) & ~3;
@@ -316,7 +320,8 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
         const int n_tiles_img = ((c->We + c->CW - 1) / c->CW) * ((c->He + c->CH - 1) / c->CH);
         c->threads = (fs > SMEM_LIMIT / 2 || n_tiles_img >= 300) ? 512 : 256;
         if (const char *e = std::getenv("TL_THREADS")) { const int v = std::atoi(e); if (v >= 32 && v <= 512 && v % 32 == 0) c->threads = v; }
-        c->fused = tl_fused_for(cfg->supersample, cfg->n_lens_light, cfg->n_source);
+        c->fused = cfg->mass_model == TL_MASS_EPL ? tl_fused_epl_for(cfg->supersample, cfg->n_lens_light, cfg->n_source)
+                                                  : tl_fused_for(cfg->supersample, cfg->n_lens_light, cfg->n_source);
         if (!cuda_ok(cudaFuncSetAttribute(c->fused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT))) { tl_destroy(c); return TL_ECUDA; }
         int occ = 0;
         if (!cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, c->fused, c->threads, fs)) || occ < 1) { tl_destroy(c); return TL_ECUDA; }
@@ -333,7 +338,8 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
         c->conv_smem = conv_smem_bytes(c, tr);
         if (!cuda_ok(cudaFuncSetAttribute(tl::conv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT))) { tl_destroy(c); return TL_ECUDA; }
         c->threads = 256; c->smem = c->conv_smem;
-        c->trace = tl_trace_for(cfg->supersample, cfg->n_lens_light, cfg->n_source);
+        c->trace = cfg->mass_model == TL_MASS_EPL ? tl_trace_epl_for(cfg->supersample, cfg->n_lens_light, cfg->n_source)
+                                                  : tl_trace_for(cfg->supersample, cfg->n_lens_light, cfg->n_source);
         if (rowtab_bytes <= 48 * 1024 && cfg->supersample <= 4) {   // S = 8 amortises row values over 8 samples already
             c->rowtab = 1; c->trace_smem = rowtab_bytes;
             if (!cuda_ok(cudaFuncSetAttribute(c->trace, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rowtab_bytes))) { tl_destroy(c); return TL_ECUDA; }
@@ -355,7 +361,8 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
             if (tr > cfg->ny) tr = cfg->ny;
             c->lin_tile_rows = tr; c->lin_n_tiles = (cfg->ny + tr - 1) / tr;
             c->lin_conv_smem = sizeof(float) * ((size_t)c->K * c->Kp + (size_t)(tr + 2 * c->h + 1) * c->pitch + c->Kp + 8);
-            c->trace_lin = tl_trace_lin_for(cfg->supersample, cfg->n_lens_light, cfg->n_source);
+            c->trace_lin = cfg->mass_model == TL_MASS_EPL ? tl_trace_lin_epl_for(cfg->supersample, cfg->n_lens_light, cfg->n_source)
+                                                          : tl_trace_lin_for(cfg->supersample, cfg->n_lens_light, cfg->n_source);
             bool okl = cuda_ok(cudaFuncSetAttribute(tl::conv_lin_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT));
             if (rowtab_bytes <= 48 * 1024) {
                 c->lin_rowtab = 1; c->lin_trace_smem = rowtab_bytes;
@@ -369,7 +376,8 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
         int rt = 0;
         if (fl + rowtab_bytes <= SMEM_LIMIT) { fl += rowtab_bytes; rt = 1; }
         if (fl <= SMEM_LIMIT) {
-            fused_fn fn = tl_fused_lin_for(cfg->supersample, cfg->n_lens_light, cfg->n_source);
+            fused_fn fn = cfg->mass_model == TL_MASS_EPL ? tl_fused_lin_epl_for(cfg->supersample, cfg->n_lens_light, cfg->n_source)
+                                                         : tl_fused_lin_for(cfg->supersample, cfg->n_lens_light, cfg->n_source);
             int occ = 0;
             if (cuda_ok(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT)) &&
                 cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, 512, fl)) && occ >= 1) {
@@ -435,6 +443,7 @@ int tl_loglike_linear_batch(tl_ctx *c, const float *params, int64_t B, float *lo
             pa.B = nb; pa.row0 = r0; pa.rows_per_lens = rpl;
             pa.P = c->P; pa.n_lens_light = c->cfg.n_lens_light; pa.n_source = c->cfg.n_source;
             pa.S = c->cfg.supersample;
+            pa.mass_model = c->cfg.mass_model; pa.lens_np = c->lens_np;
             pa.inv_u = 2.0 * c->cfg.supersample / c->cfg.pix_scale;
             pa.fov_half = 0.5 * c->cfg.pix_scale * (c->He > c->We ? c->He : c->We);
             pa.refine_tau = c->refine_tau;
@@ -478,6 +487,7 @@ int tl_loglike_linear_batch(tl_ctx *c, const float *params, int64_t B, float *lo
         pa.B = nb; pa.row0 = r0; pa.rows_per_lens = rows_per_lens;
         pa.P = c->P; pa.n_lens_light = c->cfg.n_lens_light; pa.n_source = c->cfg.n_source;
         pa.S = c->cfg.supersample;
+        pa.mass_model = c->cfg.mass_model; pa.lens_np = c->lens_np;
         pa.inv_u = 2.0 * c->cfg.supersample / c->cfg.pix_scale;
         pa.fov_half = 0.5 * c->cfg.pix_scale * (c->He > c->We ? c->He : c->We);
         pa.refine_tau = c->refine_tau;

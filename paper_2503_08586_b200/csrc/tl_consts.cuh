@@ -27,6 +27,8 @@
 namespace tl {
 
 constexpr int MAX_COMP = 3;          // n_lens_light (<= 1) + n_source (<= 2)
+constexpr int MASS_SIE = 0, MASS_EPL = 1;          // tl_config.mass_model
+constexpr int EPL_TERMS = 24;        // angular-series terms of the FP32 EPL path (rows needing more: FP64)
 
 struct LensC {                       // SIE + external shear
     float cXa, cYa;                  // centre rounded to 2^-8 u-units: X - cXa is exact
@@ -44,9 +46,18 @@ struct LensC {                       // SIE + external shear
     float fh, fl;                    // f = theta_E sqrt(q) / q', u-units
     float ft0h, ft0l;                // f theta0
     float fT2h, fT2l;                // f T0
-    int32_t mode;                    // 0: polynomial path (q >= 0.5), 1: libdevice path
+    int32_t mode;                    // SIE  0: polynomial path (q >= 0.5), 1: libdevice path
+                                     // EPL  2: FP32 series (<= EPL_TERMS terms), 3: FP64 series
     int32_t valid;
     double dcX, dcY, dc, ds, dq2, dqp, df, dg1, dg2;   // FP64 copies for the selective refinement
+    // ---- elliptical power law (mass_model = MASS_EPL only; tl_sample.cuh "EPL") ----
+    double dt, dA, dq, dfe;          // t = gamma - 1;  alpha_u = A R_u^(1-t) Omega;  q;  f = (1-q)/(1+q)
+    float eqh, eql;                  // q
+    float ekh, ekl;                  // kappa = (1 - t) / 2
+    float ea0h, ea0l;                // alpha at R = b:  2 b_u / (1 + q)
+    float einvb2;                    // 1 / b_u^2,  b = theta_E sqrt(q)
+    int32_t enterm;                  // N: Omega = e^{i phi} (1 + sum_{n=1..N} a_n e^{2 i n phi})
+    float ecoef[EPL_TERMS];          // a_n = prod_{k<=n} -f (2k - (2-t)) / (2k + (2-t)),  ecoef[n-1] = a_n
 };
 
 struct SersicC {                     // one elliptical Sersic component
@@ -77,6 +88,7 @@ struct PrologueArgs {
     int64_t row0;                    // global index of the chunk's first row
     int64_t rows_per_lens;
     int P, n_lens_light, n_source, S;
+    int mass_model, lens_np;         // MASS_SIE / MASS_EPL; floats of the lens block (7, or 8 with the slope)
     double inv_u;                    // 2 S / pix_scale   (u-units per arcsec)
     double fov_half;                 // arcsec, half the extended field of view
     double refine_tau;               // refinement threshold in units of sigma_min
@@ -161,11 +173,14 @@ __global__ void __launch_bounds__(128) prologue_kernel(PrologueArgs a)
     RowC *rc = a.rows + row;
 
     // lens shape is needed by every slot (sources live in the lens frame)
+    const int LP = a.lens_np;
     bool lens_ok = true;
-    for (int i = 0; i < 7; ++i) lens_ok = lens_ok && isfinite(p[i]);
+    for (int i = 0; i < LP; ++i) lens_ok = lens_ok && isfinite(p[i]);
     double thE = p[0], q = 1.0, c = 1.0, s = 0.0;
     lens_ok = lens_ok && (thE >= 0.0);
     lens_ok = lens_ok && shape_from_e(p[1], p[2], &q, &c, &s);
+    // EPL: Eq. 12 has a deflection for 1 < gamma < 3 only
+    if (a.mass_model == MASS_EPL) lens_ok = lens_ok && (p[7] > 1.f) && (p[7] < 3.f);
     if (!lens_ok) { thE = 0.0; q = 1.0; c = 1.0; s = 0.0; }
 
     if (slot == 0) {
@@ -181,7 +196,7 @@ __global__ void __launch_bounds__(128) prologue_kernel(PrologueArgs a)
         double n21 = -s * (1.0 + g1) + c * g2, n22 = -s * g2 + c * (1.0 - g1);
         // D0 = N c - R^T s_1: the first source's centre is folded into the linear map, so
         // (U + V, U2 + V2) - alpha' is directly the lens-frame offset R^T (beta - s_1)
-        const float *s1 = p + 7 + 7 * a.n_lens_light;
+        const float *s1 = p + LP + 7 * a.n_lens_light;
         const bool s1ok = isfinite(s1[5]) && isfinite(s1[6]);
         double s1X = (s1ok ? (double)s1[5] : 0.0) * a.inv_u, s1Y = (s1ok ? (double)s1[6] : 0.0) * a.inv_u;
         double d1 = n11 * cX + n12 * cY - (c * s1X + s * s1Y), d2 = n21 * cX + n22 * cY - (-s * s1X + c * s1Y);
@@ -213,13 +228,39 @@ __global__ void __launch_bounds__(128) prologue_kernel(PrologueArgs a)
         L.valid = lens_ok ? 1 : 0;
         L.dcX = cX; L.dcY = cY; L.dc = c; L.ds = s; L.dq2 = q * q; L.dqp = qp; L.df = f;
         L.dg1 = g1; L.dg2 = g2;
+        // ---- EPL (Eq. 12; Tessore & Metcalf 2015 angular series, G19)
+        L.dt = 1.0; L.dA = 0.0; L.dq = q; L.dfe = (1.0 - q) / (1.0 + q);
+        L.eqh = L.eql = L.ekh = L.ekl = L.ea0h = L.ea0l = 0.f; L.einvb2 = 1.f; L.enterm = 1;
+        for (int n = 0; n < EPL_TERMS; ++n) L.ecoef[n] = 0.f;
+        if (a.mass_model == MASS_EPL) {
+            const double t = lens_ok ? (double)p[7] - 1.0 : 1.0;
+            const double bu = thE * sqrt(q) * a.inv_u;                   // b = theta_E sqrt(q), u-units
+            L.dt = t;
+            L.dA = bu > 0.0 ? 2.0 * pow(bu, t) / (1.0 + q) : 0.0;
+            split2(q, &L.eqh, &L.eql);
+            split2(0.5 * (1.0 - t), &L.ekh, &L.ekl);
+            split2(bu > 1e-18 ? 2.0 * bu / (1.0 + q) : 0.0, &L.ea0h, &L.ea0l);
+            L.einvb2 = bu > 1e-18 ? (float)(1.0 / (bu * bu)) : 1.f;
+            // a_n and the number of terms that leaves a remainder below 2e-8 (|Omega| ~ 1)
+            const double fe = L.dfe, s2t = 2.0 - t;
+            double an = 1.0;
+            int N = 0;
+            for (int n = 1; n <= EPL_TERMS + 1; ++n) {
+                an *= -fe * (2.0 * n - s2t) / (2.0 * n + s2t);
+                if (fabs(an) < 2e-8 * (1.0 - fe)) { N = n - 1; break; }
+                if (n <= EPL_TERMS) L.ecoef[n - 1] = (float)an;
+                N = n;
+            }
+            L.mode = (N <= EPL_TERMS) ? 2 : 3;
+            L.enterm = N < 1 ? 1 : (N > EPL_TERMS ? EPL_TERMS : N);
+        }
         rc->lens = L;
         return;
     }
 
     const int k = slot - 1;
     const bool is_lens_light = k < a.n_lens_light;
-    const float *sp = p + 7 + 7 * k;
+    const float *sp = p + LP + 7 * k;
     SersicC C;
     bool ok = true;
     for (int i = a.unit_amp ? 1 : 0; i < 7; ++i) ok = ok && isfinite(sp[i]);
@@ -242,7 +283,7 @@ __global__ void __launch_bounds__(128) prologue_kernel(PrologueArgs a)
     else {                                                                      // lens frame
         cd = cs * c + ss * s; sd = ss * c - cs * s;                             // cos, sin(phi_s - phi)
         // R^T (s_k - s_1): offsets are measured from the first source (folded into D0)
-        const float *s1 = p + 7 + 7 * a.n_lens_light;
+        const float *s1 = p + LP + 7 * a.n_lens_light;
         const bool s1ok = isfinite(s1[5]) && isfinite(s1[6]);
         const double rX = cX - (s1ok ? (double)s1[5] : 0.0) * a.inv_u, rY = cY - (s1ok ? (double)s1[6] : 0.0) * a.inv_u;
         oX = c * rX + s * rY; oY = -s * rX + c * rY;

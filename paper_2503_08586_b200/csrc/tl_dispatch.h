@@ -1,5 +1,5 @@
-// tl_dispatch.h -- kernel tables.  The template kernels are instantiated in three translation
-// units of their own (tl_inst_fused.cu, tl_inst_split.cu, tl_inst_lin.cu) so that nvcc can compile
+// tl_dispatch.h -- kernel tables.  The template kernels are instantiated in translation units of
+// their own (tl_inst_fused.cu, tl_inst_split.cu, tl_inst_lin.cu; tl_inst_epl.cu, tl_inst_epl_lin.cu) so that nvcc can compile
 // them in parallel; tinylens.cu only asks for the function pointer that matches a context.
 #pragma once
 #include "tl_kernels.cuh"
@@ -11,3 +11,8 @@ fused_fn tl_fused_for(int S, int n_lens_light, int n_source);          // fused_
 trace_fn tl_trace_for(int S, int n_lens_light, int n_source);          // trace_kernel<S, NLL, NSRC>
 fused_fn tl_fused_lin_for(int S, int n_lens_light, int n_source);      // fused_lin_kernel<...>
 trace_fn tl_trace_lin_for(int S, int n_lens_light, int n_source);      // trace_lin_kernel<...>
+// mass_model = MASS_EPL (compile time: S = 4 unrolled, any other S through the generic loop)
+fused_fn tl_fused_epl_for(int S, int n_lens_light, int n_source);
+trace_fn tl_trace_epl_for(int S, int n_lens_light, int n_source);
+fused_fn tl_fused_lin_epl_for(int S, int n_lens_light, int n_source);
+trace_fn tl_trace_lin_epl_for(int S, int n_lens_light, int n_source);

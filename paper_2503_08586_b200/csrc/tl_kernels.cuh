@@ -12,6 +12,7 @@
 // The split path (large images) runs phase 1 into global memory (trace_kernel) and phases
 // 2-3 from shared-memory tiles of it (conv_kernel + finalize_kernel).
 #pragma once
+#include <type_traits>
 #include "tl_sample.cuh"
 
 namespace tl {
@@ -91,9 +92,9 @@ __device__ __forceinline__ RowV row_values(const RowC &rc, float Y)
 }
 
 // Register-resident constants of one row for the sample loop.
-template <int NLL, int NSRC>
+template <int NLL, int NSRC, int MASS = MASS_SIE>
 struct HotC {
-    SieHot sie;
+    typename std::conditional<MASS == MASS_EPL, EplHot, SieHot>::type sie;
     SersicHot ll;                 // lens light (NLL = 1)
     SersicHot src[NSRC];
     QuadHot q[NSRC];
@@ -107,17 +108,22 @@ struct HotC {
 
 // One sub-sample (steps a2-a4, Eq. 2): lens light at theta (added to `acc`) and
 // sources at beta (returned), both already scaled by 1/S^2 so that the caller only adds
-// (step a5, bin = mean).  FAST = polynomial SIE path (q >= 0.5).
-template <int NLL, int NSRC, bool FAST>
-__device__ __forceinline__ void sample_value(const RowC &rc, const HotC<NLL, NSRC> &h, const ColV &c, const RowV &r,
+// (step a5, bin = mean).  FAST = polynomial SIE path (q >= 0.5) / FP32 EPL series.
+template <int NLL, int NSRC, bool FAST, int MASS>
+__device__ __forceinline__ void sample_value(const RowC &rc, const HotC<NLL, NSRC, MASS> &h, const ColV &c, const RowV &r,
                                              float &acc, float (&src)[NSRC], bool &flag)
 {
     bool fl;
     if (NLL) acc = fmaf(h.ll.amp, sersic_from_t(h.ll, fmaf(c.LB, r.dyl, c.LA + r.LC), fl), acc);
     const float xp = c.Pc + r.Qs, yp = r.Qc - c.Ps;
     float axp, ayp;
-    if (FAST) sie_alpha(h.sie, xp, yp, axp, ayp);
-    else sie_alpha_slow(rc.lens, xp, yp, axp, ayp);
+    if constexpr (MASS == MASS_EPL) {
+        if (FAST) epl_alpha(h.sie, rc.lens.ecoef, xp, yp, axp, ayp);
+        else epl_alpha_slow(rc.lens, xp, yp, axp, ayp);
+    } else {
+        if (FAST) sie_alpha(h.sie, xp, yp, axp, ayp);
+        else sie_alpha_slow(rc.lens, xp, yp, axp, ayp);
+    }
     const float bx = (c.U + r.V) - axp, by = (c.U2 + r.V2) - ayp;      // R^T (beta - s_1)
     src[0] = h.src[0].amp * sersic_from_t(h.src[0], quad_form(h.q[0], bx, by), fl);
     flag = fl;
@@ -140,8 +146,8 @@ __device__ __forceinline__ void sample_value(const RowC &rc, const HotC<NLL, NSR
 // per sub-row instead of two LDS.128).
 // LIN (linear-amplitude mode): the components are kept apart and handed to store(i, j, k, v),
 // k = 0 .. NLL + NSRC - 1; otherwise their sum goes to store(i, j, v).
-template <int S_T, int NLL, int NSRC, bool FAST, bool LIN, class Next, class Store>
-__device__ __forceinline__ void trace_tiles(const RowC &rc, const HotC<NLL, NSRC> &h, const KArgs &a,
+template <int S_T, int NLL, int NSRC, bool FAST, bool LIN, int MASS, class Next, class Store>
+__device__ __forceinline__ void trace_tiles(const RowC &rc, const HotC<NLL, NSRC, MASS> &h, const KArgs &a,
                                             const RowV *rowtab, Next next, Store store)
 {
     const int S = S_T > 0 ? S_T : a.S;
@@ -179,7 +185,7 @@ __device__ __forceinline__ void trace_tiles(const RowC &rc, const HotC<NLL, NSRC
 #pragma unroll
                         for (int sb = 0; sb < S_T; ++sb) {
                             bool fl;
-                            sample_value<NLL, NSRC, FAST>(rc, h, cv[sb], rv, acc, src[sb], fl);
+                            sample_value<NLL, NSRC, FAST, MASS>(rc, h, cv[sb], rv, acc, src[sb], fl);
                             any = any || fl;
                             if (fl) src[sb][0] = __int_as_float(0x7fc00000);      // NaN marks "refine me"
                         }
@@ -190,9 +196,9 @@ __device__ __forceinline__ void trace_tiles(const RowC &rc, const HotC<NLL, NSRC
                                     if (LIN && NSRC > 1) {
 #pragma unroll
                                         for (int k = 0; k < NSRC; ++k)
-                                            src[sb][k] = refined_source_light_k(rc, NLL + k, X0 + (float)(2 * sb), Y);
+                                            src[sb][k] = refined_source_light_k<MASS>(rc, NLL + k, X0 + (float)(2 * sb), Y);
                                     } else {
-                                        src[sb][0] = refined_source_light(rc, NLL, NLL + NSRC, X0 + (float)(2 * sb), Y);
+                                        src[sb][0] = refined_source_light<MASS>(rc, NLL, NLL + NSRC, X0 + (float)(2 * sb), Y);
                                         if (NSRC > 1) src[sb][NSRC - 1] = 0.f;
                                     }
                                 }
@@ -212,10 +218,10 @@ __device__ __forceinline__ void trace_tiles(const RowC &rc, const HotC<NLL, NSRC
                             const float X = X0 + (float)(2 * sb);
                             bool fl;
                             float sv[NSRC];
-                            sample_value<NLL, NSRC, FAST>(rc, h, col_values<NLL>(rc, X), rv, acc, sv, fl);
+                            sample_value<NLL, NSRC, FAST, MASS>(rc, h, col_values<NLL>(rc, X), rv, acc, sv, fl);
                             if (fl) {
 #pragma unroll
-                                for (int k = 0; k < NSRC; ++k) sv[k] = refined_source_light_k(rc, NLL + k, X, Y);
+                                for (int k = 0; k < NSRC; ++k) sv[k] = refined_source_light_k<MASS>(rc, NLL + k, X, Y);
                             }
                             if (LIN) {
 #pragma unroll
@@ -268,12 +274,12 @@ __device__ __forceinline__ void fill_rowtab(const RowC &rc, const KArgs &a, RowV
 // CTA draw tiles from a shared-memory counter, so they all reach the barrier that ends the
 // phase within one tile of each other whatever the refinement branches cost; the value of a
 // pixel does not depend on which warp computes it, so logL stays bitwise reproducible.
-template <int S_T, int NLL, int NSRC, class Store>
+template <int S_T, int NLL, int NSRC, int MASS, class Store>
 __device__ __forceinline__ void trace_image_lin(const RowC &rc, const KArgs &a, const RowV *rowtab, int warp, int n_warps, int *counter, Store store)
 {
     const int n = a.tiles_x * a.tiles_y;
-    const HotC<NLL, NSRC> h(rc);
-    const bool fast = rc.lens.mode == 0;
+    const HotC<NLL, NSRC, MASS> h(rc);
+    const bool fast = rc.lens.mode == (MASS == MASS_EPL ? 2 : 0);
     if (counter) {
         auto next = [&]() -> int {
             int t = 0;
@@ -281,23 +287,23 @@ __device__ __forceinline__ void trace_image_lin(const RowC &rc, const KArgs &a, 
             t = __shfl_sync(0xffffffffu, t, 0);
             return t < n ? t : -1;
         };
-        if (fast) trace_tiles<S_T, NLL, NSRC, true, true>(rc, h, a, rowtab, next, store);
-        else trace_tiles<S_T, NLL, NSRC, false, true>(rc, h, a, rowtab, next, store);
+        if (fast) trace_tiles<S_T, NLL, NSRC, true, true, MASS>(rc, h, a, rowtab, next, store);
+        else trace_tiles<S_T, NLL, NSRC, false, true, MASS>(rc, h, a, rowtab, next, store);
     } else {
         int t = (int)((long long)n * warp / n_warps);
         const int t_end = (int)((long long)n * (warp + 1) / n_warps);
         auto next = [&]() -> int { return t < t_end ? t++ : -1; };
-        if (fast) trace_tiles<S_T, NLL, NSRC, true, true>(rc, h, a, rowtab, next, store);
-        else trace_tiles<S_T, NLL, NSRC, false, true>(rc, h, a, rowtab, next, store);
+        if (fast) trace_tiles<S_T, NLL, NSRC, true, true, MASS>(rc, h, a, rowtab, next, store);
+        else trace_tiles<S_T, NLL, NSRC, false, true, MASS>(rc, h, a, rowtab, next, store);
     }
 }
 
-template <int S_T, int NLL, int NSRC, class Store>
+template <int S_T, int NLL, int NSRC, int MASS, class Store>
 __device__ __forceinline__ void trace_image(const RowC &rc, const KArgs &a, const RowV *rowtab, int warp, int n_warps, int *counter, Store store)
 {
     const int n = a.tiles_x * a.tiles_y;
-    const HotC<NLL, NSRC> h(rc);
-    const bool fast = rc.lens.mode == 0;               // uniform over the CTA
+    const HotC<NLL, NSRC, MASS> h(rc);
+    const bool fast = rc.lens.mode == (MASS == MASS_EPL ? 2 : 0);      // uniform over the CTA
     if (counter) {
         auto next = [&]() -> int {
             int t = 0;
@@ -305,14 +311,14 @@ __device__ __forceinline__ void trace_image(const RowC &rc, const KArgs &a, cons
             t = __shfl_sync(0xffffffffu, t, 0);
             return t < n ? t : -1;
         };
-        if (fast) trace_tiles<S_T, NLL, NSRC, true, false>(rc, h, a, rowtab, next, store);
-        else trace_tiles<S_T, NLL, NSRC, false, false>(rc, h, a, rowtab, next, store);
+        if (fast) trace_tiles<S_T, NLL, NSRC, true, false, MASS>(rc, h, a, rowtab, next, store);
+        else trace_tiles<S_T, NLL, NSRC, false, false, MASS>(rc, h, a, rowtab, next, store);
     } else {
         int t = (int)((long long)n * warp / n_warps);
         const int t_end = (int)((long long)n * (warp + 1) / n_warps);
         auto next = [&]() -> int { return t < t_end ? t++ : -1; };
-        if (fast) trace_tiles<S_T, NLL, NSRC, true, false>(rc, h, a, rowtab, next, store);
-        else trace_tiles<S_T, NLL, NSRC, false, false>(rc, h, a, rowtab, next, store);
+        if (fast) trace_tiles<S_T, NLL, NSRC, true, false, MASS>(rc, h, a, rowtab, next, store);
+        else trace_tiles<S_T, NLL, NSRC, false, false, MASS>(rc, h, a, rowtab, next, store);
     }
 }
 
@@ -522,7 +528,7 @@ __device__ __forceinline__ double conv_chi2_rows(const KArgs &a, const float *im
 #define TL_LB_T 512
 #define TL_LB_B 1
 #endif
-template <int S_T, int NLL, int NSRC>
+template <int S_T, int NLL, int NSRC, int MASS = MASS_SIE>
 __global__ void __launch_bounds__(TL_LB_T, TL_LB_B) fused_kernel(const KArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -555,7 +561,7 @@ __global__ void __launch_bounds__(TL_LB_T, TL_LB_B) fused_kernel(const KArgs a)
         }
         // phase 1: ray-trace + light + bin into shared memory
         if (rowtab) { fill_rowtab<NLL>(*rc, a, rowtab); __syncthreads(); }
-        trace_image<S_T, NLL, NSRC>(*rc, a, rowtab, threadIdx.x >> 5, blockDim.x >> 5, tile_counter,
+        trace_image<S_T, NLL, NSRC, MASS>(*rc, a, rowtab, threadIdx.x >> 5, blockDim.x >> 5, tile_counter,
                                     [&](int i, int j, float v) { img[i * a.pitch + j] = v; });
         __syncthreads();
         // phase 2: PSF convolution from shared memory + chi^2
@@ -574,7 +580,7 @@ __global__ void __launch_bounds__(TL_LB_T, TL_LB_B) fused_kernel(const KArgs a)
 // ------------------------------------------------------------------------------ split path
 // trace_kernel: one parameter row per blockIdx.x iteration, the row's items spread over
 // gridDim.y CTAs (slabs); binned extended image -> global memory.
-template <int S_T, int NLL, int NSRC>
+template <int S_T, int NLL, int NSRC, int MASS = MASS_SIE>
 __global__ void __launch_bounds__(256, 2) trace_kernel(const KArgs a, int chunk_rows)
 {
     __shared__ RowC rc_s;
@@ -587,7 +593,7 @@ __global__ void __launch_bounds__(256, 2) trace_kernel(const KArgs a, int chunk_
         if (!row_is_valid(rc_s, a.n_comp)) continue;
         if (rowtab) { fill_rowtab<NLL>(rc_s, a, rowtab); __syncthreads(); }
         float *dst = a.ext + (size_t)r * a.He * a.pitch;
-        trace_image<S_T, NLL, NSRC>(rc_s, a, rowtab, (blockIdx.y * blockDim.x + threadIdx.x) >> 5, (gridDim.y * blockDim.x) >> 5, nullptr,
+        trace_image<S_T, NLL, NSRC, MASS>(rc_s, a, rowtab, (blockIdx.y * blockDim.x + threadIdx.x) >> 5, (gridDim.y * blockDim.x) >> 5, nullptr,
                                     [&](int i, int j, float v) { dst[i * a.pitch + j] = v; });
     }
 }
@@ -650,7 +656,7 @@ __global__ void finalize_kernel(const KArgs a, int chunk_rows)
 
 // ------------------------------------------------------------------------------ linear mode
 // (NEXT-1, Eq. 6-7)  trace_lin_kernel -> conv_lin_kernel -> solve_lin_kernel.
-template <int S_T, int NLL, int NSRC>
+template <int S_T, int NLL, int NSRC, int MASS = MASS_SIE>
 __global__ void __launch_bounds__(256, 2) trace_lin_kernel(const KArgs a, int chunk_rows)
 {
     __shared__ RowC rc_s;
@@ -665,7 +671,7 @@ __global__ void __launch_bounds__(256, 2) trace_lin_kernel(const KArgs a, int ch
         if (rowtab) { fill_rowtab<NLL>(rc_s, a, rowtab); __syncthreads(); }
         float *dst = a.ext + (size_t)r * NC * a.He * a.pitch;
         const size_t comp_stride = (size_t)a.He * a.pitch;
-        trace_image_lin<S_T, NLL, NSRC>(rc_s, a, rowtab, (blockIdx.y * blockDim.x + threadIdx.x) >> 5, (gridDim.y * blockDim.x) >> 5, nullptr,
+        trace_image_lin<S_T, NLL, NSRC, MASS>(rc_s, a, rowtab, (blockIdx.y * blockDim.x + threadIdx.x) >> 5, (gridDim.y * blockDim.x) >> 5, nullptr,
                                       [&](int i, int j, int k, float v) { dst[k * comp_stride + i * a.pitch + j] = v; });
     }
 }
@@ -799,7 +805,7 @@ __global__ void __launch_bounds__(256) solve_lin_kernel(const KArgs a, int chunk
 // fused pipeline (when the C binned component images fit in shared memory): persistent CTAs,
 // per row  trace (components apart, dynamic tile queue) -> C convolutions from shared memory,
 // blurred columns of M to a per-CTA global scratch (L2-resident) -> solve_row.
-template <int S_T, int NLL, int NSRC>
+template <int S_T, int NLL, int NSRC, int MASS = MASS_SIE>
 __global__ void __launch_bounds__(512, 1) fused_lin_kernel(const KArgs a)
 {
     constexpr int NC = NLL + NSRC;
@@ -827,7 +833,7 @@ __global__ void __launch_bounds__(512, 1) fused_lin_kernel(const KArgs a)
         __syncthreads();
         if (!row_is_valid(*rc, a.n_comp)) { invalid_row_lin(a, row); continue; }
         if (rowtab) { fill_rowtab<NLL>(*rc, a, rowtab); __syncthreads(); }
-        trace_image_lin<S_T, NLL, NSRC>(*rc, a, rowtab, threadIdx.x >> 5, blockDim.x >> 5, tile_counter,
+        trace_image_lin<S_T, NLL, NSRC, MASS>(*rc, a, rowtab, threadIdx.x >> 5, blockDim.x >> 5, tile_counter,
                                         [&](int i, int j, int k, float v) { img[k * img_stride + i * a.pitch + j] = v; });
         __syncthreads();
 #pragma unroll 1

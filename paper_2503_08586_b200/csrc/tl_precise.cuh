@@ -17,23 +17,33 @@ namespace tl {
 struct PreciseComp { double amp, inv_re, inv_n, bn, q, c, s, cx, cy; };
 struct PreciseRow {
     double thE_sq, q, qp, c, s, cx, cy, g1, g2;        // thE_sq = theta_E sqrt(q)
+    double t, A, fe;                                   // EPL: t = gamma - 1, alpha = A R^(1-t) Omega, f = (1-q)/(1+q)
     PreciseComp comp[MAX_COMP];
-    int valid;
+    int valid, epl;
 };
 
 // per row: shapes, b_n (arcsec units throughout)
-__device__ inline void precise_row_setup(const float *p, int n_lens_light, int n_source, PreciseRow *R)
+__device__ inline void precise_row_setup(const float *p, int n_lens_light, int n_source, int mass_model, PreciseRow *R)
 {
     const int nc = n_lens_light + n_source;
+    const int LP = 7 + (mass_model == MASS_EPL ? 1 : 0);
     bool ok = true;
-    for (int i = 0; i < 7 + 7 * nc; ++i) ok = ok && isfinite(p[i]);
+    for (int i = 0; i < LP + 7 * nc; ++i) ok = ok && isfinite(p[i]);
     double q = 1.0, c = 1.0, s = 0.0;
     ok = ok && (p[0] >= 0.f) && shape_from_e(p[1], p[2], &q, &c, &s);
     R->q = q; R->qp = sqrt((1.0 - q) * (1.0 + q)); R->c = c; R->s = s;
     R->thE_sq = (double)p[0] * sqrt(q);
     R->cx = p[3]; R->cy = p[4]; R->g1 = p[5]; R->g2 = p[6];
+    R->epl = mass_model == MASS_EPL; R->t = 1.0; R->A = 0.0; R->fe = (1.0 - q) / (1.0 + q);
+    if (R->epl) {
+        ok = ok && (p[7] > 1.f) && (p[7] < 3.f);
+        if (ok) {
+            R->t = (double)p[7] - 1.0;
+            R->A = R->thE_sq > 0.0 ? 2.0 * pow(R->thE_sq, R->t) / (1.0 + q) : 0.0;
+        }
+    }
     for (int k = 0; k < nc; ++k) {
-        const float *sp = p + 7 + 7 * k;
+        const float *sp = p + LP + 7 * k;
         PreciseComp &C = R->comp[k];
         double qs = 1.0, cs = 1.0, ss = 0.0;
         bool okc = (sp[1] > 0.f) && (sp[2] > 0.f) && shape_from_e(sp[3], sp[4], &qs, &cs, &ss);
@@ -61,7 +71,9 @@ __device__ inline double precise_sample(const PreciseRow &R, int n_lens_light, i
     const double xp = dx * R.c + dy * R.s, yp = dy * R.c - dx * R.s;
     const double psi = sqrt(R.q * R.q * xp * xp + yp * yp);
     double axp = 0.0, ayp = 0.0;
-    if (psi > 0.0) {
+    if (R.epl) {
+        epl_alpha_f64(R.t, R.A, R.q, R.fe, xp, yp, axp, ayp);
+    } else if (psi > 0.0) {
         // A(z) = atan(z)/z, H(z) = atanh(z)/z -> 1 as z -> 0 keeps q = 1 exact (G6)
         const double zx = R.qp * xp / psi, zy = R.qp * yp / psi;
         const double A = fabs(zx) < 1e-4 ? 1.0 - zx * zx / 3.0 : atan(zx) / zx;
@@ -84,7 +96,7 @@ struct PreciseArgs {
     double *ext;              // [chunk][He][We] binned extended image, FP64
     float *logL, *images;
     int64_t row0, rows_per_lens;
-    int P, ny, nx, K, Kp, h, He, We, S, n_lens_light, n_comp, edge_zero;
+    int P, ny, nx, K, Kp, h, He, We, S, n_lens_light, n_comp, edge_zero, mass_model;
     double pix_scale;
 };
 
@@ -93,7 +105,7 @@ __global__ void __launch_bounds__(256) precise_trace_kernel(const PreciseArgs a)
 {
     __shared__ PreciseRow R;
     const int r = blockIdx.x;
-    if (threadIdx.x == 0) precise_row_setup(a.params + (size_t)r * a.P, a.n_lens_light, a.n_comp - a.n_lens_light, &R);
+    if (threadIdx.x == 0) precise_row_setup(a.params + (size_t)r * a.P, a.n_lens_light, a.n_comp - a.n_lens_light, a.mass_model, &R);
     __syncthreads();
     if (!R.valid) return;
     double *dst = a.ext + (size_t)r * a.He * a.We;
@@ -129,8 +141,10 @@ __global__ void __launch_bounds__(256) precise_conv_kernel(const PreciseArgs a)
         bool ok = true;
         for (int i = 0; i < a.P; ++i) ok = ok && isfinite(p[i]);
         ok = ok && (p[0] >= 0.f) && (hypot((double)p[1], (double)p[2]) < 1.0);
+        const int LP = 7 + (a.mass_model == MASS_EPL ? 1 : 0);
+        if (a.mass_model == MASS_EPL) ok = ok && (p[7] > 1.f) && (p[7] < 3.f);
         for (int k = 0; k < a.n_comp; ++k) {
-            const float *sp = p + 7 + 7 * k;
+            const float *sp = p + LP + 7 * k;
             ok = ok && (sp[1] > 0.f) && (sp[2] > 0.f) && (hypot((double)sp[3], (double)sp[4]) < 1.0);
         }
         valid_s = ok ? 1 : 0;

@@ -112,6 +112,100 @@ static __device__ __noinline__ void sie_alpha_slow(const LensC &L, float xp, flo
     ayp = fmaf(L.fh, ah, L.fl * ah);
 }
 
+// ---- step a2, EPL (mass_model = MASS_EPL): elliptical power law with free slope ---------------
+// PAPER.md:158 Eq. 12, kappa = (3-gamma)/2 (theta_E/R)^(gamma-1) on the ellipses of Eq. 10
+// (G19), deflection by the angular series of Tessore & Metcalf (2015): with
+// t = gamma - 1, R = sqrt(q^2 x'^2 + y'^2), e^{i phi} = (q x' + i y')/R, b = theta_E sqrt(q),
+// f = (1-q)/(1+q),
+//     alpha_x' + i alpha_y' = 2b/(1+q) (R/b)^(1-t) e^{i phi} sum_{n>=0} a_n e^{2 i n phi},
+//     a_0 = 1,  a_n = a_{n-1} (-f) (2n - (2-t)) / (2n + (2-t)).
+// The a_n come from the prologue (FP64, rounded once); the sum is a complex Horner recurrence in
+// w = e^{2 i phi} from the smallest term up, 4 FMAs per term.  The radial factor is
+//     (R^2/b^2)^kappa = 2^(kappa lg2 v),  kappa = (1-t)/2,  v = R^2/b^2 = m 2^e:
+// lg2 v = e + lg2 m with MUFU.LG2 on the mantissa only (absolute error 2^-22, then scaled by
+// |kappa| <= 1/2), and 2^x by splitting off the integer part and a degree-6 polynomial on
+// [-1/2, 1/2] (9e-9) -- MUFU.EX2 alone would carry a 3e-8 bias into every deflection.
+struct EplHot {
+    float q2h, q2l, qh, ql, kh, kl, a0h, a0l, invb2;
+    int nterm;
+    __device__ __forceinline__ explicit EplHot(const LensC &L)
+        : q2h(L.q2h), q2l(L.q2l), qh(L.eqh), ql(L.eql), kh(L.ekh), kl(L.ekl), a0h(L.ea0h), a0l(L.ea0l),
+          invb2(L.einvb2), nterm(L.enterm) {}
+};
+
+__device__ __forceinline__ float exp2_poly(float x)      // 2^x, |x| <= 100
+{
+    const float n = rintf(x);
+    const float r = x - n;                                // exact, |r| <= 1/2
+    float p = 1.545316336e-04f;
+    p = fmaf(p, r, 1.339086331e-03f);
+    p = fmaf(p, r, 9.618083015e-03f);
+    p = fmaf(p, r, 5.550356954e-02f);
+    p = fmaf(p, r, 2.402265072e-01f);
+    p = fmaf(p, r, 6.931471825e-01f);
+    p = fmaf(p, r, 1.0f);                                 // in [0.707, 1.415]
+    return __int_as_float(__float_as_int(p) + ((int)n << 23));
+}
+
+__device__ __forceinline__ void epl_alpha(const EplHot &L, const float *coef, float xp, float yp, float &axp, float &ayp)
+{
+    const float xx = xp * xp;
+    const float psi2 = fmaf(L.q2h, xx, fmaf(L.q2l, xx, fmaf(yp, yp, 1e-30f)));       // R^2 (> 0, G6)
+    const float rinv = mufu_rsq(psi2);
+    const float cph = fmaf(xp, L.qh, xp * L.ql) * rinv, sph = yp * rinv;              // e^{i phi}
+    const float c2 = (cph - sph) * (cph + sph), s2 = 2.f * cph * sph;                 // w = e^{2 i phi}
+    float zr = coef[L.nterm - 1], zi = 0.f;
+    for (int n = L.nterm - 2; n >= 0; --n) {                                          // z <- z w + a_{n+1}
+        const float tr = fmaf(zr, c2, fmaf(-zi, s2, coef[n]));
+        zi = fmaf(zr, s2, zi * c2);
+        zr = tr;
+    }
+    const float sr = fmaf(zr, c2, fmaf(-zi, s2, 1.f)), si = fmaf(zr, s2, zi * c2);    // 1 + z w
+    const float omr = fmaf(cph, sr, -sph * si), omi = fmaf(cph, si, sph * sr);        // Omega
+    // radial factor 2 b/(1+q) (R^2/b^2)^kappa
+    const float v = psi2 * L.invb2;
+    const int vb = __float_as_int(v);
+    const float ef = (float)((vb >> 23) - 127);
+    const float lm = mufu_lg2(__int_as_float((vb & 0x007fffff) | 0x3f800000));        // lg2 of the mantissa in [1, 2)
+    float arg = fmaf(ef, L.kh, fmaf(lm, L.kh, (ef + lm) * L.kl));
+    arg = fminf(fmaxf(arg, -100.f), 100.f);
+    const float pw = exp2_poly(arg);
+    const float P = fmaf(pw, L.a0h, pw * L.a0l);
+    axp = P * omr;
+    ayp = P * omi;
+}
+
+// The same in FP64 (series summed forward until it has converged): selective refinement, rows
+// whose series needs more than EPL_TERMS terms (q < 0.35), and the FP64 validation mode.
+__device__ inline void epl_alpha_f64(double t, double A, double q, double fe, double xp, double yp,
+                                     double &axp, double &ayp)
+{
+    const double R2 = q * q * xp * xp + yp * yp;
+    axp = 0.0; ayp = 0.0;
+    if (!(R2 > 0.0) || A == 0.0) return;
+    const double rinv = 1.0 / sqrt(R2);
+    const double cph = q * xp * rinv, sph = yp * rinv;
+    const double c2 = (cph - sph) * (cph + sph), s2 = 2.0 * cph * sph;
+    const double s2t = 2.0 - t;
+    double tr = cph, ti = sph, sr = cph, si = sph;
+    for (int n = 1; n < 20000; ++n) {
+        const double fac = -fe * (2.0 * n - s2t) / (2.0 * n + s2t);
+        const double nr = fac * (tr * c2 - ti * s2), ni = fac * (tr * s2 + ti * c2);
+        tr = nr; ti = ni;
+        sr += tr; si += ti;
+        if (fabs(tr) + fabs(ti) < 1e-17) break;
+    }
+    const double P = A * exp(0.5 * (1.0 - t) * log(R2));
+    axp = P * sr; ayp = P * si;
+}
+
+static __device__ __noinline__ void epl_alpha_slow(const LensC &L, float xp, float yp, float &axp, float &ayp)
+{
+    double ax, ay;
+    epl_alpha_f64(L.dt, L.dA, L.dq, L.dfe, (double)xp, (double)yp, ax, ay);
+    axp = (float)ax; ayp = (float)ay;
+}
+
 // ---- steps a3 / a4: Sersic value from t = (R_p/r_e)^2 -----------------------------------------
 // Returns 2^(k (1 - u)), u = t^(1/2n) (the caller multiplies by amp).  `flag` is set when the
 // sample needs the FP64 refinement (meaningful for sources only; see tl_consts.cuh).
@@ -132,6 +226,7 @@ __device__ __forceinline__ float quad_form(const QuadHot &C, float x, float y)
 }
 
 // ---- step a2 in FP64 (selective refinement only): lens-frame offset R^T (beta - s) ----------
+template <int MASS>
 __device__ __forceinline__ void refine_offsets(const LensC &L, const SersicC &C, float Xf, float Yf,
                                                float &xi, float &eta)
 {
@@ -141,7 +236,9 @@ __device__ __forceinline__ void refine_offsets(const LensC &L, const SersicC &C,
     const double yp = dy * L.dc - dx * L.ds;
     const double psi = sqrt(L.dq2 * xp * xp + yp * yp);
     double axp = 0.0, ayp = 0.0;
-    if (psi > 0.0) {
+    if (MASS == MASS_EPL) {
+        epl_alpha_f64(L.dt, L.dA, L.dq, L.dfe, xp, yp, axp, ayp);
+    } else if (psi > 0.0) {
         axp = L.df * atan(L.dqp * xp / psi);
         ayp = L.df * atanh(L.dqp * yp / psi);
     }
@@ -154,13 +251,14 @@ __device__ __forceinline__ void refine_offsets(const LensC &L, const SersicC &C,
 }
 
 // Source light of one sub-sample with the ray-trace redone in FP64 (rare, out of line).
+template <int MASS>
 static __device__ __noinline__ float refined_source_light(const RowC &rc, int k0, int k1, float X, float Y)
 {
     float src = 0.f;
     for (int k = k0; k < k1; ++k) {
         const SersicC &C = rc.comp[k];
         float xi, eta;
-        refine_offsets(rc.lens, C, X, Y, xi, eta);
+        refine_offsets<MASS>(rc.lens, C, X, Y, xi, eta);
         QuadHot Q(C);
         Q.oxh = Q.oxl = Q.oyh = Q.oyl = 0.f;
         bool fl;
@@ -170,9 +268,10 @@ static __device__ __noinline__ float refined_source_light(const RowC &rc, int k0
 }
 
 // Same for one source component k only (linear-amplitude mode keeps the components apart).
+template <int MASS>
 static __device__ __noinline__ float refined_source_light_k(const RowC &rc, int k, float X, float Y)
 {
-    return refined_source_light(rc, k, k + 1, X, Y);
+    return refined_source_light<MASS>(rc, k, k + 1, X, Y);
 }
 
 }  // namespace tl
