@@ -134,6 +134,24 @@ __device__ __forceinline__ void sample_value(const RowC &rc, const HotC<NLL, NSR
     }
 }
 
+// Steps a3-a4 of one sub-sample once its deflection is known (EPL: the deflections of the S_T
+// sub-samples of a pixel row are computed together, see epl_alpha_vec).
+template <int NLL, int NSRC, int MASS>
+__device__ __forceinline__ void sample_light(const HotC<NLL, NSRC, MASS> &h, const ColV &c, const RowV &r, float axp, float ayp,
+                                             float &acc, float (&src)[NSRC], bool &flag)
+{
+    bool fl;
+    if (NLL) acc = fmaf(h.ll.amp, sersic_from_t(h.ll, fmaf(c.LB, r.dyl, c.LA + r.LC), fl), acc);
+    const float bx = (c.U + r.V) - axp, by = (c.U2 + r.V2) - ayp;      // R^T (beta - s_1)
+    src[0] = h.src[0].amp * sersic_from_t(h.src[0], quad_form(h.q[0], bx, by), fl);
+    flag = fl;
+    if (NSRC > 1) {
+        const float t2 = quad_form(h.q[1], (bx - h.q[1].oxh) - h.q[1].oxl, (by - h.q[1].oyh) - h.q[1].oyl);
+        src[NSRC - 1] = h.src[1].amp * sersic_from_t(h.src[1], t2, fl);
+        flag = flag || fl;
+    }
+}
+
 // steps a1-a5 for a run of `count` warp tiles.  A warp tile is CW x CH = 32 extended native
 // pixels (lane -> column lane % CW, row lane / CW), so the samples a warp works on are
 // neighbours in the image (coherent refinement branches) and all lanes are busy; tiles are
@@ -182,12 +200,26 @@ __device__ __forceinline__ void trace_tiles(const RowC &rc, const HotC<NLL, NSRC
                     if (S_T > 0) {
                         float src[S_T > 0 ? S_T : 1][NSRC];
                         bool any = false;
+                        if constexpr (MASS == MASS_EPL && FAST) {
+                            float xp[S_T > 0 ? S_T : 1], yp[S_T > 0 ? S_T : 1], axp[S_T > 0 ? S_T : 1], ayp[S_T > 0 ? S_T : 1];
+#pragma unroll
+                            for (int sb = 0; sb < S_T; ++sb) { xp[sb] = cv[sb].Pc + rv.Qs; yp[sb] = rv.Qc - cv[sb].Ps; }
+                            epl_alpha_vec<(S_T > 0 ? S_T : 1)>(h.sie, rc.lens.ecoef, xp, yp, axp, ayp);
+#pragma unroll
+                            for (int sb = 0; sb < S_T; ++sb) {
+                                bool fl;
+                                sample_light<NLL, NSRC, MASS>(h, cv[sb], rv, axp[sb], ayp[sb], acc, src[sb], fl);
+                                any = any || fl;
+                                if (fl) src[sb][0] = __int_as_float(0x7fc00000);
+                            }
+                        } else {
 #pragma unroll
                         for (int sb = 0; sb < S_T; ++sb) {
                             bool fl;
                             sample_value<NLL, NSRC, FAST, MASS>(rc, h, cv[sb], rv, acc, src[sb], fl);
                             any = any || fl;
                             if (fl) src[sb][0] = __int_as_float(0x7fc00000);      // NaN marks "refine me"
+                        }
                         }
                         if (any) {                                  // rare: FP64 ray-trace, out of line
 #pragma unroll

@@ -135,8 +135,10 @@ struct EplHot {
 
 __device__ __forceinline__ float exp2_poly(float x)      // 2^x, |x| <= 100
 {
-    const float n = rintf(x);
-    const float r = x - n;                                // exact, |r| <= 1/2
+    // round to nearest integer with the 1.5 * 2^23 trick: no conversion instructions (F2I / I2F /
+    // FRND issue at a quarter of the FMA rate), and the integer sits in the low mantissa bits
+    const float big = x + 12582912.f;
+    const float r = x - (big - 12582912.f);               // exact, |r| <= 1/2
     float p = 1.545316336e-04f;
     p = fmaf(p, r, 1.339086331e-03f);
     p = fmaf(p, r, 9.618083015e-03f);
@@ -144,35 +146,59 @@ __device__ __forceinline__ float exp2_poly(float x)      // 2^x, |x| <= 100
     p = fmaf(p, r, 2.402265072e-01f);
     p = fmaf(p, r, 6.931471825e-01f);
     p = fmaf(p, r, 1.0f);                                 // in [0.707, 1.415]
-    return __int_as_float(__float_as_int(p) + ((int)n << 23));
+    return __int_as_float(__float_as_int(p) + (__float_as_int(big) << 23));
+}
+
+// NS sub-samples at once: the coefficient loads and the loop control of the Horner recurrence are
+// shared by the NS independent chains.
+template <int NS>
+__device__ __forceinline__ void epl_alpha_vec(const EplHot &L, const float *coef, const float (&xp)[NS], const float (&yp)[NS],
+                                              float (&axp)[NS], float (&ayp)[NS])
+{
+    float c2[NS], s2[NS], pc[NS], ps[NS], zr[NS], zi[NS];
+    const float cN = coef[L.nterm - 1];
+#pragma unroll
+    for (int s = 0; s < NS; ++s) {
+        const float xx = xp[s] * xp[s];
+        const float psi2 = fmaf(L.q2h, xx, fmaf(L.q2l, xx, fmaf(yp[s], yp[s], 1e-30f)));   // R^2 (> 0, G6)
+        const float rinv = mufu_rsq(psi2);
+        const float cph = fmaf(xp[s], L.qh, xp[s] * L.ql) * rinv, sph = yp[s] * rinv;       // e^{i phi}
+        c2[s] = (cph - sph) * (cph + sph); s2[s] = 2.f * cph * sph;                         // w = e^{2 i phi}
+        // radial factor 2 b/(1+q) (R^2/b^2)^kappa; exponent and mantissa of v taken apart with
+        // integer ops (e = biased exponent - 127 through the 2^23 trick, again no conversion)
+        const int vb = __float_as_int(psi2 * L.invb2);
+        const float ef = __int_as_float((vb >> 23) | 0x4b000000) - 8388735.f;
+        const float lm = mufu_lg2(__int_as_float((vb & 0x007fffff) | 0x3f800000));          // mantissa in [1, 2)
+        float arg = fmaf(ef, L.kh, fmaf(lm, L.kh, (ef + lm) * L.kl));
+        arg = fminf(fmaxf(arg, -100.f), 100.f);
+        const float pw = exp2_poly(arg);
+        const float P = fmaf(pw, L.a0h, pw * L.a0l);
+        pc[s] = P * cph; ps[s] = P * sph;
+        zr[s] = cN; zi[s] = 0.f;
+    }
+    for (int n = L.nterm - 2; n >= 0; --n) {                                                // z <- z w + a_{n+1}
+        const float cn = coef[n];
+#pragma unroll
+        for (int s = 0; s < NS; ++s) {
+            const float tr = fmaf(zr[s], c2[s], fmaf(-zi[s], s2[s], cn));
+            zi[s] = fmaf(zr[s], s2[s], zi[s] * c2[s]);
+            zr[s] = tr;
+        }
+    }
+#pragma unroll
+    for (int s = 0; s < NS; ++s) {
+        const float sr = fmaf(zr[s], c2[s], fmaf(-zi[s], s2[s], 1.f)), si = fmaf(zr[s], s2[s], zi[s] * c2[s]);   // 1 + z w
+        axp[s] = fmaf(pc[s], sr, -ps[s] * si);
+        ayp[s] = fmaf(pc[s], si, ps[s] * sr);
+    }
 }
 
 __device__ __forceinline__ void epl_alpha(const EplHot &L, const float *coef, float xp, float yp, float &axp, float &ayp)
 {
-    const float xx = xp * xp;
-    const float psi2 = fmaf(L.q2h, xx, fmaf(L.q2l, xx, fmaf(yp, yp, 1e-30f)));       // R^2 (> 0, G6)
-    const float rinv = mufu_rsq(psi2);
-    const float cph = fmaf(xp, L.qh, xp * L.ql) * rinv, sph = yp * rinv;              // e^{i phi}
-    const float c2 = (cph - sph) * (cph + sph), s2 = 2.f * cph * sph;                 // w = e^{2 i phi}
-    float zr = coef[L.nterm - 1], zi = 0.f;
-    for (int n = L.nterm - 2; n >= 0; --n) {                                          // z <- z w + a_{n+1}
-        const float tr = fmaf(zr, c2, fmaf(-zi, s2, coef[n]));
-        zi = fmaf(zr, s2, zi * c2);
-        zr = tr;
-    }
-    const float sr = fmaf(zr, c2, fmaf(-zi, s2, 1.f)), si = fmaf(zr, s2, zi * c2);    // 1 + z w
-    const float omr = fmaf(cph, sr, -sph * si), omi = fmaf(cph, si, sph * sr);        // Omega
-    // radial factor 2 b/(1+q) (R^2/b^2)^kappa
-    const float v = psi2 * L.invb2;
-    const int vb = __float_as_int(v);
-    const float ef = (float)((vb >> 23) - 127);
-    const float lm = mufu_lg2(__int_as_float((vb & 0x007fffff) | 0x3f800000));        // lg2 of the mantissa in [1, 2)
-    float arg = fmaf(ef, L.kh, fmaf(lm, L.kh, (ef + lm) * L.kl));
-    arg = fminf(fmaxf(arg, -100.f), 100.f);
-    const float pw = exp2_poly(arg);
-    const float P = fmaf(pw, L.a0h, pw * L.a0l);
-    axp = P * omr;
-    ayp = P * omi;
+    const float x1[1] = {xp}, y1[1] = {yp};
+    float a1[1], b1[1];
+    epl_alpha_vec<1>(L, coef, x1, y1, a1, b1);
+    axp = a1[0]; ayp = b1[0];
 }
 
 // The same in FP64 (series summed forward until it has converged): selective refinement, rows
