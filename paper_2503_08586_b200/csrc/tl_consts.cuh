@@ -56,8 +56,8 @@ struct LensC {                       // SIE + external shear
     float ekh, ekl;                  // kappa = (1 - t) / 2
     float ea0h, ea0l;                // alpha at R = b:  2 b_u / (1 + q)
     float einvb2;                    // 1 / b_u^2,  b = theta_E sqrt(q)
-    int32_t enterm;                  // N: Omega = e^{i phi} (1 + sum_{n=1..N} a_n e^{2 i n phi})
-    float ecoef[EPL_TERMS];          // a_n = prod_{k<=n} -f (2k - (2-t)) / (2k + (2-t)),  ecoef[n-1] = a_n
+    int32_t enterm;                  // N (even): Omega = e^{i phi} (1 + sum_{n=1..N} a_n e^{2 i n phi})
+    alignas(8) float ecoef[EPL_TERMS];          // a_n = prod_{k<=n} -f (2k - (2-t)) / (2k + (2-t)),  ecoef[n-1] = a_n
 };
 
 struct SersicC {                     // one elliptical Sersic component
@@ -252,7 +252,8 @@ __global__ void __launch_bounds__(128) prologue_kernel(PrologueArgs a)
                 N = n;
             }
             L.mode = (N <= EPL_TERMS) ? 2 : 3;
-            L.enterm = N < 1 ? 1 : (N > EPL_TERMS ? EPL_TERMS : N);
+            N = (N + 1) & ~1;                                            // even: the recurrence takes two terms per trip
+            L.enterm = N < 2 ? 2 : (N > EPL_TERMS ? EPL_TERMS : N);
         }
         rc->lens = L;
         return;

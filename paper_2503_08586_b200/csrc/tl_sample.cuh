@@ -119,8 +119,11 @@ static __device__ __noinline__ void sie_alpha_slow(const LensC &L, float xp, flo
 // f = (1-q)/(1+q),
 //     alpha_x' + i alpha_y' = 2b/(1+q) (R/b)^(1-t) e^{i phi} sum_{n>=0} a_n e^{2 i n phi},
 //     a_0 = 1,  a_n = a_{n-1} (-f) (2n - (2-t)) / (2n + (2-t)).
-// The a_n come from the prologue (FP64, rounded once); the sum is a complex Horner recurrence in
-// w = e^{2 i phi} from the smallest term up, 4 FMAs per term.  The radial factor is
+// The a_n come from the prologue (FP64, rounded once).  They are real, so the complex sum is a
+// cosine and a sine series in theta = 2 phi, and ONE Clenshaw recurrence serves both:
+//     b_k = a_k + 2 cos(theta) b_{k+1} - b_{k+2}   (k = N .. 0,  b_{N+1} = b_{N+2} = 0),
+//     sum a_n cos(n theta) = b_0 - b_1 cos(theta),   sum a_n sin(n theta) = b_1 sin(theta),
+// two instructions per term (a complex Horner step takes four).  The radial factor is
 //     (R^2/b^2)^kappa = 2^(kappa lg2 v),  kappa = (1-t)/2,  v = R^2/b^2 = m 2^e:
 // lg2 v = e + lg2 m with MUFU.LG2 on the mantissa only (absolute error 2^-22, then scaled by
 // |kappa| <= 1/2), and 2^x by splitting off the integer part and a degree-6 polynomial on
@@ -155,8 +158,7 @@ template <int NS>
 __device__ __forceinline__ void epl_alpha_vec(const EplHot &L, const float *coef, const float (&xp)[NS], const float (&yp)[NS],
                                               float (&axp)[NS], float (&ayp)[NS])
 {
-    float c2[NS], s2[NS], pc[NS], ps[NS], zr[NS], zi[NS];
-    const float cN = coef[L.nterm - 1];
+    float c2[NS], s2[NS], pc[NS], ps[NS], tc[NS], b1[NS], b2[NS];
 #pragma unroll
     for (int s = 0; s < NS; ++s) {
         const float xx = xp[s] * xp[s];
@@ -174,20 +176,21 @@ __device__ __forceinline__ void epl_alpha_vec(const EplHot &L, const float *coef
         const float pw = exp2_poly(arg);
         const float P = fmaf(pw, L.a0h, pw * L.a0l);
         pc[s] = P * cph; ps[s] = P * sph;
-        zr[s] = cN; zi[s] = 0.f;
+        tc[s] = 2.f * c2[s]; b1[s] = 0.f; b2[s] = 0.f;
     }
-    for (int n = L.nterm - 2; n >= 0; --n) {                                                // z <- z w + a_{n+1}
-        const float cn = coef[n];
+    // Clenshaw, two terms per trip (nterm is even): no register moves, one LDS.64 of coefficients
+    for (int n = L.nterm; n >= 2; n -= 2) {
+        const float2 cf = *reinterpret_cast<const float2 *>(coef + n - 2);                  // a_{n-1}, a_n
 #pragma unroll
         for (int s = 0; s < NS; ++s) {
-            const float tr = fmaf(zr[s], c2[s], fmaf(-zi[s], s2[s], cn));
-            zi[s] = fmaf(zr[s], s2[s], zi[s] * c2[s]);
-            zr[s] = tr;
+            b2[s] = fmaf(tc[s], b1[s], cf.y) - b2[s];                                       // b_n
+            b1[s] = fmaf(tc[s], b2[s], cf.x) - b1[s];                                       // b_{n-1}
         }
     }
 #pragma unroll
     for (int s = 0; s < NS; ++s) {
-        const float sr = fmaf(zr[s], c2[s], fmaf(-zi[s], s2[s], 1.f)), si = fmaf(zr[s], s2[s], zi[s] * c2[s]);   // 1 + z w
+        const float b0 = fmaf(tc[s], b1[s], 1.f) - b2[s];                                   // a_0 = 1
+        const float sr = fmaf(-c2[s], b1[s], b0), si = s2[s] * b1[s];
         axp[s] = fmaf(pc[s], sr, -ps[s] * si);
         ayp[s] = fmaf(pc[s], si, ps[s] * sr);
     }
