@@ -41,6 +41,10 @@ OP_POS_FP32 = 2
 OP_SIE_FP32, OP_SIE_MUFU = 46, 4
 OP_SERSIC_FP32, OP_SERSIC_MUFU = 11, 3
 OP_CHI2_FP32 = 4
+# EPL (NEXT-2, --mass epl), same counting rules: shift/rotate 6; R^2 2; rsqrt (MUFU); e^{i phi} 3;
+# e^{2 i phi} 4; Clenshaw recurrence 2 per series term + 4 to close it; radial factor
+# (R^2/b^2)^kappa: 3 + lg2, ex2 (MUFU); Omega x radial 6; rotate back 4; shear + subtract 6.
+OP_EPL_FP32, OP_EPL_FP32_PER_TERM, OP_EPL_MUFU = 38, 2, 3
 SM_FP32_LANES = 128          # thread-instruction issue slots per SM per clock (4 warps x 32), measured 122-128
 SM_MUFU_LANES = 16           # measured 15.96 (profiles/r1_mufu_accuracy.md)
 
@@ -49,12 +53,36 @@ SM_MUFU_LANES = 16           # measured 15.96 (profiles/r1_mufu_accuracy.md)
 NCU_DRAM_BYTES_PER_LAUNCH = 2363136       # profiles/r1_fused_kernel.md: dram__bytes_read.sum 2.363136 MB + 0 B written
 
 
-def op_model(w: W.Workload) -> dict:
+def epl_mean_terms(rows: np.ndarray) -> float:
+    """Mean number of angular-series terms a row needs for a truncation error below 2e-8 (FP32
+    resolution): |a_{N+1}| < 2e-8 (1 - f), a_n = a_{n-1} (-f) (2n - (2-t)) / (2n + (2-t))."""
+    e = np.hypot(rows[:, 1].astype(np.float64), rows[:, 2].astype(np.float64))     # f = (1-q)/(1+q) = |e|
+    t = rows[:, 7].astype(np.float64) - 1.0
+    an = np.ones_like(e)
+    need = np.zeros_like(e)
+    done = np.zeros(e.shape, bool)
+    for n in range(1, 400):
+        an = an * e * np.abs(2.0 * n - (2.0 - t)) / (2.0 * n + (2.0 - t))
+        newly = (~done) & (an < 2e-8 * (1.0 - e))
+        need[newly] = n - 1
+        done |= newly
+        if done.all():
+            break
+    need[~done] = 400
+    return float(need.mean())
+
+
+def op_model(w: W.Workload, rows=None) -> dict:
     ncomp = w.n_lens_light + w.n_source
     samples = w.samples_per_likelihood
-    fp32 = samples * (OP_POS_FP32 + OP_SIE_FP32 + ncomp * OP_SERSIC_FP32) \
+    if w.mass_model == W.MASS_EPL:
+        mass_fp32 = OP_EPL_FP32 + OP_EPL_FP32_PER_TERM * epl_mean_terms(rows)
+        mass_mufu = OP_EPL_MUFU
+    else:
+        mass_fp32, mass_mufu = OP_SIE_FP32, OP_SIE_MUFU
+    fp32 = samples * (OP_POS_FP32 + mass_fp32 + ncomp * OP_SERSIC_FP32) \
         + w.ny * w.nx * (w.psf_size ** 2 + OP_CHI2_FP32)
-    mufu = samples * (OP_SIE_MUFU + ncomp * OP_SERSIC_MUFU)
+    mufu = samples * (mass_mufu + ncomp * OP_SERSIC_MUFU)
     return {"fp32_slots": fp32, "mufu_ops": mufu, "issue_slots": fp32 + mufu, "samples": samples}
 
 
@@ -173,7 +201,7 @@ def run_reference(args, w: W.Workload):
     tot = float(np.sum(times))
     value = n * len(times) / tot
     line = {
-        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "impl": "reference", "metric": METRIC + mass_tag(w), "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / len(times),
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic", "config": config_dict(w, "none (CPU)"),
@@ -185,11 +213,16 @@ def run_reference(args, w: W.Workload):
     print(json.dumps(line))
 
 
+def mass_tag(w: W.Workload) -> str:
+    return " (EPL mass model)" if w.mass_model == W.MASS_EPL else ""
+
+
 def config_dict(w: W.Workload, l2: str) -> dict:
     return {"workload": "BASELINE.json configs[%d] %s: %dx%d px, %.3g\"/px, %dx%d supersampling, %dx%d %s PSF, "
-                        "SIE+shear, %d lens-light + %d source Sersic, B=%d rows/GPU%s"
+                        "%s+shear, %d lens-light + %d source Sersic, B=%d rows/GPU%s"
                         % (w.index, w.name, w.ny, w.nx, w.pix_scale, w.supersample, w.supersample, w.psf_size,
-                           w.psf_size, w.psf_kind, w.n_lens_light, w.n_source, w.batch,
+                           w.psf_size, w.psf_kind, "EPL (free slope)" if w.mass_model == W.MASS_EPL else "SIE",
+                           w.n_lens_light, w.n_source, w.batch,
                            (", %d lenses" % w.n_lens) if w.n_lens > 1 else ""),
             "batch_per_gpu": w.batch, "n_params": w.n_params, "l2": l2, "parallelism": "rows sharded, no collective"}
 
@@ -214,7 +247,7 @@ def run_ours(args, w: W.Workload):
     def gpu_render(w1, psf, row):
         ctx = api.LensContext(w1.ny, w1.nx, w1.pix_scale, w1.supersample, w1.n_lens_light, w1.n_source,
                               psf[None], np.zeros((1, w1.ny, w1.nx), np.float32),
-                              np.ones((1, w1.ny, w1.nx), np.float32), w1.edge_mode)
+                              np.ones((1, w1.ny, w1.nx), np.float32), w1.edge_mode, mass_model=w1.mass_model)
         im = ctx.render(torch.from_numpy(np.ascontiguousarray(row[None])).to(dev)).cpu().numpy()[0]
         ctx.close()
         return im
@@ -285,7 +318,7 @@ def run_ours(args, w: W.Workload):
 
     value = world * B * args.steps / (total_ms * 1e-3)
     e2e_value = world * B * args.steps / e2e_s
-    om = op_model(w)
+    om = op_model(w, rows)
     peaks = measured_peaks()
     sm_max = float(peaks.get("sm_max_mhz", 1965.0))
     k_ms = float(np.mean(kern_ms))
@@ -295,7 +328,7 @@ def run_ours(args, w: W.Workload):
     fp32_frac = om["fp32_slots"] * B / (k_ms * 1e-3) / (info["n_sm"] * SM_FP32_LANES * sm_max * 1e6)
     hbm_bytes = B * (w.n_params + 1) * 4 + (2 * w.ny * w.nx + w.psf_size ** 2) * 4 * w.n_lens
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "metric": METRIC + mass_tag(w), "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": config_dict(w, "flushed between steps (256 MiB fill)"),
@@ -308,11 +341,12 @@ def run_ours(args, w: W.Workload):
         "roofline": {
             "bound": "alu", "kernel": "fused_kernel" if info["path"] == 0 else "trace_kernel",
             "achieved": achieved, "peak": peak, "unit": "Tinst/s", "frac": achieved / peak,
-            "traffic": NCU_DRAM_BYTES_PER_LAUNCH,
+            "traffic": NCU_DRAM_BYTES_PER_LAUNCH if (w.mass_model == W.MASS_SIE and w.index == 1) else None,
             "peak_source": "derived: %d SMs x %d issue slots/clk x %.0f MHz (MEASURED_PEAKS.json sm_max_mhz; "
                            "slots/clk measured, profiles/r1_mufu_accuracy.md)" % (info["n_sm"], SM_FP32_LANES, sm_max),
             "kernel_ms": k_ms, "fp32_pipe_frac": fp32_frac, "mufu_pipe_frac": mufu_frac,
             "algorithmic_issue_slots_per_likelihood": om["issue_slots"],
+            **({"epl_mean_series_terms": epl_mean_terms(rows)} if w.mass_model == W.MASS_EPL else {}),
             "hbm": {"algorithmic_bytes_per_step": hbm_bytes,
                     "achieved_GBs": hbm_bytes / (k_ms * 1e-3) / 1e9,
                     "peak_GBs": peaks.get("hbm_gbs"), "note": "compute-bound by design; HBM traffic is negligible"},
@@ -344,7 +378,7 @@ def run_linear(args, w: W.Workload):
     def gpu_render(w1, psf, row):
         ctx = api.LensContext(w1.ny, w1.nx, w1.pix_scale, w1.supersample, w1.n_lens_light, w1.n_source,
                               psf[None], np.zeros((1, w1.ny, w1.nx), np.float32),
-                              np.ones((1, w1.ny, w1.nx), np.float32), w1.edge_mode)
+                              np.ones((1, w1.ny, w1.nx), np.float32), w1.edge_mode, mass_model=w1.mass_model)
         im = ctx.render(torch.from_numpy(np.ascontiguousarray(row[None])).to(dev)).cpu().numpy()[0]
         ctx.close()
         return im
@@ -371,7 +405,7 @@ def run_linear(args, w: W.Workload):
         torch.cuda.synchronize()
     total_ms = float(np.sum([a.elapsed_time(b) for a, b in ev]))
     value = B * args.steps / (total_ms * 1e-3)
-    line = {"metric": METRIC + " (linear amplitudes, NNLS per row)", "value": value, "unit": UNIT, "n_gpus": 1,
+    line = {"metric": METRIC + mass_tag(w) + " (linear amplitudes, NNLS per row)", "value": value, "unit": UNIT, "n_gpus": 1,
             "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": config_dict(w, "flushed between steps (256 MiB fill)"), "clocks": clk.summary(),
@@ -380,7 +414,7 @@ def run_linear(args, w: W.Workload):
     # roofline of the fused linear kernel: op model v0 per sample (unchanged) + per native pixel
     # C convolutions, the Gram matrix / right-hand side (C (C + 3)) and the residual (C + 3)
     C_ = w.n_lens_light + w.n_source
-    om = op_model(w)
+    om = op_model(w, rows)
     slots = om["issue_slots"] + w.ny * w.nx * ((C_ - 1) * w.psf_size ** 2 + C_ * (C_ + 3) + C_ + 3 - OP_CHI2_FP32)
     info = ctx.info()
     sm_max = float(measured_peaks().get("sm_max_mhz", 1965.0))
@@ -416,8 +450,13 @@ def main():
     ap.add_argument("--mode", default="fixed", choices=["fixed", "linear"],
                     help="fixed: amplitudes are parameters (the headline metric); linear: amplitudes solved by NNLS "
                          "per row (tl_loglike_linear_batch, PAPER.md Eq. 6-7) -- a secondary line")
+    ap.add_argument("--mass", default="sie", choices=["sie", "epl"],
+                    help="sie: the headline workload; epl: the same workload with the elliptical power-law mass "
+                         "model and a free slope per row (NEXT-2, PAPER.md Eq. 12) -- a secondary line")
     args = ap.parse_args()
     w = W.workload(args.config)
+    if args.mass == "epl":
+        w = w.with_epl()
     if args.batch:
         w = w.scaled(batch=args.batch)
     world = int(os.environ.get("WORLD_SIZE", "1"))

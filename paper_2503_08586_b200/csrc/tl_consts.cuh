@@ -29,6 +29,7 @@ namespace tl {
 constexpr int MAX_COMP = 3;          // n_lens_light (<= 1) + n_source (<= 2)
 constexpr int MASS_SIE = 0, MASS_EPL = 1;          // tl_config.mass_model
 constexpr int EPL_TERMS = 24;        // angular-series terms of the FP32 EPL path (rows needing more: FP64)
+constexpr int EPL_TERMS64 = 64;      // terms kept in FP64 for the selective refinement (remainder < 1e-16)
 
 struct LensC {                       // SIE + external shear
     float cXa, cYa;                  // centre rounded to 2^-8 u-units: X - cXa is exact
@@ -57,6 +58,8 @@ struct LensC {                       // SIE + external shear
     float ea0h, ea0l;                // alpha at R = b:  2 b_u / (1 + q)
     float einvb2;                    // 1 / b_u^2,  b = theta_E sqrt(q)
     int32_t enterm;                  // N (even): Omega = e^{i phi} (1 + sum_{n=1..N} a_n e^{2 i n phi})
+    double edcoef[EPL_TERMS64];      // a_n in FP64, continued until |a_n| < 1e-16 (selective refinement)
+    int32_t ednterm, epad[3];        // number of FP64 terms (even)
     alignas(8) float ecoef[EPL_TERMS];          // a_n = prod_{k<=n} -f (2k - (2-t)) / (2k + (2-t)),  ecoef[n-1] = a_n
 };
 
@@ -184,7 +187,7 @@ __global__ void __launch_bounds__(128) prologue_kernel(PrologueArgs a)
     if (!lens_ok) { thE = 0.0; q = 1.0; c = 1.0; s = 0.0; }
 
     if (slot == 0) {
-        LensC L;
+        LensC &L = rc->lens;             // written in place: the SIE fills only the first 232 bytes
         // q' = sqrt((1-q)(1+q)); clamped away from 0 so that f = theta_E sqrt(q)/q' stays
         // finite: for q' <= 1e-6 the exact deflection differs from the clamped one by a
         // relative O(q'^2) < 1e-12 (atan(z)/z, atanh(z)/z -> 1).
@@ -229,10 +232,12 @@ __global__ void __launch_bounds__(128) prologue_kernel(PrologueArgs a)
         L.dcX = cX; L.dcY = cY; L.dc = c; L.ds = s; L.dq2 = q * q; L.dqp = qp; L.df = f;
         L.dg1 = g1; L.dg2 = g2;
         // ---- EPL (Eq. 12; Tessore & Metcalf 2015 angular series, G19)
-        L.dt = 1.0; L.dA = 0.0; L.dq = q; L.dfe = (1.0 - q) / (1.0 + q);
-        L.eqh = L.eql = L.ekh = L.ekl = L.ea0h = L.ea0l = 0.f; L.einvb2 = 1.f; L.enterm = 1;
-        for (int n = 0; n < EPL_TERMS; ++n) L.ecoef[n] = 0.f;
+        // (the EPL block of LensC is left unwritten for the SIE: nothing reads it)
         if (a.mass_model == MASS_EPL) {
+            L.dq = q; L.dfe = (1.0 - q) / (1.0 + q);
+            for (int n = 0; n < EPL_TERMS; ++n) L.ecoef[n] = 0.f;
+            for (int n = 0; n < EPL_TERMS64; ++n) L.edcoef[n] = 0.0;
+            L.ednterm = 2; L.epad[0] = L.epad[1] = L.epad[2] = 0;
             const double t = lens_ok ? (double)p[7] - 1.0 : 1.0;
             const double bu = thE * sqrt(q) * a.inv_u;                   // b = theta_E sqrt(q), u-units
             L.dt = t;
@@ -252,10 +257,21 @@ __global__ void __launch_bounds__(128) prologue_kernel(PrologueArgs a)
                 N = n;
             }
             L.mode = (N <= EPL_TERMS) ? 2 : 3;
+            if (L.mode == 2) {                                           // FP64 continuation of the same table
+                double ad = 1.0;
+                int N64 = 0;
+                for (int n = 1; n <= EPL_TERMS64; ++n) {
+                    ad *= -fe * (2.0 * n - s2t) / (2.0 * n + s2t);
+                    if (fabs(ad) < 1e-16) break;
+                    L.edcoef[n - 1] = ad;
+                    N64 = n;
+                }
+                N64 = (N64 + 1) & ~1;
+                L.ednterm = N64 < 2 ? 2 : N64;
+            }
             N = (N + 1) & ~1;                                            // even: the recurrence takes two terms per trip
             L.enterm = N < 2 ? 2 : (N > EPL_TERMS ? EPL_TERMS : N);
         }
-        rc->lens = L;
         return;
     }
 

@@ -228,6 +228,29 @@ __device__ inline void epl_alpha_f64(double t, double A, double q, double fe, do
     axp = P * sr; ayp = P * si;
 }
 
+// FP64 with the prologue's coefficient table (rows on the FP32 series path, mode 2): the same
+// Clenshaw recurrence as epl_alpha_vec over the table continued to 1e-16, no divisions.
+__device__ inline void epl_alpha_f64_tab(const LensC &L, double xp, double yp, double &axp, double &ayp)
+{
+    const double q = L.dq;
+    const double R2 = q * q * xp * xp + yp * yp;
+    axp = 0.0; ayp = 0.0;
+    if (!(R2 > 0.0) || L.dA == 0.0) return;
+    const double rinv = 1.0 / sqrt(R2);
+    const double cph = q * xp * rinv, sph = yp * rinv;
+    const double c2 = (cph - sph) * (cph + sph), s2 = 2.0 * cph * sph, tc = 2.0 * c2;
+    double b1 = 0.0, b2 = 0.0;
+    for (int n = L.ednterm; n >= 2; n -= 2) {
+        b2 = fma(tc, b1, L.edcoef[n - 1]) - b2;
+        b1 = fma(tc, b2, L.edcoef[n - 2]) - b1;
+    }
+    const double b0 = fma(tc, b1, 1.0) - b2;
+    const double sr = b0 - c2 * b1, si = s2 * b1;
+    const double P = L.dA * exp(0.5 * (1.0 - L.dt) * log(R2));
+    axp = P * (cph * sr - sph * si);
+    ayp = P * (cph * si + sph * sr);
+}
+
 static __device__ __noinline__ void epl_alpha_slow(const LensC &L, float xp, float yp, float &axp, float &ayp)
 {
     double ax, ay;
@@ -266,7 +289,8 @@ __device__ __forceinline__ void refine_offsets(const LensC &L, const SersicC &C,
     const double psi = sqrt(L.dq2 * xp * xp + yp * yp);
     double axp = 0.0, ayp = 0.0;
     if (MASS == MASS_EPL) {
-        epl_alpha_f64(L.dt, L.dA, L.dq, L.dfe, xp, yp, axp, ayp);
+        if (L.mode == 2) epl_alpha_f64_tab(L, xp, yp, axp, ayp);
+        else epl_alpha_f64(L.dt, L.dA, L.dq, L.dfe, xp, yp, axp, ayp);
     } else if (psi > 0.0) {
         axp = L.df * atan(L.dqp * xp / psi);
         ayp = L.df * atanh(L.dqp * yp / psi);
