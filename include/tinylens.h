@@ -67,7 +67,7 @@ extern "C" {
 #define TL_MASS_EPL 1 /* elliptical power law, Eq. 12 with the slope gamma a parameter  */
                       /* of every row: kappa = (3-gamma)/2 (theta_E/R_p)^(gamma-1) on the ellipses   */
                       /* R_p of Eq. 10, deflection by the angular series of Tessore & Metcalf 2015   */
-                      /* (G19).  gamma = 2 reproduces TL_MASS_SIE.                          */
+                      /* (G22).  gamma = 2 reproduces TL_MASS_SIE.                          */
 
 typedef struct tl_ctx tl_ctx;     /* opaque; owned by the library */
 

@@ -130,7 +130,7 @@ void orc_sie_deflection(double theta_e, double q, double phi, double cx, double 
 
 /* ------------------------------------------------------------------ Eq. 12 (general gamma): EPL
  * PAPER.md:156-160 Eq. 12, kappa(R) = (3-gamma)/2 (theta_E/R)^(gamma-1), made elliptical as the
- * SIE above (R -> R_p of Eq. 10; reading G19), deflection after Tessore & Metcalf
+ * SIE above (R -> R_p of Eq. 10; reading G22), deflection after Tessore & Metcalf
  * (2015), which the paper cites and does not print.  With t = gamma - 1, the elliptical radius
  * and angle  R = sqrt(q^2 x'^2 + y'^2),  R cos(phi) = q x',  R sin(phi) = y',  b = theta_E sqrt(q)
  * (so that kappa = (2-t)/2 (b/R)^t), and f = (1-q)/(1+q), the complex deflection is

@@ -231,7 +231,7 @@ __global__ void __launch_bounds__(128) prologue_kernel(PrologueArgs a)
         L.valid = lens_ok ? 1 : 0;
         L.dcX = cX; L.dcY = cY; L.dc = c; L.ds = s; L.dq2 = q * q; L.dqp = qp; L.df = f;
         L.dg1 = g1; L.dg2 = g2;
-        // ---- EPL (Eq. 12; Tessore & Metcalf 2015 angular series, G19)
+        // ---- EPL (Eq. 12; Tessore & Metcalf 2015 angular series, G22)
         // (the EPL block of LensC is left unwritten for the SIE: nothing reads it)
         if (a.mass_model == MASS_EPL) {
             L.dq = q; L.dfe = (1.0 - q) / (1.0 + q);

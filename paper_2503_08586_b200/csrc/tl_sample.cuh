@@ -114,7 +114,7 @@ static __device__ __noinline__ void sie_alpha_slow(const LensC &L, float xp, flo
 
 // ---- step a2, EPL (mass_model = MASS_EPL): elliptical power law with free slope ---------------
 // PAPER.md:158 Eq. 12, kappa = (3-gamma)/2 (theta_E/R)^(gamma-1) on the ellipses of Eq. 10
-// (G19), deflection by the angular series of Tessore & Metcalf (2015): with
+// (G22), deflection by the angular series of Tessore & Metcalf (2015): with
 // t = gamma - 1, R = sqrt(q^2 x'^2 + y'^2), e^{i phi} = (q x' + i y')/R, b = theta_E sqrt(q),
 // f = (1-q)/(1+q),
 //     alpha_x' + i alpha_y' = 2b/(1+q) (R/b)^(1-t) e^{i phi} sum_{n>=0} a_n e^{2 i n phi},
