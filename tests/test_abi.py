@@ -64,15 +64,16 @@ def test_create_rejects_bad_arguments_before_cuda(api):
     bad = [
         dict(ny=0), dict(nx=-1), dict(pix_scale=0.0), dict(pix_scale=float("nan")), dict(supersample=0),
         dict(supersample=17), dict(n_lens_light=2), dict(n_source=0), dict(n_source=3), dict(edge_mode=2),
-        dict(n_lens=0),
+        dict(n_lens=0), dict(mass_model=2), dict(mass_model=-1),
     ]
-    base = dict(ny=8, nx=8, pix_scale=0.1, supersample=2, n_lens_light=0, n_source=1, edge_mode=0, n_lens=1)
+    base = dict(ny=8, nx=8, pix_scale=0.1, supersample=2, n_lens_light=0, n_source=1, edge_mode=0, n_lens=1,
+                mass_model=0)
     lib = api.load()
     fp = C.POINTER(C.c_float)
     for b in bad:
         kw = dict(base); kw.update(b)
         cfg = api.tl_config(kw["ny"], kw["nx"], kw["pix_scale"], kw["supersample"], kw["n_lens_light"],
-                            kw["n_source"], kw["edge_mode"], kw["n_lens"])
+                            kw["n_source"], kw["edge_mode"], kw["n_lens"], kw["mass_model"])
         h = C.c_void_p(123)
         rc = lib.tl_create(C.byref(h), C.byref(cfg), psf.ctypes.data_as(fp), 3, 3,
                            data.ctypes.data_as(fp), noise.ctypes.data_as(fp), None)
