@@ -47,6 +47,10 @@ struct tl_ctx {
     void (*trace)(const tl::KArgs, int) = nullptr;
     size_t conv_smem = 0;
     int64_t chunk_rows = 0;       // rows per scratch chunk
+    // small-batch path of fused contexts (rows spread over many CTAs, bitwise equal to fused)
+    void (*sb_trace)(const tl::KArgs, int) = nullptr;
+    size_t sb_trace_smem = 0;
+    int sb_rowtab = 0, sb_max_rows = 0;
     double refine_tau = 7.5e-4;   // x S at create: a pixel averages S^2 samples
     // benchmark facility (tl_set_profiling): events around the dominant kernel of the last call
     int profile = 0;
@@ -99,6 +103,69 @@ tl::KArgs base_args(const tl_ctx *c)
     return a;
 }
 
+void fill_prologue_args(const tl_ctx *c, tl::PrologueArgs &pa, const float *params, tl::RowC *rows, int64_t nb, int64_t r0,
+                        int64_t rows_per_lens, int unit_amp)
+{
+    pa.params = params + r0 * c->P; pa.rows = rows; pa.sigma_min = c->sigma_min;
+    pa.B = nb; pa.row0 = r0; pa.rows_per_lens = rows_per_lens;
+    pa.P = c->P; pa.n_lens_light = c->cfg.n_lens_light; pa.n_source = c->cfg.n_source;
+    pa.S = c->cfg.supersample;
+    pa.mass_model = c->cfg.mass_model; pa.lens_np = c->lens_np;
+    pa.inv_u = 2.0 * c->cfg.supersample / c->cfg.pix_scale;
+    pa.fov_half = 0.5 * c->cfg.pix_scale * (c->He > c->We ? c->He : c->We);
+    pa.refine_tau = c->refine_tau;
+    pa.unit_amp = unit_amp;
+}
+
+// B <= n_sm / 2 rows on a fused context: prologue -> trace_kernel (rows x slabs) -> conv_small_kernel
+// (rows x bands) -> finalize_small_kernel; bitwise the fused kernel's result (tl_kernels.cuh)
+int run_small_batch(tl_ctx *c, const float *params, int64_t B, float *logL, float *images, cudaStream_t st)
+{
+    const int nb = (int)B;
+    const int npair = (c->cfg.ny + 1) / 2, nsx = (c->cfg.nx + 3) / 4;
+    // binned images, then one work-queue head per row; zeroed together
+    const size_t img_bytes = sizeof(float) * (size_t)nb * c->He * c->pitch;
+    const size_t ext_bytes = img_bytes + sizeof(int) * (size_t)nb;
+    tl::RowC *rows = nullptr;
+    float *ext = nullptr, *cblk = nullptr;
+    if (!cuda_ok(cudaMallocAsync(&rows, sizeof(tl::RowC) * (size_t)nb, st))) return TL_ENOMEM;
+    if (!cuda_ok(cudaMallocAsync(&ext, ext_bytes, st))) { cudaFreeAsync(rows, st); return TL_ENOMEM; }
+    if (logL && !cuda_ok(cudaMallocAsync(&cblk, sizeof(float) * (size_t)nb * npair * nsx, st))) {
+        cudaFreeAsync(rows, st); cudaFreeAsync(ext, st); return TL_ENOMEM;
+    }
+    cudaMemsetAsync(ext, 0, ext_bytes, st);          // pitch padding must read as finite zeros
+    tl::PrologueArgs pa;
+    fill_prologue_args(c, pa, params, rows, nb, 0, B / c->cfg.n_lens, 0);
+    tl::prologue_kernel<<<(unsigned)((nb * (1 + c->n_comp) + 127) / 128), 128, 0, st>>>(pa);
+    tl::KArgs a = base_args(c);
+    a.rows = rows; a.B = nb; a.rows_per_lens = B / c->cfg.n_lens; a.row0 = 0;
+    a.logL = logL; a.images = images; a.ext = ext; a.rowtab = c->sb_rowtab;
+    a.tile_counters = reinterpret_cast<int *>(reinterpret_cast<unsigned char *>(ext) + img_bytes);
+    // as many CTAs per row as are resident at once (two per SM; one more would start a second,
+    // nearly empty wave), but no more than there are warp tiles / row pairs
+    int want = 2 * c->n_sm / nb;
+    if (want < 1) want = 1;
+    const int n_wtiles = a.tiles_x * a.tiles_y;
+    int slabs = want < (n_wtiles + 7) / 8 ? want : (n_wtiles + 7) / 8;
+    int bands = want < npair ? want : npair;
+    // the whole band (+ K - 1 rows of halo) and the taps must fit in shared memory
+    const size_t fixed = sizeof(float) * ((size_t)c->K * c->Kp + c->pitch + c->Kp + 8);
+    int band_pairs = (npair + bands - 1) / bands;
+    const int max_pairs = (int)(((SMEM_LIMIT - fixed) / (sizeof(float) * c->pitch) - (c->K - 1)) / 2);
+    if (band_pairs > max_pairs) band_pairs = max_pairs;
+    bands = (npair + band_pairs - 1) / band_pairs;
+    const size_t conv_smem = fixed + sizeof(float) * (size_t)(2 * band_pairs + c->K - 1) * c->pitch;
+    if (c->profile) cudaEventRecord(c->ev0, st);
+    c->sb_trace<<<dim3((unsigned)nb, (unsigned)slabs), 256, c->sb_trace_smem, st>>>(a, nb);
+    if (c->profile) { cudaEventRecord(c->ev1, st); c->prof_pending = 1; }
+    tl::conv_small_kernel<<<dim3((unsigned)nb, (unsigned)bands), 256, conv_smem, st>>>(a, nb, band_pairs, cblk);
+    if (logL) tl::finalize_small_kernel<<<(unsigned)nb, c->threads, 0, st>>>(a, cblk);
+    const int rc = cuda_ok(cudaGetLastError()) ? TL_OK : TL_ECUDA;
+    cudaFreeAsync(rows, st); cudaFreeAsync(ext, st);
+    if (cblk) cudaFreeAsync(cblk, st);
+    return rc;
+}
+
 int run_batch(tl_ctx *c, const float *params, int64_t B, float *logL, float *images, cudaStream_t st)
 {
     if (!c || B < 0) return TL_EINVAL;
@@ -141,6 +208,7 @@ int run_batch(tl_ctx *c, const float *params, int64_t B, float *logL, float *ima
         cudaFreeAsync(pext, st);
         return prc;
     }
+    if (c->path == 0 && B <= c->sb_max_rows) return run_small_batch(c, params, B, logL, images, st);
     const int64_t chunk = c->chunk_rows < B ? c->chunk_rows : B;
     tl::RowC *rows = nullptr;
     float *ext = nullptr;
@@ -309,7 +377,7 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
     best_warp_tile(c->He, c->We, &c->CW, &c->CH);
     size_t fs = fused_smem_bytes(c);
     const size_t rowtab_bytes = sizeof(tl::RowV) * (size_t)c->He * cfg->supersample;
-    if (fs <= SMEM_LIMIT) {
+    if (fs <= SMEM_LIMIT && !std::getenv("TL_FORCE_SPLIT")) {
         // the row-value table is worth its shared memory unless it costs a resident CTA
         const size_t fs2 = ((fs + 15) & ~(size_t)15) + rowtab_bytes;
         const int per_sm_1 = (int)(SMEM_LIMIT / (fs + 1024)), per_sm_2 = (int)(SMEM_LIMIT / (fs2 + 1024));
@@ -327,6 +395,22 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
         if (!cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, c->fused, c->threads, fs)) || occ < 1) { tl_destroy(c); return TL_ECUDA; }
         c->ctas_per_sm = occ; c->grid = occ * c->n_sm;
         c->chunk_rows = CONST_CHUNK;
+        // small-batch path: needs a register-blocked PSF size and the whole image + taps in one CTA's shared memory
+        const bool kblk = c->K == 5 || c->K == 15 || c->K == 21 || c->K == 31 || c->K == 41;
+        // ... and a row long enough for three more launches to pay (measured: configs 1-3 gain, Tiny loses)
+        const int64_t samples_row = (int64_t)c->He * c->We * cfg->supersample * cfg->supersample;
+        if (kblk && samples_row >= 16384 && !std::getenv("TL_NO_SMALL_BATCH")) {
+            c->sb_trace = cfg->mass_model == TL_MASS_EPL ? tl_trace_epl_for(cfg->supersample, cfg->n_lens_light, cfg->n_source)
+                                                         : tl_trace_for(cfg->supersample, cfg->n_lens_light, cfg->n_source);
+            bool oks = cuda_ok(cudaFuncSetAttribute(tl::conv_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT));
+            if (rowtab_bytes <= 96 * 1024) {
+                c->sb_rowtab = 1; c->sb_trace_smem = rowtab_bytes;
+                oks = oks && cuda_ok(cudaFuncSetAttribute(c->sb_trace, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rowtab_bytes));
+            }
+            c->sb_max_rows = oks ? c->n_sm / 2 : 0;
+            if (const char *e = std::getenv("TL_SMALL_BATCH_ROWS")) c->sb_max_rows = oks ? std::atoi(e) : 0;
+            cudaGetLastError();
+        }
     } else {
         c->path = 1;
         // tile rows: as many as fit in ~100 KB so two CTAs share an SM

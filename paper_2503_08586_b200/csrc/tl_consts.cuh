@@ -104,10 +104,16 @@ struct PrologueArgs {
 __device__ inline double gamma_p_series(double a, double x, double *prefactor)
 {
     // P(a,x) = x^a e^-x / Gamma(a+1) * sum_{k>=0} x^k / ((a+1)...(a+k))
+    // eight terms per trip: the eight divisions are independent of the running product and
+    // pipeline, only the multiply-add chain is serial (the prologue is one thread per component
+    // and sits on the critical path of every call)
     double term = 1.0, sum = 1.0;
-    for (int k = 1; k < 4000; ++k) {
-        term *= x / (a + (double)k);
-        sum += term;
+    for (int k0 = 1; k0 < 4000; k0 += 8) {
+        double r[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j) r[j] = x / (a + (double)(k0 + j));
+#pragma unroll
+        for (int j = 0; j < 8; ++j) { term *= r[j]; sum += term; }
         if (term < sum * 1e-17) break;
     }
     double pf = exp(a * log(x) - x - lgamma(a + 1.0));

@@ -36,6 +36,7 @@ struct KArgs {
     int tile_rows, n_tiles;  // split path
     int CW, CH, tiles_x, tiles_y;   // phase-1 warp tiles (see trace_tiles)
     int rowtab;              // 1: the kernel's shared memory holds a RowV table (He * S entries)
+    int *tile_counters;      // small-batch path: [chunk] zeroed work-queue heads (one per row), else null
 };
 
 __device__ __forceinline__ bool row_is_valid(const RowC &rc, int n_comp)
@@ -625,7 +626,10 @@ __global__ void __launch_bounds__(256, 2) trace_kernel(const KArgs a, int chunk_
         if (!row_is_valid(rc_s, a.n_comp)) continue;
         if (rowtab) { fill_rowtab<NLL>(rc_s, a, rowtab); __syncthreads(); }
         float *dst = a.ext + (size_t)r * a.He * a.pitch;
-        trace_image<S_T, NLL, NSRC, MASS>(rc_s, a, rowtab, (blockIdx.y * blockDim.x + threadIdx.x) >> 5, (gridDim.y * blockDim.x) >> 5, nullptr,
+        // small batches: the row's CTAs draw warp tiles from one global queue, so a tile full of
+        // FP64-refined samples does not leave the other warps of the row waiting for its owner
+        trace_image<S_T, NLL, NSRC, MASS>(rc_s, a, rowtab, (blockIdx.y * blockDim.x + threadIdx.x) >> 5, (gridDim.y * blockDim.x) >> 5,
+                                    a.tile_counters ? a.tile_counters + r : nullptr,
                                     [&](int i, int j, float v) { dst[i * a.pitch + j] = v; });
     }
 }
@@ -682,6 +686,94 @@ __global__ void finalize_kernel(const KArgs a, int chunk_rows)
     for (int t = 0; t < a.n_tiles; ++t) s += a.partial[(size_t)r * a.n_tiles + t];
     const double ll = -0.5 * (s + a.lconst[row / a.rows_per_lens]);
     a.logL[row] = isfinite(s) ? (float)ll : -INFINITY;
+}
+
+// ------------------------------------------------------------------------------ small batches
+// (NEXT-4: the sampler hands over small proposal batches.)  With fewer rows
+// than SMs the fused path leaves most of the GPU idle and a call takes one row's time (0.18 ms on
+// configs[1]) whatever B.  Here a row is spread over many CTAs -- trace_kernel with as many slabs
+// as fill the GPU, then conv_small_kernel over bands of output row pairs, then
+// finalize_small_kernel -- and the result is BITWISE what the fused kernel gives: the pixel
+// values do not depend on which warp traces them, the 2 x 4 convolution blocks are the same
+// code, each block's chi^2 term is stored, and the final kernel adds them per thread and across
+// the CTA in exactly the fused kernel's order (same block size, same block_sum).
+template <int K>
+__device__ __forceinline__ void conv_blocks_store(const KArgs &a, const float *img, int e0, const float *taps, int p0, int p1,
+                                                  const float *data, const float *wgt, float *image_out, float *cblk)
+{
+    const int nsx = (a.nx + 3) / 4;
+    const int total = (p1 - p0) * nsx;
+    for (int s = threadIdx.x; s < total; s += blockDim.x) {
+        const int ip = s / nsx, xb = s - ip * nsx, i = 2 * (p0 + ip), x0 = xb * 4;
+        float a0[4], a1[4];
+        ConvBlock<K>::run(img + (i - e0) * a.pitch + x0, a.pitch, taps, a0, a1);
+        float c = chi2_strip(a, a0, i, x0, data, wgt, image_out);
+        if (i + 1 < a.ny) c += chi2_strip(a, a1, i + 1, x0, data, wgt, image_out);
+        if (cblk) cblk[(p0 + ip) * nsx + xb] = c;
+    }
+}
+
+// one CTA per (row, band of `band_pairs` output row pairs); cblk: [chunk][npair * nsx] or null
+__global__ void __launch_bounds__(256) conv_small_kernel(const KArgs a, int chunk_rows, int band_pairs, float *cblk)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float *taps = reinterpret_cast<float *>(smem_raw);
+    float *img = taps + a.K * a.Kp;
+    const int r = blockIdx.x;
+    const int npair = (a.ny + 1) / 2, nsx = (a.nx + 3) / 4;
+    const int p0 = blockIdx.y * band_pairs, p1 = min(npair, p0 + band_pairs);
+    if (p0 >= p1) return;
+    const int64_t row = a.row0 + r;
+    const int64_t lens = row / a.rows_per_lens;
+    const size_t npix = (size_t)a.ny * a.nx;
+    if (!row_is_valid(a.rows[r], a.n_comp)) {
+        if (a.images)
+            for (size_t i = (size_t)2 * p0 * a.nx + threadIdx.x; i < (size_t)min(a.ny, 2 * p1) * a.nx; i += blockDim.x)
+                a.images[row * npix + i] = NAN;
+        return;
+    }
+    load_psf(taps, a.psf + lens * a.K * a.Kp, a.K * a.Kp);
+    // extended rows 2 p0 .. 2 (p1 - 1) + K of this row's binned image (the last one may lie past
+    // the image when ny is odd: zeros), plus the slack the strips may touch
+    const int e0 = 2 * p0, erows = 2 * (p1 - p0) + a.K - 1, have = min(erows, a.He - e0);
+    const float4 *src = reinterpret_cast<const float4 *>(a.ext + ((size_t)r * a.He + e0) * a.pitch);
+    float4 *dst = reinterpret_cast<float4 *>(img);
+    const int n4 = have * a.pitch / 4;
+    for (int i = threadIdx.x; i < n4; i += blockDim.x) dst[i] = src[i];
+    for (int i = have * a.pitch + threadIdx.x; i < erows * a.pitch + a.pitch + a.Kp + 8; i += blockDim.x) img[i] = 0.f;
+    __syncthreads();
+    const float *data = a.logL ? a.data + lens * npix : nullptr;
+    float *image_out = a.images ? a.images + row * npix : nullptr;
+    float *cb = (a.logL && cblk) ? cblk + (size_t)r * npair * nsx : nullptr;
+#define TL_CONV_CASE(KK) \
+    case KK: conv_blocks_store<KK>(a, img, e0, taps, p0, p1, data, a.wgt + lens * npix, image_out, cb); break;
+    switch (a.K) {
+        TL_CONV_CASE(5)
+        TL_CONV_CASE(15)
+        TL_CONV_CASE(21)
+        TL_CONV_CASE(31)
+        TL_CONV_CASE(41)
+    default: break;
+    }
+#undef TL_CONV_CASE
+}
+
+// launched with the fused kernel's block size: per-thread partials and block_sum as in fused_kernel
+__global__ void finalize_small_kernel(const KArgs a, const float *cblk)
+{
+    __shared__ double red[32];
+    const int r = blockIdx.x;
+    const int64_t row = a.row0 + r;
+    if (!row_is_valid(a.rows[r], a.n_comp)) {
+        if (threadIdx.x == 0) a.logL[row] = -INFINITY;
+        return;
+    }
+    const int total = ((a.ny + 1) / 2) * ((a.nx + 3) / 4);
+    const float *cb = cblk + (size_t)r * total;
+    double part = 0.0;
+    for (int s = threadIdx.x; s < total; s += blockDim.x) part += (double)cb[s];
+    const double chi2 = block_sum(part, red);
+    if (threadIdx.x == 0) a.logL[row] = (float)(-0.5 * (chi2 + a.lconst[row / a.rows_per_lens]));
 }
 
 #endif  // TL_MAIN_TU
