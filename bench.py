@@ -337,9 +337,9 @@ def run_ours(args, w: W.Workload):
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": B * w.n_params * 4,
                 "d2h_bytes_per_step": B * 4, "api": "tl_loglike_batch_host (pinned host buffers)"},
-        "gpu_launches": info["launches_per_call"] * args.steps,
+        "gpu_launches": (4 if B <= info["small_batch_rows"] else info["launches_per_call"]) * args.steps,
         "roofline": {
-            "bound": "alu", "kernel": "fused_kernel" if info["path"] == 0 else "trace_kernel",
+            "bound": "alu", "kernel": "fused_kernel" if (info["path"] == 0 and B > info["small_batch_rows"]) else "trace_kernel",
             "achieved": achieved, "peak": peak, "unit": "Tinst/s", "frac": achieved / peak,
             "traffic": NCU_DRAM_BYTES_PER_LAUNCH if (w.mass_model == W.MASS_SIE and w.index == 1) else None,
             "peak_source": "derived: %d SMs x %d issue slots/clk x %.0f MHz (MEASURED_PEAKS.json sm_max_mhz; "
@@ -351,7 +351,8 @@ def run_ours(args, w: W.Workload):
                     "achieved_GBs": hbm_bytes / (k_ms * 1e-3) / 1e9,
                     "peak_GBs": peaks.get("hbm_gbs"), "note": "compute-bound by design; HBM traffic is negligible"},
         },
-        "launch": {k: info[k] for k in ("path", "block_threads", "ctas_per_sm", "grid", "smem_bytes")},
+        "launch": {**{k: info[k] for k in ("path", "block_threads", "ctas_per_sm", "grid", "smem_bytes")},
+                   "small_batch_path": bool(B <= info["small_batch_rows"])},
         "checksum_logL": logl_sum,
     }
     if world == 1 and not args.no_cpu_baseline:

@@ -99,6 +99,9 @@ typedef struct {
     int64_t conv_fma_per_row;  /* K*K*ny*nx                                                    */
     double  logl_const;        /* lens 0:  sum_i ln(2 pi sigma_i^2)                            */
     double  sigma_min;         /* lens 0:  min_i sigma_i                                       */
+    int32_t small_batch_rows;  /* calls with at most this many rows spread every row over many  */
+                               /* CTAs (see tl_loglike_batch); 0 = never                        */
+    int32_t reserved;
 } tl_info;
 
 /*
@@ -135,7 +138,11 @@ int tl_get_info(const tl_ctx *ctx, tl_info *info);
  *   B          rows (>= 0; multiple of n_lens)
  *   logL       DEVICE pointer, float [B], caller-owned, written
  *   cuda_stream  stream the kernels are enqueued on.  The call does NOT synchronise.
- * The result is bitwise reproducible (fixed-shape FP64 reduction, no atomics).
+ * The result is bitwise reproducible (fixed-shape FP64 reduction, no atomics), and the value of a
+ * row does not depend on the batch it is evaluated in: calls with few rows (at most
+ * tl_info.small_batch_rows = half the SM count, "CPU<->GPU" round trips of a sampler
+ * that proposes small batches) spread each row over many CTAs instead of one, 4 launches instead
+ * of 2, and return the same bits as a large batch does.
  */
 int tl_loglike_batch(tl_ctx *ctx, const float *params, int64_t B, float *logL, void *cuda_stream);
 
