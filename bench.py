@@ -322,10 +322,12 @@ def run_ours(args, w: W.Workload):
     peaks = measured_peaks()
     sm_max = float(peaks.get("sm_max_mhz", 1965.0))
     k_ms = float(np.mean(kern_ms))
-    achieved = om["issue_slots"] * B / (k_ms * 1e-3) / 1e12          # algorithmic Tinst/s
+    # a call of more than chunk_rows rows is several launches; the events are around the last one
+    k_rows = B - ((B - 1) // info["chunk_rows"]) * info["chunk_rows"]
+    achieved = om["issue_slots"] * k_rows / (k_ms * 1e-3) / 1e12     # algorithmic Tinst/s
     peak = info["n_sm"] * SM_FP32_LANES * sm_max * 1e6 / 1e12
-    mufu_frac = om["mufu_ops"] * B / (k_ms * 1e-3) / (info["n_sm"] * SM_MUFU_LANES * sm_max * 1e6)
-    fp32_frac = om["fp32_slots"] * B / (k_ms * 1e-3) / (info["n_sm"] * SM_FP32_LANES * sm_max * 1e6)
+    mufu_frac = om["mufu_ops"] * k_rows / (k_ms * 1e-3) / (info["n_sm"] * SM_MUFU_LANES * sm_max * 1e6)
+    fp32_frac = om["fp32_slots"] * k_rows / (k_ms * 1e-3) / (info["n_sm"] * SM_FP32_LANES * sm_max * 1e6)
     hbm_bytes = B * (w.n_params + 1) * 4 + (2 * w.ny * w.nx + w.psf_size ** 2) * 4 * w.n_lens
     line = {
         "metric": METRIC + mass_tag(w), "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -344,11 +346,11 @@ def run_ours(args, w: W.Workload):
             "traffic": NCU_DRAM_BYTES_PER_LAUNCH if (w.mass_model == W.MASS_SIE and w.index == 1) else None,
             "peak_source": "derived: %d SMs x %d issue slots/clk x %.0f MHz (MEASURED_PEAKS.json sm_max_mhz; "
                            "slots/clk measured, profiles/r1_mufu_accuracy.md)" % (info["n_sm"], SM_FP32_LANES, sm_max),
-            "kernel_ms": k_ms, "fp32_pipe_frac": fp32_frac, "mufu_pipe_frac": mufu_frac,
+            "kernel_ms": k_ms, "kernel_rows": k_rows, "fp32_pipe_frac": fp32_frac, "mufu_pipe_frac": mufu_frac,
             "algorithmic_issue_slots_per_likelihood": om["issue_slots"],
             **({"epl_mean_series_terms": epl_mean_terms(rows)} if w.mass_model == W.MASS_EPL else {}),
             "hbm": {"algorithmic_bytes_per_step": hbm_bytes,
-                    "achieved_GBs": hbm_bytes / (k_ms * 1e-3) / 1e9,
+                    "achieved_GBs": hbm_bytes * (k_rows / B) / (k_ms * 1e-3) / 1e9,
                     "peak_GBs": peaks.get("hbm_gbs"), "note": "compute-bound by design; HBM traffic is negligible"},
         },
         "launch": {**{k: info[k] for k in ("path", "block_threads", "ctas_per_sm", "grid", "smem_bytes")},

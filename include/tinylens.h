@@ -101,7 +101,8 @@ typedef struct {
     double  sigma_min;         /* lens 0:  min_i sigma_i                                       */
     int32_t small_batch_rows;  /* calls with at most this many rows spread every row over many  */
                                /* CTAs (see tl_loglike_batch); 0 = never                        */
-    int32_t reserved;
+    int32_t chunk_rows;        /* a call with more rows is processed in chunks of this many     */
+                               /* (one set of launches each, same stream)                       */
 } tl_info;
 
 /*

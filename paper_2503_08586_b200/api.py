@@ -42,7 +42,7 @@ class tl_info(C.Structure):
                 ("n_sm", C.c_int32), ("launches_per_call", C.c_int32),
                 ("samples_per_row", C.c_int64), ("conv_fma_per_row", C.c_int64),
                 ("logl_const", C.c_double), ("sigma_min", C.c_double),
-                ("small_batch_rows", C.c_int32), ("reserved", C.c_int32)]
+                ("small_batch_rows", C.c_int32), ("chunk_rows", C.c_int32)]
 
 
 _lib = None

@@ -487,7 +487,7 @@ int tl_get_info(const tl_ctx *c, tl_info *info)
     info->samples_per_row = hy * wx * c->cfg.supersample * c->cfg.supersample;
     info->conv_fma_per_row = (int64_t)c->K * c->K * c->cfg.ny * c->cfg.nx;
     info->logl_const = c->lconst0; info->sigma_min = c->sigma_min0;
-    info->small_batch_rows = c->path == 0 ? c->sb_max_rows : 0; info->reserved = 0;
+    info->small_batch_rows = c->path == 0 ? c->sb_max_rows : 0; info->chunk_rows = (int32_t)c->chunk_rows;
     return TL_OK;
 }
 
