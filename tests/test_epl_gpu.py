@@ -157,3 +157,16 @@ def test_epl_linear_mode(api, orc, idx, n_prior, n_near):
     tn = np.maximum(PT.logl_tol(oll), PT.fp32_floor(oimg, prob.data[lens], prob.noise[lens], w.supersample))
     dl = np.abs(ll - oll)
     assert np.all(dl <= tn), "EPL linear: worst %.3g x derived tol" % (dl / tn).max()
+
+
+@pytest.mark.parametrize("seed", range(8))
+def test_epl_random_shapes(api, orc, seed):
+    """The random geometries of tests/test_parity_gpu.py (odd / tiny sizes, S in 1..6, PSF sizes on
+    both convolution paths, both edge modes, 1-3 components) with the EPL mass model."""
+    from tests.test_parity_gpu import _random_case, _small_problem
+    rng = np.random.default_rng(2000 + seed)
+    w, prob = _small_problem(orc, index=40 + seed, mass_model=W.MASS_EPL, **_random_case(rng))
+    rows, isnear = PT.rows_with_near(W, w, prob, 6, 2)
+    ll, im, _ = _gpu(api, prob, rows)
+    oll, oim = PT.oracle_reference(orc, w, prob, rows)
+    _compare(w, prob, rows, np.ones(len(rows), bool), ll, im, oll, oim)

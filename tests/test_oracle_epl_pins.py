@@ -133,3 +133,25 @@ def test_linear_mode_uses_the_epl_layout():
     # at the truth the solved amplitudes are the true I_e up to the noise
     assert abs(amps[0] / row[8] - 1.0) < 0.05 and abs(amps[1] / row[15] - 1.0) < 0.25
     assert ll >= O.loglike(cfg, prob.psf[0], prob.data[0], prob.noise[0], row) - 1e-9
+
+
+def test_scaling_rotation_and_parity_symmetries():
+    """kappa is homogeneous of degree 1 - gamma, so alpha(lambda theta) = lambda^(2-gamma) alpha(theta);
+    rotating the lens and the position together rotates the deflection; alpha(-theta) = -alpha(theta)."""
+    rng = np.random.default_rng(9)
+    for _ in range(40):
+        g, q, phi = rng.uniform(1.2, 2.8), rng.uniform(0.2, 1.0), rng.uniform(0, math.pi)
+        x, y = rng.uniform(-2, 2, 2)
+        lam, rot = rng.uniform(0.3, 3.0), rng.uniform(0, 2 * math.pi)
+        ax, ay = O.epl_deflection(1.1, g, q, phi, 0.0, 0.0, x, y)
+        sx, sy = O.epl_deflection(1.1, g, q, phi, 0.0, 0.0, lam * x, lam * y)
+        f = lam ** (2.0 - g)
+        assert abs(sx - f * ax) < 1e-12 * (1 + abs(f * ax)) and abs(sy - f * ay) < 1e-12 * (1 + abs(f * ay))
+        c, s = math.cos(rot), math.sin(rot)
+        rx, ry = O.epl_deflection(1.1, g, q, phi + rot, 0.0, 0.0, c * x - s * y, s * x + c * y)
+        assert abs(rx - (c * ax - s * ay)) < 1e-12 and abs(ry - (s * ax + c * ay)) < 1e-12
+        mx, my = O.epl_deflection(1.1, g, q, phi, 0.0, 0.0, -x, -y)
+        assert abs(mx + ax) < 1e-14 and abs(my + ay) < 1e-14
+        # theta_E scaling: alpha is proportional to theta_E^(gamma-1)
+        tx, ty = O.epl_deflection(2.2, g, q, phi, 0.0, 0.0, x, y)
+        assert abs(tx - 2.0 ** (g - 1.0) * ax) < 1e-12 * (1 + abs(tx))
