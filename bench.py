@@ -339,7 +339,7 @@ def run_ours(args, w: W.Workload):
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": B * w.n_params * 4,
                 "d2h_bytes_per_step": B * 4, "api": "tl_loglike_batch_host (pinned host buffers)"},
-        "gpu_launches": (4 if B <= info["small_batch_rows"] else info["launches_per_call"]) * args.steps,
+        "gpu_launches": (3 if B <= info["small_batch_rows"] else info["launches_per_call"]) * args.steps,
         "roofline": {
             "bound": "alu", "kernel": "fused_kernel" if (info["path"] == 0 and B > info["small_batch_rows"]) else "trace_kernel",
             "achieved": achieved, "peak": peak, "unit": "Tinst/s", "frac": achieved / peak,

@@ -118,14 +118,14 @@ void fill_prologue_args(const tl_ctx *c, tl::PrologueArgs &pa, const float *para
 }
 
 // B <= n_sm / 2 rows on a fused context: prologue -> trace_kernel (rows x slabs) -> conv_small_kernel
-// (rows x bands) -> finalize_small_kernel; bitwise the fused kernel's result (tl_kernels.cuh)
+// (rows x bands; the row's last band reduces); bitwise the fused kernel's result (tl_kernels.cuh)
 int run_small_batch(tl_ctx *c, const float *params, int64_t B, float *logL, float *images, cudaStream_t st)
 {
     const int nb = (int)B;
     const int npair = (c->cfg.ny + 1) / 2, nsx = (c->cfg.nx + 3) / 4;
-    // binned images, then one work-queue head per row; zeroed together
+    // binned images, then one work-queue head and one finished-band counter per row; zeroed together
     const size_t img_bytes = sizeof(float) * (size_t)nb * c->He * c->pitch;
-    const size_t ext_bytes = img_bytes + sizeof(int) * (size_t)nb;
+    const size_t ext_bytes = img_bytes + 2 * sizeof(int) * (size_t)nb;     // + finished-band counters
     tl::RowC *rows = nullptr;
     float *ext = nullptr, *cblk = nullptr;
     if (!cuda_ok(cudaMallocAsync(&rows, sizeof(tl::RowC) * (size_t)nb, st))) return TL_ENOMEM;
@@ -151,15 +151,14 @@ int run_small_batch(tl_ctx *c, const float *params, int64_t B, float *logL, floa
     // the whole band (+ K - 1 rows of halo) and the taps must fit in shared memory
     const size_t fixed = sizeof(float) * ((size_t)c->K * c->Kp + c->pitch + c->Kp + 8);
     int band_pairs = (npair + bands - 1) / bands;
-    const int max_pairs = (int)(((SMEM_LIMIT - fixed) / (sizeof(float) * c->pitch) - (c->K - 1)) / 2);
+    const int max_pairs = (int)(((SMEM_LIMIT - 1024 - fixed) / (sizeof(float) * c->pitch) - (c->K - 1)) / 2);
     if (band_pairs > max_pairs) band_pairs = max_pairs;
     bands = (npair + band_pairs - 1) / band_pairs;
     const size_t conv_smem = fixed + sizeof(float) * (size_t)(2 * band_pairs + c->K - 1) * c->pitch;
     if (c->profile) cudaEventRecord(c->ev0, st);
     c->sb_trace<<<dim3((unsigned)nb, (unsigned)slabs), 256, c->sb_trace_smem, st>>>(a, nb);
     if (c->profile) { cudaEventRecord(c->ev1, st); c->prof_pending = 1; }
-    tl::conv_small_kernel<<<dim3((unsigned)nb, (unsigned)bands), 256, conv_smem, st>>>(a, nb, band_pairs, cblk);
-    if (logL) tl::finalize_small_kernel<<<(unsigned)nb, c->threads, 0, st>>>(a, cblk);
+    tl::conv_small_kernel<<<dim3((unsigned)nb, (unsigned)bands), c->threads, conv_smem, st>>>(a, nb, band_pairs, cblk);
     const int rc = cuda_ok(cudaGetLastError()) ? TL_OK : TL_ECUDA;
     cudaFreeAsync(rows, st); cudaFreeAsync(ext, st);
     if (cblk) cudaFreeAsync(cblk, st);
@@ -402,7 +401,7 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
         if (kblk && samples_row >= 16384 && !std::getenv("TL_NO_SMALL_BATCH")) {
             c->sb_trace = cfg->mass_model == TL_MASS_EPL ? tl_trace_epl_for(cfg->supersample, cfg->n_lens_light, cfg->n_source)
                                                          : tl_trace_for(cfg->supersample, cfg->n_lens_light, cfg->n_source);
-            bool oks = cuda_ok(cudaFuncSetAttribute(tl::conv_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT));
+            bool oks = cuda_ok(cudaFuncSetAttribute(tl::conv_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SMEM_LIMIT - 1024)));   // 1 KB: its static shared memory
             if (rowtab_bytes <= 96 * 1024) {
                 c->sb_rowtab = 1; c->sb_trace_smem = rowtab_bytes;
                 oks = oks && cuda_ok(cudaFuncSetAttribute(c->sb_trace, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rowtab_bytes));

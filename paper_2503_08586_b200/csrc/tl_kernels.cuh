@@ -692,11 +692,11 @@ __global__ void finalize_kernel(const KArgs a, int chunk_rows)
 // (NEXT-4: the sampler hands over small proposal batches.)  With fewer rows
 // than SMs the fused path leaves most of the GPU idle and a call takes one row's time (0.18 ms on
 // configs[1]) whatever B.  Here a row is spread over many CTAs -- trace_kernel with as many slabs
-// as fill the GPU, then conv_small_kernel over bands of output row pairs, then
-// finalize_small_kernel -- and the result is BITWISE what the fused kernel gives: the pixel
-// values do not depend on which warp traces them, the 2 x 4 convolution blocks are the same
-// code, each block's chi^2 term is stored, and the final kernel adds them per thread and across
-// the CTA in exactly the fused kernel's order (same block size, same block_sum).
+// as fill the GPU, then conv_small_kernel over bands of output row pairs -- and the result is
+// BITWISE what the fused kernel gives: the pixel values do not depend on which warp traces them,
+// the 2 x 4 convolution blocks are the same code, each block's chi^2 term is stored, and the
+// row's last CTA to finish (conv_small_kernel runs with the fused kernel's block size) adds them
+// per thread and across the CTA in exactly the fused kernel's order (same block_sum).
 template <int K>
 __device__ __forceinline__ void conv_blocks_store(const KArgs &a, const float *img, int e0, const float *taps, int p0, int p1,
                                                   const float *data, const float *wgt, float *image_out, float *cblk)
@@ -713,9 +713,12 @@ __device__ __forceinline__ void conv_blocks_store(const KArgs &a, const float *i
     }
 }
 
-// one CTA per (row, band of `band_pairs` output row pairs); cblk: [chunk][npair * nsx] or null
-__global__ void __launch_bounds__(256) conv_small_kernel(const KArgs a, int chunk_rows, int band_pairs, float *cblk)
+// one CTA per (row, band of `band_pairs` output row pairs); cblk: [chunk][npair * nsx] or null;
+// a.tile_counters[chunk_rows + r] (zeroed) counts the finished bands of row r
+__global__ void __launch_bounds__(512) conv_small_kernel(const KArgs a, int chunk_rows, int band_pairs, float *cblk)
 {
+    __shared__ double red[32];
+    __shared__ int is_last;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float *taps = reinterpret_cast<float *>(smem_raw);
     float *img = taps + a.K * a.Kp;
@@ -730,6 +733,7 @@ __global__ void __launch_bounds__(256) conv_small_kernel(const KArgs a, int chun
         if (a.images)
             for (size_t i = (size_t)2 * p0 * a.nx + threadIdx.x; i < (size_t)min(a.ny, 2 * p1) * a.nx; i += blockDim.x)
                 a.images[row * npix + i] = NAN;
+        if (a.logL && blockIdx.y == 0 && threadIdx.x == 0) a.logL[row] = -INFINITY;
         return;
     }
     load_psf(taps, a.psf + lens * a.K * a.Kp, a.K * a.Kp);
@@ -756,24 +760,20 @@ __global__ void __launch_bounds__(256) conv_small_kernel(const KArgs a, int chun
     default: break;
     }
 #undef TL_CONV_CASE
-}
-
-// launched with the fused kernel's block size: per-thread partials and block_sum as in fused_kernel
-__global__ void finalize_small_kernel(const KArgs a, const float *cblk)
-{
-    __shared__ double red[32];
-    const int r = blockIdx.x;
-    const int64_t row = a.row0 + r;
-    if (!row_is_valid(a.rows[r], a.n_comp)) {
-        if (threadIdx.x == 0) a.logL[row] = -INFINITY;
-        return;
-    }
-    const int total = ((a.ny + 1) / 2) * ((a.nx + 3) / 4);
-    const float *cb = cblk + (size_t)r * total;
+    if (!cb) return;
+    // the row's last band to finish reduces the stored terms: per-thread partials over
+    // s = tid, tid + blockDim, ... and block_sum, exactly as fused_kernel does
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) is_last = atomicAdd(a.tile_counters + chunk_rows + r, 1) == (int)gridDim.y - 1;
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    const int total = npair * nsx;
     double part = 0.0;
-    for (int s = threadIdx.x; s < total; s += blockDim.x) part += (double)cb[s];
+    for (int s = threadIdx.x; s < total; s += blockDim.x) part += (double)__ldcg(cb + s);
     const double chi2 = block_sum(part, red);
-    if (threadIdx.x == 0) a.logL[row] = (float)(-0.5 * (chi2 + a.lconst[row / a.rows_per_lens]));
+    if (threadIdx.x == 0) a.logL[row] = (float)(-0.5 * (chi2 + a.lconst[lens]));
 }
 
 #endif  // TL_MAIN_TU

@@ -170,3 +170,21 @@ def test_epl_random_shapes(api, orc, seed):
     ll, im, _ = _gpu(api, prob, rows)
     oll, oim = PT.oracle_reference(orc, w, prob, rows)
     _compare(w, prob, rows, np.ones(len(rows), bool), ll, im, oll, oim)
+
+
+def test_epl_full_size_csst_batch_sampled_against_oracle(api, orc):
+    """configs[1] with the EPL mass model at its full B = 4096, in the launch configuration
+    `bench.py --mass epl` times: every logL finite, a seeded sample of rows against the oracle."""
+    import torch
+    w = W.workload(1).with_epl()
+    prob = W.make_problem(w, orc.render_for_workloads)
+    rows = W.batch_rows(w)
+    ctx = api.LensContext.from_problem(prob)
+    ll = ctx.loglike(torch.from_numpy(rows).cuda()).cpu().numpy().astype(np.float64)
+    info = ctx.info()
+    ctx.close()
+    assert info["path"] == 0 and info["block_threads"] == 512 and len(ll) == 4096 > info["small_batch_rows"]
+    assert np.all(np.isfinite(ll))
+    pick = np.random.default_rng(17).choice(4096, 24, replace=False)
+    oll, _ = orc.loglike_batch(orc.config_of(w), prob.psf, prob.data, prob.noise, rows[pick])
+    assert np.all(np.abs(ll[pick] - oll) <= PT.logl_tol(oll))
