@@ -65,6 +65,14 @@ def lib():
         L.orc_loglike_linear.restype = d; L.orc_loglike_linear.argtypes = [cp, fp, i32, fp, fp, fp, dp]
         L.orc_loglike_linear_batch.restype = i32
         L.orc_loglike_linear_batch.argtypes = [cp, i32, fp, i32, fp, fp, fp, i64, dp, dp, i32]
+        L.orc_gauss.restype = d; L.orc_gauss.argtypes = [d] * 7
+        L.orc_mge_row_valid.restype = i32; L.orc_mge_row_valid.argtypes = [cp, fp]
+        L.orc_mge_component_images.restype = i32
+        L.orc_mge_component_images.argtypes = [cp, fp, i32, fp, fp, i32, dp]
+        L.orc_nnls_enum.restype = None; L.orc_nnls_enum.argtypes = [i32, dp, dp, dp]
+        L.orc_loglike_mge.restype = d; L.orc_loglike_mge.argtypes = [cp, fp, i32, fp, fp, fp, fp, i32, dp]
+        L.orc_loglike_mge_batch.restype = i32
+        L.orc_loglike_mge_batch.argtypes = [cp, i32, fp, i32, fp, fp, fp, i64, fp, i32, dp, dp, i32]
         _lib = L
     return _lib
 
@@ -245,4 +253,44 @@ def loglike_linear_batch(cfg: OrcConfig, psf, data, noise, rows, n_lens: int = 1
     amps = np.empty((B, cfg.n_lens_light + cfg.n_source), np.float64)
     lib().orc_loglike_linear_batch(C.byref(cfg), int(n_lens), _fp(p), int(p.shape[-1]), _fp(d), _fp(s), _fp(r),
                                    B, _dp(out), _dp(amps), int(threads))
+    return out, amps
+
+
+# ---- NEXT-3: MGE lens light with linear amplitudes (reading G23) -----------
+
+def gauss(sigma, q, phi, cx, cy, x, y) -> float:
+    return lib().orc_gauss(sigma, q, phi, cx, cy, x, y)
+
+
+def nnls_enum(G, b) -> np.ndarray:
+    G = np.ascontiguousarray(G, dtype=np.float64); b = np.ascontiguousarray(b, dtype=np.float64)
+    n = b.size
+    s = np.zeros(n, np.float64)
+    lib().orc_nnls_enum(int(n), _dp(G), _dp(b), _dp(s))
+    return s
+
+
+def mge_component_images(cfg: OrcConfig, psf, row, sigmas) -> np.ndarray:
+    p, r, sg = _f32(psf), _f32(row), _f32(sigmas)
+    out = np.full((sg.size + cfg.n_source, cfg.ny, cfg.nx), np.nan, np.float64)
+    lib().orc_mge_component_images(C.byref(cfg), _fp(p), int(p.shape[-1]), _fp(r), _fp(sg), int(sg.size), _dp(out))
+    return out
+
+
+def loglike_mge(cfg: OrcConfig, psf, data, noise, row, sigmas):
+    """(logL at the NNLS amplitudes, amplitudes [n_gauss + n_source])."""
+    p, d, s, r, sg = _f32(psf), _f32(data), _f32(noise), _f32(row), _f32(sigmas)
+    amps = np.empty(sg.size + cfg.n_source, np.float64)
+    ll = lib().orc_loglike_mge(C.byref(cfg), _fp(p), int(p.shape[-1]), _fp(d), _fp(s), _fp(r), _fp(sg), int(sg.size),
+                               _dp(amps))
+    return ll, amps
+
+
+def loglike_mge_batch(cfg: OrcConfig, psf, data, noise, rows, sigmas, n_lens: int = 1, threads: int = 0):
+    p, d, s, r, sg = _f32(psf), _f32(data), _f32(noise), _f32(rows), _f32(sigmas)
+    B = r.shape[0]
+    out = np.empty(B, np.float64)
+    amps = np.empty((B, sg.size + cfg.n_source), np.float64)
+    lib().orc_loglike_mge_batch(C.byref(cfg), int(n_lens), _fp(p), int(p.shape[-1]), _fp(d), _fp(s), _fp(r), B,
+                                _fp(sg), int(sg.size), _dp(out), _dp(amps), int(threads))
     return out, amps

@@ -530,3 +530,213 @@ int orc_loglike_linear_batch(const orc_config *cfg, int n_lens, const float *psf
 #endif
     return used;
 }
+
+/* ================================================================== NEXT-3: MGE lens light
+ * PAPER.md:291-293 (section 4.3): "we have implemented the Multiple Gaussian Expansion (MGE)
+ * model, which can describe arbitrary radial profiles ... in lens galaxies".  The paper gives
+ * no formula; reading G23: the lens light is a sum of n_g elliptical Gaussians on
+ * the ellipses R_p of PAPER.md:143-148 Eq. 10, sharing one centre and one (q, phi),
+ *     I_l(theta) = sum_k a_k exp( -R_p(theta)^2 / (2 sigma_k^2) ),
+ * with fixed dispersions sigma_k (arcsec) and amplitudes a_k >= 0 that are linear parameters
+ * (PAPER.md:86-93 Eq. 6, :97-129 Eq. 7): together with the N_s source amplitudes they are the
+ * non-negative least-squares minimiser of || (M s - d) / n ||^2, M = B [G_1 .. G_ng | L_s],
+ * and logL is Eq. 5 at that optimum.
+ *
+ * The row is the usual one with n_lens_light = 1; of the lens-light block only e1, e2, cx, cy
+ * (entries 3..6) are read -- I_e, r_e, n (0..2) are ignored.  The I_e of the sources is ignored
+ * too (as in orc_loglike_linear).
+ *
+ * NNLS by its definition, as orc_nnls_small: every support is tried, the normal equations are
+ * solved on it, and of the feasible candidates the one with the smallest penalty
+ * s'Gs - 2b's (evaluated explicitly) wins.  2^n supports: the oracle takes n <= 16 columns.
+ */
+#define ORC_MGE_MAXCOL 16
+
+/* one elliptical Gaussian of unit central brightness on the ellipses of Eq. 10 */
+double orc_gauss(double sigma, double q, double phi, double cx, double cy, double x, double y)
+{
+    double c = cos(phi), s = sin(phi);
+    double x1 = (x - cx) * c + (y - cy) * s;
+    double x2 = -(x - cx) * s + (y - cy) * c;
+    double rp2 = x1 * x1 * q + x2 * x2 / q;
+    return exp(-rp2 / (2.0 * sigma * sigma));
+}
+
+/* validity for the MGE call: lens block and sources as orc_row_valid (source I_e ignored),
+ * lens-light block: only its shape and centre are read                                    */
+int orc_mge_row_valid(const orc_config *cfg, const float *row)
+{
+    if (cfg->n_lens_light != 1) return 0;
+    int LP = lens_np(cfg), ncomp = 1 + cfg->n_source;
+    for (int i = 0; i < LP; ++i) if (!isfinite((double)row[i])) return 0;
+    if (row[0] < 0.0f) return 0;
+    if (hypot((double)row[1], (double)row[2]) >= 1.0) return 0;
+    if (cfg->mass_model == ORC_MASS_EPL && !(row[7] > 1.0f && row[7] < 3.0f)) return 0;
+    const float *l = row + LP;
+    for (int i = 3; i < 7; ++i) if (!isfinite((double)l[i])) return 0;
+    if (hypot((double)l[3], (double)l[4]) >= 1.0) return 0;
+    for (int k = 1; k < ncomp; ++k) {
+        const float *s = row + LP + 7 * k;
+        for (int i = 1; i < 7; ++i) if (!isfinite((double)s[i])) return 0;
+        if (!(s[1] > 0.0f) || !(s[2] > 0.0f)) return 0;
+        if (hypot((double)s[3], (double)s[4]) >= 1.0) return 0;
+    }
+    return 1;
+}
+
+/* columns of M: n_gauss blurred unit-amplitude Gaussians, then the N_s blurred unit-amplitude
+ * sources.  M[(n_gauss + n_source)][ny*nx].  Returns 0 for an invalid row.                  */
+int orc_mge_component_images(const orc_config *cfg, const float *psf, int K, const float *row,
+                             const float *sigmas, int n_gauss, double *M)
+{
+    if (!orc_mge_row_valid(cfg, row)) return 0;
+    int LP = lens_np(cfg), S = cfg->supersample, ny = cfg->ny, nx = cfg->nx;
+    size_t n = (size_t)ny * nx;
+    int g = halo_of(cfg, K), hy = ny + 2 * g, wx = nx + 2 * g;
+    double s = cfg->pix_scale, q, phi;
+    const float *l = row + LP;
+    orc_shape(l[3], l[4], &q, &phi);
+    double *ext = (double *)malloc(sizeof(double) * (size_t)hy * wx);
+    for (int k = 0; k < n_gauss; ++k) {
+        for (int i = 0; i < hy; ++i) {
+            double yi = (i - g - (ny - 1) / 2.0) * s;
+            for (int j = 0; j < wx; ++j) {
+                double xj = (j - g - (nx - 1) / 2.0) * s;
+                double acc = 0.0;
+                for (int a = 0; a < S; ++a) {
+                    double y = yi + ((a + 0.5) / S - 0.5) * s;
+                    for (int b = 0; b < S; ++b) {
+                        double x = xj + ((b + 0.5) / S - 0.5) * s;
+                        acc += orc_gauss((double)sigmas[k], q, phi, l[5], l[6], x, y);
+                    }
+                }
+                ext[(size_t)i * wx + j] = acc / (double)(S * S);             /* bin: mean */
+            }
+        }
+        orc_convolve(ny, nx, g, ext, psf, K, M + (size_t)k * n);            /* Eq. 3 */
+    }
+    free(ext);
+    /* sources through the plain forward model: a harmless lens-light Sersic of amplitude 0 */
+    float tmp[8 + 7 * 8];
+    int P = LP + 7 * (1 + cfg->n_source);
+    for (int ks = 0; ks < cfg->n_source; ++ks) {
+        memcpy(tmp, row, sizeof(float) * (size_t)P);
+        tmp[LP + 0] = 0.0f; tmp[LP + 1] = 1.0f; tmp[LP + 2] = 1.0f;
+        for (int j = 0; j < cfg->n_source; ++j) tmp[LP + 7 * (1 + j)] = (j == ks) ? 1.0f : 0.0f;
+        if (!orc_render(cfg, psf, K, tmp, M + (size_t)(n_gauss + ks) * n)) return 0;
+    }
+    return 1;
+}
+
+/* minimise s'G s - 2 b's over s >= 0, n <= ORC_MGE_MAXCOL, by enumeration of the supports */
+void orc_nnls_enum(int n, const double *G, const double *b, double *s_out)
+{
+    double best = 0.0;                                   /* empty support: s = 0 */
+    for (int i = 0; i < n; ++i) s_out[i] = 0.0;
+    if (n > ORC_MGE_MAXCOL) { for (int i = 0; i < n; ++i) s_out[i] = NAN; return; }
+    for (long mask = 1; mask < (1L << n); ++mask) {
+        int idx[ORC_MGE_MAXCOL], m = 0;
+        for (int i = 0; i < n; ++i) if (mask & (1L << i)) idx[m++] = i;
+        double A[ORC_MGE_MAXCOL][ORC_MGE_MAXCOL + 1];
+        for (int r = 0; r < m; ++r) {
+            for (int c = 0; c < m; ++c) A[r][c] = G[idx[r] * n + idx[c]];
+            A[r][m] = b[idx[r]];
+        }
+        int singular = 0;
+        for (int c = 0; c < m && !singular; ++c) {       /* Gaussian elimination, partial pivoting */
+            int p = c;
+            for (int r = c + 1; r < m; ++r) if (fabs(A[r][c]) > fabs(A[p][c])) p = r;
+            if (!(fabs(A[p][c]) > 1e-300)) { singular = 1; break; }
+            if (p != c) for (int k = 0; k <= m; ++k) { double t = A[c][k]; A[c][k] = A[p][k]; A[p][k] = t; }
+            for (int r = c + 1; r < m; ++r) {
+                double f = A[r][c] / A[c][c];
+                for (int k = c; k <= m; ++k) A[r][k] -= f * A[c][k];
+            }
+        }
+        if (singular) continue;
+        double x[ORC_MGE_MAXCOL];
+        int feasible = 1;
+        for (int r = m - 1; r >= 0; --r) {
+            double t = A[r][m];
+            for (int k = r + 1; k < m; ++k) t -= A[r][k] * x[k];
+            x[r] = t / A[r][r];
+        }
+        for (int r = 0; r < m; ++r) if (!(x[r] >= 0.0)) feasible = 0;
+        if (!feasible) continue;
+        double f = 0.0;                                  /* the penalty itself, not its stationary form */
+        for (int r = 0; r < m; ++r) {
+            double gx = 0.0;
+            for (int c = 0; c < m; ++c) gx += G[idx[r] * n + idx[c]] * x[c];
+            f += x[r] * (gx - 2.0 * b[idx[r]]);
+        }
+        if (f < best) {
+            best = f;
+            for (int i = 0; i < n; ++i) s_out[i] = 0.0;
+            for (int r = 0; r < m; ++r) s_out[idx[r]] = x[r];
+        }
+    }
+}
+
+double orc_loglike_mge(const orc_config *cfg, const float *psf, int K, const float *data, const float *noise,
+                       const float *row, const float *sigmas, int n_gauss, double *amps)
+{
+    int C = n_gauss + cfg->n_source;
+    size_t n = (size_t)cfg->ny * cfg->nx;
+    for (int k = 0; k < C; ++k) if (amps) amps[k] = NAN;
+    if (C > ORC_MGE_MAXCOL || !orc_mge_row_valid(cfg, row)) return -INFINITY;
+    double *M = (double *)malloc(sizeof(double) * n * (size_t)C);
+    double *model = (double *)malloc(sizeof(double) * n);
+    orc_mge_component_images(cfg, psf, K, row, sigmas, n_gauss, M);
+    double G[ORC_MGE_MAXCOL * ORC_MGE_MAXCOL], b[ORC_MGE_MAXCOL], s[ORC_MGE_MAXCOL];
+    for (int k = 0; k < C; ++k) {
+        double bk = 0.0;
+        for (size_t i = 0; i < n; ++i) bk += M[k * n + i] * (double)data[i] / ((double)noise[i] * noise[i]);
+        b[k] = bk;
+        for (int l = 0; l < C; ++l) {
+            double gg = 0.0;
+            for (size_t i = 0; i < n; ++i) gg += M[k * n + i] * M[l * n + i] / ((double)noise[i] * noise[i]);
+            G[k * C + l] = gg;
+        }
+    }
+    orc_nnls_enum(C, G, b, s);
+    for (size_t i = 0; i < n; ++i) {
+        double m = 0.0;
+        for (int k = 0; k < C; ++k) m += s[k] * M[k * n + i];
+        model[i] = m;
+    }
+    double ll = orc_loglike_from_image(model, data, noise, n);     /* Eq. 5 at the optimal amplitudes (Eq. 6) */
+    if (amps) for (int k = 0; k < C; ++k) amps[k] = s[k];
+    free(M); free(model);
+    return ll;
+}
+
+int orc_loglike_mge_batch(const orc_config *cfg, int n_lens, const float *psf, int K, const float *data,
+                          const float *noise, const float *rows, int64_t B, const float *sigmas, int n_gauss,
+                          double *logl, double *amps, int threads)
+{
+    int C = n_gauss + cfg->n_source, P = lens_np(cfg) + 7 * (1 + cfg->n_source);
+    size_t n = (size_t)cfg->ny * cfg->nx;
+    int64_t per = B / (n_lens > 0 ? n_lens : 1);
+    int used = 1;
+#ifdef _OPENMP
+    if (threads > 0) omp_set_num_threads(threads);
+#pragma omp parallel
+    {
+#pragma omp single
+        used = omp_get_num_threads();
+#pragma omp for schedule(dynamic, 1)
+        for (int64_t r = 0; r < B; ++r) {
+            int64_t l = n_lens > 1 ? r / per : 0;
+            logl[r] = orc_loglike_mge(cfg, psf + (size_t)l * K * K, K, data + l * n, noise + l * n,
+                                      rows + r * P, sigmas, n_gauss, amps ? amps + r * C : NULL);
+        }
+    }
+#else
+    for (int64_t r = 0; r < B; ++r) {
+        int64_t l = n_lens > 1 ? r / per : 0;
+        logl[r] = orc_loglike_mge(cfg, psf + (size_t)l * K * K, K, data + l * n, noise + l * n,
+                                  rows + r * P, sigmas, n_gauss, amps ? amps + r * C : NULL);
+    }
+#endif
+    return used;
+}
