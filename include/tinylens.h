@@ -174,6 +174,44 @@ int tl_loglike_linear_batch(tl_ctx *ctx, const float *params, int64_t B, float *
                             void *cuda_stream);
 
 /*
+ * MGE lens light with linear amplitudes (section 4.3: "we have implemented the
+ * Multiple Gaussian Expansion (MGE) model, which can describe arbitrary radial profiles ... in
+ * lens galaxies"; the paper gives no formula -- reading G23 of DESIGN.md).  The lens light is
+ *     I_l(theta) = sum_{k < n_gauss} a_k exp( -R_p(theta)^2 / (2 sigma_k^2) ),
+ * R_p on the ellipses of PAPER.md:143-148 Eq. 10 with one centre and one (e1, e2) for the whole
+ * set, fixed dispersions sigma_k, and the a_k >= 0 are linear parameters solved per row together
+ * with the source amplitudes (PAPER.md:86-93 Eq. 6, :97-129 Eq. 7), as in
+ * tl_loglike_linear_batch but with n_gauss + n_source columns.
+ *
+ * tl_set_mge -- define the Gaussian set of a context created with n_lens_light = 1.
+ *   sigmas     HOST pointer, float [n_gauss], arcsec, finite and > 0 (copied)
+ *   n_gauss    1 .. 16
+ * Synchronous; not thread-safe with respect to calls in flight on the same context.  May be
+ * called again to change the set.  TL_OK, TL_EINVAL (also: n_lens_light != 1), TL_ESIZE,
+ * TL_ENOMEM or TL_ECUDA.
+ *
+ * tl_mge_columns -- n_gauss + n_source (the width of `amps`), or < 0 when no set is defined.
+ *
+ * tl_loglike_mge_batch -- logL[r] = Eq. 5 at the NNLS-optimal amplitudes of row r.
+ *   params   DEVICE pointer, float [B][P], the context's usual row layout; of the lens-light
+ *            block only e1, e2, cx, cy (entries +3..+6) are read -- its I_e, r_e, n and the
+ *            I_e of the sources are ignored and may hold anything
+ *   logL     DEVICE pointer, float [B], written (-INFINITY for invalid rows)
+ *   amps     DEVICE pointer, float [B][n_gauss + n_source] (Gaussians in the order of sigmas,
+ *            then sources), written (NaN for invalid rows), or NULL.  Neighbouring Gaussians are
+ *            nearly collinear, so individual amplitudes are ill-conditioned; logL and the
+ *            fitted image M s are not.
+ * Asynchronous on cuda_stream; bitwise reproducible (fixed-order FP64 sums, no atomics).  The
+ * NNLS problem is solved on the Gram matrix by the active-set iteration of Bro & De Jong
+ * (PAPER.md:123-129).  Returns TL_OK, TL_EINVAL (no set defined, bad pointers, B not a
+ * multiple of n_lens), TL_ENOMEM, TL_ECUDA or TL_ESIZE.
+ */
+int tl_set_mge(tl_ctx *ctx, const float *sigmas, int32_t n_gauss);
+int tl_mge_columns(const tl_ctx *ctx);
+int tl_loglike_mge_batch(tl_ctx *ctx, const float *params, int64_t B, float *logL, float *amps,
+                         void *cuda_stream);
+
+/*
  * tl_loglike_batch_host -- end-to-end convenience for a host-side sampler (PAPER.md:250 names
  * the CPU<->GPU transfers as part of the cost): copies params (HOST, float [B][P], ideally
  * pinned) to the device, runs tl_loglike_batch, copies logL back to logL (HOST, float [B]),

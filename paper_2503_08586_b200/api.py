@@ -72,6 +72,9 @@ def load(build_if_missing: bool = True):
     L.tl_render_batch.restype = C.c_int; L.tl_render_batch.argtypes = [vp, vp, i64, vp, vp]
     L.tl_loglike_batch_host.restype = C.c_int; L.tl_loglike_batch_host.argtypes = [vp, vp, i64, vp, vp]
     L.tl_loglike_linear_batch.restype = C.c_int; L.tl_loglike_linear_batch.argtypes = [vp, vp, i64, vp, vp, vp]
+    L.tl_set_mge.restype = C.c_int; L.tl_set_mge.argtypes = [vp, fp, i32]
+    L.tl_mge_columns.restype = C.c_int; L.tl_mge_columns.argtypes = [vp]
+    L.tl_loglike_mge_batch.restype = C.c_int; L.tl_loglike_mge_batch.argtypes = [vp, vp, i64, vp, vp, vp]
     L.tl_set_precision.restype = C.c_int; L.tl_set_precision.argtypes = [vp, C.c_int]
     L.tl_set_profiling.restype = C.c_int; L.tl_set_profiling.argtypes = [vp, C.c_int]
     L.tl_last_kernel_ms.restype = C.c_int; L.tl_last_kernel_ms.argtypes = [vp, C.POINTER(C.c_float)]
@@ -188,6 +191,33 @@ def tl_loglike_linear_batch(handle: int, params, n_comp: int, out=None, amps=Non
     return out, amps
 
 
+def tl_set_mge(handle: int, sigmas):
+    """sigmas: host float32 [n_gauss] (arcsec) -- the Gaussian set of the MGE lens light."""
+    sg = _f32c(sigmas).reshape(-1)
+    _check(load().tl_set_mge(handle, sg.ctypes.data_as(C.POINTER(C.c_float)), int(sg.size)), "tl_set_mge")
+
+
+def tl_mge_columns(handle: int) -> int:
+    return load().tl_mge_columns(handle)
+
+
+def tl_loglike_mge_batch(handle: int, params, out=None, amps=None, want_amps=True, stream=None):
+    """params: CUDA float32 [B,P] -> (logL CUDA float32 [B], amplitudes CUDA float32 [B,n_gauss+n_source] or None)."""
+    import torch
+    B = _dev_rows(handle, params)
+    n_col = tl_mge_columns(handle)
+    if n_col < 0:
+        raise TinyLensError(TL_EINVAL, "tl_loglike_mge_batch (no Gaussian set: call tl_set_mge)")
+    if out is None:
+        out = torch.empty(B, dtype=torch.float32, device=params.device)
+    if amps is None and want_amps:
+        amps = torch.empty((B, n_col), dtype=torch.float32, device=params.device)
+    _check(load().tl_loglike_mge_batch(handle, params.data_ptr(), B, out.data_ptr(),
+                                       amps.data_ptr() if amps is not None else None, _stream_handle(stream)),
+           "tl_loglike_mge_batch")
+    return out, amps
+
+
 def tl_loglike_batch_host(handle: int, params_host, out_host=None, stream=None):
     """params_host: host float32 [B,P] (torch CPU tensor, ideally pinned, or numpy) -> host logL [B].
     Host->device copy, kernels, device->host copy and a stream synchronise, all inside the call."""
@@ -254,6 +284,12 @@ class LensContext:
 
     def loglike_linear(self, params, out=None, amps=None, want_amps=True, stream=None):
         return tl_loglike_linear_batch(self.handle, params, self.n_comp, out, amps, want_amps, stream)
+
+    def set_mge(self, sigmas):
+        tl_set_mge(self.handle, sigmas)
+
+    def loglike_mge(self, params, out=None, amps=None, want_amps=True, stream=None):
+        return tl_loglike_mge_batch(self.handle, params, out, amps, want_amps, stream)
 
     def loglike_host(self, params_host, out_host=None, stream=None):
         return tl_loglike_batch_host(self.handle, params_host, out_host, stream)

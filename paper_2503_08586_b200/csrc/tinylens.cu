@@ -16,6 +16,7 @@
 #include "tl_kernels.cuh"
 #include "tl_dispatch.h"
 #include "tl_precise.cuh"
+#include "tl_mge.cuh"
 
 #define TL_VERSION_STRING "tinylens-b200 0.2 (sm_100a)"
 
@@ -51,6 +52,9 @@ struct tl_ctx {
     void (*sb_trace)(const tl::KArgs, int) = nullptr;
     size_t sb_trace_smem = 0;
     int sb_rowtab = 0, sb_max_rows = 0;
+    // MGE mode (tl_set_mge / tl_loglike_mge_batch)
+    float *mge_c = nullptr;       // device [n_gauss]: log2(e) / (2 sigma_k^2)
+    int n_gauss = 0;
     double refine_tau = 7.5e-4;   // x S at create: a pixel averages S^2 samples
     // benchmark facility (tl_set_profiling): events around the dominant kernel of the last call
     int profile = 0;
@@ -114,7 +118,7 @@ void fill_prologue_args(const tl_ctx *c, tl::PrologueArgs &pa, const float *para
     pa.inv_u = 2.0 * c->cfg.supersample / c->cfg.pix_scale;
     pa.fov_half = 0.5 * c->cfg.pix_scale * (c->He > c->We ? c->He : c->We);
     pa.refine_tau = c->refine_tau;
-    pa.unit_amp = unit_amp;
+    pa.unit_amp = unit_amp; pa.mge = 0;
 }
 
 // B <= n_sm / 2 rows on a fused context: prologue -> trace_kernel (rows x slabs) -> conv_small_kernel
@@ -236,7 +240,7 @@ int run_batch(tl_ctx *c, const float *params, int64_t B, float *logL, float *ima
         pa.inv_u = 2.0 * c->cfg.supersample / c->cfg.pix_scale;
         pa.fov_half = 0.5 * c->cfg.pix_scale * (c->He > c->We ? c->He : c->We);
         pa.refine_tau = c->refine_tau;
-        pa.unit_amp = 0;
+        pa.unit_amp = 0; pa.mge = 0;
         const int64_t nthr = nb * (1 + c->n_comp);
         tl::prologue_kernel<<<(unsigned)((nthr + 127) / 128), 128, 0, st>>>(pa);
 
@@ -531,7 +535,7 @@ int tl_loglike_linear_batch(tl_ctx *c, const float *params, int64_t B, float *lo
             pa.inv_u = 2.0 * c->cfg.supersample / c->cfg.pix_scale;
             pa.fov_half = 0.5 * c->cfg.pix_scale * (c->He > c->We ? c->He : c->We);
             pa.refine_tau = c->refine_tau;
-            pa.unit_amp = 1;
+            pa.unit_amp = 1; pa.mge = 0;
             const int64_t nthr = nb * (1 + c->n_comp);
             tl::prologue_kernel<<<(unsigned)((nthr + 127) / 128), 128, 0, st>>>(pa);
             tl::KArgs a = base_args(c);
@@ -575,7 +579,7 @@ int tl_loglike_linear_batch(tl_ctx *c, const float *params, int64_t B, float *lo
         pa.inv_u = 2.0 * c->cfg.supersample / c->cfg.pix_scale;
         pa.fov_half = 0.5 * c->cfg.pix_scale * (c->He > c->We ? c->He : c->We);
         pa.refine_tau = c->refine_tau;
-        pa.unit_amp = 1;
+        pa.unit_amp = 1; pa.mge = 0;
         const int64_t nthr = nb * (1 + c->n_comp);
         tl::prologue_kernel<<<(unsigned)((nthr + 127) / 128), 128, 0, st>>>(pa);
         tl::KArgs a = base_args(c);
@@ -589,6 +593,90 @@ int tl_loglike_linear_batch(tl_ctx *c, const float *params, int64_t B, float *lo
         dim3 cg((unsigned)nb, (unsigned)c->lin_n_tiles, (unsigned)NC);
         tl::conv_lin_kernel<<<cg, 256, c->lin_conv_smem, st>>>(a, (int)nb);
         tl::solve_lin_kernel<<<(unsigned)nb, 256, 0, st>>>(a, (int)nb);
+        if (!cuda_ok(cudaGetLastError())) rc = TL_ECUDA;
+    }
+    cudaFreeAsync(rows, st); cudaFreeAsync(ext, st); cudaFreeAsync(mimg, st);
+    return rc;
+}
+
+int tl_set_mge(tl_ctx *c, const float *sigmas, int32_t n_gauss)
+{
+    if (!c || !sigmas || n_gauss < 1 || n_gauss > tl::MGE_MAX_GAUSS) return TL_EINVAL;
+    if (c->cfg.n_lens_light != 1) return TL_EINVAL;
+    if (!c->trace_lin) return TL_ESIZE;
+    float ck[tl::MGE_MAX_GAUSS];
+    for (int k = 0; k < n_gauss; ++k) {
+        if (!std::isfinite(sigmas[k]) || !(sigmas[k] > 0.f)) return TL_EINVAL;
+        ck[k] = (float)(1.4426950408889634074 / (2.0 * (double)sigmas[k] * (double)sigmas[k]));
+        if (!std::isfinite(ck[k])) return TL_EINVAL;
+    }
+    int dev = -1;
+    if (!cuda_ok(cudaGetDevice(&dev))) return TL_ECUDA;
+    if (dev != c->device && !cuda_ok(cudaSetDevice(c->device))) return TL_ECUDA;
+    if (!c->mge_c && !cuda_ok(cudaMalloc(&c->mge_c, sizeof(float) * tl::MGE_MAX_GAUSS))) return TL_ENOMEM;
+    if (!cuda_ok(cudaMemcpy(c->mge_c, ck, sizeof(float) * n_gauss, cudaMemcpyHostToDevice))) return TL_ECUDA;
+    c->n_gauss = n_gauss;
+    return TL_OK;
+}
+
+int tl_mge_columns(const tl_ctx *c) { return (c && c->n_gauss > 0) ? c->n_gauss + c->cfg.n_source : TL_EINVAL; }
+
+int tl_loglike_mge_batch(tl_ctx *c, const float *params, int64_t B, float *logL, float *amps, void *cuda_stream)
+{
+    if (!c || B < 0) return TL_EINVAL;
+    if (c->n_gauss < 1) return TL_EINVAL;
+    if (B == 0) return TL_OK;
+    if (!params || !logL || (B % c->cfg.n_lens)) return TL_EINVAL;
+    if (!c->trace_lin) return TL_ESIZE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = -1;
+    if (!cuda_ok(cudaGetDevice(&dev))) return TL_ECUDA;
+    if (dev != c->device && !cuda_ok(cudaSetDevice(c->device))) return TL_ECUDA;
+    const int NG = c->n_gauss, NC = NG + c->cfg.n_source;
+    const size_t npix = (size_t)c->cfg.ny * c->cfg.nx;
+    const size_t ext_row = sizeof(float) * (size_t)NC * c->He * c->pitch, m_row = sizeof(float) * NC * npix;
+    int64_t chunk = (int64_t)(EXT_SCRATCH_BYTES / (ext_row + m_row));
+    if (chunk < 1) chunk = 1;
+    if (chunk > 65535) chunk = 65535;
+    if (chunk > B) chunk = B;
+    tl::RowC *rows = nullptr;
+    float *ext = nullptr, *mimg = nullptr;
+    if (!cuda_ok(cudaMallocAsync(&rows, sizeof(tl::RowC) * (size_t)chunk, st))) return TL_ENOMEM;
+    if (!cuda_ok(cudaMallocAsync(&ext, ext_row * (size_t)chunk, st)) ||
+        !cuda_ok(cudaMallocAsync(&mimg, m_row * (size_t)chunk, st))) {
+        cudaFreeAsync(rows, st);
+        if (ext) cudaFreeAsync(ext, st);
+        return TL_ENOMEM;
+    }
+    cudaMemsetAsync(ext, 0, ext_row * (size_t)chunk, st);      // pitch padding must read as finite zeros
+    const int64_t rows_per_lens = B / c->cfg.n_lens;
+    int gslabs = (c->He * c->We + 255) / 256;
+    if (gslabs > 16) gslabs = 16;
+    int rc = TL_OK;
+    for (int64_t r0 = 0; r0 < B && rc == TL_OK; r0 += chunk) {
+        const int64_t nb = (B - r0 < chunk) ? (B - r0) : chunk;
+        tl::PrologueArgs pa;
+        fill_prologue_args(c, pa, params, rows, nb, r0, rows_per_lens, 1);
+        pa.mge = 1;
+        const int64_t nthr = nb * (1 + c->n_comp);
+        tl::prologue_kernel<<<(unsigned)((nthr + 127) / 128), 128, 0, st>>>(pa);
+        tl::KArgs a = base_args(c);
+        a.rows = rows; a.B = nb; a.rows_per_lens = rows_per_lens; a.row0 = r0;
+        a.logL = logL; a.amps = amps; a.ext = ext; a.mimg = mimg;
+        a.tile_rows = c->lin_tile_rows; a.n_tiles = c->lin_n_tiles; a.rowtab = c->lin_rowtab;
+        // trace_lin_kernel writes its 1 + n_source components from slot NG - 1 on: the (unused)
+        // Sersic stand-in of the lens light lands on slot NG - 1, which mge_gauss_kernel then
+        // overwrites with the last Gaussian; the sources land on slots NG, NG + 1
+        a.ext_nc = NC; a.ext_k0 = NG - 1; a.n_gauss = NG; a.mge_c = c->mge_c;
+        dim3 tg((unsigned)nb, 8);
+        c->trace_lin<<<tg, 256, c->lin_trace_smem, st>>>(a, (int)nb);
+        dim3 gg((unsigned)nb, (unsigned)gslabs);
+        tl::mge_gauss_kernel<<<gg, 256, 0, st>>>(a, (int)nb);
+        dim3 cg((unsigned)nb, (unsigned)c->lin_n_tiles, (unsigned)NC);
+        if (c->profile) cudaEventRecord(c->ev0, st);
+        tl::conv_lin_kernel<<<cg, 256, c->lin_conv_smem, st>>>(a, (int)nb);
+        if (c->profile) { cudaEventRecord(c->ev1, st); c->prof_pending = 1; }
+        tl::solve_mge_kernel<<<(unsigned)nb, 256, 0, st>>>(a, (int)nb);
         if (!cuda_ok(cudaGetLastError())) rc = TL_ECUDA;
     }
     cudaFreeAsync(rows, st); cudaFreeAsync(ext, st); cudaFreeAsync(mimg, st);
@@ -643,6 +731,7 @@ void tl_destroy(tl_ctx *c)
     if (!c) return;
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
+    cudaFree(c->mge_c);
     cudaFree(c->psf); cudaFree(c->data); cudaFree(c->wgt); cudaFree(c->noise); cudaFree(c->sigma_min); cudaFree(c->lconst);
     delete c;
 }

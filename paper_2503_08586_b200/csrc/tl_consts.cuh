@@ -96,6 +96,8 @@ struct PrologueArgs {
     double fov_half;                 // arcsec, half the extended field of view
     double refine_tau;               // refinement threshold in units of sigma_min
     int unit_amp;                    // linear-amplitude mode: every I_e is taken as 1
+    int mge;                         // MGE mode (tl_loglike_mge_batch): of the lens-light block only e1, e2, cx, cy are
+                                     // read; its quadratic form becomes t = R_p^2 in arcsec^2 (r_e := 1, n := 1)
 };
 
 // ---- b_n of PAPER.md:139 Eq. 9:  P(2n, b_n) = 1/2 ---------------------------------------
@@ -286,11 +288,13 @@ __global__ void __launch_bounds__(128) prologue_kernel(PrologueArgs a)
     const float *sp = p + LP + 7 * k;
     SersicC C;
     bool ok = true;
-    for (int i = a.unit_amp ? 1 : 0; i < 7; ++i) ok = ok && isfinite(sp[i]);
+    const bool mge_shape = a.mge && is_lens_light;
+    for (int i = mge_shape ? 3 : (a.unit_amp ? 1 : 0); i < 7; ++i) ok = ok && isfinite(sp[i]);
     // linear mode: unit amplitude; the row's own I_e (when usable) only scales the refinement
     // criterion, as a hint of the magnitude the solved amplitude will have
     const double Ie_hint = (isfinite(sp[0]) && fabsf(sp[0]) > 1.f) ? fabs((double)sp[0]) : 1.0;
     double Ie = a.unit_amp ? 1.0 : (double)sp[0], re = sp[1], n = sp[2], qs = 1.0, cs = 1.0, ss = 0.0;
+    if (mge_shape) { Ie = 1.0; re = 1.0; n = 1.0; }
     ok = ok && (re > 0.0) && (n > 0.0);
     ok = ok && shape_from_e(sp[3], sp[4], &qs, &cs, &ss);
     if (!ok) { Ie = 0.0; re = 1.0; n = 1.0; qs = 1.0; cs = 1.0; ss = 0.0; }

@@ -37,6 +37,10 @@ struct KArgs {
     int CW, CH, tiles_x, tiles_y;   // phase-1 warp tiles (see trace_tiles)
     int rowtab;              // 1: the kernel's shared memory holds a RowV table (He * S entries)
     int *tile_counters;      // small-batch path: [chunk] zeroed work-queue heads (one per row), else null
+    // MGE mode (tl_mge.cuh): ext / mimg hold ext_nc = n_gauss + n_source components per row;
+    // trace_lin_kernel writes its components from slot ext_k0 on (0, 0 = the linear-mode layout)
+    int ext_nc, ext_k0, n_gauss;
+    const float *mge_c;      // [n_gauss] log2(e) / (2 sigma_k^2), arcsec^-2
 };
 
 __device__ __forceinline__ bool row_is_valid(const RowC &rc, int n_comp)
@@ -793,7 +797,7 @@ __global__ void __launch_bounds__(256, 2) trace_lin_kernel(const KArgs a, int ch
         __syncthreads();
         if (!row_is_valid(rc_s, a.n_comp)) continue;
         if (rowtab) { fill_rowtab<NLL>(rc_s, a, rowtab); __syncthreads(); }
-        float *dst = a.ext + (size_t)r * NC * a.He * a.pitch;
+        float *dst = a.ext + ((size_t)r * (a.ext_nc ? a.ext_nc : NC) + a.ext_k0) * a.He * a.pitch;
         const size_t comp_stride = (size_t)a.He * a.pitch;
         trace_image_lin<S_T, NLL, NSRC, MASS>(rc_s, a, rowtab, (blockIdx.y * blockDim.x + threadIdx.x) >> 5, (gridDim.y * blockDim.x) >> 5, nullptr,
                                       [&](int i, int j, int k, float v) { dst[k * comp_stride + i * a.pitch + j] = v; });

@@ -1,0 +1,234 @@
+// tl_mge.cuh -- NEXT-3: MGE lens light with linear amplitudes (tl_loglike_mge_batch).
+//
+// PAPER.md:291-293 (section 4.3) names the Multiple Gaussian Expansion; reading G23:
+//     I_l(theta) = sum_k a_k exp(-R_p(theta)^2 / (2 sigma_k^2)),   R_p of PAPER.md:143-148 Eq. 10,
+// one centre and one (q, phi) for the set, fixed sigma_k, and the a_k >= 0 solved together with
+// the source amplitudes as the NNLS minimiser of PAPER.md:86-93 Eq. 6 / :97-129 Eq. 7.
+//
+// Pipeline per chunk of rows (all on one stream; included by tinylens.cu only):
+//   prologue_kernel (mge = 1)  lens-light quadratic form becomes t = R_p^2 in arcsec^2
+//   trace_lin_kernel           ray-traced unit-amplitude source images -> component slots n_gauss..
+//   mge_gauss_kernel           the n_gauss binned Gaussians -> component slots 0..n_gauss-1
+//   conv_lin_kernel            every component blurred with the PSF (columns of M)
+//   solve_mge_kernel           G = M'WM, b = M'Wd in FP64 (fixed summation order), NNLS by the
+//                              Gram-matrix active-set iteration of Bro & De Jong (the paper's
+//                              solver), chi^2 of the residual d - M s -> logL
+#pragma once
+#include "tl_kernels.cuh"
+
+namespace tl {
+
+constexpr int MGE_MAX_GAUSS = 16;
+constexpr int MGE_MAX_COL = MGE_MAX_GAUSS + 2;       // + n_source
+constexpr int MGE_TILE = 64;                         // pixels staged per step of the Gram reduction
+
+// One thread per extended native pixel (grid.x = row in chunk, grid.y = slabs of the image).
+// t = R_p^2 is evaluated exactly like the lens-light term of col_values / row_values (hi/lo
+// constants, exact first differences), each Gaussian is one FMUL + MUFU.EX2 per sub-sample.
+__global__ void __launch_bounds__(256) mge_gauss_kernel(const KArgs a, int chunk_rows)
+{
+    const int r = blockIdx.x;
+    if (r >= chunk_rows) return;
+    const RowC &rc = a.rows[r];
+    if (!row_is_valid(rc, a.n_comp)) return;
+    const SersicC &C = rc.comp[0];
+    const float cXh = C.cXh, cXl = C.cXl, cYh = C.cYh, cYl = C.cYl;
+    const float ah = C.ah, al = C.al, b2h = C.b2h, b2l = C.b2l, cch = C.cch, ccl = C.ccl;
+    const int ng = a.n_gauss, S = a.S;
+    float ck[MGE_MAX_GAUSS];
+#pragma unroll
+    for (int k = 0; k < MGE_MAX_GAUSS; ++k) ck[k] = k < ng ? -a.mge_c[k] : 0.f;
+    const float inv_s2 = 1.f / (float)(S * S);
+    const size_t comp_stride = (size_t)a.He * a.pitch;
+    float *dst = a.ext + (size_t)r * a.ext_nc * comp_stride;
+    const int npx = a.He * a.We;
+    for (int p = blockIdx.y * blockDim.x + threadIdx.x; p < npx; p += gridDim.y * blockDim.x) {
+        const int i = p / a.We, j = p - i * a.We;
+        float acc[MGE_MAX_GAUSS];
+#pragma unroll
+        for (int k = 0; k < MGE_MAX_GAUSS; ++k) acc[k] = 0.f;
+        const bool edge = a.edge_zero && (j < a.h || j >= a.We - a.h || i < a.h || i >= a.He - a.h);
+        if (!edge) {
+            const float X0 = (float)(2 * j * S + 1 - S * a.We), Y0 = (float)(2 * i * S + 1 - S * a.He);
+#pragma unroll 1
+            for (int sa = 0; sa < S; ++sa) {
+                const float dyl = ((Y0 + (float)(2 * sa)) - cYh) - cYl;
+                const float y2 = dyl * dyl;
+                const float LC = fmaf(cch, y2, ccl * y2);
+#pragma unroll 1
+                for (int sb = 0; sb < S; ++sb) {
+                    const float dxl = ((X0 + (float)(2 * sb)) - cXh) - cXl;
+                    const float x2 = dxl * dxl;
+                    const float LA = fmaf(ah, x2, al * x2);
+                    const float LB = fmaf(dxl, b2h, dxl * b2l);
+                    const float t = fmaf(LB, dyl, LA + LC);
+#pragma unroll
+                    for (int k = 0; k < MGE_MAX_GAUSS; ++k)
+                        if (k < ng) acc[k] += mufu_ex2(t * ck[k]);
+                }
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < MGE_MAX_GAUSS; ++k)
+            if (k < ng) dst[k * comp_stride + (size_t)i * a.pitch + j] = acc[k] * inv_s2;
+    }
+}
+
+// minimise s'G s - 2 b's over s >= 0 (n <= MGE_MAX_COL) -- one thread.  Active-set iteration on
+// the Gram matrix (Lawson & Hanson; in this cross-product form Bro & De Jong's "fast NNLS"):
+// the passive set P grows by the column with the largest positive gradient w = b - G s, the
+// unconstrained problem on P is solved by Cholesky, and a step towards it that would leave the
+// feasible region is cut at the boundary, the columns that reach 0 leaving P.
+// G is [n][ldg]; L (scratch) [MGE_MAX_COL][MGE_MAX_COL]; dwd = d'Wd sets the scale of "zero".
+__device__ inline void nnls_gram(int n, const double *G, int ldg, const double *b, double dwd, double *s,
+                                 double *L, double *z)
+{
+    int idx[MGE_MAX_COL];
+    int m = 0;
+    unsigned passive = 0u, banned = 0u;
+    for (int i = 0; i < n; ++i) s[i] = 0.0;
+    const double eps = 1e-10;
+    for (int outer = 0; outer < 3 * n + 3; ++outer) {
+        int j = -1;
+        double wbest = 0.0;
+        for (int i = 0; i < n; ++i) {
+            if ((passive | banned) & (1u << i)) continue;
+            double w = b[i];
+            for (int k = 0; k < n; ++k) w -= G[i * ldg + k] * s[k];
+            const double thr = eps * sqrt(fmax(G[i * ldg + i] * dwd, 0.0));
+            if (w > thr && w > wbest) { wbest = w; j = i; }
+        }
+        if (j < 0) break;
+        passive |= 1u << j;
+        bool first = true, added = true;
+        for (int inner = 0; inner <= n; ++inner) {
+            m = 0;
+            for (int i = 0; i < n; ++i) if (passive & (1u << i)) idx[m++] = i;
+            // Cholesky G_PP = L L'
+            bool pd = true;
+            for (int r = 0; r < m && pd; ++r) {
+                for (int c = 0; c <= r; ++c) {
+                    double v = G[idx[r] * ldg + idx[c]];
+                    for (int k = 0; k < c; ++k) v -= L[r * MGE_MAX_COL + k] * L[c * MGE_MAX_COL + k];
+                    if (c == r) {
+                        if (!(v > 1e-13 * G[idx[r] * ldg + idx[r]])) { pd = false; break; }
+                        L[r * MGE_MAX_COL + r] = sqrt(v);
+                    } else L[r * MGE_MAX_COL + c] = v / L[c * MGE_MAX_COL + c];
+                }
+            }
+            if (pd) {
+                for (int r = 0; r < m; ++r) {
+                    double v = b[idx[r]];
+                    for (int k = 0; k < r; ++k) v -= L[r * MGE_MAX_COL + k] * z[k];
+                    z[r] = v / L[r * MGE_MAX_COL + r];
+                }
+                for (int r = m - 1; r >= 0; --r) {
+                    double v = z[r];
+                    for (int k = r + 1; k < m; ++k) v -= L[k * MGE_MAX_COL + r] * z[k];
+                    z[r] = v / L[r * MGE_MAX_COL + r];
+                }
+            }
+            if (first) {
+                // the entering column must come out positive; if it is numerically dependent on P
+                // (or rounding makes it non-positive) it is set aside until P changes
+                int pj = 0;
+                for (int r = 0; r < m; ++r) if (idx[r] == j) pj = r;
+                if (!pd || !(z[pj] > 0.0)) { passive &= ~(1u << j); banned |= 1u << j; added = false; break; }
+                first = false;
+            } else if (!pd) break;                       // cannot happen for a subset of a PD set; keep s
+            double alpha = 2.0;
+            int rmin = -1;
+            for (int r = 0; r < m; ++r)
+                if (!(z[r] > 0.0)) {
+                    const double si = s[idx[r]];
+                    const double al = si / (si - z[r]);
+                    if (al < alpha) { alpha = al; rmin = r; }
+                }
+            if (rmin < 0) {                               // all positive: accept
+                for (int r = 0; r < m; ++r) s[idx[r]] = z[r];
+                break;
+            }
+            for (int r = 0; r < m; ++r) {
+                const int i = idx[r];
+                s[i] += alpha * (z[r] - s[i]);
+                if (r == rmin || !(s[i] > 0.0)) { s[i] = 0.0; passive &= ~(1u << i); }
+            }
+        }
+        if (added) banned = 0u;
+    }
+}
+
+// one CTA of 256 threads per row.  Thread p < n_pairs owns one entry of [G | b | d'Wd]: the
+// pixels are staged through shared memory MGE_TILE at a time (w m_k and m_k, d as doubles) and
+// every entry is summed over the pixels in index order, so the result is bitwise reproducible.
+__global__ void __launch_bounds__(256) solve_mge_kernel(const KArgs a, int chunk_rows)
+{
+    constexpr int NCP = MGE_MAX_COL + 1;
+    __shared__ double As[MGE_TILE][NCP];               // w_i m_ki   (column n: w_i d_i)
+    __shared__ double Bs[MGE_TILE][NCP];               // m_ki       (column n: d_i)
+    __shared__ double Gs[MGE_MAX_COL][NCP];            // G, column n = b
+    __shared__ double Ls[MGE_MAX_COL * MGE_MAX_COL];
+    __shared__ double zs[MGE_MAX_COL], ss[MGE_MAX_COL], bs[MGE_MAX_COL];
+    __shared__ double red[32];
+    __shared__ double dwd_s;
+    const int r = blockIdx.x;
+    if (r >= chunk_rows) return;
+    const int64_t row = a.row0 + r;
+    const int n = a.ext_nc;
+    if (!row_is_valid(a.rows[r], a.n_comp)) {
+        if (threadIdx.x == 0) {
+            a.logL[row] = -INFINITY;
+            if (a.amps) for (int k = 0; k < n; ++k) a.amps[row * n + k] = NAN;
+        }
+        return;
+    }
+    const int64_t lens = row / a.rows_per_lens;
+    const int npix = a.ny * a.nx;
+    const float *M = a.mimg + (size_t)r * n * npix;
+    const float *d = a.data + lens * (size_t)npix, *w = a.wgt + lens * (size_t)npix;
+    // pair owned by this thread: (k, l) with k <= l <= n, k <= n  (l = n: the data column)
+    const int n1 = n + 1, n_pairs = n1 * (n1 + 1) / 2;
+    int pk = -1, pl = -1;
+    {
+        int p = threadIdx.x, k = 0;
+        if (p < n_pairs) {
+            while (p >= n1 - k) { p -= n1 - k; ++k; }
+            pk = k; pl = k + p;
+        }
+    }
+    double acc = 0.0;
+    for (int t0 = 0; t0 < npix; t0 += MGE_TILE) {
+        __syncthreads();
+        for (int e = threadIdx.x; e < MGE_TILE * n1; e += blockDim.x) {
+            const int k = e / MGE_TILE, ii = e - k * MGE_TILE, i = t0 + ii;
+            double v = 0.0, wv = 0.0;
+            if (i < npix) { v = k < n ? (double)M[(size_t)k * npix + i] : (double)d[i]; wv = (double)w[i] * v; }
+            As[ii][k] = wv; Bs[ii][k] = v;
+        }
+        __syncthreads();
+        if (pk >= 0) {
+#pragma unroll 8
+            for (int ii = 0; ii < MGE_TILE; ++ii) acc = fma(As[ii][pk], Bs[ii][pl], acc);
+        }
+    }
+    if (pk >= 0) {
+        if (pk < n && pl < n) { Gs[pk][pl] = acc; Gs[pl][pk] = acc; }
+        else if (pk < n) { Gs[pk][n] = acc; bs[pk] = acc; }
+        else dwd_s = acc;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) nnls_gram(n, &Gs[0][0], NCP, bs, dwd_s, ss, Ls, zs);
+    __syncthreads();
+    double part = 0.0;
+    for (int i = threadIdx.x; i < npix; i += blockDim.x) {
+        double m = 0.0;
+        for (int k = 0; k < n; ++k) m += ss[k] * (double)M[(size_t)k * npix + i];
+        const double res = (double)d[i] - m;
+        part += res * res * (double)w[i];
+    }
+    const double chi2 = block_sum(part, red);
+    if (threadIdx.x == 0) a.logL[row] = (float)(-0.5 * (chi2 + a.lconst[lens]));
+    if (a.amps && threadIdx.x < n) a.amps[row * n + threadIdx.x] = (float)ss[threadIdx.x];
+}
+
+}  // namespace tl

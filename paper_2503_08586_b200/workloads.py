@@ -110,6 +110,15 @@ WORKLOADS = (
 )
 
 
+def mge_sigmas(w: Workload, n_gauss: int = 10) -> np.ndarray:
+    """Dispersions (arcsec, float32) of the MGE lens-light set used by the tests and bench.py
+    --mode mge: log-spaced from 0.6 native pixels to half the field of view (input recipe,
+    DESIGN.md section 13; the paper gives no set)."""
+    lo = 0.6 * w.pix_scale
+    hi = 0.5 * w.pix_scale * max(w.ny, w.nx)
+    return np.geomspace(lo, hi, int(n_gauss)).astype(np.float32)
+
+
 def workload(index_or_name) -> Workload:
     for w in WORKLOADS:
         if w.index == index_or_name or w.name == index_or_name:

@@ -1,0 +1,136 @@
+"""GPU parity of tl_loglike_mge_batch (NEXT-3: MGE lens light with linear amplitudes,
+PAPER.md:291-293 reading G23, amplitudes by PAPER.md:86-129 Eq. 6-7) against the oracle."""
+import numpy as np
+import pytest
+
+from paper_2503_08586_b200 import workloads as W
+from tests import parity as PT
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def api():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_2503_08586_b200 import api as _api
+    _api.load()
+    return _api
+
+
+def _check(api, orc, w, prob, rows, sigmas, amp_rtol=None):
+    import torch
+    ctx = api.LensContext.from_problem(prob)
+    ctx.set_mge(sigmas)
+    d = torch.from_numpy(rows).cuda()
+    ll, amps = ctx.loglike_mge(d)
+    ll2, _ = ctx.loglike_mge(d, want_amps=False)
+    torch.cuda.synchronize()
+    assert torch.equal(ll, ll2)                      # bitwise reproducible
+    ctx.close()
+    ll = ll.cpu().numpy().astype(np.float64); amps = amps.cpu().numpy().astype(np.float64)
+    cfg = orc.config_of(w)
+    oll, oamps = orc.loglike_mge_batch(cfg, prob.psf, prob.data, prob.noise, rows, sigmas, n_lens=w.n_lens)
+    n_col = len(sigmas) + w.n_source
+    assert amps.shape == (len(rows), n_col)
+    assert np.all(np.isfinite(ll)) and np.all(amps >= 0.0)
+    per = len(rows) // w.n_lens
+    lens = np.arange(len(rows)) // per
+    dl = np.abs(ll - oll)
+    tol = PT.logl_tol(oll)
+    worst_fit = 0.0
+    floors = np.empty(len(rows))
+    for r in range(len(rows)):
+        M = orc.mge_component_images(cfg, prob.psf[lens[r]], rows[r], sigmas)
+        oimg = np.tensordot(oamps[r], M, axes=1)
+        floors[r] = PT.fp32_floor(oimg[None], prob.data[lens[r]][None], prob.noise[lens[r]][None], w.supersample)[0]
+        # what is unique: the fitted image M s.  The GPU's amplitudes, put through the ORACLE's
+        # columns, must reach the oracle's optimum (neighbouring Gaussians are nearly collinear,
+        # so the amplitudes themselves are compared only when the set is well separated)
+        gimg = np.tensordot(amps[r], M, axes=1)
+        ll_at = orc.loglike_from_image(gimg, prob.data[lens[r]], prob.noise[lens[r]])
+        assert ll_at <= oll[r] + 1e-9 * abs(oll[r])                 # the oracle's is the maximum
+        assert oll[r] - ll_at <= max(tol[r], floors[r]), (r, oll[r] - ll_at, tol[r], floors[r])
+        worst_fit = max(worst_fit, np.abs(gimg - oimg).max() / oimg.max())
+    assert worst_fit <= 1e-4, worst_fit                             # fitted image, relative to its peak
+    tn = np.maximum(tol, floors)
+    assert np.all(dl <= tn), "MGE logL parity: worst %.3g x derived tol (%.3g x north-star)" % ((dl / tn).max(), (dl / tol).max())
+    if amp_rtol is not None:
+        scale = np.maximum(np.abs(oamps).max(axis=1, keepdims=True), 1e-30)
+        assert np.all(np.abs(amps - oamps) <= amp_rtol * scale), np.abs((amps - oamps) / scale).max()
+    print("%s MGE (%d columns): logL %.3g x north-star tol, %.3g x derived; fitted image %.2e x peak"
+          % (w.name, n_col, (dl / tol).max(), (dl / tn).max(), worst_fit))
+    return ll, amps, oll, oamps
+
+
+def test_mge_small_image_well_separated_set(api, orc):
+    """Odd-sized image with a ragged tail, sigmas a factor 3 apart: amplitudes are well conditioned."""
+    w = W.Workload(index=9, name="mge-small", ny=37, nx=45, pix_scale=0.12, supersample=2, psf_size=7,
+                   psf_kind="gaussian", psf_fwhm=0.3, psf_beta=0.0, n_lens_light=1, n_source=1,
+                   noise_bg=0.05, noise_exptime=100.0, source_amp=(1.0, 20.0), batch=24)
+    prob = W.make_problem(w, orc.render_for_workloads)
+    rows, _ = PT.rows_with_near(W, w, prob, 16, 8)
+    rows[::3, 7] = np.nan; rows[1::3, 8] = -1.0; rows[2::3, 9] = np.inf     # ignored entries
+    rows[::2, 14] = np.nan
+    sigmas = np.array([0.1, 0.3, 0.9, 2.7], np.float32)
+    _check(api, orc, w, prob, rows, sigmas, amp_rtol=2e-4)
+
+
+@pytest.mark.parametrize("idx,n_prior,n_near,n_lens,n_gauss", [(1, 6, 6, 1, 10), (3, 4, 4, 3, 8), (4, 1, 1, 1, 6)])
+def test_mge_matches_oracle_on_configs(api, orc, idx, n_prior, n_near, n_lens, n_gauss):
+    w = W.workload(idx).scaled(batch=n_lens * n_prior, n_lens=n_lens)
+    prob = W.make_problem(w, orc.render_for_workloads)
+    rows, _ = PT.rows_with_near(W, w, prob, n_prior, n_near)
+    _check(api, orc, w, prob, rows, W.mge_sigmas(w, n_gauss))
+
+
+def test_mge_zero_edge_and_epl(api, orc):
+    from dataclasses import replace
+    w = replace(W.workload(1).with_epl().scaled(batch=6), ny=40, nx=52, psf_size=9, edge_mode=1)
+    prob = W.make_problem(w, orc.render_for_workloads)
+    rows = W.batch_rows(w, 6)
+    _check(api, orc, w, prob, rows, W.mge_sigmas(w, 7))
+
+
+def test_mge_recovers_known_amplitudes_and_flags_invalid_rows(api, orc):
+    import torch
+    w = W.Workload(index=9, name="mge-rec", ny=48, nx=48, pix_scale=0.1, supersample=2, psf_size=5,
+                   psf_kind="gaussian", psf_fwhm=0.25, psf_beta=0.0, n_lens_light=1, n_source=2,
+                   noise_bg=0.05, noise_exptime=100.0, source_amp=(1.0, 20.0), batch=8)
+    prob = W.make_problem(w, orc.render_for_workloads)
+    cfg = orc.config_of(w)
+    row = prob.truth[0].copy()
+    sigmas = np.array([0.12, 0.36, 1.1], np.float32)
+    M = orc.mge_component_images(cfg, prob.psf[0], row, sigmas)
+    true_amps = np.array([30.0, 0.0, 4.5, 2.0, 9.0])
+    data = np.tensordot(true_amps, M, axes=1).astype(np.float32)[None]
+    noise = np.full_like(data, 0.1)
+    rows = np.stack([row] * 8)
+    rows[1, 0] = -1.0                 # theta_E < 0
+    rows[2, 10] = 0.9; rows[2, 11] = 0.9    # |e| >= 1 of the MGE shape
+    rows[3, 13] = np.nan              # MGE centre not finite
+    rows[4, 16] = 0.0                 # source n = 0
+    ctx = api.LensContext(w.ny, w.nx, w.pix_scale, w.supersample, 1, 2, prob.psf, data, noise)
+    with pytest.raises(api.TinyLensError):
+        ctx.loglike_mge(torch.from_numpy(rows).cuda())          # no Gaussian set yet
+    with pytest.raises(api.TinyLensError):
+        ctx.set_mge(np.array([0.1, -0.2], np.float32))
+    with pytest.raises(api.TinyLensError):
+        ctx.set_mge(np.full(17, 0.1, np.float32))
+    ctx.set_mge(sigmas)
+    ll, amps = ctx.loglike_mge(torch.from_numpy(rows).cuda())
+    ll = ll.cpu().numpy(); amps = amps.cpu().numpy()
+    ctx.close()
+    for r in (1, 2, 3, 4):
+        assert ll[r] == -np.inf and np.all(np.isnan(amps[r]))
+    const = -0.5 * data.size * np.log(2 * np.pi * 0.1 ** 2)
+    for r in (0, 5, 6, 7):
+        assert np.allclose(amps[r], true_amps, rtol=2e-4, atol=2e-3), amps[r]
+        assert abs(ll[r] - const) <= 1e-3 + 1e-6 * abs(const) + 0.05     # chi^2 ~ (1e-7 x SNR)^2 summed
+    # a context without lens light has no MGE
+    w0 = W.workload(0)
+    p0 = W.make_problem(w0, orc.render_for_workloads)
+    c0 = api.LensContext.from_problem(p0)
+    with pytest.raises(api.TinyLensError):
+        c0.set_mge(sigmas)
+    c0.close()
