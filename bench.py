@@ -390,6 +390,10 @@ def run_linear(args, w: W.Workload):
     ctx = api.LensContext.from_problem(prob)
     rows = W.batch_rows(w)
     B = rows.shape[0]
+    mge = args.mode == "mge"
+    if mge:
+        run_mge(args, w, prob, ctx, rows)
+        return
     d_rows = torch.from_numpy(rows).to(dev)
     out = torch.empty(B, dtype=torch.float32, device=dev)
     amps = torch.empty((B, w.n_lens_light + w.n_source), dtype=torch.float32, device=dev)
@@ -440,6 +444,69 @@ def run_linear(args, w: W.Workload):
     print(json.dumps(line))
 
 
+def run_mge(args, w: W.Workload, prob, ctx, rows):
+    """Secondary line: MGE lens light with linear amplitudes (NEXT-3, tl_loglike_mge_batch): the
+    same workload, its lens light fitted by n_gauss elliptical Gaussians, n_gauss + n_source
+    amplitudes solved per row."""
+    import torch
+    from paper_2503_08586_b200 import api
+    dev = torch.device("cuda", 0)
+    sigmas = W.mge_sigmas(w, args.n_gauss)
+    ctx.set_mge(sigmas)
+    B = rows.shape[0]
+    NC = len(sigmas) + w.n_source
+    d_rows = torch.from_numpy(rows).to(dev)
+    out = torch.empty(B, dtype=torch.float32, device=dev)
+    amps = torch.empty((B, NC), dtype=torch.float32, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    ctx.set_profiling(True)
+    for _ in range(max(args.warmup, 3)):
+        ctx.loglike_mge(d_rows, out, amps)
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    kern_ms = []
+    with ClockSampler(0) as clk:
+        for s in range(args.steps):
+            flush.fill_(s & 0xff)
+            ev[s][0].record(); ctx.loglike_mge(d_rows, out, amps); ev[s][1].record()
+            kern_ms.append(ctx.last_kernel_ms())
+        torch.cuda.synchronize()
+    total_ms = float(np.sum([a.elapsed_time(b) for a, b in ev]))
+    value = B * args.steps / (total_ms * 1e-3)
+    chunk = api.tl_mge_chunk_rows(ctx.handle)
+    n_chunks = (B + chunk - 1) // chunk
+    last_rows = B - (n_chunks - 1) * chunk
+    line = {"metric": METRIC + mass_tag(w) + " (MGE lens light, %d Gaussians + %d source amplitudes by NNLS per row)" % (len(sigmas), w.n_source),
+            "value": value, "unit": UNIT, "n_gpus": 1,
+            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": config_dict(w, "flushed between steps (256 MiB fill)"), "clocks": clk.summary(),
+            "pixel_evals_per_s": value * w.ny * w.nx, "mode": "mge", "mge_sigmas_arcsec": [float(x) for x in sigmas],
+            "chunk_rows": int(chunk), "gpu_launches": int(args.steps * 5 * n_chunks), "checksum_logL": float(out.double().sum())}
+    # dominant kernel: conv_lin_kernel, the NC PSF convolutions of a row (NC K^2 FMAs per native pixel);
+    # the events bracket the conv launch of the call's last chunk
+    info = ctx.info()
+    sm_max = float(measured_peaks().get("sm_max_mhz", 1965.0))
+    k_ms = float(np.mean(kern_ms))
+    slots = NC * w.psf_size ** 2 * w.ny * w.nx
+    ach = slots * last_rows / (k_ms * 1e-3) / 1e12
+    peak = info["n_sm"] * SM_FP32_LANES * sm_max * 1e6 / 1e12
+    line["roofline"] = {"bound": "alu", "kernel": "conv_lin_kernel", "achieved": ach, "peak": peak, "unit": "Tinst/s",
+                        "frac": ach / peak, "traffic": None, "kernel_ms": k_ms, "kernel_rows": int(last_rows),
+                        "algorithmic_issue_slots_per_likelihood": slots,
+                        "peak_source": "as in the default mode (FP32 FMA issue slots)"}
+    if not args.no_cpu_baseline:
+        from oracle import oracle as O
+        O.lib()
+        n = min(args.ref_rows, 64)
+        t0 = time.perf_counter()
+        O.loglike_mge_batch(O.config_of(w), prob.psf, prob.data, prob.noise, rows[:n], sigmas, n_lens=w.n_lens)
+        dt = time.perf_counter() - t0
+        line["cpu_baseline"] = {"value": n / dt, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle",
+                                "sample": "first %d of the %d rows, %.1f s" % (n, B, dt)}
+    print(json.dumps(line))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -450,9 +517,12 @@ def main():
     ap.add_argument("--batch", type=int, default=0, help="override rows per GPU (parity/debug only)")
     ap.add_argument("--ref-rows", type=int, default=512, help="oracle sample size per step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--mode", default="fixed", choices=["fixed", "linear"],
+    ap.add_argument("--mode", default="fixed", choices=["fixed", "linear", "mge"],
                     help="fixed: amplitudes are parameters (the headline metric); linear: amplitudes solved by NNLS "
-                         "per row (tl_loglike_linear_batch, PAPER.md Eq. 6-7) -- a secondary line")
+                         "per row (tl_loglike_linear_batch, PAPER.md Eq. 6-7) -- a secondary line; mge: the lens "
+                         "light as n_gauss elliptical Gaussians with NNLS amplitudes (tl_loglike_mge_batch, "
+                         "PAPER.md:291-293) -- a secondary line")
+    ap.add_argument("--n-gauss", type=int, default=10, help="--mode mge: Gaussians in the lens-light set (<= 16)")
     ap.add_argument("--mass", default="sie", choices=["sie", "epl"],
                     help="sie: the headline workload; epl: the same workload with the elliptical power-law mass "
                          "model and a free slope per row (NEXT-2, PAPER.md Eq. 12) -- a secondary line")
@@ -465,7 +535,7 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if world != args.gpus and world > 1:
         raise SystemExit("--gpus %d does not match WORLD_SIZE %d" % (args.gpus, world))
-    if args.mode == "linear":
+    if args.mode in ("linear", "mge"):
         run_linear(args, w)
     elif args.impl == "reference":
         run_reference(args, w)

@@ -191,6 +191,9 @@ int tl_loglike_linear_batch(tl_ctx *ctx, const float *params, int64_t B, float *
  * TL_ENOMEM or TL_ECUDA.
  *
  * tl_mge_columns -- n_gauss + n_source (the width of `amps`), or < 0 when no set is defined.
+ * tl_mge_chunk_rows -- a call with more rows is processed in chunks of this many (five launches
+ *   each, same stream; the component images of a chunk are staged in <= 8 GB of scratch from
+ *   the stream-ordered allocator); < 0 when no set is defined.
  *
  * tl_loglike_mge_batch -- logL[r] = Eq. 5 at the NNLS-optimal amplitudes of row r.
  *   params   DEVICE pointer, float [B][P], the context's usual row layout; of the lens-light
@@ -208,6 +211,7 @@ int tl_loglike_linear_batch(tl_ctx *ctx, const float *params, int64_t B, float *
  */
 int tl_set_mge(tl_ctx *ctx, const float *sigmas, int32_t n_gauss);
 int tl_mge_columns(const tl_ctx *ctx);
+int64_t tl_mge_chunk_rows(const tl_ctx *ctx);
 int tl_loglike_mge_batch(tl_ctx *ctx, const float *params, int64_t B, float *logL, float *amps,
                          void *cuda_stream);
 

@@ -74,6 +74,7 @@ def load(build_if_missing: bool = True):
     L.tl_loglike_linear_batch.restype = C.c_int; L.tl_loglike_linear_batch.argtypes = [vp, vp, i64, vp, vp, vp]
     L.tl_set_mge.restype = C.c_int; L.tl_set_mge.argtypes = [vp, fp, i32]
     L.tl_mge_columns.restype = C.c_int; L.tl_mge_columns.argtypes = [vp]
+    L.tl_mge_chunk_rows.restype = i64; L.tl_mge_chunk_rows.argtypes = [vp]
     L.tl_loglike_mge_batch.restype = C.c_int; L.tl_loglike_mge_batch.argtypes = [vp, vp, i64, vp, vp, vp]
     L.tl_set_precision.restype = C.c_int; L.tl_set_precision.argtypes = [vp, C.c_int]
     L.tl_set_profiling.restype = C.c_int; L.tl_set_profiling.argtypes = [vp, C.c_int]
@@ -199,6 +200,10 @@ def tl_set_mge(handle: int, sigmas):
 
 def tl_mge_columns(handle: int) -> int:
     return load().tl_mge_columns(handle)
+
+
+def tl_mge_chunk_rows(handle: int) -> int:
+    return int(load().tl_mge_chunk_rows(handle))
 
 
 def tl_loglike_mge_batch(handle: int, params, out=None, amps=None, want_amps=True, stream=None):

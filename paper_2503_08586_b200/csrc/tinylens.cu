@@ -79,6 +79,7 @@ void best_warp_tile(int He, int We, int *CW, int *CH)
 constexpr size_t SMEM_LIMIT = 227 * 1024;
 constexpr int64_t CONST_CHUNK = 1 << 17;        // rows of RowC scratch per chunk (fused path)
 constexpr size_t EXT_SCRATCH_BYTES = 512u << 20; // split path: binned-image scratch per chunk
+constexpr size_t MGE_SCRATCH_BYTES = (size_t)8 << 30;  // MGE: component images of a chunk (180 GB of HBM: keep whole batches resident)
 
 inline bool cuda_ok(cudaError_t e) { return e == cudaSuccess; }
 
@@ -619,6 +620,21 @@ int tl_set_mge(tl_ctx *c, const float *sigmas, int32_t n_gauss)
     return TL_OK;
 }
 
+namespace {
+int64_t mge_chunk_rows(const tl_ctx *c)
+{
+    const int NC = c->n_gauss + c->cfg.n_source;
+    const size_t npix = (size_t)c->cfg.ny * c->cfg.nx;
+    const size_t ext_row = sizeof(float) * (size_t)NC * c->He * c->pitch, m_row = sizeof(float) * NC * npix;
+    int64_t chunk = (int64_t)(MGE_SCRATCH_BYTES / (ext_row + m_row));
+    if (chunk < 1) chunk = 1;
+    if (chunk > 65535) chunk = 65535;
+    return chunk;
+}
+}  // namespace
+
+int64_t tl_mge_chunk_rows(const tl_ctx *c) { return (c && c->n_gauss > 0) ? mge_chunk_rows(c) : (int64_t)TL_EINVAL; }
+
 int tl_mge_columns(const tl_ctx *c) { return (c && c->n_gauss > 0) ? c->n_gauss + c->cfg.n_source : TL_EINVAL; }
 
 int tl_loglike_mge_batch(tl_ctx *c, const float *params, int64_t B, float *logL, float *amps, void *cuda_stream)
@@ -635,9 +651,7 @@ int tl_loglike_mge_batch(tl_ctx *c, const float *params, int64_t B, float *logL,
     const int NG = c->n_gauss, NC = NG + c->cfg.n_source;
     const size_t npix = (size_t)c->cfg.ny * c->cfg.nx;
     const size_t ext_row = sizeof(float) * (size_t)NC * c->He * c->pitch, m_row = sizeof(float) * NC * npix;
-    int64_t chunk = (int64_t)(EXT_SCRATCH_BYTES / (ext_row + m_row));
-    if (chunk < 1) chunk = 1;
-    if (chunk > 65535) chunk = 65535;
+    int64_t chunk = mge_chunk_rows(c);
     if (chunk > B) chunk = B;
     tl::RowC *rows = nullptr;
     float *ext = nullptr, *mimg = nullptr;
@@ -648,9 +662,9 @@ int tl_loglike_mge_batch(tl_ctx *c, const float *params, int64_t B, float *logL,
         if (ext) cudaFreeAsync(ext, st);
         return TL_ENOMEM;
     }
-    cudaMemsetAsync(ext, 0, ext_row * (size_t)chunk, st);      // pitch padding must read as finite zeros
+    // (the pitch padding of ext, which must read as finite zeros, is written by mge_gauss_kernel)
     const int64_t rows_per_lens = B / c->cfg.n_lens;
-    int gslabs = (c->He * c->We + 255) / 256;
+    int gslabs = (c->He * c->pitch + 255) / 256;
     if (gslabs > 16) gslabs = 16;
     int rc = TL_OK;
     for (int64_t r0 = 0; r0 < B && rc == TL_OK; r0 += chunk) {
@@ -676,7 +690,7 @@ int tl_loglike_mge_batch(tl_ctx *c, const float *params, int64_t B, float *logL,
         if (c->profile) cudaEventRecord(c->ev0, st);
         tl::conv_lin_kernel<<<cg, 256, c->lin_conv_smem, st>>>(a, (int)nb);
         if (c->profile) { cudaEventRecord(c->ev1, st); c->prof_pending = 1; }
-        tl::solve_mge_kernel<<<(unsigned)nb, 256, 0, st>>>(a, (int)nb);
+        tl::solve_mge_kernel<<<(unsigned)nb, tl::MGE_SOLVE_THREADS, 0, st>>>(a, (int)nb);
         if (!cuda_ok(cudaGetLastError())) rc = TL_ECUDA;
     }
     cudaFreeAsync(rows, st); cudaFreeAsync(ext, st); cudaFreeAsync(mimg, st);

@@ -20,7 +20,8 @@ namespace tl {
 
 constexpr int MGE_MAX_GAUSS = 16;
 constexpr int MGE_MAX_COL = MGE_MAX_GAUSS + 2;       // + n_source
-constexpr int MGE_TILE = 64;                         // pixels staged per step of the Gram reduction
+constexpr int MGE_SOLVE_THREADS = 128;
+constexpr int MGE_TILE = 32;                         // pixels staged per step of the Gram reduction
 
 // One thread per extended native pixel (grid.x = row in chunk, grid.y = slabs of the image).
 // t = R_p^2 is evaluated exactly like the lens-light term of col_values / row_values (hi/lo
@@ -41,9 +42,13 @@ __global__ void __launch_bounds__(256) mge_gauss_kernel(const KArgs a, int chunk
     const float inv_s2 = 1.f / (float)(S * S);
     const size_t comp_stride = (size_t)a.He * a.pitch;
     float *dst = a.ext + (size_t)r * a.ext_nc * comp_stride;
-    const int npx = a.He * a.We;
+    const int npx = a.He * a.pitch;
     for (int p = blockIdx.y * blockDim.x + threadIdx.x; p < npx; p += gridDim.y * blockDim.x) {
-        const int i = p / a.We, j = p - i * a.We;
+        const int i = p / a.pitch, j = p - i * a.pitch;
+        if (j >= a.We) {                               // pitch padding of every component reads as zero
+            for (int k = 0; k < a.ext_nc; ++k) dst[k * comp_stride + (size_t)i * a.pitch + j] = 0.f;
+            continue;
+        }
         float acc[MGE_MAX_GAUSS];
 #pragma unroll
         for (int k = 0; k < MGE_MAX_GAUSS; ++k) acc[k] = 0.f;
@@ -55,7 +60,7 @@ __global__ void __launch_bounds__(256) mge_gauss_kernel(const KArgs a, int chunk
                 const float dyl = ((Y0 + (float)(2 * sa)) - cYh) - cYl;
                 const float y2 = dyl * dyl;
                 const float LC = fmaf(cch, y2, ccl * y2);
-#pragma unroll 1
+#pragma unroll 2
                 for (int sb = 0; sb < S; ++sb) {
                     const float dxl = ((X0 + (float)(2 * sb)) - cXh) - cXl;
                     const float x2 = dxl * dxl;
@@ -158,10 +163,11 @@ __device__ inline void nnls_gram(int n, const double *G, int ldg, const double *
     }
 }
 
-// one CTA of 256 threads per row.  Thread p < n_pairs owns one entry of [G | b | d'Wd]: the
+// one CTA of 128 threads per row (the NNLS iteration runs on one thread and is latency-bound:
+// small CTAs keep up to 14 rows resident per SM).  Thread p owns entries p and p + 128 of [G | b | d'Wd]: the
 // pixels are staged through shared memory MGE_TILE at a time (w m_k and m_k, d as doubles) and
 // every entry is summed over the pixels in index order, so the result is bitwise reproducible.
-__global__ void __launch_bounds__(256) solve_mge_kernel(const KArgs a, int chunk_rows)
+__global__ void __launch_bounds__(MGE_SOLVE_THREADS) solve_mge_kernel(const KArgs a, int chunk_rows)
 {
     constexpr int NCP = MGE_MAX_COL + 1;
     __shared__ double As[MGE_TILE][NCP];               // w_i m_ki   (column n: w_i d_i)
@@ -188,15 +194,16 @@ __global__ void __launch_bounds__(256) solve_mge_kernel(const KArgs a, int chunk
     const float *d = a.data + lens * (size_t)npix, *w = a.wgt + lens * (size_t)npix;
     // pair owned by this thread: (k, l) with k <= l <= n, k <= n  (l = n: the data column)
     const int n1 = n + 1, n_pairs = n1 * (n1 + 1) / 2;
-    int pk = -1, pl = -1;
-    {
-        int p = threadIdx.x, k = 0;
+    int pk[2] = {-1, -1}, pl[2] = {-1, -1};
+#pragma unroll
+    for (int u = 0; u < 2; ++u) {
+        int p = threadIdx.x + u * MGE_SOLVE_THREADS, k = 0;
         if (p < n_pairs) {
             while (p >= n1 - k) { p -= n1 - k; ++k; }
-            pk = k; pl = k + p;
+            pk[u] = k; pl[u] = k + p;
         }
     }
-    double acc = 0.0;
+    double acc[2] = {0.0, 0.0};
     for (int t0 = 0; t0 < npix; t0 += MGE_TILE) {
         __syncthreads();
         for (int e = threadIdx.x; e < MGE_TILE * n1; e += blockDim.x) {
@@ -206,16 +213,28 @@ __global__ void __launch_bounds__(256) solve_mge_kernel(const KArgs a, int chunk
             As[ii][k] = wv; Bs[ii][k] = v;
         }
         __syncthreads();
-        if (pk >= 0) {
+        if (pk[0] >= 0) {
+            const int k0 = pk[0], l0 = pl[0];
+            if (pk[1] >= 0) {
+                const int k1 = pk[1], l1 = pl[1];
 #pragma unroll 8
-            for (int ii = 0; ii < MGE_TILE; ++ii) acc = fma(As[ii][pk], Bs[ii][pl], acc);
+                for (int ii = 0; ii < MGE_TILE; ++ii) {
+                    acc[0] = fma(As[ii][k0], Bs[ii][l0], acc[0]);
+                    acc[1] = fma(As[ii][k1], Bs[ii][l1], acc[1]);
+                }
+            } else {
+#pragma unroll 8
+                for (int ii = 0; ii < MGE_TILE; ++ii) acc[0] = fma(As[ii][k0], Bs[ii][l0], acc[0]);
+            }
         }
     }
-    if (pk >= 0) {
-        if (pk < n && pl < n) { Gs[pk][pl] = acc; Gs[pl][pk] = acc; }
-        else if (pk < n) { Gs[pk][n] = acc; bs[pk] = acc; }
-        else dwd_s = acc;
-    }
+#pragma unroll
+    for (int u = 0; u < 2; ++u)
+        if (pk[u] >= 0) {
+            if (pk[u] < n && pl[u] < n) { Gs[pk[u]][pl[u]] = acc[u]; Gs[pl[u]][pk[u]] = acc[u]; }
+            else if (pk[u] < n) { Gs[pk[u]][n] = acc[u]; bs[pk[u]] = acc[u]; }
+            else dwd_s = acc[u];
+        }
     __syncthreads();
     if (threadIdx.x == 0) nnls_gram(n, &Gs[0][0], NCP, bs, dwd_s, ss, Ls, zs);
     __syncthreads();
