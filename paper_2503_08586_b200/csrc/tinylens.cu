@@ -452,6 +452,8 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
             c->trace_lin = cfg->mass_model == TL_MASS_EPL ? tl_trace_lin_epl_for(cfg->supersample, cfg->n_lens_light, cfg->n_source)
                                                           : tl_trace_lin_for(cfg->supersample, cfg->n_lens_light, cfg->n_source);
             bool okl = cuda_ok(cudaFuncSetAttribute(tl::conv_lin_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT));
+            // two or three tiles per SM: ask for the largest shared-memory carveout
+            okl = okl && cuda_ok(cudaFuncSetAttribute(tl::conv_lin_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
             if (rowtab_bytes <= 48 * 1024) {
                 c->lin_rowtab = 1; c->lin_trace_smem = rowtab_bytes;
                 okl = okl && cuda_ok(cudaFuncSetAttribute(c->trace_lin, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rowtab_bytes));
@@ -685,7 +687,7 @@ int tl_loglike_mge_batch(tl_ctx *c, const float *params, int64_t B, float *logL,
         dim3 tg((unsigned)nb, 8);
         c->trace_lin<<<tg, 256, c->lin_trace_smem, st>>>(a, (int)nb);
         dim3 gg((unsigned)nb, (unsigned)gslabs);
-        tl::mge_gauss_kernel<<<gg, 256, 0, st>>>(a, (int)nb);
+        tl::mge_gauss_for(NG)<<<gg, 256, 0, st>>>(a, (int)nb);
         dim3 cg((unsigned)nb, (unsigned)c->lin_n_tiles, (unsigned)NC);
         if (c->profile) cudaEventRecord(c->ev0, st);
         tl::conv_lin_kernel<<<cg, 256, c->lin_conv_smem, st>>>(a, (int)nb);

@@ -806,7 +806,7 @@ __global__ void __launch_bounds__(256, 2) trace_lin_kernel(const KArgs a, int ch
 
 #ifdef TL_MAIN_TU
 // one CTA per (row_in_chunk, tile of output rows, component): M_k = K (*) L_k  (blurring matrix B)
-__global__ void __launch_bounds__(256) conv_lin_kernel(const KArgs a, int chunk_rows)
+__global__ void __launch_bounds__(256, 2) conv_lin_kernel(const KArgs a, int chunk_rows)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float *taps = reinterpret_cast<float *>(smem_raw);

@@ -21,11 +21,15 @@ namespace tl {
 constexpr int MGE_MAX_GAUSS = 16;
 constexpr int MGE_MAX_COL = MGE_MAX_GAUSS + 2;       // + n_source
 constexpr int MGE_SOLVE_THREADS = 128;
-constexpr int MGE_TILE = 32;                         // pixels staged per step of the Gram reduction
+constexpr int MGE_TILE = 64;                         // pixels staged per step of the Gram reduction
 
 // One thread per extended native pixel (grid.x = row in chunk, grid.y = slabs of the image).
 // t = R_p^2 is evaluated exactly like the lens-light term of col_values / row_values (hi/lo
-// constants, exact first differences), each Gaussian is one FMUL + MUFU.EX2 per sub-sample.
+// constants, exact first differences), each Gaussian is one FMUL + MUFU.EX2 per sub-sample: the
+// kernel is bound by the MUFU pipe (NG ex2 per sample), so NG is a template parameter (no
+// predicated-off MUFU issue) and the sub-sample offsets advance by exact FP32 additions (no I2F,
+// which shares that pipe).
+template <int NG>
 __global__ void __launch_bounds__(256) mge_gauss_kernel(const KArgs a, int chunk_rows)
 {
     const int r = blockIdx.x;
@@ -35,10 +39,10 @@ __global__ void __launch_bounds__(256) mge_gauss_kernel(const KArgs a, int chunk
     const SersicC &C = rc.comp[0];
     const float cXh = C.cXh, cXl = C.cXl, cYh = C.cYh, cYl = C.cYl;
     const float ah = C.ah, al = C.al, b2h = C.b2h, b2l = C.b2l, cch = C.cch, ccl = C.ccl;
-    const int ng = a.n_gauss, S = a.S;
-    float ck[MGE_MAX_GAUSS];
+    const int S = a.S;
+    float ck[NG];
 #pragma unroll
-    for (int k = 0; k < MGE_MAX_GAUSS; ++k) ck[k] = k < ng ? -a.mge_c[k] : 0.f;
+    for (int k = 0; k < NG; ++k) ck[k] = -a.mge_c[k];
     const float inv_s2 = 1.f / (float)(S * S);
     const size_t comp_stride = (size_t)a.He * a.pitch;
     float *dst = a.ext + (size_t)r * a.ext_nc * comp_stride;
@@ -49,33 +53,47 @@ __global__ void __launch_bounds__(256) mge_gauss_kernel(const KArgs a, int chunk
             for (int k = 0; k < a.ext_nc; ++k) dst[k * comp_stride + (size_t)i * a.pitch + j] = 0.f;
             continue;
         }
-        float acc[MGE_MAX_GAUSS];
+        float acc[NG];
 #pragma unroll
-        for (int k = 0; k < MGE_MAX_GAUSS; ++k) acc[k] = 0.f;
+        for (int k = 0; k < NG; ++k) acc[k] = 0.f;
         const bool edge = a.edge_zero && (j < a.h || j >= a.We - a.h || i < a.h || i >= a.He - a.h);
         if (!edge) {
-            const float X0 = (float)(2 * j * S + 1 - S * a.We), Y0 = (float)(2 * i * S + 1 - S * a.He);
+            const float X0 = (float)(2 * j * S + 1 - S * a.We);
+            float Y = (float)(2 * i * S + 1 - S * a.He);          // small integers: the additions below are exact
 #pragma unroll 1
-            for (int sa = 0; sa < S; ++sa) {
-                const float dyl = ((Y0 + (float)(2 * sa)) - cYh) - cYl;
+            for (int sa = 0; sa < S; ++sa, Y += 2.f) {
+                const float dyl = (Y - cYh) - cYl;
                 const float y2 = dyl * dyl;
                 const float LC = fmaf(cch, y2, ccl * y2);
+                float X = X0;
 #pragma unroll 2
-                for (int sb = 0; sb < S; ++sb) {
-                    const float dxl = ((X0 + (float)(2 * sb)) - cXh) - cXl;
+                for (int sb = 0; sb < S; ++sb, X += 2.f) {
+                    const float dxl = (X - cXh) - cXl;
                     const float x2 = dxl * dxl;
                     const float LA = fmaf(ah, x2, al * x2);
                     const float LB = fmaf(dxl, b2h, dxl * b2l);
                     const float t = fmaf(LB, dyl, LA + LC);
 #pragma unroll
-                    for (int k = 0; k < MGE_MAX_GAUSS; ++k)
-                        if (k < ng) acc[k] += mufu_ex2(t * ck[k]);
+                    for (int k = 0; k < NG; ++k) acc[k] += mufu_ex2(t * ck[k]);
                 }
             }
         }
 #pragma unroll
-        for (int k = 0; k < MGE_MAX_GAUSS; ++k)
-            if (k < ng) dst[k * comp_stride + (size_t)i * a.pitch + j] = acc[k] * inv_s2;
+        for (int k = 0; k < NG; ++k) dst[k * comp_stride + (size_t)i * a.pitch + j] = acc[k] * inv_s2;
+    }
+}
+
+typedef void (*mge_gauss_fn)(const KArgs, int);
+inline mge_gauss_fn mge_gauss_for(int ng)
+{
+    switch (ng) {
+    case 1: return mge_gauss_kernel<1>;   case 2: return mge_gauss_kernel<2>;   case 3: return mge_gauss_kernel<3>;
+    case 4: return mge_gauss_kernel<4>;   case 5: return mge_gauss_kernel<5>;   case 6: return mge_gauss_kernel<6>;
+    case 7: return mge_gauss_kernel<7>;   case 8: return mge_gauss_kernel<8>;   case 9: return mge_gauss_kernel<9>;
+    case 10: return mge_gauss_kernel<10>; case 11: return mge_gauss_kernel<11>; case 12: return mge_gauss_kernel<12>;
+    case 13: return mge_gauss_kernel<13>; case 14: return mge_gauss_kernel<14>; case 15: return mge_gauss_kernel<15>;
+    case 16: return mge_gauss_kernel<16>;
+    default: return nullptr;
     }
 }
 
@@ -204,15 +222,30 @@ __global__ void __launch_bounds__(MGE_SOLVE_THREADS) solve_mge_kernel(const KArg
         }
     }
     double acc[2] = {0.0, 0.0};
+    // the next tile's values are fetched into registers while the current one is consumed, so the
+    // global-memory latency (M does not fit in L2 for a whole batch) overlaps the FP64 sums
+    constexpr int EPT = (MGE_TILE * NCP + MGE_SOLVE_THREADS - 1) / MGE_SOLVE_THREADS;
+    float fv[EPT], fw[EPT];
+    auto fetch = [&](int t0) {
+#pragma unroll
+        for (int u = 0; u < EPT; ++u) {
+            const int e = threadIdx.x + u * MGE_SOLVE_THREADS;
+            const int k = e / MGE_TILE, i = t0 + (e - k * MGE_TILE);
+            fv[u] = 0.f; fw[u] = 0.f;
+            if (k < n1 && i < npix) { fv[u] = k < n ? M[(size_t)k * npix + i] : d[i]; fw[u] = w[i]; }
+        }
+    };
+    fetch(0);
     for (int t0 = 0; t0 < npix; t0 += MGE_TILE) {
         __syncthreads();
-        for (int e = threadIdx.x; e < MGE_TILE * n1; e += blockDim.x) {
-            const int k = e / MGE_TILE, ii = e - k * MGE_TILE, i = t0 + ii;
-            double v = 0.0, wv = 0.0;
-            if (i < npix) { v = k < n ? (double)M[(size_t)k * npix + i] : (double)d[i]; wv = (double)w[i] * v; }
-            As[ii][k] = wv; Bs[ii][k] = v;
+#pragma unroll
+        for (int u = 0; u < EPT; ++u) {
+            const int e = threadIdx.x + u * MGE_SOLVE_THREADS;
+            const int k = e / MGE_TILE, ii = e - k * MGE_TILE;
+            if (k < n1) { As[ii][k] = (double)fw[u] * (double)fv[u]; Bs[ii][k] = (double)fv[u]; }
         }
         __syncthreads();
+        if (t0 + MGE_TILE < npix) fetch(t0 + MGE_TILE);
         if (pk[0] >= 0) {
             const int k0 = pk[0], l0 = pl[0];
             if (pk[1] >= 0) {
