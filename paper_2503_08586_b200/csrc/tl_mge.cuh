@@ -135,20 +135,20 @@ __device__ inline void nnls_gram(int n, const double *G, int ldg, const double *
                     for (int k = 0; k < c; ++k) v -= L[r * MGE_MAX_COL + k] * L[c * MGE_MAX_COL + k];
                     if (c == r) {
                         if (!(v > 1e-13 * G[idx[r] * ldg + idx[r]])) { pd = false; break; }
-                        L[r * MGE_MAX_COL + r] = sqrt(v);
-                    } else L[r * MGE_MAX_COL + c] = v / L[c * MGE_MAX_COL + c];
+                        L[r * MGE_MAX_COL + r] = rsqrt(v);             // the diagonal is kept as 1 / l_rr
+                    } else L[r * MGE_MAX_COL + c] = v * L[c * MGE_MAX_COL + c];
                 }
             }
             if (pd) {
                 for (int r = 0; r < m; ++r) {
                     double v = b[idx[r]];
                     for (int k = 0; k < r; ++k) v -= L[r * MGE_MAX_COL + k] * z[k];
-                    z[r] = v / L[r * MGE_MAX_COL + r];
+                    z[r] = v * L[r * MGE_MAX_COL + r];
                 }
                 for (int r = m - 1; r >= 0; --r) {
                     double v = z[r];
                     for (int k = r + 1; k < m; ++k) v -= L[k * MGE_MAX_COL + r] * z[k];
-                    z[r] = v / L[r * MGE_MAX_COL + r];
+                    z[r] = v * L[r * MGE_MAX_COL + r];
                 }
             }
             if (first) {
@@ -273,8 +273,12 @@ __global__ void __launch_bounds__(MGE_SOLVE_THREADS) solve_mge_kernel(const KArg
     __syncthreads();
     double part = 0.0;
     for (int i = threadIdx.x; i < npix; i += blockDim.x) {
+        float mv[MGE_MAX_COL];
+#pragma unroll
+        for (int k = 0; k < MGE_MAX_COL; ++k) mv[k] = k < n ? M[(size_t)k * npix + i] : 0.f;     // independent loads in flight
         double m = 0.0;
-        for (int k = 0; k < n; ++k) m += ss[k] * (double)M[(size_t)k * npix + i];
+#pragma unroll
+        for (int k = 0; k < MGE_MAX_COL; ++k) if (k < n) m += ss[k] * (double)mv[k];
         const double res = (double)d[i] - m;
         part += res * res * (double)w[i];
     }
