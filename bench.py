@@ -432,6 +432,11 @@ def run_linear(args, w: W.Workload):
                         "frac": ach / peak, "traffic": None, "kernel_ms": k_ms,
                         "algorithmic_issue_slots_per_likelihood": slots,
                         "peak_source": "as in the default mode"}
+    if os.environ.get("TL_LINEAR_STAGED"):
+        # staged pipeline forced: the events bracket trace_lin_kernel of the last chunk only, which
+        # is not the whole of the op model above -- no roofline fraction is claimed for this run
+        line["roofline"] = {"bound": "alu", "kernel": "trace_lin_kernel (staged pipeline forced by TL_LINEAR_STAGED)",
+                            "achieved": None, "peak": peak, "unit": "Tinst/s", "frac": None, "traffic": None, "kernel_ms": k_ms}
     if not args.no_cpu_baseline:
         from oracle import oracle as O
         O.lib()
