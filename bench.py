@@ -487,7 +487,7 @@ def run_mge(args, w: W.Workload, prob, ctx, rows):
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": config_dict(w, "flushed between steps (256 MiB fill)"), "clocks": clk.summary(),
             "pixel_evals_per_s": value * w.ny * w.nx, "mode": "mge", "mge_sigmas_arcsec": [float(x) for x in sigmas],
-            "chunk_rows": int(chunk), "gpu_launches": int(args.steps * 5 * n_chunks), "checksum_logL": float(out.double().sum())}
+            "chunk_rows": int(chunk), "gpu_launches": int(args.steps * 7 * n_chunks), "checksum_logL": float(out.double().sum())}
     # dominant kernel: conv_lin_kernel, the NC PSF convolutions of a row (NC K^2 FMAs per native pixel);
     # the events bracket the conv launch of the call's last chunk
     info = ctx.info()

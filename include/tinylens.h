@@ -191,7 +191,7 @@ int tl_loglike_linear_batch(tl_ctx *ctx, const float *params, int64_t B, float *
  * TL_ENOMEM or TL_ECUDA.
  *
  * tl_mge_columns -- n_gauss + n_source (the width of `amps`), or < 0 when no set is defined.
- * tl_mge_chunk_rows -- a call with more rows is processed in chunks of this many (five launches
+ * tl_mge_chunk_rows -- a call with more rows is processed in chunks of this many (seven launches
  *   each, same stream; the component images of a chunk are staged in <= 8 GB of scratch from
  *   the stream-ordered allocator); < 0 when no set is defined.
  *

@@ -657,11 +657,15 @@ int tl_loglike_mge_batch(tl_ctx *c, const float *params, int64_t B, float *logL,
     if (chunk > B) chunk = B;
     tl::RowC *rows = nullptr;
     float *ext = nullptr, *mimg = nullptr;
+    double *gram = nullptr;                                    // [chunk][MGE_GRAM_STRIDE + MGE_MAX_COL]
+    const size_t g_row = sizeof(double) * (tl::MGE_GRAM_STRIDE + tl::MGE_MAX_COL);
     if (!cuda_ok(cudaMallocAsync(&rows, sizeof(tl::RowC) * (size_t)chunk, st))) return TL_ENOMEM;
     if (!cuda_ok(cudaMallocAsync(&ext, ext_row * (size_t)chunk, st)) ||
-        !cuda_ok(cudaMallocAsync(&mimg, m_row * (size_t)chunk, st))) {
+        !cuda_ok(cudaMallocAsync(&mimg, m_row * (size_t)chunk, st)) ||
+        !cuda_ok(cudaMallocAsync(&gram, g_row * (size_t)chunk, st))) {
         cudaFreeAsync(rows, st);
         if (ext) cudaFreeAsync(ext, st);
+        if (mimg) cudaFreeAsync(mimg, st);
         return TL_ENOMEM;
     }
     // (the pitch padding of ext, which must read as finite zeros, is written by mge_gauss_kernel)
@@ -684,6 +688,7 @@ int tl_loglike_mge_batch(tl_ctx *c, const float *params, int64_t B, float *logL,
         // Sersic stand-in of the lens light lands on slot NG - 1, which mge_gauss_kernel then
         // overwrites with the last Gaussian; the sources land on slots NG, NG + 1
         a.ext_nc = NC; a.ext_k0 = NG - 1; a.n_gauss = NG; a.mge_c = c->mge_c;
+        a.mge_gram = gram; a.mge_sol = gram + (size_t)chunk * tl::MGE_GRAM_STRIDE;
         dim3 tg((unsigned)nb, 8);
         c->trace_lin<<<tg, 256, c->lin_trace_smem, st>>>(a, (int)nb);
         dim3 gg((unsigned)nb, (unsigned)gslabs);
@@ -692,10 +697,12 @@ int tl_loglike_mge_batch(tl_ctx *c, const float *params, int64_t B, float *logL,
         if (c->profile) cudaEventRecord(c->ev0, st);
         tl::conv_lin_kernel<<<cg, 256, c->lin_conv_smem, st>>>(a, (int)nb);
         if (c->profile) { cudaEventRecord(c->ev1, st); c->prof_pending = 1; }
-        tl::solve_mge_kernel<<<(unsigned)nb, tl::MGE_SOLVE_THREADS, 0, st>>>(a, (int)nb);
+        tl::gram_mge_kernel<<<(unsigned)nb, tl::MGE_SOLVE_THREADS, 0, st>>>(a, (int)nb);
+        tl::nnls_mge_kernel<<<(unsigned)((nb + tl::MGE_NNLS_WARPS - 1) / tl::MGE_NNLS_WARPS), 32 * tl::MGE_NNLS_WARPS, 0, st>>>(a, (int)nb);
+        tl::resid_mge_kernel<<<(unsigned)nb, 256, 0, st>>>(a, (int)nb);
         if (!cuda_ok(cudaGetLastError())) rc = TL_ECUDA;
     }
-    cudaFreeAsync(rows, st); cudaFreeAsync(ext, st); cudaFreeAsync(mimg, st);
+    cudaFreeAsync(rows, st); cudaFreeAsync(ext, st); cudaFreeAsync(mimg, st); cudaFreeAsync(gram, st);
     return rc;
 }
 

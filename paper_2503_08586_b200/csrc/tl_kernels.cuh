@@ -41,6 +41,8 @@ struct KArgs {
     // trace_lin_kernel writes its components from slot ext_k0 on (0, 0 = the linear-mode layout)
     int ext_nc, ext_k0, n_gauss;
     const float *mge_c;      // [n_gauss] log2(e) / (2 sigma_k^2), arcsec^-2
+    double *mge_gram;        // [chunk][MGE_GRAM_STRIDE]  G | b | d'Wd
+    double *mge_sol;         // [chunk][MGE_MAX_COL]      solved amplitudes (FP64)
 };
 
 __device__ __forceinline__ bool row_is_valid(const RowC &rc, int n_comp)

@@ -10,9 +10,10 @@
 //   trace_lin_kernel           ray-traced unit-amplitude source images -> component slots n_gauss..
 //   mge_gauss_kernel           the n_gauss binned Gaussians -> component slots 0..n_gauss-1
 //   conv_lin_kernel            every component blurred with the PSF (columns of M)
-//   solve_mge_kernel           G = M'WM, b = M'Wd in FP64 (fixed summation order), NNLS by the
-//                              Gram-matrix active-set iteration of Bro & De Jong (the paper's
-//                              solver), chi^2 of the residual d - M s -> logL
+//   gram_mge_kernel            G = M'WM, b = M'Wd, d'Wd in FP64 (fixed summation order) -> global
+//   nnls_mge_kernel            NNLS by the Gram-matrix active-set iteration of Bro & De Jong (the
+//                              paper's solver), one warp per row -> amplitudes
+//   resid_mge_kernel           chi^2 of the residual d - M s in FP64 -> logL
 #pragma once
 #include "tl_kernels.cuh"
 
@@ -21,6 +22,8 @@ namespace tl {
 constexpr int MGE_MAX_GAUSS = 16;
 constexpr int MGE_MAX_COL = MGE_MAX_GAUSS + 2;       // + n_source
 constexpr int MGE_SOLVE_THREADS = 128;
+constexpr int MGE_GRAM_STRIDE = MGE_MAX_COL * (MGE_MAX_COL + 1) + MGE_MAX_COL + 2;   // doubles per row: G [n][NCP] | b [n] | d'Wd
+constexpr int MGE_NNLS_WARPS = 4;                    // rows per CTA of nnls_mge_kernel (one warp each)
 constexpr int MGE_TILE = 64;                         // pixels staged per step of the Gram reduction
 
 // One thread per extended native pixel (grid.x = row in chunk, grid.y = slabs of the image).
@@ -181,35 +184,25 @@ __device__ inline void nnls_gram(int n, const double *G, int ldg, const double *
     }
 }
 
-// one CTA of 128 threads per row (the NNLS iteration runs on one thread and is latency-bound:
-// small CTAs keep up to 14 rows resident per SM).  Thread p owns entries p and p + 128 of [G | b | d'Wd]: the
-// pixels are staged through shared memory MGE_TILE at a time (w m_k and m_k, d as doubles) and
-// every entry is summed over the pixels in index order, so the result is bitwise reproducible.
-__global__ void __launch_bounds__(MGE_SOLVE_THREADS) solve_mge_kernel(const KArgs a, int chunk_rows)
+// G = M'WM, b = M'Wd, d'Wd: one CTA of 128 threads per row.  Thread p owns entries p and p + 128 of
+// [G | b | d'Wd]; the pixels are staged through shared memory MGE_TILE at a time (w m_k and m_k, d
+// as doubles, the next tile prefetched into registers) and every entry is summed over the pixels in
+// index order, so the result is bitwise reproducible.  Output: a.mge_gram[r][MGE_GRAM_STRIDE].
+__global__ void __launch_bounds__(MGE_SOLVE_THREADS) gram_mge_kernel(const KArgs a, int chunk_rows)
 {
     constexpr int NCP = MGE_MAX_COL + 1;
     __shared__ double As[MGE_TILE][NCP];               // w_i m_ki   (column n: w_i d_i)
     __shared__ double Bs[MGE_TILE][NCP];               // m_ki       (column n: d_i)
-    __shared__ double Gs[MGE_MAX_COL][NCP];            // G, column n = b
-    __shared__ double Ls[MGE_MAX_COL * MGE_MAX_COL];
-    __shared__ double zs[MGE_MAX_COL], ss[MGE_MAX_COL], bs[MGE_MAX_COL];
-    __shared__ double red[32];
-    __shared__ double dwd_s;
     const int r = blockIdx.x;
     if (r >= chunk_rows) return;
     const int64_t row = a.row0 + r;
     const int n = a.ext_nc;
-    if (!row_is_valid(a.rows[r], a.n_comp)) {
-        if (threadIdx.x == 0) {
-            a.logL[row] = -INFINITY;
-            if (a.amps) for (int k = 0; k < n; ++k) a.amps[row * n + k] = NAN;
-        }
-        return;
-    }
+    if (!row_is_valid(a.rows[r], a.n_comp)) return;   // nnls_mge_kernel reports the row
     const int64_t lens = row / a.rows_per_lens;
     const int npix = a.ny * a.nx;
     const float *M = a.mimg + (size_t)r * n * npix;
     const float *d = a.data + lens * (size_t)npix, *w = a.wgt + lens * (size_t)npix;
+    double *gout = a.mge_gram + (size_t)r * MGE_GRAM_STRIDE;
     // pair owned by this thread: (k, l) with k <= l <= n, k <= n  (l = n: the data column)
     const int n1 = n + 1, n_pairs = n1 * (n1 + 1) / 2;
     int pk[2] = {-1, -1}, pl[2] = {-1, -1};
@@ -264,18 +257,66 @@ __global__ void __launch_bounds__(MGE_SOLVE_THREADS) solve_mge_kernel(const KArg
 #pragma unroll
     for (int u = 0; u < 2; ++u)
         if (pk[u] >= 0) {
-            if (pk[u] < n && pl[u] < n) { Gs[pk[u]][pl[u]] = acc[u]; Gs[pl[u]][pk[u]] = acc[u]; }
-            else if (pk[u] < n) { Gs[pk[u]][n] = acc[u]; bs[pk[u]] = acc[u]; }
-            else dwd_s = acc[u];
+            if (pk[u] < n && pl[u] < n) { gout[pk[u] * NCP + pl[u]] = acc[u]; gout[pl[u] * NCP + pk[u]] = acc[u]; }
+            else if (pk[u] < n) gout[MGE_MAX_COL * NCP + pk[u]] = acc[u];
+            else gout[MGE_MAX_COL * NCP + MGE_MAX_COL] = acc[u];
         }
-    __syncthreads();
-    if (threadIdx.x == 0) nnls_gram(n, &Gs[0][0], NCP, bs, dwd_s, ss, Ls, zs);
+}
+
+// NNLS: one warp per row (lane 0 iterates; the iteration is a chain of dependent FP64 operations
+// through shared memory, so what matters is how many rows are in flight per SM: 4 warps per CTA,
+// ~6 KB of shared memory each).  Writes the amplitudes (FP64, for resid_mge_kernel; float for the
+// caller) and reports invalid rows.
+__global__ void __launch_bounds__(32 * MGE_NNLS_WARPS) nnls_mge_kernel(const KArgs a, int chunk_rows)
+{
+    constexpr int NCP = MGE_MAX_COL + 1;
+    __shared__ double Gw[MGE_NNLS_WARPS][MGE_GRAM_STRIDE];
+    __shared__ double Lw[MGE_NNLS_WARPS][MGE_MAX_COL * MGE_MAX_COL];
+    __shared__ double zw[MGE_NNLS_WARPS][MGE_MAX_COL], sw[MGE_NNLS_WARPS][MGE_MAX_COL];
+    const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int r = blockIdx.x * MGE_NNLS_WARPS + wid;
+    if (r >= chunk_rows) return;
+    const int64_t row = a.row0 + r;
+    const int n = a.ext_nc;
+    if (!row_is_valid(a.rows[r], a.n_comp)) {
+        if (lane == 0) a.logL[row] = -INFINITY;
+        if (a.amps && lane < n) a.amps[row * n + lane] = NAN;
+        return;
+    }
+    const double *gin = a.mge_gram + (size_t)r * MGE_GRAM_STRIDE;
+    for (int e = lane; e < MGE_GRAM_STRIDE; e += 32) Gw[wid][e] = gin[e];
+    __syncwarp();
+    if (lane == 0)
+        nnls_gram(n, Gw[wid], NCP, Gw[wid] + MGE_MAX_COL * NCP, Gw[wid][MGE_MAX_COL * NCP + MGE_MAX_COL], sw[wid], Lw[wid], zw[wid]);
+    __syncwarp();
+    if (lane < n) {
+        a.mge_sol[(size_t)r * MGE_MAX_COL + lane] = sw[wid][lane];
+        if (a.amps) a.amps[row * n + lane] = (float)sw[wid][lane];
+    }
+}
+
+// chi^2 of the residual d - M s in FP64 (never via d'Wd - 2 s'b + s'Gs, which cancels) -> logL.
+// One CTA per row; the loads of a pixel's n columns are independent.
+__global__ void __launch_bounds__(256) resid_mge_kernel(const KArgs a, int chunk_rows)
+{
+    __shared__ double red[32];
+    __shared__ double ss[MGE_MAX_COL];
+    const int r = blockIdx.x;
+    if (r >= chunk_rows) return;
+    const int64_t row = a.row0 + r;
+    const int n = a.ext_nc;
+    if (!row_is_valid(a.rows[r], a.n_comp)) return;
+    const int64_t lens = row / a.rows_per_lens;
+    const int npix = a.ny * a.nx;
+    const float *M = a.mimg + (size_t)r * n * npix;
+    const float *d = a.data + lens * (size_t)npix, *w = a.wgt + lens * (size_t)npix;
+    if (threadIdx.x < MGE_MAX_COL) ss[threadIdx.x] = threadIdx.x < n ? a.mge_sol[(size_t)r * MGE_MAX_COL + threadIdx.x] : 0.0;
     __syncthreads();
     double part = 0.0;
     for (int i = threadIdx.x; i < npix; i += blockDim.x) {
         float mv[MGE_MAX_COL];
 #pragma unroll
-        for (int k = 0; k < MGE_MAX_COL; ++k) mv[k] = k < n ? M[(size_t)k * npix + i] : 0.f;     // independent loads in flight
+        for (int k = 0; k < MGE_MAX_COL; ++k) mv[k] = k < n ? M[(size_t)k * npix + i] : 0.f;
         double m = 0.0;
 #pragma unroll
         for (int k = 0; k < MGE_MAX_COL; ++k) if (k < n) m += ss[k] * (double)mv[k];
@@ -284,7 +325,6 @@ __global__ void __launch_bounds__(MGE_SOLVE_THREADS) solve_mge_kernel(const KArg
     }
     const double chi2 = block_sum(part, red);
     if (threadIdx.x == 0) a.logL[row] = (float)(-0.5 * (chi2 + a.lconst[lens]));
-    if (a.amps && threadIdx.x < n) a.amps[row * n + threadIdx.x] = (float)ss[threadIdx.x];
 }
 
 }  // namespace tl
