@@ -184,15 +184,15 @@ __device__ inline void nnls_gram(int n, const double *G, int ldg, const double *
     }
 }
 
-// G = M'WM, b = M'Wd, d'Wd: one CTA of 128 threads per row.  Thread p owns entries p and p + 128 of
-// [G | b | d'Wd]; the pixels are staged through shared memory MGE_TILE at a time (w m_k and m_k, d
-// as doubles, the next tile prefetched into registers) and every entry is summed over the pixels in
-// index order, so the result is bitwise reproducible.  Output: a.mge_gram[r][MGE_GRAM_STRIDE].
+// G = M'WM, b = M'Wd, d'Wd: one CTA of 128 threads per row.  The pixels are staged through shared
+// memory MGE_TILE at a time (w m_k and m_k, d as doubles, the next tile prefetched into registers);
+// every sum has a fixed order, so the result is bitwise reproducible.
+// Output: a.mge_gram[r][MGE_GRAM_STRIDE].
 __global__ void __launch_bounds__(MGE_SOLVE_THREADS) gram_mge_kernel(const KArgs a, int chunk_rows)
 {
-    constexpr int NCP = MGE_MAX_COL + 1;
-    __shared__ double As[MGE_TILE][NCP];               // w_i m_ki   (column n: w_i d_i)
-    __shared__ double Bs[MGE_TILE][NCP];               // m_ki       (column n: d_i)
+    constexpr int NCP = MGE_MAX_COL + 2;               // columns + data, rounded up to even
+    __shared__ __align__(16) double As[MGE_TILE][NCP]; // w_i m_ki   (column n: w_i d_i)
+    __shared__ __align__(16) double Bs[MGE_TILE][NCP]; // m_ki       (column n: d_i)
     const int r = blockIdx.x;
     if (r >= chunk_rows) return;
     const int64_t row = a.row0 + r;
@@ -203,64 +203,82 @@ __global__ void __launch_bounds__(MGE_SOLVE_THREADS) gram_mge_kernel(const KArgs
     const float *M = a.mimg + (size_t)r * n * npix;
     const float *d = a.data + lens * (size_t)npix, *w = a.wgt + lens * (size_t)npix;
     double *gout = a.mge_gram + (size_t)r * MGE_GRAM_STRIDE;
-    // pair owned by this thread: (k, l) with k <= l <= n, k <= n  (l = n: the data column)
-    const int n1 = n + 1, n_pairs = n1 * (n1 + 1) / 2;
-    int pk[2] = {-1, -1}, pl[2] = {-1, -1};
-#pragma unroll
-    for (int u = 0; u < 2; ++u) {
-        int p = threadIdx.x + u * MGE_SOLVE_THREADS, k = 0;
-        if (p < n_pairs) {
-            while (p >= n1 - k) { p -= n1 - k; ++k; }
-            pk[u] = k; pl[u] = k + p;
-        }
+    // [G | b | d'Wd] = A'B with A = [w m_k | w d], B = [m_k | d]  (n1 = n + 1 columns, the data last).
+    // Register blocking: a thread owns a 2 x 2 block of entries (columns 2bi, 2bi+1 of A against
+    // 2bj, 2bj+1 of B, bi <= bj) and every Q-th pixel of a tile, so one LDS.128 of A and one of B
+    // feed four DFMAs (one entry per thread is bound by the shared-memory pipe); the Q pixel
+    // slices of an entry are then added in slice order -- a fixed summation order.
+    const int n1 = n + 1, NB = (n1 + 1) >> 1, nblk = NB * (NB + 1) / 2;
+    const int Q = MGE_SOLVE_THREADS / nblk;                       // >= 2 (nblk <= 55)
+    const int slice = threadIdx.x / nblk;
+    int bi = 0, bj = 0;
+    {
+        int p = threadIdx.x - slice * nblk;
+        while (p >= NB - bi) { p -= NB - bi; ++bi; }
+        bj = bi + p;
     }
-    double acc[2] = {0.0, 0.0};
+    const bool gram_thread = slice < Q;
+    double acc[4] = {0.0, 0.0, 0.0, 0.0};
     // the next tile's values are fetched into registers while the current one is consumed, so the
-    // global-memory latency (M does not fit in L2 for a whole batch) overlaps the FP64 sums
+    // global-memory latency (M does not fit in L2 for a whole batch) overlaps the FP64 sums.
+    // Thread t stages pixel t % MGE_TILE of the tile for the columns t / MGE_TILE, + 2, + 4, ...
     constexpr int EPT = (MGE_TILE * NCP + MGE_SOLVE_THREADS - 1) / MGE_SOLVE_THREADS;
-    float fv[EPT], fw[EPT];
+    static_assert(MGE_SOLVE_THREADS % MGE_TILE == 0, "a thread stages one pixel of the tile");
+    const int ncol = 2 * NB;                                      // n1 rounded up to even: a zero column
+    const int sii = threadIdx.x % MGE_TILE, sk0 = threadIdx.x / MGE_TILE;
+    float fv[EPT], fwv = 0.f;
     auto fetch = [&](int t0) {
+        const int i = t0 + sii;
+        fwv = i < npix ? w[i] : 0.f;
 #pragma unroll
         for (int u = 0; u < EPT; ++u) {
-            const int e = threadIdx.x + u * MGE_SOLVE_THREADS;
-            const int k = e / MGE_TILE, i = t0 + (e - k * MGE_TILE);
-            fv[u] = 0.f; fw[u] = 0.f;
-            if (k < n1 && i < npix) { fv[u] = k < n ? M[(size_t)k * npix + i] : d[i]; fw[u] = w[i]; }
+            const int k = sk0 + u * (MGE_SOLVE_THREADS / MGE_TILE);
+            fv[u] = 0.f;
+            if (k < n1 && i < npix) fv[u] = k < n ? M[(size_t)k * npix + i] : d[i];
         }
     };
     fetch(0);
     for (int t0 = 0; t0 < npix; t0 += MGE_TILE) {
         __syncthreads();
+        {
+            const double wd = (double)fwv;
 #pragma unroll
-        for (int u = 0; u < EPT; ++u) {
-            const int e = threadIdx.x + u * MGE_SOLVE_THREADS;
-            const int k = e / MGE_TILE, ii = e - k * MGE_TILE;
-            if (k < n1) { As[ii][k] = (double)fw[u] * (double)fv[u]; Bs[ii][k] = (double)fv[u]; }
+            for (int u = 0; u < EPT; ++u) {
+                const int k = sk0 + u * (MGE_SOLVE_THREADS / MGE_TILE);
+                if (k < ncol) { const double v = (double)fv[u]; As[sii][k] = wd * v; Bs[sii][k] = v; }
+            }
         }
         __syncthreads();
         if (t0 + MGE_TILE < npix) fetch(t0 + MGE_TILE);
-        if (pk[0] >= 0) {
-            const int k0 = pk[0], l0 = pl[0];
-            if (pk[1] >= 0) {
-                const int k1 = pk[1], l1 = pl[1];
-#pragma unroll 8
-                for (int ii = 0; ii < MGE_TILE; ++ii) {
-                    acc[0] = fma(As[ii][k0], Bs[ii][l0], acc[0]);
-                    acc[1] = fma(As[ii][k1], Bs[ii][l1], acc[1]);
-                }
-            } else {
-#pragma unroll 8
-                for (int ii = 0; ii < MGE_TILE; ++ii) acc[0] = fma(As[ii][k0], Bs[ii][l0], acc[0]);
+        if (gram_thread) {
+#pragma unroll 4
+            for (int ii = slice; ii < MGE_TILE; ii += Q) {
+                const double2 av = *reinterpret_cast<const double2 *>(&As[ii][2 * bi]);
+                const double2 bv = *reinterpret_cast<const double2 *>(&Bs[ii][2 * bj]);
+                acc[0] = fma(av.x, bv.x, acc[0]); acc[1] = fma(av.x, bv.y, acc[1]);
+                acc[2] = fma(av.y, bv.x, acc[2]); acc[3] = fma(av.y, bv.y, acc[3]);
             }
         }
     }
+    __syncthreads();
+    double *Ps = &As[0][0];                                       // [Q * nblk][4] partial blocks (As is free now)
+    if (gram_thread) {
 #pragma unroll
-    for (int u = 0; u < 2; ++u)
-        if (pk[u] >= 0) {
-            if (pk[u] < n && pl[u] < n) { gout[pk[u] * NCP + pl[u]] = acc[u]; gout[pl[u] * NCP + pk[u]] = acc[u]; }
-            else if (pk[u] < n) gout[MGE_MAX_COL * NCP + pk[u]] = acc[u];
-            else gout[MGE_MAX_COL * NCP + MGE_MAX_COL] = acc[u];
-        }
+        for (int e = 0; e < 4; ++e) Ps[(size_t)threadIdx.x * 4 + e] = acc[e];
+    }
+    __syncthreads();
+    constexpr int NCG = MGE_MAX_COL + 1;                          // row pitch of G in a.mge_gram
+    for (int t = threadIdx.x; t < nblk * 4; t += blockDim.x) {
+        const int blk = t >> 2, e = t & 3;
+        double v = 0.0;
+        for (int q = 0; q < Q; ++q) v += Ps[(size_t)(q * nblk + blk) * 4 + e];
+        int ci = 0, p = blk;
+        while (p >= NB - ci) { p -= NB - ci; ++ci; }
+        const int k = 2 * ci + (e >> 1), l = 2 * (ci + p) + (e & 1);
+        if (k < n && l < n) { gout[k * NCG + l] = v; gout[l * NCG + k] = v; }
+        else if (k < n && l == n) gout[MGE_MAX_COL * NCG + k] = v;
+        else if (k == n && l == n) gout[MGE_MAX_COL * NCG + MGE_MAX_COL] = v;
+    }
 }
 
 // NNLS: one warp per row (lane 0 iterates; the iteration is a chain of dependent FP64 operations
