@@ -107,6 +107,13 @@ def test_null_context_calls_are_errors_not_crashes(api):
     assert lib.tl_loglike_batch(None, None, 4, None, None) == api.TL_EINVAL
     assert lib.tl_render_batch(None, None, 4, None, None) == api.TL_EINVAL
     assert lib.tl_loglike_batch_host(None, None, 4, None, None) == api.TL_EINVAL
+    assert lib.tl_loglike_linear_batch(None, None, 4, None, None, None) == api.TL_EINVAL
+    # MGE entry points (NEXT-3)
+    sg = np.array([0.1, 0.3], np.float32)
+    assert lib.tl_set_mge(None, sg.ctypes.data_as(C.POINTER(C.c_float)), 2) == api.TL_EINVAL
+    assert lib.tl_mge_columns(None) < 0
+    assert lib.tl_mge_chunk_rows(None) < 0
+    assert lib.tl_loglike_mge_batch(None, None, 4, None, None, None) == api.TL_EINVAL
     lib.tl_destroy(None)
 
 
