@@ -191,8 +191,12 @@ __device__ inline void nnls_gram(int n, const double *G, int ldg, const double *
 __global__ void __launch_bounds__(MGE_SOLVE_THREADS) gram_mge_kernel(const KArgs a, int chunk_rows)
 {
     constexpr int NCP = MGE_MAX_COL + 2;               // columns + data, rounded up to even
-    __shared__ __align__(16) double As[MGE_TILE][NCP]; // w_i m_ki   (column n: w_i d_i)
-    __shared__ __align__(16) double Bs[MGE_TILE][NCP]; // m_ki       (column n: d_i)
+    // column-major tiles with an odd pitch: the staging stores of a warp (consecutive pixels of one
+    // column) and the loads of the sums (one pixel, different columns) are both free of bank conflicts
+    // (pixel-major rows of 20 doubles made every staging store an 8-way conflict)
+    constexpr int TP = MGE_TILE + 1;
+    __shared__ double As[NCP][TP];                     // w_i m_ki   (column n: w_i d_i)
+    __shared__ double Bs[NCP][TP];                     // m_ki       (column n: d_i)
     const int r = blockIdx.x;
     if (r >= chunk_rows) return;
     const int64_t row = a.row0 + r;
@@ -205,7 +209,7 @@ __global__ void __launch_bounds__(MGE_SOLVE_THREADS) gram_mge_kernel(const KArgs
     double *gout = a.mge_gram + (size_t)r * MGE_GRAM_STRIDE;
     // [G | b | d'Wd] = A'B with A = [w m_k | w d], B = [m_k | d]  (n1 = n + 1 columns, the data last).
     // Register blocking: a thread owns a 2 x 2 block of entries (columns 2bi, 2bi+1 of A against
-    // 2bj, 2bj+1 of B, bi <= bj) and every Q-th pixel of a tile, so one LDS.128 of A and one of B
+    // 2bj, 2bj+1 of B, bi <= bj) and every Q-th pixel of a tile, so two loads of A and two of B
     // feed four DFMAs (one entry per thread is bound by the shared-memory pipe); the Q pixel
     // slices of an entry are then added in slice order -- a fixed summation order.
     const int n1 = n + 1, NB = (n1 + 1) >> 1, nblk = NB * (NB + 1) / 2;
@@ -245,7 +249,7 @@ __global__ void __launch_bounds__(MGE_SOLVE_THREADS) gram_mge_kernel(const KArgs
 #pragma unroll
             for (int u = 0; u < EPT; ++u) {
                 const int k = sk0 + u * (MGE_SOLVE_THREADS / MGE_TILE);
-                if (k < ncol) { const double v = (double)fv[u]; As[sii][k] = wd * v; Bs[sii][k] = v; }
+                if (k < ncol) { const double v = (double)fv[u]; As[k][sii] = wd * v; Bs[k][sii] = v; }
             }
         }
         __syncthreads();
@@ -253,10 +257,10 @@ __global__ void __launch_bounds__(MGE_SOLVE_THREADS) gram_mge_kernel(const KArgs
         if (gram_thread) {
 #pragma unroll 4
             for (int ii = slice; ii < MGE_TILE; ii += Q) {
-                const double2 av = *reinterpret_cast<const double2 *>(&As[ii][2 * bi]);
-                const double2 bv = *reinterpret_cast<const double2 *>(&Bs[ii][2 * bj]);
-                acc[0] = fma(av.x, bv.x, acc[0]); acc[1] = fma(av.x, bv.y, acc[1]);
-                acc[2] = fma(av.y, bv.x, acc[2]); acc[3] = fma(av.y, bv.y, acc[3]);
+                const double ax = As[2 * bi][ii], ay = As[2 * bi + 1][ii];
+                const double bx = Bs[2 * bj][ii], by = Bs[2 * bj + 1][ii];
+                acc[0] = fma(ax, bx, acc[0]); acc[1] = fma(ax, by, acc[1]);
+                acc[2] = fma(ay, bx, acc[2]); acc[3] = fma(ay, by, acc[3]);
             }
         }
     }
