@@ -134,3 +134,45 @@ def test_mge_recovers_known_amplitudes_and_flags_invalid_rows(api, orc):
     with pytest.raises(api.TinyLensError):
         c0.set_mge(sigmas)
     c0.close()
+
+
+def test_mge_full_size_batch_sampled(api, orc):
+    """configs[1] at the batch bench.py --mode mge times (B = 4096, one chunk): the oracle on a
+    sample of rows, properties on all of them, and the value of a row does not depend on the batch."""
+    import torch
+    w = W.workload(1)
+    prob = W.make_problem(w, orc.render_for_workloads)
+    rows = W.batch_rows(w)
+    assert rows.shape[0] == 4096
+    sigmas = W.mge_sigmas(w, 10)
+    ctx = api.LensContext.from_problem(prob)
+    ctx.set_mge(sigmas)
+    assert api.tl_mge_columns(ctx.handle) == 11 and api.tl_mge_chunk_rows(ctx.handle) >= 4096
+    d = torch.from_numpy(rows).cuda()
+    ll, amps = ctx.loglike_mge(d)
+    sample = np.arange(7, 4096, 273)                       # 15 rows across the batch
+    ll_s, amps_s = ctx.loglike_mge(d[torch.from_numpy(sample).cuda()].contiguous())
+    torch.cuda.synchronize()
+    ctx.close()
+    assert torch.equal(ll[sample], ll_s) and torch.equal(amps[sample], amps_s)
+    ll = ll.cpu().numpy().astype(np.float64); amps = amps.cpu().numpy().astype(np.float64)
+    assert np.all(np.isfinite(ll)) and np.all(amps >= 0.0) and np.all(np.isfinite(amps))
+    cfg = orc.config_of(w)
+    oll, oamps = orc.loglike_mge_batch(cfg, prob.psf, prob.data, prob.noise, rows[sample], sigmas)
+    tol = PT.logl_tol(oll)
+    for t, r in enumerate(sample):
+        M = orc.mge_component_images(cfg, prob.psf[0], rows[r], sigmas)
+        oimg = np.tensordot(oamps[t], M, axes=1)
+        floor = PT.fp32_floor(oimg[None], prob.data[0][None], prob.noise[0][None], w.supersample)[0]
+        assert abs(ll[r] - oll[t]) <= max(tol[t], floor), (r, ll[r] - oll[t], tol[t], floor)
+        gimg = np.tensordot(amps[r], M, axes=1)
+        assert np.abs(gimg - oimg).max() <= 1e-4 * oimg.max()
+    # Eq. 6: the solved likelihood is a maximum over amplitudes, so never below the fixed-amplitude
+    # likelihood of a Sersic lens light that the Gaussian set can reproduce poorly -- not comparable;
+    # what is comparable: more Gaussians never fit worse than a subset of them
+    ctx2 = api.LensContext.from_problem(prob)
+    ctx2.set_mge(sigmas[::2])
+    ll_sub, _ = ctx2.loglike_mge(d[:256].contiguous())
+    ctx2.close()
+    ll_sub = ll_sub.cpu().numpy().astype(np.float64)
+    assert np.all(ll[:256] >= ll_sub - 1e-3 - 2e-6 * np.abs(ll_sub))
