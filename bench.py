@@ -168,11 +168,18 @@ def measured_peaks() -> dict:
         return {}
 
 
-def oracle_time(w: W.Workload, prob, rows: np.ndarray, threads: int = 0):
+def oracle_time(w: W.Workload, prob, rows: np.ndarray, threads: int = 0, mode: str = "fixed", sigmas=None):
     from oracle import oracle as O
     cfg = O.config_of(w)
     t0 = time.perf_counter()
-    _, used = O.loglike_batch(cfg, prob.psf, prob.data, prob.noise, rows, n_lens=w.n_lens, threads=threads)
+    if mode == "linear":
+        O.loglike_linear_batch(cfg, prob.psf, prob.data, prob.noise, rows, n_lens=w.n_lens, threads=threads)
+        used = os.cpu_count()
+    elif mode == "mge":
+        O.loglike_mge_batch(cfg, prob.psf, prob.data, prob.noise, rows, sigmas, n_lens=w.n_lens, threads=threads)
+        used = os.cpu_count()
+    else:
+        _, used = O.loglike_batch(cfg, prob.psf, prob.data, prob.noise, rows, n_lens=w.n_lens, threads=threads)
     return time.perf_counter() - t0, used
 
 
@@ -191,17 +198,23 @@ def run_reference(args, w: W.Workload):
     prob = reference_problem(w)
     rows_all = W.batch_rows(w)
     n = args.ref_rows
+    mode_tag, sigmas = "", None
+    if args.mode == "linear":
+        n = min(n, 128); mode_tag = " (linear amplitudes, NNLS per row)"
+    elif args.mode == "mge":
+        n = min(n, 64); sigmas = W.mge_sigmas(w, args.n_gauss)
+        mode_tag = " (MGE lens light, %d Gaussians + %d source amplitudes by NNLS per row)" % (len(sigmas), w.n_source)
     # bounded sample per step: the first n rows of each step's window of the workload
     times, used = [], 1
     for s in range(args.warmup + args.steps):
         lo = (s * n) % max(1, len(rows_all) - n)
-        dt, used = oracle_time(w, prob, rows_all[lo:lo + n])
+        dt, used = oracle_time(w, prob, rows_all[lo:lo + n], mode=args.mode, sigmas=sigmas)
         if s >= args.warmup:
             times.append(dt)
     tot = float(np.sum(times))
     value = n * len(times) / tot
     line = {
-        "impl": "reference", "metric": METRIC + mass_tag(w), "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "impl": "reference", "metric": METRIC + mass_tag(w) + mode_tag, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / len(times),
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic", "config": config_dict(w, "none (CPU)"),
@@ -540,10 +553,12 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if world != args.gpus and world > 1:
         raise SystemExit("--gpus %d does not match WORLD_SIZE %d" % (args.gpus, world))
-    if args.mode in ("linear", "mge"):
-        run_linear(args, w)
-    elif args.impl == "reference":
+    if args.mode == "mge" and w.n_lens_light != 1:
+        raise SystemExit("bench.py --mode mge needs a workload with lens light (configs 1-4)")
+    if args.impl == "reference":
         run_reference(args, w)
+    elif args.mode in ("linear", "mge"):
+        run_linear(args, w)
     else:
         run_ours(args, w)
 
