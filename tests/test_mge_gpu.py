@@ -176,3 +176,38 @@ def test_mge_full_size_batch_sampled(api, orc):
     ctx2.close()
     ll_sub = ll_sub.cpu().numpy().astype(np.float64)
     assert np.all(ll[:256] >= ll_sub - 1e-3 - 2e-6 * np.abs(ll_sub))
+
+
+def test_mge_call_is_cuda_graph_capturable(api, orc):
+    """NEXT-4: tl_loglike_mge_batch makes no host sync and takes its scratch from the
+    stream-ordered allocator, so a sampler can capture the seven launches in a CUDA graph."""
+    import torch
+    w = W.Workload(index=9, name="mge-graph", ny=30, nx=34, pix_scale=0.12, supersample=2, psf_size=5,
+                   psf_kind="gaussian", psf_fwhm=0.3, psf_beta=0.0, n_lens_light=1, n_source=1,
+                   noise_bg=0.05, noise_exptime=100.0, source_amp=(1.0, 20.0), batch=40)
+    prob = W.make_problem(w, orc.render_for_workloads)
+    rows = W.batch_rows(w)
+    ctx = api.LensContext.from_problem(prob)
+    ctx.set_mge(W.mge_sigmas(w, 6))
+    d = torch.from_numpy(rows).cuda()
+    ref, ref_amps = ctx.loglike_mge(d)
+    ref, ref_amps = ref.clone(), ref_amps.clone()
+    out, amps = torch.empty_like(ref), torch.empty_like(ref_amps)
+    s = torch.cuda.Stream()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(s):
+        ctx.loglike_mge(d, out, amps, stream=s)
+        s.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            ctx.loglike_mge(d, out, amps, stream=s)
+    out.zero_(); amps.zero_()
+    g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(out, ref) and torch.equal(amps, ref_amps)
+    d.copy_(torch.from_numpy(rows[::-1].copy()).cuda())       # new parameters, same buffers
+    g.replay()
+    torch.cuda.synchronize()
+    assert torch.equal(out, ref.flip(0)) and torch.equal(amps, ref_amps.flip(0))
+    del g
+    ctx.close()
