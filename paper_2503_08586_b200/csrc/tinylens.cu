@@ -631,6 +631,10 @@ int64_t mge_chunk_rows(const tl_ctx *c)
     int64_t chunk = (int64_t)(MGE_SCRATCH_BYTES / (ext_row + m_row));
     if (chunk < 1) chunk = 1;
     if (chunk > 65535) chunk = 65535;
+    if (const char *e = std::getenv("TL_MGE_CHUNK_ROWS")) {      // tests: force the multi-chunk path
+        const long v = std::atol(e);
+        if (v >= 1 && v < chunk) chunk = v;
+    }
     return chunk;
 }
 }  // namespace
@@ -659,14 +663,20 @@ int tl_loglike_mge_batch(tl_ctx *c, const float *params, int64_t B, float *logL,
     float *ext = nullptr, *mimg = nullptr;
     double *gram = nullptr;                                    // [chunk][MGE_GRAM_STRIDE + MGE_MAX_COL]
     const size_t g_row = sizeof(double) * (tl::MGE_GRAM_STRIDE + tl::MGE_MAX_COL);
-    if (!cuda_ok(cudaMallocAsync(&rows, sizeof(tl::RowC) * (size_t)chunk, st))) return TL_ENOMEM;
-    if (!cuda_ok(cudaMallocAsync(&ext, ext_row * (size_t)chunk, st)) ||
-        !cuda_ok(cudaMallocAsync(&mimg, m_row * (size_t)chunk, st)) ||
-        !cuda_ok(cudaMallocAsync(&gram, g_row * (size_t)chunk, st))) {
-        cudaFreeAsync(rows, st);
+    // the budget is a target, not a promise: when the device cannot give that much, halve the chunk
+    for (;;) {
+        rows = nullptr; ext = nullptr; mimg = nullptr; gram = nullptr;
+        if (cuda_ok(cudaMallocAsync(&rows, sizeof(tl::RowC) * (size_t)chunk, st)) &&
+            cuda_ok(cudaMallocAsync(&ext, ext_row * (size_t)chunk, st)) &&
+            cuda_ok(cudaMallocAsync(&mimg, m_row * (size_t)chunk, st)) &&
+            cuda_ok(cudaMallocAsync(&gram, g_row * (size_t)chunk, st))) break;
+        cudaGetLastError();                                    // an allocation failure is not sticky
+        if (rows) cudaFreeAsync(rows, st);
         if (ext) cudaFreeAsync(ext, st);
         if (mimg) cudaFreeAsync(mimg, st);
-        return TL_ENOMEM;
+        if (gram) cudaFreeAsync(gram, st);
+        if (chunk == 1) return TL_ENOMEM;
+        chunk = (chunk + 1) / 2;
     }
     // (the pitch padding of ext, which must read as finite zeros, is written by mge_gauss_kernel)
     const int64_t rows_per_lens = B / c->cfg.n_lens;

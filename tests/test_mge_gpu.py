@@ -211,3 +211,25 @@ def test_mge_call_is_cuda_graph_capturable(api, orc):
     assert torch.equal(out, ref.flip(0)) and torch.equal(amps, ref_amps.flip(0))
     del g
     ctx.close()
+
+
+def test_mge_chunked_call_equals_single_chunk(api, orc, monkeypatch):
+    """A call larger than the scratch budget is processed in chunks (TL_MGE_CHUNK_ROWS forces that
+    here, with a ragged last chunk, on three lenses): identical bits."""
+    import torch
+    w = W.workload(3).scaled(batch=3 * 14, n_lens=3)
+    prob = W.make_problem(w, orc.render_for_workloads)
+    rows = W.batch_rows(w, 14)
+    rows[5, 0] = -1.0                                   # an invalid row inside a chunk
+    ctx = api.LensContext.from_problem(prob)
+    ctx.set_mge(W.mge_sigmas(w, 7))
+    d = torch.from_numpy(rows).cuda()
+    ll1, am1 = ctx.loglike_mge(d)
+    torch.cuda.synchronize()
+    monkeypatch.setenv("TL_MGE_CHUNK_ROWS", "5")
+    assert api.tl_mge_chunk_rows(ctx.handle) == 5
+    ll2, am2 = ctx.loglike_mge(d)
+    torch.cuda.synchronize()
+    ctx.close()
+    assert torch.equal(ll1, ll2) and torch.equal(am1.nan_to_num(-1.0), am2.nan_to_num(-1.0))
+    assert ll1[5].item() == -np.inf
