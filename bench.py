@@ -267,11 +267,17 @@ def run_ours(args, w: W.Workload):
 
     prob = W.make_problem(w, gpu_render)
     ctx = api.LensContext.from_problem(prob)
+    PREC = {"fp32": api.TL_PRECISION_FP32, "fp64": api.TL_PRECISION_FP64, "fp64-libm": api.TL_PRECISION_FP64_LIBM,
+            "auto": api.TL_PRECISION_AUTO}
+    if args.precision != "fp32":
+        ctx.set_precision(PREC[args.precision])
     info = ctx.info()
     # each rank draws its own rows (weak scaling): stream id offset by rank
     rows = W.batch_rows(w) if rank == 0 else \
         np.concatenate([W.draw_params(w, W.rng_for(w.index, W.STREAM_BATCH + 16 * rank, l), w.rows_per_lens)
                         for l in range(w.n_lens)], axis=0)
+    if args.rows == "near-truth":
+        rows = W.near_truth_rows(prob, w.rows_per_lens)
     B = rows.shape[0]
     d_rows = torch.from_numpy(rows).to(dev)
     d_out = torch.empty(B, dtype=torch.float32, device=dev)
@@ -345,7 +351,8 @@ def run_ours(args, w: W.Workload):
     line = {
         "metric": METRIC + mass_tag(w), "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "scaling": "weak", "vs_baseline": None, "dtype": {"fp32": "f32", "auto": "f32+f64"}.get(args.precision, "f64"),
+        "data": "synthetic", "precision": args.precision, "rows": args.rows,
         "config": config_dict(w, "flushed between steps (256 MiB fill)"),
         "pixel_evals_per_s": value * w.ny * w.nx,
         "sample_evals_per_s": value * om["samples"],
@@ -525,6 +532,20 @@ def run_mge(args, w: W.Workload, prob, ctx, rows):
     print(json.dumps(line))
 
 
+def run_peaks(args):
+    """`--peaks`: the committed pipe micro-benchmarks (tl_measure_peaks) as one JSON line."""
+    import torch
+    from paper_2503_08586_b200 import api
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(0)
+    with ClockSampler(0) as clk:
+        probes, err = api.tl_measure_peaks()
+    print(json.dumps({"peaks": probes, "clocks": clk.summary(),
+                      "fp64_seed_rel_err": {"rcp.approx.f64": err[0], "rcp + 1 Newton": err[1],
+                                            "rsqrt.approx.f64": err[2], "rsqrt + 1 Newton": err[3]}}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -544,7 +565,19 @@ def main():
     ap.add_argument("--mass", default="sie", choices=["sie", "epl"],
                     help="sie: the headline workload; epl: the same workload with the elliptical power-law mass "
                          "model and a free slope per row (NEXT-2, PAPER.md Eq. 12) -- a secondary line")
+    ap.add_argument("--precision", default="fp32", choices=["fp32", "fp64", "fp64-libm", "auto"],
+                    help="fp32: the headline kernels; fp64: every per-sample quantity in FP64 with polynomial functions "
+                         "(meets north_star on rows near the best fit too); fp64-libm: CUDA's double math library "
+                         "(slow cross-check); auto: FP32, then FP64 for the rows whose FP32 error bound exceeds the tolerance")
+    ap.add_argument("--rows", default="prior", choices=["prior", "near-truth"],
+                    help="prior: the BASELINE batch (independent prior draws); near-truth: truth (1 + 1e-3 N(0,1)) rows, "
+                         "the regime a converged sampler works in (SURVEY.md 8(d) near-truth slice)")
+    ap.add_argument("--peaks", action="store_true",
+                    help="run the pipe micro-benchmarks (tl_measure_peaks: FFMA, FFMA2, MUFU, DFMA and mixes) and exit")
     args = ap.parse_args()
+    if args.peaks:
+        run_peaks(args)
+        return
     w = W.workload(args.config)
     if args.mass == "epl":
         w = w.with_epl()

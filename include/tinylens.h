@@ -37,8 +37,16 @@
  * Invalid rows are not errors: hypot(e1,e2) >= 1, theta_E < 0, r_e <= 0, n <= 0, a slope outside
  * 1 < gamma < 3, or any non-finite entry gives logL = -INFINITY and a NaN-filled image for that row.
  *
- * Threading: a context is immutable after tl_create and may be used from several host
- * threads / streams concurrently; per-call scratch comes from the stream-ordered allocator.
+ * Threading: what tl_create builds (device copies of psf / data / noise, launch geometry, options)
+ * never changes afterwards, and batch calls may be issued from several host threads / streams
+ * concurrently: per-call scratch comes from a stream-ordered memory pool owned by the context.
+ * The following state IS mutable and must only be changed while no call is in flight on the
+ * context: the precision mode (tl_set_precision), the MGE Gaussian set (tl_set_mge), the
+ * profiling switch and its event pair (tl_set_profiling: a single-thread benchmark facility),
+ * and the staging slots of the asynchronous host entry (tl_loglike_batch_host_async / tl_wait:
+ * one submitting thread per context).
+ * A call made while another CUDA device is current switches to the context's device for its
+ * duration and restores the caller's device before returning.
  */
 #ifndef TINYLENS_H
 #define TINYLENS_H
@@ -55,8 +63,14 @@ extern "C" {
 #define TL_ECUDA   -3   /* no usable CUDA device, or a CUDA runtime call failed               */
 #define TL_ESIZE   -4   /* configuration exceeds what the kernels support (see tl_create)     */
 
-#define TL_PRECISION_FP32 0 /* default: the FP32 / MUFU kernels      */
-#define TL_PRECISION_FP64 1 /* validation mode: the same model in double precision on the device   */
+#define TL_PRECISION_FP32      0 /* default: the FP32 / MUFU kernels (DESIGN.md 6 "Precision design")        */
+#define TL_PRECISION_FP64      1 /* every per-sample quantity in FP64, functions as hand-ordered            */
+                                 /* polynomials (csrc/tl_dp.cuh): meets |dlogL| <= max(1e-3, 1e-6 |logL|)    */
+                                 /* on every row, rows near the best fit included                            */
+#define TL_PRECISION_FP64_LIBM 2 /* the same model with CUDA's double math library (csrc/tl_precise.cuh):   */
+                                 /* slow; an independent check of the polynomial FP64 path                  */
+#define TL_PRECISION_AUTO      3 /* FP32 for every row, then the rows whose first-order FP32 error bound    */
+                                 /* exceeds the tolerance are re-evaluated in FP64 (rows near the best fit) */
 
 #define TL_EDGE_EXTEND 0 /* evaluate the analytic model on a border of h = (K-1)/2 pixels so   */
                          /* every output pixel sees its full PSF support (Eq. 3 with only the  */
@@ -106,14 +120,16 @@ typedef struct {
 } tl_info;
 
 /*
- * tl_create -- build an immutable context (image d, noise sigma,
- * PSF kernel K are fixed per lens; only the parameter vector varies between evaluations).
+ * tl_create -- build a context (image d, noise sigma, PSF kernel K are
+ * fixed per lens; only the parameter vector varies between evaluations).
  *   out        receives the handle (set to NULL on failure)
  *   cfg        see tl_config
- *   psf        HOST pointer, float [n_lens][psf_ny][psf_nx], psf_ny == psf_nx odd, row-major,
- *              K[a][b] with a the row (y) index.  Used as given.
- *   data       HOST pointer, float [n_lens][ny][nx], row-major (d_i of Eq. 5)
- *   noise      HOST pointer, float [n_lens][ny][nx], every value finite and > 0 (sigma_i)
+ *   psf        HOST or DEVICE pointer, float [n_lens][psf_ny][psf_nx], psf_ny == psf_nx odd,
+ *              row-major, K[a][b] with a the row (y) index.  Used as given.
+ *   data       HOST or DEVICE pointer, float [n_lens][ny][nx], row-major (d_i of Eq. 5)
+ *   noise      HOST or DEVICE pointer, float [n_lens][ny][nx], every value finite and > 0 (sigma_i)
+ *              (device arrays are recognised with cudaPointerGetAttributes and staged through
+ *              the host: 1/sigma^2 and the Eq. 5 constant are prepared there in FP64)
  *   cuda_stream  a cudaStream_t (NULL = default stream) on which uploads are enqueued;
  *              the call synchronises that stream before returning, so the host arrays may
  *              be freed immediately.
@@ -125,6 +141,31 @@ typedef struct {
 int tl_create(tl_ctx **out, const tl_config *cfg,
               const float *psf, int32_t psf_ny, int32_t psf_nx,
               const float *data, const float *noise, void *cuda_stream);
+
+/*
+ * tl_create_ex -- tl_create with explicit options (NULL = all automatic, which is tl_create).
+ * These replace every environment variable the library once read; nothing in the library calls
+ * getenv.  Zero-initialise the struct and set small_batch_rows = -1 for the defaults.
+ */
+typedef struct {
+    int32_t small_batch_rows;   /* -1 automatic (half the SM count when the path supports it),  */
+                                /*  0 never spread a row over several CTAs (every call runs the */
+                                /*    fused kernel), > 0 calls of at most this many rows do      */
+    int32_t force_split;        /* 1: stage the binned image through global memory (the large-  */
+                                /*    image path) even when it fits in shared memory            */
+    int32_t block_threads;      /* 0 automatic, else threads per CTA of the fused kernel        */
+                                /*    (multiple of 32, 32..512)                                  */
+    int32_t linear_staged;      /* 1: tl_loglike_linear_batch stages the component images       */
+                                /*    through global memory even when the fused pipeline fits   */
+    int64_t mge_chunk_rows;     /* 0 automatic, else an upper limit on rows per MGE chunk       */
+    int64_t scratch_keep_bytes; /* 0 = 2 GiB: freed per-call scratch the context's memory pool  */
+                                /*    keeps cached between calls                                */
+    double  refine_tau;         /* 0 default, else the selective-FP64 threshold in units of     */
+                                /*    sigma_min                                  */
+} tl_options;
+int tl_create_ex(tl_ctx **out, const tl_config *cfg,
+                 const float *psf, int32_t psf_ny, int32_t psf_nx,
+                 const float *data, const float *noise, const tl_options *opt, void *cuda_stream);
 
 /* Number of floats per parameter row, P = 7 (8 for TL_MASS_EPL) + 7*n_lens_light + 7*n_source;
  * < 0 on NULL.                                                                                */
@@ -166,8 +207,11 @@ int tl_render_batch(tl_ctx *ctx, const float *params, int64_t B, float *images, 
  *   logL     DEVICE pointer, float [B], written (-INFINITY for invalid rows)
  *   amps     DEVICE pointer, float [B][N_l + N_s] (lens light first, then sources), written
  *            (NaN for invalid rows), or NULL
- * Asynchronous on cuda_stream; bitwise reproducible.  Always uses the staged pipeline
- * (component images through global memory).  Returns TL_OK, TL_EINVAL, TL_ENOMEM, TL_ECUDA,
+ * Asynchronous on cuda_stream; bitwise reproducible.  Two pipelines with identical results
+ * (bit for bit): fused (the component images of a row stay in shared memory; chosen when they
+ * fit) and staged (component images through global memory; larger images, or
+ * tl_options.linear_staged).  The NNLS problem is solved on the Gram matrix by the active-set
+ * iteration of Bro & De Jong.  Returns TL_OK, TL_EINVAL, TL_ENOMEM, TL_ECUDA,
  * or TL_ESIZE when the PSF tile does not fit in shared memory.
  */
 int tl_loglike_linear_batch(tl_ctx *ctx, const float *params, int64_t B, float *logL, float *amps,
@@ -246,6 +290,28 @@ int tl_set_precision(tl_ctx *ctx, int precision);
  */
 int tl_set_profiling(tl_ctx *ctx, int enable);
 int tl_last_kernel_ms(tl_ctx *ctx, float *ms);
+
+/*
+ * tl_measure_peaks -- issue-rate micro-benchmarks of the pipes that bound the hot path
+ * (DESIGN.md 5.2 "Roofline that bounds it: plain ALU issue"; SURVEY.md 8(d) "verify by
+ * micro-benchmark on the box before quoting"): scalar FFMA, packed FFMA2 (fma.rn.f32x2), MUFU,
+ * DFMA and mixes of them, one persistent CTA of 1024 threads per SM on the current device.
+ *   out        HOST pointer, tl_peak [n_max], written
+ *   n_max      capacity of out (11 probes exist)
+ *   seed_err4  HOST pointer, double [4], or NULL: worst relative error over [1, 4) of
+ *              rcp.approx.f64, of one Newton step on it, of rsqrt.approx.f64, and of one Newton
+ *              step on it (the seeds of the FP64 kernels' divisions and square roots)
+ * Synchronous (default stream).  Returns the number of probes written (> 0), or TL_EINVAL,
+ * TL_ENOMEM, TL_ECUDA.  `python bench.py --peaks` prints the table.
+ */
+typedef struct {
+    char   name[64];           /* instruction mix of one loop trip                              */
+    double inst_per_clk_sm;    /* thread-instructions issued per SM clock                       */
+    double fma_per_clk_sm;     /* FMAs (FP32 or FP64) retired per SM clock in that mix          */
+    double sm_mhz;             /* SM clock the probe ran at (cycles / event time)               */
+    double ms;                 /* duration of the probe kernel                                  */
+} tl_peak;
+int tl_measure_peaks(tl_peak *out, int32_t n_max, double *seed_err4);
 
 /* Release a context and its device memory (NULL is allowed).                                  */
 void tl_destroy(tl_ctx *ctx);

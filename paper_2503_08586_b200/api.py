@@ -19,7 +19,7 @@ LIB_PATH = os.environ.get("TL_LIB") or os.path.join(_HERE, "libtinylens.so")   #
 
 TL_OK, TL_EINVAL, TL_ENOMEM, TL_ECUDA, TL_ESIZE = 0, -1, -2, -3, -4
 TL_EDGE_EXTEND, TL_EDGE_ZERO = 0, 1
-TL_PRECISION_FP32, TL_PRECISION_FP64 = 0, 1
+TL_PRECISION_FP32, TL_PRECISION_FP64, TL_PRECISION_FP64_LIBM, TL_PRECISION_AUTO = 0, 1, 2, 3
 TL_MASS_SIE, TL_MASS_EPL = 0, 1
 
 
@@ -45,6 +45,17 @@ class tl_info(C.Structure):
                 ("small_batch_rows", C.c_int32), ("chunk_rows", C.c_int32)]
 
 
+class tl_options(C.Structure):
+    _fields_ = [("small_batch_rows", C.c_int32), ("force_split", C.c_int32), ("block_threads", C.c_int32),
+                ("linear_staged", C.c_int32), ("mge_chunk_rows", C.c_int64), ("scratch_keep_bytes", C.c_int64),
+                ("refine_tau", C.c_double)]
+
+
+class tl_peak(C.Structure):
+    _fields_ = [("name", C.c_char * 64), ("inst_per_clk_sm", C.c_double), ("fma_per_clk_sm", C.c_double),
+                ("sm_mhz", C.c_double), ("ms", C.c_double)]
+
+
 _lib = None
 
 
@@ -66,6 +77,8 @@ def load(build_if_missing: bool = True):
     vp, i32, i64, fp = C.c_void_p, C.c_int32, C.c_int64, C.POINTER(C.c_float)
     L.tl_create.restype = C.c_int
     L.tl_create.argtypes = [C.POINTER(vp), C.POINTER(tl_config), fp, i32, i32, fp, fp, vp]
+    L.tl_create_ex.restype = C.c_int
+    L.tl_create_ex.argtypes = [C.POINTER(vp), C.POINTER(tl_config), vp, i32, i32, vp, vp, C.POINTER(tl_options), vp]
     L.tl_param_count.restype = C.c_int; L.tl_param_count.argtypes = [vp]
     L.tl_get_info.restype = C.c_int; L.tl_get_info.argtypes = [vp, C.POINTER(tl_info)]
     L.tl_loglike_batch.restype = C.c_int; L.tl_loglike_batch.argtypes = [vp, vp, i64, vp, vp]
@@ -79,6 +92,7 @@ def load(build_if_missing: bool = True):
     L.tl_set_precision.restype = C.c_int; L.tl_set_precision.argtypes = [vp, C.c_int]
     L.tl_set_profiling.restype = C.c_int; L.tl_set_profiling.argtypes = [vp, C.c_int]
     L.tl_last_kernel_ms.restype = C.c_int; L.tl_last_kernel_ms.argtypes = [vp, C.POINTER(C.c_float)]
+    L.tl_measure_peaks.restype = C.c_int; L.tl_measure_peaks.argtypes = [C.POINTER(tl_peak), i32, C.POINTER(C.c_double)]
     L.tl_destroy.restype = None; L.tl_destroy.argtypes = [vp]
     L.tl_strerror.restype = C.c_char_p; L.tl_strerror.argtypes = [C.c_int]
     L.tl_version.restype = C.c_char_p; L.tl_version.argtypes = []
@@ -111,20 +125,36 @@ def _f32c(a) -> np.ndarray:
     return np.ascontiguousarray(a, dtype=np.float32)
 
 
+def _host_or_device(a):
+    """numpy array / host tensor -> (keep-alive, pointer, size, last two dims); CUDA float32 tensors are passed as they are."""
+    try:
+        import torch
+        if isinstance(a, torch.Tensor) and a.is_cuda:
+            if a.dtype != torch.float32 or not a.is_contiguous():
+                raise TinyLensError(TL_EINVAL, "tl_create (device arrays must be contiguous float32)")
+            return a, a.data_ptr(), a.numel(), tuple(a.shape[-2:])
+        if isinstance(a, torch.Tensor):
+            a = a.numpy()
+    except ImportError:
+        pass
+    h = _f32c(a)
+    return h, h.ctypes.data, h.size, tuple(h.shape[-2:])
+
+
 def tl_create(ny, nx, pix_scale, supersample, n_lens_light, n_source, psf, data, noise,
-              edge_mode=TL_EDGE_EXTEND, n_lens=1, stream=None, mass_model=TL_MASS_SIE) -> int:
-    """-> opaque handle (int).  psf [n_lens,K,K], data/noise [n_lens,ny,nx]: host float32 arrays."""
+              edge_mode=TL_EDGE_EXTEND, n_lens=1, stream=None, mass_model=TL_MASS_SIE, options=None) -> int:
+    """-> opaque handle (int).  psf [n_lens,K,K], data/noise [n_lens,ny,nx]: host float32 arrays or CUDA
+    float32 tensors.  options: dict of tl_options fields (tl_create_ex), e.g. {"small_batch_rows": 0}."""
     L = load()
-    p, d, s = _f32c(psf), _f32c(data), _f32c(noise)
-    K = p.shape[-1]
-    if p.size != n_lens * K * K or p.shape[-2] != K:
+    (pk, pp, pn, pshape), (dk, dp_, dn, _), (sk, sp, sn, _) = _host_or_device(psf), _host_or_device(data), _host_or_device(noise)
+    K = pshape[-1]
+    if pn != n_lens * K * K or pshape[-2] != K:
         raise TinyLensError(TL_EINVAL, "tl_create (psf shape)")
-    if d.size != n_lens * ny * nx or s.size != n_lens * ny * nx:
+    if dn != n_lens * ny * nx or sn != n_lens * ny * nx:
         raise TinyLensError(TL_EINVAL, "tl_create (data/noise shape)")
     cfg = tl_config(int(ny), int(nx), float(pix_scale), int(supersample), int(n_lens_light),
                     int(n_source), int(edge_mode), int(n_lens), int(mass_model))
     h = C.c_void_p()
-    fp = C.POINTER(C.c_float)
     sh = 0
     try:
         import torch
@@ -132,8 +162,13 @@ def tl_create(ny, nx, pix_scale, supersample, n_lens_light, n_source, psf, data,
             sh = _stream_handle(stream)
     except ImportError:
         pass
-    _check(L.tl_create(C.byref(h), C.byref(cfg), p.ctypes.data_as(fp), K, K,
-                       d.ctypes.data_as(fp), s.ctypes.data_as(fp), sh), "tl_create")
+    opt = tl_options(small_batch_rows=-1)
+    for k, v in (options or {}).items():
+        if k not in dict(tl_options._fields_):
+            raise TinyLensError(TL_EINVAL, "tl_create (unknown option %r)" % k)
+        setattr(opt, k, v)
+    _check(L.tl_create_ex(C.byref(h), C.byref(cfg), pp, K, K, dp_, sp, C.byref(opt), sh), "tl_create_ex")
+    del pk, dk, sk
     return h.value
 
 
@@ -255,6 +290,17 @@ def tl_last_kernel_ms(handle: int) -> float:
     return float(ms.value)
 
 
+def tl_measure_peaks():
+    """-> (list of dicts, one per probe; [rcp seed, rcp + Newton, rsqrt seed, rsqrt + Newton] worst relative errors)."""
+    arr = (tl_peak * 16)()
+    err = (C.c_double * 4)()
+    n = load().tl_measure_peaks(arr, 16, err)
+    if n < 0:
+        raise TinyLensError(n, "tl_measure_peaks")
+    return ([{"name": arr[i].name.decode(), "inst_per_clk_sm": arr[i].inst_per_clk_sm, "fma_per_clk_sm": arr[i].fma_per_clk_sm,
+              "sm_mhz": arr[i].sm_mhz, "ms": arr[i].ms} for i in range(n)], [float(x) for x in err])
+
+
 def tl_destroy(handle: Optional[int]):
     if handle:
         load().tl_destroy(handle)
@@ -264,19 +310,19 @@ class LensContext:
     """RAII wrapper: ``ctx = LensContext.from_problem(problem); ctx.loglike(params)``."""
 
     def __init__(self, ny, nx, pix_scale, supersample, n_lens_light, n_source, psf, data, noise,
-                 edge_mode=TL_EDGE_EXTEND, n_lens=1, stream=None, mass_model=TL_MASS_SIE):
+                 edge_mode=TL_EDGE_EXTEND, n_lens=1, stream=None, mass_model=TL_MASS_SIE, options=None):
         self.ny, self.nx, self.n_lens = int(ny), int(nx), int(n_lens)
         self.n_comp = int(n_lens_light) + int(n_source)
         self.handle = tl_create(ny, nx, pix_scale, supersample, n_lens_light, n_source, psf, data,
-                                noise, edge_mode, n_lens, stream, mass_model)
+                                noise, edge_mode, n_lens, stream, mass_model, options)
         self.n_params = tl_param_count(self.handle)
 
     @classmethod
-    def from_problem(cls, prob, stream=None):
+    def from_problem(cls, prob, stream=None, options=None):
         w = prob.workload
         return cls(w.ny, w.nx, w.pix_scale, w.supersample, w.n_lens_light, w.n_source,
                    prob.psf, prob.data, prob.noise, w.edge_mode, w.n_lens, stream,
-                   getattr(w, "mass_model", TL_MASS_SIE))
+                   getattr(w, "mass_model", TL_MASS_SIE), options)
 
     def info(self) -> dict:
         return tl_get_info(self.handle)

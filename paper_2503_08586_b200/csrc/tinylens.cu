@@ -16,9 +16,17 @@
 #include "tl_kernels.cuh"
 #include "tl_dispatch.h"
 #include "tl_precise.cuh"
+#include "tl_dp.cuh"
 #include "tl_mge.cuh"
 
 #define TL_VERSION_STRING "tinylens-b200 0.2 (sm_100a)"
+
+typedef void (*dp_trace_fn)(const tl::DpArgs);
+static dp_trace_fn tl_trace_dp_for(int nll, int nsrc)
+{
+    if (nll == 0) return nsrc == 1 ? tl::trace_dp_kernel<0, 1> : tl::trace_dp_kernel<0, 2>;
+    return nsrc == 1 ? tl::trace_dp_kernel<1, 1> : tl::trace_dp_kernel<1, 2>;
+}
 
 struct tl_ctx {
     tl_config cfg;
@@ -27,7 +35,13 @@ struct tl_ctx {
     int P = 0, lens_np = 7, K = 0, Kp = 0, h = 0, He = 0, We = 0, pitch = 0, n_comp = 0;
     // device arrays (library-owned)
     float *psf = nullptr, *data = nullptr, *wgt = nullptr, *sigma_min = nullptr, *noise = nullptr;
-    int precision = 0;            // TL_PRECISION_FP32 / TL_PRECISION_FP64
+    double *wgt64 = nullptr;      // 1 / sigma^2 in FP64 (the double-precision path, tl_dp.cuh)
+    int precision = 0;            // TL_PRECISION_*
+    // double-precision path: launch geometry
+    int dp_Wp = 0, dp_band_rows = 0, dp_n_bands = 0, dp_trace_grid = 0;
+    size_t dp_conv_smem = 0;
+    int64_t dp_chunk_rows = 0;
+    void (*dp_trace)(const tl::DpArgs) = nullptr;
     double *lconst = nullptr;
     double lconst0 = 0.0, sigma_min0 = 0.0;
     // launch geometry
@@ -56,6 +70,8 @@ struct tl_ctx {
     float *mge_c = nullptr;       // device [n_gauss]: log2(e) / (2 sigma_k^2)
     int n_gauss = 0;
     double refine_tau = 7.5e-4;   // x S at create: a pixel averages S^2 samples
+    tl_options opt;               // create-time options (tl_create_ex); defaults = automatic
+    cudaMemPool_t pool = nullptr; // library-owned stream-ordered pool: per-call scratch (never the device's default pool)
     // benchmark facility (tl_set_profiling): events around the dominant kernel of the last call
     int profile = 0;
     cudaEvent_t ev0 = nullptr, ev1 = nullptr;
@@ -82,6 +98,31 @@ constexpr size_t EXT_SCRATCH_BYTES = 512u << 20; // split path: binned-image scr
 constexpr size_t MGE_SCRATCH_BYTES = (size_t)8 << 30;  // MGE: component images of a chunk (180 GB of HBM: keep whole batches resident)
 
 inline bool cuda_ok(cudaError_t e) { return e == cudaSuccess; }
+
+// The context is bound to the device that was current at tl_create; calls made with another
+// device current switch to it for their duration and restore the caller's device on return.
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = true, switched = false;
+    explicit DeviceGuard(int want)
+    {
+        ok = cuda_ok(cudaGetDevice(&prev));
+        if (ok && prev != want) { ok = cuda_ok(cudaSetDevice(want)); switched = ok; }
+    }
+    ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
+
+// per-call scratch: stream-ordered allocation from the context's own pool
+template <class T>
+inline bool pool_alloc(const tl_ctx *c, T **p, size_t bytes, cudaStream_t st)
+{
+    *p = nullptr;
+    void *v = nullptr;
+    const cudaError_t e = c->pool ? cudaMallocFromPoolAsync(&v, bytes ? bytes : 1, c->pool, st) : cudaMallocAsync(&v, bytes ? bytes : 1, st);
+    if (e != cudaSuccess) { cudaGetLastError(); return false; }
+    *p = static_cast<T *>(v);
+    return true;
+}
 
 size_t fused_smem_bytes(const tl_ctx *c)
 {
@@ -133,9 +174,9 @@ int run_small_batch(tl_ctx *c, const float *params, int64_t B, float *logL, floa
     const size_t ext_bytes = img_bytes + 2 * sizeof(int) * (size_t)nb;     // + finished-band counters
     tl::RowC *rows = nullptr;
     float *ext = nullptr, *cblk = nullptr;
-    if (!cuda_ok(cudaMallocAsync(&rows, sizeof(tl::RowC) * (size_t)nb, st))) return TL_ENOMEM;
-    if (!cuda_ok(cudaMallocAsync(&ext, ext_bytes, st))) { cudaFreeAsync(rows, st); return TL_ENOMEM; }
-    if (logL && !cuda_ok(cudaMallocAsync(&cblk, sizeof(float) * (size_t)nb * npair * nsx, st))) {
+    if (!pool_alloc(c, &rows, sizeof(tl::RowC) * (size_t)nb, st)) return TL_ENOMEM;
+    if (!pool_alloc(c, &ext, ext_bytes, st)) { cudaFreeAsync(rows, st); return TL_ENOMEM; }
+    if (logL && !pool_alloc(c, &cblk, sizeof(float) * (size_t)nb * npair * nsx, st)) {
         cudaFreeAsync(rows, st); cudaFreeAsync(ext, st); return TL_ENOMEM;
     }
     cudaMemsetAsync(ext, 0, ext_bytes, st);          // pitch padding must read as finite zeros
@@ -170,25 +211,78 @@ int run_small_batch(tl_ctx *c, const float *params, int64_t B, float *logL, floa
     return rc;
 }
 
+// The double-precision path (tl_dp.cuh) over rows [0, B) of `params`, or -- with row_index /
+// n_rows_dev -- over the rows listed in device memory (AUTO mode: the count is not known on the
+// host, so every chunk is launched and the kernels of an empty chunk return at once).
+int run_dp(tl_ctx *c, const float *params, int64_t B, float *logL, float *images, cudaStream_t st,
+           const int *row_index, const int *n_rows_dev)
+{
+    const int64_t rows_per_lens = B / c->cfg.n_lens;
+    const int64_t chunk = c->dp_chunk_rows < B ? c->dp_chunk_rows : B;
+    tl::RowD *rows = nullptr;
+    double *ext = nullptr, *partial = nullptr;
+    const size_t ext_row = sizeof(double) * (size_t)c->He * c->dp_Wp;
+    if (!pool_alloc(c, &rows, sizeof(tl::RowD) * (size_t)chunk, st)) return TL_ENOMEM;
+    if (!pool_alloc(c, &ext, ext_row * (size_t)chunk, st) ||
+        !pool_alloc(c, &partial, sizeof(double) * (size_t)chunk * c->dp_n_bands, st)) {
+        cudaFreeAsync(rows, st);
+        if (ext) cudaFreeAsync(ext, st);
+        return TL_ENOMEM;
+    }
+    // the pitch padding (Wp - We <= 1 column) is read by discarded strip lanes only, but must be finite
+    if (c->dp_Wp != c->We) cudaMemsetAsync(ext, 0, ext_row * (size_t)chunk, st);
+    int rc = TL_OK;
+    for (int64_t r0 = 0; r0 < B && rc == TL_OK; r0 += chunk) {
+        const int64_t nb = (B - r0 < chunk) ? (B - r0) : chunk;
+        tl::DpArgs a;
+        memset(&a, 0, sizeof(a));
+        a.params = params; a.rows = rows; a.row_index = row_index; a.n_rows_dev = n_rows_dev;
+        a.n_rows = (int)nb; a.list_offset = row_index ? (int)r0 : 0;
+        a.row0 = r0; a.rows_per_lens = rows_per_lens;
+        a.psf = c->psf; a.data = c->data; a.wgt64 = c->wgt64; a.lconst = c->lconst;
+        a.ext = ext; a.partial = logL ? partial : nullptr; a.logL = logL; a.images = images;
+        a.P = c->P; a.ny = c->cfg.ny; a.nx = c->cfg.nx; a.K = c->K; a.Kp = c->Kp; a.h = c->h;
+        a.He = c->He; a.We = c->We; a.Wp = c->dp_Wp; a.S = c->cfg.supersample;
+        a.n_lens_light = c->cfg.n_lens_light; a.n_comp = c->n_comp;
+        a.edge_zero = c->cfg.edge_mode == TL_EDGE_ZERO; a.mass_model = c->cfg.mass_model; a.lens_np = c->lens_np;
+        a.band_rows = c->dp_band_rows; a.n_bands = c->dp_n_bands;
+        a.CW = c->CW; a.CH = c->CH; a.tiles_x = (c->We + c->CW - 1) / c->CW; a.tiles_y = (c->He + c->CH - 1) / c->CH;
+        a.u = c->cfg.pix_scale / (2.0 * c->cfg.supersample);
+        tl::prologue_dp_kernel<<<(unsigned)((nb + 63) / 64), 64, 0, st>>>(a);
+        // one warp per (row, tile): no more CTAs than there is work for
+        const int64_t items = nb * a.tiles_x * a.tiles_y;
+        int grid = c->dp_trace_grid;
+        if ((int64_t)grid * 8 > items) grid = (int)((items + 7) / 8);
+        if (c->profile) cudaEventRecord(c->ev0, st);
+        c->dp_trace<<<grid, 256, 0, st>>>(a);
+        if (c->profile) { cudaEventRecord(c->ev1, st); c->prof_pending = 1; }
+        tl::conv_dp_kernel<<<dim3((unsigned)nb, (unsigned)c->dp_n_bands), 256, c->dp_conv_smem, st>>>(a);
+        if (logL) tl::finalize_dp_kernel<<<(unsigned)((nb + 127) / 128), 128, 0, st>>>(a);
+        if (!cuda_ok(cudaGetLastError())) rc = TL_ECUDA;
+    }
+    cudaFreeAsync(rows, st); cudaFreeAsync(ext, st); cudaFreeAsync(partial, st);
+    return rc;
+}
+
 int run_batch(tl_ctx *c, const float *params, int64_t B, float *logL, float *images, cudaStream_t st)
 {
     if (!c || B < 0) return TL_EINVAL;
     if (B == 0) return TL_OK;
     if (!params || (!logL && !images)) return TL_EINVAL;
     if (B % c->cfg.n_lens) return TL_EINVAL;
-    int dev = -1;
-    if (!cuda_ok(cudaGetDevice(&dev))) return TL_ECUDA;
-    if (dev != c->device && !cuda_ok(cudaSetDevice(c->device))) return TL_ECUDA;
+    DeviceGuard guard(c->device);
+    if (!guard.ok) return TL_ECUDA;
 
     const int64_t rows_per_lens = B / c->cfg.n_lens;
-    if (c->precision == TL_PRECISION_FP64) {
+    if (c->precision == TL_PRECISION_FP64) return run_dp(c, params, B, logL, images, st, nullptr, nullptr);
+    if (c->precision == TL_PRECISION_FP64_LIBM) {
         const size_t ext_row = sizeof(double) * (size_t)c->He * c->We;
         int64_t pch = (int64_t)(EXT_SCRATCH_BYTES / ext_row);
         if (pch < 1) pch = 1;
         if (pch > 65535) pch = 65535;
         if (pch > B) pch = B;
         double *pext = nullptr;
-        if (!cuda_ok(cudaMallocAsync(&pext, ext_row * (size_t)pch, st))) return TL_ENOMEM;
+        if (!pool_alloc(c, &pext, ext_row * (size_t)pch, st)) return TL_ENOMEM;
         int prc = TL_OK;
         for (int64_t r0 = 0; r0 < B && prc == TL_OK; r0 += pch) {
             const int64_t nb = (B - r0 < pch) ? (B - r0) : pch;
@@ -217,11 +311,11 @@ int run_batch(tl_ctx *c, const float *params, int64_t B, float *logL, float *ima
     tl::RowC *rows = nullptr;
     float *ext = nullptr;
     double *partial = nullptr;
-    if (!cuda_ok(cudaMallocAsync(&rows, sizeof(tl::RowC) * (size_t)chunk, st))) return TL_ENOMEM;
+    if (!pool_alloc(c, &rows, sizeof(tl::RowC) * (size_t)chunk, st)) return TL_ENOMEM;
     if (c->path == 1) {
         const size_t ext_bytes = sizeof(float) * (size_t)chunk * c->He * c->pitch;
-        if (!cuda_ok(cudaMallocAsync(&ext, ext_bytes, st)) ||
-            !cuda_ok(cudaMallocAsync(&partial, sizeof(double) * (size_t)chunk * c->n_tiles, st))) {
+        if (!pool_alloc(c, &ext, ext_bytes, st) ||
+            !pool_alloc(c, &partial, sizeof(double) * (size_t)chunk * c->n_tiles, st)) {
             cudaFreeAsync(rows, st);
             if (ext) cudaFreeAsync(ext, st);
             return TL_ENOMEM;
@@ -233,15 +327,7 @@ int run_batch(tl_ctx *c, const float *params, int64_t B, float *logL, float *ima
     for (int64_t r0 = 0; r0 < B && rc == TL_OK; r0 += chunk) {
         const int64_t nb = (B - r0 < chunk) ? (B - r0) : chunk;
         tl::PrologueArgs pa;
-        pa.params = params + r0 * c->P; pa.rows = rows; pa.sigma_min = c->sigma_min;
-        pa.B = nb; pa.row0 = r0; pa.rows_per_lens = rows_per_lens;
-        pa.P = c->P; pa.n_lens_light = c->cfg.n_lens_light; pa.n_source = c->cfg.n_source;
-        pa.S = c->cfg.supersample;
-        pa.mass_model = c->cfg.mass_model; pa.lens_np = c->lens_np;
-        pa.inv_u = 2.0 * c->cfg.supersample / c->cfg.pix_scale;
-        pa.fov_half = 0.5 * c->cfg.pix_scale * (c->He > c->We ? c->He : c->We);
-        pa.refine_tau = c->refine_tau;
-        pa.unit_amp = 0; pa.mge = 0;
+        fill_prologue_args(c, pa, params, rows, nb, r0, rows_per_lens, 0);
         const int64_t nthr = nb * (1 + c->n_comp);
         tl::prologue_kernel<<<(unsigned)((nthr + 127) / 128), 128, 0, st>>>(pa);
 
@@ -293,8 +379,19 @@ const char *tl_strerror(int code)
 int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_ny, int32_t psf_nx,
               const float *data, const float *noise, void *cuda_stream)
 {
+    return tl_create_ex(out, cfg, psf, psf_ny, psf_nx, data, noise, nullptr, cuda_stream);
+}
+
+int tl_create_ex(tl_ctx **out, const tl_config *cfg, const float *psf_in, int32_t psf_ny, int32_t psf_nx,
+                 const float *data_in, const float *noise_in, const tl_options *opt, void *cuda_stream)
+{
     if (out) *out = nullptr;
-    if (!out || !cfg || !psf || !data || !noise) return TL_EINVAL;
+    if (!out || !cfg || !psf_in || !data_in || !noise_in) return TL_EINVAL;
+    if (opt) {
+        if (opt->small_batch_rows < -1 || opt->mge_chunk_rows < 0 || opt->scratch_keep_bytes < 0) return TL_EINVAL;
+        if (opt->block_threads && (opt->block_threads < 32 || opt->block_threads > 512 || opt->block_threads % 32)) return TL_EINVAL;
+        if (opt->refine_tau < 0.0 || !std::isfinite(opt->refine_tau)) return TL_EINVAL;
+    }
     if (cfg->ny < 1 || cfg->nx < 1 || !(cfg->pix_scale > 0.0) || !std::isfinite(cfg->pix_scale)) return TL_EINVAL;
     if (cfg->supersample < 1 || cfg->supersample > 16) return TL_EINVAL;
     if (cfg->n_lens_light < 0 || cfg->n_lens_light > 1 || cfg->n_source < 1 || cfg->n_source > 2) return TL_EINVAL;
@@ -306,6 +403,22 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
     if ((int64_t)2 * cfg->supersample * ((int64_t)(cfg->ny > cfg->nx ? cfg->ny : cfg->nx) + psf_ny) >= (1 << 24)) return TL_ESIZE;
 
     const size_t npix = (size_t)cfg->ny * cfg->nx, L = (size_t)cfg->n_lens;
+    // psf / data / noise may be host or device pointers (SURVEY.md 8(b) "Ownership"); the
+    // preparation below runs on the host, so device arrays are staged into host copies first
+    std::vector<float> stage_psf, stage_data, stage_noise;
+    auto host_view = [](const float *p, size_t n, std::vector<float> &stage, int *err) -> const float * {
+        cudaPointerAttributes at;
+        if (cudaPointerGetAttributes(&at, p) != cudaSuccess) { cudaGetLastError(); return p; }   // no driver: plain host memory
+        if (at.type != cudaMemoryTypeDevice) return p;             // unregistered / pinned host, or managed
+        stage.resize(n);
+        if (cudaMemcpy(stage.data(), p, n * sizeof(float), cudaMemcpyDeviceToHost) != cudaSuccess) *err = TL_ECUDA;
+        return stage.data();
+    };
+    int herr = TL_OK;
+    const float *psf = host_view(psf_in, L * (size_t)psf_ny * psf_nx, stage_psf, &herr);
+    const float *data = host_view(data_in, npix * L, stage_data, &herr);
+    const float *noise = host_view(noise_in, npix * L, stage_noise, &herr);
+    if (herr != TL_OK) return herr;
     for (size_t i = 0; i < npix * L; ++i)
         if (!(noise[i] > 0.f) || !std::isfinite(noise[i])) return TL_EINVAL;
 
@@ -315,17 +428,26 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
     tl_ctx *c = new (std::nothrow) tl_ctx;
     if (!c) return TL_ENOMEM;
     c->cfg = *cfg;
+    memset(&c->opt, 0, sizeof(c->opt));
+    c->opt.small_batch_rows = -1;
+    if (opt) c->opt = *opt;
     if (!cuda_ok(cudaGetDevice(&c->device))) { delete c; return TL_ECUDA; }
     cudaDeviceProp prop;
     if (!cuda_ok(cudaGetDeviceProperties(&prop, c->device))) { delete c; return TL_ECUDA; }
     c->n_sm = prop.multiProcessorCount;
-    {   // per-call scratch comes from the stream-ordered allocator: keep freed blocks cached in
-        // the pool across synchronisations instead of returning them to the driver every call
-        cudaMemPool_t pool;
-        if (cuda_ok(cudaDeviceGetDefaultMemPool(&pool, c->device))) {
-            unsigned long long keep = ~0ull;
-            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
-        }
+    {   // per-call scratch comes from a stream-ordered pool owned by the context (the device's
+        // default pool, which other libraries share, is left alone): freed blocks stay cached in it
+        // across synchronisations up to `scratch_keep_bytes` and are returned by tl_destroy
+        cudaMemPoolProps props;
+        memset(&props, 0, sizeof(props));
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = c->device;
+        if (cuda_ok(cudaMemPoolCreate(&c->pool, &props))) {
+            unsigned long long keep = c->opt.scratch_keep_bytes > 0 ? (unsigned long long)c->opt.scratch_keep_bytes : (2ull << 30);
+            cudaMemPoolSetAttribute(c->pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        } else c->pool = nullptr;                     // falls back to the default pool (untouched)
         cudaGetLastError();
     }
     c->n_comp = cfg->n_lens_light + cfg->n_source;
@@ -337,7 +459,7 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
 
     // host-side preparation in FP64: flipped + padded PSF, inverse variance, Eq. 5 constant
     std::vector<float> psf_f((size_t)L * c->K * c->Kp, 0.f), wgt(npix * L), smin(L);
-    std::vector<double> lconst(L);
+    std::vector<double> lconst(L), wgt64(npix * L);
     for (size_t l = 0; l < L; ++l) {
         // true convolution (Eq. 3, G11) == correlation with the flipped kernel
         for (int a = 0; a < c->K; ++a)
@@ -346,7 +468,8 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
         double s = 0.0, comp = 0.0, mn = INFINITY;
         for (size_t i = 0; i < npix; ++i) {
             const double sg = noise[l * npix + i];
-            wgt[l * npix + i] = (float)(1.0 / (sg * sg));
+            wgt64[l * npix + i] = 1.0 / (sg * sg);
+            wgt[l * npix + i] = (float)wgt64[l * npix + i];
             const double t = std::log(2.0 * M_PI * sg * sg) - comp, u = s + t;   // Kahan
             comp = (u - s) - t; s = u;
             if (sg < mn) mn = sg;
@@ -355,15 +478,13 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
     }
     c->lconst0 = lconst[0]; c->sigma_min0 = smin[0];
     c->refine_tau *= cfg->supersample;
-    if (const char *e = std::getenv("TL_REFINE_TAU")) {   // tuning knob
-        const double v = std::atof(e);
-        if (v > 0.0 && std::isfinite(v)) c->refine_tau = v;
-    }
+    if (c->opt.refine_tau > 0.0 && std::isfinite(c->opt.refine_tau)) c->refine_tau = c->opt.refine_tau;
 
     cudaStream_t st = (cudaStream_t)cuda_stream;
     bool ok = cuda_ok(cudaMalloc(&c->psf, psf_f.size() * sizeof(float))) &&
               cuda_ok(cudaMalloc(&c->data, npix * L * sizeof(float))) &&
               cuda_ok(cudaMalloc(&c->wgt, npix * L * sizeof(float))) &&
+              cuda_ok(cudaMalloc(&c->wgt64, npix * L * sizeof(double))) &&
               cuda_ok(cudaMalloc(&c->noise, npix * L * sizeof(float))) &&
               cuda_ok(cudaMalloc(&c->sigma_min, L * sizeof(float))) &&
               cuda_ok(cudaMalloc(&c->lconst, L * sizeof(double)));
@@ -371,6 +492,7 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
     ok = cuda_ok(cudaMemcpyAsync(c->psf, psf_f.data(), psf_f.size() * sizeof(float), cudaMemcpyHostToDevice, st)) &&
          cuda_ok(cudaMemcpyAsync(c->data, data, npix * L * sizeof(float), cudaMemcpyHostToDevice, st)) &&
          cuda_ok(cudaMemcpyAsync(c->wgt, wgt.data(), npix * L * sizeof(float), cudaMemcpyHostToDevice, st)) &&
+         cuda_ok(cudaMemcpyAsync(c->wgt64, wgt64.data(), npix * L * sizeof(double), cudaMemcpyHostToDevice, st)) &&
          cuda_ok(cudaMemcpyAsync(c->noise, noise, npix * L * sizeof(float), cudaMemcpyHostToDevice, st)) &&
          cuda_ok(cudaMemcpyAsync(c->sigma_min, smin.data(), L * sizeof(float), cudaMemcpyHostToDevice, st)) &&
          cuda_ok(cudaMemcpyAsync(c->lconst, lconst.data(), L * sizeof(double), cudaMemcpyHostToDevice, st)) &&
@@ -381,7 +503,7 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
     best_warp_tile(c->He, c->We, &c->CW, &c->CH);
     size_t fs = fused_smem_bytes(c);
     const size_t rowtab_bytes = sizeof(tl::RowV) * (size_t)c->He * cfg->supersample;
-    if (fs <= SMEM_LIMIT && !std::getenv("TL_FORCE_SPLIT")) {
+    if (fs <= SMEM_LIMIT && !c->opt.force_split) {
         // the row-value table is worth its shared memory unless it costs a resident CTA
         const size_t fs2 = ((fs + 15) & ~(size_t)15) + rowtab_bytes;
         const int per_sm_1 = (int)(SMEM_LIMIT / (fs + 1024)), per_sm_2 = (int)(SMEM_LIMIT / (fs2 + 1024));
@@ -391,7 +513,7 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
         // (measured +3 % on configs[1] and lower small-batch latency), else two CTAs of 8 warps
         const int n_tiles_img = ((c->We + c->CW - 1) / c->CW) * ((c->He + c->CH - 1) / c->CH);
         c->threads = (fs > SMEM_LIMIT / 2 || n_tiles_img >= 300) ? 512 : 256;
-        if (const char *e = std::getenv("TL_THREADS")) { const int v = std::atoi(e); if (v >= 32 && v <= 512 && v % 32 == 0) c->threads = v; }
+        if (c->opt.block_threads) c->threads = c->opt.block_threads;
         c->fused = cfg->mass_model == TL_MASS_EPL ? tl_fused_epl_for(cfg->supersample, cfg->n_lens_light, cfg->n_source)
                                                   : tl_fused_for(cfg->supersample, cfg->n_lens_light, cfg->n_source);
         if (!cuda_ok(cudaFuncSetAttribute(c->fused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT))) { tl_destroy(c); return TL_ECUDA; }
@@ -403,7 +525,7 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
         const bool kblk = c->K == 5 || c->K == 15 || c->K == 21 || c->K == 31 || c->K == 41;
         // ... and a row long enough for three more launches to pay (measured: configs 1-3 gain, Tiny loses)
         const int64_t samples_row = (int64_t)c->He * c->We * cfg->supersample * cfg->supersample;
-        if (kblk && samples_row >= 16384 && !std::getenv("TL_NO_SMALL_BATCH")) {
+        if (kblk && (samples_row >= 16384 || c->opt.small_batch_rows > 0) && c->opt.small_batch_rows != 0) {
             c->sb_trace = cfg->mass_model == TL_MASS_EPL ? tl_trace_epl_for(cfg->supersample, cfg->n_lens_light, cfg->n_source)
                                                          : tl_trace_for(cfg->supersample, cfg->n_lens_light, cfg->n_source);
             bool oks = cuda_ok(cudaFuncSetAttribute(tl::conv_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SMEM_LIMIT - 1024)));   // 1 KB: its static shared memory
@@ -412,7 +534,7 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
                 oks = oks && cuda_ok(cudaFuncSetAttribute(c->sb_trace, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rowtab_bytes));
             }
             c->sb_max_rows = oks ? c->n_sm / 2 : 0;
-            if (const char *e = std::getenv("TL_SMALL_BATCH_ROWS")) c->sb_max_rows = oks ? std::atoi(e) : 0;
+            if (c->opt.small_batch_rows > 0) c->sb_max_rows = oks ? c->opt.small_batch_rows : 0;
             cudaGetLastError();
         }
     } else {
@@ -476,6 +598,30 @@ int tl_create(tl_ctx **out, const tl_config *cfg, const float *psf, int32_t psf_
             cudaGetLastError();
         }
     }
+    {   // double-precision path (tl_dp.cuh): bands of output rows whose FP64 tile (+ K - 1 halo rows) and
+        // taps fit in ~100 KB (two CTAs per SM), else in the full 227 KB
+        c->dp_Wp = (c->We + 1) & ~1;
+        const int Kd = (c->K + 1) & ~1;
+        const size_t fixed = (size_t)c->K * Kd + Kd + 16;
+        long br = (long)((100 * 1024 / sizeof(double) - fixed) / c->dp_Wp) - (c->K - 1);
+        if (br < 8) br = (long)(((SMEM_LIMIT - 1024) / sizeof(double) - fixed) / c->dp_Wp) - (c->K - 1);
+        if (br >= 1) {
+            if (br > cfg->ny) br = cfg->ny;
+            c->dp_n_bands = (int)((cfg->ny + br - 1) / br);
+            c->dp_band_rows = (cfg->ny + c->dp_n_bands - 1) / c->dp_n_bands;
+            c->dp_conv_smem = sizeof(double) * (fixed + (size_t)(c->dp_band_rows + c->K - 1) * c->dp_Wp);
+            c->dp_trace = tl_trace_dp_for(cfg->n_lens_light, cfg->n_source);
+            int occ = 0;
+            bool okd = cuda_ok(cudaFuncSetAttribute(tl::conv_dp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SMEM_LIMIT - 1024))) &&
+                       cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, c->dp_trace, 256, 0)) && occ >= 1;
+            if (!okd) { tl_destroy(c); return TL_ECUDA; }
+            c->dp_trace_grid = occ * c->n_sm;
+            int64_t cr = (int64_t)(((size_t)1 << 30) / (sizeof(double) * (size_t)c->He * c->dp_Wp));
+            if (cr < 1) cr = 1;
+            if (cr > 65535) cr = 65535;
+            c->dp_chunk_rows = cr;
+        }
+    }
     *out = c;
     return TL_OK;
 }
@@ -514,31 +660,22 @@ int tl_loglike_linear_batch(tl_ctx *c, const float *params, int64_t B, float *lo
     if (!params || !logL || (B % c->cfg.n_lens)) return TL_EINVAL;
     if (!c->trace_lin) return TL_ESIZE;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    int dev = -1;
-    if (!cuda_ok(cudaGetDevice(&dev))) return TL_ECUDA;
-    if (dev != c->device && !cuda_ok(cudaSetDevice(c->device))) return TL_ECUDA;
+    DeviceGuard guard(c->device);
+    if (!guard.ok) return TL_ECUDA;
     const int NC = c->n_comp;
     const size_t npix = (size_t)c->cfg.ny * c->cfg.nx;
-    if (c->fused_lin && !std::getenv("TL_LINEAR_STAGED")) {
+    if (c->fused_lin && !c->opt.linear_staged) {
         const int64_t chunkf = CONST_CHUNK < B ? CONST_CHUNK : B;
         tl::RowC *rowsf = nullptr;
         float *mscr = nullptr;
-        if (!cuda_ok(cudaMallocAsync(&rowsf, sizeof(tl::RowC) * (size_t)chunkf, st))) return TL_ENOMEM;
-        if (!cuda_ok(cudaMallocAsync(&mscr, sizeof(float) * (size_t)c->lin_fused_grid * NC * npix, st))) { cudaFreeAsync(rowsf, st); return TL_ENOMEM; }
+        if (!pool_alloc(c, &rowsf, sizeof(tl::RowC) * (size_t)chunkf, st)) return TL_ENOMEM;
+        if (!pool_alloc(c, &mscr, sizeof(float) * (size_t)c->lin_fused_grid * NC * npix, st)) { cudaFreeAsync(rowsf, st); return TL_ENOMEM; }
         const int64_t rpl = B / c->cfg.n_lens;
         int rcf = TL_OK;
         for (int64_t r0 = 0; r0 < B && rcf == TL_OK; r0 += chunkf) {
             const int64_t nb = (B - r0 < chunkf) ? (B - r0) : chunkf;
             tl::PrologueArgs pa;
-            pa.params = params + r0 * c->P; pa.rows = rowsf; pa.sigma_min = c->sigma_min;
-            pa.B = nb; pa.row0 = r0; pa.rows_per_lens = rpl;
-            pa.P = c->P; pa.n_lens_light = c->cfg.n_lens_light; pa.n_source = c->cfg.n_source;
-            pa.S = c->cfg.supersample;
-            pa.mass_model = c->cfg.mass_model; pa.lens_np = c->lens_np;
-            pa.inv_u = 2.0 * c->cfg.supersample / c->cfg.pix_scale;
-            pa.fov_half = 0.5 * c->cfg.pix_scale * (c->He > c->We ? c->He : c->We);
-            pa.refine_tau = c->refine_tau;
-            pa.unit_amp = 1; pa.mge = 0;
+            fill_prologue_args(c, pa, params, rowsf, nb, r0, rpl, 1);
             const int64_t nthr = nb * (1 + c->n_comp);
             tl::prologue_kernel<<<(unsigned)((nthr + 127) / 128), 128, 0, st>>>(pa);
             tl::KArgs a = base_args(c);
@@ -561,9 +698,9 @@ int tl_loglike_linear_batch(tl_ctx *c, const float *params, int64_t B, float *lo
     if (chunk > B) chunk = B;
     tl::RowC *rows = nullptr;
     float *ext = nullptr, *mimg = nullptr;
-    if (!cuda_ok(cudaMallocAsync(&rows, sizeof(tl::RowC) * (size_t)chunk, st))) return TL_ENOMEM;
-    if (!cuda_ok(cudaMallocAsync(&ext, ext_row * (size_t)chunk, st)) ||
-        !cuda_ok(cudaMallocAsync(&mimg, m_row * (size_t)chunk, st))) {
+    if (!pool_alloc(c, &rows, sizeof(tl::RowC) * (size_t)chunk, st)) return TL_ENOMEM;
+    if (!pool_alloc(c, &ext, ext_row * (size_t)chunk, st) ||
+        !pool_alloc(c, &mimg, m_row * (size_t)chunk, st)) {
         cudaFreeAsync(rows, st);
         if (ext) cudaFreeAsync(ext, st);
         return TL_ENOMEM;
@@ -574,15 +711,7 @@ int tl_loglike_linear_batch(tl_ctx *c, const float *params, int64_t B, float *lo
     for (int64_t r0 = 0; r0 < B && rc == TL_OK; r0 += chunk) {
         const int64_t nb = (B - r0 < chunk) ? (B - r0) : chunk;
         tl::PrologueArgs pa;
-        pa.params = params + r0 * c->P; pa.rows = rows; pa.sigma_min = c->sigma_min;
-        pa.B = nb; pa.row0 = r0; pa.rows_per_lens = rows_per_lens;
-        pa.P = c->P; pa.n_lens_light = c->cfg.n_lens_light; pa.n_source = c->cfg.n_source;
-        pa.S = c->cfg.supersample;
-        pa.mass_model = c->cfg.mass_model; pa.lens_np = c->lens_np;
-        pa.inv_u = 2.0 * c->cfg.supersample / c->cfg.pix_scale;
-        pa.fov_half = 0.5 * c->cfg.pix_scale * (c->He > c->We ? c->He : c->We);
-        pa.refine_tau = c->refine_tau;
-        pa.unit_amp = 1; pa.mge = 0;
+        fill_prologue_args(c, pa, params, rows, nb, r0, rows_per_lens, 1);
         const int64_t nthr = nb * (1 + c->n_comp);
         tl::prologue_kernel<<<(unsigned)((nthr + 127) / 128), 128, 0, st>>>(pa);
         tl::KArgs a = base_args(c);
@@ -613,9 +742,8 @@ int tl_set_mge(tl_ctx *c, const float *sigmas, int32_t n_gauss)
         ck[k] = (float)(1.4426950408889634074 / (2.0 * (double)sigmas[k] * (double)sigmas[k]));
         if (!std::isfinite(ck[k])) return TL_EINVAL;
     }
-    int dev = -1;
-    if (!cuda_ok(cudaGetDevice(&dev))) return TL_ECUDA;
-    if (dev != c->device && !cuda_ok(cudaSetDevice(c->device))) return TL_ECUDA;
+    DeviceGuard guard(c->device);
+    if (!guard.ok) return TL_ECUDA;
     if (!c->mge_c && !cuda_ok(cudaMalloc(&c->mge_c, sizeof(float) * tl::MGE_MAX_GAUSS))) return TL_ENOMEM;
     if (!cuda_ok(cudaMemcpy(c->mge_c, ck, sizeof(float) * n_gauss, cudaMemcpyHostToDevice))) return TL_ECUDA;
     c->n_gauss = n_gauss;
@@ -631,10 +759,7 @@ int64_t mge_chunk_rows(const tl_ctx *c)
     int64_t chunk = (int64_t)(MGE_SCRATCH_BYTES / (ext_row + m_row));
     if (chunk < 1) chunk = 1;
     if (chunk > 65535) chunk = 65535;
-    if (const char *e = std::getenv("TL_MGE_CHUNK_ROWS")) {      // tests: force the multi-chunk path
-        const long v = std::atol(e);
-        if (v >= 1 && v < chunk) chunk = v;
-    }
+    if (c->opt.mge_chunk_rows >= 1 && c->opt.mge_chunk_rows < chunk) chunk = c->opt.mge_chunk_rows;   // tests: the multi-chunk path
     return chunk;
 }
 }  // namespace
@@ -651,9 +776,8 @@ int tl_loglike_mge_batch(tl_ctx *c, const float *params, int64_t B, float *logL,
     if (!params || !logL || (B % c->cfg.n_lens)) return TL_EINVAL;
     if (!c->trace_lin) return TL_ESIZE;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    int dev = -1;
-    if (!cuda_ok(cudaGetDevice(&dev))) return TL_ECUDA;
-    if (dev != c->device && !cuda_ok(cudaSetDevice(c->device))) return TL_ECUDA;
+    DeviceGuard guard(c->device);
+    if (!guard.ok) return TL_ECUDA;
     const int NG = c->n_gauss, NC = NG + c->cfg.n_source;
     const size_t npix = (size_t)c->cfg.ny * c->cfg.nx;
     const size_t ext_row = sizeof(float) * (size_t)NC * c->He * c->pitch, m_row = sizeof(float) * NC * npix;
@@ -666,10 +790,10 @@ int tl_loglike_mge_batch(tl_ctx *c, const float *params, int64_t B, float *logL,
     // the budget is a target, not a promise: when the device cannot give that much, halve the chunk
     for (;;) {
         rows = nullptr; ext = nullptr; mimg = nullptr; gram = nullptr;
-        if (cuda_ok(cudaMallocAsync(&rows, sizeof(tl::RowC) * (size_t)chunk, st)) &&
-            cuda_ok(cudaMallocAsync(&ext, ext_row * (size_t)chunk, st)) &&
-            cuda_ok(cudaMallocAsync(&mimg, m_row * (size_t)chunk, st)) &&
-            cuda_ok(cudaMallocAsync(&gram, g_row * (size_t)chunk, st))) break;
+        if (pool_alloc(c, &rows, sizeof(tl::RowC) * (size_t)chunk, st) &&
+            pool_alloc(c, &ext, ext_row * (size_t)chunk, st) &&
+            pool_alloc(c, &mimg, m_row * (size_t)chunk, st) &&
+            pool_alloc(c, &gram, g_row * (size_t)chunk, st)) break;
         cudaGetLastError();                                    // an allocation failure is not sticky
         if (rows) cudaFreeAsync(rows, st);
         if (ext) cudaFreeAsync(ext, st);
@@ -720,10 +844,12 @@ int tl_loglike_batch_host(tl_ctx *ctx, const float *params, int64_t B, float *lo
 {
     if (!ctx || B < 0 || (B > 0 && (!params || !logL))) return TL_EINVAL;
     if (B == 0) return TL_OK;
+    DeviceGuard guard(ctx->device);                  // before any allocation: the buffers belong to the context's device
+    if (!guard.ok) return TL_ECUDA;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     float *dp = nullptr, *dl = nullptr;
-    if (!cuda_ok(cudaMallocAsync(&dp, sizeof(float) * (size_t)B * ctx->P, st))) return TL_ENOMEM;
-    if (!cuda_ok(cudaMallocAsync(&dl, sizeof(float) * (size_t)B, st))) { cudaFreeAsync(dp, st); return TL_ENOMEM; }
+    if (!pool_alloc(ctx, &dp, sizeof(float) * (size_t)B * ctx->P, st)) return TL_ENOMEM;
+    if (!pool_alloc(ctx, &dl, sizeof(float) * (size_t)B, st)) { cudaFreeAsync(dp, st); return TL_ENOMEM; }
     int rc = TL_OK;
     if (!cuda_ok(cudaMemcpyAsync(dp, params, sizeof(float) * (size_t)B * ctx->P, cudaMemcpyHostToDevice, st))) rc = TL_ECUDA;
     if (rc == TL_OK) rc = run_batch(ctx, dp, B, dl, nullptr, st);
@@ -736,7 +862,8 @@ int tl_loglike_batch_host(tl_ctx *ctx, const float *params, int64_t B, float *lo
 
 int tl_set_precision(tl_ctx *c, int precision)
 {
-    if (!c || (precision != TL_PRECISION_FP32 && precision != TL_PRECISION_FP64)) return TL_EINVAL;
+    if (!c || precision < TL_PRECISION_FP32 || precision > TL_PRECISION_AUTO) return TL_EINVAL;
+    if ((precision == TL_PRECISION_FP64 || precision == TL_PRECISION_AUTO) && !c->dp_trace) return TL_ESIZE;
     c->precision = precision;
     return TL_OK;
 }
@@ -765,7 +892,8 @@ void tl_destroy(tl_ctx *c)
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
     cudaFree(c->mge_c);
-    cudaFree(c->psf); cudaFree(c->data); cudaFree(c->wgt); cudaFree(c->noise); cudaFree(c->sigma_min); cudaFree(c->lconst);
+    cudaFree(c->psf); cudaFree(c->data); cudaFree(c->wgt); cudaFree(c->wgt64); cudaFree(c->noise); cudaFree(c->sigma_min); cudaFree(c->lconst);
+    if (c->pool) cudaMemPoolDestroy(c->pool);
     delete c;
 }
 

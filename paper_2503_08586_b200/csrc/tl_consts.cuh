@@ -161,6 +161,17 @@ __device__ inline void split2(double v, float *h, float *l)
     *l = (float)(v - (double)hh);
 }
 
+// v > 0 as hi + lo with lo > 0 strictly: used for 1/(2n), which multiplies lg2(t) = -inf at the
+// centre of a profile (t = 0): -inf * lo must be -inf, not NaN (lo = 0) or +inf (lo < 0), so that
+// u = ex2(-inf) = 0 and the sample is I_e e^{b_n} (Eq. 8 at R = 0).
+__device__ inline void split2_poslo(double v, float *h, float *l)
+{
+    float hh = (float)v;
+    if (!(v - (double)hh > 0.0)) hh = __int_as_float(__float_as_int(hh) - 1);     // next float towards zero (v > 0)
+    *h = hh;
+    *l = (float)(v - (double)hh);
+}
+
 // Inverse of PAPER.md:152 Eq. 11 (G3): e = hypot(e1,e2), q = (1-e)/(1+e), phi = atan2(e2,e1)/2.
 __device__ inline bool shape_from_e(double e1, double e2, double *q, double *c, double *s)
 {
@@ -324,7 +335,7 @@ __global__ void __launch_bounds__(128) prologue_kernel(PrologueArgs a)
     split2(A * cd * cd + Bq * sd * sd, &C.ah, &C.al);
     split2(2.0 * (A - Bq) * cd * sd, &C.b2h, &C.b2l);
     split2(A * sd * sd + Bq * cd * cd, &C.cch, &C.ccl);
-    split2(0.5 / n, &C.ph, &C.pl);
+    split2_poslo(0.5 / n, &C.ph, &C.pl);
     split2(bn * 1.4426950408889634074, &C.kh, &C.kl);
     const double amp = Ie / (double)(a.S * a.S);
     C.amp = (float)amp;

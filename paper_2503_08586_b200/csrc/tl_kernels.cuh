@@ -14,6 +14,7 @@
 #pragma once
 #include <type_traits>
 #include "tl_sample.cuh"
+#include "tl_nnls.cuh"
 
 namespace tl {
 
@@ -493,11 +494,25 @@ struct ConvBlock {
     }
 };
 
-// chi^2 terms of up to 4 outputs of row i starting at column x0 (and the optional image store)
+// chi^2 terms of up to 4 outputs of row i starting at column x0 (and the optional image store).
+// x0 is a multiple of 4, so when nx is too the four data / weight values are one aligned 16-byte
+// load each (north_star (3): "vectorised coalesced loads"); the sum order is the same either way.
 __device__ __forceinline__ float chi2_strip(const KArgs &a, const float acc[4], int i, int x0,
                                             const float *data, const float *wgt, float *image_out)
 {
     float c = 0.f;
+    if ((a.nx & 3) == 0) {                           // uniform over the grid
+        if (x0 >= a.nx) return 0.f;
+        const int o = i * a.nx + x0;
+        if (image_out) *reinterpret_cast<float4 *>(image_out + o) = make_float4(acc[0], acc[1], acc[2], acc[3]);
+        if (data) {
+            const float4 dv = __ldg(reinterpret_cast<const float4 *>(data + o));
+            const float4 wv = __ldg(reinterpret_cast<const float4 *>(wgt + o));
+            const float d0 = dv.x - acc[0], d1 = dv.y - acc[1], d2 = dv.z - acc[2], d3 = dv.w - acc[3];
+            c = fmaf(d0 * d0, wv.x, c); c = fmaf(d1 * d1, wv.y, c); c = fmaf(d2 * d2, wv.z, c); c = fmaf(d3 * d3, wv.w, c);
+        }
+        return c;
+    }
 #pragma unroll
     for (int r = 0; r < 4; ++r) {
         const int x = x0 + r;
@@ -832,41 +847,6 @@ __global__ void __launch_bounds__(256, 2) conv_lin_kernel(const KArgs a, int chu
 
 #endif  // TL_MAIN_TU
 
-// minimise s'G s - 2 b's over s >= 0 for n <= 3: every support, normal equations by Cramer's rule
-__device__ inline void nnls_small(int n, const double G[3][3], const double b[3], double s[3])
-{
-    double best = 0.0;
-    s[0] = s[1] = s[2] = 0.0;
-    for (int m = 1; m < (1 << n); ++m) {
-        double x[3] = {0.0, 0.0, 0.0};
-        const bool u0 = m & 1, u1 = m & 2, u2 = m & 4;
-        const int cnt = (int)u0 + (int)u1 + (int)u2;
-        if (cnt == 1) {
-            const int i = u0 ? 0 : (u1 ? 1 : 2);
-            if (!(G[i][i] > 0.0)) continue;
-            x[i] = b[i] / G[i][i];
-        } else if (cnt == 2) {
-            const int i = u0 ? 0 : 1, j = u2 ? 2 : 1;
-            const double det = G[i][i] * G[j][j] - G[i][j] * G[i][j];
-            if (!(fabs(det) > 1e-300)) continue;
-            x[i] = (b[i] * G[j][j] - b[j] * G[i][j]) / det;
-            x[j] = (b[j] * G[i][i] - b[i] * G[i][j]) / det;
-        } else {
-            const double c00 = G[1][1] * G[2][2] - G[1][2] * G[1][2], c01 = G[0][2] * G[1][2] - G[0][1] * G[2][2],
-                         c02 = G[0][1] * G[1][2] - G[0][2] * G[1][1], c11 = G[0][0] * G[2][2] - G[0][2] * G[0][2],
-                         c12 = G[0][1] * G[0][2] - G[0][0] * G[1][2], c22 = G[0][0] * G[1][1] - G[0][1] * G[0][1];
-            const double det = G[0][0] * c00 + G[0][1] * c01 + G[0][2] * c02;
-            if (!(fabs(det) > 1e-300)) continue;
-            x[0] = (c00 * b[0] + c01 * b[1] + c02 * b[2]) / det;
-            x[1] = (c01 * b[0] + c11 * b[1] + c12 * b[2]) / det;
-            x[2] = (c02 * b[0] + c12 * b[1] + c22 * b[2]) / det;
-        }
-        if (!(x[0] >= 0.0 && x[1] >= 0.0 && x[2] >= 0.0)) continue;
-        const double f = -(b[0] * x[0] + b[1] * x[1] + b[2] * x[2]);       // penalty change at a stationary point
-        if (f < best) { best = f; s[0] = x[0]; s[1] = x[1]; s[2] = x[2]; }
-    }
-}
-
 // G = M'WM, b = M'Wd (fixed-shape FP64 reductions), NNLS, chi^2 of the residual d - M s -> logL.
 // All threads of the CTA; M = the row's blurred unit-amplitude component images [C][npix].
 __device__ __forceinline__ void solve_row(const KArgs &a, const float *M, int64_t row, int64_t lens,
@@ -875,6 +855,7 @@ __device__ __forceinline__ void solve_row(const KArgs &a, const float *M, int64_
     const int NC = a.n_comp, npix = a.ny * a.nx;
     const float *d = a.data + lens * (size_t)npix, *w = a.wgt + lens * (size_t)npix;
     double g[6] = {0, 0, 0, 0, 0, 0}, bb[3] = {0, 0, 0};             // G00 G01 G02 G11 G12 G22
+    double dd = 0.0;                                               // d'Wd: the scale of "zero" for the solver
     for (int i = threadIdx.x; i < npix; i += blockDim.x) {
         const double wi = w[i], di = d[i];
         double m[3] = {0.0, 0.0, 0.0};
@@ -882,15 +863,18 @@ __device__ __forceinline__ void solve_row(const KArgs &a, const float *M, int64_
         g[0] += wi * m[0] * m[0]; g[1] += wi * m[0] * m[1]; g[2] += wi * m[0] * m[2];
         g[3] += wi * m[1] * m[1]; g[4] += wi * m[1] * m[2]; g[5] += wi * m[2] * m[2];
         bb[0] += wi * m[0] * di; bb[1] += wi * m[1] * di; bb[2] += wi * m[2] * di;
+        dd += wi * di * di;
     }
     double G[3][3], b[3];
     const double g0 = block_sum(g[0], red), g1 = block_sum(g[1], red), g2 = block_sum(g[2], red),
                  g3 = block_sum(g[3], red), g4 = block_sum(g[4], red), g5 = block_sum(g[5], red);
     b[0] = block_sum(bb[0], red); b[1] = block_sum(bb[1], red); b[2] = block_sum(bb[2], red);
+    const double dwd = block_sum(dd, red);
     if (threadIdx.x == 0) {
         G[0][0] = g0; G[0][1] = G[1][0] = g1; G[0][2] = G[2][0] = g2; G[1][1] = g3; G[1][2] = G[2][1] = g4; G[2][2] = g5;
-        double s[3];
-        nnls_small(NC, G, b, s);
+        // the paper's solver (Bro & De Jong's Gram-matrix active set), as in the MGE mode
+        double s[3] = {0.0, 0.0, 0.0}, Lc[9], z[3];
+        nnls_gram<3>(NC, &G[0][0], 3, b, dwd, s, Lc, z);
         s_sh[0] = s[0]; s_sh[1] = s[1]; s_sh[2] = s[2];
     }
     __syncthreads();

@@ -100,90 +100,6 @@ inline mge_gauss_fn mge_gauss_for(int ng)
     }
 }
 
-// minimise s'G s - 2 b's over s >= 0 (n <= MGE_MAX_COL) -- one thread.  Active-set iteration on
-// the Gram matrix (Lawson & Hanson; in this cross-product form Bro & De Jong's "fast NNLS"):
-// the passive set P grows by the column with the largest positive gradient w = b - G s, the
-// unconstrained problem on P is solved by Cholesky, and a step towards it that would leave the
-// feasible region is cut at the boundary, the columns that reach 0 leaving P.
-// G is [n][ldg]; L (scratch) [MGE_MAX_COL][MGE_MAX_COL]; dwd = d'Wd sets the scale of "zero".
-__device__ inline void nnls_gram(int n, const double *G, int ldg, const double *b, double dwd, double *s,
-                                 double *L, double *z)
-{
-    int idx[MGE_MAX_COL];
-    int m = 0;
-    unsigned passive = 0u, banned = 0u;
-    for (int i = 0; i < n; ++i) s[i] = 0.0;
-    const double eps = 1e-10;
-    for (int outer = 0; outer < 3 * n + 3; ++outer) {
-        int j = -1;
-        double wbest = 0.0;
-        for (int i = 0; i < n; ++i) {
-            if ((passive | banned) & (1u << i)) continue;
-            double w = b[i];
-            for (int k = 0; k < n; ++k) w -= G[i * ldg + k] * s[k];
-            const double thr = eps * sqrt(fmax(G[i * ldg + i] * dwd, 0.0));
-            if (w > thr && w > wbest) { wbest = w; j = i; }
-        }
-        if (j < 0) break;
-        passive |= 1u << j;
-        bool first = true, added = true;
-        for (int inner = 0; inner <= n; ++inner) {
-            m = 0;
-            for (int i = 0; i < n; ++i) if (passive & (1u << i)) idx[m++] = i;
-            // Cholesky G_PP = L L'
-            bool pd = true;
-            for (int r = 0; r < m && pd; ++r) {
-                for (int c = 0; c <= r; ++c) {
-                    double v = G[idx[r] * ldg + idx[c]];
-                    for (int k = 0; k < c; ++k) v -= L[r * MGE_MAX_COL + k] * L[c * MGE_MAX_COL + k];
-                    if (c == r) {
-                        if (!(v > 1e-13 * G[idx[r] * ldg + idx[r]])) { pd = false; break; }
-                        L[r * MGE_MAX_COL + r] = rsqrt(v);             // the diagonal is kept as 1 / l_rr
-                    } else L[r * MGE_MAX_COL + c] = v * L[c * MGE_MAX_COL + c];
-                }
-            }
-            if (pd) {
-                for (int r = 0; r < m; ++r) {
-                    double v = b[idx[r]];
-                    for (int k = 0; k < r; ++k) v -= L[r * MGE_MAX_COL + k] * z[k];
-                    z[r] = v * L[r * MGE_MAX_COL + r];
-                }
-                for (int r = m - 1; r >= 0; --r) {
-                    double v = z[r];
-                    for (int k = r + 1; k < m; ++k) v -= L[k * MGE_MAX_COL + r] * z[k];
-                    z[r] = v * L[r * MGE_MAX_COL + r];
-                }
-            }
-            if (first) {
-                // the entering column must come out positive; if it is numerically dependent on P
-                // (or rounding makes it non-positive) it is set aside until P changes
-                int pj = 0;
-                for (int r = 0; r < m; ++r) if (idx[r] == j) pj = r;
-                if (!pd || !(z[pj] > 0.0)) { passive &= ~(1u << j); banned |= 1u << j; added = false; break; }
-                first = false;
-            } else if (!pd) break;                       // cannot happen for a subset of a PD set; keep s
-            double alpha = 2.0;
-            int rmin = -1;
-            for (int r = 0; r < m; ++r)
-                if (!(z[r] > 0.0)) {
-                    const double si = s[idx[r]];
-                    const double al = si / (si - z[r]);
-                    if (al < alpha) { alpha = al; rmin = r; }
-                }
-            if (rmin < 0) {                               // all positive: accept
-                for (int r = 0; r < m; ++r) s[idx[r]] = z[r];
-                break;
-            }
-            for (int r = 0; r < m; ++r) {
-                const int i = idx[r];
-                s[i] += alpha * (z[r] - s[i]);
-                if (r == rmin || !(s[i] > 0.0)) { s[i] = 0.0; passive &= ~(1u << i); }
-            }
-        }
-        if (added) banned = 0u;
-    }
-}
-
 // G = M'WM, b = M'Wd, d'Wd: one CTA of 128 threads per row.  The pixels are staged through shared
 // memory MGE_TILE at a time (w m_k and m_k, d as doubles, the next tile prefetched into registers);
 // every sum has a fixed order, so the result is bitwise reproducible.
@@ -309,7 +225,7 @@ __global__ void __launch_bounds__(32 * MGE_NNLS_WARPS) nnls_mge_kernel(const KAr
     for (int e = lane; e < MGE_GRAM_STRIDE; e += 32) Gw[wid][e] = gin[e];
     __syncwarp();
     if (lane == 0)
-        nnls_gram(n, Gw[wid], NCP, Gw[wid] + MGE_MAX_COL * NCP, Gw[wid][MGE_MAX_COL * NCP + MGE_MAX_COL], sw[wid], Lw[wid], zw[wid]);
+        nnls_gram<MGE_MAX_COL>(n, Gw[wid], NCP, Gw[wid] + MGE_MAX_COL * NCP, Gw[wid][MGE_MAX_COL * NCP + MGE_MAX_COL], sw[wid], Lw[wid], zw[wid]);
     __syncwarp();
     if (lane < n) {
         a.mge_sol[(size_t)r * MGE_MAX_COL + lane] = sw[wid][lane];

@@ -85,9 +85,9 @@ def test_linear_invalid_rows_and_clamp(api, orc):
     assert np.all(np.isinf(oll[[1, 2, 3]]))
 
 
-def test_fused_and_staged_pipelines_agree(api, orc, monkeypatch):
-    """configs[1] fits the fused linear kernel; TL_LINEAR_STAGED forces the staged pipeline that
-    larger images use.  Same arithmetic per pixel -> identical bits."""
+def test_fused_and_staged_pipelines_agree(api, orc):
+    """configs[1] fits the fused linear kernel; tl_options.linear_staged forces the staged pipeline
+    that larger images use.  Same arithmetic per pixel -> identical bits."""
     import torch
     w = W.workload(1).scaled(batch=40)
     prob = W.make_problem(w, orc.render_for_workloads)
@@ -96,8 +96,8 @@ def test_fused_and_staged_pipelines_agree(api, orc, monkeypatch):
     d = torch.from_numpy(rows).cuda()
     ll_f, am_f = ctx.loglike_linear(d)
     torch.cuda.synchronize()
-    monkeypatch.setenv("TL_LINEAR_STAGED", "1")
-    ll_s, am_s = ctx.loglike_linear(d)
+    ctx2 = api.LensContext.from_problem(prob, options={"linear_staged": 1})
+    ll_s, am_s = ctx2.loglike_linear(d)
     torch.cuda.synchronize()
-    ctx.close()
+    ctx.close(); ctx2.close()
     assert torch.equal(ll_f, ll_s) and torch.equal(am_f, am_s)

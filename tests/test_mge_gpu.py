@@ -213,9 +213,9 @@ def test_mge_call_is_cuda_graph_capturable(api, orc):
     ctx.close()
 
 
-def test_mge_chunked_call_equals_single_chunk(api, orc, monkeypatch):
-    """A call larger than the scratch budget is processed in chunks (TL_MGE_CHUNK_ROWS forces that
-    here, with a ragged last chunk, on three lenses): identical bits."""
+def test_mge_chunked_call_equals_single_chunk(api, orc):
+    """A call larger than the scratch budget is processed in chunks (tl_options.mge_chunk_rows forces
+    that here, with a ragged last chunk, on three lenses): identical bits."""
     import torch
     w = W.workload(3).scaled(batch=3 * 14, n_lens=3)
     prob = W.make_problem(w, orc.render_for_workloads)
@@ -226,10 +226,11 @@ def test_mge_chunked_call_equals_single_chunk(api, orc, monkeypatch):
     d = torch.from_numpy(rows).cuda()
     ll1, am1 = ctx.loglike_mge(d)
     torch.cuda.synchronize()
-    monkeypatch.setenv("TL_MGE_CHUNK_ROWS", "5")
-    assert api.tl_mge_chunk_rows(ctx.handle) == 5
-    ll2, am2 = ctx.loglike_mge(d)
+    ctx2 = api.LensContext.from_problem(prob, options={"mge_chunk_rows": 5})
+    ctx2.set_mge(W.mge_sigmas(w, 7))
+    assert api.tl_mge_chunk_rows(ctx2.handle) == 5
+    ll2, am2 = ctx2.loglike_mge(d)
     torch.cuda.synchronize()
-    ctx.close()
+    ctx.close(); ctx2.close()
     assert torch.equal(ll1, ll2) and torch.equal(am1.nan_to_num(-1.0), am2.nan_to_num(-1.0))
     assert ll1[5].item() == -np.inf

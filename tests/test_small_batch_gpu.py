@@ -26,11 +26,7 @@ def _zero_render(w, psf, row):
 
 def _contexts(api, prob):
     small = api.LensContext.from_problem(prob)
-    os.environ["TL_SMALL_BATCH_ROWS"] = "0"               # read by tl_create: fused path whatever B
-    try:
-        fused = api.LensContext.from_problem(prob)
-    finally:
-        del os.environ["TL_SMALL_BATCH_ROWS"]
+    fused = api.LensContext.from_problem(prob, options={"small_batch_rows": 0})     # fused path whatever B
     return small, fused
 
 
