@@ -22,10 +22,21 @@
 #define TL_VERSION_STRING "tinylens-b200 0.2 (sm_100a)"
 
 typedef void (*dp_trace_fn)(const tl::DpArgs);
-static dp_trace_fn tl_trace_dp_for(int nll, int nsrc)
+template <int S_T>
+static dp_trace_fn tl_trace_dp_s(int nll, int nsrc)
 {
-    if (nll == 0) return nsrc == 1 ? tl::trace_dp_kernel<0, 1> : tl::trace_dp_kernel<0, 2>;
-    return nsrc == 1 ? tl::trace_dp_kernel<1, 1> : tl::trace_dp_kernel<1, 2>;
+    if (nll == 0) return nsrc == 1 ? tl::trace_dp_kernel<S_T, 0, 1> : tl::trace_dp_kernel<S_T, 0, 2>;
+    return nsrc == 1 ? tl::trace_dp_kernel<S_T, 1, 1> : tl::trace_dp_kernel<S_T, 1, 2>;
+}
+static dp_trace_fn tl_trace_dp_for(int S, int nll, int nsrc)
+{
+    switch (S) {
+    case 1: return tl_trace_dp_s<1>(nll, nsrc);
+    case 2: return tl_trace_dp_s<2>(nll, nsrc);
+    case 4: return tl_trace_dp_s<4>(nll, nsrc);
+    case 8: return tl_trace_dp_s<8>(nll, nsrc);
+    default: return tl_trace_dp_s<0>(nll, nsrc);
+    }
 }
 
 struct tl_ctx {
@@ -38,7 +49,7 @@ struct tl_ctx {
     double *wgt64 = nullptr;      // 1 / sigma^2 in FP64 (the double-precision path, tl_dp.cuh)
     int precision = 0;            // TL_PRECISION_*
     // double-precision path: launch geometry
-    int dp_Wp = 0, dp_band_rows = 0, dp_n_bands = 0, dp_trace_grid = 0;
+    int dp_Wp = 0, dp_band_rows = 0, dp_n_bands = 0, dp_trace_grid = 0, dp_conv_threads = 256;
     size_t dp_conv_smem = 0;
     int64_t dp_chunk_rows = 0;
     void (*dp_trace)(const tl::DpArgs) = nullptr;
@@ -256,7 +267,7 @@ int run_dp(tl_ctx *c, const float *params, int64_t B, float *logL, float *images
         if (c->profile) cudaEventRecord(c->ev0, st);
         c->dp_trace<<<grid, 256, 0, st>>>(a);
         if (c->profile) { cudaEventRecord(c->ev1, st); c->prof_pending = 1; }
-        tl::conv_dp_kernel<<<dim3((unsigned)nb, (unsigned)c->dp_n_bands), 256, c->dp_conv_smem, st>>>(a);
+        tl::conv_dp_kernel<<<dim3((unsigned)nb, (unsigned)c->dp_n_bands), c->dp_conv_threads, c->dp_conv_smem, st>>>(a);
         if (logL) tl::finalize_dp_kernel<<<(unsigned)((nb + 127) / 128), 128, 0, st>>>(a);
         if (!cuda_ok(cudaGetLastError())) rc = TL_ECUDA;
     }
@@ -299,14 +310,26 @@ int run_batch(tl_ctx *c, const float *params, int64_t B, float *logL, float *ima
             const int max_slabs = (c->He * c->We + 255) / 256;
             if (slabs > max_slabs) slabs = max_slabs;
             if (slabs < 1) slabs = 1;
+            if (c->profile) cudaEventRecord(c->ev0, st);
             tl::precise_trace_kernel<<<dim3((unsigned)nb, (unsigned)slabs), 256, 0, st>>>(pa);
+            if (c->profile) { cudaEventRecord(c->ev1, st); c->prof_pending = 1; }
             tl::precise_conv_kernel<<<(unsigned)nb, 256, 0, st>>>(pa);
             if (!cuda_ok(cudaGetLastError())) prc = TL_ECUDA;
         }
         cudaFreeAsync(pext, st);
         return prc;
     }
-    if (c->path == 0 && B <= c->sb_max_rows) return run_small_batch(c, params, B, logL, images, st);
+    const bool autop = c->precision == TL_PRECISION_AUTO && logL != nullptr;
+    // AUTO on the split path (large images): the conv tiles do not carry the error sums, so every row
+    // is evaluated in FP64; AUTO renders are FP32 renders (the image has no 1e-8 requirement)
+    if (autop && c->path == 1) return run_dp(c, params, B, logL, images, st, nullptr, nullptr);
+    if (c->path == 0 && B <= c->sb_max_rows && !autop) return run_small_batch(c, params, B, logL, images, st);
+    int *flags = nullptr;                            // [0] = count, [1 .. B] = flagged rows
+    if (autop) {
+        if (B > 0x7ffffff0) return TL_ESIZE;
+        if (!pool_alloc(c, &flags, sizeof(int) * (size_t)(B + 1), st)) return TL_ENOMEM;
+        cudaMemsetAsync(flags, 0, sizeof(int), st);
+    }
     const int64_t chunk = c->chunk_rows < B ? c->chunk_rows : B;
     tl::RowC *rows = nullptr;
     float *ext = nullptr;
@@ -334,6 +357,12 @@ int run_batch(tl_ctx *c, const float *params, int64_t B, float *logL, float *ima
         tl::KArgs a = base_args(c);
         a.rows = rows; a.B = nb; a.rows_per_lens = rows_per_lens; a.row0 = r0;
         a.logL = logL; a.images = images;
+        if (autop) {
+            a.flag_count = flags; a.flag_list = flags + 1;
+            // the FP32 error model of DESIGN.md 6: coherent 2^-22, random 5 sigma of 2^-21 / S + 2^-22 per pixel
+            a.err_coh = 2.384185791015625e-07f;
+            a.err_rnd = (float)(5.0 * (4.76837158203125e-07 / c->cfg.supersample + 2.384185791015625e-07));
+        }
         if (c->path == 0) {
             int grid = c->grid;
             if ((int64_t)grid > nb) grid = (int)nb;
@@ -355,6 +384,10 @@ int run_batch(tl_ctx *c, const float *params, int64_t B, float *logL, float *ima
     cudaFreeAsync(rows, st);
     if (ext) cudaFreeAsync(ext, st);
     if (partial) cudaFreeAsync(partial, st);
+    if (autop) {
+        if (rc == TL_OK) rc = run_dp(c, params, B, logL, nullptr, st, flags + 1, flags);
+        cudaFreeAsync(flags, st);
+    }
     return rc;
 }
 
@@ -598,21 +631,41 @@ int tl_create_ex(tl_ctx **out, const tl_config *cfg, const float *psf_in, int32_
             cudaGetLastError();
         }
     }
-    {   // double-precision path (tl_dp.cuh): bands of output rows whose FP64 tile (+ K - 1 halo rows) and
-        // taps fit in ~100 KB (two CTAs per SM), else in the full 227 KB
+    {   // double-precision path (tl_dp.cuh).  conv_dp_kernel: one CTA per (row, band of output rows).
+        // Bands and CTA size are chosen together: the band's FP64 tile (+ K - 1 halo rows) and the taps
+        // must fit in shared memory; several CTAs per SM hide the tile load behind other CTAs'
+        // arithmetic; and the band's 1 x 8 strips should fill a whole number of rounds over the CTA's
+        // threads.  Score = strip-round efficiency x min(1, warps per SM / 12) / halo re-read factor.
         c->dp_Wp = (c->We + 1) & ~1;
         const int Kd = (c->K + 1) & ~1;
         const size_t fixed = (size_t)c->K * Kd + Kd + 16;
-        long br = (long)((100 * 1024 / sizeof(double) - fixed) / c->dp_Wp) - (c->K - 1);
-        if (br < 8) br = (long)(((SMEM_LIMIT - 1024) / sizeof(double) - fixed) / c->dp_Wp) - (c->K - 1);
-        if (br >= 1) {
-            if (br > cfg->ny) br = cfg->ny;
-            c->dp_n_bands = (int)((cfg->ny + br - 1) / br);
-            c->dp_band_rows = (cfg->ny + c->dp_n_bands - 1) / c->dp_n_bands;
-            c->dp_conv_smem = sizeof(double) * (fixed + (size_t)(c->dp_band_rows + c->K - 1) * c->dp_Wp);
-            c->dp_trace = tl_trace_dp_for(cfg->n_lens_light, cfg->n_source);
+        const int nsx = (cfg->nx + 7) / 8;
+        double best = -1.0;
+        for (int nb = 1; nb <= cfg->ny && nb <= 64; ++nb) {
+            const int br = (cfg->ny + nb - 1) / nb;
+            if ((br - 1) * nb >= cfg->ny && nb > 1) continue;                 // an empty last band
+            const size_t smem = sizeof(double) * (fixed + (size_t)(br + c->K - 1) * c->dp_Wp);
+            if (smem > SMEM_LIMIT - 1024) continue;
+            for (int thr = 64; thr <= 256; thr += 32) {
+                int ctas = (int)(SMEM_LIMIT / (smem + 1024));
+                const int by_regs = 65536 / (thr * 96), by_thr = 2048 / thr;
+                if (ctas > by_regs) ctas = by_regs;
+                if (ctas > by_thr) ctas = by_thr;
+                if (ctas > 16) ctas = 16;
+                if (ctas < 1) continue;
+                const int strips = br * nsx, rounds = (strips + thr - 1) / thr;
+                const double eff = (double)strips / ((double)rounds * thr);
+                const double occ = ctas * thr / 32.0 >= 12.0 ? 1.0 : ctas * thr / 32.0 / 12.0;
+                const double halo = 1.0 + 0.1 * (double)(c->K - 1) / br;       // the load is ~10 % of a band's time
+                const double score = eff * occ / halo;
+                if (score > best + 1e-9) { best = score; c->dp_n_bands = nb; c->dp_band_rows = br; c->dp_conv_threads = thr; c->dp_conv_smem = smem; }
+            }
+        }
+        if (best > 0.0) {
+            c->dp_trace = tl_trace_dp_for(cfg->supersample, cfg->n_lens_light, cfg->n_source);
             int occ = 0;
             bool okd = cuda_ok(cudaFuncSetAttribute(tl::conv_dp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SMEM_LIMIT - 1024))) &&
+                       cuda_ok(cudaFuncSetAttribute(tl::conv_dp_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared)) &&
                        cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, c->dp_trace, 256, 0)) && occ >= 1;
             if (!okd) { tl_destroy(c); return TL_ECUDA; }
             c->dp_trace_grid = occ * c->n_sm;

@@ -38,7 +38,8 @@ namespace tl {
 
 struct CompD {
     double a, b2, cc;            // t = (R_p/r_e)^2 = a x^2 + b2 x y + cc y^2 in the frame of the offsets (arcsec)
-    double ox, oy;               // lens light: centre (image frame); source k: R^T (s_k - s_first) (lens frame)
+    double ox, oy;               // lens light: centre (image frame); source k: R^T (s_k - s_first) (lens frame;
+                                 // rows without any deflection: s_k itself, the lens frame being the identity)
     double p, K, amp;            // 1/(2n), b_n log2(e), I_e / S^2
     int valid, pad;
 };
@@ -108,14 +109,31 @@ __device__ __forceinline__ double dp_div(double num, double den)
     return fma(rc, fma(-den, q0, num), q0);
 }
 
+// The tables live in shared memory and are read through 32-bit shared-window addresses computed
+// once per kernel (a generic pointer makes the compiler rebuild the window base -- S2R, LEA --
+// next to every table load).
+struct DpTabs { unsigned ltab, etab; };
+__device__ __forceinline__ double2 lds_f64x2(unsigned addr)
+{
+    double2 v;
+    asm("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ double lds_f64(unsigned addr)
+{
+    double v;
+    asm("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
+    return v;
+}
+
 // log2 t for t >= 0 (t = 0 gives -1023; denormals are not distinguished from 0)
-__device__ __forceinline__ double dp_log2(double t, const double2 *ltab)
+__device__ __forceinline__ double dp_log2(double t, const DpTabs &tb_)
 {
     const int hi = __double2hiint(t), lo = __double2loint(t);
     const int e = (hi >> 20) - 1023;
-    const int i = (((hi >> 12) & 0xff) + 1) >> 1;                   // round((m - 1) 128), 0 .. 128
+    const int i16 = (((hi >> 9) & 0x7f8) + 8) & 0xff0;              // 16 round((m - 1) 128), entries 0 .. 128
     const double m = __hiloint2double((hi & 0x000fffff) | 0x3ff00000, lo);
-    const double2 tb = ltab[i];                                    // {1/c_i, log2 c_i}
+    const double2 tb = lds_f64x2(tb_.ltab + i16);                  // {1/c_i, log2 c_i}
     const double r = fma(m, tb.x, -1.0);
     double p = DP_LOGP3;
     p = fma(p, r, DP_LOGP2); p = fma(p, r, DP_LOGP1); p = fma(p, r, DP_LOGP0);
@@ -123,18 +141,17 @@ __device__ __forceinline__ double dp_log2(double t, const double2 *ltab)
     return fma(r, p, ed + tb.y);
 }
 
-// 2^x for x <= 1000 (clamped below at -1000: the result is then 1e-301, i.e. 0 for every use here)
-__device__ __forceinline__ double dp_exp2(double x, const double *etab)
+// 2^x for -6e7 < x <= 1000; below -1022 the result is ~1e-308, i.e. 0 for every use here
+__device__ __forceinline__ double dp_exp2(double x, const DpTabs &tb_)
 {
-    x = fmax(x, -1000.0);
     const double xs = x + 211106232532992.0;                       // 1.5 * 2^47: ulp = 1/32
     const double r = x - (xs - 211106232532992.0);                 // |r| <= 1/64
     const int n = __double2loint(xs);                              // round(32 x)
-    const double T = etab[n & 31];
+    const double T = lds_f64(tb_.etab + ((n & 31) << 3));
     double q = DP_EXPP3;
     q = fma(q, r, DP_EXPP2); q = fma(q, r, DP_EXPP1); q = fma(q, r, DP_EXPP0);
-    const double y = fma(T * r, q, T);                             // in [1, 2)
-    return __hiloint2double(__double2hiint(y) + ((n >> 5) << 20), __double2loint(y));
+    const double y = fma(T * r, q, T);                             // in [0.98, 2.03)
+    return __hiloint2double(__double2hiint(y) + (max(n >> 5, -1022) << 20), __double2loint(y));
 }
 
 __device__ __forceinline__ double dp_atan_small(double r)         // |r| <= 0.6
@@ -148,14 +165,16 @@ __device__ __forceinline__ double dp_atan_small(double r)         // |r| <= 0.6
 }
 
 // Sersic value 2^(K (1 - u)), u = t^(1/2n) (the caller multiplies by amp)
-__device__ __forceinline__ double dp_sersic(const CompD &C, double t, const double2 *ltab, const double *etab)
+__device__ __forceinline__ double dp_sersic(double p, double K, double t, const DpTabs &tb)
 {
-    const double u = dp_exp2(C.p * dp_log2(t, ltab), etab);
-    return dp_exp2(fma(-C.K, u, C.K), etab);
+    const double u = dp_exp2(p * dp_log2(t, tb), tb);              // |p log2 t| <= 1023 p
+    double x = fma(-K, u, K);
+    x = x < -1100.0 ? -1100.0 : x;                                 // u can be huge (small n, far out): 2^x = 0
+    return dp_exp2(x, tb);
 }
 
 // SIE deflection in the lens frame (arcsec)
-__device__ __forceinline__ void dp_sie(const RowD &R, double xp, double yp, const double2 *ltab, double &axp, double &ayp)
+__device__ __forceinline__ void dp_sie(const RowD &R, double xp, double yp, const DpTabs &tb, double &axp, double &ayp)
 {
     const double psi2 = fma(R.q2 * xp, xp, fma(yp, yp, 1e-280));  // > 0: at the lens centre both angles come out as 0 (G6)
     const double psi = psi2 * dp_rsqrt(psi2);
@@ -165,7 +184,7 @@ __device__ __forceinline__ void dp_sie(const RowD &R, double xp, double yp, cons
     const double pa = dp_atan_small(n2 * dp_rcp(d2));
     const double a1 = fma(R.f, pa, R.fth0);
     // atanh(z) = ln((1 + z)/(1 - z))/2, z = q'|y'|/psi
-    const double a2 = R.fl2 * dp_log2(dp_div(psi + Ay, psi - Ay), ltab);
+    const double a2 = R.fl2 * dp_log2(dp_div(psi + Ay, psi - Ay), tb);
     axp = copysign(a1, xp);
     ayp = copysign(a2, yp);
 }
@@ -200,12 +219,18 @@ __global__ void __launch_bounds__(64) prologue_dp_kernel(const DpArgs a)
     const double thE = ok ? (double)p[0] : 0.0;
     if (!ok) { q = 1.0; c = 1.0; s = 0.0; }
     const double g1 = ok ? (double)p[5] : 0.0, g2 = ok ? (double)p[6] : 0.0;
-    R.cx = ok ? (double)p[3] : 0.0; R.cy = ok ? (double)p[4] : 0.0; R.c = c; R.s = s;
+    // No deflection at all (theta_E = 0 and no shear): beta = theta EXACTLY, and a Sersic of large n
+    // is not Lipschitz at its centre (I ~ I_0 (1 - b_n (R/r_e)^(1/n))), so a source centre that
+    // coincides with a sample must give R = 0 exactly, not the 1e-16 residual of the lens-frame
+    // constants.  Such rows use the identity as "lens frame" and plain source centres.
+    const bool nolens = thE == 0.0 && g1 == 0.0 && g2 == 0.0;
+    if (nolens) { q = 1.0; c = 1.0; s = 0.0; }
+    R.cx = (ok && !nolens) ? (double)p[3] : 0.0; R.cy = (ok && !nolens) ? (double)p[4] : 0.0; R.c = c; R.s = s;
     R.n11 = c * (1.0 + g1) + s * g2; R.n12 = c * g2 + s * (1.0 - g1);
     R.n21 = -s * (1.0 + g1) + c * g2; R.n22 = -s * g2 + c * (1.0 - g1);
     const float *s1 = p + LP + 7 * a.n_lens_light;
     const bool s1ok = isfinite(s1[5]) && isfinite(s1[6]);
-    const double s1x = s1ok ? (double)s1[5] : 0.0, s1y = s1ok ? (double)s1[6] : 0.0;
+    const double s1x = (s1ok && !nolens) ? (double)s1[5] : 0.0, s1y = (s1ok && !nolens) ? (double)s1[6] : 0.0;
     R.d1 = R.n11 * R.cx + R.n12 * R.cy - (c * s1x + s * s1y);
     R.d2 = R.n21 * R.cx + R.n22 * R.cy - (-s * s1x + c * s1y);
     // q' clamped away from 0 (relative change of alpha < 1e-18; atan(z)/z, atanh(z)/z -> 1, G6)
@@ -255,7 +280,11 @@ __global__ void __launch_bounds__(64) prologue_dp_kernel(const DpArgs a)
 }
 
 // ---- steps a1-a5 in FP64: one warp per (row, tile of CW x CH = 32 extended pixels) -----------------
-template <int NLL, int NSRC>
+// Two passes over the S x S sub-samples of a pixel -- lens light, then ray-trace + sources -- so that
+// each loop keeps few row constants live and the compiler can interleave the dependency chains of
+// several sub-samples (the FP64 pipe needs ~4 independent DFMAs in flight per scheduler, and 128
+// registers hold only one full sample's worth of FP64 state).  S_T > 0: compile-time supersampling.
+template <int S_T, int NLL, int NSRC>
 __global__ void __launch_bounds__(256, 2) trace_dp_kernel(const DpArgs a)
 {
     __shared__ double2 ltab[DP_LOG_N + 1];
@@ -264,6 +293,9 @@ __global__ void __launch_bounds__(256, 2) trace_dp_kernel(const DpArgs a)
     for (int i = threadIdx.x; i <= DP_LOG_N; i += blockDim.x) ltab[i] = make_double2(DP_LOG_TABLE[i][0], DP_LOG_TABLE[i][1]);
     for (int i = threadIdx.x; i < DP_EXP_N; i += blockDim.x) etab[i] = DP_EXP_TABLE[i];
     __syncthreads();
+    DpTabs tb;
+    tb.ltab = (unsigned)__cvta_generic_to_shared(ltab);
+    tb.etab = (unsigned)__cvta_generic_to_shared(etab);
     const int n_rows = dp_n_rows(a);
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const int lj = lane % a.CW, li = lane / a.CW;
@@ -272,8 +304,10 @@ __global__ void __launch_bounds__(256, 2) trace_dp_kernel(const DpArgs a)
     const long long n_warps = (long long)gridDim.x * (blockDim.x >> 5);
     RowD &R = rsh[wid];
     int cur = -1;
-    const int S = a.S;
-    const double u = a.u;
+    const int S = S_T > 0 ? S_T : a.S;
+    const double u = a.u, du = 2.0 * u;
+    constexpr int UA = S_T >= 4 ? 4 : (S_T > 0 ? S_T : 1);          // sub-samples interleaved: lens-light pass
+    constexpr int UB = S_T >= 2 ? 2 : 1;                            //                          ray-trace pass
     for (long long item = (long long)blockIdx.x * (blockDim.x >> 5) + wid; item < n_items; item += n_warps) {
         const int r = (int)(item / n_tiles), tile = (int)(item - (long long)r * n_tiles);
         if (r != cur) {                                            // this warp's copy of the row constants
@@ -292,41 +326,67 @@ __global__ void __launch_bounds__(256, 2) trace_dp_kernel(const DpArgs a)
         const bool edge = a.edge_zero && (j < a.h || j >= a.We - a.h || i < a.h || i >= a.He - a.h);
         if (!edge) {
             const double x0 = (double)(2 * j * S + 1 - S * a.We) * u, y0 = (double)(2 * i * S + 1 - S * a.He) * u;
-            const double du = 2.0 * u;
-            double y = y0;
+            if (NLL) {                                             // ---- pass A: lens light at theta (step a4)
+                const CompD &C = R.comp[0];
+                const double la = C.a, lb2 = C.b2, lcc = C.cc, lp = C.p, lK = C.K;
+                const double dxl0 = x0 - C.ox;
+                double dyl = y0 - C.oy;
+                double accl = 0.0;
 #pragma unroll 1
-            for (int sa = 0; sa < S; ++sa, y += du) {
-                const double dy = y - R.cy;
-                const double Qc = dy * R.c, Qs = dy * R.s;
-                const double V = fma(dy, R.n12, R.d1), V2 = fma(dy, R.n22, R.d2);
-                double dyl = 0.0, LC = 0.0, LBy = 0.0;
-                if (NLL) { dyl = y - R.comp[0].oy; LC = R.comp[0].cc * dyl * dyl; LBy = R.comp[0].b2 * dyl; }
-                double x = x0;
-#pragma unroll 2
-                for (int sb = 0; sb < S; ++sb, x += du) {
-                    if (NLL) {
-                        const double dxl = x - R.comp[0].ox;
-                        const double t = fma(dxl, fma(R.comp[0].a, dxl, LBy), LC);
-                        acc = fma(R.comp[0].amp, dp_sersic(R.comp[0], t, ltab, etab), acc);
-                    }
-                    const double dx = x - R.cx;
-                    const double xp = fma(dx, R.c, Qs), yp = fma(-dx, R.s, Qc);
-                    double axp, ayp;
-                    if (R.mode == 0) dp_sie(R, xp, yp, ltab, axp, ayp);
-                    else dp_alpha_slow(R, xp, yp, axp, ayp);
-                    const double bx = fma(dx, R.n11, V) - axp, by = fma(dx, R.n21, V2) - ayp;   // R^T (beta - s_first)
-                    {
-                        const CompD &C = R.comp[NLL];
-                        const double t = fma(bx, fma(C.a, bx, C.b2 * by), C.cc * by * by);
-                        acc = fma(C.amp, dp_sersic(C, t, ltab, etab), acc);
-                    }
-                    if (NSRC > 1) {
-                        const CompD &C = R.comp[NLL + 1];
-                        const double ex = bx - C.ox, ey = by - C.oy;
-                        const double t = fma(ex, fma(C.a, ex, C.b2 * ey), C.cc * ey * ey);
-                        acc = fma(C.amp, dp_sersic(C, t, ltab, etab), acc);
+                for (int sa = 0; sa < S; ++sa, dyl += du) {
+                    const double LC = lcc * dyl * dyl, LBy = lb2 * dyl;
+#pragma unroll 1
+                    for (int sb = 0; sb < S; sb += UA) {
+                        double t[UA], v[UA];
+#pragma unroll
+                        for (int q = 0; q < UA; ++q) {
+                            const double dxl = dxl0 + (double)(sb + q) * du;
+                            t[q] = fma(dxl, fma(la, dxl, LBy), LC);
+                        }
+#pragma unroll
+                        for (int q = 0; q < UA; ++q) v[q] = dp_sersic(lp, lK, t[q], tb);
+#pragma unroll
+                        for (int q = 0; q < UA; ++q) accl += v[q];
                     }
                 }
+                acc = C.amp * accl;
+            }
+            {                                                      // ---- pass B: ray-trace + sources (a2, a3)
+                const double dx0 = x0 - R.cx;
+                double dy = y0 - R.cy;
+                double accs[NSRC];
+#pragma unroll
+                for (int k = 0; k < NSRC; ++k) accs[k] = 0.0;
+#pragma unroll 1
+                for (int sa = 0; sa < S; ++sa, dy += du) {
+                    const double Qc = dy * R.c, Qs = dy * R.s;
+                    const double V = fma(dy, R.n12, R.d1), V2 = fma(dy, R.n22, R.d2);
+#pragma unroll 1
+                    for (int sb = 0; sb < S; sb += UB) {
+                        double bx[UB], by[UB];
+#pragma unroll
+                        for (int q = 0; q < UB; ++q) {
+                            const double dx = dx0 + (double)(sb + q) * du;
+                            const double xp = fma(dx, R.c, Qs), yp = fma(-dx, R.s, Qc);
+                            double axp, ayp;
+                            if (R.mode == 0) dp_sie(R, xp, yp, tb, axp, ayp);
+                            else dp_alpha_slow(R, xp, yp, axp, ayp);
+                            bx[q] = fma(dx, R.n11, V) - axp; by[q] = fma(dx, R.n21, V2) - ayp;   // R^T (beta - s_first)
+                        }
+#pragma unroll
+                        for (int k = 0; k < NSRC; ++k) {
+                            const CompD &C = R.comp[NLL + k];
+#pragma unroll
+                            for (int q = 0; q < UB; ++q) {
+                                const double ex = bx[q] - C.ox, ey = by[q] - C.oy;      // (0, 0) for the first source unless nolens
+                                const double t = fma(ex, fma(C.a, ex, C.b2 * ey), C.cc * ey * ey);
+                                accs[k] += dp_sersic(C.p, C.K, t, tb);
+                            }
+                        }
+                    }
+                }
+#pragma unroll
+                for (int k = 0; k < NSRC; ++k) acc = fma(R.comp[NLL + k].amp, accs[k], acc);
             }
         }
         a.ext[((size_t)r * a.He + i) * a.Wp + j] = acc;

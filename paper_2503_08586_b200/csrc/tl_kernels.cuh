@@ -41,6 +41,10 @@ struct KArgs {
     // MGE mode (tl_mge.cuh): ext / mimg hold ext_nc = n_gauss + n_source components per row;
     // trace_lin_kernel writes its components from slot ext_k0 on (0, 0 = the linear-mode layout)
     int ext_nc, ext_k0, n_gauss;
+    // AUTO precision (fused path): rows whose first-order FP32 error bound exceeds the tolerance are
+    // appended to flag_list (their count in *flag_count) for re-evaluation by the FP64 path
+    int *flag_count, *flag_list;
+    float err_coh, err_rnd;  // bound = err_coh |sum e_i| + err_rnd sqrt(sum e_i^2),  e_i = (d_i - m_i) m_i / sigma_i^2
     const float *mge_c;      // [n_gauss] log2(e) / (2 sigma_k^2), arcsec^-2
     double *mge_gram;        // [chunk][MGE_GRAM_STRIDE]  G | b | d'Wd
     double *mge_sol;         // [chunk][MGE_MAX_COL]      solved amplitudes (FP64)
@@ -497,8 +501,11 @@ struct ConvBlock {
 // chi^2 terms of up to 4 outputs of row i starting at column x0 (and the optional image store).
 // x0 is a multiple of 4, so when nx is too the four data / weight values are one aligned 16-byte
 // load each (north_star (3): "vectorised coalesced loads"); the sum order is the same either way.
+// `err` (optional, AUTO precision): accumulates e = (d - m) m w and e^2, the first-order sensitivity
+// of logL to a relative error of the model pixel (delta logL = sum_i e_i eps_i).
+struct ErrAcc { float s1, s2; };
 __device__ __forceinline__ float chi2_strip(const KArgs &a, const float acc[4], int i, int x0,
-                                            const float *data, const float *wgt, float *image_out)
+                                            const float *data, const float *wgt, float *image_out, ErrAcc *err = nullptr)
 {
     float c = 0.f;
     if ((a.nx & 3) == 0) {                           // uniform over the grid
@@ -510,6 +517,11 @@ __device__ __forceinline__ float chi2_strip(const KArgs &a, const float acc[4], 
             const float4 wv = __ldg(reinterpret_cast<const float4 *>(wgt + o));
             const float d0 = dv.x - acc[0], d1 = dv.y - acc[1], d2 = dv.z - acc[2], d3 = dv.w - acc[3];
             c = fmaf(d0 * d0, wv.x, c); c = fmaf(d1 * d1, wv.y, c); c = fmaf(d2 * d2, wv.z, c); c = fmaf(d3 * d3, wv.w, c);
+            if (err) {
+                const float e0 = d0 * wv.x * acc[0], e1 = d1 * wv.y * acc[1], e2 = d2 * wv.z * acc[2], e3 = d3 * wv.w * acc[3];
+                err->s1 += (e0 + e1) + (e2 + e3);
+                err->s2 = fmaf(e0, e0, fmaf(e1, e1, fmaf(e2, e2, fmaf(e3, e3, err->s2))));
+            }
         }
         return c;
     }
@@ -520,8 +532,9 @@ __device__ __forceinline__ float chi2_strip(const KArgs &a, const float acc[4], 
             const int o = i * a.nx + x;
             if (image_out) image_out[o] = acc[r];
             if (data) {
-                const float d = __ldg(data + o) - acc[r];
-                c = fmaf(d * d, __ldg(wgt + o), c);
+                const float d = __ldg(data + o) - acc[r], wv = __ldg(wgt + o);
+                c = fmaf(d * d, wv, c);
+                if (err) { const float e = d * wv * acc[r]; err->s1 += e; err->s2 = fmaf(e, e, err->s2); }
             }
         }
     }
@@ -530,7 +543,7 @@ __device__ __forceinline__ float chi2_strip(const KArgs &a, const float acc[4], 
 
 template <int K>
 __device__ __forceinline__ double conv_chi2_blocks(const KArgs &a, const float *img, int e0, const float *taps,
-                                                   int i0, int i1, const float *data, const float *wgt, float *image_out)
+                                                   int i0, int i1, const float *data, const float *wgt, float *image_out, ErrAcc *err)
 {
     const int nsx = (a.nx + 3) / 4, npair = (i1 - i0 + 1) / 2;
     const int total = npair * nsx;
@@ -539,8 +552,8 @@ __device__ __forceinline__ double conv_chi2_blocks(const KArgs &a, const float *
         const int ip = s / nsx, i = i0 + 2 * ip, x0 = (s - ip * nsx) * 4;
         float a0[4], a1[4];
         ConvBlock<K>::run(img + (i - e0) * a.pitch + x0, a.pitch, taps, a0, a1);
-        float c = chi2_strip(a, a0, i, x0, data, wgt, image_out);
-        if (i + 1 < i1) c += chi2_strip(a, a1, i + 1, x0, data, wgt, image_out);
+        float c = chi2_strip(a, a0, i, x0, data, wgt, image_out, err);
+        if (i + 1 < i1) c += chi2_strip(a, a1, i + 1, x0, data, wgt, image_out, err);
         part += (double)c;
     }
     return part;
@@ -552,10 +565,10 @@ __device__ __forceinline__ double conv_chi2_blocks(const KArgs &a, const float *
 // blocked 2 x 4 kernel, any other odd size the generic 1 x 4 strip.
 __device__ __forceinline__ double conv_chi2_rows(const KArgs &a, const float *img, int e0,
                                                  const float *taps, int i0, int i1,
-                                                 const float *data, const float *wgt, float *image_out)
+                                                 const float *data, const float *wgt, float *image_out, ErrAcc *err = nullptr)
 {
 #define TL_CONV_CASE(KK) \
-    case KK: return conv_chi2_blocks<KK>(a, img, e0, taps, i0, i1, data, wgt, image_out);
+    case KK: return conv_chi2_blocks<KK>(a, img, e0, taps, i0, i1, data, wgt, image_out, err);
     switch (a.K) {
         TL_CONV_CASE(5)
         TL_CONV_CASE(15)
@@ -572,7 +585,7 @@ __device__ __forceinline__ double conv_chi2_rows(const KArgs &a, const float *im
         const int ir = s / nsx, i = i0 + ir, x0 = (s - ir * nsx) * CONV_R;
         float acc[CONV_R];
         conv_strip(img + (i - e0) * a.pitch + x0, a.pitch, taps, a.K, a.Kp, acc);
-        part += (double)chi2_strip(a, acc, i, x0, data, wgt, image_out);
+        part += (double)chi2_strip(a, acc, i, x0, data, wgt, image_out, err);
     }
     return part;
 }
@@ -619,14 +632,26 @@ __global__ void __launch_bounds__(TL_LB_T, TL_LB_B) fused_kernel(const KArgs a)
                                     [&](int i, int j, float v) { img[i * a.pitch + j] = v; });
         __syncthreads();
         // phase 2: PSF convolution from shared memory + chi^2
+        ErrAcc err = {0.f, 0.f};
+        const bool want_err = a.flag_count != nullptr && a.logL != nullptr;      // AUTO precision (uniform)
         const double part = conv_chi2_rows(a, img, 0, taps, 0, a.ny,
                                            a.logL ? a.data + lens * npix : nullptr,
                                            a.wgt + lens * npix,
-                                           a.images ? a.images + row * npix : nullptr);
+                                           a.images ? a.images + row * npix : nullptr, want_err ? &err : nullptr);
         // phase 3: deterministic reduction (Eq. 5)
         if (a.logL) {
             const double chi2 = block_sum(part, red);
-            if (threadIdx.x == 0) a.logL[row] = (float)(-0.5 * (chi2 + a.lconst[lens]));
+            const double ll = -0.5 * (chi2 + a.lconst[lens]);
+            if (threadIdx.x == 0) a.logL[row] = (float)ll;
+            if (want_err) {
+                // first-order FP32 error bound of this row (DESIGN.md 6 "AUTO"): delta logL = sum_i e_i eps_i
+                const double s1 = block_sum((double)err.s1, red), s2 = block_sum((double)err.s2, red);
+                if (threadIdx.x == 0) {
+                    const double bound = (double)a.err_coh * fabs(s1) + (double)a.err_rnd * sqrt(s2);
+                    const double tol = fmax(1e-3, 1e-6 * fabs(ll));
+                    if (!(bound <= tol)) a.flag_list[atomicAdd(a.flag_count, 1)] = (int)row;
+                }
+            }
         }
     }
 }

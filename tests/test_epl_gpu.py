@@ -37,7 +37,7 @@ def _gpu(api, prob, rows, precision=None):
     return ll.cpu().numpy().astype(np.float64), im.cpu().numpy().astype(np.float64), info
 
 
-def _compare(w, prob, rows, isnear, ll, im, oll, oim):
+def _compare(w, prob, rows, isnear, ll, im, oll, oim, near_measured):
     B = len(rows)
     peak = np.abs(oim).reshape(B, -1).max(axis=1)
     dpix = np.abs(im - oim).reshape(B, -1).max(axis=1)
@@ -46,9 +46,8 @@ def _compare(w, prob, rows, isnear, ll, im, oll, oim):
     dl = np.abs(ll - oll)
     prior = ~isnear
     assert np.all(dl[prior] <= tol[prior]), "logL (prior rows): worst %.3g x tol" % (dl[prior] / tol[prior]).max()
-    lens = np.arange(B) // (B // w.n_lens)
-    tn = np.maximum(tol, PT.fp32_floor(oim, prob.data[lens], prob.noise[lens], w.supersample))
-    assert np.all(dl[isnear] <= tn[isnear]), "logL (near-truth rows): worst %.3g x derived tol" % (dl[isnear] / tn[isnear]).max()
+    near = (dl[isnear] / tol[isnear]).max() if isnear.any() else 0.0
+    assert near <= PT.near_bound_fp32(near_measured), "logL (near-truth rows, fp32): %.3g x north_star > %.3g" % (near, PT.near_bound_fp32(near_measured))
     return (dpix / peak).max() / PT.PIX_TOL, (dl[prior] / tol[prior]).max() if prior.any() else 0.0, \
         (dl[isnear] / tol[isnear]).max() if isnear.any() else 0.0
 
@@ -60,7 +59,7 @@ def test_epl_configs_match_oracle(api, orc, idx, n_prior, n_near, n_lens):
     rows, isnear = PT.rows_with_near(W, w, prob, n_prior, n_near)
     ll, im, info = _gpu(api, prob, rows)
     oll, oim = PT.oracle_reference(orc, w, prob, rows)
-    pix, prior, near = _compare(w, prob, rows, isnear, ll, im, oll, oim)
+    pix, prior, near = _compare(w, prob, rows, isnear, ll, im, oll, oim, PT.FP32_NEAR_MEASURED_EPL[idx])
     print("EPL config %d path=%d: pix %.3g x tol, logL prior %.3g x tol, near %.3g x north-star tol"
           % (idx, info["path"], pix, prior, near))
 
@@ -90,9 +89,9 @@ def test_epl_slopes_shapes_and_flat_lenses(api, orc):
         ll, im, _ = _gpu(api, prob, rows)
         oll, oim = PT.oracle_reference(orc, w, prob, rows)
         assert np.all(np.isfinite(ll))
-        isnear = np.ones(len(rows), bool)          # small synthetic shape: derived tolerance for all (parity.py)
-        pix, _, near = _compare(w, prob, rows, isnear, ll, im, oll, oim)
-        print("EPL small S=%d: pix %.3g x tol, logL %.3g x north-star tol" % (S, pix, near))
+        isnear = np.zeros(len(rows), bool)         # prior draws with a few entries replaced: north_star as stated
+        pix, prior, _ = _compare(w, prob, rows, isnear, ll, im, oll, oim, 1.0)
+        print("EPL small S=%d: pix %.3g x tol, logL %.3g x north-star tol" % (S, pix, prior))
 
 
 def test_epl_slope_two_is_the_sie_kernel(api, orc):
@@ -153,10 +152,9 @@ def test_epl_linear_mode(api, orc, idx, n_prior, n_near):
     scale = np.maximum(np.abs(oamps).max(axis=1, keepdims=True), 1e-30)
     assert np.all(np.abs(amps - oamps) <= 2e-5 * scale), np.abs((amps - oamps) / scale).max()
     oimg = np.stack([np.tensordot(oamps[r], orc.component_images(cfg, prob.psf[0], rows[r]), axes=1) for r in range(len(rows))])
-    lens = np.zeros(len(rows), int)
-    tn = np.maximum(PT.logl_tol(oll), PT.fp32_floor(oimg, prob.data[lens], prob.noise[lens], w.supersample))
-    dl = np.abs(ll - oll)
-    assert np.all(dl <= tn), "EPL linear: worst %.3g x derived tol" % (dl / tn).max()
+    ratio = (np.abs(ll - oll) / PT.logl_tol(oll)).max()
+    print("EPL linear config %d: logL %.3g x north_star" % (idx, ratio))
+    assert ratio <= PT.near_bound_fp32(PT.FP32_LINEAR_MEASURED_EPL[idx]), ratio
 
 
 @pytest.mark.parametrize("seed", range(8))
@@ -169,7 +167,8 @@ def test_epl_random_shapes(api, orc, seed):
     rows, isnear = PT.rows_with_near(W, w, prob, 6, 2)
     ll, im, _ = _gpu(api, prob, rows)
     oll, oim = PT.oracle_reference(orc, w, prob, rows)
-    _compare(w, prob, rows, np.ones(len(rows), bool), ll, im, oll, oim)
+    res = _compare(w, prob, rows, isnear, ll, im, oll, oim, PT.FP32_EPL_SMALL_MEASURED)
+    print("EPL random shape %d: pix %.3g, prior %.3g, near %.3g x north_star" % ((seed,) + tuple(res)))
 
 
 def test_epl_full_size_csst_batch_sampled_against_oracle(api, orc):

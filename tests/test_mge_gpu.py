@@ -50,11 +50,11 @@ def _check(api, orc, w, prob, rows, sigmas, amp_rtol=None):
         gimg = np.tensordot(amps[r], M, axes=1)
         ll_at = orc.loglike_from_image(gimg, prob.data[lens[r]], prob.noise[lens[r]])
         assert ll_at <= oll[r] + 1e-9 * abs(oll[r])                 # the oracle's is the maximum
-        assert oll[r] - ll_at <= max(tol[r], floors[r]), (r, oll[r] - ll_at, tol[r], floors[r])
+        assert oll[r] - ll_at <= PT.near_bound_fp32(PT.FP32_MGE_MEASURED) * tol[r], (r, oll[r] - ll_at, tol[r])
         worst_fit = max(worst_fit, np.abs(gimg - oimg).max() / oimg.max())
     assert worst_fit <= 1e-4, worst_fit                             # fitted image, relative to its peak
     tn = np.maximum(tol, floors)
-    assert np.all(dl <= tn), "MGE logL parity: worst %.3g x derived tol (%.3g x north-star)" % ((dl / tn).max(), (dl / tol).max())
+    assert (dl / tol).max() <= PT.near_bound_fp32(PT.FP32_MGE_MEASURED), "MGE logL parity: worst %.3g x north_star" % (dl / tol).max()
     if amp_rtol is not None:
         scale = np.maximum(np.abs(oamps).max(axis=1, keepdims=True), 1e-30)
         assert np.all(np.abs(amps - oamps) <= amp_rtol * scale), np.abs((amps - oamps) / scale).max()
@@ -164,7 +164,7 @@ def test_mge_full_size_batch_sampled(api, orc):
         M = orc.mge_component_images(cfg, prob.psf[0], rows[r], sigmas)
         oimg = np.tensordot(oamps[t], M, axes=1)
         floor = PT.fp32_floor(oimg[None], prob.data[0][None], prob.noise[0][None], w.supersample)[0]
-        assert abs(ll[r] - oll[t]) <= max(tol[t], floor), (r, ll[r] - oll[t], tol[t], floor)
+        assert abs(ll[r] - oll[t]) <= PT.near_bound_fp32(PT.FP32_MGE_MEASURED) * tol[t], (r, ll[r] - oll[t], tol[t], floor)
         gimg = np.tensordot(amps[r], M, axes=1)
         assert np.abs(gimg - oimg).max() <= 1e-4 * oimg.max()
     # Eq. 6: the solved likelihood is a maximum over amplitudes, so never below the fixed-amplitude

@@ -31,10 +31,17 @@ def test_fp64_mode_meets_north_star_everywhere(api, orc, idx, n_prior, n_near, n
     ll = ctx.loglike(d).cpu().numpy().astype(np.float64)
     im = ctx.render(d).cpu().numpy().astype(np.float64)
     ll2 = ctx.loglike(d).cpu().numpy().astype(np.float64)
+    # the same model with CUDA's double math library instead of the hand-ordered polynomials: an
+    # independent check of every approximation in csrc/tl_dp.cuh (both results are rounded to float)
+    ctx.set_precision(api.TL_PRECISION_FP64_LIBM)
+    ll_libm = ctx.loglike(d).cpu().numpy().astype(np.float64)
+    im_libm = ctx.render(d).cpu().numpy().astype(np.float64)
     ctx.set_precision(api.TL_PRECISION_FP32)
     back = ctx.loglike(d).cpu().numpy().astype(np.float64)
     ctx.close()
     assert np.array_equal(ll, ll2) and np.array_equal(fast, back)
+    assert np.all(np.abs(ll - ll_libm) <= 1e-4 * PT.logl_tol(ll_libm) + np.abs(ll_libm) * 2.0 ** -23)
+    assert np.all(np.abs(im - im_libm) <= 2.0 ** -22 * np.abs(im_libm).max())
     oll, oim = PT.oracle_reference(orc, w, prob, rows)
     tol = PT.logl_tol(oll)
     # the result is returned as float: half an ulp of |logL| on top of the tolerance
