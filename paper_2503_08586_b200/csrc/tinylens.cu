@@ -137,12 +137,12 @@ inline bool pool_alloc(const tl_ctx *c, T **p, size_t bytes, cudaStream_t st)
 
 size_t fused_smem_bytes(const tl_ctx *c)
 {
-    return sizeof(tl::RowC) + 32 * sizeof(double) + sizeof(float) * ((size_t)c->K * c->Kp + (size_t)(c->He + 1) * c->pitch + c->Kp + 8);
+    return sizeof(tl::RowC) + 32 * sizeof(double) + sizeof(float) * (2 * (size_t)c->K * c->Kp + (size_t)(c->He + 1) * c->pitch + c->Kp + 8);
 }
 
 size_t conv_smem_bytes(const tl_ctx *c, int tile_rows)
 {
-    return 32 * sizeof(double) + sizeof(float) * ((size_t)c->K * c->Kp + (size_t)(tile_rows + 2 * c->h + 1) * c->pitch + c->Kp + 8);
+    return 32 * sizeof(double) + sizeof(float) * (2 * (size_t)c->K * c->Kp + (size_t)(tile_rows + 2 * c->h + 1) * c->pitch + c->Kp + 8);
 }
 
 tl::KArgs base_args(const tl_ctx *c)
@@ -206,7 +206,7 @@ int run_small_batch(tl_ctx *c, const float *params, int64_t B, float *logL, floa
     int slabs = want < (n_wtiles + 7) / 8 ? want : (n_wtiles + 7) / 8;
     int bands = want < npair ? want : npair;
     // the whole band (+ K - 1 rows of halo) and the taps must fit in shared memory
-    const size_t fixed = sizeof(float) * ((size_t)c->K * c->Kp + c->pitch + c->Kp + 8);
+    const size_t fixed = sizeof(float) * (2 * (size_t)c->K * c->Kp + c->pitch + c->Kp + 8);
     int band_pairs = (npair + bands - 1) / bands;
     const int max_pairs = (int)(((SMEM_LIMIT - 1024 - fixed) / (sizeof(float) * c->pitch) - (c->K - 1)) / 2);
     if (band_pairs > max_pairs) band_pairs = max_pairs;
@@ -573,8 +573,8 @@ int tl_create_ex(tl_ctx **out, const tl_config *cfg, const float *psf_in, int32_
     } else {
         c->path = 1;
         // tile rows: as many as fit in ~100 KB so two CTAs share an SM
-        int tr = (int)((100 * 1024 / sizeof(float) - (size_t)c->K * c->Kp - c->Kp - 8) / c->pitch) - 2 * c->h - 1;
-        if (tr < 4) tr = (int)((SMEM_LIMIT / sizeof(float) - 64 - (size_t)c->K * c->Kp - c->Kp - 8) / c->pitch) - 2 * c->h - 1;
+        int tr = (int)((100 * 1024 / sizeof(float) - 2 * (size_t)c->K * c->Kp - c->Kp - 8) / c->pitch) - 2 * c->h - 1;
+        if (tr < 4) tr = (int)((SMEM_LIMIT / sizeof(float) - 64 - 2 * (size_t)c->K * c->Kp - c->Kp - 8) / c->pitch) - 2 * c->h - 1;
         if (tr < 1) { tl_destroy(c); return TL_ESIZE; }
         if (tr > cfg->ny) tr = cfg->ny;
         c->tile_rows = tr; c->n_tiles = (cfg->ny + tr - 1) / tr;
@@ -598,12 +598,12 @@ int tl_create_ex(tl_ctx **out, const tl_config *cfg, const float *psf_in, int32_
         c->chunk_rows = cr;
     }
     {   // linear-amplitude pipeline: conv tiles of ~100 KB, row-value table when small
-        int tr = (int)((100 * 1024 / sizeof(float) - (size_t)c->K * c->Kp - c->Kp - 8) / c->pitch) - 2 * c->h - 1;
-        if (tr < 4) tr = (int)((SMEM_LIMIT / sizeof(float) - 64 - (size_t)c->K * c->Kp - c->Kp - 8) / c->pitch) - 2 * c->h - 1;
+        int tr = (int)((100 * 1024 / sizeof(float) - 2 * (size_t)c->K * c->Kp - c->Kp - 8) / c->pitch) - 2 * c->h - 1;
+        if (tr < 4) tr = (int)((SMEM_LIMIT / sizeof(float) - 64 - 2 * (size_t)c->K * c->Kp - c->Kp - 8) / c->pitch) - 2 * c->h - 1;
         if (tr >= 1) {
             if (tr > cfg->ny) tr = cfg->ny;
             c->lin_tile_rows = tr; c->lin_n_tiles = (cfg->ny + tr - 1) / tr;
-            c->lin_conv_smem = sizeof(float) * ((size_t)c->K * c->Kp + (size_t)(tr + 2 * c->h + 1) * c->pitch + c->Kp + 8);
+            c->lin_conv_smem = sizeof(float) * (2 * (size_t)c->K * c->Kp + (size_t)(tr + 2 * c->h + 1) * c->pitch + c->Kp + 8);
             c->trace_lin = cfg->mass_model == TL_MASS_EPL ? tl_trace_lin_epl_for(cfg->supersample, cfg->n_lens_light, cfg->n_source)
                                                           : tl_trace_lin_for(cfg->supersample, cfg->n_lens_light, cfg->n_source);
             bool okl = cuda_ok(cudaFuncSetAttribute(tl::conv_lin_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT));
@@ -617,7 +617,7 @@ int tl_create_ex(tl_ctx **out, const tl_config *cfg, const float *psf_in, int32_
         }
         // fused variant: C binned component images (+ the row-value table) in shared memory
         const size_t img_floats = ((size_t)c->He * c->pitch + c->pitch + c->Kp + 8 + 3) & ~(size_t)3;
-        size_t fl = sizeof(tl::RowC) + 32 * sizeof(double) + sizeof(float) * ((size_t)c->K * c->Kp + (size_t)c->n_comp * img_floats);
+        size_t fl = sizeof(tl::RowC) + 32 * sizeof(double) + sizeof(float) * (2 * (size_t)c->K * c->Kp + (size_t)c->n_comp * img_floats);
         int rt = 0;
         if (fl + rowtab_bytes <= SMEM_LIMIT) { fl += rowtab_bytes; rt = 1; }
         if (fl <= SMEM_LIMIT) {
@@ -636,7 +636,7 @@ int tl_create_ex(tl_ctx **out, const tl_config *cfg, const float *psf_in, int32_
         // must fit in shared memory; several CTAs per SM hide the tile load behind other CTAs'
         // arithmetic; and the band's 1 x 8 strips should fill a whole number of rounds over the CTA's
         // threads.  Score = strip-round efficiency x min(1, warps per SM / 12) / halo re-read factor.
-        c->dp_Wp = (c->We + 1) & ~1;
+        c->dp_Wp = ((c->We + 13) & ~15) + 2;        // >= We and = 2 (mod 16): see conv_dp_kernel
         const int Kd = (c->K + 1) & ~1;
         const size_t fixed = (size_t)c->K * Kd + Kd + 16;
         const int nsx = (cfg->nx + 7) / 8;

@@ -465,12 +465,17 @@ __global__ void __launch_bounds__(256) conv_dp_kernel(const DpArgs a)
     for (int t = threadIdx.x; t < n2; t += blockDim.x) dst[t] = src[t];
     for (int t = threadIdx.x; t < Kd + 16; t += blockDim.x) img[erows * a.Wp + t] = 0.0;     // read by discarded lanes only
     __syncthreads();
-    const int nsx = (a.nx + 7) / 8, total = (i1 - i0) * nsx;
+    // strips are numbered with the ROW fastest: the lanes of a warp then read window addresses one row
+    // pitch apart, and the pitch is 2 (mod 16) doubles = 16 bytes (mod 128), so the 8 lanes of a
+    // quarter-warp cover 8 different 16-byte bank groups: every LDS.128 is conflict-free.  (With the
+    // column fastest the lanes sit 64 bytes apart -- a 4-way conflict that made the kernel
+    // shared-memory bound at a third of the FP64 peak.)
+    const int nsx = (a.nx + 7) / 8, nrow = i1 - i0, total = nrow * nsx;
     const float *data = a.data + lens * npix;
     const double *wgt = a.wgt64 + lens * npix;
     double part = 0.0;
     for (int sIdx = threadIdx.x; sIdx < total; sIdx += blockDim.x) {
-        const int ir = sIdx / nsx, x0 = (sIdx - ir * nsx) * 8, i = i0 + ir;
+        const int xs = sIdx / nrow, ir = sIdx - xs * nrow, x0 = xs * 8, i = i0 + ir;
         double acc[8];
 #pragma unroll
         for (int o = 0; o < 8; ++o) acc[o] = 0.0;
