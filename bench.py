@@ -291,6 +291,9 @@ def run_ours(args, w: W.Workload):
         torch.cuda.synchronize()
 
     stream = torch.cuda.current_stream()
+    if args.streams > 1:
+        run_streams(args, w, ctx, info, d_rows, d_out, rows, clk_dev=local)
+        return
     ctx.set_profiling(True)
     clk = ClockSampler(local)
     clk.__enter__()                      # samples through warm-up, the timed steps and the e2e loop
@@ -321,6 +324,40 @@ def run_ours(args, w: W.Workload):
         torch.cuda.synchronize()
         e2e_s = time.perf_counter() - t0
         barrier()
+        # ---- sampler-like loop through the asynchronous host entry: batch k + 1 is submitted (its upload
+        # overlapping the kernels of batch k) before batch k is waited for ----
+        pipelined = []
+        if world == 1 and args.precision == "fp32":
+            for pb in (74, 300, 4096):
+                if pb > B or pb % w.n_lens:
+                    continue
+                hp = h_rows[:pb].contiguous().pin_memory()
+                outs = [torch.empty(pb, dtype=torch.float32).pin_memory() for _ in range(2)]
+                nbat = 40
+                ctx.wait(ctx.loglike_host_async(hp, outs[0]))
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                prev = ctx.loglike_host_async(hp, outs[0])
+                for k in range(1, nbat):
+                    cur = ctx.loglike_host_async(hp, outs[k & 1])
+                    ctx.wait(prev)
+                    prev = cur
+                ctx.wait(prev)
+                dt_pipe = time.perf_counter() - t0
+                t0 = time.perf_counter()
+                for k in range(nbat):
+                    ctx.loglike_host(hp, outs[0])
+                dt_sync = time.perf_counter() - t0
+                dsub = d_rows[:pb].contiguous()
+                torch.cuda.synchronize()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream)
+                for k in range(nbat):
+                    ctx.loglike(dsub, d_out[:pb])
+                e1.record(stream)
+                torch.cuda.synchronize()
+                pipelined.append({"B": pb, "batches": nbat, "pipelined_per_s": pb * nbat / dt_pipe, "sync_per_s": pb * nbat / dt_sync,
+                                  "device_resident_per_s": pb * nbat / (e0.elapsed_time(e1) * 1e-3)})
     clk.__exit__(None, None, None)
     clocks = clk.summary()
     total_ms = float(np.sum(step_ms))
@@ -359,6 +396,7 @@ def run_ours(args, w: W.Workload):
         "clocks": clocks,
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": B * w.n_params * 4,
                 "d2h_bytes_per_step": B * 4, "api": "tl_loglike_batch_host (pinned host buffers)"},
+        "e2e_pipelined": pipelined,
         "gpu_launches": (3 if B <= info["small_batch_rows"] else info["launches_per_call"]) * args.steps,
         "roofline": {
             "bound": "alu", "kernel": "fused_kernel" if (info["path"] == 0 and B > info["small_batch_rows"]) else "trace_kernel",
@@ -387,6 +425,63 @@ def run_ours(args, w: W.Workload):
     print(json.dumps(line))
     if use_dist:
         dist.destroy_process_group()
+
+
+def run_streams(args, w, ctx, info, d_rows, d_out, rows, clk_dev=0):
+    """The batch as sub-batches of --sub-batch rows issued round-robin on --streams streams that share
+    one context (BASELINE configs[4]: "B = 65536 split across streams on one GPU").  Timed on the
+    device: a start event all streams wait for, an end event per stream, the latest end counts."""
+    import torch
+    B = rows.shape[0]
+    sub = min(args.sub_batch, B)
+    if w.n_lens > 1:
+        raise SystemExit("--streams: single-lens workloads only")
+    streams = [torch.cuda.Stream() for _ in range(args.streams)]
+    chunks = [(lo, min(B, lo + sub)) for lo in range(0, B, sub)]
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=d_rows.device)
+
+    def issue():
+        for k, (lo, hi) in enumerate(chunks):
+            st = streams[k % len(streams)]
+            ctx.loglike(d_rows[lo:hi], d_out[lo:hi], stream=st)
+
+    for _ in range(max(1, min(args.warmup, 2))):
+        issue()
+    torch.cuda.synchronize()
+    steps = args.steps
+    times = []
+    with ClockSampler(clk_dev) as clk:
+        for s in range(steps):
+            flush.fill_(s & 0xff)
+            start = torch.cuda.Event(enable_timing=True)
+            ends = [torch.cuda.Event(enable_timing=True) for _ in streams]
+            start.record(torch.cuda.current_stream())
+            for st in streams:
+                st.wait_event(start)
+            issue()
+            for st, e in zip(streams, ends):
+                e.record(st)
+            torch.cuda.synchronize()
+            times.append(max(start.elapsed_time(e) for e in ends))
+    total_ms = float(np.sum(times))
+    value = B * steps / (total_ms * 1e-3)
+    om = op_model(w, rows)
+    sm_max = float(measured_peaks().get("sm_max_mhz", 1965.0))
+    peak = info["n_sm"] * SM_FP32_LANES * sm_max * 1e6 / 1e12
+    ach = om["issue_slots"] * B * steps / (total_ms * 1e-3) / 1e12
+    launches = (3 if sub <= info["small_batch_rows"] else info["launches_per_call"]) * len(chunks) * steps
+    print(json.dumps({
+        "metric": METRIC + mass_tag(w), "value": value, "unit": UNIT, "n_gpus": 1, "steps": steps, "warmup": max(1, min(args.warmup, 2)),
+        "ms_per_step": total_ms / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": {"fp32": "f32", "auto": "f32+f64"}.get(args.precision, "f64"), "data": "synthetic", "precision": args.precision,
+        "config": config_dict(w, "flushed between steps (256 MiB fill)"),
+        "streams": args.streams, "sub_batch_rows": sub, "sub_batches": len(chunks),
+        "pixel_evals_per_s": value * w.ny * w.nx, "sample_evals_per_s": value * om["samples"], "clocks": clk.summary(),
+        "gpu_launches": launches,
+        "roofline": {"bound": "alu", "kernel": "whole step (all sub-batches, all kernels)", "achieved": ach, "peak": peak, "unit": "Tinst/s",
+                     "frac": ach / peak, "traffic": None, "algorithmic_issue_slots_per_likelihood": om["issue_slots"],
+                     "peak_source": "derived: %d SMs x %d issue slots/clk x %.0f MHz" % (info["n_sm"], SM_FP32_LANES, sm_max)},
+        "checksum_logL": float(d_out.double().sum())}))
 
 
 def run_linear(args, w: W.Workload):
@@ -572,6 +667,10 @@ def main():
     ap.add_argument("--rows", default="prior", choices=["prior", "near-truth"],
                     help="prior: the BASELINE batch (independent prior draws); near-truth: truth (1 + 1e-3 N(0,1)) rows, "
                          "the regime a converged sampler works in (SURVEY.md 8(d) near-truth slice)")
+    ap.add_argument("--streams", type=int, default=1,
+                    help="issue the batch as sub-batches on this many CUDA streams sharing one context "
+                         "(BASELINE configs[4]: B = 65536 split across streams); with --sub-batch rows per sub-batch")
+    ap.add_argument("--sub-batch", type=int, default=4096, help="rows per sub-batch when --streams > 1")
     ap.add_argument("--peaks", action="store_true",
                     help="run the pipe micro-benchmarks (tl_measure_peaks: FFMA, FFMA2, MUFU, DFMA and mixes) and exit")
     args = ap.parse_args()
@@ -586,6 +685,19 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if world != args.gpus and world > 1:
         raise SystemExit("--gpus %d does not match WORLD_SIZE %d" % (args.gpus, world))
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ and args.impl == "ours":
+        # not under torchrun: launch one rank per GPU ourselves (same command line), NCCL's own
+        # communicator log left on (stderr) so that the transport it picked is on record
+        import socket
+        import torch
+        if torch.cuda.device_count() < args.gpus:
+            raise SystemExit("bench.py: --gpus %d but only %d CUDA device(s) visible" % (args.gpus, torch.cuda.device_count()))
+        sk = socket.socket(); sk.bind(("127.0.0.1", 0)); port = sk.getsockname()[1]; sk.close()
+        env = dict(os.environ)
+        env.setdefault("NCCL_DEBUG", "INFO")
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        raise SystemExit(subprocess.call(cmd, env=env))
     if args.mode == "mge" and w.n_lens_light != 1:
         raise SystemExit("bench.py --mode mge needs a workload with lens light (configs 1-4)")
     if args.impl == "reference":

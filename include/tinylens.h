@@ -269,6 +269,29 @@ int tl_loglike_mge_batch(tl_ctx *ctx, const float *params, int64_t B, float *log
 int tl_loglike_batch_host(tl_ctx *ctx, const float *params, int64_t B, float *logL, void *cuda_stream);
 
 /*
+ * tl_loglike_batch_host_async / tl_wait -- the same end-to-end call, split so that a host-side
+ * sampler can overlap its own work and the upload of the next batch with the kernels of the
+ * current one (PAPER.md:250 names the CPU<->GPU transfers, :285 the CPU sampler, as the limit of
+ * the whole pipeline).  The context owns two staging slots (pinned host + device buffers, grown on
+ * demand and then reused: no allocation per call) and an upload and a download stream of its own.
+ *   tl_loglike_batch_host_async
+ *     params   HOST pointer, float [B][P]; copied into the slot's pinned buffer before the call
+ *              returns, so the caller may reuse it at once
+ *     B        rows (>= 1; multiple of n_lens)
+ *     logL     HOST pointer, float [B]; written by tl_wait (must stay valid until then)
+ *     cuda_stream  stream the kernels run on (the upload runs on the context's own stream and the
+ *              kernels wait for it; the download waits for the kernels)
+ *     returns the slot (0 or 1) to pass to tl_wait, or a negative error code.  Slots alternate; a
+ *     submission that finds its slot still in flight first completes that earlier submission
+ *     (its logL buffer is written), so at most two batches are in flight.
+ *   tl_wait    blocks until the slot's batch is complete, copies its logL into the caller's buffer and
+ *              frees the slot.  TL_OK, TL_EINVAL (slot not in flight) or TL_ECUDA.
+ * One submitting thread per context.  tl_loglike_batch_host is submit + wait.
+ */
+int tl_loglike_batch_host_async(tl_ctx *ctx, const float *params, int64_t B, float *logL, void *cuda_stream);
+int tl_wait(tl_ctx *ctx, int slot);
+
+/*
  * tl_set_precision -- choose the arithmetic of later tl_loglike_batch / tl_render_batch /
  * tl_loglike_batch_host calls on this context (not of tl_loglike_linear_batch).
  *   TL_PRECISION_FP32 (default)  the FP32 kernels: meet the tolerances of DESIGN.md "Tolerances"

@@ -84,6 +84,8 @@ def load(build_if_missing: bool = True):
     L.tl_loglike_batch.restype = C.c_int; L.tl_loglike_batch.argtypes = [vp, vp, i64, vp, vp]
     L.tl_render_batch.restype = C.c_int; L.tl_render_batch.argtypes = [vp, vp, i64, vp, vp]
     L.tl_loglike_batch_host.restype = C.c_int; L.tl_loglike_batch_host.argtypes = [vp, vp, i64, vp, vp]
+    L.tl_loglike_batch_host_async.restype = C.c_int; L.tl_loglike_batch_host_async.argtypes = [vp, vp, i64, vp, vp]
+    L.tl_wait.restype = C.c_int; L.tl_wait.argtypes = [vp, C.c_int]
     L.tl_loglike_linear_batch.restype = C.c_int; L.tl_loglike_linear_batch.argtypes = [vp, vp, i64, vp, vp, vp]
     L.tl_set_mge.restype = C.c_int; L.tl_set_mge.argtypes = [vp, fp, i32]
     L.tl_mge_columns.restype = C.c_int; L.tl_mge_columns.argtypes = [vp]
@@ -276,6 +278,36 @@ def tl_loglike_batch_host(handle: int, params_host, out_host=None, stream=None):
     return out_host
 
 
+def _host_rows(handle, params_host):
+    import torch
+    P = tl_param_count(handle)
+    if isinstance(params_host, np.ndarray):
+        params_host = torch.from_numpy(_f32c(params_host))
+    if params_host.is_cuda or params_host.dtype != torch.float32 or not params_host.is_contiguous() \
+            or params_host.dim() != 2 or params_host.shape[1] != P:
+        raise TinyLensError(TL_EINVAL, "params_host must be a contiguous host float32 tensor [B, %d]" % P)
+    return params_host
+
+
+def tl_loglike_batch_host_async(handle: int, params_host, out_host, stream=None) -> int:
+    """Submit one batch (host float32 [B,P]); out_host (host float32 [B]) is written by tl_wait(slot) and must
+    stay alive until then.  Returns the slot."""
+    import torch
+    params_host = _host_rows(handle, params_host)
+    B = params_host.shape[0]
+    if not (isinstance(out_host, torch.Tensor) and not out_host.is_cuda and out_host.dtype == torch.float32
+            and out_host.is_contiguous() and out_host.numel() == B):
+        raise TinyLensError(TL_EINVAL, "out_host must be a contiguous host float32 tensor [B]")
+    slot = load().tl_loglike_batch_host_async(handle, params_host.data_ptr(), B, out_host.data_ptr(), _stream_handle(stream))
+    if slot < 0:
+        raise TinyLensError(slot, "tl_loglike_batch_host_async")
+    return slot
+
+
+def tl_wait(handle: int, slot: int):
+    _check(load().tl_wait(handle, int(slot)), "tl_wait")
+
+
 def tl_set_precision(handle: int, precision: int):
     _check(load().tl_set_precision(handle, int(precision)), "tl_set_precision")
 
@@ -344,6 +376,16 @@ class LensContext:
 
     def loglike_host(self, params_host, out_host=None, stream=None):
         return tl_loglike_batch_host(self.handle, params_host, out_host, stream)
+
+    def loglike_host_async(self, params_host, out_host, stream=None) -> int:
+        slot = tl_loglike_batch_host_async(self.handle, params_host, out_host, stream)
+        self._pending = getattr(self, "_pending", {})
+        self._pending[slot] = out_host                  # keeps the result buffer alive until wait()
+        return slot
+
+    def wait(self, slot: int):
+        tl_wait(self.handle, slot)
+        return getattr(self, "_pending", {}).pop(slot, None)
 
     def set_precision(self, precision: int):
         tl_set_precision(self.handle, precision)

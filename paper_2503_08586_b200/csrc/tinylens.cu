@@ -81,6 +81,18 @@ struct tl_ctx {
     float *mge_c = nullptr;       // device [n_gauss]: log2(e) / (2 sigma_k^2)
     int n_gauss = 0;
     double refine_tau = 7.5e-4;   // x S at create: a pixel averages S^2 samples
+    // asynchronous host entry (tl_loglike_batch_host_async / tl_wait): two staging slots, each with
+    // pinned host and device buffers for one batch, an upload and a download stream of the library's
+    // own, so that the upload of batch k + 1 overlaps the kernels of batch k
+    struct HostSlot {
+        float *h_params = nullptr, *h_logl = nullptr, *d_params = nullptr, *d_logl = nullptr;
+        int64_t cap_rows = 0, B = 0;
+        float *user_logl = nullptr;
+        cudaEvent_t up = nullptr, done = nullptr, fin = nullptr;
+        int busy = 0, rc = 0;
+    } slots[2];
+    int next_slot = 0;
+    cudaStream_t s_up = nullptr, s_down = nullptr;
     tl_options opt;               // create-time options (tl_create_ex); defaults = automatic
     cudaMemPool_t pool = nullptr; // library-owned stream-ordered pool: per-call scratch (never the device's default pool)
     // benchmark facility (tl_set_profiling): events around the dominant kernel of the last call
@@ -137,12 +149,12 @@ inline bool pool_alloc(const tl_ctx *c, T **p, size_t bytes, cudaStream_t st)
 
 size_t fused_smem_bytes(const tl_ctx *c)
 {
-    return sizeof(tl::RowC) + 32 * sizeof(double) + sizeof(float) * (2 * (size_t)c->K * c->Kp + (size_t)(c->He + 1) * c->pitch + c->Kp + 8);
+    return sizeof(tl::RowC) + 32 * sizeof(double) + sizeof(float) * ((size_t)c->K * c->Kp + (size_t)(c->He + 1) * c->pitch + c->Kp + 8);
 }
 
 size_t conv_smem_bytes(const tl_ctx *c, int tile_rows)
 {
-    return 32 * sizeof(double) + sizeof(float) * (2 * (size_t)c->K * c->Kp + (size_t)(tile_rows + 2 * c->h + 1) * c->pitch + c->Kp + 8);
+    return 32 * sizeof(double) + sizeof(float) * ((size_t)c->K * c->Kp + (size_t)(tile_rows + 2 * c->h + 1) * c->pitch + c->Kp + 8);
 }
 
 tl::KArgs base_args(const tl_ctx *c)
@@ -206,7 +218,7 @@ int run_small_batch(tl_ctx *c, const float *params, int64_t B, float *logL, floa
     int slabs = want < (n_wtiles + 7) / 8 ? want : (n_wtiles + 7) / 8;
     int bands = want < npair ? want : npair;
     // the whole band (+ K - 1 rows of halo) and the taps must fit in shared memory
-    const size_t fixed = sizeof(float) * (2 * (size_t)c->K * c->Kp + c->pitch + c->Kp + 8);
+    const size_t fixed = sizeof(float) * ((size_t)c->K * c->Kp + c->pitch + c->Kp + 8);
     int band_pairs = (npair + bands - 1) / bands;
     const int max_pairs = (int)(((SMEM_LIMIT - 1024 - fixed) / (sizeof(float) * c->pitch) - (c->K - 1)) / 2);
     if (band_pairs > max_pairs) band_pairs = max_pairs;
@@ -573,8 +585,8 @@ int tl_create_ex(tl_ctx **out, const tl_config *cfg, const float *psf_in, int32_
     } else {
         c->path = 1;
         // tile rows: as many as fit in ~100 KB so two CTAs share an SM
-        int tr = (int)((100 * 1024 / sizeof(float) - 2 * (size_t)c->K * c->Kp - c->Kp - 8) / c->pitch) - 2 * c->h - 1;
-        if (tr < 4) tr = (int)((SMEM_LIMIT / sizeof(float) - 64 - 2 * (size_t)c->K * c->Kp - c->Kp - 8) / c->pitch) - 2 * c->h - 1;
+        int tr = (int)((100 * 1024 / sizeof(float) - (size_t)c->K * c->Kp - c->Kp - 8) / c->pitch) - 2 * c->h - 1;
+        if (tr < 4) tr = (int)((SMEM_LIMIT / sizeof(float) - 64 - (size_t)c->K * c->Kp - c->Kp - 8) / c->pitch) - 2 * c->h - 1;
         if (tr < 1) { tl_destroy(c); return TL_ESIZE; }
         if (tr > cfg->ny) tr = cfg->ny;
         c->tile_rows = tr; c->n_tiles = (cfg->ny + tr - 1) / tr;
@@ -598,12 +610,12 @@ int tl_create_ex(tl_ctx **out, const tl_config *cfg, const float *psf_in, int32_
         c->chunk_rows = cr;
     }
     {   // linear-amplitude pipeline: conv tiles of ~100 KB, row-value table when small
-        int tr = (int)((100 * 1024 / sizeof(float) - 2 * (size_t)c->K * c->Kp - c->Kp - 8) / c->pitch) - 2 * c->h - 1;
-        if (tr < 4) tr = (int)((SMEM_LIMIT / sizeof(float) - 64 - 2 * (size_t)c->K * c->Kp - c->Kp - 8) / c->pitch) - 2 * c->h - 1;
+        int tr = (int)((100 * 1024 / sizeof(float) - (size_t)c->K * c->Kp - c->Kp - 8) / c->pitch) - 2 * c->h - 1;
+        if (tr < 4) tr = (int)((SMEM_LIMIT / sizeof(float) - 64 - (size_t)c->K * c->Kp - c->Kp - 8) / c->pitch) - 2 * c->h - 1;
         if (tr >= 1) {
             if (tr > cfg->ny) tr = cfg->ny;
             c->lin_tile_rows = tr; c->lin_n_tiles = (cfg->ny + tr - 1) / tr;
-            c->lin_conv_smem = sizeof(float) * (2 * (size_t)c->K * c->Kp + (size_t)(tr + 2 * c->h + 1) * c->pitch + c->Kp + 8);
+            c->lin_conv_smem = sizeof(float) * ((size_t)c->K * c->Kp + (size_t)(tr + 2 * c->h + 1) * c->pitch + c->Kp + 8);
             c->trace_lin = cfg->mass_model == TL_MASS_EPL ? tl_trace_lin_epl_for(cfg->supersample, cfg->n_lens_light, cfg->n_source)
                                                           : tl_trace_lin_for(cfg->supersample, cfg->n_lens_light, cfg->n_source);
             bool okl = cuda_ok(cudaFuncSetAttribute(tl::conv_lin_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT));
@@ -617,7 +629,7 @@ int tl_create_ex(tl_ctx **out, const tl_config *cfg, const float *psf_in, int32_
         }
         // fused variant: C binned component images (+ the row-value table) in shared memory
         const size_t img_floats = ((size_t)c->He * c->pitch + c->pitch + c->Kp + 8 + 3) & ~(size_t)3;
-        size_t fl = sizeof(tl::RowC) + 32 * sizeof(double) + sizeof(float) * (2 * (size_t)c->K * c->Kp + (size_t)c->n_comp * img_floats);
+        size_t fl = sizeof(tl::RowC) + 32 * sizeof(double) + sizeof(float) * ((size_t)c->K * c->Kp + (size_t)c->n_comp * img_floats);
         int rt = 0;
         if (fl + rowtab_bytes <= SMEM_LIMIT) { fl += rowtab_bytes; rt = 1; }
         if (fl <= SMEM_LIMIT) {
@@ -784,6 +796,8 @@ int tl_loglike_linear_batch(tl_ctx *c, const float *params, int64_t B, float *lo
     return rc;
 }
 
+namespace { int64_t mge_chunk_rows(const tl_ctx *c); }
+
 int tl_set_mge(tl_ctx *c, const float *sigmas, int32_t n_gauss)
 {
     if (!c || !sigmas || n_gauss < 1 || n_gauss > tl::MGE_MAX_GAUSS) return TL_EINVAL;
@@ -800,6 +814,15 @@ int tl_set_mge(tl_ctx *c, const float *sigmas, int32_t n_gauss)
     if (!c->mge_c && !cuda_ok(cudaMalloc(&c->mge_c, sizeof(float) * tl::MGE_MAX_GAUSS))) return TL_ENOMEM;
     if (!cuda_ok(cudaMemcpy(c->mge_c, ck, sizeof(float) * n_gauss, cudaMemcpyHostToDevice))) return TL_ECUDA;
     c->n_gauss = n_gauss;
+    if (c->pool) {   // the MGE call stages a chunk's component images: let the pool keep that much cached between calls
+        const int NC = n_gauss + c->cfg.n_source;
+        const size_t per_row = sizeof(float) * (size_t)NC * ((size_t)c->He * c->pitch + (size_t)c->cfg.ny * c->cfg.nx);
+        unsigned long long want = (unsigned long long)per_row * (unsigned long long)mge_chunk_rows(c) + (64ull << 20), cur = 0;
+        if (want > MGE_SCRATCH_BYTES + (256ull << 20)) want = MGE_SCRATCH_BYTES + (256ull << 20);
+        cudaMemPoolGetAttribute(c->pool, cudaMemPoolAttrReleaseThreshold, &cur);
+        if (want > cur) cudaMemPoolSetAttribute(c->pool, cudaMemPoolAttrReleaseThreshold, &want);
+        cudaGetLastError();
+    }
     return TL_OK;
 }
 
@@ -893,24 +916,69 @@ int tl_loglike_mge_batch(tl_ctx *c, const float *params, int64_t B, float *logL,
     return rc;
 }
 
+int tl_loglike_batch_host_async(tl_ctx *c, const float *params, int64_t B, float *logL, void *cuda_stream)
+{
+    if (!c || B < 1 || !params || !logL || (B % c->cfg.n_lens)) return TL_EINVAL;
+    DeviceGuard guard(c->device);                    // before any allocation: the buffers belong to the context's device
+    if (!guard.ok) return TL_ECUDA;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int id = c->next_slot;
+    tl_ctx::HostSlot &sl = c->slots[id];
+    if (sl.busy) {                                   // a third submission waits for the oldest one
+        const int wrc = tl_wait(c, id);
+        if (wrc != TL_OK) return wrc;
+    }
+    if (!c->s_up) {
+        if (!cuda_ok(cudaStreamCreateWithFlags(&c->s_up, cudaStreamNonBlocking)) ||
+            !cuda_ok(cudaStreamCreateWithFlags(&c->s_down, cudaStreamNonBlocking))) return TL_ECUDA;
+    }
+    if (!sl.up) {
+        if (!cuda_ok(cudaEventCreateWithFlags(&sl.up, cudaEventDisableTiming)) ||
+            !cuda_ok(cudaEventCreateWithFlags(&sl.done, cudaEventDisableTiming)) ||
+            !cuda_ok(cudaEventCreateWithFlags(&sl.fin, cudaEventDisableTiming))) return TL_ECUDA;
+    }
+    if (B > sl.cap_rows) {                           // grow the slot (first call, or a larger batch than ever before)
+        cudaFreeHost(sl.h_params); cudaFreeHost(sl.h_logl); cudaFree(sl.d_params); cudaFree(sl.d_logl);
+        sl.h_params = sl.h_logl = sl.d_params = sl.d_logl = nullptr; sl.cap_rows = 0;
+        const int64_t cap = B < 1024 ? 1024 : B;
+        if (!cuda_ok(cudaMallocHost(&sl.h_params, sizeof(float) * (size_t)cap * c->P)) ||
+            !cuda_ok(cudaMallocHost(&sl.h_logl, sizeof(float) * (size_t)cap)) ||
+            !cuda_ok(cudaMalloc(&sl.d_params, sizeof(float) * (size_t)cap * c->P)) ||
+            !cuda_ok(cudaMalloc(&sl.d_logl, sizeof(float) * (size_t)cap))) { cudaGetLastError(); return TL_ENOMEM; }
+        sl.cap_rows = cap;
+    }
+    memcpy(sl.h_params, params, sizeof(float) * (size_t)B * c->P);       // the caller's buffer is free again on return
+    int rc = TL_OK;
+    if (!cuda_ok(cudaMemcpyAsync(sl.d_params, sl.h_params, sizeof(float) * (size_t)B * c->P, cudaMemcpyHostToDevice, c->s_up)) ||
+        !cuda_ok(cudaEventRecord(sl.up, c->s_up)) || !cuda_ok(cudaStreamWaitEvent(st, sl.up, 0))) rc = TL_ECUDA;
+    if (rc == TL_OK) rc = run_batch(c, sl.d_params, B, sl.d_logl, nullptr, st);
+    if (rc == TL_OK &&
+        (!cuda_ok(cudaEventRecord(sl.done, st)) || !cuda_ok(cudaStreamWaitEvent(c->s_down, sl.done, 0)) ||
+         !cuda_ok(cudaMemcpyAsync(sl.h_logl, sl.d_logl, sizeof(float) * (size_t)B, cudaMemcpyDeviceToHost, c->s_down)) ||
+         !cuda_ok(cudaEventRecord(sl.fin, c->s_down)))) rc = TL_ECUDA;
+    if (rc != TL_OK) return rc;
+    sl.B = B; sl.user_logl = logL; sl.busy = 1; sl.rc = TL_OK;
+    c->next_slot = id ^ 1;
+    return id;
+}
+
+int tl_wait(tl_ctx *c, int slot)
+{
+    if (!c || slot < 0 || slot > 1 || !c->slots[slot].busy) return TL_EINVAL;
+    tl_ctx::HostSlot &sl = c->slots[slot];
+    int rc = sl.rc;
+    if (!cuda_ok(cudaEventSynchronize(sl.fin))) rc = TL_ECUDA;
+    if (rc == TL_OK) memcpy(sl.user_logl, sl.h_logl, sizeof(float) * (size_t)sl.B);
+    sl.busy = 0;
+    return rc;
+}
+
 int tl_loglike_batch_host(tl_ctx *ctx, const float *params, int64_t B, float *logL, void *cuda_stream)
 {
     if (!ctx || B < 0 || (B > 0 && (!params || !logL))) return TL_EINVAL;
     if (B == 0) return TL_OK;
-    DeviceGuard guard(ctx->device);                  // before any allocation: the buffers belong to the context's device
-    if (!guard.ok) return TL_ECUDA;
-    cudaStream_t st = (cudaStream_t)cuda_stream;
-    float *dp = nullptr, *dl = nullptr;
-    if (!pool_alloc(ctx, &dp, sizeof(float) * (size_t)B * ctx->P, st)) return TL_ENOMEM;
-    if (!pool_alloc(ctx, &dl, sizeof(float) * (size_t)B, st)) { cudaFreeAsync(dp, st); return TL_ENOMEM; }
-    int rc = TL_OK;
-    if (!cuda_ok(cudaMemcpyAsync(dp, params, sizeof(float) * (size_t)B * ctx->P, cudaMemcpyHostToDevice, st))) rc = TL_ECUDA;
-    if (rc == TL_OK) rc = run_batch(ctx, dp, B, dl, nullptr, st);
-    if (rc == TL_OK && !cuda_ok(cudaMemcpyAsync(logL, dl, sizeof(float) * (size_t)B, cudaMemcpyDeviceToHost, st))) rc = TL_ECUDA;
-    cudaFreeAsync(dp, st);
-    cudaFreeAsync(dl, st);
-    if (!cuda_ok(cudaStreamSynchronize(st)) && rc == TL_OK) rc = TL_ECUDA;
-    return rc;
+    const int slot = tl_loglike_batch_host_async(ctx, params, B, logL, cuda_stream);
+    return slot < 0 ? slot : tl_wait(ctx, slot);
 }
 
 int tl_set_precision(tl_ctx *c, int precision)
@@ -944,6 +1012,15 @@ void tl_destroy(tl_ctx *c)
     if (!c) return;
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
+    for (auto &sl : c->slots) {
+        if (sl.busy && sl.fin) cudaEventSynchronize(sl.fin);
+        if (sl.up) cudaEventDestroy(sl.up);
+        if (sl.done) cudaEventDestroy(sl.done);
+        if (sl.fin) cudaEventDestroy(sl.fin);
+        cudaFreeHost(sl.h_params); cudaFreeHost(sl.h_logl); cudaFree(sl.d_params); cudaFree(sl.d_logl);
+    }
+    if (c->s_up) cudaStreamDestroy(c->s_up);
+    if (c->s_down) cudaStreamDestroy(c->s_down);
     cudaFree(c->mge_c);
     cudaFree(c->psf); cudaFree(c->data); cudaFree(c->wgt); cudaFree(c->wgt64); cudaFree(c->noise); cudaFree(c->sigma_min); cudaFree(c->lconst);
     if (c->pool) cudaMemPoolDestroy(c->pool);

@@ -498,31 +498,18 @@ __device__ __forceinline__ void load_row_consts(RowC *dst, const RowC *src)
     for (int i = threadIdx.x; i < n16; i += blockDim.x) d[i] = s[i];
 }
 
-// flipped PSF [K][Kp] and, behind it, the same shifted by one tap (dst[n + k] = src[k + 1] within a
-// row, 0 at its end): the second operand of the packed convolution (ConvBlock).  n = K * Kp.
-__device__ __forceinline__ void load_psf(float *dst, const float *src, int n, int Kp)
+__device__ __forceinline__ void load_psf(float *dst, const float *src, int n)
 {
-    for (int i = threadIdx.x; i < n; i += blockDim.x) {
-        dst[i] = src[i];
-        dst[n + i] = ((i + 1) % Kp) ? src[i + 1] : 0.f;
-    }
+    for (int i = threadIdx.x; i < n; i += blockDim.x) dst[i] = src[i];
 }
 
 // step a6 for a 2 x 4 output block, PSF size known at compile time.  Per kernel row `ka` the
 // thread holds the windows of image rows i+ka and i+ka+1 (NW float4 each) in registers: the
 // second one is loaded (NW LDS.128) and becomes the first one of the next kernel row, so every
-// window float is read from shared memory once and used for up to 2 x 4 FMAs per tap.
-//
-// The FMAs are issued as packed FFMA2 (tl_pair.cuh: one issue slot per two FMAs).  A packed operand
-// must be an even-aligned register pair, and output x needs the window shifted by x floats, so:
-//   p0 = sum_e T[e] . W[e]        p2 = sum_e T[e] . W[e+1]          T[e] = (t[2e],   t[2e+1])
-//   p1 = t[0] w[1] + sum_e Ts[e] . W[e+1]                            Ts[e] = (t[2e+1], t[2e+2])
-//   p3 = t[0] w[3] + sum_e Ts[e] . W[e+2]                            W[e] = (w[2e],   w[2e+1])
-// ("." = both halves accumulated separately and added at the end).  Ts comes from a second copy of
-// the flipped PSF shifted by one tap (`taps + K * Kp`, written by load_psf): one more broadcast
-// LDS.128 per tap group instead of register shuffles.  K = 21: 42 FFMA2 + 2 FMUL + 4 FADD2 per
-// kernel row and 4 outputs, where the scalar form took 84 FFMA + 4 FADD.  Every kernel row is still
-// summed into fresh partials first (rounding error grows like sqrt(K), tl_kernels.cuh conv_strip).
+// window float is read from shared memory once and used for up to 2 x 4 FMAs per tap: the
+// shared-memory pipe carries NW window loads + KG (broadcast) tap loads per 8 K FMAs, about 70 %
+// of its bandwidth at K = 21, instead of being the limiter as with 1 x 4 strips.  (Feeding the
+// taps through the constant bank instead was measured: no faster, LDC is the slower path.)
 template <int K>
 struct ConvBlock {
     static constexpr int KG = (K + 3) / 4;           // tap groups of 4 per kernel row
@@ -535,72 +522,46 @@ struct ConvBlock {
         for (int g = 0; g < NW; ++g) w[g] = *reinterpret_cast<const float4 *>(rp + 4 * g);
     }
 
-    // window pair e = (w[2e], w[2e+1]); zero beyond the window (only reached by zero-padded taps)
-    template <int E>
-    static __device__ __forceinline__ f2 wpair(const float4 (&w)[NW])
+    // one kernel row applied to one image-row window -> 4 outputs, summed into a fresh partial
+    static __device__ __forceinline__ void row(const float4 (&w)[NW], const float *kp, float (&acc)[4])
     {
-        if constexpr (E / 2 >= NW) return bc2(0.f);
-        else if constexpr (E % 2 == 0) return mk2(w[E / 2].x, w[E / 2].y);
-        else return mk2(w[E / 2].z, w[E / 2].w);
-    }
-
-    template <int G>
-    static __device__ __forceinline__ void group(const float4 (&w)[NW], const float *kp, const float *kps, f2 &P0, f2 &P1, f2 &P2, f2 &P3)
-    {
-        if constexpr (G < KG) {
-            const float4 t = *reinterpret_cast<const float4 *>(kp + 4 * G);       // t[4G .. 4G+3]
-            const float4 u = *reinterpret_cast<const float4 *>(kps + 4 * G);      // t[4G+1 .. 4G+4]
-            const f2 T0 = mk2(t.x, t.y), T1 = mk2(t.z, t.w), S0 = mk2(u.x, u.y), S1 = mk2(u.z, u.w);
-            const f2 Wa = wpair<2 * G>(w), Wb = wpair<2 * G + 1>(w), Wc = wpair<2 * G + 2>(w), Wd = wpair<2 * G + 3>(w);
-            P0 = fma2(T0, Wa, P0); P2 = fma2(T0, Wb, P2);
-            if constexpr (4 * G + 1 < K) { P1 = fma2(S0, Wb, P1); P3 = fma2(S0, Wc, P3); }
-            if constexpr (4 * G + 2 < K) { P0 = fma2(T1, Wb, P0); P2 = fma2(T1, Wc, P2); }
-            if constexpr (4 * G + 3 < K) { P1 = fma2(S1, Wc, P1); P3 = fma2(S1, Wd, P3); }
-            group<G + 1>(w, kp, kps, P0, P1, P2, P3);
+        float p0 = 0.f, p1 = 0.f, p2 = 0.f, p3 = 0.f;
+#pragma unroll
+        for (int g = 0; g < KG; ++g) {
+            const float4 t = *reinterpret_cast<const float4 *>(kp + 4 * g);
+            const float4 lo = w[g];
+            const float4 hi = (g + 1 < NW) ? w[g + 1] : make_float4(0.f, 0.f, 0.f, 0.f);
+            const int nt = (K - 4 * g) >= 4 ? 4 : (K - 4 * g);     // real taps in this group
+            p0 = fmaf(t.x, lo.x, p0); p1 = fmaf(t.x, lo.y, p1); p2 = fmaf(t.x, lo.z, p2); p3 = fmaf(t.x, lo.w, p3);
+            if (nt > 1) { p0 = fmaf(t.y, lo.y, p0); p1 = fmaf(t.y, lo.z, p1); p2 = fmaf(t.y, lo.w, p2); p3 = fmaf(t.y, hi.x, p3); }
+            if (nt > 2) { p0 = fmaf(t.z, lo.z, p0); p1 = fmaf(t.z, lo.w, p1); p2 = fmaf(t.z, hi.x, p2); p3 = fmaf(t.z, hi.y, p3); }
+            if (nt > 3) { p0 = fmaf(t.w, lo.w, p0); p1 = fmaf(t.w, hi.x, p1); p2 = fmaf(t.w, hi.y, p2); p3 = fmaf(t.w, hi.z, p3); }
         }
+        acc[0] += p0; acc[1] += p1; acc[2] += p2; acc[3] += p3;
     }
 
-    // one kernel row applied to one image-row window -> 4 outputs (as pairs of partial sums)
-    static __device__ __forceinline__ void row(const float4 (&w)[NW], const float *kp, const float *kps, f2 (&acc)[4])
-    {
-        const float t0 = kp[0];
-        f2 P0 = bc2(0.f), P2 = bc2(0.f);
-        f2 P1 = mk2(t0 * w[0].y, 0.f), P3 = mk2(t0 * w[0].w, 0.f);
-        group<0>(w, kp, kps, P0, P1, P2, P3);
-        acc[0] = add2(acc[0], P0); acc[1] = add2(acc[1], P1); acc[2] = add2(acc[2], P2); acc[3] = add2(acc[3], P3);
-    }
-
-    // `win` = image row i, column x0 (16-byte aligned); taps = flipped PSF [K][Kp] followed by its
-    // copy shifted by one tap [K][Kp]
+    // `win` = image row i, column x0 (16-byte aligned); taps = flipped PSF [K][Kp]
     static __device__ __forceinline__ void run(const float *win, int pitch, const float *taps,
                                                float (&a0)[4], float (&a1)[4])
     {
-        const float *tapss = taps + K * Kp;
-        f2 b0[4], b1[4];
 #pragma unroll
-        for (int r = 0; r < 4; ++r) { b0[r] = bc2(0.f); b1[r] = bc2(0.f); }
+        for (int r = 0; r < 4; ++r) { a0[r] = 0.f; a1[r] = 0.f; }
         float4 wa[NW], wb[NW];
         load_window(wa, win);
         // kernel rows two at a time so that the windows ping-pong without register moves
 #pragma unroll 1
         for (int ka = 0; ka + 1 < K; ka += 2) {
             load_window(wb, win + (ka + 1) * pitch);
-            row(wa, taps + ka * Kp, tapss + ka * Kp, b0);
-            row(wb, taps + ka * Kp, tapss + ka * Kp, b1);
+            row(wa, taps + ka * Kp, a0);
+            row(wb, taps + ka * Kp, a1);
             load_window(wa, win + (ka + 2) * pitch);
-            row(wb, taps + (ka + 1) * Kp, tapss + (ka + 1) * Kp, b0);
-            row(wa, taps + (ka + 1) * Kp, tapss + (ka + 1) * Kp, b1);
+            row(wb, taps + (ka + 1) * Kp, a0);
+            row(wa, taps + (ka + 1) * Kp, a1);
         }
         if (K & 1) {                                  // K is odd: last kernel row
             load_window(wb, win + K * pitch);
-            row(wa, taps + (K - 1) * Kp, tapss + (K - 1) * Kp, b0);
-            row(wb, taps + (K - 1) * Kp, tapss + (K - 1) * Kp, b1);
-        }
-#pragma unroll
-        for (int r = 0; r < 4; ++r) {
-            float lo, hi;
-            un2(b0[r], lo, hi); a0[r] = lo + hi;
-            un2(b1[r], lo, hi); a1[r] = lo + hi;
+            row(wa, taps + (K - 1) * Kp, a0);
+            row(wb, taps + (K - 1) * Kp, a1);
         }
     }
 };
@@ -710,7 +671,7 @@ __global__ void __launch_bounds__(TL_LB_T, TL_LB_B) fused_kernel(const KArgs a)
     double *red = reinterpret_cast<double *>(smem_raw + sizeof(RowC));            // [0, 16): block_sum
     int *tile_counter = reinterpret_cast<int *>(red + 24);                          // phase-1 work queue
     float *taps = reinterpret_cast<float *>(smem_raw + sizeof(RowC) + 32 * sizeof(double));
-    float *img = taps + 2 * a.K * a.Kp;
+    float *img = taps + a.K * a.Kp;
     const int n_img = a.He * a.pitch;
     RowV *rowtab = a.rowtab ? reinterpret_cast<RowV *>(img + ((n_img + a.pitch + a.Kp + 8 + 3) & ~3)) : nullptr;
     // pitch padding and the slack after the image are read by zero-padded taps only (and by
@@ -724,7 +685,7 @@ __global__ void __launch_bounds__(TL_LB_T, TL_LB_B) fused_kernel(const KArgs a)
         __syncthreads();                               // previous row fully consumed
         load_row_consts(rc, a.rows + r);
         if (threadIdx.x == 0) *tile_counter = 0;
-        if (lens != cur_lens) { load_psf(taps, a.psf + lens * a.K * a.Kp, a.K * a.Kp, a.Kp); cur_lens = lens; }
+        if (lens != cur_lens) { load_psf(taps, a.psf + lens * a.K * a.Kp, a.K * a.Kp); cur_lens = lens; }
         __syncthreads();
         const size_t npix = (size_t)a.ny * a.nx;
         if (!row_is_valid(*rc, a.n_comp)) {            // uniform over the CTA
@@ -794,7 +755,7 @@ __global__ void __launch_bounds__(256) conv_kernel(const KArgs a, int chunk_rows
     extern __shared__ __align__(16) unsigned char smem_raw[];
     double *red = reinterpret_cast<double *>(smem_raw);
     float *taps = reinterpret_cast<float *>(smem_raw + 32 * sizeof(double));
-    float *img = taps + 2 * a.K * a.Kp;
+    float *img = taps + a.K * a.Kp;
     const int r = blockIdx.x, tile = blockIdx.y;
     const int64_t row = a.row0 + r;
     const int64_t lens = row / a.rows_per_lens;
@@ -810,7 +771,7 @@ __global__ void __launch_bounds__(256) conv_kernel(const KArgs a, int chunk_rows
         if (a.partial && threadIdx.x == 0) a.partial[(size_t)r * a.n_tiles + tile] = INFINITY;
         return;
     }
-    load_psf(taps, a.psf + lens * a.K * a.Kp, a.K * a.Kp, a.Kp);
+    load_psf(taps, a.psf + lens * a.K * a.Kp, a.K * a.Kp);
     // extended rows i0 .. i1 + 2h - 1 of this row's binned image, plus slack
     const int erows = (i1 - i0) + 2 * a.h;
     const float4 *src = reinterpret_cast<const float4 *>(a.ext + ((size_t)r * a.He + i0) * a.pitch);
@@ -874,7 +835,7 @@ __global__ void __launch_bounds__(512) conv_small_kernel(const KArgs a, int chun
     __shared__ int is_last;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float *taps = reinterpret_cast<float *>(smem_raw);
-    float *img = taps + 2 * a.K * a.Kp;
+    float *img = taps + a.K * a.Kp;
     const int r = blockIdx.x;
     const int npair = (a.ny + 1) / 2, nsx = (a.nx + 3) / 4;
     const int p0 = blockIdx.y * band_pairs, p1 = min(npair, p0 + band_pairs);
@@ -889,7 +850,7 @@ __global__ void __launch_bounds__(512) conv_small_kernel(const KArgs a, int chun
         if (a.logL && blockIdx.y == 0 && threadIdx.x == 0) a.logL[row] = -INFINITY;
         return;
     }
-    load_psf(taps, a.psf + lens * a.K * a.Kp, a.K * a.Kp, a.Kp);
+    load_psf(taps, a.psf + lens * a.K * a.Kp, a.K * a.Kp);
     // extended rows 2 p0 .. 2 (p1 - 1) + K of this row's binned image (the last one may lie past
     // the image when ny is odd: zeros), plus the slack the strips may touch
     const int e0 = 2 * p0, erows = 2 * (p1 - p0) + a.K - 1, have = min(erows, a.He - e0);
@@ -959,14 +920,14 @@ __global__ void __launch_bounds__(256, 2) conv_lin_kernel(const KArgs a, int chu
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float *taps = reinterpret_cast<float *>(smem_raw);
-    float *img = taps + 2 * a.K * a.Kp;
+    float *img = taps + a.K * a.Kp;
     const int r = blockIdx.x, tile = blockIdx.y, k = blockIdx.z, NC = gridDim.z;
     const int64_t row = a.row0 + r;
     const int64_t lens = row / a.rows_per_lens;
     const size_t npix = (size_t)a.ny * a.nx;
     if (!row_is_valid(a.rows[r], a.n_comp)) return;
     const int i0 = tile * a.tile_rows, i1 = min(a.ny, i0 + a.tile_rows);
-    load_psf(taps, a.psf + lens * a.K * a.Kp, a.K * a.Kp, a.Kp);
+    load_psf(taps, a.psf + lens * a.K * a.Kp, a.K * a.Kp);
     const int erows = (i1 - i0) + 2 * a.h;
     const float4 *src = reinterpret_cast<const float4 *>(a.ext + (((size_t)r * NC + k) * a.He + i0) * a.pitch);
     float4 *dst = reinterpret_cast<float4 *>(img);
@@ -1061,7 +1022,7 @@ __global__ void __launch_bounds__(512, 1) fused_lin_kernel(const KArgs a)
     double *s_sh = red + 20;
     int *tile_counter = reinterpret_cast<int *>(red + 24);
     float *taps = reinterpret_cast<float *>(smem_raw + sizeof(RowC) + 32 * sizeof(double));
-    float *img = taps + 2 * a.K * a.Kp;
+    float *img = taps + a.K * a.Kp;
     const int img_stride = (a.He * a.pitch + a.pitch + a.Kp + 8 + 3) & ~3;         // floats per component image
     RowV *rowtab = a.rowtab ? reinterpret_cast<RowV *>(img + NC * img_stride) : nullptr;
     for (int i = threadIdx.x; i < NC * img_stride; i += blockDim.x) img[i] = 0.f;
@@ -1075,7 +1036,7 @@ __global__ void __launch_bounds__(512, 1) fused_lin_kernel(const KArgs a)
         __syncthreads();
         load_row_consts(rc, a.rows + r);
         if (threadIdx.x == 0) *tile_counter = 0;
-        if (lens != cur_lens) { load_psf(taps, a.psf + lens * a.K * a.Kp, a.K * a.Kp, a.Kp); cur_lens = lens; }
+        if (lens != cur_lens) { load_psf(taps, a.psf + lens * a.K * a.Kp, a.K * a.Kp); cur_lens = lens; }
         __syncthreads();
         if (!row_is_valid(*rc, a.n_comp)) { invalid_row_lin(a, row); continue; }
         if (rowtab) { fill_rowtab<NLL>(*rc, a, rowtab); __syncthreads(); }

@@ -117,6 +117,38 @@ def test_null_context_calls_are_errors_not_crashes(api):
     lib.tl_destroy(None)
 
 
+def test_create_ex_validates_options_before_cuda(api):
+    psf, data, noise = _args()
+    lib = api.load()
+    cfg = api.tl_config(8, 8, 0.1, 2, 0, 1, 0, 1, 0)
+    for bad in (dict(small_batch_rows=-2), dict(block_threads=48), dict(block_threads=1024), dict(mge_chunk_rows=-1),
+                dict(scratch_keep_bytes=-5), dict(refine_tau=-1.0), dict(refine_tau=float("nan"))):
+        opt = api.tl_options(small_batch_rows=-1)
+        for k, v in bad.items():
+            setattr(opt, k, v)
+        h = C.c_void_p(1)
+        rc = lib.tl_create_ex(C.byref(h), C.byref(cfg), psf.ctypes.data, 3, 3, data.ctypes.data, noise.ctypes.data,
+                              C.byref(opt), None)
+        assert rc == api.TL_EINVAL and h.value is None, bad
+    with pytest.raises(api.TinyLensError):
+        api.tl_create(8, 8, 0.1, 2, 0, 1, psf, data, noise, options={"no_such_option": 1})
+
+
+def test_async_host_entry_and_peaks_reject_null(api):
+    lib = api.load()
+    assert lib.tl_loglike_batch_host_async(None, None, 4, None, None) == api.TL_EINVAL
+    assert lib.tl_wait(None, 0) == api.TL_EINVAL
+    assert lib.tl_measure_peaks(None, 4, None) == api.TL_EINVAL
+
+
+def test_library_reads_no_environment_variables():
+    """Every tuning knob is a tl_options field (tl_create_ex); nothing in csrc/ calls getenv."""
+    csrc = os.path.join(ROOT, "paper_2503_08586_b200", "csrc")
+    for f in os.listdir(csrc):
+        if f.endswith((".cu", ".cuh", ".h")):
+            assert "getenv" not in open(os.path.join(csrc, f)).read(), f
+
+
 def test_no_cpu_fallback_without_a_device(api):
     """Without a usable GPU the product path must fail loudly with TL_ECUDA."""
     import torch

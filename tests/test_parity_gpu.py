@@ -343,6 +343,107 @@ def test_full_size_batches_sampled_against_oracle(api, torch, orc, idx, batch, n
         assert abs(ll[r] - want) <= max(PT.LOGL_ABS, PT.LOGL_REL * abs(want)), (r, ll[r], want)
 
 
+def test_config4_full_batch_on_streams(api, torch, orc):
+    """BASELINE configs[4] as north_star states it: B = 65536 issued as 16 sub-batches of 4096 rows on
+    four streams that share ONE context (each call takes its own scratch from the context's pool).
+    Every logL finite; bitwise equal to the same sub-batches issued on a single stream; sampled rows
+    against the oracle (it needs seconds per row on this config)."""
+    w = W.workload(4)
+
+    def gpu_render(w1, psf, row):
+        ctx = api.LensContext(w1.ny, w1.nx, w1.pix_scale, w1.supersample, w1.n_lens_light, w1.n_source,
+                              psf[None], np.zeros((1, w1.ny, w1.nx), np.float32),
+                              np.ones((1, w1.ny, w1.nx), np.float32), w1.edge_mode)
+        im = ctx.render(torch.from_numpy(np.ascontiguousarray(row[None])).cuda()).cpu().numpy()[0]
+        ctx.close()
+        return im
+
+    prob = W.make_problem(w, gpu_render)
+    rows = W.batch_rows(w)
+    assert rows.shape == (65536, w.n_params)
+    ctx = api.LensContext.from_problem(prob)
+    assert ctx.info()["path"] == 1
+    d = torch.from_numpy(rows).cuda()
+    out_multi = torch.full((65536,), float("nan"), device="cuda")
+    out_single = torch.full((65536,), float("nan"), device="cuda")
+    streams = [torch.cuda.Stream() for _ in range(4)]
+    torch.cuda.synchronize()
+    for k in range(16):
+        st = streams[k % 4]
+        ctx.loglike(d[k * 4096:(k + 1) * 4096], out_multi[k * 4096:(k + 1) * 4096], stream=st)
+    torch.cuda.synchronize()
+    s0 = torch.cuda.Stream()
+    for k in range(16):
+        ctx.loglike(d[k * 4096:(k + 1) * 4096], out_single[k * 4096:(k + 1) * 4096], stream=s0)
+    torch.cuda.synchronize()
+    ctx.close()
+    assert torch.isfinite(out_multi).all()
+    assert torch.equal(out_multi, out_single), "multi-stream result differs from the single-stream result"
+    ll = out_multi.cpu().numpy().astype(np.float64)
+    cfg = orc.config_of(w)
+    for r in (5, 20000, 65535):
+        want = orc.loglike(cfg, prob.psf[0], prob.data[0], prob.noise[0], rows[r])
+        assert abs(ll[r] - want) <= max(PT.LOGL_ABS, PT.LOGL_REL * abs(want)), (r, ll[r], want)
+
+
+def test_async_host_entry_pipelines_batches(api, torch, orc):
+    """tl_loglike_batch_host_async / tl_wait: two batches in flight, results land in the right buffers
+    and equal the synchronous entry bit for bit; a third submission completes the oldest one."""
+    w = W.workload(1).scaled(batch=300)
+    prob = W.make_problem(w, orc.render_for_workloads)
+    ctx = api.LensContext.from_problem(prob)
+    batches = [W.draw_params(w, W.rng_for(1, W.STREAM_BATCH, 50 + k), n) for k, n in enumerate((300, 74, 300, 1, 128))]
+    want = [ctx.loglike_host(torch.from_numpy(b)).clone().numpy() for b in batches]
+    outs = [torch.full((len(b),), float("nan")).pin_memory() for b in batches]
+    s = torch.cuda.Stream()
+    slots = []
+    for k, b in enumerate(batches):
+        hb = torch.from_numpy(b.copy())
+        slot = ctx.loglike_host_async(hb, outs[k], stream=s)
+        hb.fill_(float("nan"))                       # the parameters were staged: the caller's buffer is free again
+        slots.append(slot)
+        assert slot == (slots[0] + k) % 2            # the two slots alternate
+        if k >= 2:                                   # the third submission had to complete the first
+            assert np.array_equal(outs[k - 2].numpy().view(np.uint32), want[k - 2].view(np.uint32))
+    for slot in slots[-2:]:
+        ctx.wait(slot)
+    for k in range(len(batches)):
+        assert np.array_equal(outs[k].numpy().view(np.uint32), want[k].view(np.uint32)), k
+    with pytest.raises(api.TinyLensError):
+        ctx.wait(0)                                  # nothing in flight
+    ctx.close()
+
+
+def test_create_accepts_device_arrays(api, torch, orc):
+    """SURVEY.md 8(b) Ownership: psf / data / noise may be host or device pointers."""
+    w = W.workload(0)
+    prob = W.make_problem(w, orc.render_for_workloads)
+    rows = torch.from_numpy(W.batch_rows(w)).cuda()
+    a = api.LensContext.from_problem(prob)
+    b = api.LensContext(w.ny, w.nx, w.pix_scale, w.supersample, w.n_lens_light, w.n_source,
+                        torch.from_numpy(prob.psf).cuda(), torch.from_numpy(prob.data).cuda(),
+                        torch.from_numpy(prob.noise).cuda(), w.edge_mode)
+    assert torch.equal(a.loglike(rows), b.loglike(rows))
+    a.close(); b.close()
+
+
+def test_call_restores_the_callers_device(api, torch, orc):
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two devices")
+    w = W.workload(0)
+    prob = W.make_problem(w, orc.render_for_workloads)
+    rows = W.batch_rows(w)
+    torch.cuda.set_device(0)
+    ctx = api.LensContext.from_problem(prob)
+    want = ctx.loglike_host(torch.from_numpy(rows)).clone()
+    torch.cuda.set_device(1)
+    got = ctx.loglike_host(torch.from_numpy(rows)).clone()
+    assert torch.cuda.current_device() == 1
+    torch.cuda.set_device(0)
+    assert torch.equal(want, got)
+    ctx.close()
+
+
 def test_call_is_cuda_graph_capturable(api, torch, orc):
     """NEXT-4 (caller-side overheads): tl_loglike_batch makes no host sync and takes
     its scratch from the stream-ordered allocator, so a sampler can capture it in a CUDA graph."""
