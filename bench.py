@@ -48,9 +48,23 @@ OP_EPL_FP32, OP_EPL_FP32_PER_TERM, OP_EPL_MUFU = 38, 2, 3
 SM_FP32_LANES = 128          # thread-instruction issue slots per SM per clock (4 warps x 32), measured 122-128
 SM_MUFU_LANES = 16           # measured 15.96 (profiles/r1_mufu_accuracy.md)
 
-# dram bytes of the dominant kernel per launch from the committed `ncu --set full` capture
-# (profiles/): filled in by hand after each capture; None until one exists.
-NCU_DRAM_BYTES_PER_LAUNCH = 2363136       # profiles/r1_fused_kernel.md: dram__bytes_read.sum 2.363136 MB + 0 B written
+def ncu_dram_bytes(summary="r2_fused_kernel.md"):
+    """dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, parsed from the
+    committed `ncu --set full` summary under profiles/ (None when there is none)."""
+    import re
+    try:
+        txt = open(os.path.join(ROOT, "profiles", summary)).read()
+    except OSError:
+        return None
+    unit = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    tot, seen = 0.0, 0
+    for name in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+        m = re.search(r"`%s`\s*\|\s*([0-9.eE+-]+)\s*\|\s*(\w+)" % re.escape(name), txt)
+        if m and m.group(2) in unit:
+            tot += float(m.group(1)) * unit[m.group(2)]
+            seen += 1
+    return int(round(tot)) if seen == 2 else None
+
 
 
 def epl_mean_terms(rows: np.ndarray) -> float:
@@ -401,7 +415,8 @@ def run_ours(args, w: W.Workload):
         "roofline": {
             "bound": "alu", "kernel": "fused_kernel" if (info["path"] == 0 and B > info["small_batch_rows"]) else "trace_kernel",
             "achieved": achieved, "peak": peak, "unit": "Tinst/s", "frac": achieved / peak,
-            "traffic": NCU_DRAM_BYTES_PER_LAUNCH if (w.mass_model == W.MASS_SIE and w.index == 1) else None,
+            "traffic": ncu_dram_bytes() if (w.mass_model == W.MASS_SIE and w.index == 1 and args.precision == "fp32"
+                                            and args.rows == "prior") else None,
             "peak_source": "derived: %d SMs x %d issue slots/clk x %.0f MHz (MEASURED_PEAKS.json sm_max_mhz; "
                            "slots/clk measured, profiles/r1_mufu_accuracy.md)" % (info["n_sm"], SM_FP32_LANES, sm_max),
             "kernel_ms": k_ms, "kernel_rows": k_rows, "fp32_pipe_frac": fp32_frac, "mufu_pipe_frac": mufu_frac,
@@ -420,7 +435,7 @@ def run_ours(args, w: W.Workload):
         O.lib()
         n = args.ref_rows
         dt, used = oracle_time(w, prob, rows[:n])
-        line["cpu_baseline"] = {"value": n / dt, "unit": UNIT, "cores": used, "kind": "oracle",
+        line["cpu_baseline"] = {"value": n / dt, "unit": UNIT, "cores": used, "kind": "oracle", "per_core": n / dt / max(1, used),
                                 "sample": "first %d of the %d rows of the step, %.1f s" % (n, B, dt)}
     print(json.dumps(line))
     if use_dist:

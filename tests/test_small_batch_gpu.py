@@ -62,6 +62,33 @@ def test_small_batches_equal_the_fused_kernel_bitwise(api, w):
     small.close(); fused.close()
 
 
+def test_small_batch_handoff_stress(api):
+    """compute-sanitizer (racecheck) is closed on this GPU pool, so the cross-CTA hand-off of
+    conv_small_kernel (__threadfence + a finished-band counter per row; the row's last band reduces
+    the stored terms) and the per-row work-queue heads of trace_kernel are hammered instead: 300
+    calls of varying small sizes on two streams at once, every result bitwise equal to the fused kernel's."""
+    import torch
+    w = [c for c in CASES if c.name == "odd"][0]
+    prob = W.make_problem(w, _zero_render)
+    small, fused = _contexts(api, prob)
+    assert small.info()["small_batch_rows"] > 0
+    rows = W.batch_rows(w, 40)
+    d = torch.from_numpy(rows).cuda()
+    want = fused.loglike(d).clone()
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    torch.cuda.synchronize()
+    outs = []
+    for it in range(150):
+        n1, n2 = 1 + (it * 7) % 40, 1 + (it * 11) % 37
+        a = small.loglike(d[:n1], stream=s1)
+        b = small.loglike(d[40 - n2:], stream=s2)
+        outs.append((n1, n2, a, b))
+    torch.cuda.synchronize()
+    for n1, n2, a, b in outs:
+        assert torch.equal(a, want[:n1]) and torch.equal(b, want[40 - n2:]), (n1, n2)
+    small.close(); fused.close()
+
+
 def test_small_batch_latency(api):
     """A handful of rows must not cost a whole row-time of one SM (0.18 ms on configs[1])."""
     import torch
