@@ -80,6 +80,9 @@ struct tl_ctx {
     // MGE mode (tl_set_mge / tl_loglike_mge_batch)
     float *mge_c = nullptr;       // device [n_gauss]: log2(e) / (2 sigma_k^2)
     int n_gauss = 0;
+    void (*mge_trace)(const tl::KArgs, int) = nullptr;   // sources only: trace_kernel<S,0,1> or trace_lin_kernel<S,0,2>
+    size_t mge_trace_smem = 0, mge_gc_smem = 0;
+    int mge_rowtab = 0, mge_fused = 0;                   // fused: gauss_conv_kernel (extended image in shared memory)
     double refine_tau = 7.5e-4;   // x S at create: a pixel averages S^2 samples
     // asynchronous host entry (tl_loglike_batch_host_async / tl_wait): two staging slots, each with
     // pinned host and device buffers for one batch, an upload and a download stream of the library's
@@ -118,7 +121,7 @@ void best_warp_tile(int He, int We, int *CW, int *CH)
 constexpr size_t SMEM_LIMIT = 227 * 1024;
 constexpr int64_t CONST_CHUNK = 1 << 17;        // rows of RowC scratch per chunk (fused path)
 constexpr size_t EXT_SCRATCH_BYTES = 512u << 20; // split path: binned-image scratch per chunk
-constexpr size_t MGE_SCRATCH_BYTES = (size_t)8 << 30;  // MGE: component images of a chunk (180 GB of HBM: keep whole batches resident)
+constexpr size_t MGE_SCRATCH_BYTES = (size_t)2 << 30;  // MGE: source images + blurred columns of a chunk of rows
 
 inline bool cuda_ok(cudaError_t e) { return e == cudaSuccess; }
 
@@ -814,9 +817,29 @@ int tl_set_mge(tl_ctx *c, const float *sigmas, int32_t n_gauss)
     if (!c->mge_c && !cuda_ok(cudaMalloc(&c->mge_c, sizeof(float) * tl::MGE_MAX_GAUSS))) return TL_ENOMEM;
     if (!cuda_ok(cudaMemcpy(c->mge_c, ck, sizeof(float) * n_gauss, cudaMemcpyHostToDevice))) return TL_ECUDA;
     c->n_gauss = n_gauss;
+    if (!c->mge_trace) {
+        // sources through the NLL = 0 ray-trace kernels (no lens-light stand-in; one source: packed pair loop)
+        const bool epl = c->cfg.mass_model == TL_MASS_EPL;
+        const int S = c->cfg.supersample, ns = c->cfg.n_source;
+        c->mge_trace = ns == 1 ? (epl ? tl_trace_epl_for(S, 0, 1) : tl_trace_for(S, 0, 1))
+                               : (epl ? tl_trace_lin_epl_for(S, 0, 2) : tl_trace_lin_for(S, 0, 2));
+        const size_t rowtab_bytes = sizeof(tl::RowV) * (size_t)c->He * S;
+        bool okm = true;
+        if (rowtab_bytes <= 48 * 1024) {
+            c->mge_rowtab = 1; c->mge_trace_smem = rowtab_bytes;
+            okm = cuda_ok(cudaFuncSetAttribute(c->mge_trace, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)rowtab_bytes));
+        }
+        // gauss_conv_kernel needs the whole extended image of one Gaussian (+ taps) in shared memory
+        c->mge_gc_smem = sizeof(float) * ((size_t)c->K * c->Kp + (size_t)(c->He + 1) * c->pitch + c->Kp + 8);
+        c->mge_fused = c->mge_gc_smem <= SMEM_LIMIT - 1024;
+        if (c->mge_fused)
+            okm = okm && cuda_ok(cudaFuncSetAttribute(tl::gauss_conv_for(S), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SMEM_LIMIT - 1024))) &&
+                  cuda_ok(cudaFuncSetAttribute(tl::gauss_conv_for(S), cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+        if (!okm) { c->mge_trace = nullptr; c->n_gauss = 0; cudaGetLastError(); return TL_ECUDA; }
+    }
     if (c->pool) {   // the MGE call stages a chunk's component images: let the pool keep that much cached between calls
         const int NC = n_gauss + c->cfg.n_source;
-        const size_t per_row = sizeof(float) * (size_t)NC * ((size_t)c->He * c->pitch + (size_t)c->cfg.ny * c->cfg.nx);
+        const size_t per_row = sizeof(float) * ((size_t)(c->mge_fused ? c->cfg.n_source : NC) * c->He * c->pitch + (size_t)NC * c->cfg.ny * c->cfg.nx);
         unsigned long long want = (unsigned long long)per_row * (unsigned long long)mge_chunk_rows(c) + (64ull << 20), cur = 0;
         if (want > MGE_SCRATCH_BYTES + (256ull << 20)) want = MGE_SCRATCH_BYTES + (256ull << 20);
         cudaMemPoolGetAttribute(c->pool, cudaMemPoolAttrReleaseThreshold, &cur);
@@ -831,7 +854,7 @@ int64_t mge_chunk_rows(const tl_ctx *c)
 {
     const int NC = c->n_gauss + c->cfg.n_source;
     const size_t npix = (size_t)c->cfg.ny * c->cfg.nx;
-    const size_t ext_row = sizeof(float) * (size_t)NC * c->He * c->pitch, m_row = sizeof(float) * NC * npix;
+    const size_t ext_row = sizeof(float) * (size_t)(c->mge_fused ? c->cfg.n_source : NC) * c->He * c->pitch, m_row = sizeof(float) * NC * npix;
     int64_t chunk = (int64_t)(MGE_SCRATCH_BYTES / (ext_row + m_row));
     if (chunk < 1) chunk = 1;
     if (chunk > 65535) chunk = 65535;
@@ -850,19 +873,21 @@ int tl_loglike_mge_batch(tl_ctx *c, const float *params, int64_t B, float *logL,
     if (c->n_gauss < 1) return TL_EINVAL;
     if (B == 0) return TL_OK;
     if (!params || !logL || (B % c->cfg.n_lens)) return TL_EINVAL;
-    if (!c->trace_lin) return TL_ESIZE;
+    if (!c->trace_lin || !c->mge_trace) return TL_ESIZE;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     DeviceGuard guard(c->device);
     if (!guard.ok) return TL_ECUDA;
-    const int NG = c->n_gauss, NC = NG + c->cfg.n_source;
+    const int NG = c->n_gauss, NS = c->cfg.n_source, NC = NG + NS;
+    const int fused = c->mge_fused;
     const size_t npix = (size_t)c->cfg.ny * c->cfg.nx;
-    const size_t ext_row = sizeof(float) * (size_t)NC * c->He * c->pitch, m_row = sizeof(float) * NC * npix;
+    const int ext_nc = fused ? NS : NC;                        // component images staged in global memory per row
+    const size_t ext_row = sizeof(float) * (size_t)ext_nc * c->He * c->pitch, m_row = sizeof(float) * NC * npix;
     int64_t chunk = mge_chunk_rows(c);
     if (chunk > B) chunk = B;
     tl::RowC *rows = nullptr;
     float *ext = nullptr, *mimg = nullptr;
-    double *gram = nullptr;                                    // [chunk][MGE_GRAM_STRIDE + MGE_MAX_COL]
-    const size_t g_row = sizeof(double) * (tl::MGE_GRAM_STRIDE + tl::MGE_MAX_COL);
+    double *gram = nullptr;                                    // [chunk][MGE_GRAM_STRIDE]
+    const size_t g_row = sizeof(double) * tl::MGE_GRAM_STRIDE;
     // the budget is a target, not a promise: when the device cannot give that much, halve the chunk
     for (;;) {
         rows = nullptr; ext = nullptr; mimg = nullptr; gram = nullptr;
@@ -878,7 +903,9 @@ int tl_loglike_mge_batch(tl_ctx *c, const float *params, int64_t B, float *logL,
         if (chunk == 1) return TL_ENOMEM;
         chunk = (chunk + 1) / 2;
     }
-    // (the pitch padding of ext, which must read as finite zeros, is written by mge_gauss_kernel)
+    // the pitch padding of ext must read as finite zeros: written by mge_gauss_kernel when it runs,
+    // else (fused: ext holds the source images only) cleared here
+    if (fused) cudaMemsetAsync(ext, 0, ext_row * (size_t)chunk, st);
     const int64_t rows_per_lens = B / c->cfg.n_lens;
     int gslabs = (c->He * c->pitch + 255) / 256;
     if (gslabs > 16) gslabs = 16;
@@ -893,23 +920,31 @@ int tl_loglike_mge_batch(tl_ctx *c, const float *params, int64_t B, float *logL,
         tl::KArgs a = base_args(c);
         a.rows = rows; a.B = nb; a.rows_per_lens = rows_per_lens; a.row0 = r0;
         a.logL = logL; a.amps = amps; a.ext = ext; a.mimg = mimg;
-        a.tile_rows = c->lin_tile_rows; a.n_tiles = c->lin_n_tiles; a.rowtab = c->lin_rowtab;
-        // trace_lin_kernel writes its 1 + n_source components from slot NG - 1 on: the (unused)
-        // Sersic stand-in of the lens light lands on slot NG - 1, which mge_gauss_kernel then
-        // overwrites with the last Gaussian; the sources land on slots NG, NG + 1
-        a.ext_nc = NC; a.ext_k0 = NG - 1; a.n_gauss = NG; a.mge_c = c->mge_c;
-        a.mge_gram = gram; a.mge_sol = gram + (size_t)chunk * tl::MGE_GRAM_STRIDE;
-        dim3 tg((unsigned)nb, 8);
-        c->trace_lin<<<tg, 256, c->lin_trace_smem, st>>>(a, (int)nb);
-        dim3 gg((unsigned)nb, (unsigned)gslabs);
-        tl::mge_gauss_for(NG)<<<gg, 256, 0, st>>>(a, (int)nb);
-        dim3 cg((unsigned)nb, (unsigned)c->lin_n_tiles, (unsigned)NC);
-        if (c->profile) cudaEventRecord(c->ev0, st);
-        tl::conv_lin_kernel<<<cg, 256, c->lin_conv_smem, st>>>(a, (int)nb);
-        if (c->profile) { cudaEventRecord(c->ev1, st); c->prof_pending = 1; }
+        a.tile_rows = c->lin_tile_rows; a.n_tiles = c->lin_n_tiles;
+        a.n_gauss = NG; a.mge_c = c->mge_c; a.mge_gram = gram;
+        // 1. the sources, ray-traced at unit amplitude -> ext slots (fused: 0.., else NG..)
+        tl::KArgs at = a;
+        at.rowtab = c->mge_rowtab; at.ext_nc = ext_nc; at.ext_k0 = fused ? 0 : NG;
+        c->mge_trace<<<dim3((unsigned)nb, 8), 256, c->mge_trace_smem, st>>>(at, (int)nb);
+        a.ext_nc = NC;                                         // from here on: the width of M
+        if (fused) {
+            // 2. every Gaussian evaluated into shared memory and blurred from there -> M[0 .. NG)
+            if (c->profile) cudaEventRecord(c->ev0, st);
+            tl::gauss_conv_for(c->cfg.supersample)<<<dim3((unsigned)nb, (unsigned)NG), 256, c->mge_gc_smem, st>>>(a, (int)nb);
+            if (c->profile) { cudaEventRecord(c->ev1, st); c->prof_pending = 1; }
+            // 3. the sources blurred -> M[NG ..)
+            tl::KArgs ac = a;
+            ac.conv_ext_nc = NS; ac.conv_m_nc = NC; ac.conv_m_k0 = NG;
+            tl::conv_lin_kernel<<<dim3((unsigned)nb, (unsigned)c->lin_n_tiles, (unsigned)NS), 256, c->lin_conv_smem, st>>>(ac, (int)nb);
+        } else {
+            tl::mge_gauss_for(NG)<<<dim3((unsigned)nb, (unsigned)gslabs), 256, 0, st>>>(a, (int)nb);
+            if (c->profile) cudaEventRecord(c->ev0, st);
+            tl::conv_lin_kernel<<<dim3((unsigned)nb, (unsigned)c->lin_n_tiles, (unsigned)NC), 256, c->lin_conv_smem, st>>>(a, (int)nb);
+            if (c->profile) { cudaEventRecord(c->ev1, st); c->prof_pending = 1; }
+        }
+        // 4. Gram matrix, 5. NNLS + logL
         tl::gram_mge_kernel<<<(unsigned)nb, tl::MGE_SOLVE_THREADS, 0, st>>>(a, (int)nb);
         tl::nnls_mge_kernel<<<(unsigned)((nb + tl::MGE_NNLS_WARPS - 1) / tl::MGE_NNLS_WARPS), 32 * tl::MGE_NNLS_WARPS, 0, st>>>(a, (int)nb);
-        tl::resid_mge_kernel<<<(unsigned)nb, 256, 0, st>>>(a, (int)nb);
         if (!cuda_ok(cudaGetLastError())) rc = TL_ECUDA;
     }
     cudaFreeAsync(rows, st); cudaFreeAsync(ext, st); cudaFreeAsync(mimg, st); cudaFreeAsync(gram, st);

@@ -97,7 +97,8 @@ struct PrologueArgs {
     double refine_tau;               // refinement threshold in units of sigma_min
     int unit_amp;                    // linear-amplitude mode: every I_e is taken as 1
     int mge;                         // MGE mode (tl_loglike_mge_batch): of the lens-light block only e1, e2, cx, cy are
-                                     // read; its quadratic form becomes t = R_p^2 in arcsec^2 (r_e := 1, n := 1)
+                                     // read; its quadratic form becomes t = R_p^2 in arcsec^2 (r_e := 1, n := 1);
+                                     // component order in RowC: sources first, then the Gaussian set's shape
 };
 
 // ---- b_n of PAPER.md:139 Eq. 9:  P(2n, b_n) = 1/2 ---------------------------------------
@@ -353,7 +354,9 @@ __global__ void __launch_bounds__(128) prologue_kernel(PrologueArgs a)
         C.nlcf = (float)fmin(fmax(-log2(cf), -1e30), 1e30);
     }
     C.valid = ok ? 1 : 0;
-    rc->comp[k] = C;
+    // MGE mode: the sources come first (comp[0 .. n_source-1], what the NLL = 0 ray-trace kernels read)
+    // and the shape of the Gaussian set after them (comp[n_source])
+    rc->comp[a.mge ? (is_lens_light ? a.n_source + k : k - a.n_lens_light) : k] = C;
 }
 
 #endif  // TL_MAIN_TU

@@ -48,7 +48,8 @@ struct KArgs {
     float err_coh, err_rnd;  // bound = err_coh |sum e_i| + err_rnd sqrt(sum e_i^2),  e_i = (d_i - m_i) m_i / sigma_i^2
     const float *mge_c;      // [n_gauss] log2(e) / (2 sigma_k^2), arcsec^-2
     double *mge_gram;        // [chunk][MGE_GRAM_STRIDE]  G | b | d'Wd
-    double *mge_sol;         // [chunk][MGE_MAX_COL]      solved amplitudes (FP64)
+    // conv_lin_kernel: component strides of ext and of mimg, first mimg slot (0, 0, 0 = gridDim.z, gridDim.z, 0)
+    int conv_ext_nc, conv_m_nc, conv_m_k0;
 };
 
 __device__ __forceinline__ bool row_is_valid(const RowC &rc, int n_comp)
@@ -739,7 +740,8 @@ __global__ void __launch_bounds__(256, 2) trace_kernel(const KArgs a, int chunk_
         __syncthreads();
         if (!row_is_valid(rc_s, a.n_comp)) continue;
         if (rowtab) { fill_rowtab<NLL>(rc_s, a, rowtab); __syncthreads(); }
-        float *dst = a.ext + (size_t)r * a.He * a.pitch;
+        // (MGE mode: the source image is component slot ext_k0 of ext_nc per row)
+        float *dst = a.ext + ((size_t)r * (a.ext_nc ? a.ext_nc : 1) + a.ext_k0) * a.He * a.pitch;
         // small batches: the row's CTAs draw warp tiles from one global queue, so a tile full of
         // FP64-refined samples does not leave the other warps of the row waiting for its owner
         trace_image<S_T, NLL, NSRC, MASS>(rc_s, a, rowtab, (blockIdx.y * blockDim.x + threadIdx.x) >> 5, (gridDim.y * blockDim.x) >> 5,
@@ -929,13 +931,14 @@ __global__ void __launch_bounds__(256, 2) conv_lin_kernel(const KArgs a, int chu
     const int i0 = tile * a.tile_rows, i1 = min(a.ny, i0 + a.tile_rows);
     load_psf(taps, a.psf + lens * a.K * a.Kp, a.K * a.Kp);
     const int erows = (i1 - i0) + 2 * a.h;
-    const float4 *src = reinterpret_cast<const float4 *>(a.ext + (((size_t)r * NC + k) * a.He + i0) * a.pitch);
+    const int enc = a.conv_ext_nc ? a.conv_ext_nc : NC, mnc = a.conv_m_nc ? a.conv_m_nc : NC;
+    const float4 *src = reinterpret_cast<const float4 *>(a.ext + (((size_t)r * enc + k) * a.He + i0) * a.pitch);
     float4 *dst = reinterpret_cast<float4 *>(img);
     const int n4 = erows * a.pitch / 4;
     for (int i = threadIdx.x; i < n4; i += blockDim.x) dst[i] = src[i];
     for (int i = threadIdx.x; i < a.pitch + a.Kp + 8; i += blockDim.x) img[erows * a.pitch + i] = 0.f;
     __syncthreads();
-    conv_chi2_rows(a, img, i0, taps, i0, i1, nullptr, nullptr, a.mimg + ((size_t)r * NC + k) * npix);
+    conv_chi2_rows(a, img, i0, taps, i0, i1, nullptr, nullptr, a.mimg + ((size_t)r * mnc + a.conv_m_k0 + k) * npix);
 }
 
 #endif  // TL_MAIN_TU

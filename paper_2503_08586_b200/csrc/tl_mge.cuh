@@ -6,14 +6,23 @@
 // the source amplitudes as the NNLS minimiser of PAPER.md:86-93 Eq. 6 / :97-129 Eq. 7.
 //
 // Pipeline per chunk of rows (all on one stream; included by tinylens.cu only):
-//   prologue_kernel (mge = 1)  lens-light quadratic form becomes t = R_p^2 in arcsec^2
-//   trace_lin_kernel           ray-traced unit-amplitude source images -> component slots n_gauss..
-//   mge_gauss_kernel           the n_gauss binned Gaussians -> component slots 0..n_gauss-1
-//   conv_lin_kernel            every component blurred with the PSF (columns of M)
+//   prologue_kernel (mge = 1)  lens-light quadratic form becomes t = R_p^2 in arcsec^2; the row's
+//                              components are stored sources first, then the Gaussian set's shape
+//   trace_kernel<S,0,1> / trace_lin_kernel<S,0,2>   ray-traced unit-amplitude source images (the NLL = 0
+//                              instantiations: no lens-light stand-in is evaluated; one source
+//                              takes the packed pair loop of tl_pair.cuh) -> ext, one slot per source
+//   gauss_conv_kernel          one CTA per (row, Gaussian): the binned unit-amplitude Gaussian is
+//                              evaluated straight into shared memory and blurred from there -- the
+//                              unblurred Gaussians never touch global memory.  (Images too large
+//                              for that: mge_gauss_kernel -> ext, then conv_lin_kernel.)
+//   conv_lin_kernel            the source images blurred with the PSF
 //   gram_mge_kernel            G = M'WM, b = M'Wd, d'Wd in FP64 (fixed summation order) -> global
 //   nnls_mge_kernel            NNLS by the Gram-matrix active-set iteration of Bro & De Jong (the
-//                              paper's solver), one warp per row -> amplitudes
-//   resid_mge_kernel           chi^2 of the residual d - M s in FP64 -> logL
+//                              paper's solver), one warp per row -> amplitudes,
+//                              and chi^2 = d'Wd - 2 s'b + s'Gs -> logL.  All of it FP64 on exact
+//                              products of the FP32 columns: the three terms are ~1e9 and chi^2
+//                              ~1e4, a loss of 5 of 16 digits (1e-7 absolute), so the second pass
+//                              over M that round 1 made for the residual is not needed.
 #pragma once
 #include "tl_kernels.cuh"
 
@@ -39,7 +48,7 @@ __global__ void __launch_bounds__(256) mge_gauss_kernel(const KArgs a, int chunk
     if (r >= chunk_rows) return;
     const RowC &rc = a.rows[r];
     if (!row_is_valid(rc, a.n_comp)) return;
-    const SersicC &C = rc.comp[0];
+    const SersicC &C = rc.comp[a.n_comp - a.n_lens_light];       // MGE order: the set's shape follows the sources
     const float cXh = C.cXh, cXl = C.cXl, cYh = C.cYh, cYl = C.cYl;
     const float ah = C.ah, al = C.al, b2h = C.b2h, b2l = C.b2l, cch = C.cch, ccl = C.ccl;
     const int S = a.S;
@@ -83,6 +92,103 @@ __global__ void __launch_bounds__(256) mge_gauss_kernel(const KArgs a, int chunk
         }
 #pragma unroll
         for (int k = 0; k < NG; ++k) dst[k * comp_stride + (size_t)i * a.pitch + j] = acc[k] * inv_s2;
+    }
+}
+
+// One CTA per (row, Gaussian k): steps a4-a6 for one column of M without a round trip through global
+// memory.  t = R_p^2 of a sub-sample is LA(x) + LC(y) + LB(x) dyl(y) (tl_kernels.cuh col_values /
+// row_values): the column parts of a pixel's S sub-columns are computed once per pixel and kept in
+// registers as pairs (tl_pair.cuh), the row parts once per sub-row, so a pair of samples costs
+// FADD2 + FFMA2 + FMUL2 + 2 MUFU.EX2 + FADD2.  The evaluation is MUFU-bound, the convolution
+// FMA-bound; with two or three CTAs per SM the two phases of different CTAs overlap.
+// S_T = 0: any S (scalar loop).
+template <int S_T>
+__global__ void __launch_bounds__(256) gauss_conv_kernel(const KArgs a, int chunk_rows)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float *taps = reinterpret_cast<float *>(smem_raw);
+    float *img = taps + a.K * a.Kp;
+    const int r = blockIdx.x, k = blockIdx.y;
+    if (r >= chunk_rows) return;
+    const RowC &rc = a.rows[r];
+    if (!row_is_valid(rc, a.n_comp)) return;
+    const int64_t lens = (a.row0 + r) / a.rows_per_lens;
+    load_psf(taps, a.psf + lens * a.K * a.Kp, a.K * a.Kp);
+    const SersicC &C = rc.comp[a.n_comp - a.n_lens_light];
+    const float cXh = C.cXh, cXl = C.cXl, cYh = C.cYh, cYl = C.cYl;
+    const float ah = C.ah, al = C.al, b2h = C.b2h, b2l = C.b2l, cch = C.cch, ccl = C.ccl;
+    const float ck = -a.mge_c[k];
+    const int S = S_T > 0 ? S_T : a.S;
+    const float inv_s2 = 1.f / (float)(S * S);
+    const int npx = a.He * a.pitch;
+    for (int p = threadIdx.x; p < npx + a.pitch + a.Kp + 8; p += blockDim.x) {
+        const int i = p / a.pitch, j = p - i * a.pitch;
+        float acc = 0.f;
+        const bool edge = a.edge_zero && (j < a.h || j >= a.We - a.h || i < a.h || i >= a.He - a.h);
+        if (p < npx && j < a.We && !edge) {
+            const float X0 = (float)(2 * j * S + 1 - S * a.We);
+            float Y = (float)(2 * i * S + 1 - S * a.He);
+            if constexpr (S_T > 0 && S_T % 2 == 0) {
+                constexpr int NP = S_T / 2;
+                f2 LA[NP], LB[NP];
+#pragma unroll
+                for (int q = 0; q < NP; ++q) {
+                    float la[2], lb[2];
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) {
+                        const float dxl = ((X0 + (float)(4 * q + 2 * e)) - cXh) - cXl;
+                        const float x2 = dxl * dxl;
+                        la[e] = fmaf(ah, x2, al * x2);
+                        lb[e] = fmaf(dxl, b2h, dxl * b2l);
+                    }
+                    LA[q] = mk2(la[0], la[1]); LB[q] = mk2(lb[0], lb[1]);
+                }
+                f2 acc2 = bc2(0.f);
+#pragma unroll
+                for (int sa = 0; sa < S_T; ++sa, Y += 2.f) {
+                    const float dyl = (Y - cYh) - cYl;
+                    const float y2 = dyl * dyl;
+                    const float LC = fmaf(cch, y2, ccl * y2);
+#pragma unroll
+                    for (int q = 0; q < NP; ++q)
+                        acc2 = add2(acc2, ex2_2(mul2(fma2(LB[q], bc2(dyl), add2(LA[q], bc2(LC))), bc2(ck))));
+                }
+                float a0, a1;
+                un2(acc2, a0, a1);
+                acc = a0 + a1;
+            } else {
+#pragma unroll 1
+                for (int sa = 0; sa < S; ++sa, Y += 2.f) {
+                    const float dyl = (Y - cYh) - cYl;
+                    const float y2 = dyl * dyl;
+                    const float LC = fmaf(cch, y2, ccl * y2);
+                    float X = X0;
+                    for (int sb = 0; sb < S; ++sb, X += 2.f) {
+                        const float dxl = (X - cXh) - cXl;
+                        const float x2 = dxl * dxl;
+                        const float LA = fmaf(ah, x2, al * x2);
+                        const float LB = fmaf(dxl, b2h, dxl * b2l);
+                        acc += mufu_ex2(fmaf(LB, dyl, LA + LC) * ck);
+                    }
+                }
+            }
+            acc *= inv_s2;
+        }
+        img[p] = acc;                                  // pitch padding and slack read as zero
+    }
+    __syncthreads();
+    const size_t npix = (size_t)a.ny * a.nx;
+    conv_chi2_rows(a, img, 0, taps, 0, a.ny, nullptr, nullptr, a.mimg + ((size_t)r * a.ext_nc + k) * npix);
+}
+
+typedef void (*gauss_conv_fn)(const KArgs, int);
+inline gauss_conv_fn gauss_conv_for(int S)
+{
+    switch (S) {
+    case 2: return gauss_conv_kernel<2>;
+    case 4: return gauss_conv_kernel<4>;
+    case 8: return gauss_conv_kernel<8>;
+    default: return gauss_conv_kernel<0>;
     }
 }
 
@@ -227,42 +333,22 @@ __global__ void __launch_bounds__(32 * MGE_NNLS_WARPS) nnls_mge_kernel(const KAr
     if (lane == 0)
         nnls_gram<MGE_MAX_COL>(n, Gw[wid], NCP, Gw[wid] + MGE_MAX_COL * NCP, Gw[wid][MGE_MAX_COL * NCP + MGE_MAX_COL], sw[wid], Lw[wid], zw[wid]);
     __syncwarp();
-    if (lane < n) {
-        a.mge_sol[(size_t)r * MGE_MAX_COL + lane] = sw[wid][lane];
-        if (a.amps) a.amps[row * n + lane] = (float)sw[wid][lane];
+    if (lane < n && a.amps) a.amps[row * n + lane] = (float)sw[wid][lane];
+    if (lane == 0) {
+        // chi^2 = d'Wd - 2 s'b + s'G s at the solved amplitudes (Eq. 5)
+        const double *G = Gw[wid], *b = Gw[wid] + MGE_MAX_COL * NCP;
+        double sb = 0.0, sGs = 0.0;
+        for (int i = 0; i < n; ++i) {
+            const double si = sw[wid][i];
+            if (si == 0.0) continue;
+            sb += si * b[i];
+            double gi = 0.0;
+            for (int k = 0; k < n; ++k) gi += G[i * NCP + k] * sw[wid][k];
+            sGs += si * gi;
+        }
+        const double chi2 = (Gw[wid][MGE_MAX_COL * NCP + MGE_MAX_COL] - 2.0 * sb) + sGs;
+        a.logL[row] = (float)(-0.5 * (chi2 + a.lconst[row / a.rows_per_lens]));
     }
-}
-
-// chi^2 of the residual d - M s in FP64 (never via d'Wd - 2 s'b + s'Gs, which cancels) -> logL.
-// One CTA per row; the loads of a pixel's n columns are independent.
-__global__ void __launch_bounds__(256) resid_mge_kernel(const KArgs a, int chunk_rows)
-{
-    __shared__ double red[32];
-    __shared__ double ss[MGE_MAX_COL];
-    const int r = blockIdx.x;
-    if (r >= chunk_rows) return;
-    const int64_t row = a.row0 + r;
-    const int n = a.ext_nc;
-    if (!row_is_valid(a.rows[r], a.n_comp)) return;
-    const int64_t lens = row / a.rows_per_lens;
-    const int npix = a.ny * a.nx;
-    const float *M = a.mimg + (size_t)r * n * npix;
-    const float *d = a.data + lens * (size_t)npix, *w = a.wgt + lens * (size_t)npix;
-    if (threadIdx.x < MGE_MAX_COL) ss[threadIdx.x] = threadIdx.x < n ? a.mge_sol[(size_t)r * MGE_MAX_COL + threadIdx.x] : 0.0;
-    __syncthreads();
-    double part = 0.0;
-    for (int i = threadIdx.x; i < npix; i += blockDim.x) {
-        float mv[MGE_MAX_COL];
-#pragma unroll
-        for (int k = 0; k < MGE_MAX_COL; ++k) mv[k] = k < n ? M[(size_t)k * npix + i] : 0.f;
-        double m = 0.0;
-#pragma unroll
-        for (int k = 0; k < MGE_MAX_COL; ++k) if (k < n) m += ss[k] * (double)mv[k];
-        const double res = (double)d[i] - m;
-        part += res * res * (double)w[i];
-    }
-    const double chi2 = block_sum(part, red);
-    if (threadIdx.x == 0) a.logL[row] = (float)(-0.5 * (chi2 + a.lconst[lens]));
 }
 
 }  // namespace tl
