@@ -518,6 +518,8 @@ def run_linear(args, w: W.Workload):
 
     prob = W.make_problem(w, gpu_render)
     ctx = api.LensContext.from_problem(prob)
+    if args.precision != "fp32" and args.mode == "linear":
+        ctx.set_precision({"fp64": api.TL_PRECISION_FP64, "fp64-libm": api.TL_PRECISION_FP64_LIBM, "auto": api.TL_PRECISION_AUTO}[args.precision])
     rows = W.batch_rows(w)
     B = rows.shape[0]
     mge = args.mode == "mge"
@@ -544,7 +546,8 @@ def run_linear(args, w: W.Workload):
     value = B * args.steps / (total_ms * 1e-3)
     line = {"metric": METRIC + mass_tag(w) + " (linear amplitudes, NNLS per row)", "value": value, "unit": UNIT, "n_gpus": 1,
             "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps,
-            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32" if args.precision == "fp32" else "f64", "precision": args.precision, "data": "synthetic",
             "config": config_dict(w, "flushed between steps (256 MiB fill)"), "clocks": clk.summary(),
             "pixel_evals_per_s": value * w.ny * w.nx, "mode": "linear",
             "gpu_launches": args.steps * 2, "checksum_logL": float(out.double().sum())}

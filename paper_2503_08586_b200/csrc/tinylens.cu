@@ -241,18 +241,24 @@ int run_small_batch(tl_ctx *c, const float *params, int64_t B, float *logL, floa
 // n_rows_dev -- over the rows listed in device memory (AUTO mode: the count is not known on the
 // host, so every chunk is launched and the kernels of an empty chunk return at once).
 int run_dp(tl_ctx *c, const float *params, int64_t B, float *logL, float *images, cudaStream_t st,
-           const int *row_index, const int *n_rows_dev)
+           const int *row_index, const int *n_rows_dev, int lin = 0, float *amps = nullptr)
 {
     const int64_t rows_per_lens = B / c->cfg.n_lens;
-    const int64_t chunk = c->dp_chunk_rows < B ? c->dp_chunk_rows : B;
+    const int NCL = lin ? c->n_comp : 1;                         // component images kept apart (linear mode)
+    int64_t chunk = c->dp_chunk_rows / (lin ? 2 * NCL : 1);
+    if (chunk < 1) chunk = 1;
+    if (chunk > B) chunk = B;
     tl::RowD *rows = nullptr;
-    double *ext = nullptr, *partial = nullptr;
-    const size_t ext_row = sizeof(double) * (size_t)c->He * c->dp_Wp;
+    double *ext = nullptr, *partial = nullptr, *m64 = nullptr;
+    const size_t ext_row = sizeof(double) * (size_t)NCL * c->He * c->dp_Wp;
+    const size_t m_row = sizeof(double) * (size_t)NCL * c->cfg.ny * c->cfg.nx;
     if (!pool_alloc(c, &rows, sizeof(tl::RowD) * (size_t)chunk, st)) return TL_ENOMEM;
     if (!pool_alloc(c, &ext, ext_row * (size_t)chunk, st) ||
-        !pool_alloc(c, &partial, sizeof(double) * (size_t)chunk * c->dp_n_bands, st)) {
+        !pool_alloc(c, &partial, sizeof(double) * (size_t)chunk * c->dp_n_bands, st) ||
+        (lin && !pool_alloc(c, &m64, m_row * (size_t)chunk, st))) {
         cudaFreeAsync(rows, st);
         if (ext) cudaFreeAsync(ext, st);
+        if (partial) cudaFreeAsync(partial, st);
         return TL_ENOMEM;
     }
     // the pitch padding (Wp - We <= 1 column) is read by discarded strip lanes only, but must be finite
@@ -267,6 +273,7 @@ int run_dp(tl_ctx *c, const float *params, int64_t B, float *logL, float *images
         a.row0 = r0; a.rows_per_lens = rows_per_lens;
         a.psf = c->psf; a.data = c->data; a.wgt64 = c->wgt64; a.lconst = c->lconst;
         a.ext = ext; a.partial = logL ? partial : nullptr; a.logL = logL; a.images = images;
+        a.lin = lin; a.m64 = m64; a.amps = amps;
         a.P = c->P; a.ny = c->cfg.ny; a.nx = c->cfg.nx; a.K = c->K; a.Kp = c->Kp; a.h = c->h;
         a.He = c->He; a.We = c->We; a.Wp = c->dp_Wp; a.S = c->cfg.supersample;
         a.n_lens_light = c->cfg.n_lens_light; a.n_comp = c->n_comp;
@@ -282,11 +289,13 @@ int run_dp(tl_ctx *c, const float *params, int64_t B, float *logL, float *images
         if (c->profile) cudaEventRecord(c->ev0, st);
         c->dp_trace<<<grid, 256, 0, st>>>(a);
         if (c->profile) { cudaEventRecord(c->ev1, st); c->prof_pending = 1; }
-        tl::conv_dp_kernel<<<dim3((unsigned)nb, (unsigned)c->dp_n_bands), c->dp_conv_threads, c->dp_conv_smem, st>>>(a);
-        if (logL) tl::finalize_dp_kernel<<<(unsigned)((nb + 127) / 128), 128, 0, st>>>(a);
+        tl::conv_dp_kernel<<<dim3((unsigned)nb, (unsigned)c->dp_n_bands, (unsigned)NCL), c->dp_conv_threads, c->dp_conv_smem, st>>>(a);
+        if (lin) tl::solve_dp_kernel<<<(unsigned)nb, 256, 0, st>>>(a);
+        else if (logL) tl::finalize_dp_kernel<<<(unsigned)((nb + 127) / 128), 128, 0, st>>>(a);
         if (!cuda_ok(cudaGetLastError())) rc = TL_ECUDA;
     }
     cudaFreeAsync(rows, st); cudaFreeAsync(ext, st); cudaFreeAsync(partial, st);
+    if (m64) cudaFreeAsync(m64, st);
     return rc;
 }
 
@@ -732,6 +741,9 @@ int tl_loglike_linear_batch(tl_ctx *c, const float *params, int64_t B, float *lo
     if (!guard.ok) return TL_ECUDA;
     const int NC = c->n_comp;
     const size_t npix = (size_t)c->cfg.ny * c->cfg.nx;
+    // FP64 (and AUTO: with the amplitudes solved every row is near its best fit, so every row needs it)
+    if (c->precision == TL_PRECISION_FP64 || c->precision == TL_PRECISION_AUTO)
+        return run_dp(c, params, B, logL, nullptr, st, nullptr, nullptr, 1, amps);
     if (c->fused_lin && !c->opt.linear_staged) {
         const int64_t chunkf = CONST_CHUNK < B ? CONST_CHUNK : B;
         tl::RowC *rowsf = nullptr;

@@ -72,6 +72,10 @@ struct DpArgs {
     double *ext;                 // [chunk][He][Wp] binned extended images
     double *partial;             // [chunk][n_bands]
     float *logL, *images;
+    // linear-amplitude mode (tl_loglike_linear_batch in FP64): the components are kept apart
+    int lin;                     // 1: ext is [chunk][n_comp][He][Wp], unit amplitudes; conv writes m64
+    double *m64;                 // [chunk][n_comp][ny][nx] blurred unit-amplitude component images (columns of M)
+    float *amps;                 // [B][n_comp] or null
     int P, ny, nx, K, Kp, h, He, We, Wp, S, n_lens_light, n_comp, edge_zero, mass_model, lens_np;
     int band_rows, n_bands;
     int CW, CH, tiles_x, tiles_y;
@@ -255,8 +259,9 @@ __global__ void __launch_bounds__(64) prologue_dp_kernel(const DpArgs a)
         bool okc = true;
         for (int i = 0; i < 7; ++i) okc = okc && isfinite(sp[i]);
         double qs = 1.0, cs = 1.0, ss = 0.0;
+        if (a.lin) { okc = true; for (int i = 1; i < 7; ++i) okc = okc && isfinite(sp[i]); }
         okc = okc && (sp[1] > 0.f) && (sp[2] > 0.f) && shape_from_e(sp[3], sp[4], &qs, &cs, &ss);
-        const double Ie = okc ? (double)sp[0] : 0.0, re = okc ? (double)sp[1] : 1.0, n = okc ? (double)sp[2] : 1.0;
+        const double Ie = a.lin ? 1.0 : (okc ? (double)sp[0] : 0.0), re = okc ? (double)sp[1] : 1.0, n = okc ? (double)sp[2] : 1.0;
         if (!okc) { qs = 1.0; cs = 1.0; ss = 0.0; }
         const double bn = sersic_bn(n);
         const double A = qs / (re * re), Bq = 1.0 / (qs * re * re);     // Eq. 10: t = A x1^2 + B x2^2
@@ -323,6 +328,9 @@ __global__ void __launch_bounds__(256, 2) trace_dp_kernel(const DpArgs a)
         const int j = tc * a.CW + lj, i = tr * a.CH + li;
         if (i >= a.He || j >= a.We) continue;
         double acc = 0.0;
+        double comp_out[NLL + NSRC];                               // linear mode: the components, each on its own
+#pragma unroll
+        for (int k = 0; k < NLL + NSRC; ++k) comp_out[k] = 0.0;
         const bool edge = a.edge_zero && (j < a.h || j >= a.We - a.h || i < a.h || i >= a.He - a.h);
         if (!edge) {
             const double x0 = (double)(2 * j * S + 1 - S * a.We) * u, y0 = (double)(2 * i * S + 1 - S * a.He) * u;
@@ -350,6 +358,7 @@ __global__ void __launch_bounds__(256, 2) trace_dp_kernel(const DpArgs a)
                     }
                 }
                 acc = C.amp * accl;
+                comp_out[0] = acc;
             }
             {                                                      // ---- pass B: ray-trace + sources (a2, a3)
                 const double dx0 = x0 - R.cx;
@@ -386,10 +395,15 @@ __global__ void __launch_bounds__(256, 2) trace_dp_kernel(const DpArgs a)
                     }
                 }
 #pragma unroll
-                for (int k = 0; k < NSRC; ++k) acc = fma(R.comp[NLL + k].amp, accs[k], acc);
+                for (int k = 0; k < NSRC; ++k) { comp_out[NLL + k] = R.comp[NLL + k].amp * accs[k]; acc += comp_out[NLL + k]; }
             }
         }
-        a.ext[((size_t)r * a.He + i) * a.Wp + j] = acc;
+        if (a.lin) {
+#pragma unroll
+            for (int k = 0; k < NLL + NSRC; ++k) a.ext[(((size_t)r * (NLL + NSRC) + k) * a.He + i) * a.Wp + j] = comp_out[k];
+        } else {
+            a.ext[((size_t)r * a.He + i) * a.Wp + j] = acc;
+        }
     }
 }
 
@@ -438,13 +452,14 @@ __global__ void __launch_bounds__(256) conv_dp_kernel(const DpArgs a)
     extern __shared__ __align__(16) unsigned char dp_dyn[];
     __shared__ double red[32];
     const int n_rows = dp_n_rows(a);
-    const int r = blockIdx.x, band = blockIdx.y;
+    const int r = blockIdx.x, band = blockIdx.y, comp = blockIdx.z, ncmp = gridDim.z;   // (linear mode: one component per z)
     if (r >= n_rows) return;
     const int64_t row = dp_row(a, r);
     const int64_t lens = row / a.rows_per_lens;
     const size_t npix = (size_t)a.ny * a.nx;
     const int i0 = band * a.band_rows, i1 = min(a.ny, i0 + a.band_rows);
     if (!a.rows[r].valid) {
+        if (a.lin) return;                                         // solve_dp_kernel reports the row
         if (a.images)
             for (size_t i = (size_t)i0 * a.nx + threadIdx.x; i < (size_t)i1 * a.nx; i += blockDim.x) a.images[row * npix + i] = NAN;
         if (a.partial && threadIdx.x == 0) a.partial[(size_t)r * a.n_bands + band] = INFINITY;
@@ -459,7 +474,7 @@ __global__ void __launch_bounds__(256) conv_dp_kernel(const DpArgs a)
         taps[t] = kb < a.K ? (double)tsrc[ka * a.Kp + kb] : 0.0;
     }
     const int erows = (i1 - i0) + a.K - 1;
-    const double2 *src = reinterpret_cast<const double2 *>(a.ext + ((size_t)r * a.He + i0) * a.Wp);
+    const double2 *src = reinterpret_cast<const double2 *>(a.ext + (((size_t)r * ncmp + comp) * a.He + i0) * a.Wp);
     double2 *dst = reinterpret_cast<double2 *>(img);
     const int n2 = erows * a.Wp / 2;
     for (int t = threadIdx.x; t < n2; t += blockDim.x) dst[t] = src[t];
@@ -493,14 +508,76 @@ __global__ void __launch_bounds__(256) conv_dp_kernel(const DpArgs a)
             const int x = x0 + o;
             if (x < a.nx) {
                 const size_t off = (size_t)i * a.nx + x;
+                if (a.lin) { a.m64[((size_t)r * ncmp + comp) * npix + off] = acc[o]; continue; }
                 if (a.images) a.images[row * npix + off] = (float)acc[o];
                 if (a.partial) { const double d = (double)data[off] - acc[o]; part = fma(d * d, wgt[off], part); }
             }
         }
     }
-    if (a.partial) {
+    if (a.partial && !a.lin) {
         const double sum = block_sum(part, red);
         if (threadIdx.x == 0) a.partial[(size_t)r * a.n_bands + band] = sum;
+    }
+}
+
+// linear-amplitude mode in FP64 (PAPER.md:86-93 Eq. 6, :97-129 Eq. 7): one CTA per row.  G = M'WM,
+// b = M'Wd, d'Wd by fixed-shape block sums over the FP64 columns, the paper's NNLS (tl_nnls.cuh),
+// then chi^2 of the residual d - M s -> logL, amplitudes.
+__global__ void __launch_bounds__(256) solve_dp_kernel(const DpArgs a)
+{
+    __shared__ double red[32];
+    __shared__ double s_sh[3];
+    const int n_rows = dp_n_rows(a);
+    const int r = blockIdx.x;
+    if (r >= n_rows) return;
+    const int64_t row = dp_row(a, r);
+    const int NC = a.n_comp, npix = a.ny * a.nx;
+    if (!a.rows[r].valid) {
+        if (threadIdx.x == 0) {
+            a.logL[row] = -INFINITY;
+            if (a.amps) for (int k = 0; k < NC; ++k) a.amps[row * NC + k] = NAN;
+        }
+        return;
+    }
+    const int64_t lens = row / a.rows_per_lens;
+    const double *M = a.m64 + (size_t)r * NC * npix;
+    const float *d = a.data + lens * (size_t)npix;
+    const double *w = a.wgt64 + lens * (size_t)npix;
+    double g[6] = {0, 0, 0, 0, 0, 0}, bb[3] = {0, 0, 0}, dd = 0.0;
+    for (int i = threadIdx.x; i < npix; i += blockDim.x) {
+        const double wi = w[i], di = d[i];
+        double m[3] = {0.0, 0.0, 0.0};
+        for (int k = 0; k < NC; ++k) m[k] = M[(size_t)k * npix + i];
+        g[0] += wi * m[0] * m[0]; g[1] += wi * m[0] * m[1]; g[2] += wi * m[0] * m[2];
+        g[3] += wi * m[1] * m[1]; g[4] += wi * m[1] * m[2]; g[5] += wi * m[2] * m[2];
+        bb[0] += wi * m[0] * di; bb[1] += wi * m[1] * di; bb[2] += wi * m[2] * di;
+        dd += wi * di * di;
+    }
+    double G[3][3], b[3];
+    const double g0 = block_sum(g[0], red), g1 = block_sum(g[1], red), g2 = block_sum(g[2], red),
+                 g3 = block_sum(g[3], red), g4 = block_sum(g[4], red), g5 = block_sum(g[5], red);
+    b[0] = block_sum(bb[0], red); b[1] = block_sum(bb[1], red); b[2] = block_sum(bb[2], red);
+    const double dwd = block_sum(dd, red);
+    if (threadIdx.x == 0) {
+        G[0][0] = g0; G[0][1] = G[1][0] = g1; G[0][2] = G[2][0] = g2; G[1][1] = g3; G[1][2] = G[2][1] = g4; G[2][2] = g5;
+        double s[3] = {0.0, 0.0, 0.0}, Lc[9], z[3];
+        nnls_gram<3>(NC, &G[0][0], 3, b, dwd, s, Lc, z);
+        s_sh[0] = s[0]; s_sh[1] = s[1]; s_sh[2] = s[2];
+    }
+    __syncthreads();
+    const double s0 = s_sh[0], s1 = s_sh[1], s2 = s_sh[2];
+    double part = 0.0;
+    for (int i = threadIdx.x; i < npix; i += blockDim.x) {
+        double m = s0 * M[i];
+        if (NC > 1) m += s1 * M[(size_t)npix + i];
+        if (NC > 2) m += s2 * M[2 * (size_t)npix + i];
+        const double res = (double)d[i] - m;
+        part += res * res * w[i];
+    }
+    const double chi2 = block_sum(part, red);
+    if (threadIdx.x == 0) {
+        a.logL[row] = (float)(-0.5 * (chi2 + a.lconst[lens]));
+        if (a.amps) { a.amps[row * NC] = (float)s0; if (NC > 1) a.amps[row * NC + 1] = (float)s1; if (NC > 2) a.amps[row * NC + 2] = (float)s2; }
     }
 }
 
