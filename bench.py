@@ -46,7 +46,7 @@ OP_CHI2_FP32 = 4
 # (R^2/b^2)^kappa: 3 + lg2, ex2 (MUFU); Omega x radial 6; rotate back 4; shear + subtract 6.
 OP_EPL_FP32, OP_EPL_FP32_PER_TERM, OP_EPL_MUFU = 38, 2, 3
 SM_FP32_LANES = 128          # thread-instruction issue slots per SM per clock (4 warps x 32), measured 122-128
-SM_MUFU_LANES = 16           # measured 15.96 (profiles/r1_mufu_accuracy.md)
+SM_MUFU_LANES = 16           # measured 15.96 (profiles/r2_peaks.md)
 
 def ncu_dram_bytes(summary="r2_fused_kernel.md"):
     """dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, parsed from the
@@ -394,6 +394,11 @@ def run_ours(args, w: W.Workload):
     k_ms = float(np.mean(kern_ms))
     # a call of more than chunk_rows rows is several launches; the events are around the last one
     k_rows = B - ((B - 1) // info["chunk_rows"]) * info["chunk_rows"]
+    whole_step = info["path"] == 1 or args.precision != "fp32"
+    if whole_step:
+        # split path (large images) and the FP64 / AUTO modes: several kernels share the work of the op
+        # model, so the fraction is taken over the whole step, not over one kernel
+        k_ms, k_rows = total_ms / args.steps, B
     achieved = om["issue_slots"] * k_rows / (k_ms * 1e-3) / 1e12     # algorithmic Tinst/s
     peak = info["n_sm"] * SM_FP32_LANES * sm_max * 1e6 / 1e12
     mufu_frac = om["mufu_ops"] * k_rows / (k_ms * 1e-3) / (info["n_sm"] * SM_MUFU_LANES * sm_max * 1e6)
@@ -411,14 +416,18 @@ def run_ours(args, w: W.Workload):
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": B * w.n_params * 4,
                 "d2h_bytes_per_step": B * 4, "api": "tl_loglike_batch_host (pinned host buffers)"},
         "e2e_pipelined": pipelined,
-        "gpu_launches": (3 if B <= info["small_batch_rows"] else info["launches_per_call"]) * args.steps,
+        "gpu_launches": ({"fp64": 4, "fp64-libm": 2}.get(args.precision,
+                                                         (3 if (B <= info["small_batch_rows"] and args.precision == "fp32") else info["launches_per_call"])
+                                                         + (4 if args.precision == "auto" else 0))
+                         * ((B + info["chunk_rows"] - 1) // info["chunk_rows"] if args.precision in ("fp32", "auto") else 1)) * args.steps,
         "roofline": {
-            "bound": "alu", "kernel": "fused_kernel" if (info["path"] == 0 and B > info["small_batch_rows"]) else "trace_kernel",
+            "bound": "alu", "kernel": ("whole step (all kernels)" if whole_step else
+                                       "fused_kernel" if B > info["small_batch_rows"] else "trace_kernel + conv_small_kernel"),
             "achieved": achieved, "peak": peak, "unit": "Tinst/s", "frac": achieved / peak,
             "traffic": ncu_dram_bytes() if (w.mass_model == W.MASS_SIE and w.index == 1 and args.precision == "fp32"
                                             and args.rows == "prior") else None,
             "peak_source": "derived: %d SMs x %d issue slots/clk x %.0f MHz (MEASURED_PEAKS.json sm_max_mhz; "
-                           "slots/clk measured, profiles/r1_mufu_accuracy.md)" % (info["n_sm"], SM_FP32_LANES, sm_max),
+                           "slots/clk measured, profiles/r2_peaks.md)" % (info["n_sm"], SM_FP32_LANES, sm_max),
             "kernel_ms": k_ms, "kernel_rows": k_rows, "fp32_pipe_frac": fp32_frac, "mufu_pipe_frac": mufu_frac,
             "algorithmic_issue_slots_per_likelihood": om["issue_slots"],
             **({"epl_mean_series_terms": epl_mean_terms(rows)} if w.mass_model == W.MASS_EPL else {}),
@@ -426,6 +435,12 @@ def run_ours(args, w: W.Workload):
                     "achieved_GBs": hbm_bytes * (k_rows / B) / (k_ms * 1e-3) / 1e9,
                     "peak_GBs": peaks.get("hbm_gbs"), "note": "compute-bound by design; HBM traffic is negligible"},
         },
+        **({"roofline_fp64": {"bound": "alu", "note": "FP64 pipe: 64 DFMA lanes/clk/SM; op model v0 with every FP32 slot and every "
+                              "transcendental counted as ONE FP64 operation (the polynomials are overhead)",
+                              "achieved": (om["fp32_slots"] + om["mufu_ops"]) * B / (total_ms / args.steps * 1e-3) / 1e12,
+                              "peak": info["n_sm"] * 64 * sm_max * 1e6 / 1e12, "unit": "Tinst/s",
+                              "frac": (om["fp32_slots"] + om["mufu_ops"]) * B / (total_ms / args.steps * 1e-3) / (info["n_sm"] * 64 * sm_max * 1e6)}}
+           if args.precision == "fp64" else {}),
         "launch": {**{k: info[k] for k in ("path", "block_threads", "ctas_per_sm", "grid", "smem_bytes")},
                    "small_batch_path": bool(B <= info["small_batch_rows"])},
         "checksum_logL": logl_sum,
@@ -550,7 +565,7 @@ def run_linear(args, w: W.Workload):
             "dtype": "f32" if args.precision == "fp32" else "f64", "precision": args.precision, "data": "synthetic",
             "config": config_dict(w, "flushed between steps (256 MiB fill)"), "clocks": clk.summary(),
             "pixel_evals_per_s": value * w.ny * w.nx, "mode": "linear",
-            "gpu_launches": args.steps * 2, "checksum_logL": float(out.double().sum())}
+            "gpu_launches": args.steps * (2 if args.precision == "fp32" else 4), "checksum_logL": float(out.double().sum())}
     # roofline of the fused linear kernel: op model v0 per sample (unchanged) + per native pixel
     # C convolutions, the Gram matrix / right-hand side (C (C + 3)) and the residual (C + 3)
     C_ = w.n_lens_light + w.n_source
@@ -565,11 +580,11 @@ def run_linear(args, w: W.Workload):
                         "frac": ach / peak, "traffic": None, "kernel_ms": k_ms,
                         "algorithmic_issue_slots_per_likelihood": slots,
                         "peak_source": "as in the default mode"}
-    if os.environ.get("TL_LINEAR_STAGED"):
-        # staged pipeline forced: the events bracket trace_lin_kernel of the last chunk only, which
-        # is not the whole of the op model above -- no roofline fraction is claimed for this run
-        line["roofline"] = {"bound": "alu", "kernel": "trace_lin_kernel (staged pipeline forced by TL_LINEAR_STAGED)",
-                            "achieved": None, "peak": peak, "unit": "Tinst/s", "frac": None, "traffic": None, "kernel_ms": k_ms}
+    if args.precision != "fp32":
+        # FP64 pipeline: several kernels; the fraction is taken over the whole step against the same issue roofline
+        ach = slots * B / (total_ms / args.steps * 1e-3) / 1e12
+        line["roofline"] = {"bound": "alu", "kernel": "whole step (trace_dp + conv_dp + solve_dp)", "achieved": ach, "peak": peak,
+                            "unit": "Tinst/s", "frac": ach / peak, "traffic": None, "kernel_ms": total_ms / args.steps}
     if not args.no_cpu_baseline:
         from oracle import oracle as O
         O.lib()
@@ -620,16 +635,17 @@ def run_mge(args, w: W.Workload, prob, ctx, rows):
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": config_dict(w, "flushed between steps (256 MiB fill)"), "clocks": clk.summary(),
             "pixel_evals_per_s": value * w.ny * w.nx, "mode": "mge", "mge_sigmas_arcsec": [float(x) for x in sigmas],
-            "chunk_rows": int(chunk), "gpu_launches": int(args.steps * 7 * n_chunks), "checksum_logL": float(out.double().sum())}
-    # dominant kernel: conv_lin_kernel, the NC PSF convolutions of a row (NC K^2 FMAs per native pixel);
-    # the events bracket the conv launch of the call's last chunk
+            "chunk_rows": int(chunk), "gpu_launches": int(args.steps * 6 * n_chunks), "checksum_logL": float(out.double().sum())}
+    # (the events bracket the gauss_conv launch of the call's last chunk)
     info = ctx.info()
     sm_max = float(measured_peaks().get("sm_max_mhz", 1965.0))
     k_ms = float(np.mean(kern_ms))
-    slots = NC * w.psf_size ** 2 * w.ny * w.nx
+    # dominant kernel: gauss_conv_kernel -- per Gaussian, 4 slots per sub-sample (t from its row / column parts,
+    # scale, MUFU.EX2, accumulate) and the PSF convolution (K^2 FMAs per native pixel)
+    slots = len(sigmas) * (4 * w.samples_per_likelihood + w.psf_size ** 2 * w.ny * w.nx)
     ach = slots * last_rows / (k_ms * 1e-3) / 1e12
     peak = info["n_sm"] * SM_FP32_LANES * sm_max * 1e6 / 1e12
-    line["roofline"] = {"bound": "alu", "kernel": "conv_lin_kernel", "achieved": ach, "peak": peak, "unit": "Tinst/s",
+    line["roofline"] = {"bound": "alu", "kernel": "gauss_conv_kernel", "achieved": ach, "peak": peak, "unit": "Tinst/s",
                         "frac": ach / peak, "traffic": None, "kernel_ms": k_ms, "kernel_rows": int(last_rows),
                         "algorithmic_issue_slots_per_likelihood": slots,
                         "peak_source": "as in the default mode (FP32 FMA issue slots)"}

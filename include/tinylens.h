@@ -89,7 +89,8 @@ typedef struct {
     int32_t ny, nx;          /* native image size (rows, columns)                              */
     double  pix_scale;       /* arcsec per native pixel, > 0                                   */
     int32_t supersample;     /* S >= 1: S x S samples per native pixel, S <= 16  */
-    int32_t n_lens_light;    /* 0 or 1 Sersic components evaluated at theta                    */
+    int32_t n_lens_light;    /* 0 or 1 Sersic components evaluated at theta (2: two MGE sets,  */
+                             /* tl_set_mge_sets; such a context serves tl_loglike_mge_batch only) */
     int32_t n_source;        /* 1 or 2 Sersic components evaluated at beta                     */
     int32_t edge_mode;       /* TL_EDGE_EXTEND or TL_EDGE_ZERO                                 */
     int32_t n_lens;          /* 1, or L for a heterogeneous batch of L lenses (own psf, data,  */
@@ -235,7 +236,7 @@ int tl_loglike_linear_batch(tl_ctx *ctx, const float *params, int64_t B, float *
  *
  * tl_set_mge -- define the Gaussian set of a context created with n_lens_light = 1.
  *   sigmas     HOST pointer, float [n_gauss], arcsec, finite and > 0 (copied)
- *   n_gauss    1 .. 16
+ *   n_gauss    1 .. 30
  * Synchronous; not thread-safe with respect to calls in flight on the same context.  May be
  * called again to change the set.  TL_OK, TL_EINVAL (also: n_lens_light != 1), TL_ESIZE,
  * TL_ENOMEM or TL_ECUDA.
@@ -261,6 +262,18 @@ int tl_loglike_linear_batch(tl_ctx *ctx, const float *params, int64_t B, float *
  * multiple of n_lens), TL_ENOMEM, TL_ECUDA or TL_ESIZE.
  */
 int tl_set_mge(tl_ctx *ctx, const float *sigmas, int32_t n_gauss);
+/*
+ * tl_set_mge_sets -- several Gaussian sets, each with its own ellipticity, position angle and centre
+ * ("isophote twists").  The context must have been created with n_lens_light =
+ * n_sets (1 or 2): lens-light block j of the parameter row supplies (e1, e2, cx, cy) of set j (its
+ * I_e, r_e, n are ignored).  A context with n_lens_light = 2 serves tl_loglike_mge_batch only (the
+ * other batch calls return TL_EINVAL).
+ *   sigmas      HOST pointer, float [sum_j n_per_set[j]]: the dispersions of set 0, then of set 1
+ *   n_per_set   HOST pointer, int32 [n_sets], each >= 1; at most 30 Gaussians in total (the NNLS then
+ *               has up to 30 + n_source <= 32 columns)
+ * tl_set_mge(ctx, sigmas, n) is tl_set_mge_sets with one set.  Same return codes.
+ */
+int tl_set_mge_sets(tl_ctx *ctx, const float *sigmas, const int32_t *n_per_set, int32_t n_sets);
 int tl_mge_columns(const tl_ctx *ctx);
 int64_t tl_mge_chunk_rows(const tl_ctx *ctx);
 int tl_loglike_mge_batch(tl_ctx *ctx, const float *params, int64_t B, float *logL, float *amps,

@@ -88,6 +88,7 @@ def load(build_if_missing: bool = True):
     L.tl_wait.restype = C.c_int; L.tl_wait.argtypes = [vp, C.c_int]
     L.tl_loglike_linear_batch.restype = C.c_int; L.tl_loglike_linear_batch.argtypes = [vp, vp, i64, vp, vp, vp]
     L.tl_set_mge.restype = C.c_int; L.tl_set_mge.argtypes = [vp, fp, i32]
+    L.tl_set_mge_sets.restype = C.c_int; L.tl_set_mge_sets.argtypes = [vp, fp, C.POINTER(i32), i32]
     L.tl_mge_columns.restype = C.c_int; L.tl_mge_columns.argtypes = [vp]
     L.tl_mge_chunk_rows.restype = i64; L.tl_mge_chunk_rows.argtypes = [vp]
     L.tl_loglike_mge_batch.restype = C.c_int; L.tl_loglike_mge_batch.argtypes = [vp, vp, i64, vp, vp, vp]
@@ -235,6 +236,15 @@ def tl_set_mge(handle: int, sigmas):
     _check(load().tl_set_mge(handle, sg.ctypes.data_as(C.POINTER(C.c_float)), int(sg.size)), "tl_set_mge")
 
 
+def tl_set_mge_sets(handle: int, sigma_sets):
+    """sigma_sets: list of 1-D float arrays (arcsec), one per Gaussian set; set j takes its shape and centre
+    from lens-light block j of the parameter rows (the context's n_lens_light must equal len(sigma_sets))."""
+    sets = [_f32c(sg).reshape(-1) for sg in sigma_sets]
+    allsg = np.concatenate(sets)
+    per = (C.c_int32 * len(sets))(*[int(sg.size) for sg in sets])
+    _check(load().tl_set_mge_sets(handle, allsg.ctypes.data_as(C.POINTER(C.c_float)), per, len(sets)), "tl_set_mge_sets")
+
+
 def tl_mge_columns(handle: int) -> int:
     return load().tl_mge_columns(handle)
 
@@ -370,6 +380,9 @@ class LensContext:
 
     def set_mge(self, sigmas):
         tl_set_mge(self.handle, sigmas)
+
+    def set_mge_sets(self, sigma_sets):
+        tl_set_mge_sets(self.handle, sigma_sets)
 
     def loglike_mge(self, params, out=None, amps=None, want_amps=True, stream=None):
         return tl_loglike_mge_batch(self.handle, params, out, amps, want_amps, stream)

@@ -79,7 +79,8 @@ struct tl_ctx {
     int sb_rowtab = 0, sb_max_rows = 0;
     // MGE mode (tl_set_mge / tl_loglike_mge_batch)
     float *mge_c = nullptr;       // device [n_gauss]: log2(e) / (2 sigma_k^2)
-    int n_gauss = 0;
+    int *mge_set = nullptr;       // device [n_gauss]: the set each Gaussian belongs to
+    int n_gauss = 0, mge_n_sets = 0, mge_per_set[tl::MGE_MAX_SETS] = {0, 0};
     void (*mge_trace)(const tl::KArgs, int) = nullptr;   // sources only: trace_kernel<S,0,1> or trace_lin_kernel<S,0,2>
     size_t mge_trace_smem = 0, mge_gc_smem = 0;
     int mge_rowtab = 0, mge_fused = 0;                   // fused: gauss_conv_kernel (extended image in shared memory)
@@ -302,6 +303,7 @@ int run_dp(tl_ctx *c, const float *params, int64_t B, float *logL, float *images
 int run_batch(tl_ctx *c, const float *params, int64_t B, float *logL, float *images, cudaStream_t st)
 {
     if (!c || B < 0) return TL_EINVAL;
+    if (c->cfg.n_lens_light > 1) return TL_EINVAL;               // several lens-light blocks: MGE sets only
     if (B == 0) return TL_OK;
     if (!params || (!logL && !images)) return TL_EINVAL;
     if (B % c->cfg.n_lens) return TL_EINVAL;
@@ -451,7 +453,8 @@ int tl_create_ex(tl_ctx **out, const tl_config *cfg, const float *psf_in, int32_
     }
     if (cfg->ny < 1 || cfg->nx < 1 || !(cfg->pix_scale > 0.0) || !std::isfinite(cfg->pix_scale)) return TL_EINVAL;
     if (cfg->supersample < 1 || cfg->supersample > 16) return TL_EINVAL;
-    if (cfg->n_lens_light < 0 || cfg->n_lens_light > 1 || cfg->n_source < 1 || cfg->n_source > 2) return TL_EINVAL;
+    // n_lens_light = 2: two MGE sets with their own shapes; such a context serves tl_loglike_mge_batch only
+    if (cfg->n_lens_light < 0 || cfg->n_lens_light > tl::MGE_MAX_SETS || cfg->n_source < 1 || cfg->n_source > 2) return TL_EINVAL;
     if (cfg->edge_mode != TL_EDGE_EXTEND && cfg->edge_mode != TL_EDGE_ZERO) return TL_EINVAL;
     if (cfg->n_lens < 1) return TL_EINVAL;
     if (cfg->mass_model != TL_MASS_SIE && cfg->mass_model != TL_MASS_EPL) return TL_EINVAL;
@@ -734,7 +737,7 @@ int tl_loglike_linear_batch(tl_ctx *c, const float *params, int64_t B, float *lo
 {
     if (!c || B < 0) return TL_EINVAL;
     if (B == 0) return TL_OK;
-    if (!params || !logL || (B % c->cfg.n_lens)) return TL_EINVAL;
+    if (!params || !logL || (B % c->cfg.n_lens) || c->cfg.n_lens_light > 1) return TL_EINVAL;
     if (!c->trace_lin) return TL_ESIZE;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     DeviceGuard guard(c->device);
@@ -815,19 +818,34 @@ namespace { int64_t mge_chunk_rows(const tl_ctx *c); }
 
 int tl_set_mge(tl_ctx *c, const float *sigmas, int32_t n_gauss)
 {
-    if (!c || !sigmas || n_gauss < 1 || n_gauss > tl::MGE_MAX_GAUSS) return TL_EINVAL;
-    if (c->cfg.n_lens_light != 1) return TL_EINVAL;
+    return tl_set_mge_sets(c, sigmas, &n_gauss, 1);
+}
+
+int tl_set_mge_sets(tl_ctx *c, const float *sigmas, const int32_t *n_per_set, int32_t n_sets)
+{
+    if (!c || !sigmas || !n_per_set || n_sets < 1 || n_sets > tl::MGE_MAX_SETS) return TL_EINVAL;
+    if (c->cfg.n_lens_light != n_sets) return TL_EINVAL;           // one lens-light block of the row per set
+    int n_gauss = 0;
+    for (int j = 0; j < n_sets; ++j) { if (n_per_set[j] < 1) return TL_EINVAL; n_gauss += n_per_set[j]; }
+    if (n_gauss > tl::MGE_MAX_GAUSS) return TL_EINVAL;
     if (!c->trace_lin) return TL_ESIZE;
     float ck[tl::MGE_MAX_GAUSS];
-    for (int k = 0; k < n_gauss; ++k) {
+    int set_of[tl::MGE_MAX_GAUSS];
+    for (int k = 0, j = 0, left = n_per_set[0]; k < n_gauss; ++k, --left) {
+        while (left == 0) left = n_per_set[++j];
+        set_of[k] = j;
         if (!std::isfinite(sigmas[k]) || !(sigmas[k] > 0.f)) return TL_EINVAL;
         ck[k] = (float)(1.4426950408889634074 / (2.0 * (double)sigmas[k] * (double)sigmas[k]));
         if (!std::isfinite(ck[k])) return TL_EINVAL;
     }
     DeviceGuard guard(c->device);
     if (!guard.ok) return TL_ECUDA;
-    if (!c->mge_c && !cuda_ok(cudaMalloc(&c->mge_c, sizeof(float) * tl::MGE_MAX_GAUSS))) return TL_ENOMEM;
-    if (!cuda_ok(cudaMemcpy(c->mge_c, ck, sizeof(float) * n_gauss, cudaMemcpyHostToDevice))) return TL_ECUDA;
+    if (!c->mge_c && (!cuda_ok(cudaMalloc(&c->mge_c, sizeof(float) * tl::MGE_MAX_GAUSS)) ||
+                      !cuda_ok(cudaMalloc(&c->mge_set, sizeof(int) * tl::MGE_MAX_GAUSS)))) return TL_ENOMEM;
+    if (!cuda_ok(cudaMemcpy(c->mge_c, ck, sizeof(float) * n_gauss, cudaMemcpyHostToDevice)) ||
+        !cuda_ok(cudaMemcpy(c->mge_set, set_of, sizeof(int) * n_gauss, cudaMemcpyHostToDevice))) return TL_ECUDA;
+    c->mge_n_sets = n_sets;
+    for (int j = 0; j < tl::MGE_MAX_SETS; ++j) c->mge_per_set[j] = j < n_sets ? n_per_set[j] : 0;
     c->n_gauss = n_gauss;
     if (!c->mge_trace) {
         // sources through the NLL = 0 ray-trace kernels (no lens-light stand-in; one source: packed pair loop)
@@ -847,6 +865,8 @@ int tl_set_mge(tl_ctx *c, const float *sigmas, int32_t n_gauss)
         if (c->mge_fused)
             okm = okm && cuda_ok(cudaFuncSetAttribute(tl::gauss_conv_for(S), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SMEM_LIMIT - 1024))) &&
                   cuda_ok(cudaFuncSetAttribute(tl::gauss_conv_for(S), cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+        okm = okm && cuda_ok(cudaFuncSetAttribute(tl::nnls_mge_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                  (int)(sizeof(double) * tl::MGE_NNLS_WARPS * (2 * tl::MGE_MAX_COL * tl::MGE_MAX_COL + 3 * tl::MGE_MAX_COL))));
         if (!okm) { c->mge_trace = nullptr; c->n_gauss = 0; cudaGetLastError(); return TL_ECUDA; }
     }
     if (c->pool) {   // the MGE call stages a chunk's component images: let the pool keep that much cached between calls
@@ -933,7 +953,7 @@ int tl_loglike_mge_batch(tl_ctx *c, const float *params, int64_t B, float *logL,
         a.rows = rows; a.B = nb; a.rows_per_lens = rows_per_lens; a.row0 = r0;
         a.logL = logL; a.amps = amps; a.ext = ext; a.mimg = mimg;
         a.tile_rows = c->lin_tile_rows; a.n_tiles = c->lin_n_tiles;
-        a.n_gauss = NG; a.mge_c = c->mge_c; a.mge_gram = gram;
+        a.n_gauss = NG; a.mge_c = c->mge_c; a.mge_set = c->mge_set; a.mge_gram = gram;
         // 1. the sources, ray-traced at unit amplitude -> ext slots (fused: 0.., else NG..)
         tl::KArgs at = a;
         at.rowtab = c->mge_rowtab; at.ext_nc = ext_nc; at.ext_k0 = fused ? 0 : NG;
@@ -949,14 +969,20 @@ int tl_loglike_mge_batch(tl_ctx *c, const float *params, int64_t B, float *logL,
             ac.conv_ext_nc = NS; ac.conv_m_nc = NC; ac.conv_m_k0 = NG;
             tl::conv_lin_kernel<<<dim3((unsigned)nb, (unsigned)c->lin_n_tiles, (unsigned)NS), 256, c->lin_conv_smem, st>>>(ac, (int)nb);
         } else {
-            tl::mge_gauss_for(NG)<<<dim3((unsigned)nb, (unsigned)gslabs), 256, 0, st>>>(a, (int)nb);
+            for (int j = 0, k0 = 0; j < c->mge_n_sets; k0 += c->mge_per_set[j], ++j) {          // one launch per set
+                tl::KArgs ag = a;
+                ag.mge_k0 = k0; ag.mge_shape = j;
+                tl::mge_gauss_for(c->mge_per_set[j])<<<dim3((unsigned)nb, (unsigned)gslabs), 256, 0, st>>>(ag, (int)nb);
+            }
             if (c->profile) cudaEventRecord(c->ev0, st);
             tl::conv_lin_kernel<<<dim3((unsigned)nb, (unsigned)c->lin_n_tiles, (unsigned)NC), 256, c->lin_conv_smem, st>>>(a, (int)nb);
             if (c->profile) { cudaEventRecord(c->ev1, st); c->prof_pending = 1; }
         }
         // 4. Gram matrix, 5. NNLS + logL
-        tl::gram_mge_kernel<<<(unsigned)nb, tl::MGE_SOLVE_THREADS, 0, st>>>(a, (int)nb);
-        tl::nnls_mge_kernel<<<(unsigned)((nb + tl::MGE_NNLS_WARPS - 1) / tl::MGE_NNLS_WARPS), 32 * tl::MGE_NNLS_WARPS, 0, st>>>(a, (int)nb);
+        if (NC + 1 <= 20) tl::gram_mge_kernel<128><<<(unsigned)nb, 128, 0, st>>>(a, (int)nb);
+        else tl::gram_mge_kernel<512><<<(unsigned)nb, 512, 0, st>>>(a, (int)nb);
+        const size_t nnls_smem = sizeof(double) * tl::MGE_NNLS_WARPS * (size_t)(2 * NC * NC + 3 * NC);
+        tl::nnls_mge_kernel<<<(unsigned)((nb + tl::MGE_NNLS_WARPS - 1) / tl::MGE_NNLS_WARPS), 32 * tl::MGE_NNLS_WARPS, nnls_smem, st>>>(a, (int)nb);
         if (!cuda_ok(cudaGetLastError())) rc = TL_ECUDA;
     }
     cudaFreeAsync(rows, st); cudaFreeAsync(ext, st); cudaFreeAsync(mimg, st); cudaFreeAsync(gram, st);
@@ -1068,7 +1094,7 @@ void tl_destroy(tl_ctx *c)
     }
     if (c->s_up) cudaStreamDestroy(c->s_up);
     if (c->s_down) cudaStreamDestroy(c->s_down);
-    cudaFree(c->mge_c);
+    cudaFree(c->mge_c); cudaFree(c->mge_set);
     cudaFree(c->psf); cudaFree(c->data); cudaFree(c->wgt); cudaFree(c->wgt64); cudaFree(c->noise); cudaFree(c->sigma_min); cudaFree(c->lconst);
     if (c->pool) cudaMemPoolDestroy(c->pool);
     delete c;

@@ -26,7 +26,7 @@
 
 namespace tl {
 
-constexpr int MAX_COMP = 3;          // n_lens_light (<= 1) + n_source (<= 2)
+constexpr int MAX_COMP = 4;          // n_lens_light (<= 1; MGE mode: <= 2 sets) + n_source (<= 2)
 constexpr int MASS_SIE = 0, MASS_EPL = 1;          // tl_config.mass_model
 constexpr int EPL_TERMS = 24;        // angular-series terms of the FP32 EPL path (rows needing more: FP64)
 constexpr int EPL_TERMS64 = 64;      // terms kept in FP64 for the selective refinement (remainder < 1e-16)

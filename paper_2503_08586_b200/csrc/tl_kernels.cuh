@@ -47,6 +47,8 @@ struct KArgs {
     int *flag_count, *flag_list;
     float err_coh, err_rnd;  // bound = err_coh |sum e_i| + err_rnd sqrt(sum e_i^2),  e_i = (d_i - m_i) m_i / sigma_i^2
     const float *mge_c;      // [n_gauss] log2(e) / (2 sigma_k^2), arcsec^-2
+    const int *mge_set;      // [n_gauss] the set (0 .. n_lens_light-1) Gaussian k belongs to: its shape is comp[n_source + set]
+    int mge_k0, mge_shape;   // mge_gauss_kernel (unfused path, one launch per set): first Gaussian and set of this launch
     double *mge_gram;        // [chunk][MGE_GRAM_STRIDE]  G | b | d'Wd
     // conv_lin_kernel: component strides of ext and of mimg, first mimg slot (0, 0, 0 = gridDim.z, gridDim.z, 0)
     int conv_ext_nc, conv_m_nc, conv_m_k0;

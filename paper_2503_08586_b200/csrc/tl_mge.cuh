@@ -28,9 +28,10 @@
 
 namespace tl {
 
-constexpr int MGE_MAX_GAUSS = 16;
-constexpr int MGE_MAX_COL = MGE_MAX_GAUSS + 2;       // + n_source
-constexpr int MGE_SOLVE_THREADS = 128;
+constexpr int MGE_MAX_GAUSS = 30;                    // over all sets ("several dozen amplitudes")
+constexpr int MGE_MAX_COL = MGE_MAX_GAUSS + 2;       // + n_source: 32, the width of the solver's bit masks
+constexpr int MGE_MAX_SETS = 2;                      // Gaussian sets with their own (e1, e2, centre) = n_lens_light
+constexpr int MGE_SOLVE_THREADS = 128;               // gram_mge_kernel: 128 threads up to 20 columns + data, else 512
 constexpr int MGE_GRAM_STRIDE = MGE_MAX_COL * (MGE_MAX_COL + 1) + MGE_MAX_COL + 2;   // doubles per row: G [n][NCP] | b [n] | d'Wd
 constexpr int MGE_NNLS_WARPS = 4;                    // rows per CTA of nnls_mge_kernel (one warp each)
 constexpr int MGE_TILE = 64;                         // pixels staged per step of the Gram reduction
@@ -48,21 +49,21 @@ __global__ void __launch_bounds__(256) mge_gauss_kernel(const KArgs a, int chunk
     if (r >= chunk_rows) return;
     const RowC &rc = a.rows[r];
     if (!row_is_valid(rc, a.n_comp)) return;
-    const SersicC &C = rc.comp[a.n_comp - a.n_lens_light];       // MGE order: the set's shape follows the sources
+    const SersicC &C = rc.comp[a.n_comp - a.n_lens_light + a.mge_shape];   // MGE order: the sets' shapes follow the sources
     const float cXh = C.cXh, cXl = C.cXl, cYh = C.cYh, cYl = C.cYl;
     const float ah = C.ah, al = C.al, b2h = C.b2h, b2l = C.b2l, cch = C.cch, ccl = C.ccl;
     const int S = a.S;
     float ck[NG];
 #pragma unroll
-    for (int k = 0; k < NG; ++k) ck[k] = -a.mge_c[k];
+    for (int k = 0; k < NG; ++k) ck[k] = -a.mge_c[a.mge_k0 + k];
     const float inv_s2 = 1.f / (float)(S * S);
     const size_t comp_stride = (size_t)a.He * a.pitch;
-    float *dst = a.ext + (size_t)r * a.ext_nc * comp_stride;
+    float *dst = a.ext + ((size_t)r * a.ext_nc + a.mge_k0) * comp_stride;     // this set's slots
     const int npx = a.He * a.pitch;
     for (int p = blockIdx.y * blockDim.x + threadIdx.x; p < npx; p += gridDim.y * blockDim.x) {
         const int i = p / a.pitch, j = p - i * a.pitch;
         if (j >= a.We) {                               // pitch padding of every component reads as zero
-            for (int k = 0; k < a.ext_nc; ++k) dst[k * comp_stride + (size_t)i * a.pitch + j] = 0.f;
+            for (int k = -a.mge_k0; k < a.ext_nc - a.mge_k0; ++k) dst[k * (long long)comp_stride + (size_t)i * a.pitch + j] = 0.f;
             continue;
         }
         float acc[NG];
@@ -114,7 +115,7 @@ __global__ void __launch_bounds__(256) gauss_conv_kernel(const KArgs a, int chun
     if (!row_is_valid(rc, a.n_comp)) return;
     const int64_t lens = (a.row0 + r) / a.rows_per_lens;
     load_psf(taps, a.psf + lens * a.K * a.Kp, a.K * a.Kp);
-    const SersicC &C = rc.comp[a.n_comp - a.n_lens_light];
+    const SersicC &C = rc.comp[a.n_comp - a.n_lens_light + a.mge_set[k]];     // the shape of this Gaussian's set
     const float cXh = C.cXh, cXl = C.cXl, cYh = C.cYh, cYl = C.cYl;
     const float ah = C.ah, al = C.al, b2h = C.b2h, b2l = C.b2l, cch = C.cch, ccl = C.ccl;
     const float ck = -a.mge_c[k];
@@ -202,6 +203,11 @@ inline mge_gauss_fn mge_gauss_for(int ng)
     case 10: return mge_gauss_kernel<10>; case 11: return mge_gauss_kernel<11>; case 12: return mge_gauss_kernel<12>;
     case 13: return mge_gauss_kernel<13>; case 14: return mge_gauss_kernel<14>; case 15: return mge_gauss_kernel<15>;
     case 16: return mge_gauss_kernel<16>;
+    case 17: return mge_gauss_kernel<17>; case 18: return mge_gauss_kernel<18>; case 19: return mge_gauss_kernel<19>;
+    case 20: return mge_gauss_kernel<20>; case 21: return mge_gauss_kernel<21>; case 22: return mge_gauss_kernel<22>;
+    case 23: return mge_gauss_kernel<23>; case 24: return mge_gauss_kernel<24>; case 25: return mge_gauss_kernel<25>;
+    case 26: return mge_gauss_kernel<26>; case 27: return mge_gauss_kernel<27>; case 28: return mge_gauss_kernel<28>;
+    case 29: return mge_gauss_kernel<29>; case 30: return mge_gauss_kernel<30>;
     default: return nullptr;
     }
 }
@@ -210,7 +216,8 @@ inline mge_gauss_fn mge_gauss_for(int ng)
 // memory MGE_TILE at a time (w m_k and m_k, d as doubles, the next tile prefetched into registers);
 // every sum has a fixed order, so the result is bitwise reproducible.
 // Output: a.mge_gram[r][MGE_GRAM_STRIDE].
-__global__ void __launch_bounds__(MGE_SOLVE_THREADS) gram_mge_kernel(const KArgs a, int chunk_rows)
+template <int THREADS>
+__global__ void __launch_bounds__(THREADS) gram_mge_kernel(const KArgs a, int chunk_rows)
 {
     constexpr int NCP = MGE_MAX_COL + 2;               // columns + data, rounded up to even
     // column-major tiles with an odd pitch: the staging stores of a warp (consecutive pixels of one
@@ -235,7 +242,7 @@ __global__ void __launch_bounds__(MGE_SOLVE_THREADS) gram_mge_kernel(const KArgs
     // feed four DFMAs (one entry per thread is bound by the shared-memory pipe); the Q pixel
     // slices of an entry are then added in slice order -- a fixed summation order.
     const int n1 = n + 1, NB = (n1 + 1) >> 1, nblk = NB * (NB + 1) / 2;
-    const int Q = MGE_SOLVE_THREADS / nblk;                       // >= 2 (nblk <= 55)
+    const int Q = THREADS / nblk;                                 // >= 2 (nblk <= 55 at 128 threads, <= 153 at 512)
     const int slice = threadIdx.x / nblk;
     int bi = 0, bj = 0;
     {
@@ -248,8 +255,8 @@ __global__ void __launch_bounds__(MGE_SOLVE_THREADS) gram_mge_kernel(const KArgs
     // the next tile's values are fetched into registers while the current one is consumed, so the
     // global-memory latency (M does not fit in L2 for a whole batch) overlaps the FP64 sums.
     // Thread t stages pixel t % MGE_TILE of the tile for the columns t / MGE_TILE, + 2, + 4, ...
-    constexpr int EPT = (MGE_TILE * NCP + MGE_SOLVE_THREADS - 1) / MGE_SOLVE_THREADS;
-    static_assert(MGE_SOLVE_THREADS % MGE_TILE == 0, "a thread stages one pixel of the tile");
+    constexpr int EPT = (MGE_TILE * NCP + THREADS - 1) / THREADS;
+    static_assert(THREADS % MGE_TILE == 0, "a thread stages one pixel of the tile");
     const int ncol = 2 * NB;                                      // n1 rounded up to even: a zero column
     const int sii = threadIdx.x % MGE_TILE, sk0 = threadIdx.x / MGE_TILE;
     float fv[EPT], fwv = 0.f;
@@ -258,7 +265,7 @@ __global__ void __launch_bounds__(MGE_SOLVE_THREADS) gram_mge_kernel(const KArgs
         fwv = i < npix ? w[i] : 0.f;
 #pragma unroll
         for (int u = 0; u < EPT; ++u) {
-            const int k = sk0 + u * (MGE_SOLVE_THREADS / MGE_TILE);
+            const int k = sk0 + u * (THREADS / MGE_TILE);
             fv[u] = 0.f;
             if (k < n1 && i < npix) fv[u] = k < n ? M[(size_t)k * npix + i] : d[i];
         }
@@ -270,7 +277,7 @@ __global__ void __launch_bounds__(MGE_SOLVE_THREADS) gram_mge_kernel(const KArgs
             const double wd = (double)fwv;
 #pragma unroll
             for (int u = 0; u < EPT; ++u) {
-                const int k = sk0 + u * (MGE_SOLVE_THREADS / MGE_TILE);
+                const int k = sk0 + u * (THREADS / MGE_TILE);
                 if (k < ncol) { const double v = (double)fv[u]; As[k][sii] = wd * v; Bs[k][sii] = v; }
             }
         }
@@ -313,40 +320,41 @@ __global__ void __launch_bounds__(MGE_SOLVE_THREADS) gram_mge_kernel(const KArgs
 // caller) and reports invalid rows.
 __global__ void __launch_bounds__(32 * MGE_NNLS_WARPS) nnls_mge_kernel(const KArgs a, int chunk_rows)
 {
-    constexpr int NCP = MGE_MAX_COL + 1;
-    __shared__ double Gw[MGE_NNLS_WARPS][MGE_GRAM_STRIDE];
-    __shared__ double Lw[MGE_NNLS_WARPS][MGE_MAX_COL * MGE_MAX_COL];
-    __shared__ double zw[MGE_NNLS_WARPS][MGE_MAX_COL], sw[MGE_NNLS_WARPS][MGE_MAX_COL];
+    // per warp (dynamic shared memory, sized by the actual column count n): G [n][n] | b [n] | L [n][n] | z [n] | s [n]
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int NCG = MGE_MAX_COL + 1;                          // row pitch of G in a.mge_gram
     const int wid = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int r = blockIdx.x * MGE_NNLS_WARPS + wid;
     if (r >= chunk_rows) return;
     const int64_t row = a.row0 + r;
     const int n = a.ext_nc;
+    double *Gs = reinterpret_cast<double *>(smem_raw) + (size_t)wid * (2 * n * n + 3 * n);
+    double *bs = Gs + n * n, *Ls = bs + n, *zs = Ls + n * n, *ss = zs + n;
     if (!row_is_valid(a.rows[r], a.n_comp)) {
         if (lane == 0) a.logL[row] = -INFINITY;
         if (a.amps && lane < n) a.amps[row * n + lane] = NAN;
         return;
     }
     const double *gin = a.mge_gram + (size_t)r * MGE_GRAM_STRIDE;
-    for (int e = lane; e < MGE_GRAM_STRIDE; e += 32) Gw[wid][e] = gin[e];
+    for (int e = lane; e < n * n; e += 32) Gs[e] = gin[(e / n) * NCG + (e % n)];
+    if (lane < n) bs[lane] = gin[MGE_MAX_COL * NCG + lane];
+    const double dwd = gin[MGE_MAX_COL * NCG + MGE_MAX_COL];
     __syncwarp();
-    if (lane == 0)
-        nnls_gram<MGE_MAX_COL>(n, Gw[wid], NCP, Gw[wid] + MGE_MAX_COL * NCP, Gw[wid][MGE_MAX_COL * NCP + MGE_MAX_COL], sw[wid], Lw[wid], zw[wid]);
+    if (lane == 0) nnls_gram<MGE_MAX_COL>(n, Gs, n, bs, dwd, ss, Ls, zs, n);
     __syncwarp();
-    if (lane < n && a.amps) a.amps[row * n + lane] = (float)sw[wid][lane];
+    if (lane < n && a.amps) a.amps[row * n + lane] = (float)ss[lane];
     if (lane == 0) {
         // chi^2 = d'Wd - 2 s'b + s'G s at the solved amplitudes (Eq. 5)
-        const double *G = Gw[wid], *b = Gw[wid] + MGE_MAX_COL * NCP;
         double sb = 0.0, sGs = 0.0;
         for (int i = 0; i < n; ++i) {
-            const double si = sw[wid][i];
+            const double si = ss[i];
             if (si == 0.0) continue;
-            sb += si * b[i];
+            sb += si * bs[i];
             double gi = 0.0;
-            for (int k = 0; k < n; ++k) gi += G[i * NCP + k] * sw[wid][k];
+            for (int k = 0; k < n; ++k) gi += Gs[i * n + k] * ss[k];
             sGs += si * gi;
         }
-        const double chi2 = (Gw[wid][MGE_MAX_COL * NCP + MGE_MAX_COL] - 2.0 * sb) + sGs;
+        const double chi2 = (dwd - 2.0 * sb) + sGs;
         a.logL[row] = (float)(-0.5 * (chi2 + a.lconst[row / a.rows_per_lens]));
     }
 }

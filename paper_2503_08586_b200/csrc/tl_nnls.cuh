@@ -15,10 +15,10 @@ namespace tl {
 // the passive set P grows by the column with the largest positive gradient w = b - G s, the
 // unconstrained problem on P is solved by Cholesky, and a step towards it that would leave the
 // feasible region is cut at the boundary, the columns that reach 0 leaving P.
-// G is [n][ldg]; L (scratch) [MAXC][MAXC]; z (scratch) [MAXC]; dwd = d'Wd sets the scale of "zero".
+// G is [n][ldg]; L (scratch) [n][ldl]; z (scratch) [n]; dwd = d'Wd sets the scale of "zero".
 template <int MAXC>
 __device__ inline void nnls_gram(int n, const double *G, int ldg, const double *b, double dwd, double *s,
-                                 double *L, double *z)
+                                 double *L, double *z, int ldl = MAXC)
 {
     int idx[MAXC];
     int m = 0;
@@ -46,23 +46,23 @@ __device__ inline void nnls_gram(int n, const double *G, int ldg, const double *
             for (int r = 0; r < m && pd; ++r) {
                 for (int c = 0; c <= r; ++c) {
                     double v = G[idx[r] * ldg + idx[c]];
-                    for (int k = 0; k < c; ++k) v -= L[r * MAXC + k] * L[c * MAXC + k];
+                    for (int k = 0; k < c; ++k) v -= L[r * ldl + k] * L[c * ldl + k];
                     if (c == r) {
                         if (!(v > 1e-13 * G[idx[r] * ldg + idx[r]])) { pd = false; break; }
-                        L[r * MAXC + r] = rsqrt(v);             // the diagonal is kept as 1 / l_rr
-                    } else L[r * MAXC + c] = v * L[c * MAXC + c];
+                        L[r * ldl + r] = rsqrt(v);             // the diagonal is kept as 1 / l_rr
+                    } else L[r * ldl + c] = v * L[c * ldl + c];
                 }
             }
             if (pd) {
                 for (int r = 0; r < m; ++r) {
                     double v = b[idx[r]];
-                    for (int k = 0; k < r; ++k) v -= L[r * MAXC + k] * z[k];
-                    z[r] = v * L[r * MAXC + r];
+                    for (int k = 0; k < r; ++k) v -= L[r * ldl + k] * z[k];
+                    z[r] = v * L[r * ldl + r];
                 }
                 for (int r = m - 1; r >= 0; --r) {
                     double v = z[r];
-                    for (int k = r + 1; k < m; ++k) v -= L[k * MAXC + r] * z[k];
-                    z[r] = v * L[r * MAXC + r];
+                    for (int k = r + 1; k < m; ++k) v -= L[k * ldl + r] * z[k];
+                    z[r] = v * L[r * ldl + r];
                 }
             }
             if (first) {
