@@ -294,3 +294,58 @@ def loglike_mge_batch(cfg: OrcConfig, psf, data, noise, rows, sigmas, n_lens: in
     lib().orc_loglike_mge_batch(C.byref(cfg), int(n_lens), _fp(p), int(p.shape[-1]), _fp(d), _fp(s), _fp(r), B,
                                 _fp(sg), int(sg.size), _dp(out), _dp(amps), int(threads))
     return out, amps
+
+
+# ---- NEXT-3, several Gaussian sets (isophote twists; G23) ----------
+# The row of a context with n_lens_light = n_sets carries one lens-light block per set; set j takes
+# its (e1, e2, cx, cy) from block j (entries +3..+6; I_e, r_e, n ignored).  Plain and slow, out of the
+# single-set pieces above: the columns of set j are the Gaussian columns of `mge_component_images`
+# on the single-set view of the row (lens | block j | sources); the sources come from the first view.
+# The NNLS optimum is taken by its definition (every support enumerated, orc_nnls_enum) up to 16
+# columns; beyond that 2^n supports are out of reach and the library routine scipy.optimize.nnls
+# (Lawson-Hanson on the whitened design matrix) serves as the step -- pinned against the enumeration
+# on random problems of <= 10 columns and against it on MGE problems of <= 16 columns
+# (tests/test_oracle_mge_pins.py).
+
+def _single_set_view(cfg: OrcConfig, row, j: int):
+    lp = 7 + (1 if cfg.mass_model == 1 else 0)
+    r = np.asarray(row, np.float32)
+    nll = cfg.n_lens_light
+    view = np.concatenate([r[:lp], r[lp + 7 * j: lp + 7 * (j + 1)], r[lp + 7 * nll:]]).astype(np.float32)
+    c1 = config(cfg.ny, cfg.nx, cfg.pix_scale, cfg.supersample, 1, cfg.n_source, cfg.edge_mode, cfg.mass_model)
+    return c1, view
+
+
+def mge_sets_component_images(cfg: OrcConfig, psf, row, sigma_sets):
+    """Columns of M: the Gaussians of set 0, of set 1, ..., then the sources; None for an invalid row."""
+    cols, src = [], None
+    for j, sg in enumerate(sigma_sets):
+        c1, view = _single_set_view(cfg, row, j)
+        if not lib().orc_mge_row_valid(C.byref(c1), _fp(_f32(view))):
+            return None
+        M = mge_component_images(c1, psf, view, sg)
+        cols.append(M[:len(sg)])
+        if src is None:
+            src = M[len(sg):]
+    return np.concatenate(cols + [src], axis=0)
+
+
+def nnls_design(A, y, enum_max: int = 16) -> np.ndarray:
+    """argmin ||A s - y||^2 over s >= 0: enumeration of supports up to enum_max columns, else scipy's nnls."""
+    A = np.asarray(A, np.float64); y = np.asarray(y, np.float64)
+    if A.shape[1] <= enum_max:
+        return nnls_enum(A.T @ A, A.T @ y)
+    from scipy.optimize import nnls as _nnls
+    return _nnls(A, y, maxiter=50 * A.shape[1])[0]
+
+
+def loglike_mge_sets(cfg: OrcConfig, psf, data, noise, row, sigma_sets, enum_max: int = 16):
+    """(logL of PAPER.md:82 Eq. 5 at the NNLS amplitudes of Eq. 6-7, amplitudes)."""
+    M = mge_sets_component_images(cfg, psf, row, sigma_sets)
+    n_col = sum(len(s) for s in sigma_sets) + cfg.n_source
+    if M is None:
+        return -np.inf, np.full(n_col, np.nan)
+    sig = np.asarray(noise, np.float64).reshape(-1)
+    A = (M.reshape(n_col, -1) / sig).T
+    s = nnls_design(A, np.asarray(data, np.float64).reshape(-1) / sig, enum_max)
+    return loglike_from_image(np.tensordot(s, M, axes=1), data, noise), s

@@ -116,7 +116,7 @@ def test_mge_recovers_known_amplitudes_and_flags_invalid_rows(api, orc):
     with pytest.raises(api.TinyLensError):
         ctx.set_mge(np.array([0.1, -0.2], np.float32))
     with pytest.raises(api.TinyLensError):
-        ctx.set_mge(np.full(17, 0.1, np.float32))
+        ctx.set_mge(np.full(31, 0.1, np.float32))          # more than 30 Gaussians
     ctx.set_mge(sigmas)
     ll, amps = ctx.loglike_mge(torch.from_numpy(rows).cuda())
     ll = ll.cpu().numpy(); amps = amps.cpu().numpy()
@@ -234,3 +234,84 @@ def test_mge_chunked_call_equals_single_chunk(api, orc):
     ctx.close(); ctx2.close()
     assert torch.equal(ll1, ll2) and torch.equal(am1.nan_to_num(-1.0), am2.nan_to_num(-1.0))
     assert ll1[5].item() == -np.inf
+
+
+# ---- several Gaussian sets with their own shapes (tl_set_mge_sets; "isophote twists") ----
+
+def _two_set_case(orc, n0, n1, ny=36, nx=44, S=2, K=7, batch=12):
+    w = W.Workload(index=9, name="mge-sets", ny=ny, nx=nx, pix_scale=0.12, supersample=S, psf_size=K,
+                   psf_kind="gaussian", psf_fwhm=0.3, psf_beta=0.0, n_lens_light=2, n_source=1,
+                   noise_bg=0.05, noise_exptime=100.0, source_amp=(1.0, 20.0), batch=batch)
+    w1 = W.Workload(**{**w.__dict__, "n_lens_light": 1})
+    rows = W.batch_rows(w, batch)
+    truth1 = np.concatenate([rows[0][:14], rows[0][21:]]).astype(np.float32)
+    prob = W.make_problem(w1, lambda ww, psf, row: orc.render_for_workloads(ww, psf, truth1))
+    prob = type(prob)(w, prob.psf, prob.data, prob.noise, rows[:1].copy())
+    sets = [W.mge_sigmas(w, n0), (W.mge_sigmas(w, n1) * 1.3).astype(np.float32)]
+    return w, prob, rows, sets
+
+
+@pytest.mark.parametrize("n0,n1", [(6, 5), (14, 12), (16, 14)])
+def test_mge_two_sets_match_oracle(api, orc, n0, n1):
+    """Two Gaussian sets, each on its own ellipses, 12 / 27 / 31 columns (the last two beyond what the
+    oracle can enumerate: scipy's NNLS is its step there, pinned against the enumeration on CPU).
+    Compared: logL, and the fitted image through the oracle's own columns."""
+    import torch
+    w, prob, rows, sets = _two_set_case(orc, n0, n1)
+    rows = rows.copy()
+    rows[3, 17] = 0.9; rows[3, 18] = 0.9                 # second set's shape invalid -> invalid row
+    rows[5, 7:10] = np.nan; rows[5, 14:17] = np.nan      # ignored entries of both blocks
+    ctx = api.LensContext.from_problem(prob)
+    ctx.set_mge_sets(sets)
+    n_col = n0 + n1 + 1
+    assert api.tl_mge_columns(ctx.handle) == n_col
+    d = torch.from_numpy(rows).cuda()
+    ll, amps = ctx.loglike_mge(d)
+    ll2, _ = ctx.loglike_mge(d, want_amps=False)
+    # a context with two lens-light blocks serves the MGE call only
+    with pytest.raises(api.TinyLensError):
+        ctx.loglike(d)
+    with pytest.raises(api.TinyLensError):
+        ctx.set_mge(sets[0])
+    ctx.close()
+    assert torch.equal(ll, ll2)
+    ll = ll.cpu().numpy().astype(np.float64); amps = amps.cpu().numpy().astype(np.float64)
+    cfg = orc.config_of(w)
+    worst, worst_fit = 0.0, 0.0
+    for r in range(len(rows)):
+        oll, oamps = orc.loglike_mge_sets(cfg, prob.psf[0], prob.data[0], prob.noise[0], rows[r], sets)
+        if r == 3:
+            assert oll == -np.inf and ll[r] == -np.inf and np.all(np.isnan(amps[r]))
+            continue
+        assert np.isfinite(ll[r]) and np.all(amps[r] >= 0.0)
+        tol = max(PT.LOGL_ABS, PT.LOGL_REL * abs(oll))
+        worst = max(worst, abs(ll[r] - oll) / tol)
+        M = orc.mge_sets_component_images(cfg, prob.psf[0], rows[r], sets)
+        oimg, gimg = np.tensordot(oamps, M, axes=1), np.tensordot(amps[r], M, axes=1)
+        worst_fit = max(worst_fit, np.abs(gimg - oimg).max() / oimg.max())
+        # the GPU's amplitudes, through the oracle's columns, reach the oracle's optimum
+        ll_at = orc.loglike_from_image(gimg, prob.data[0], prob.noise[0])
+        assert oll - ll_at <= PT.near_bound_fp32(PT.FP32_MGE_MEASURED) * tol, (r, oll - ll_at, tol)
+    print("two sets (%d + %d Gaussians, %d columns): logL %.3g x north_star, fitted image %.2e x peak" % (n0, n1, n_col, worst, worst_fit))
+    assert worst <= PT.near_bound_fp32(PT.FP32_MGE_MEASURED) and worst_fit <= 1e-4
+
+
+def test_mge_two_identical_sets_equal_one_set(api, orc):
+    """Two sets with the same shape = one set with the dispersions concatenated (logL to FP32 noise;
+    the Gaussians are evaluated by the same kernel either way)."""
+    import torch
+    w, prob, rows, sets = _two_set_case(orc, 4, 3)
+    rows = rows.copy()
+    rows[:, 14:21] = rows[:, 7:14]
+    ctx2 = api.LensContext.from_problem(prob)
+    ctx2.set_mge_sets(sets)
+    ll2, a2 = ctx2.loglike_mge(torch.from_numpy(rows).cuda())
+    ctx2.close()
+    w1 = W.Workload(**{**w.__dict__, "n_lens_light": 1})
+    prob1 = type(prob)(w1, prob.psf, prob.data, prob.noise, prob.truth)
+    rows1 = np.ascontiguousarray(np.concatenate([rows[:, :14], rows[:, 21:]], axis=1))
+    ctx1 = api.LensContext.from_problem(prob1)
+    ctx1.set_mge(np.concatenate(sets))
+    ll1, a1 = ctx1.loglike_mge(torch.from_numpy(rows1).cuda())
+    ctx1.close()
+    assert torch.equal(ll1, ll2) and torch.equal(a1, a2)

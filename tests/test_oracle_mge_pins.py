@@ -138,3 +138,68 @@ def test_mge_likelihood_is_the_maximum_over_amplitudes(orc):
     ll2, a2 = orc.loglike_linear(cfg, prob.psf[0], prob.data[0], prob.noise[0], row)
     assert abs(ll1 - ll2) <= 2e-5 * abs(ll2)
     assert np.allclose(a1, [2 * a2[0], a2[1]], rtol=1e-4, atol=1e-6)
+
+
+# ---- several Gaussian sets (oracle.loglike_mge_sets) -------------------------------------------
+
+def _two_set_problem(orc):
+    w = W.Workload(index=9, name="mge2", ny=20, nx=24, pix_scale=0.15, supersample=2, psf_size=5,
+                   psf_kind="gaussian", psf_fwhm=0.3, psf_beta=0.0, n_lens_light=2, n_source=1,
+                   noise_bg=0.05, noise_exptime=100.0, source_amp=(1.0, 20.0), batch=4)
+    w1 = W.Workload(**{**w.__dict__, "n_lens_light": 1})
+    rows = W.batch_rows(w, 4)
+    # mock data from a single-Sersic lens light (the first lens-light block) + source
+    truth1 = np.concatenate([rows[0][:14], rows[0][21:]]).astype(np.float32)
+    prob1 = W.make_problem(w1, lambda ww, psf, row: orc.render_for_workloads(ww, psf, truth1))
+    return w, prob1, rows
+
+
+def test_two_identical_sets_equal_one_set(orc):
+    """Sets that share shape and centre are one set with the dispersions concatenated."""
+    w, prob, rows = _two_set_problem(orc)
+    cfg = orc.config_of(w)
+    row = rows[1].copy()
+    row[14:21] = row[7:14]                                   # block 1 := block 0
+    s0, s1 = np.array([0.1, 0.4], np.float32), np.array([0.2, 0.9, 2.0], np.float32)
+    ll2, a2 = orc.loglike_mge_sets(cfg, prob.psf[0], prob.data[0], prob.noise[0], row, [s0, s1])
+    w1 = W.Workload(**{**w.__dict__, "n_lens_light": 1})
+    row1 = np.concatenate([row[:14], row[21:]]).astype(np.float32)
+    ll1, a1 = orc.loglike_mge(orc.config_of(w1), prob.psf[0], prob.data[0], prob.noise[0], row1, np.concatenate([s0, s1]))
+    assert abs(ll2 - ll1) <= 1e-9 * abs(ll1) and np.allclose(a2, a1, rtol=1e-6, atol=1e-9 * a1.max())
+
+
+def test_second_set_uses_its_own_shape(orc):
+    """The columns of set 1 are Gaussians on ITS ellipses: equal to the single-set columns of a row
+    that carries block 1 as its lens light, and different from set 0's when the shapes differ."""
+    w, prob, rows = _two_set_problem(orc)
+    cfg = orc.config_of(w)
+    row = rows[2]
+    sg = np.array([0.3, 1.0], np.float32)
+    M = orc.mge_sets_component_images(cfg, prob.psf[0], row, [sg, sg])
+    assert M.shape == (5, w.ny, w.nx)
+    w1 = W.Workload(**{**w.__dict__, "n_lens_light": 1})
+    rowb = np.concatenate([row[:7], row[14:21], row[21:]]).astype(np.float32)
+    Mb = orc.mge_component_images(orc.config_of(w1), prob.psf[0], rowb, sg)
+    assert np.array_equal(M[2:4], Mb[:2]) and np.array_equal(M[4], Mb[2])
+    assert np.abs(M[0] - M[2]).max() > 1e-3 * M[0].max()
+    # invalid second shape -> invalid row
+    bad = row.copy(); bad[17] = 0.9; bad[18] = 0.8
+    ll, amps = orc.loglike_mge_sets(cfg, prob.psf[0], prob.data[0], prob.noise[0], bad, [sg, sg])
+    assert ll == -np.inf and np.all(np.isnan(amps))
+
+
+def test_library_nnls_equals_enumeration_on_mge_problems(orc):
+    """Beyond 16 columns the oracle takes scipy.optimize.nnls as its step; on MGE problems small
+    enough to enumerate (12 nearly collinear columns) both give the same logL and fitted image."""
+    w, prob, rows = _two_set_problem(orc)
+    cfg = orc.config_of(w)
+    sets = [W.mge_sigmas(w, 6), W.mge_sigmas(w, 5)]
+    for r in range(3):
+        ll_e, a_e = orc.loglike_mge_sets(cfg, prob.psf[0], prob.data[0], prob.noise[0], rows[r], sets, enum_max=16)
+        ll_s, a_s = orc.loglike_mge_sets(cfg, prob.psf[0], prob.data[0], prob.noise[0], rows[r], sets, enum_max=0)
+        assert np.all(a_e >= 0) and np.all(a_s >= 0)
+        assert abs(ll_e - ll_s) <= 1e-8 * abs(ll_e) + 1e-6, (ll_e, ll_s)
+        M = orc.mge_sets_component_images(cfg, prob.psf[0], rows[r], sets)
+        fe, fs = np.tensordot(a_e, M, axes=1), np.tensordot(a_s, M, axes=1)
+        assert np.abs(fe - fs).max() <= 1e-6 * np.abs(fe).max()
+        assert ll_e >= ll_s - 1e-6                          # the enumeration is the exact optimum
