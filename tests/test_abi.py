@@ -63,7 +63,7 @@ def test_create_rejects_bad_arguments_before_cuda(api):
     psf, data, noise = _args()
     bad = [
         dict(ny=0), dict(nx=-1), dict(pix_scale=0.0), dict(pix_scale=float("nan")), dict(supersample=0),
-        dict(supersample=17), dict(n_lens_light=2), dict(n_source=0), dict(n_source=3), dict(edge_mode=2),
+        dict(supersample=17), dict(n_lens_light=3), dict(n_lens_light=-1), dict(n_source=0), dict(n_source=3), dict(edge_mode=2),
         dict(n_lens=0), dict(mass_model=2), dict(mass_model=-1),
     ]
     base = dict(ny=8, nx=8, pix_scale=0.1, supersample=2, n_lens_light=0, n_source=1, edge_mode=0, n_lens=1,
@@ -111,6 +111,8 @@ def test_null_context_calls_are_errors_not_crashes(api):
     # MGE entry points (NEXT-3)
     sg = np.array([0.1, 0.3], np.float32)
     assert lib.tl_set_mge(None, sg.ctypes.data_as(C.POINTER(C.c_float)), 2) == api.TL_EINVAL
+    per = (C.c_int32 * 2)(1, 1)
+    assert lib.tl_set_mge_sets(None, sg.ctypes.data_as(C.POINTER(C.c_float)), per, 2) == api.TL_EINVAL
     assert lib.tl_mge_columns(None) < 0
     assert lib.tl_mge_chunk_rows(None) < 0
     assert lib.tl_loglike_mge_batch(None, None, 4, None, None, None) == api.TL_EINVAL
