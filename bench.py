@@ -533,7 +533,7 @@ def run_linear(args, w: W.Workload):
 
     prob = W.make_problem(w, gpu_render)
     ctx = api.LensContext.from_problem(prob)
-    if args.precision != "fp32" and args.mode == "linear":
+    if args.precision != "fp32" and args.mode in ("linear", "mge"):
         ctx.set_precision({"fp64": api.TL_PRECISION_FP64, "fp64-libm": api.TL_PRECISION_FP64_LIBM, "auto": api.TL_PRECISION_AUTO}[args.precision])
     rows = W.batch_rows(w)
     B = rows.shape[0]

@@ -312,9 +312,10 @@ int tl_wait(tl_ctx *ctx, int slot);
 
 /*
  * tl_set_precision -- choose the arithmetic of later tl_loglike_batch / tl_render_batch /
- * tl_loglike_batch_host(_async) / tl_loglike_linear_batch calls on this context (tl_loglike_mge_batch
- * has FP32 kernels only).  In tl_loglike_linear_batch both TL_PRECISION_FP64 and TL_PRECISION_AUTO
- * run the FP64 pipeline on every row (with solved amplitudes every row is near its best fit).
+ * tl_loglike_batch_host(_async) / tl_loglike_linear_batch / tl_loglike_mge_batch calls on this context.
+ * In the two linear-amplitude calls both TL_PRECISION_FP64 and TL_PRECISION_AUTO run the FP64 pipeline
+ * on every row (with solved amplitudes every row is near its best fit); TL_PRECISION_FP64_LIBM is the
+ * FP32 pipeline there.
  *   TL_PRECISION_FP32 (default)  the FP32 kernels: meet the tolerances of DESIGN.md "Tolerances"
  *   TL_PRECISION_FP64            the same forward model in double precision on the device, about
  *                                ten times slower; agrees with an FP64 CPU evaluation to ~1e-9

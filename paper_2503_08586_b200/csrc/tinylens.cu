@@ -53,6 +53,7 @@ struct tl_ctx {
     size_t dp_conv_smem = 0;
     int64_t dp_chunk_rows = 0;
     void (*dp_trace)(const tl::DpArgs) = nullptr;
+    void (*mge_dp_trace)(const tl::DpArgs) = nullptr;   // FP64 MGE pipeline: the sources only (NLL = 0)
     double *lconst = nullptr;
     double lconst0 = 0.0, sigma_min0 = 0.0;
     // launch geometry
@@ -690,6 +691,7 @@ int tl_create_ex(tl_ctx **out, const tl_config *cfg, const float *psf_in, int32_
         }
         if (best > 0.0) {
             c->dp_trace = tl_trace_dp_for(cfg->supersample, cfg->n_lens_light, cfg->n_source);
+            c->mge_dp_trace = tl_trace_dp_for(cfg->supersample, 0, cfg->n_source);
             int occ = 0;
             bool okd = cuda_ok(cudaFuncSetAttribute(tl::conv_dp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SMEM_LIMIT - 1024))) &&
                        cuda_ok(cudaFuncSetAttribute(tl::conv_dp_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared)) &&
@@ -899,6 +901,81 @@ int64_t tl_mge_chunk_rows(const tl_ctx *c) { return (c && c->n_gauss > 0) ? mge_
 
 int tl_mge_columns(const tl_ctx *c) { return (c && c->n_gauss > 0) ? c->n_gauss + c->cfg.n_source : TL_EINVAL; }
 
+namespace {
+// tl_loglike_mge_batch in FP64 (TL_PRECISION_FP64 / AUTO: with solved amplitudes every row is near its best
+// fit): the sources through trace_dp_kernel<S,0,NSRC> with the components apart, the Gaussians by
+// gauss_dp_kernel, every column blurred by conv_dp_kernel, then the Gram / NNLS kernels of tl_mge.cuh on
+// the FP64 columns.  The FP32 prologue also runs: the solver kernels take the row validity from RowC.
+int run_mge_dp(tl_ctx *c, const float *params, int64_t B, float *logL, float *amps, cudaStream_t st)
+{
+    const int NG = c->n_gauss, NS = c->cfg.n_source, NC = NG + NS;
+    const size_t npix = (size_t)c->cfg.ny * c->cfg.nx;
+    const size_t ext_row = sizeof(double) * (size_t)NC * c->He * c->dp_Wp, m_row = sizeof(double) * NC * npix;
+    int64_t chunk = (int64_t)(MGE_SCRATCH_BYTES / (ext_row + m_row));
+    if (chunk < 1) chunk = 1;
+    if (chunk > 65535) chunk = 65535;
+    if (c->opt.mge_chunk_rows >= 1 && c->opt.mge_chunk_rows < chunk) chunk = c->opt.mge_chunk_rows;
+    if (chunk > B) chunk = B;
+    tl::RowC *rows = nullptr;
+    tl::RowD *rowsd = nullptr;
+    double *ext = nullptr, *m64 = nullptr, *gram = nullptr;
+    const size_t g_row = sizeof(double) * tl::MGE_GRAM_STRIDE;
+    if (!pool_alloc(c, &rows, sizeof(tl::RowC) * (size_t)chunk, st) || !pool_alloc(c, &rowsd, sizeof(tl::RowD) * (size_t)chunk, st) ||
+        !pool_alloc(c, &ext, ext_row * (size_t)chunk, st) || !pool_alloc(c, &m64, m_row * (size_t)chunk, st) ||
+        !pool_alloc(c, &gram, g_row * (size_t)chunk, st)) {
+        if (rows) cudaFreeAsync(rows, st);
+        if (rowsd) cudaFreeAsync(rowsd, st);
+        if (ext) cudaFreeAsync(ext, st);
+        if (m64) cudaFreeAsync(m64, st);
+        return TL_ENOMEM;
+    }
+    if (c->dp_Wp != c->We) cudaMemsetAsync(ext, 0, ext_row * (size_t)chunk, st);     // pitch padding must be finite
+    const int64_t rows_per_lens = B / c->cfg.n_lens;
+    int rc = TL_OK;
+    for (int64_t r0 = 0; r0 < B && rc == TL_OK; r0 += chunk) {
+        const int64_t nb = (B - r0 < chunk) ? (B - r0) : chunk;
+        tl::PrologueArgs pa;
+        fill_prologue_args(c, pa, params, rows, nb, r0, rows_per_lens, 1);
+        pa.mge = 1;
+        tl::prologue_kernel<<<(unsigned)((nb * (1 + c->n_comp) + 127) / 128), 128, 0, st>>>(pa);
+        tl::DpArgs d;
+        memset(&d, 0, sizeof(d));
+        d.params = params; d.rows = rowsd; d.n_rows = (int)nb; d.row0 = r0; d.rows_per_lens = rows_per_lens;
+        d.psf = c->psf; d.data = c->data; d.wgt64 = c->wgt64; d.lconst = c->lconst;
+        d.ext = ext; d.m64 = m64; d.logL = logL; d.amps = amps; d.lin = 1; d.mge = 1;
+        d.ext_nc = NC; d.ext_k0 = NG; d.n_gauss = NG; d.n_source = NS; d.mge_c = c->mge_c; d.mge_set = c->mge_set;
+        d.P = c->P; d.ny = c->cfg.ny; d.nx = c->cfg.nx; d.K = c->K; d.Kp = c->Kp; d.h = c->h;
+        d.He = c->He; d.We = c->We; d.Wp = c->dp_Wp; d.S = c->cfg.supersample;
+        d.n_lens_light = c->cfg.n_lens_light; d.n_comp = c->n_comp;
+        d.edge_zero = c->cfg.edge_mode == TL_EDGE_ZERO; d.mass_model = c->cfg.mass_model; d.lens_np = c->lens_np;
+        d.band_rows = c->dp_band_rows; d.n_bands = c->dp_n_bands;
+        d.CW = c->CW; d.CH = c->CH; d.tiles_x = (c->We + c->CW - 1) / c->CW; d.tiles_y = (c->He + c->CH - 1) / c->CH;
+        d.u = c->cfg.pix_scale / (2.0 * c->cfg.supersample);
+        tl::prologue_dp_kernel<<<(unsigned)((nb + 63) / 64), 64, 0, st>>>(d);
+        const int64_t items = nb * d.tiles_x * d.tiles_y;
+        int grid = c->dp_trace_grid;
+        if ((int64_t)grid * 8 > items) grid = (int)((items + 7) / 8);
+        c->mge_dp_trace<<<grid, 256, 0, st>>>(d);
+        int gslabs = (int)(((int64_t)c->He * c->We * NG + 255) / 256);
+        if (gslabs > 64) gslabs = 64;
+        tl::gauss_dp_kernel<<<dim3((unsigned)nb, (unsigned)gslabs), 256, 0, st>>>(d);
+        if (c->profile) cudaEventRecord(c->ev0, st);
+        tl::conv_dp_kernel<<<dim3((unsigned)nb, (unsigned)c->dp_n_bands, (unsigned)NC), c->dp_conv_threads, c->dp_conv_smem, st>>>(d);
+        if (c->profile) { cudaEventRecord(c->ev1, st); c->prof_pending = 1; }
+        tl::KArgs a = base_args(c);
+        a.rows = rows; a.B = nb; a.rows_per_lens = rows_per_lens; a.row0 = r0;
+        a.logL = logL; a.amps = amps; a.ext_nc = NC; a.mimg64 = m64; a.wgt64 = c->wgt64; a.mge_gram = gram;
+        if (NC + 1 <= 20) tl::gram_mge_kernel<128, double><<<(unsigned)nb, 128, 0, st>>>(a, (int)nb);
+        else tl::gram_mge_kernel<512, double><<<(unsigned)nb, 512, 0, st>>>(a, (int)nb);
+        const size_t nnls_smem = sizeof(double) * tl::MGE_NNLS_WARPS * (size_t)(2 * NC * NC + 3 * NC);
+        tl::nnls_mge_kernel<<<(unsigned)((nb + tl::MGE_NNLS_WARPS - 1) / tl::MGE_NNLS_WARPS), 32 * tl::MGE_NNLS_WARPS, nnls_smem, st>>>(a, (int)nb);
+        if (!cuda_ok(cudaGetLastError())) rc = TL_ECUDA;
+    }
+    cudaFreeAsync(rows, st); cudaFreeAsync(rowsd, st); cudaFreeAsync(ext, st); cudaFreeAsync(m64, st); cudaFreeAsync(gram, st);
+    return rc;
+}
+}  // namespace
+
 int tl_loglike_mge_batch(tl_ctx *c, const float *params, int64_t B, float *logL, float *amps, void *cuda_stream)
 {
     if (!c || B < 0) return TL_EINVAL;
@@ -909,6 +986,10 @@ int tl_loglike_mge_batch(tl_ctx *c, const float *params, int64_t B, float *logL,
     cudaStream_t st = (cudaStream_t)cuda_stream;
     DeviceGuard guard(c->device);
     if (!guard.ok) return TL_ECUDA;
+    if (c->precision == TL_PRECISION_FP64 || c->precision == TL_PRECISION_AUTO) {
+        if (!c->mge_dp_trace) return TL_ESIZE;
+        return run_mge_dp(c, params, B, logL, amps, st);
+    }
     const int NG = c->n_gauss, NS = c->cfg.n_source, NC = NG + NS;
     const int fused = c->mge_fused;
     const size_t npix = (size_t)c->cfg.ny * c->cfg.nx;

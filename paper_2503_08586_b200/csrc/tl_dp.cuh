@@ -76,6 +76,12 @@ struct DpArgs {
     int lin;                     // 1: ext is [chunk][n_comp][He][Wp], unit amplitudes; conv writes m64
     double *m64;                 // [chunk][n_comp][ny][nx] blurred unit-amplitude component images (columns of M)
     float *amps;                 // [B][n_comp] or null
+    // MGE mode in FP64 (tl_loglike_mge_batch under TL_PRECISION_FP64): RowD holds the sources first, then the
+    // shapes of the Gaussian sets (r_e := 1: t = R_p^2 in arcsec^2); ext / m64 have ext_nc = n_gauss + n_source
+    // components per row, the ray-traced sources from slot ext_k0 = n_gauss on
+    int mge, ext_nc, ext_k0, n_gauss, n_source;
+    const float *mge_c;          // [n_gauss] log2(e) / (2 sigma_k^2)
+    const int *mge_set;          // [n_gauss] set of Gaussian k
     int P, ny, nx, K, Kp, h, He, We, Wp, S, n_lens_light, n_comp, edge_zero, mass_model, lens_np;
     int band_rows, n_bands;
     int CW, CH, tiles_x, tiles_y;
@@ -255,13 +261,22 @@ __global__ void __launch_bounds__(64) prologue_dp_kernel(const DpArgs a)
     bool all_ok = ok;
     for (int k = 0; k < a.n_comp; ++k) {
         const float *sp = p + LP + 7 * k;
-        CompD &C = R.comp[k];
+        // MGE order: sources first (what the NLL = 0 trace kernel reads), then the sets' shapes
+        CompD &C = R.comp[a.mge ? (k < a.n_lens_light ? a.n_comp - a.n_lens_light + k : k - a.n_lens_light) : k];
         bool okc = true;
         for (int i = 0; i < 7; ++i) okc = okc && isfinite(sp[i]);
         double qs = 1.0, cs = 1.0, ss = 0.0;
         if (a.lin) { okc = true; for (int i = 1; i < 7; ++i) okc = okc && isfinite(sp[i]); }
-        okc = okc && (sp[1] > 0.f) && (sp[2] > 0.f) && shape_from_e(sp[3], sp[4], &qs, &cs, &ss);
-        const double Ie = a.lin ? 1.0 : (okc ? (double)sp[0] : 0.0), re = okc ? (double)sp[1] : 1.0, n = okc ? (double)sp[2] : 1.0;
+        const bool set_shape = a.mge && k < a.n_lens_light;       // MGE: only e1, e2, cx, cy of a lens-light block are read
+        if (set_shape) {
+            okc = true;
+            for (int i = 3; i < 7; ++i) okc = okc && isfinite(sp[i]);
+            okc = okc && shape_from_e(sp[3], sp[4], &qs, &cs, &ss);
+        } else {
+            okc = okc && (sp[1] > 0.f) && (sp[2] > 0.f) && shape_from_e(sp[3], sp[4], &qs, &cs, &ss);
+        }
+        const double Ie = a.lin ? 1.0 : (okc ? (double)sp[0] : 0.0);
+        const double re = (okc && !set_shape) ? (double)sp[1] : 1.0, n = (okc && !set_shape) ? (double)sp[2] : 1.0;
         if (!okc) { qs = 1.0; cs = 1.0; ss = 0.0; }
         const double bn = sersic_bn(n);
         const double A = qs / (re * re), Bq = 1.0 / (qs * re * re);     // Eq. 10: t = A x1^2 + B x2^2
@@ -400,10 +415,49 @@ __global__ void __launch_bounds__(256, 2) trace_dp_kernel(const DpArgs a)
         }
         if (a.lin) {
 #pragma unroll
-            for (int k = 0; k < NLL + NSRC; ++k) a.ext[(((size_t)r * (NLL + NSRC) + k) * a.He + i) * a.Wp + j] = comp_out[k];
+            for (int k = 0; k < NLL + NSRC; ++k)
+                a.ext[(((size_t)r * (a.ext_nc ? a.ext_nc : NLL + NSRC) + a.ext_k0 + k) * a.He + i) * a.Wp + j] = comp_out[k];
         } else {
             a.ext[((size_t)r * a.He + i) * a.Wp + j] = acc;
         }
+    }
+}
+
+// ---- MGE in FP64: the binned unit-amplitude Gaussians (reading G23) --------------
+// one thread per (row, extended pixel, Gaussian): exp(-R_p^2 / 2 sigma_k^2) = 2^(-t c_k) at every sub-sample
+__global__ void __launch_bounds__(256) gauss_dp_kernel(const DpArgs a)
+{
+    __shared__ double etab[DP_EXP_N];
+    for (int i = threadIdx.x; i < DP_EXP_N; i += blockDim.x) etab[i] = DP_EXP_TABLE[i];
+    __syncthreads();
+    DpTabs tb;
+    tb.ltab = 0; tb.etab = (unsigned)__cvta_generic_to_shared(etab);
+    const int n_rows = dp_n_rows(a);
+    const int r = blockIdx.x;
+    if (r >= n_rows || !a.rows[r].valid) return;
+    const RowD &R = a.rows[r];
+    const int S = a.S, npx = a.He * a.We;
+    const double u = a.u, du = 2.0 * u, inv_s2 = 1.0 / (double)(S * S);
+    for (int w = blockIdx.y * blockDim.x + threadIdx.x; w < npx * a.n_gauss; w += gridDim.y * blockDim.x) {
+        const int k = w / npx, pix = w - k * npx, i = pix / a.We, j = pix - i * a.We;
+        const CompD &C = R.comp[a.n_source + a.mge_set[k]];
+        const double ck = -(double)a.mge_c[k];
+        double acc = 0.0;
+        const bool edge = a.edge_zero && (j < a.h || j >= a.We - a.h || i < a.h || i >= a.He - a.h);
+        if (!edge) {
+            const double dx0 = (double)(2 * j * S + 1 - S * a.We) * u - C.ox;
+            double dy = (double)(2 * i * S + 1 - S * a.He) * u - C.oy;
+            for (int sa = 0; sa < S; ++sa, dy += du) {
+                const double LC = C.cc * dy * dy, LBy = C.b2 * dy;
+                double dx = dx0;
+                for (int sb = 0; sb < S; ++sb, dx += du) {
+                    double x = fma(dx, fma(C.a, dx, LBy), LC) * ck;
+                    x = x < -1100.0 ? -1100.0 : x;
+                    acc += dp_exp2(x, tb);
+                }
+            }
+        }
+        a.ext[(((size_t)r * a.ext_nc + k) * a.He + i) * a.Wp + j] = acc * inv_s2;
     }
 }
 

@@ -50,6 +50,8 @@ struct KArgs {
     const int *mge_set;      // [n_gauss] the set (0 .. n_lens_light-1) Gaussian k belongs to: its shape is comp[n_source + set]
     int mge_k0, mge_shape;   // mge_gauss_kernel (unfused path, one launch per set): first Gaussian and set of this launch
     double *mge_gram;        // [chunk][MGE_GRAM_STRIDE]  G | b | d'Wd
+    const double *mimg64;    // FP64 MGE pipeline: [chunk][C][ny][nx] blurred columns in double, and
+    const double *wgt64;     //                    [n_lens][ny][nx] 1 / sigma^2 in double
     // conv_lin_kernel: component strides of ext and of mimg, first mimg slot (0, 0, 0 = gridDim.z, gridDim.z, 0)
     int conv_ext_nc, conv_m_nc, conv_m_k0;
 };

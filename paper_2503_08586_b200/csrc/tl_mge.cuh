@@ -216,7 +216,8 @@ inline mge_gauss_fn mge_gauss_for(int ng)
 // memory MGE_TILE at a time (w m_k and m_k, d as doubles, the next tile prefetched into registers);
 // every sum has a fixed order, so the result is bitwise reproducible.
 // Output: a.mge_gram[r][MGE_GRAM_STRIDE].
-template <int THREADS>
+// T = float: the FP32 pipeline's columns and weights; T = double: the FP64 pipeline's (a.mimg64, a.wgt64).
+template <int THREADS, typename T = float>
 __global__ void __launch_bounds__(THREADS) gram_mge_kernel(const KArgs a, int chunk_rows)
 {
     constexpr int NCP = MGE_MAX_COL + 2;               // columns + data, rounded up to even
@@ -233,8 +234,9 @@ __global__ void __launch_bounds__(THREADS) gram_mge_kernel(const KArgs a, int ch
     if (!row_is_valid(a.rows[r], a.n_comp)) return;   // nnls_mge_kernel reports the row
     const int64_t lens = row / a.rows_per_lens;
     const int npix = a.ny * a.nx;
-    const float *M = a.mimg + (size_t)r * n * npix;
-    const float *d = a.data + lens * (size_t)npix, *w = a.wgt + lens * (size_t)npix;
+    const T *M = (sizeof(T) == 8 ? reinterpret_cast<const T *>(a.mimg64) : reinterpret_cast<const T *>(a.mimg)) + (size_t)r * n * npix;
+    const float *d = a.data + lens * (size_t)npix;
+    const T *w = (sizeof(T) == 8 ? reinterpret_cast<const T *>(a.wgt64) : reinterpret_cast<const T *>(a.wgt)) + lens * (size_t)npix;
     double *gout = a.mge_gram + (size_t)r * MGE_GRAM_STRIDE;
     // [G | b | d'Wd] = A'B with A = [w m_k | w d], B = [m_k | d]  (n1 = n + 1 columns, the data last).
     // Register blocking: a thread owns a 2 x 2 block of entries (columns 2bi, 2bi+1 of A against
@@ -259,15 +261,15 @@ __global__ void __launch_bounds__(THREADS) gram_mge_kernel(const KArgs a, int ch
     static_assert(THREADS % MGE_TILE == 0, "a thread stages one pixel of the tile");
     const int ncol = 2 * NB;                                      // n1 rounded up to even: a zero column
     const int sii = threadIdx.x % MGE_TILE, sk0 = threadIdx.x / MGE_TILE;
-    float fv[EPT], fwv = 0.f;
+    T fv[EPT], fwv = (T)0;
     auto fetch = [&](int t0) {
         const int i = t0 + sii;
-        fwv = i < npix ? w[i] : 0.f;
+        fwv = i < npix ? w[i] : (T)0;
 #pragma unroll
         for (int u = 0; u < EPT; ++u) {
             const int k = sk0 + u * (THREADS / MGE_TILE);
-            fv[u] = 0.f;
-            if (k < n1 && i < npix) fv[u] = k < n ? M[(size_t)k * npix + i] : d[i];
+            fv[u] = (T)0;
+            if (k < n1 && i < npix) fv[u] = k < n ? M[(size_t)k * npix + i] : (T)d[i];
         }
     };
     fetch(0);

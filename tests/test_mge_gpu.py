@@ -18,10 +18,14 @@ def api():
     return _api
 
 
-def _check(api, orc, w, prob, rows, sigmas, amp_rtol=None):
+def _check(api, orc, w, prob, rows, sigmas, amp_rtol=None, precision=0):
+    """precision 0: the FP32 pipeline, held to NEAR_MARGIN x its measured worst (every MGE row is near its
+    best fit); TL_PRECISION_FP64 / AUTO: the FP64 pipeline, north_star as stated on every row."""
     import torch
     ctx = api.LensContext.from_problem(prob)
     ctx.set_mge(sigmas)
+    ctx.set_precision(precision)
+    bound = PT.near_bound_fp32(PT.FP32_MGE_MEASURED) if precision == 0 else 1.0
     d = torch.from_numpy(rows).cuda()
     ll, amps = ctx.loglike_mge(d)
     ll2, _ = ctx.loglike_mge(d, want_amps=False)
@@ -50,16 +54,17 @@ def _check(api, orc, w, prob, rows, sigmas, amp_rtol=None):
         gimg = np.tensordot(amps[r], M, axes=1)
         ll_at = orc.loglike_from_image(gimg, prob.data[lens[r]], prob.noise[lens[r]])
         assert ll_at <= oll[r] + 1e-9 * abs(oll[r])                 # the oracle's is the maximum
-        assert oll[r] - ll_at <= PT.near_bound_fp32(PT.FP32_MGE_MEASURED) * tol[r], (r, oll[r] - ll_at, tol[r])
+        assert oll[r] - ll_at <= bound * tol[r], (r, oll[r] - ll_at, tol[r])
         worst_fit = max(worst_fit, np.abs(gimg - oimg).max() / oimg.max())
     assert worst_fit <= 1e-4, worst_fit                             # fitted image, relative to its peak
     tn = np.maximum(tol, floors)
-    assert (dl / tol).max() <= PT.near_bound_fp32(PT.FP32_MGE_MEASURED), "MGE logL parity: worst %.3g x north_star" % (dl / tol).max()
+    tolf = tol + np.abs(oll) * 2.0 ** -24                           # the result is returned as float
+    assert (dl / tolf).max() <= bound, "MGE logL parity (precision %d): worst %.3g x north_star" % (precision, (dl / tolf).max())
     if amp_rtol is not None:
         scale = np.maximum(np.abs(oamps).max(axis=1, keepdims=True), 1e-30)
         assert np.all(np.abs(amps - oamps) <= amp_rtol * scale), np.abs((amps - oamps) / scale).max()
-    print("%s MGE (%d columns): logL %.3g x north-star tol, %.3g x derived; fitted image %.2e x peak"
-          % (w.name, n_col, (dl / tol).max(), (dl / tn).max(), worst_fit))
+    print("%s MGE (%d columns, precision %d): logL %.3g x north-star tol, %.3g x derived; fitted image %.2e x peak"
+          % (w.name, n_col, precision, (dl / tol).max(), (dl / tn).max(), worst_fit))
     return ll, amps, oll, oamps
 
 
@@ -74,14 +79,16 @@ def test_mge_small_image_well_separated_set(api, orc):
     rows[::2, 14] = np.nan
     sigmas = np.array([0.1, 0.3, 0.9, 2.7], np.float32)
     _check(api, orc, w, prob, rows, sigmas, amp_rtol=2e-4)
+    _check(api, orc, w, prob, rows, sigmas, amp_rtol=1e-6, precision=api.TL_PRECISION_FP64)
 
 
+@pytest.mark.parametrize("precision", [0, 1, 3])
 @pytest.mark.parametrize("idx,n_prior,n_near,n_lens,n_gauss", [(1, 6, 6, 1, 10), (3, 4, 4, 3, 8), (4, 1, 1, 1, 6)])
-def test_mge_matches_oracle_on_configs(api, orc, idx, n_prior, n_near, n_lens, n_gauss):
+def test_mge_matches_oracle_on_configs(api, orc, idx, n_prior, n_near, n_lens, n_gauss, precision):
     w = W.workload(idx).scaled(batch=n_lens * n_prior, n_lens=n_lens)
     prob = W.make_problem(w, orc.render_for_workloads)
     rows, _ = PT.rows_with_near(W, w, prob, n_prior, n_near)
-    _check(api, orc, w, prob, rows, W.mge_sigmas(w, n_gauss))
+    _check(api, orc, w, prob, rows, W.mge_sigmas(w, n_gauss), precision=precision)
 
 
 def test_mge_zero_edge_and_epl(api, orc):
@@ -90,6 +97,7 @@ def test_mge_zero_edge_and_epl(api, orc):
     prob = W.make_problem(w, orc.render_for_workloads)
     rows = W.batch_rows(w, 6)
     _check(api, orc, w, prob, rows, W.mge_sigmas(w, 7))
+    _check(api, orc, w, prob, rows, W.mge_sigmas(w, 7), precision=api.TL_PRECISION_FP64)
 
 
 def test_mge_recovers_known_amplitudes_and_flags_invalid_rows(api, orc):
@@ -251,8 +259,9 @@ def _two_set_case(orc, n0, n1, ny=36, nx=44, S=2, K=7, batch=12):
     return w, prob, rows, sets
 
 
+@pytest.mark.parametrize("precision", [0, 1])
 @pytest.mark.parametrize("n0,n1", [(6, 5), (14, 12), (16, 14)])
-def test_mge_two_sets_match_oracle(api, orc, n0, n1):
+def test_mge_two_sets_match_oracle(api, orc, n0, n1, precision):
     """Two Gaussian sets, each on its own ellipses, 12 / 27 / 31 columns (the last two beyond what the
     oracle can enumerate: scipy's NNLS is its step there, pinned against the enumeration on CPU).
     Compared: logL, and the fitted image through the oracle's own columns."""
@@ -263,6 +272,8 @@ def test_mge_two_sets_match_oracle(api, orc, n0, n1):
     rows[5, 7:10] = np.nan; rows[5, 14:17] = np.nan      # ignored entries of both blocks
     ctx = api.LensContext.from_problem(prob)
     ctx.set_mge_sets(sets)
+    ctx.set_precision(precision)
+    bound = PT.near_bound_fp32(PT.FP32_MGE_MEASURED) if precision == 0 else 1.0
     n_col = n0 + n1 + 1
     assert api.tl_mge_columns(ctx.handle) == n_col
     d = torch.from_numpy(rows).cuda()
@@ -291,9 +302,10 @@ def test_mge_two_sets_match_oracle(api, orc, n0, n1):
         worst_fit = max(worst_fit, np.abs(gimg - oimg).max() / oimg.max())
         # the GPU's amplitudes, through the oracle's columns, reach the oracle's optimum
         ll_at = orc.loglike_from_image(gimg, prob.data[0], prob.noise[0])
-        assert oll - ll_at <= PT.near_bound_fp32(PT.FP32_MGE_MEASURED) * tol, (r, oll - ll_at, tol)
-    print("two sets (%d + %d Gaussians, %d columns): logL %.3g x north_star, fitted image %.2e x peak" % (n0, n1, n_col, worst, worst_fit))
-    assert worst <= PT.near_bound_fp32(PT.FP32_MGE_MEASURED) and worst_fit <= 1e-4
+        assert oll - ll_at <= bound * tol, (r, oll - ll_at, tol)
+    print("two sets (%d + %d Gaussians, %d columns, precision %d): logL %.3g x north_star, fitted image %.2e x peak"
+          % (n0, n1, n_col, precision, worst, worst_fit))
+    assert worst <= bound and worst_fit <= 1e-4
 
 
 def test_mge_two_identical_sets_equal_one_set(api, orc):
