@@ -194,12 +194,22 @@ def _dev_rows(handle, params):
     return params.shape[0]
 
 
+def _check_out(t, shape, device, what):
+    """A caller-supplied result tensor must be a contiguous CUDA float32 tensor of exactly the shape the kernels write."""
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.device == device and t.dtype == torch.float32
+            and t.is_contiguous() and tuple(t.shape) == tuple(shape)):
+        raise TinyLensError(TL_EINVAL, "%s must be a contiguous CUDA float32 tensor of shape %s on %s" % (what, tuple(shape), device))
+
+
 def tl_loglike_batch(handle: int, params, out=None, stream=None):
     """params: CUDA float32 [B,P] -> logL CUDA float32 [B] (enqueued on `stream`, no sync)."""
     import torch
     B = _dev_rows(handle, params)
     if out is None:
         out = torch.empty(B, dtype=torch.float32, device=params.device)
+    else:
+        _check_out(out, (B,), params.device, "out")
     _check(load().tl_loglike_batch(handle, params.data_ptr(), B, out.data_ptr(), _stream_handle(stream)),
            "tl_loglike_batch")
     return out
@@ -211,6 +221,8 @@ def tl_render_batch(handle: int, params, ny: int, nx: int, out=None, stream=None
     B = _dev_rows(handle, params)
     if out is None:
         out = torch.empty((B, ny, nx), dtype=torch.float32, device=params.device)
+    else:
+        _check_out(out, (B, ny, nx), params.device, "out")
     _check(load().tl_render_batch(handle, params.data_ptr(), B, out.data_ptr(), _stream_handle(stream)),
            "tl_render_batch")
     return out
@@ -222,8 +234,12 @@ def tl_loglike_linear_batch(handle: int, params, n_comp: int, out=None, amps=Non
     B = _dev_rows(handle, params)
     if out is None:
         out = torch.empty(B, dtype=torch.float32, device=params.device)
+    else:
+        _check_out(out, (B,), params.device, "out")
     if amps is None and want_amps:
         amps = torch.empty((B, n_comp), dtype=torch.float32, device=params.device)
+    elif amps is not None:
+        _check_out(amps, (B, n_comp), params.device, "amps")
     _check(load().tl_loglike_linear_batch(handle, params.data_ptr(), B, out.data_ptr(),
                                           amps.data_ptr() if amps is not None else None, _stream_handle(stream)),
            "tl_loglike_linear_batch")
@@ -262,8 +278,12 @@ def tl_loglike_mge_batch(handle: int, params, out=None, amps=None, want_amps=Tru
         raise TinyLensError(TL_EINVAL, "tl_loglike_mge_batch (no Gaussian set: call tl_set_mge)")
     if out is None:
         out = torch.empty(B, dtype=torch.float32, device=params.device)
+    else:
+        _check_out(out, (B,), params.device, "out")
     if amps is None and want_amps:
         amps = torch.empty((B, n_col), dtype=torch.float32, device=params.device)
+    elif amps is not None:
+        _check_out(amps, (B, n_col), params.device, "amps")
     _check(load().tl_loglike_mge_batch(handle, params.data_ptr(), B, out.data_ptr(),
                                        amps.data_ptr() if amps is not None else None, _stream_handle(stream)),
            "tl_loglike_mge_batch")

@@ -189,6 +189,7 @@ void fill_prologue_args(const tl_ctx *c, tl::PrologueArgs &pa, const float *para
     pa.fov_half = 0.5 * c->cfg.pix_scale * (c->He > c->We ? c->He : c->We);
     pa.refine_tau = c->refine_tau;
     pa.unit_amp = unit_amp; pa.mge = 0;
+    pa.zero_words = nullptr; pa.n_zero_words = 0; pa.pad_ext = nullptr; pa.pad_rows = 0; pa.pad_pitch = 0; pa.pad_We = 0;
 }
 
 // B <= n_sm / 2 rows on a fused context: prologue -> trace_kernel (rows x slabs) -> conv_small_kernel
@@ -200,16 +201,20 @@ int run_small_batch(tl_ctx *c, const float *params, int64_t B, float *logL, floa
     // binned images, then one work-queue head and one finished-band counter per row; zeroed together
     const size_t img_bytes = sizeof(float) * (size_t)nb * c->He * c->pitch;
     const size_t ext_bytes = img_bytes + 2 * sizeof(int) * (size_t)nb;     // + finished-band counters
-    tl::RowC *rows = nullptr;
-    float *ext = nullptr, *cblk = nullptr;
-    if (!pool_alloc(c, &rows, sizeof(tl::RowC) * (size_t)nb, st)) return TL_ENOMEM;
-    if (!pool_alloc(c, &ext, ext_bytes, st)) { cudaFreeAsync(rows, st); return TL_ENOMEM; }
-    if (logL && !pool_alloc(c, &cblk, sizeof(float) * (size_t)nb * npair * nsx, st)) {
-        cudaFreeAsync(rows, st); cudaFreeAsync(ext, st); return TL_ENOMEM;
-    }
-    cudaMemsetAsync(ext, 0, ext_bytes, st);          // pitch padding must read as finite zeros
+    // ONE allocation (rows | images + counters | chi^2 terms) and no memset: on this path the host-side
+    // API calls are the cost (a one-row call is ~25 us of GPU work)
+    const size_t rows_bytes = (sizeof(tl::RowC) * (size_t)nb + 255) & ~(size_t)255;
+    const size_t ext_al = (ext_bytes + 255) & ~(size_t)255;
+    const size_t cblk_bytes = logL ? sizeof(float) * (size_t)nb * npair * nsx : 0;
+    unsigned char *blob = nullptr;
+    if (!pool_alloc(c, &blob, rows_bytes + ext_al + cblk_bytes, st)) return TL_ENOMEM;
+    tl::RowC *rows = reinterpret_cast<tl::RowC *>(blob);
+    float *ext = reinterpret_cast<float *>(blob + rows_bytes);
+    float *cblk = logL ? reinterpret_cast<float *>(blob + rows_bytes + ext_al) : nullptr;
     tl::PrologueArgs pa;
     fill_prologue_args(c, pa, params, rows, nb, 0, B / c->cfg.n_lens, 0);
+    pa.zero_words = reinterpret_cast<int *>(reinterpret_cast<unsigned char *>(ext) + img_bytes); pa.n_zero_words = 2 * nb;
+    pa.pad_ext = ext; pa.pad_rows = nb * c->He; pa.pad_pitch = c->pitch; pa.pad_We = c->We;
     tl::prologue_kernel<<<(unsigned)((nb * (1 + c->n_comp) + 127) / 128), 128, 0, st>>>(pa);
     tl::KArgs a = base_args(c);
     a.rows = rows; a.B = nb; a.rows_per_lens = B / c->cfg.n_lens; a.row0 = 0;
@@ -234,8 +239,7 @@ int run_small_batch(tl_ctx *c, const float *params, int64_t B, float *logL, floa
     if (c->profile) { cudaEventRecord(c->ev1, st); c->prof_pending = 1; }
     tl::conv_small_kernel<<<dim3((unsigned)nb, (unsigned)bands), c->threads, conv_smem, st>>>(a, nb, band_pairs, cblk);
     const int rc = cuda_ok(cudaGetLastError()) ? TL_OK : TL_ECUDA;
-    cudaFreeAsync(rows, st); cudaFreeAsync(ext, st);
-    if (cblk) cudaFreeAsync(cblk, st);
+    cudaFreeAsync(blob, st);
     return rc;
 }
 

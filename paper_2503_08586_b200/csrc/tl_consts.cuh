@@ -23,6 +23,7 @@
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
+#include "tl_bn_table.h"
 
 namespace tl {
 
@@ -95,6 +96,11 @@ struct PrologueArgs {
     double inv_u;                    // 2 S / pix_scale   (u-units per arcsec)
     double fov_half;                 // arcsec, half the extended field of view
     double refine_tau;               // refinement threshold in units of sigma_min
+    // small-batch path: what a cudaMemsetAsync used to do, folded into this launch (one API call less on
+    // a path whose cost is host-side latency): work-queue / band counters, and the pitch padding of the
+    // binned images (read by zero-padded taps only, but it must be finite)
+    int *zero_words; int n_zero_words;
+    float *pad_ext; int pad_rows, pad_pitch, pad_We;     // pad_rows = B * He image rows of pad_pitch floats
     int unit_amp;                    // linear-amplitude mode: every I_e is taken as 1
     int mge;                         // MGE mode (tl_loglike_mge_batch): of the lens-light block only e1, e2, cx, cy are
                                      // read; its quadratic form becomes t = R_p^2 in arcsec^2 (r_e := 1, n := 1);
@@ -124,7 +130,22 @@ __device__ inline double gamma_p_series(double a, double x, double *prefactor)
     return pf * sum;
 }
 
+// b_n from the Chebyshev table of tl_bn_table.h (n in [0.3, 15]: 2e-15 relative; Clenshaw recurrence),
+// else by the iteration below.  The iterative solve drags in lgamma / exp / log and ~60 divisions --
+// most of the prologue kernel's code, whose instruction-cache misses were most of a one-row call.
+static __device__ __noinline__ double sersic_bn_solve(double n);
 __device__ inline double sersic_bn(double n)
+{
+    if (!(n >= BN_N_LO && n <= BN_N_HI)) return sersic_bn_solve(n);
+    const double *T = n >= BN_N_MID ? BN_PIECE0 : BN_PIECE1;
+    const double x = 1.0 / n, xa = T[0], xb = T[1];
+    const double y = (2.0 * x - (xa + xb)) / (xb - xa), y2 = 2.0 * y;
+    double b1 = 0.0, b2 = 0.0;
+    for (int k = BN_NCOEF - 1; k >= 1; --k) { const double b0 = fma(y2, b1, T[2 + k] - b2); b2 = b1; b1 = b0; }
+    return (2.0 * n - 1.0 / 3.0) + (fma(y, b1, T[2]) - b2);
+}
+
+static __device__ __noinline__ double sersic_bn_solve(double n)
 {
     const double a = 2.0 * n;
     double lo = 0.0, hi = INFINITY, pf;
@@ -174,13 +195,24 @@ __device__ inline void split2_poslo(double v, float *h, float *l)
 }
 
 // Inverse of PAPER.md:152 Eq. 11 (G3): e = hypot(e1,e2), q = (1-e)/(1+e), phi = atan2(e2,e1)/2.
+// cos / sin of phi in (-pi/2, pi/2] by the half-angle formulas from (cos 2phi, sin 2phi) = (e1, e2)/e,
+// taking the square root of whichever of (1 +- cos 2phi)/2 does not cancel (no atan2 / sincos: their
+// code was a large part of the prologue's instruction footprint).
 __device__ inline bool shape_from_e(double e1, double e2, double *q, double *c, double *s)
 {
-    double e = hypot(e1, e2);
+    const double e = sqrt(e1 * e1 + e2 * e2);
     if (!(e < 1.0)) return false;
     *q = (1.0 - e) / (1.0 + e);
-    double phi = 0.5 * atan2(e2, e1);
-    sincos(phi, s, c);
+    if (!(e > 0.0)) { *c = 1.0; *s = 0.0; return true; }          // atan2(0, 0) = 0
+    const double c2 = e1 / e, s2 = e2 / e;
+    if (c2 >= 0.0) {
+        const double cc = sqrt(0.5 * (1.0 + c2));
+        *c = cc; *s = s2 / (2.0 * cc);
+    } else {
+        const double sa = sqrt(0.5 * (1.0 - c2));                 // |sin phi| >= 0.707
+        const double ss = e2 < 0.0 ? -sa : sa;                    // phi = +pi/2 for e2 = +0 (atan2(+0, -1) = pi)
+        *s = ss; *c = s2 / (2.0 * ss);
+    }
     return true;
 }
 
@@ -189,6 +221,14 @@ __global__ void __launch_bounds__(128) prologue_kernel(PrologueArgs a)
 {
     const int nslot = 1 + a.n_lens_light + a.n_source;
     int64_t gid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (a.zero_words || a.pad_ext) {
+        const int64_t nthr = (int64_t)gridDim.x * blockDim.x;
+        for (int64_t i = gid; i < a.n_zero_words; i += nthr) a.zero_words[i] = 0;
+        const int pw = a.pad_pitch - a.pad_We;
+        if (a.pad_ext && pw > 0)
+            for (int64_t i = gid; i < (int64_t)a.pad_rows * pw; i += nthr)
+                a.pad_ext[(i / pw) * a.pad_pitch + a.pad_We + (i % pw)] = 0.f;
+    }
     if (gid >= a.B * nslot) return;
     int64_t row = gid / nslot;
     int slot = (int)(gid - row * nslot);
@@ -223,8 +263,10 @@ __global__ void __launch_bounds__(128) prologue_kernel(PrologueArgs a)
         const bool s1ok = isfinite(s1[5]) && isfinite(s1[6]);
         double s1X = (s1ok ? (double)s1[5] : 0.0) * a.inv_u, s1Y = (s1ok ? (double)s1[6] : 0.0) * a.inv_u;
         double d1 = n11 * cX + n12 * cY - (c * s1X + s * s1Y), d2 = n21 * cX + n22 * cY - (-s * s1X + c * s1Y);
-        double th0 = 0.5 * atan2(qp, q), c0 = cos(th0), s0 = sin(th0);
-        double T = atanh(fmin(qp, 1.0 - 1e-16)), z0 = tanh(0.5 * T);
+        // theta0 = atan(q'/q)/2 with (cos, sin)(2 theta0) = (q, q'): half-angle formulas; z0 = tanh(atanh(q')/2)
+        // = q'/(1 + q).  (Only their float roundings are used: the angles added back come from those.)
+        double c0 = sqrt(0.5 * (1.0 + q)), s0 = qp / (2.0 * c0);
+        double z0 = qp / (1.0 + q);
         // centre = (multiple of 2^-8) + remainder: sub-sample coordinates are odd integers, so
         // X - cXa is exact in FP32 and the remainder enters through small additive constants
         L.cXa = (float)(rint(cX * 256.0) / 256.0); L.cYa = (float)(rint(cY * 256.0) / 256.0);
@@ -351,7 +393,7 @@ __global__ void __launch_bounds__(128) prologue_kernel(PrologueArgs a)
         double dbeta = 2.4e-7 * (fmax((double)p[0], 0.0) + a.fov_half);               // arcsec
         double smin = a.sigma_min[(a.row0 + row) / a.rows_per_lens];
         double cf = fabs(amp) * (a.unit_amp ? Ie_hint : 1.0) * (bn / n) * dbeta / (re * a.refine_tau * smin);
-        C.nlcf = (float)fmin(fmax(-log2(cf), -1e30), 1e30);
+        C.nlcf = fminf(fmaxf(-__log2f((float)cf), -1e30f), 1e30f);      // a threshold: MUFU accuracy is plenty
     }
     C.valid = ok ? 1 : 0;
     // MGE mode: the sources come first (comp[0 .. n_source-1], what the NLL = 0 ray-trace kernels read)

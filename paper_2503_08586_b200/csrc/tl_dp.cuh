@@ -247,8 +247,7 @@ __global__ void __launch_bounds__(64) prologue_dp_kernel(const DpArgs a)
     const double qp = fmax(sqrt((1.0 - q) * (1.0 + q)), 1e-9);
     R.q2 = q * q; R.qp = qp; R.q = q; R.thE_sq = thE * sqrt(q);
     R.f = R.thE_sq / qp;
-    const double th0 = 0.5 * atan2(qp, q);
-    sincos(th0, &R.s0, &R.c0);
+    R.c0 = sqrt(0.5 * (1.0 + q)); R.s0 = qp / (2.0 * R.c0);   // ~ (cos, sin)(atan(q'/q)/2): half-angle formulas
     R.fth0 = R.f * atan2(R.s0, R.c0);                 // the angle the stored pair really encodes
     R.fl2 = R.f * 0.34657359027997265471;             // ln(2)/2
     R.g1 = g1; R.g2 = g2;
