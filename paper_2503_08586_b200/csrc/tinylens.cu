@@ -234,11 +234,21 @@ int run_small_batch(tl_ctx *c, const float *params, int64_t B, float *logL, floa
     if (band_pairs > max_pairs) band_pairs = max_pairs;
     bands = (npair + band_pairs - 1) / band_pairs;
     const size_t conv_smem = fixed + sizeof(float) * (size_t)(2 * band_pairs + c->K - 1) * c->pitch;
+    // programmatic dependent launch: the next kernel's CTAs are scheduled while the previous one drains
+    // (the kernels wait with griddepcontrol.wait before touching what their predecessor wrote)
+    cudaLaunchAttribute pdl;
+    pdl.id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    pdl.val.programmaticStreamSerializationAllowed = c->profile ? 0 : 1;     // (profiling events sit between the kernels)
+    cudaLaunchConfig_t lc;
+    memset(&lc, 0, sizeof(lc));
+    lc.stream = st; lc.attrs = &pdl; lc.numAttrs = 1;
     if (c->profile) cudaEventRecord(c->ev0, st);
-    c->sb_trace<<<dim3((unsigned)nb, (unsigned)slabs), 256, c->sb_trace_smem, st>>>(a, nb);
+    lc.gridDim = dim3((unsigned)nb, (unsigned)slabs); lc.blockDim = dim3(256); lc.dynamicSmemBytes = c->sb_trace_smem;
+    bool okl = cuda_ok(cudaLaunchKernelEx(&lc, c->sb_trace, (const tl::KArgs)a, nb));
     if (c->profile) { cudaEventRecord(c->ev1, st); c->prof_pending = 1; }
-    tl::conv_small_kernel<<<dim3((unsigned)nb, (unsigned)bands), c->threads, conv_smem, st>>>(a, nb, band_pairs, cblk);
-    const int rc = cuda_ok(cudaGetLastError()) ? TL_OK : TL_ECUDA;
+    lc.gridDim = dim3((unsigned)nb, (unsigned)bands); lc.blockDim = dim3((unsigned)c->threads); lc.dynamicSmemBytes = conv_smem;
+    okl = okl && cuda_ok(cudaLaunchKernelEx(&lc, tl::conv_small_kernel, (const tl::KArgs)a, nb, band_pairs, cblk));
+    const int rc = (okl && cuda_ok(cudaGetLastError())) ? TL_OK : TL_ECUDA;
     cudaFreeAsync(blob, st);
     return rc;
 }

@@ -219,6 +219,7 @@ __device__ inline bool shape_from_e(double e1, double e2, double *q, double *c, 
 #ifdef TL_MAIN_TU
 __global__ void __launch_bounds__(128) prologue_kernel(PrologueArgs a)
 {
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // (small-batch path: see tl_kernels.cuh pdl_*)
     const int nslot = 1 + a.n_lens_light + a.n_source;
     int64_t gid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (a.zero_words || a.pad_ext) {

@@ -21,6 +21,13 @@ namespace tl {
 
 constexpr int CONV_R = 4;            // outputs per thread strip (along x)
 
+// Programmatic dependent launch (the small-batch path, whose cost is launch latency): a kernel launched
+// with cudaLaunchAttributeProgrammaticStreamSerialization may start while its predecessor still runs;
+// pdl_wait() blocks until the predecessor has completed and its writes are visible, pdl_launch() lets
+// the successor's CTAs be scheduled early.  Both are no-ops for ordinary launches.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 struct KArgs {
     const RowC *rows;        // [B] derived constants
     const float *psf;        // [n_lens][K][Kp]  flipped, rows zero-padded to Kp (multiple of 4)
@@ -738,6 +745,8 @@ __global__ void __launch_bounds__(256, 2) trace_kernel(const KArgs a, int chunk_
     __shared__ RowC rc_s;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     RowV *rowtab = a.rowtab ? reinterpret_cast<RowV *>(smem_raw) : nullptr;
+    pdl_launch();
+    pdl_wait();                                        // the row constants come from the prologue kernel
     for (int r = blockIdx.x; r < chunk_rows; r += gridDim.x) {
         __syncthreads();
         load_row_consts(&rc_s, a.rows + r);
@@ -849,6 +858,8 @@ __global__ void __launch_bounds__(512) conv_small_kernel(const KArgs a, int chun
     const int64_t row = a.row0 + r;
     const int64_t lens = row / a.rows_per_lens;
     const size_t npix = (size_t)a.ny * a.nx;
+    load_psf(taps, a.psf + lens * a.K * a.Kp, a.K * a.Kp);          // context data: before the wait
+    pdl_wait();                                                   // rows / ext come from the preceding kernels
     if (!row_is_valid(a.rows[r], a.n_comp)) {
         if (a.images)
             for (size_t i = (size_t)2 * p0 * a.nx + threadIdx.x; i < (size_t)min(a.ny, 2 * p1) * a.nx; i += blockDim.x)
@@ -856,7 +867,6 @@ __global__ void __launch_bounds__(512) conv_small_kernel(const KArgs a, int chun
         if (a.logL && blockIdx.y == 0 && threadIdx.x == 0) a.logL[row] = -INFINITY;
         return;
     }
-    load_psf(taps, a.psf + lens * a.K * a.Kp, a.K * a.Kp);
     // extended rows 2 p0 .. 2 (p1 - 1) + K of this row's binned image (the last one may lie past
     // the image when ny is odd: zeros), plus the slack the strips may touch
     const int e0 = 2 * p0, erows = 2 * (p1 - p0) + a.K - 1, have = min(erows, a.He - e0);
