@@ -76,6 +76,8 @@ struct tl_ctx {
     int64_t chunk_rows = 0;       // rows per scratch chunk
     // small-batch path of fused contexts (rows spread over many CTAs, bitwise equal to fused)
     void (*sb_trace)(const tl::KArgs, int) = nullptr;
+    void (*sb_pairs)(const tl::KArgs, int) = nullptr;      // trace_pairs_kernel: calls of at most sb_pairs_rows rows
+    int sb_pairs_rows = 0;
     size_t sb_trace_smem = 0;
     int sb_rowtab = 0, sb_max_rows = 0;
     // MGE mode (tl_set_mge / tl_loglike_mge_batch)
@@ -233,7 +235,16 @@ int run_small_batch(tl_ctx *c, const float *params, int64_t B, float *logL, floa
     const int max_pairs = (int)(((SMEM_LIMIT - 1024 - fixed) / (sizeof(float) * c->pitch) - (c->K - 1)) / 2);
     if (band_pairs > max_pairs) band_pairs = max_pairs;
     bands = (npair + band_pairs - 1) / band_pairs;
-    const size_t conv_smem = fixed + sizeof(float) * (size_t)(2 * band_pairs + c->K - 1) * c->pitch;
+    // few rows: the K kernel rows of a 2 x 4 block on K threads (conv_blocks_split), the CTAs left over
+    // splitting the bands along x; it pays while a CTA gets through its blocks in one or two passes
+    const int per_pass = c->threads / c->K;
+    int xseg = want / bands;
+    const int one_pass = (band_pairs * nsx + per_pass - 1) / per_pass;
+    if (xseg > one_pass) xseg = one_pass;
+    if (xseg > nsx) xseg = nsx;
+    if (xseg < 1) xseg = 1;
+    if ((band_pairs * ((nsx + xseg - 1) / xseg) + per_pass - 1) / per_pass > 2) xseg = 0;
+    const size_t conv_smem = fixed + sizeof(float) * ((size_t)(2 * band_pairs + c->K - 1) * c->pitch + (xseg ? (size_t)per_pass * c->K * 8 : 0));
     // programmatic dependent launch: the next kernel's CTAs are scheduled while the previous one drains
     // (the kernels wait with griddepcontrol.wait before touching what their predecessor wrote)
     cudaLaunchAttribute pdl;
@@ -243,11 +254,22 @@ int run_small_batch(tl_ctx *c, const float *params, int64_t B, float *logL, floa
     memset(&lc, 0, sizeof(lc));
     lc.stream = st; lc.attrs = &pdl; lc.numAttrs = 1;
     if (c->profile) cudaEventRecord(c->ev0, st);
-    lc.gridDim = dim3((unsigned)nb, (unsigned)slabs); lc.blockDim = dim3(256); lc.dynamicSmemBytes = c->sb_trace_smem;
-    bool okl = cuda_ok(cudaLaunchKernelEx(&lc, c->sb_trace, (const tl::KArgs)a, nb));
+    bool okl;
+    if (c->sb_pairs && nb <= c->sb_pairs_rows) {
+        // one pair of sub-samples per lane, one warp tile per warp (tl_kernels.cuh trace_pairs_kernel)
+        const int S = c->cfg.supersample, ppw = 32 / (S * S / 2);
+        const int n_wt = (c->He * c->We + ppw - 1) / ppw;
+        a.rowtab = 0;
+        const int per_row = want < (n_wt + 7) / 8 ? want : (n_wt + 7) / 8;
+        lc.gridDim = dim3((unsigned)nb, (unsigned)per_row); lc.blockDim = dim3(256); lc.dynamicSmemBytes = 0;
+        okl = cuda_ok(cudaLaunchKernelEx(&lc, c->sb_pairs, (const tl::KArgs)a, nb));
+    } else {
+        lc.gridDim = dim3((unsigned)nb, (unsigned)slabs); lc.blockDim = dim3(256); lc.dynamicSmemBytes = c->sb_trace_smem;
+        okl = cuda_ok(cudaLaunchKernelEx(&lc, c->sb_trace, (const tl::KArgs)a, nb));
+    }
     if (c->profile) { cudaEventRecord(c->ev1, st); c->prof_pending = 1; }
-    lc.gridDim = dim3((unsigned)nb, (unsigned)bands); lc.blockDim = dim3((unsigned)c->threads); lc.dynamicSmemBytes = conv_smem;
-    okl = okl && cuda_ok(cudaLaunchKernelEx(&lc, tl::conv_small_kernel, (const tl::KArgs)a, nb, band_pairs, cblk));
+    lc.gridDim = dim3((unsigned)nb, (unsigned)(bands * (xseg ? xseg : 1))); lc.blockDim = dim3((unsigned)c->threads); lc.dynamicSmemBytes = conv_smem;
+    okl = okl && cuda_ok(cudaLaunchKernelEx(&lc, tl::conv_small_kernel, (const tl::KArgs)a, nb, band_pairs, xseg, cblk));
     const int rc = (okl && cuda_ok(cudaGetLastError())) ? TL_OK : TL_ECUDA;
     cudaFreeAsync(blob, st);
     return rc;
@@ -610,6 +632,10 @@ int tl_create_ex(tl_ctx **out, const tl_config *cfg, const float *psf_in, int32_
             }
             c->sb_max_rows = oks ? c->n_sm / 2 : 0;
             if (c->opt.small_batch_rows > 0) c->sb_max_rows = oks ? c->opt.small_batch_rows : 0;
+            if (cfg->mass_model != TL_MASS_EPL) {
+                c->sb_pairs = tl_trace_pairs_for(cfg->supersample, cfg->n_lens_light, cfg->n_source);
+                c->sb_pairs_rows = 16;             // measured on configs[1]: faster than trace_kernel up to ~20 rows
+            }
             cudaGetLastError();
         }
     } else {

@@ -9,6 +9,7 @@ typedef void (*trace_fn)(const tl::KArgs, int);
 
 fused_fn tl_fused_for(int S, int n_lens_light, int n_source);          // fused_kernel<S, NLL, NSRC>
 trace_fn tl_trace_for(int S, int n_lens_light, int n_source);          // trace_kernel<S, NLL, NSRC>
+trace_fn tl_trace_pairs_for(int S, int n_lens_light, int n_source);    // trace_pairs_kernel<S, NLL, NSRC>, or null (odd S)
 fused_fn tl_fused_lin_for(int S, int n_lens_light, int n_source);      // fused_lin_kernel<...>
 trace_fn tl_trace_lin_for(int S, int n_lens_light, int n_source);      // trace_lin_kernel<...>
 // mass_model = MASS_EPL (compile time: S = 4 unrolled, any other S through the generic loop)

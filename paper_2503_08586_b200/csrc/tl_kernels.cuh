@@ -171,15 +171,13 @@ __device__ __forceinline__ void sample_value(const RowC &rc, const HotC<NLL, NSR
     }
 }
 
-// Two horizontally adjacent sub-samples at once with packed FP32 arithmetic (tl_pair.cuh): lens
-// light added to `acc2`, sources returned (a half is NaN when that sample wants the FP64 ray-trace).
+// Two horizontally adjacent sub-samples at once with packed FP32 arithmetic (tl_pair.cuh): the
+// lens-light profile values go to `llv` (not yet scaled by the amplitude), the sources are returned
+// (a half is NaN when that sample wants the FP64 ray-trace).
 template <int NLL, int NSRC>
-__device__ __forceinline__ f2 sample_pair(const HotC<NLL, NSRC, MASS_SIE> &h, const ColV2 &c, const RowV &r, f2 &acc2, bool &any)
+__device__ __forceinline__ f2 sample_pair_parts(const HotC<NLL, NSRC, MASS_SIE> &h, const ColV2 &c, const RowV &r, f2 &llv, bool &any)
 {
-    if (NLL) {
-        const f2 t = fma2(c.LB, bc2(r.dyl), add2(c.LA, bc2(r.LC)));
-        acc2 = fma2(bc2(h.ll.amp), sersic_from_t2(h.ll, t), acc2);
-    }
+    if (NLL) llv = sersic_from_t2(h.ll, fma2(c.LB, bc2(r.dyl), add2(c.LA, bc2(r.LC))));
     const f2 xp = add2(c.Pc, bc2(r.Qs)), yp = fma2(c.Ps, bc2(-1.f), bc2(r.Qc));
     f2 axp, ayp;
     sie_alpha2(h.sie, xp, yp, axp, ayp);
@@ -198,6 +196,16 @@ __device__ __forceinline__ f2 sample_pair(const HotC<NLL, NSRC, MASS_SIE> &h, co
     if (f1) s1 = __int_as_float(0x7fc00000);
     any = any || f0 || f1;
     return mk2(s0, s1);
+}
+// ... with the lens light added to `acc2`
+template <int NLL, int NSRC>
+__device__ __forceinline__ f2 sample_pair(const HotC<NLL, NSRC, MASS_SIE> &h, const ColV2 &c, const RowV &r, f2 &acc2, bool &any)
+{
+    f2 llv;
+    llv.v = 0ull;
+    const f2 s = sample_pair_parts<NLL, NSRC>(h, c, r, llv, any);
+    if (NLL) acc2 = fma2(bc2(h.ll.amp), llv, acc2);
+    return s;
 }
 
 // Steps a3-a4 of one sub-sample once its deflection is known (EPL: the deflections of the S_T
@@ -763,6 +771,91 @@ __global__ void __launch_bounds__(256, 2) trace_kernel(const KArgs a, int chunk_
     }
 }
 
+// trace_pairs_kernel: the ray-trace of calls with a handful of rows (run_small_batch), where the time
+// of a call is the longest dependent chain, not the arithmetic.  A lane takes ONE pair of horizontally
+// adjacent sub-samples, the S^2 / 2 lanes of a native pixel sit side by side in a warp, and the pixel's
+// sum is formed from their values in the order of trace_tiles (per sub-sample row: lens light left to
+// right, then the sources left to right), so that the pixel is BITWISE what trace_tiles gives.  The
+// longest chain of the call -- the FP64 refinement of the samples next to the source centre, which
+// trace_tiles runs sixteen deep per lane at S = 4 -- becomes two deep, and one row fills the GPU.
+// Rows on the q < 0.5 branch go through trace_tiles.  Grid (rows, CTAs per row): as many as are resident at once.
+template <int S_T, int NLL, int NSRC>
+__global__ void __launch_bounds__(256, 2) trace_pairs_kernel(const KArgs a, int chunk_rows)
+{
+    static_assert(S_T == 2 || S_T == 4 || S_T == 8, "S^2 / 2 lanes per pixel must divide a warp");
+    constexpr int NP = S_T / 2, LPP = S_T * NP, PPW = 32 / LPP;
+    __shared__ RowC rc_s;
+    pdl_launch();
+    pdl_wait();                                        // the row constants come from the prologue kernel
+    const int r = blockIdx.x;
+    if (r >= chunk_rows) return;
+    load_row_consts(&rc_s, a.rows + r);
+    __syncthreads();
+    if (!row_is_valid(rc_s, a.n_comp)) return;
+    float *dst = a.ext + (size_t)r * a.He * a.pitch;
+    const int warp = (blockIdx.y * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    const HotC<NLL, NSRC, MASS_SIE> h(rc_s);
+    if (rc_s.lens.mode != 0) {                         // uniform over the row
+        const int n = a.tiles_x * a.tiles_y, n_warps = (gridDim.y * blockDim.x) >> 5;
+        int t = (int)((long long)n * warp / n_warps);
+        const int t_end = (int)((long long)n * (warp + 1) / n_warps);
+        trace_tiles<S_T, NLL, NSRC, false, false, MASS_SIE>(rc_s, h, a, nullptr, [&]() -> int { return t < t_end ? t++ : -1; },
+                                                            [&](int i, int j, float v) { dst[i * a.pitch + j] = v; });
+        return;
+    }
+    const int sub = lane % LPP, sa = sub / NP, sp = sub - sa * NP, base = lane - sub;
+    const int npix = a.He * a.We, n_warps = (gridDim.y * blockDim.x) >> 5;
+    // warp tiles of PPW pixels, dealt out round-robin: neighbouring tiles (the refined ones cluster
+    // round the source centre) go to different warps
+    for (int p0 = warp * PPW; p0 < npix; p0 += n_warps * PPW) {
+        const int pix = p0 + lane / LPP;
+        const bool live = pix < npix;
+        const int pc = live ? pix : npix - 1;
+        const int i = pc / a.We, j = pc - i * a.We;
+        const bool edge = a.edge_zero && (j < a.h || j >= a.We - a.h || i < a.h || i >= a.He - a.h);
+        f2 llv, s;
+        llv.v = 0ull; s.v = 0ull;
+        if (!edge) {
+            // u-units, as in trace_tiles: X = 2 (j S + b) + 1 - S We, Y = 2 (i S + sa) + 1 - S He
+            const float X = (float)(2 * j * S_T + 1 - S_T * a.We) + (float)(4 * sp);
+            const float Y = (float)(2 * i * S_T + 1 - S_T * a.He) + (float)(2 * sa);
+            const ColV2 cv = col_values2<NLL>(rc_s, X, X + 2.f);
+            const RowV rv = row_values<NLL>(rc_s, Y);
+            bool any = false;
+            s = sample_pair_parts<NLL, NSRC>(h, cv, rv, llv, any);
+            if (any) {                                 // rare: FP64 ray-trace, out of line
+                float s0, s1;
+                un2(s, s0, s1);
+                if (s0 != s0) s0 = refined_source_light<MASS_SIE>(rc_s, NLL, NLL + NSRC, X, Y);
+                if (s1 != s1) s1 = refined_source_light<MASS_SIE>(rc_s, NLL, NLL + NSRC, X + 2.f, Y);
+                s = mk2(s0, s1);
+            }
+        }
+        __syncwarp();
+        f2 acc2 = bc2(0.f);
+#pragma unroll
+        for (int ra = 0; ra < S_T; ++ra) {
+            if (NLL) {
+#pragma unroll
+                for (int b = 0; b < NP; ++b) {
+                    f2 v;
+                    v.v = __shfl_sync(0xffffffffu, llv.v, base + ra * NP + b);
+                    acc2 = fma2(bc2(h.ll.amp), v, acc2);
+                }
+            }
+#pragma unroll
+            for (int b = 0; b < NP; ++b) {
+                f2 v;
+                v.v = __shfl_sync(0xffffffffu, s.v, base + ra * NP + b);
+                acc2 = add2(acc2, v);
+            }
+        }
+        float a0, a1;
+        un2(acc2, a0, a1);
+        if (live && sub == 0) dst[i * a.pitch + j] = edge ? 0.f : a0 + a1;
+    }
+}
+
 #ifdef TL_MAIN_TU
 // conv_kernel: one CTA per (row_in_chunk, tile of `tile_rows` output rows).
 __global__ void __launch_bounds__(256) conv_kernel(const KArgs a, int chunk_rows)
@@ -842,26 +935,88 @@ __device__ __forceinline__ void conv_blocks_store(const KArgs &a, const float *i
     }
 }
 
-// one CTA per (row, band of `band_pairs` output row pairs); cblk: [chunk][npair * nsx] or null;
-// a.tile_counters[chunk_rows + r] (zeroed) counts the finished bands of row r
-__global__ void __launch_bounds__(512) conv_small_kernel(const KArgs a, int chunk_rows, int band_pairs, float *cblk)
+// The 2 x 4 blocks of output row pairs [p0, p1) x strips [xb0, xb1), with the K kernel rows of a block
+// on K different threads: thread (block, ka) forms the two fresh per-kernel-row partials of
+// ConvBlock<K>::run (same code: ConvBlock<K>::row), they go to `part` in shared memory, and one
+// thread per (block, output row) adds them in the order ka = 0 .. K-1 -- the sums ConvBlock<K>::run
+// forms, bit for bit, in 1/K of its time.  `part`: [blockDim.x / K blocks][K][8] floats.
+template <int K>
+__device__ __forceinline__ void conv_blocks_split(const KArgs &a, const float *img, int e0, const float *taps, float *part,
+                                                  int p0, int p1, int xb0, int xb1,
+                                                  const float *data, const float *wgt, float *image_out, float *cblk)
+{
+    using CB = ConvBlock<K>;
+    const int nsx = (a.nx + 3) / 4;
+    const int nbx = xb1 - xb0, nblk = (p1 - p0) * nbx;
+    const int per_pass = blockDim.x / K;               // whole blocks per pass
+    for (int b0 = 0; b0 < nblk; b0 += per_pass) {
+        const int nb = min(per_pass, nblk - b0);
+        if (b0) __syncthreads();                       // the previous pass has read `part`
+        if ((int)threadIdx.x < nb * K) {
+            const int bl = threadIdx.x / K, ka = threadIdx.x - bl * K, blk = b0 + bl;
+            const int ip = blk / nbx, xb = xb0 + (blk - ip * nbx), i = 2 * (p0 + ip), x0 = xb * 4;
+            const float *win = img + (i - e0 + ka) * a.pitch + x0;
+            float4 wa[CB::NW], wb[CB::NW];
+            CB::load_window(wa, win);
+            CB::load_window(wb, win + a.pitch);
+            float q0[4] = {0.f, 0.f, 0.f, 0.f}, q1[4] = {0.f, 0.f, 0.f, 0.f};
+            CB::row(wa, taps + ka * CB::Kp, q0);
+            CB::row(wb, taps + ka * CB::Kp, q1);
+            float4 *dst = reinterpret_cast<float4 *>(part + (size_t)threadIdx.x * 8);
+            dst[0] = make_float4(q0[0], q0[1], q0[2], q0[3]);
+            dst[1] = make_float4(q1[0], q1[1], q1[2], q1[3]);
+        }
+        __syncthreads();
+        // (block, output row) on adjacent lanes; whole warps take part in the shuffle
+        if ((int)(threadIdx.x & ~31u) < 2 * nb) {
+            const int t = threadIdx.x, bl = t >> 1, rs = t & 1, blk = b0 + bl;
+            float c = 0.f;
+            int ip = 0, xb = 0;
+            if (t < 2 * nb) {
+                ip = blk / nbx; xb = xb0 + (blk - ip * nbx);
+                const int i = 2 * (p0 + ip) + rs, x0 = xb * 4;
+                float acc[4] = {0.f, 0.f, 0.f, 0.f};
+                const float4 *src = reinterpret_cast<const float4 *>(part + (size_t)bl * K * 8 + rs * 4);
+#pragma unroll
+                for (int ka = 0; ka < K; ++ka) {
+                    const float4 v = src[2 * ka];
+                    acc[0] += v.x; acc[1] += v.y; acc[2] += v.z; acc[3] += v.w;
+                }
+                if (i < a.ny) c = chi2_strip(a, acc, i, x0, data, wgt, image_out);
+            }
+            const float c1 = __shfl_down_sync(0xffffffffu, c, 1);
+            if (t < 2 * nb && rs == 0) {
+                if (2 * (p0 + ip) + 1 < a.ny) c += c1;
+                if (cblk) cblk[(p0 + ip) * nsx + xb] = c;
+            }
+        }
+    }
+}
+
+// one CTA per (row, band of `band_pairs` output row pairs x one of `xseg` runs of strips); cblk:
+// [chunk][npair * nsx] or null; a.tile_counters[chunk_rows + r] (zeroed) counts the finished CTAs of row r.
+// xseg = 0: whole bands, one thread per block (conv_blocks_store: more rows than the split form pays for)
+__global__ void __launch_bounds__(512) conv_small_kernel(const KArgs a, int chunk_rows, int band_pairs, int xseg, float *cblk)
 {
     __shared__ double red[32];
     __shared__ int is_last;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float *taps = reinterpret_cast<float *>(smem_raw);
-    float *img = taps + a.K * a.Kp;
+    float *part = taps + a.K * a.Kp;                                // [blockDim.x / K][K][8]
+    float *img = xseg ? part + (blockDim.x / a.K) * a.K * 8 : part;
     const int r = blockIdx.x;
     const int npair = (a.ny + 1) / 2, nsx = (a.nx + 3) / 4;
-    const int p0 = blockIdx.y * band_pairs, p1 = min(npair, p0 + band_pairs);
-    if (p0 >= p1) return;
+    const int nseg = xseg ? xseg : 1;
+    const int band = blockIdx.y / nseg, seg = blockIdx.y - band * nseg;
+    const int p0 = band * band_pairs, p1 = min(npair, p0 + band_pairs);
+    const int xb0 = (int)((long long)nsx * seg / nseg), xb1 = (int)((long long)nsx * (seg + 1) / nseg);
     const int64_t row = a.row0 + r;
     const int64_t lens = row / a.rows_per_lens;
     const size_t npix = (size_t)a.ny * a.nx;
     load_psf(taps, a.psf + lens * a.K * a.Kp, a.K * a.Kp);          // context data: before the wait
     pdl_wait();                                                   // rows / ext come from the preceding kernels
     if (!row_is_valid(a.rows[r], a.n_comp)) {
-        if (a.images)
+        if (a.images && seg == 0)
             for (size_t i = (size_t)2 * p0 * a.nx + threadIdx.x; i < (size_t)min(a.ny, 2 * p1) * a.nx; i += blockDim.x)
                 a.images[row * npix + i] = NAN;
         if (a.logL && blockIdx.y == 0 && threadIdx.x == 0) a.logL[row] = -INFINITY;
@@ -879,8 +1034,11 @@ __global__ void __launch_bounds__(512) conv_small_kernel(const KArgs a, int chun
     const float *data = a.logL ? a.data + lens * npix : nullptr;
     float *image_out = a.images ? a.images + row * npix : nullptr;
     float *cb = (a.logL && cblk) ? cblk + (size_t)r * npair * nsx : nullptr;
-#define TL_CONV_CASE(KK) \
-    case KK: conv_blocks_store<KK>(a, img, e0, taps, p0, p1, data, a.wgt + lens * npix, image_out, cb); break;
+#define TL_CONV_CASE(KK)                                                                                                       \
+    case KK:                                                                                                                   \
+        if (xseg) conv_blocks_split<KK>(a, img, e0, taps, part, p0, p1, xb0, xb1, data, a.wgt + lens * npix, image_out, cb);   \
+        else conv_blocks_store<KK>(a, img, e0, taps, p0, p1, data, a.wgt + lens * npix, image_out, cb);                        \
+        break;
     switch (a.K) {
         TL_CONV_CASE(5)
         TL_CONV_CASE(15)
@@ -900,9 +1058,9 @@ __global__ void __launch_bounds__(512) conv_small_kernel(const KArgs a, int chun
     if (!is_last) return;
     __threadfence();
     const int total = npair * nsx;
-    double part = 0.0;
-    for (int s = threadIdx.x; s < total; s += blockDim.x) part += (double)__ldcg(cb + s);
-    const double chi2 = block_sum(part, red);
+    double psum = 0.0;
+    for (int s = threadIdx.x; s < total; s += blockDim.x) psum += (double)__ldcg(cb + s);
+    const double chi2 = block_sum(psum, red);
     if (threadIdx.x == 0) a.logL[row] = (float)(-0.5 * (chi2 + a.lconst[lens]));
 }
 

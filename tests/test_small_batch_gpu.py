@@ -47,9 +47,12 @@ def test_small_batches_equal_the_fused_kernel_bitwise(api, w):
     prob = W.make_problem(w, _zero_render)
     small, fused = _contexts(api, prob)
     n_sm = small.info()["n_sm"]
-    for per_lens in (1, 3, 17, n_sm // 2 // w.n_lens):
+    # (up to 16 rows per call: one pair of sub-samples per lane, trace_pairs_kernel, where S is even)
+    for per_lens in (1, 2, 3, 8, 16 // w.n_lens, 17, n_sm // 2 // w.n_lens):
         rows = W.batch_rows(w, per_lens)
         rows[0, 0] = -1.0 if per_lens == 3 else rows[0, 0]                # an invalid row in one of the batches
+        if per_lens in (2, 8):                                            # q = 0.4: the q < 0.5 branch of the SIE
+            rows[-1, 1], rows[-1, 2] = 0.3, -0.305
         d = torch.from_numpy(rows).cuda()
         a, b = small.loglike(d), fused.loglike(d)
         ia, ib = small.render(d), fused.render(d)
