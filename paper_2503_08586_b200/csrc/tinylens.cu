@@ -217,7 +217,7 @@ int run_small_batch(tl_ctx *c, const float *params, int64_t B, float *logL, floa
     fill_prologue_args(c, pa, params, rows, nb, 0, B / c->cfg.n_lens, 0);
     pa.zero_words = reinterpret_cast<int *>(reinterpret_cast<unsigned char *>(ext) + img_bytes); pa.n_zero_words = 2 * nb;
     pa.pad_ext = ext; pa.pad_rows = nb * c->He; pa.pad_pitch = c->pitch; pa.pad_We = c->We;
-    tl::prologue_kernel<<<(unsigned)((nb * (1 + c->n_comp) + 127) / 128), 128, 0, st>>>(pa);
+    tl::prologue_kernel<<<tl::prologue_blocks(nb), 128, 0, st>>>(pa);
     tl::KArgs a = base_args(c);
     a.rows = rows; a.B = nb; a.rows_per_lens = B / c->cfg.n_lens; a.row0 = 0;
     a.logL = logL; a.images = images; a.ext = ext; a.rowtab = c->sb_rowtab;
@@ -414,8 +414,7 @@ int run_batch(tl_ctx *c, const float *params, int64_t B, float *logL, float *ima
         const int64_t nb = (B - r0 < chunk) ? (B - r0) : chunk;
         tl::PrologueArgs pa;
         fill_prologue_args(c, pa, params, rows, nb, r0, rows_per_lens, 0);
-        const int64_t nthr = nb * (1 + c->n_comp);
-        tl::prologue_kernel<<<(unsigned)((nthr + 127) / 128), 128, 0, st>>>(pa);
+        tl::prologue_kernel<<<tl::prologue_blocks(nb), 128, 0, st>>>(pa);
 
         tl::KArgs a = base_args(c);
         a.rows = rows; a.B = nb; a.rows_per_lens = rows_per_lens; a.row0 = r0;
@@ -801,8 +800,7 @@ int tl_loglike_linear_batch(tl_ctx *c, const float *params, int64_t B, float *lo
             const int64_t nb = (B - r0 < chunkf) ? (B - r0) : chunkf;
             tl::PrologueArgs pa;
             fill_prologue_args(c, pa, params, rowsf, nb, r0, rpl, 1);
-            const int64_t nthr = nb * (1 + c->n_comp);
-            tl::prologue_kernel<<<(unsigned)((nthr + 127) / 128), 128, 0, st>>>(pa);
+            tl::prologue_kernel<<<tl::prologue_blocks(nb), 128, 0, st>>>(pa);
             tl::KArgs a = base_args(c);
             a.rows = rowsf; a.B = nb; a.rows_per_lens = rpl; a.row0 = r0;
             a.logL = logL; a.amps = amps; a.mimg = mscr; a.rowtab = c->lin_fused_rowtab;
@@ -837,8 +835,7 @@ int tl_loglike_linear_batch(tl_ctx *c, const float *params, int64_t B, float *lo
         const int64_t nb = (B - r0 < chunk) ? (B - r0) : chunk;
         tl::PrologueArgs pa;
         fill_prologue_args(c, pa, params, rows, nb, r0, rows_per_lens, 1);
-        const int64_t nthr = nb * (1 + c->n_comp);
-        tl::prologue_kernel<<<(unsigned)((nthr + 127) / 128), 128, 0, st>>>(pa);
+        tl::prologue_kernel<<<tl::prologue_blocks(nb), 128, 0, st>>>(pa);
         tl::KArgs a = base_args(c);
         a.rows = rows; a.B = nb; a.rows_per_lens = rows_per_lens; a.row0 = r0;
         a.logL = logL; a.amps = amps; a.ext = ext; a.mimg = mimg;
@@ -977,7 +974,7 @@ int run_mge_dp(tl_ctx *c, const float *params, int64_t B, float *logL, float *am
         tl::PrologueArgs pa;
         fill_prologue_args(c, pa, params, rows, nb, r0, rows_per_lens, 1);
         pa.mge = 1;
-        tl::prologue_kernel<<<(unsigned)((nb * (1 + c->n_comp) + 127) / 128), 128, 0, st>>>(pa);
+        tl::prologue_kernel<<<tl::prologue_blocks(nb), 128, 0, st>>>(pa);
         tl::DpArgs d;
         memset(&d, 0, sizeof(d));
         d.params = params; d.rows = rowsd; d.n_rows = (int)nb; d.row0 = r0; d.rows_per_lens = rows_per_lens;
@@ -1068,8 +1065,7 @@ int tl_loglike_mge_batch(tl_ctx *c, const float *params, int64_t B, float *logL,
         tl::PrologueArgs pa;
         fill_prologue_args(c, pa, params, rows, nb, r0, rows_per_lens, 1);
         pa.mge = 1;
-        const int64_t nthr = nb * (1 + c->n_comp);
-        tl::prologue_kernel<<<(unsigned)((nthr + 127) / 128), 128, 0, st>>>(pa);
+        tl::prologue_kernel<<<tl::prologue_blocks(nb), 128, 0, st>>>(pa);
         tl::KArgs a = base_args(c);
         a.rows = rows; a.B = nb; a.rows_per_lens = rows_per_lens; a.row0 = r0;
         a.logL = logL; a.amps = amps; a.ext = ext; a.mimg = mimg;

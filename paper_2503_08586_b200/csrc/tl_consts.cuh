@@ -217,22 +217,9 @@ __device__ inline bool shape_from_e(double e1, double e2, double *q, double *c, 
 }
 
 #ifdef TL_MAIN_TU
-__global__ void __launch_bounds__(128) prologue_kernel(PrologueArgs a)
+// the constants of one slot of one row: slot 0 = lens, slot 1 + k = Sersic component k
+__device__ __forceinline__ void prologue_slot(const PrologueArgs &a, int64_t row, int slot)
 {
-    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // (small-batch path: see tl_kernels.cuh pdl_*)
-    const int nslot = 1 + a.n_lens_light + a.n_source;
-    int64_t gid = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (a.zero_words || a.pad_ext) {
-        const int64_t nthr = (int64_t)gridDim.x * blockDim.x;
-        for (int64_t i = gid; i < a.n_zero_words; i += nthr) a.zero_words[i] = 0;
-        const int pw = a.pad_pitch - a.pad_We;
-        if (a.pad_ext && pw > 0)
-            for (int64_t i = gid; i < (int64_t)a.pad_rows * pw; i += nthr)
-                a.pad_ext[(i / pw) * a.pad_pitch + a.pad_We + (i % pw)] = 0.f;
-    }
-    if (gid >= a.B * nslot) return;
-    int64_t row = gid / nslot;
-    int slot = (int)(gid - row * nslot);
     const float *p = a.params + row * a.P;
     RowC *rc = a.rows + row;
 
@@ -401,6 +388,30 @@ __global__ void __launch_bounds__(128) prologue_kernel(PrologueArgs a)
     // and the shape of the Gaussian set after them (comp[n_source])
     rc->comp[a.mge ? (is_lens_light ? a.n_source + k : k - a.n_lens_light) : k] = C;
 }
+
+// One block = 32 rows; warp w takes slot w, w + 4, ... of them, so that the lens branch and the Sersic
+// branch never share a warp (they are long FP64 chains: side by side in a warp they run one after the
+// other, which was half of a one-row call's prologue).  Grid: prologue_blocks(B).
+__global__ void __launch_bounds__(128) prologue_kernel(PrologueArgs a)
+{
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // (small-batch path: see tl_kernels.cuh pdl_*)
+    const int nslot = 1 + a.n_lens_light + a.n_source;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+    const int64_t row = (int64_t)blockIdx.x * 32 + lane;
+    if (a.zero_words || a.pad_ext) {
+        // the idle warps of the last block first: on a one-row call the lens / Sersic warps do not wait for this
+        const int64_t nthr = (int64_t)gridDim.x * blockDim.x;
+        const int64_t gid = nthr - 1 - ((int64_t)blockIdx.x * blockDim.x + threadIdx.x);
+        for (int64_t i = gid; i < a.n_zero_words; i += nthr) a.zero_words[i] = 0;
+        const int pw = a.pad_pitch - a.pad_We;
+        if (a.pad_ext && pw > 0)
+            for (int64_t i = gid; i < (int64_t)a.pad_rows * pw; i += nthr)
+                a.pad_ext[(i / pw) * a.pad_pitch + a.pad_We + (i % pw)] = 0.f;
+    }
+    if (row >= a.B) return;
+    for (int slot = warp; slot < nslot; slot += nwarp) prologue_slot(a, row, slot);
+}
+inline unsigned prologue_blocks(int64_t B) { return (unsigned)((B + 31) / 32); }
 
 #endif  // TL_MAIN_TU
 
