@@ -197,6 +197,34 @@ __device__ __forceinline__ f2 sample_pair_parts(const HotC<NLL, NSRC, MASS_SIE> 
     any = any || f0 || f1;
     return mk2(s0, s1);
 }
+// Linear-amplitude mode: the sources stay apart (s[k], each at its unit amplitude); a half of s[0] is NaN
+// when that sample wants the FP64 ray-trace.
+template <int NLL, int NSRC>
+__device__ __forceinline__ void sample_pair_comps(const HotC<NLL, NSRC, MASS_SIE> &h, const ColV2 &c, const RowV &r, f2 &llv,
+                                                  f2 (&s)[NSRC], bool &any)
+{
+    if (NLL) llv = sersic_from_t2(h.ll, fma2(c.LB, bc2(r.dyl), add2(c.LA, bc2(r.LC))));
+    const f2 xp = add2(c.Pc, bc2(r.Qs)), yp = fma2(c.Ps, bc2(-1.f), bc2(r.Qc));
+    f2 axp, ayp;
+    sie_alpha2(h.sie, xp, yp, axp, ayp);
+    const f2 bx = fma2(axp, bc2(-1.f), add2(c.U, bc2(r.V))), by = fma2(ayp, bc2(-1.f), add2(c.U2, bc2(r.V2)));   // R^T (beta - s_1)
+    bool f0, f1;
+    s[0] = mul2(bc2(h.src[0].amp), sersic_from_t2(h.src[0], quad_form2(h.q[0], bx, by), f0, f1));
+    if (NSRC > 1) {
+        const f2 ex = add2(add2(bx, bc2(-h.q[1].oxh)), bc2(-h.q[1].oxl)), ey = add2(add2(by, bc2(-h.q[1].oyh)), bc2(-h.q[1].oyl));
+        bool g0, g1;
+        s[NSRC - 1] = mul2(bc2(h.src[1].amp), sersic_from_t2(h.src[1], quad_form2(h.q[1], ex, ey), g0, g1));
+        f0 = f0 || g0; f1 = f1 || g1;
+    }
+    if (f0 || f1) {
+        float s0, s1;
+        un2(s[0], s0, s1);
+        if (f0) s0 = __int_as_float(0x7fc00000);       // NaN marks "refine me"
+        if (f1) s1 = __int_as_float(0x7fc00000);
+        s[0] = mk2(s0, s1);
+        any = true;
+    }
+}
 // ... with the lens light added to `acc2`
 template <int NLL, int NSRC>
 __device__ __forceinline__ f2 sample_pair(const HotC<NLL, NSRC, MASS_SIE> &h, const ColV2 &c, const RowV &r, f2 &acc2, bool &any)
@@ -252,7 +280,7 @@ __device__ __forceinline__ void trace_tiles(const RowC &rc, const HotC<NLL, NSRC
     // u-units: X = 2 (j S + b) + 1 - S We is the exact sub-sample abscissa (DESIGN.md a1)
     float X0 = (float)(2 * j * S + 1 - S * a.We);
     // even compile-time S, SIE polynomial path, components summed: pairs of sub-samples (tl_pair.cuh)
-    constexpr bool PAIR = S_T > 0 && S_T % 2 == 0 && MASS == MASS_SIE && FAST && !LIN;
+    constexpr bool PAIR = S_T > 0 && S_T % 2 == 0 && MASS == MASS_SIE && FAST;
     constexpr int NP = PAIR ? S_T / 2 : 1;
     ColV cv[(S_T > 0 && !PAIR) ? S_T : 1];
     ColV2 cv2[NP];
@@ -278,11 +306,45 @@ __device__ __forceinline__ void trace_tiles(const RowC &rc, const HotC<NLL, NSRC
             if (!edge) {
                 const float Y0 = (float)(2 * i * S + 1 - S * a.He);
                 f2 acc2 = bc2(0.f);
+                f2 accs2[NSRC];                        // (LIN with pairs)
+#pragma unroll
+                for (int k = 0; k < NSRC; ++k) accs2[k] = bc2(0.f);
 #pragma unroll 1
                 for (int sa = 0; sa < S; ++sa) {
                     const float Y = Y0 + (float)(2 * sa);
                     const RowV rv = rowtab ? rowtab[i * S + sa] : row_values<NLL>(rc, Y);
-                    if constexpr (PAIR) {
+                    if constexpr (PAIR && LIN) {
+                        f2 sk[NP][NSRC];
+                        bool any = false;
+#pragma unroll
+                        for (int sp = 0; sp < NP; ++sp) {
+                            f2 llv;
+                            llv.v = 0ull;
+                            sample_pair_comps<NLL, NSRC>(h, cv2[sp], rv, llv, sk[sp], any);
+                            if (NLL) acc2 = fma2(bc2(h.ll.amp), llv, acc2);
+                        }
+                        if (any) {                                  // rare: FP64 ray-trace, out of line
+#pragma unroll
+                            for (int sp = 0; sp < NP; ++sp) {
+                                float m0, m1;
+                                un2(sk[sp][0], m0, m1);
+                                if (m0 != m0 || m1 != m1) {
+#pragma unroll
+                                    for (int k = 0; k < NSRC; ++k) {
+                                        float s0, s1;
+                                        un2(sk[sp][k], s0, s1);
+                                        if (m0 != m0) s0 = refined_source_light_k<MASS>(rc, NLL + k, X0 + (float)(4 * sp), Y);
+                                        if (m1 != m1) s1 = refined_source_light_k<MASS>(rc, NLL + k, X0 + (float)(4 * sp + 2), Y);
+                                        sk[sp][k] = mk2(s0, s1);
+                                    }
+                                }
+                            }
+                        }
+#pragma unroll
+                        for (int sp = 0; sp < NP; ++sp)
+#pragma unroll
+                            for (int k = 0; k < NSRC; ++k) accs2[k] = add2(accs2[k], sk[sp][k]);
+                    } else if constexpr (PAIR) {
                         f2 src2[NP];
                         bool any = false;
 #pragma unroll
@@ -368,6 +430,10 @@ __device__ __forceinline__ void trace_tiles(const RowC &rc, const HotC<NLL, NSRC
                     }
                 }
                 if constexpr (PAIR) { float a0, a1; un2(acc2, a0, a1); acc = a0 + a1; }
+                if constexpr (PAIR && LIN) {
+#pragma unroll
+                    for (int k = 0; k < NSRC; ++k) { float a0, a1; un2(accs2[k], a0, a1); accs[k] = a0 + a1; }
+                }
             }
             if constexpr (LIN) {
                 if (NLL) store(i, j, 0, acc);
