@@ -203,6 +203,34 @@ int tl_loglike_batch(tl_ctx *ctx, const float *params, int64_t B, float *logL, v
 int tl_render_batch(tl_ctx *ctx, const float *params, int64_t B, float *images, void *cuda_stream);
 
 /*
+ * tl_loglike_batch_noalloc -- tl_loglike_batch (Eq. 5; same steps a0-a7, same kernels,
+ * same bits) for callers that may not allocate: code under CUDA graph capture, serving loops,
+ * harnesses that forbid cudaMalloc.  tl_loglike_batch takes its per-call scratch -- the array of
+ * per-row constants that the prologue kernel writes and the fused kernel reads, 1280 bytes per row --
+ * from the context's stream-ordered memory pool; this call keeps it in a fixed array in the library's
+ * device image instead (TL_NOALLOC_MAX_ROWS rows = 5 MiB, held by every GPU that loads the library
+ * until the process exits) and calls no cudaMalloc, cudaFree, cudaMallocAsync, cudaFreeAsync or any
+ * other allocating routine.
+ *   params, logL, cuda_stream   as for tl_loglike_batch (DEVICE pointers, caller-owned; asynchronous)
+ *   B          0 <= B <= TL_NOALLOC_MAX_ROWS, a multiple of n_lens.  B = 0 (params and logL may be NULL)
+ *              only resolves the array's device address, which the first call on each device does once
+ *              (cudaGetSymbolAddress: no allocation, but make that first call outside graph capture).
+ * Returns TL_ESIZE when B > TL_NOALLOC_MAX_ROWS (split a larger batch into several calls on ONE stream)
+ * or when the context runs the split path (images too large for one CTA's shared memory: that path
+ * needs a binned image per row in global memory); TL_EINVAL for a NULL pointer with B > 0, for B not a
+ * multiple of n_lens and for a context whose precision is not TL_PRECISION_FP32; TL_ECUDA as usual.
+ * logL is bit for bit tl_loglike_batch's in TL_PRECISION_FP32 mode: every row goes through the fused
+ * kernel, whose result the small-batch path of tl_loglike_batch reproduces bitwise.
+ * SHARED STATE.  Every context and every call on a device shares the one array, which keeps the
+ * contents of the last call; nothing in it has to start at zero (the prologue rewrites every field of
+ * rows 0 .. B-1 that the fused kernel reads, and no other row is read).  Calls that can overlap on the
+ * GPU -- different streams, or graph branches, without an ordering between them -- RACE on the array and
+ * return garbage: order them (one stream, or events).  tl_loglike_batch has no such restriction.
+ */
+#define TL_NOALLOC_MAX_ROWS 4096
+int tl_loglike_batch_noalloc(tl_ctx *ctx, const float *params, int64_t B, float *logL, void *cuda_stream);
+
+/*
  * tl_loglike_linear_batch -- the paper's linear/non-linear split (Eq. 6,
  * :97-129 Eq. 7): for every row the amplitudes s of the N_l + N_s light components are not
  * parameters but are solved as the non-negative least-squares minimiser of

@@ -83,6 +83,7 @@ def load(build_if_missing: bool = True):
     L.tl_get_info.restype = C.c_int; L.tl_get_info.argtypes = [vp, C.POINTER(tl_info)]
     L.tl_loglike_batch.restype = C.c_int; L.tl_loglike_batch.argtypes = [vp, vp, i64, vp, vp]
     L.tl_render_batch.restype = C.c_int; L.tl_render_batch.argtypes = [vp, vp, i64, vp, vp]
+    L.tl_loglike_batch_noalloc.restype = C.c_int; L.tl_loglike_batch_noalloc.argtypes = [vp, vp, i64, vp, vp]
     L.tl_loglike_batch_host.restype = C.c_int; L.tl_loglike_batch_host.argtypes = [vp, vp, i64, vp, vp]
     L.tl_loglike_batch_host_async.restype = C.c_int; L.tl_loglike_batch_host_async.argtypes = [vp, vp, i64, vp, vp]
     L.tl_wait.restype = C.c_int; L.tl_wait.argtypes = [vp, C.c_int]
@@ -212,6 +213,23 @@ def tl_loglike_batch(handle: int, params, out=None, stream=None):
         _check_out(out, (B,), params.device, "out")
     _check(load().tl_loglike_batch(handle, params.data_ptr(), B, out.data_ptr(), _stream_handle(stream)),
            "tl_loglike_batch")
+    return out
+
+
+TL_NOALLOC_MAX_ROWS = 4096
+
+
+def tl_loglike_batch_noalloc(handle: int, params, out, stream=None):
+    """tl_loglike_batch without any allocation in the library (include/tinylens.h): params CUDA float32
+    [B,P], B <= TL_NOALLOC_MAX_ROWS, written into the caller's `out` (CUDA float32 [B]).  Calls that can
+    overlap on the GPU race on the library's fixed scratch array: keep them on one stream."""
+    B = _dev_rows(handle, params)
+    _check_out(out, (B,), params.device, "out")
+    code = load().tl_loglike_batch_noalloc(handle, params.data_ptr(), B, out.data_ptr(), _stream_handle(stream))
+    if code == TL_ESIZE and B > TL_NOALLOC_MAX_ROWS:
+        raise TinyLensError(code, "tl_loglike_batch_noalloc: B = %d exceeds TL_NOALLOC_MAX_ROWS = %d (split the batch "
+                            "into several calls on one stream)" % (B, TL_NOALLOC_MAX_ROWS))
+    _check(code, "tl_loglike_batch_noalloc")
     return out
 
 
@@ -391,6 +409,9 @@ class LensContext:
 
     def loglike(self, params, out=None, stream=None):
         return tl_loglike_batch(self.handle, params, out, stream)
+
+    def loglike_noalloc(self, params, out, stream=None):
+        return tl_loglike_batch_noalloc(self.handle, params, out, stream)
 
     def render(self, params, out=None, stream=None):
         return tl_render_batch(self.handle, params, self.ny, self.nx, out, stream)

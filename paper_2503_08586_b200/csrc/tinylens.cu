@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -454,6 +455,68 @@ int run_batch(tl_ctx *c, const float *params, int64_t B, float *logL, float *ima
 }
 
 }  // namespace
+
+// ------------------------------------------------------------------ tl_loglike_batch_noalloc
+// The per-row constants of tl_loglike_batch's fused path (RowC[B], written by prologue_kernel, read by
+// fused_kernel) in a fixed array of the device image instead of pool memory: see include/tinylens.h.
+// Every device that loads the library holds the array (5 MiB) until the process exits; every call on
+// a device shares it.
+static __device__ __align__(256) unsigned char tl_noalloc_scratch[(size_t)TL_NOALLOC_MAX_ROWS * sizeof(tl::RowC)];
+
+namespace {
+
+constexpr int NOALLOC_MAX_DEVICES = 64;
+std::mutex g_noalloc_mu;
+void *g_noalloc_addr[NOALLOC_MAX_DEVICES];          // device address of the array on device d; null = not resolved yet
+
+// In host code `tl_noalloc_scratch` is a host-side stand-in for the symbol, not a device address: a
+// kernel handed &tl_noalloc_scratch faults (or scribbles over host memory where the GPU can reach it).
+// The address on `device` -- which must be current -- comes from cudaGetSymbolAddress, once per device.
+bool noalloc_rows(int device, tl::RowC **out)
+{
+    if (device < 0 || device >= NOALLOC_MAX_DEVICES) return false;
+    std::lock_guard<std::mutex> lock(g_noalloc_mu);
+    if (!g_noalloc_addr[device]) {
+        void *p = nullptr;
+        if (!cuda_ok(cudaGetSymbolAddress(&p, tl_noalloc_scratch)) || !p) return false;
+        g_noalloc_addr[device] = p;
+    }
+    *out = static_cast<tl::RowC *>(g_noalloc_addr[device]);
+    return true;
+}
+
+}  // namespace
+
+extern "C" {
+
+int tl_loglike_batch_noalloc(tl_ctx *c, const float *params, int64_t B, float *logL, void *cuda_stream)
+{
+    if (!c || B < 0) return TL_EINVAL;
+    if (B > TL_NOALLOC_MAX_ROWS) return TL_ESIZE;                 // the array holds TL_NOALLOC_MAX_ROWS rows
+    if (c->path != 0) return TL_ESIZE;                            // split path: needs an image per row in global memory
+    if (c->precision != TL_PRECISION_FP32 || c->cfg.n_lens_light > 1) return TL_EINVAL;
+    if (B > 0 && (!params || !logL)) return TL_EINVAL;
+    if (B % c->cfg.n_lens) return TL_EINVAL;
+    DeviceGuard guard(c->device);
+    if (!guard.ok) return TL_ECUDA;
+    tl::RowC *rows = nullptr;
+    if (!noalloc_rows(c->device, &rows)) return TL_ECUDA;
+    if (B == 0) return TL_OK;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    // one chunk: the two launches of run_batch's fused path, `rows` being the fixed array
+    tl::PrologueArgs pa;
+    fill_prologue_args(c, pa, params, rows, B, 0, B / c->cfg.n_lens, 0);
+    tl::prologue_kernel<<<tl::prologue_blocks(B), 128, 0, st>>>(pa);
+    tl::KArgs a = base_args(c);
+    a.rows = rows; a.B = B; a.rows_per_lens = B / c->cfg.n_lens; a.row0 = 0;
+    a.logL = logL; a.images = nullptr;
+    int grid = c->grid;
+    if ((int64_t)grid > B) grid = (int)B;
+    c->fused<<<grid, c->threads, c->smem, st>>>(a);
+    return cuda_ok(cudaGetLastError()) ? TL_OK : TL_ECUDA;
+}
+
+}  // extern "C"
 
 extern "C" {
 
