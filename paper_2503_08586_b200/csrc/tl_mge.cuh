@@ -96,12 +96,45 @@ __global__ void __launch_bounds__(256) mge_gauss_kernel(const KArgs a, int chunk
     }
 }
 
+// The 2 x 4 blocks of output row pairs ip0 .. ip1 x strips xb0 .. xb1 (inclusive) of one blurred image
+// -> image_out; every other pixel of image_out is written as 0.  (gauss_conv_kernel: outside that
+// rectangle every window holds nothing but exact zeros, and ConvBlock's sums of +-0 products are +0.)
+template <int K>
+__device__ __forceinline__ void conv_blocks_rect(const KArgs &a, const float *img, const float *taps,
+                                                 int ip0, int ip1, int xb0, int xb1, float *image_out)
+{
+    const int nsx = (a.nx + 3) / 4, npair = (a.ny + 1) / 2;
+    const int nbx = xb1 - xb0 + 1, nby = ip1 - ip0 + 1;
+    const float zero[4] = {0.f, 0.f, 0.f, 0.f};
+    if (nbx > 0 && nby > 0) {
+        for (int s = threadIdx.x; s < nby * nbx; s += blockDim.x) {
+            const int iy = s / nbx, i = 2 * (ip0 + iy), x0 = 4 * (xb0 + s - iy * nbx);
+            float a0[4], a1[4];
+            ConvBlock<K>::run(img + i * a.pitch + x0, a.pitch, taps, a0, a1);
+            chi2_strip(a, a0, i, x0, nullptr, nullptr, image_out);
+            if (i + 1 < a.ny) chi2_strip(a, a1, i + 1, x0, nullptr, nullptr, image_out);
+        }
+    }
+    for (int s = threadIdx.x; s < npair * nsx; s += blockDim.x) {
+        const int ip = s / nsx, xb = s - ip * nsx;
+        if (ip >= ip0 && ip <= ip1 && xb >= xb0 && xb <= xb1) continue;
+        chi2_strip(a, zero, 2 * ip, 4 * xb, nullptr, nullptr, image_out);
+        if (2 * ip + 1 < a.ny) chi2_strip(a, zero, 2 * ip + 1, 4 * xb, nullptr, nullptr, image_out);
+    }
+}
+
 // One CTA per (row, Gaussian k): steps a4-a6 for one column of M without a round trip through global
 // memory.  t = R_p^2 of a sub-sample is LA(x) + LC(y) + LB(x) dyl(y) (tl_kernels.cuh col_values /
 // row_values): the column parts of a pixel's S sub-columns are computed once per pixel and kept in
 // registers as pairs (tl_pair.cuh), the row parts once per sub-row, so a pair of samples costs
 // FADD2 + FFMA2 + FMUL2 + 2 MUFU.EX2 + FADD2.  The evaluation is MUFU-bound, the convolution
 // FMA-bound; with two or three CTAs per SM the two phases of different CTAs overlap.
+// Support box: 2^(-c_k t) is flushed to an exact 0 once c_k t > 126 (ex2.approx.ftz), and
+// t >= lambda_min rho^2, lambda_min the smaller eigenvalue of the set's quadratic form and rho the
+// distance from the centre; so outside a box of half-width rho_k = sqrt(130 / (0.98 lambda_min c_k))
+// round the centre every sub-sample is exactly 0.  Only the pixels of the box are evaluated and only
+// the outputs whose window meets the box are convolved; the rest of the column is written as 0 --
+// the same bits as evaluating everything (a 0.6-pixel Gaussian covers 1/30 of a 120 x 120 image).
 // S_T = 0: any S (scalar loop).
 template <int S_T>
 __global__ void __launch_bounds__(256) gauss_conv_kernel(const KArgs a, int chunk_rows)
@@ -122,11 +155,34 @@ __global__ void __launch_bounds__(256) gauss_conv_kernel(const KArgs a, int chun
     const int S = S_T > 0 ? S_T : a.S;
     const float inv_s2 = 1.f / (float)(S * S);
     const int npx = a.He * a.pitch;
-    for (int p = threadIdx.x; p < npx + a.pitch + a.Kp + 8; p += blockDim.x) {
-        const int i = p / a.pitch, j = p - i * a.pitch;
+    // the support box in extended pixels [i_lo, i_hi] x [j_lo, j_hi] (one pixel of slack on every side)
+    int i_lo = 0, i_hi = a.He - 1, j_lo = 0, j_hi = a.We - 1;
+    {
+        const float hd = 0.5f * (ah - cch), hb = 0.5f * b2h;
+        const float lmax = 0.5f * (ah + cch) + sqrtf(fmaf(hd, hd, hb * hb));
+        const float lmin = fmaf(ah, cch, -hb * hb) / lmax;
+        const float rho = sqrtf(130.f / (0.98f * lmin * -ck));              // u-units
+        if (lmin > 0.f && ck < 0.f && rho < 1e7f) {
+            const float inv2s = 0.5f / (float)S, cX = cXh + cXl, cY = cYh + cYl;
+            // pixel j spans X0 .. X0 + 2 (S - 1), X0 = 2 j S + 1 - S We
+            j_lo = max(j_lo, (int)floorf((cX - rho - (float)(2 * S - 1) + (float)(S * a.We)) * inv2s) - 1);
+            j_hi = min(j_hi, (int)ceilf((cX + rho - 1.f + (float)(S * a.We)) * inv2s) + 1);
+            i_lo = max(i_lo, (int)floorf((cY - rho - (float)(2 * S - 1) + (float)(S * a.He)) * inv2s) - 1);
+            i_hi = min(i_hi, (int)ceilf((cY + rho - 1.f + (float)(S * a.He)) * inv2s) + 1);
+        }
+    }
+    const int bw = j_hi - j_lo + 1, bh = i_hi - i_lo + 1;
+    {   // everything outside the box, the pitch padding and the slack read as zero
+        float4 *z = reinterpret_cast<float4 *>(img);
+        const int n4 = (npx + a.pitch + a.Kp + 8 + 3) / 4;
+        for (int p = threadIdx.x; p < n4; p += blockDim.x) z[p] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    __syncthreads();
+    for (int p = threadIdx.x; p < bw * bh; p += blockDim.x) {
+        const int ib = p / bw, i = i_lo + ib, j = j_lo + (p - ib * bw);
         float acc = 0.f;
         const bool edge = a.edge_zero && (j < a.h || j >= a.We - a.h || i < a.h || i >= a.He - a.h);
-        if (p < npx && j < a.We && !edge) {
+        if (!edge) {
             const float X0 = (float)(2 * j * S + 1 - S * a.We);
             float Y = (float)(2 * i * S + 1 - S * a.He);
             if constexpr (S_T > 0 && S_T % 2 == 0) {
@@ -175,11 +231,27 @@ __global__ void __launch_bounds__(256) gauss_conv_kernel(const KArgs a, int chun
             }
             acc *= inv_s2;
         }
-        img[p] = acc;                                  // pitch padding and slack read as zero
+        img[i * a.pitch + j] = acc;
     }
     __syncthreads();
     const size_t npix = (size_t)a.ny * a.nx;
-    conv_chi2_rows(a, img, 0, taps, 0, a.ny, nullptr, nullptr, a.mimg + ((size_t)r * a.ext_nc + k) * npix);
+    float *out = a.mimg + ((size_t)r * a.ext_nc + k) * npix;
+    // output (i, x) reads extended rows i .. i + K - 1 and columns x .. x + K - 1
+    const int oi0 = max(0, i_lo - a.K + 1), oi1 = min(a.ny - 1, i_hi), ox0 = max(0, j_lo - a.K + 1), ox1 = min(a.nx - 1, j_hi);
+    const bool none = bw <= 0 || bh <= 0 || oi0 > oi1 || ox0 > ox1;
+    const int ip0 = none ? 1 : oi0 / 2, ip1 = none ? 0 : oi1 / 2, xb0 = none ? 1 : ox0 / 4, xb1 = none ? 0 : ox1 / 4;
+#define TL_CONV_CASE(KK) \
+    case KK: conv_blocks_rect<KK>(a, img, taps, ip0, ip1, xb0, xb1, out); return;
+    switch (a.K) {
+        TL_CONV_CASE(5)
+        TL_CONV_CASE(15)
+        TL_CONV_CASE(21)
+        TL_CONV_CASE(31)
+        TL_CONV_CASE(41)
+    default: break;
+    }
+#undef TL_CONV_CASE
+    conv_chi2_rows(a, img, 0, taps, 0, a.ny, nullptr, nullptr, out);       // other PSF sizes: the generic strips, whole image
 }
 
 typedef void (*gauss_conv_fn)(const KArgs, int);
