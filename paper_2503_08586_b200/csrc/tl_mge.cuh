@@ -388,6 +388,102 @@ __global__ void __launch_bounds__(THREADS) gram_mge_kernel(const KArgs a, int ch
     }
 }
 
+// The same sums for up to MGE_GRAM_REG_COLS columns + data (the FP32 pipeline), every entry in a REGISTER
+// of every thread: gram_mge_kernel reads one operand from shared memory per DFMA and is bound by that
+// pipe at a quarter of the FP64 rate; here a thread takes two neighbouring pixels per step (one
+// 8-byte load per column, the next step's loads in flight meanwhile), forms w m_k once and feeds the
+// N1 (N1 + 1) / 2 entries from registers.  Fixed order: a thread's pixels in sequence, then a butterfly
+// over the warp and the four warps in order.  Needs an even pixel count.
+constexpr int MGE_GRAM_REG_COLS = 11;          // (13 columns + data would spill)
+template <int N1>
+__global__ void __launch_bounds__(128) gram_reg_kernel(const KArgs a, int chunk_rows)
+{
+    constexpr int NE = N1 * (N1 + 1) / 2;
+    __shared__ double red[4][NE];
+    const int r = blockIdx.x;
+    if (r >= chunk_rows) return;
+    const int64_t row = a.row0 + r;
+    constexpr int n = N1 - 1;
+    if (!row_is_valid(a.rows[r], a.n_comp)) return;   // nnls_mge_kernel reports the row
+    const int64_t lens = row / a.rows_per_lens;
+    const int npix = a.ny * a.nx, np2 = npix >> 1;
+    const float2 *M2 = reinterpret_cast<const float2 *>(a.mimg + (size_t)r * n * npix);
+    const float2 *d2 = reinterpret_cast<const float2 *>(a.data + lens * (size_t)npix);
+    const float2 *w2 = reinterpret_cast<const float2 *>(a.wgt + lens * (size_t)npix);
+    double acc[NE];
+#pragma unroll
+    for (int e = 0; e < NE; ++e) acc[e] = 0.0;
+    float2 cur[N1], nxt[N1], wc, wn;
+    auto fetch = [&](int p, float2 (&v)[N1], float2 &wv) {
+        if (p < np2) {
+#pragma unroll
+            for (int k = 0; k < n; ++k) v[k] = __ldg(M2 + (size_t)k * np2 + p);
+            v[n] = __ldg(d2 + p);
+            wv = __ldg(w2 + p);
+        } else {
+#pragma unroll
+            for (int k = 0; k < N1; ++k) v[k] = make_float2(0.f, 0.f);
+            wv = make_float2(0.f, 0.f);
+        }
+    };
+    auto pixel = [&](const double (&v)[N1], double wd) {
+        int e = 0;
+#pragma unroll
+        for (int k = 0; k < N1; ++k) {
+            const double wk = wd * v[k];
+#pragma unroll
+            for (int l = k; l < N1; ++l, ++e) acc[e] = fma(wk, v[l], acc[e]);
+        }
+    };
+    fetch(threadIdx.x, cur, wc);
+#pragma unroll 1
+    for (int p = threadIdx.x; p < np2; p += 128) {
+        fetch(p + 128, nxt, wn);
+        double v[N1];
+#pragma unroll
+        for (int k = 0; k < N1; ++k) v[k] = (double)cur[k].x;
+        pixel(v, (double)wc.x);
+#pragma unroll
+        for (int k = 0; k < N1; ++k) v[k] = (double)cur[k].y;
+        pixel(v, (double)wc.y);
+#pragma unroll
+        for (int k = 0; k < N1; ++k) cur[k] = nxt[k];
+        wc = wn;
+    }
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+#pragma unroll
+    for (int e = 0; e < NE; ++e) {
+        double v = acc[e];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0) red[warp][e] = v;
+    }
+    __syncthreads();
+    constexpr int NCG = MGE_MAX_COL + 1;                          // row pitch of G in a.mge_gram
+    double *gout = a.mge_gram + (size_t)r * MGE_GRAM_STRIDE;
+    for (int e = threadIdx.x; e < NE; e += 128) {
+        const double v = ((red[0][e] + red[1][e]) + red[2][e]) + red[3][e];
+        int k = 0, q = e;
+        while (q >= N1 - k) { q -= N1 - k; ++k; }
+        const int l = k + q;
+        if (l < n) { gout[k * NCG + l] = v; gout[l * NCG + k] = v; }
+        else if (k < n) gout[MGE_MAX_COL * NCG + k] = v;
+        else gout[MGE_MAX_COL * NCG + MGE_MAX_COL] = v;
+    }
+}
+
+typedef void (*gram_reg_fn)(const KArgs, int);
+inline gram_reg_fn gram_reg_for(int n1)
+{
+    switch (n1) {
+    case 2: return gram_reg_kernel<2>;   case 3: return gram_reg_kernel<3>;   case 4: return gram_reg_kernel<4>;
+    case 5: return gram_reg_kernel<5>;   case 6: return gram_reg_kernel<6>;   case 7: return gram_reg_kernel<7>;
+    case 8: return gram_reg_kernel<8>;   case 9: return gram_reg_kernel<9>;   case 10: return gram_reg_kernel<10>;
+    case 11: return gram_reg_kernel<11>; case 12: return gram_reg_kernel<12>;
+    default: return nullptr;
+    }
+}
+
 // NNLS: one warp per row (lane 0 iterates; the iteration is a chain of dependent FP64 operations
 // through shared memory, so what matters is how many rows are in flight per SM: 4 warps per CTA,
 // ~6 KB of shared memory each).  Writes the amplitudes (FP64, for resid_mge_kernel; float for the
