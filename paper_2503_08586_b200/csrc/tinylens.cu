@@ -1104,7 +1104,7 @@ int tl_loglike_mge_batch(tl_ctx *c, const float *params, int64_t B, float *logL,
     // the budget is a target, not a promise: when the device cannot give that much, halve the chunk
     for (;;) {
         rows = nullptr; ext = nullptr; mimg = nullptr; gram = nullptr;
-        if (pool_alloc(c, &rows, sizeof(tl::RowC) * (size_t)chunk, st) &&
+        if (pool_alloc(c, &rows, (sizeof(tl::RowC) + sizeof(int)) * (size_t)chunk, st) &&    // + one tile-queue head per row
             pool_alloc(c, &ext, ext_row * (size_t)chunk, st) &&
             pool_alloc(c, &mimg, m_row * (size_t)chunk, st) &&
             pool_alloc(c, &gram, g_row * (size_t)chunk, st)) break;
@@ -1135,9 +1135,13 @@ int tl_loglike_mge_batch(tl_ctx *c, const float *params, int64_t B, float *logL,
         a.tile_rows = c->lin_tile_rows; a.n_tiles = c->lin_n_tiles;
         a.n_gauss = NG; a.mge_c = c->mge_c; a.mge_set = c->mge_set; a.mge_gram = gram;
         // 1. the sources, ray-traced at unit amplitude -> ext slots (fused: 0.., else NG..)
+        // (the row's CTAs draw warp tiles from one queue per row: the tile next to the source centre, full of
+        // FP64-refined samples, costs several times an ordinary one and a static split leaves its CTA's other warps idle)
         tl::KArgs at = a;
         at.rowtab = c->mge_rowtab; at.ext_nc = ext_nc; at.ext_k0 = fused ? 0 : NG;
-        c->mge_trace<<<dim3((unsigned)nb, 8), 256, c->mge_trace_smem, st>>>(at, (int)nb);
+        at.tile_counters = reinterpret_cast<int *>(rows + chunk);
+        cudaMemsetAsync(at.tile_counters, 0, sizeof(int) * (size_t)nb, st);
+        c->mge_trace<<<dim3((unsigned)nb, 2), 256, c->mge_trace_smem, st>>>(at, (int)nb);       // (slabs per row: 1 .. 4 measured equal, 8 1 % slower)
         a.ext_nc = NC;                                         // from here on: the width of M
         if (fused) {
             // 2. every Gaussian evaluated into shared memory and blurred from there -> M[0 .. NG)

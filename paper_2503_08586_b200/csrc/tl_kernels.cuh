@@ -1149,7 +1149,8 @@ __global__ void __launch_bounds__(256, 2) trace_lin_kernel(const KArgs a, int ch
         if (rowtab) { fill_rowtab<NLL>(rc_s, a, rowtab); __syncthreads(); }
         float *dst = a.ext + ((size_t)r * (a.ext_nc ? a.ext_nc : NC) + a.ext_k0) * a.He * a.pitch;
         const size_t comp_stride = (size_t)a.He * a.pitch;
-        trace_image_lin<S_T, NLL, NSRC, MASS>(rc_s, a, rowtab, (blockIdx.y * blockDim.x + threadIdx.x) >> 5, (gridDim.y * blockDim.x) >> 5, nullptr,
+        trace_image_lin<S_T, NLL, NSRC, MASS>(rc_s, a, rowtab, (blockIdx.y * blockDim.x + threadIdx.x) >> 5, (gridDim.y * blockDim.x) >> 5,
+                                      a.tile_counters ? a.tile_counters + r : nullptr,
                                       [&](int i, int j, int k, float v) { dst[k * comp_stride + i * a.pitch + j] = v; });
     }
 }

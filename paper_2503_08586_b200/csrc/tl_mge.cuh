@@ -510,19 +510,24 @@ __global__ void __launch_bounds__(32 * MGE_NNLS_WARPS) nnls_mge_kernel(const KAr
     if (lane < n) bs[lane] = gin[MGE_MAX_COL * NCG + lane];
     const double dwd = gin[MGE_MAX_COL * NCG + MGE_MAX_COL];
     __syncwarp();
-    if (lane == 0) nnls_gram<MGE_MAX_COL>(n, Gs, n, bs, dwd, ss, Ls, zs, n);
-    __syncwarp();
+    nnls_gram_warp<MGE_MAX_COL>(n, Gs, n, bs, dwd, ss, Ls, n);
     if (lane < n && a.amps) a.amps[row * n + lane] = (float)ss[lane];
+    // chi^2 = d'Wd - 2 s'b + s'G s at the solved amplitudes (Eq. 5): lane i forms its terms,
+    // lane 0 adds them in column order
+    if (lane < n) {
+        const double si = ss[lane];
+        double gi = 0.0;
+        for (int k = 0; k < n; ++k) gi += Gs[lane * n + k] * ss[k];
+        zs[lane] = si * bs[lane];
+        Ls[lane] = si * gi;
+    }
+    __syncwarp();
     if (lane == 0) {
-        // chi^2 = d'Wd - 2 s'b + s'G s at the solved amplitudes (Eq. 5)
         double sb = 0.0, sGs = 0.0;
         for (int i = 0; i < n; ++i) {
-            const double si = ss[i];
-            if (si == 0.0) continue;
-            sb += si * bs[i];
-            double gi = 0.0;
-            for (int k = 0; k < n; ++k) gi += Gs[i * n + k] * ss[k];
-            sGs += si * gi;
+            if (ss[i] == 0.0) continue;
+            sb += zs[i];
+            sGs += Ls[i];
         }
         const double chi2 = (dwd - 2.0 * sb) + sGs;
         a.logL[row] = (float)(-0.5 * (chi2 + a.lconst[row / a.rows_per_lens]));
