@@ -174,13 +174,16 @@ __device__ __forceinline__ void sample_value(const RowC &rc, const HotC<NLL, NSR
 // Two horizontally adjacent sub-samples at once with packed FP32 arithmetic (tl_pair.cuh): the
 // lens-light profile values go to `llv` (not yet scaled by the amplitude), the sources are returned
 // (a half is NaN when that sample wants the FP64 ray-trace).
-template <int NLL, int NSRC>
-__device__ __forceinline__ f2 sample_pair_parts(const HotC<NLL, NSRC, MASS_SIE> &h, const ColV2 &c, const RowV &r, f2 &llv, bool &any)
+// MASS_EPL: (axp, ayp) come from the caller, which deflects the pairs of a sub-row together (epl_alpha_pairs).
+template <int NLL, int NSRC, int MASS = MASS_SIE>
+__device__ __forceinline__ f2 sample_pair_parts(const HotC<NLL, NSRC, MASS> &h, const ColV2 &c, const RowV &r, f2 &llv, bool &any,
+                                                f2 axp = f2{0ull}, f2 ayp = f2{0ull})
 {
     if (NLL) llv = sersic_from_t2(h.ll, fma2(c.LB, bc2(r.dyl), add2(c.LA, bc2(r.LC))));
-    const f2 xp = add2(c.Pc, bc2(r.Qs)), yp = fma2(c.Ps, bc2(-1.f), bc2(r.Qc));
-    f2 axp, ayp;
-    sie_alpha2(h.sie, xp, yp, axp, ayp);
+    if constexpr (MASS == MASS_SIE) {
+        const f2 xp = add2(c.Pc, bc2(r.Qs)), yp = fma2(c.Ps, bc2(-1.f), bc2(r.Qc));
+        sie_alpha2(h.sie, xp, yp, axp, ayp);
+    }
     const f2 bx = fma2(axp, bc2(-1.f), add2(c.U, bc2(r.V))), by = fma2(ayp, bc2(-1.f), add2(c.U2, bc2(r.V2)));   // R^T (beta - s_1)
     bool f0, f1;
     f2 s = mul2(bc2(h.src[0].amp), sersic_from_t2(h.src[0], quad_form2(h.q[0], bx, by), f0, f1));
@@ -199,14 +202,15 @@ __device__ __forceinline__ f2 sample_pair_parts(const HotC<NLL, NSRC, MASS_SIE> 
 }
 // Linear-amplitude mode: the sources stay apart (s[k], each at its unit amplitude); a half of s[0] is NaN
 // when that sample wants the FP64 ray-trace.
-template <int NLL, int NSRC>
-__device__ __forceinline__ void sample_pair_comps(const HotC<NLL, NSRC, MASS_SIE> &h, const ColV2 &c, const RowV &r, f2 &llv,
-                                                  f2 (&s)[NSRC], bool &any)
+template <int NLL, int NSRC, int MASS = MASS_SIE>
+__device__ __forceinline__ void sample_pair_comps(const HotC<NLL, NSRC, MASS> &h, const ColV2 &c, const RowV &r, f2 &llv,
+                                                  f2 (&s)[NSRC], bool &any, f2 axp = f2{0ull}, f2 ayp = f2{0ull})
 {
     if (NLL) llv = sersic_from_t2(h.ll, fma2(c.LB, bc2(r.dyl), add2(c.LA, bc2(r.LC))));
-    const f2 xp = add2(c.Pc, bc2(r.Qs)), yp = fma2(c.Ps, bc2(-1.f), bc2(r.Qc));
-    f2 axp, ayp;
-    sie_alpha2(h.sie, xp, yp, axp, ayp);
+    if constexpr (MASS == MASS_SIE) {
+        const f2 xp = add2(c.Pc, bc2(r.Qs)), yp = fma2(c.Ps, bc2(-1.f), bc2(r.Qc));
+        sie_alpha2(h.sie, xp, yp, axp, ayp);
+    }
     const f2 bx = fma2(axp, bc2(-1.f), add2(c.U, bc2(r.V))), by = fma2(ayp, bc2(-1.f), add2(c.U2, bc2(r.V2)));   // R^T (beta - s_1)
     bool f0, f1;
     s[0] = mul2(bc2(h.src[0].amp), sersic_from_t2(h.src[0], quad_form2(h.q[0], bx, by), f0, f1));
@@ -226,12 +230,13 @@ __device__ __forceinline__ void sample_pair_comps(const HotC<NLL, NSRC, MASS_SIE
     }
 }
 // ... with the lens light added to `acc2`
-template <int NLL, int NSRC>
-__device__ __forceinline__ f2 sample_pair(const HotC<NLL, NSRC, MASS_SIE> &h, const ColV2 &c, const RowV &r, f2 &acc2, bool &any)
+template <int NLL, int NSRC, int MASS = MASS_SIE>
+__device__ __forceinline__ f2 sample_pair(const HotC<NLL, NSRC, MASS> &h, const ColV2 &c, const RowV &r, f2 &acc2, bool &any,
+                                          f2 axp = f2{0ull}, f2 ayp = f2{0ull})
 {
     f2 llv;
     llv.v = 0ull;
-    const f2 s = sample_pair_parts<NLL, NSRC>(h, c, r, llv, any);
+    const f2 s = sample_pair_parts<NLL, NSRC, MASS>(h, c, r, llv, any, axp, ayp);
     if (NLL) acc2 = fma2(bc2(h.ll.amp), llv, acc2);
     return s;
 }
@@ -280,7 +285,7 @@ __device__ __forceinline__ void trace_tiles(const RowC &rc, const HotC<NLL, NSRC
     // u-units: X = 2 (j S + b) + 1 - S We is the exact sub-sample abscissa (DESIGN.md a1)
     float X0 = (float)(2 * j * S + 1 - S * a.We);
     // even compile-time S, SIE polynomial path, components summed: pairs of sub-samples (tl_pair.cuh)
-    constexpr bool PAIR = S_T > 0 && S_T % 2 == 0 && MASS == MASS_SIE && FAST;
+    constexpr bool PAIR = S_T > 0 && S_T % 2 == 0 && FAST;     // SIE polynomial path / FP32 EPL series
     constexpr int NP = PAIR ? S_T / 2 : 1;
     ColV cv[(S_T > 0 && !PAIR) ? S_T : 1];
     ColV2 cv2[NP];
@@ -313,6 +318,19 @@ __device__ __forceinline__ void trace_tiles(const RowC &rc, const HotC<NLL, NSRC
                 for (int sa = 0; sa < S; ++sa) {
                     const float Y = Y0 + (float)(2 * sa);
                     const RowV rv = rowtab ? rowtab[i * S + sa] : row_values<NLL>(rc, Y);
+                    f2 dax[NP], day[NP];                            // EPL: the deflections of the sub-row's pairs, together
+                    if constexpr (PAIR && MASS == MASS_EPL) {
+                        f2 xp[NP], yp[NP];
+#pragma unroll
+                        for (int sp = 0; sp < NP; ++sp) {
+                            xp[sp] = add2(cv2[sp].Pc, bc2(rv.Qs));
+                            yp[sp] = fma2(cv2[sp].Ps, bc2(-1.f), bc2(rv.Qc));
+                        }
+                        epl_alpha_pairs<NP>(h.sie, rc.lens.ecoef, xp, yp, dax, day);
+                    } else {
+#pragma unroll
+                        for (int sp = 0; sp < NP; ++sp) { dax[sp].v = 0ull; day[sp].v = 0ull; }
+                    }
                     if constexpr (PAIR && LIN) {
                         f2 sk[NP][NSRC];
                         bool any = false;
@@ -320,7 +338,7 @@ __device__ __forceinline__ void trace_tiles(const RowC &rc, const HotC<NLL, NSRC
                         for (int sp = 0; sp < NP; ++sp) {
                             f2 llv;
                             llv.v = 0ull;
-                            sample_pair_comps<NLL, NSRC>(h, cv2[sp], rv, llv, sk[sp], any);
+                            sample_pair_comps<NLL, NSRC, MASS>(h, cv2[sp], rv, llv, sk[sp], any, dax[sp], day[sp]);
                             if (NLL) acc2 = fma2(bc2(h.ll.amp), llv, acc2);
                         }
                         if (any) {                                  // rare: FP64 ray-trace, out of line
@@ -348,7 +366,7 @@ __device__ __forceinline__ void trace_tiles(const RowC &rc, const HotC<NLL, NSRC
                         f2 src2[NP];
                         bool any = false;
 #pragma unroll
-                        for (int sp = 0; sp < NP; ++sp) src2[sp] = sample_pair<NLL, NSRC>(h, cv2[sp], rv, acc2, any);
+                        for (int sp = 0; sp < NP; ++sp) src2[sp] = sample_pair<NLL, NSRC, MASS>(h, cv2[sp], rv, acc2, any, dax[sp], day[sp]);
                         if (any) {                                  // rare: FP64 ray-trace, out of line
 #pragma unroll
                             for (int sp = 0; sp < NP; ++sp) {

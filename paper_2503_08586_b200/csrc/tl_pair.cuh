@@ -107,4 +107,69 @@ __device__ __forceinline__ f2 quad_form2(const QuadHot &C, f2 x, f2 y)      // t
     return fma2(x, w, fma2(mul2(bc2(C.cch), y), y, mul2(mul2(bc2(C.ccl), y), y)));
 }
 
+// step a2, EPL, for NP pairs of sub-samples at once (tl_sample.cuh epl_alpha_vec: same formulas, same
+// operations in the same order on each half, so the deflections are bit for bit the scalar ones; x - y is
+// fma(y, -1, x), exact like the subtraction).  The exponent / mantissa split and the clamp stay scalar.
+__device__ __forceinline__ f2 exp2_poly2(f2 x)                  // tl_sample.cuh exp2_poly
+{
+    const f2 big = add2(x, bc2(12582912.f));
+    const f2 r = fma2(add2(big, bc2(-12582912.f)), bc2(-1.f), x);
+    f2 p = bc2(1.545316336e-04f);
+    p = fma2(p, r, bc2(1.339086331e-03f));
+    p = fma2(p, r, bc2(9.618083015e-03f));
+    p = fma2(p, r, bc2(5.550356954e-02f));
+    p = fma2(p, r, bc2(2.402265072e-01f));
+    p = fma2(p, r, bc2(6.931471825e-01f));
+    p = fma2(p, r, bc2(1.0f));
+    float p0, p1, b0, b1;
+    un2(p, p0, p1); un2(big, b0, b1);
+    return mk2(__int_as_float(__float_as_int(p0) + (__float_as_int(b0) << 23)),
+               __int_as_float(__float_as_int(p1) + (__float_as_int(b1) << 23)));
+}
+
+template <int NP>
+__device__ __forceinline__ void epl_alpha_pairs(const EplHot &L, const float *coef, const f2 (&xp)[NP], const f2 (&yp)[NP],
+                                                f2 (&axp)[NP], f2 (&ayp)[NP])
+{
+    const f2 m1 = bc2(-1.f);
+    f2 c2[NP], s2[NP], pc[NP], ps[NP], tc[NP], b1[NP], b2[NP];
+#pragma unroll
+    for (int s = 0; s < NP; ++s) {
+        const f2 xx = mul2(xp[s], xp[s]);
+        const f2 psi2 = fma2(bc2(L.q2h), xx, fma2(bc2(L.q2l), xx, fma2(yp[s], yp[s], bc2(1e-30f))));   // R^2 (> 0, G6)
+        const f2 rinv = rsq_2(psi2);
+        const f2 cph = mul2(fma2(xp[s], bc2(L.qh), mul2(xp[s], bc2(L.ql))), rinv), sph = mul2(yp[s], rinv);   // e^{i phi}
+        c2[s] = mul2(fma2(sph, m1, cph), add2(cph, sph));
+        s2[s] = mul2(mul2(bc2(2.f), cph), sph);                                                         // w = e^{2 i phi}
+        float v0, v1;
+        un2(mul2(psi2, bc2(L.invb2)), v0, v1);
+        const int vb0 = __float_as_int(v0), vb1 = __float_as_int(v1);
+        const f2 ef = add2(mk2(__int_as_float((vb0 >> 23) | 0x4b000000), __int_as_float((vb1 >> 23) | 0x4b000000)), bc2(-8388735.f));
+        const f2 lm = mk2(mufu_lg2(__int_as_float((vb0 & 0x007fffff) | 0x3f800000)),
+                          mufu_lg2(__int_as_float((vb1 & 0x007fffff) | 0x3f800000)));                    // mantissas in [1, 2)
+        float a0, a1;
+        un2(fma2(ef, bc2(L.kh), fma2(lm, bc2(L.kh), mul2(add2(ef, lm), bc2(L.kl)))), a0, a1);
+        const f2 pw = exp2_poly2(mk2(fminf(fmaxf(a0, -100.f), 100.f), fminf(fmaxf(a1, -100.f), 100.f)));
+        const f2 P = fma2(pw, bc2(L.a0h), mul2(pw, bc2(L.a0l)));
+        pc[s] = mul2(P, cph); ps[s] = mul2(P, sph);
+        tc[s] = mul2(bc2(2.f), c2[s]); b1[s] = bc2(0.f); b2[s] = bc2(0.f);
+    }
+    // Clenshaw, two terms per trip (nterm is even)
+    for (int n = L.nterm; n >= 2; n -= 2) {
+        const float2 cf = *reinterpret_cast<const float2 *>(coef + n - 2);                  // a_{n-1}, a_n
+#pragma unroll
+        for (int s = 0; s < NP; ++s) {
+            b2[s] = fma2(b2[s], m1, fma2(tc[s], b1[s], bc2(cf.y)));                         // b_n
+            b1[s] = fma2(b1[s], m1, fma2(tc[s], b2[s], bc2(cf.x)));                         // b_{n-1}
+        }
+    }
+#pragma unroll
+    for (int s = 0; s < NP; ++s) {
+        const f2 b0 = fma2(b2[s], m1, fma2(tc[s], b1[s], bc2(1.f)));                        // a_0 = 1
+        const f2 sr = fma2(mul2(c2[s], m1), b1[s], b0), si = mul2(s2[s], b1[s]);
+        axp[s] = fma2(pc[s], sr, mul2(mul2(ps[s], m1), si));
+        ayp[s] = fma2(pc[s], si, mul2(ps[s], sr));
+    }
+}
+
 }  // namespace tl
