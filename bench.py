@@ -632,7 +632,8 @@ def run_mge(args, w: W.Workload, prob, ctx, rows):
     line = {"metric": METRIC + mass_tag(w) + " (MGE lens light, %d Gaussians + %d source amplitudes by NNLS per row)" % (len(sigmas), w.n_source),
             "value": value, "unit": UNIT, "n_gpus": 1,
             "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps,
-            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32" if args.precision == "fp32" else "f64", "precision": args.precision, "data": "synthetic",
             "config": config_dict(w, "flushed between steps (256 MiB fill)"), "clocks": clk.summary(),
             "pixel_evals_per_s": value * w.ny * w.nx, "mode": "mge", "mge_sigmas_arcsec": [float(x) for x in sigmas],
             "chunk_rows": int(chunk), "gpu_launches": int(args.steps * 6 * n_chunks), "checksum_logL": float(out.double().sum())}
@@ -648,7 +649,15 @@ def run_mge(args, w: W.Workload, prob, ctx, rows):
     line["roofline"] = {"bound": "alu", "kernel": "gauss_conv_kernel", "achieved": ach, "peak": peak, "unit": "Tinst/s",
                         "frac": ach / peak, "traffic": None, "kernel_ms": k_ms, "kernel_rows": int(last_rows),
                         "algorithmic_issue_slots_per_likelihood": slots,
-                        "peak_source": "as in the default mode (FP32 FMA issue slots)"}
+                        "peak_source": "as in the default mode (FP32 FMA issue slots)",
+                        "note": "the slots are those of evaluating and blurring every Gaussian over the whole image; the kernel "
+                                "leaves out the part of a narrow Gaussian that is exactly 0 (DESIGN.md 13), so the fraction of "
+                                "what it executes is lower (profiles/r2_modes.md: issue port, FMA pipe)"}
+    if args.precision != "fp32":
+        # FP64 pipeline (trace_dp / gauss_dp / conv_dp / gram / nnls): the fraction over the whole step, same issue roofline
+        ach = slots * B / (total_ms / args.steps * 1e-3) / 1e12
+        line["roofline"] = {"bound": "alu", "kernel": "whole step (FP64 MGE pipeline)", "achieved": ach, "peak": peak,
+                            "unit": "Tinst/s", "frac": ach / peak, "traffic": None, "kernel_ms": total_ms / args.steps}
     if not args.no_cpu_baseline:
         from oracle import oracle as O
         O.lib()
