@@ -965,8 +965,8 @@ int tl_set_mge_sets(tl_ctx *c, const float *sigmas, const int32_t *n_per_set, in
         c->mge_gc_smem = sizeof(float) * ((size_t)c->K * c->Kp + (size_t)(c->He + 1) * c->pitch + c->Kp + 8);
         c->mge_fused = c->mge_gc_smem <= SMEM_LIMIT - 1024;
         if (c->mge_fused)
-            okm = okm && cuda_ok(cudaFuncSetAttribute(tl::gauss_conv_for(S), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SMEM_LIMIT - 1024))) &&
-                  cuda_ok(cudaFuncSetAttribute(tl::gauss_conv_for(S), cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+            okm = okm && cuda_ok(cudaFuncSetAttribute(tl::gauss_conv_for(S, c->K), cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SMEM_LIMIT - 1024))) &&
+                  cuda_ok(cudaFuncSetAttribute(tl::gauss_conv_for(S, c->K), cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
         okm = okm && cuda_ok(cudaFuncSetAttribute(tl::nnls_mge_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                                   (int)(sizeof(double) * tl::MGE_NNLS_WARPS * (2 * tl::MGE_MAX_COL * tl::MGE_MAX_COL + 3 * tl::MGE_MAX_COL))));
         if (!okm) { c->mge_trace = nullptr; c->n_gauss = 0; cudaGetLastError(); return TL_ECUDA; }
@@ -1146,7 +1146,7 @@ int tl_loglike_mge_batch(tl_ctx *c, const float *params, int64_t B, float *logL,
         if (fused) {
             // 2. every Gaussian evaluated into shared memory and blurred from there -> M[0 .. NG)
             if (c->profile) cudaEventRecord(c->ev0, st);
-            tl::gauss_conv_for(c->cfg.supersample)<<<dim3((unsigned)nb, (unsigned)NG), 256, c->mge_gc_smem, st>>>(a, (int)nb);
+            tl::gauss_conv_for(c->cfg.supersample, c->K)<<<dim3((unsigned)nb, (unsigned)NG), 256, c->mge_gc_smem, st>>>(a, (int)nb);
             if (c->profile) { cudaEventRecord(c->ev1, st); c->prof_pending = 1; }
             // 3. the sources blurred -> M[NG ..)
             tl::KArgs ac = a;

@@ -136,8 +136,11 @@ __device__ __forceinline__ void conv_blocks_rect(const KArgs &a, const float *im
 // the outputs whose window meets the box are convolved; the rest of the column is written as 0 --
 // the same bits as evaluating everything (a 0.6-pixel Gaussian covers 1/30 of a 120 x 120 image).
 // S_T = 0: any S (scalar loop).
-template <int S_T>
-__global__ void __launch_bounds__(256) gauss_conv_kernel(const KArgs a, int chunk_rows)
+// K_T: the PSF size when it has a register-blocked convolution (a kernel of its own per size, so that the
+// small sizes are not held to the registers of the 41 x 41 blocks: up to 21 x 21 three CTAs share an SM),
+// 0 = any other size.
+template <int S_T, int K_T>
+__global__ void __launch_bounds__(256, (K_T > 0 && K_T <= 21) ? 3 : 2) gauss_conv_kernel(const KArgs a, int chunk_rows)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float *taps = reinterpret_cast<float *>(smem_raw);
@@ -240,28 +243,37 @@ __global__ void __launch_bounds__(256) gauss_conv_kernel(const KArgs a, int chun
     const int oi0 = max(0, i_lo - a.K + 1), oi1 = min(a.ny - 1, i_hi), ox0 = max(0, j_lo - a.K + 1), ox1 = min(a.nx - 1, j_hi);
     const bool none = bw <= 0 || bh <= 0 || oi0 > oi1 || ox0 > ox1;
     const int ip0 = none ? 1 : oi0 / 2, ip1 = none ? 0 : oi1 / 2, xb0 = none ? 1 : ox0 / 4, xb1 = none ? 0 : ox1 / 4;
-#define TL_CONV_CASE(KK) \
-    case KK: conv_blocks_rect<KK>(a, img, taps, ip0, ip1, xb0, xb1, out); return;
-    switch (a.K) {
-        TL_CONV_CASE(5)
-        TL_CONV_CASE(15)
-        TL_CONV_CASE(21)
-        TL_CONV_CASE(31)
-        TL_CONV_CASE(41)
-    default: break;
+    if constexpr (K_T > 0) { conv_blocks_rect<K_T>(a, img, taps, ip0, ip1, xb0, xb1, out); return; }
+    // other PSF sizes: the generic 1 x 4 strips over the whole image
+    const int nsx = (a.nx + CONV_R - 1) / CONV_R;
+    for (int s = threadIdx.x; s < a.ny * nsx; s += blockDim.x) {
+        const int i = s / nsx, x0 = (s - i * nsx) * CONV_R;
+        float acc[CONV_R];
+        conv_strip(img + i * a.pitch + x0, a.pitch, taps, a.K, a.Kp, acc);
+        chi2_strip(a, acc, i, x0, nullptr, nullptr, out);
     }
-#undef TL_CONV_CASE
-    conv_chi2_rows(a, img, 0, taps, 0, a.ny, nullptr, nullptr, out);       // other PSF sizes: the generic strips, whole image
 }
 
 typedef void (*gauss_conv_fn)(const KArgs, int);
-inline gauss_conv_fn gauss_conv_for(int S)
+template <int S_T>
+inline gauss_conv_fn gauss_conv_for_k(int K)
+{
+    switch (K) {
+    case 5: return gauss_conv_kernel<S_T, 5>;
+    case 15: return gauss_conv_kernel<S_T, 15>;
+    case 21: return gauss_conv_kernel<S_T, 21>;
+    case 31: return gauss_conv_kernel<S_T, 31>;
+    case 41: return gauss_conv_kernel<S_T, 41>;
+    default: return gauss_conv_kernel<S_T, 0>;
+    }
+}
+inline gauss_conv_fn gauss_conv_for(int S, int K)
 {
     switch (S) {
-    case 2: return gauss_conv_kernel<2>;
-    case 4: return gauss_conv_kernel<4>;
-    case 8: return gauss_conv_kernel<8>;
-    default: return gauss_conv_kernel<0>;
+    case 2: return gauss_conv_for_k<2>(K);
+    case 4: return gauss_conv_for_k<4>(K);
+    case 8: return gauss_conv_for_k<8>(K);
+    default: return gauss_conv_for_k<0>(K);
     }
 }
 
