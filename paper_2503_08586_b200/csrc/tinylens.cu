@@ -675,6 +675,11 @@ int tl_create_ex(tl_ctx **out, const tl_config *cfg, const float *psf_in, int32_
         if (c->opt.block_threads) c->threads = c->opt.block_threads;
         c->fused = cfg->mass_model == TL_MASS_EPL ? tl_fused_epl_for(cfg->supersample, cfg->n_lens_light, cfg->n_source)
                                                   : tl_fused_for(cfg->supersample, cfg->n_lens_light, cfg->n_source);
+        // small rows (256-thread CTAs), S = 2, PSF up to 21 x 21: the variant that fits three CTAs per SM
+        if (c->threads == 256 && c->K <= 21 && cfg->mass_model != TL_MASS_EPL && 3 * (fs + 1024) <= SMEM_LIMIT) {
+            fused_fn small = tl_fused_small_for(cfg->supersample, cfg->n_lens_light, cfg->n_source);
+            if (small) c->fused = small;
+        }
         if (!cuda_ok(cudaFuncSetAttribute(c->fused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_LIMIT))) { tl_destroy(c); return TL_ECUDA; }
         int occ = 0;
         if (!cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, c->fused, c->threads, fs)) || occ < 1) { tl_destroy(c); return TL_ECUDA; }

@@ -8,6 +8,7 @@ typedef void (*fused_fn)(const tl::KArgs);
 typedef void (*trace_fn)(const tl::KArgs, int);
 
 fused_fn tl_fused_for(int S, int n_lens_light, int n_source);          // fused_kernel<S, NLL, NSRC>
+fused_fn tl_fused_small_for(int S, int n_lens_light, int n_source);    // fused_kernel<S, NLL, NSRC, SIE, 1> (256 threads, K <= 21), or null
 trace_fn tl_trace_for(int S, int n_lens_light, int n_source);          // trace_kernel<S, NLL, NSRC>
 trace_fn tl_trace_pairs_for(int S, int n_lens_light, int n_source);    // trace_pairs_kernel<S, NLL, NSRC>, or null (odd S)
 fused_fn tl_fused_lin_for(int S, int n_lens_light, int n_source);      // fused_lin_kernel<...>

@@ -17,3 +17,12 @@ fused_fn tl_fused_for(int S, int nll, int nsrc)
     default: return pick_fused<0>(nll, nsrc);
     }
 }
+
+// the three-CTAs-per-SM variant (256 threads, PSF up to 21 x 21): S = 2 only, where the pair loop holds one
+// pair per sub-row and fits in 85 registers
+fused_fn tl_fused_small_for(int S, int nll, int nsrc)
+{
+    if (S != 2) return nullptr;
+    if (nll == 0) return nsrc == 1 ? tl::fused_kernel<2, 0, 1, tl::MASS_SIE, 1> : tl::fused_kernel<2, 0, 2, tl::MASS_SIE, 1>;
+    return nsrc == 1 ? tl::fused_kernel<2, 1, 1, tl::MASS_SIE, 1> : tl::fused_kernel<2, 1, 2, tl::MASS_SIE, 1>;
+}

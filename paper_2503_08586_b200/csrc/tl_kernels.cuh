@@ -735,19 +735,31 @@ __device__ __forceinline__ double conv_chi2_blocks(const KArgs &a, const float *
 // whose row 0 corresponds to extended row `e0` (one spare row after the last one must be
 // readable).  Returns this thread's chi^2 partial.  The common PSF sizes get the register-
 // blocked 2 x 4 kernel, any other odd size the generic 1 x 4 strip.
+// KSMALL: only the blocks up to 21 x 21 are compiled in (a kernel that holds the 41 x 41 blocks is held to
+// their ~120 registers whatever PSF it is run with).
+template <bool KSMALL = false>
 __device__ __forceinline__ double conv_chi2_rows(const KArgs &a, const float *img, int e0,
                                                  const float *taps, int i0, int i1,
                                                  const float *data, const float *wgt, float *image_out, ErrAcc *err = nullptr)
 {
 #define TL_CONV_CASE(KK) \
     case KK: return conv_chi2_blocks<KK>(a, img, e0, taps, i0, i1, data, wgt, image_out, err);
-    switch (a.K) {
-        TL_CONV_CASE(5)
-        TL_CONV_CASE(15)
-        TL_CONV_CASE(21)
-        TL_CONV_CASE(31)
-        TL_CONV_CASE(41)
-    default: break;
+    if constexpr (KSMALL) {
+        switch (a.K) {
+            TL_CONV_CASE(5)
+            TL_CONV_CASE(15)
+            TL_CONV_CASE(21)
+        default: break;
+        }
+    } else {
+        switch (a.K) {
+            TL_CONV_CASE(5)
+            TL_CONV_CASE(15)
+            TL_CONV_CASE(21)
+            TL_CONV_CASE(31)
+            TL_CONV_CASE(41)
+        default: break;
+        }
     }
 #undef TL_CONV_CASE
     const int nsx = (a.nx + CONV_R - 1) / CONV_R;
@@ -767,8 +779,9 @@ __device__ __forceinline__ double conv_chi2_rows(const KArgs &a, const float *im
 #define TL_LB_T 512
 #define TL_LB_B 1
 #endif
-template <int S_T, int NLL, int NSRC, int MASS = MASS_SIE>
-__global__ void __launch_bounds__(TL_LB_T, TL_LB_B) fused_kernel(const KArgs a)
+// VAR = 1: the variant for small rows (256 threads, PSF up to 21 x 21): three CTAs per SM.
+template <int S_T, int NLL, int NSRC, int MASS = MASS_SIE, int VAR = 0>
+__global__ void __launch_bounds__(VAR ? 256 : TL_LB_T, VAR ? 3 : TL_LB_B) fused_kernel(const KArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     RowC *rc = reinterpret_cast<RowC *>(smem_raw);
@@ -806,7 +819,7 @@ __global__ void __launch_bounds__(TL_LB_T, TL_LB_B) fused_kernel(const KArgs a)
         // phase 2: PSF convolution from shared memory + chi^2
         ErrAcc err = {0.f, 0.f};
         const bool want_err = a.flag_count != nullptr && a.logL != nullptr;      // AUTO precision (uniform)
-        const double part = conv_chi2_rows(a, img, 0, taps, 0, a.ny,
+        const double part = conv_chi2_rows<VAR != 0>(a, img, 0, taps, 0, a.ny,
                                            a.logL ? a.data + lens * npix : nullptr,
                                            a.wgt + lens * npix,
                                            a.images ? a.images + row * npix : nullptr, want_err ? &err : nullptr);
