@@ -398,7 +398,8 @@ int run_batch(tl_ctx *c, const float *params, int64_t B, float *logL, float *ima
     tl::RowC *rows = nullptr;
     float *ext = nullptr;
     double *partial = nullptr;
-    if (!pool_alloc(c, &rows, sizeof(tl::RowC) * (size_t)chunk, st)) return TL_ENOMEM;
+    // (split path: + one tile-queue head per row for the ray-trace kernel)
+    if (!pool_alloc(c, &rows, (sizeof(tl::RowC) + (c->path == 1 ? sizeof(int) : 0)) * (size_t)chunk, st)) return TL_ENOMEM;
     if (c->path == 1) {
         const size_t ext_bytes = sizeof(float) * (size_t)chunk * c->He * c->pitch;
         if (!pool_alloc(c, &ext, ext_bytes, st) ||
@@ -434,6 +435,12 @@ int run_batch(tl_ctx *c, const float *params, int64_t B, float *logL, float *ima
             if (c->profile) { cudaEventRecord(c->ev1, st); c->prof_pending = 1; }
         } else {
             a.ext = ext; a.partial = logL ? partial : nullptr;
+            // the row's CTAs draw warp tiles from one queue: the tiles next to a source centre, full of FP64-refined
+            // samples, cost several times an ordinary one, and a static split leaves their CTA's other warps idle
+            if (nb <= 65535) {
+                a.tile_counters = reinterpret_cast<int *>(rows + chunk);
+                cudaMemsetAsync(a.tile_counters, 0, sizeof(int) * (size_t)nb, st);
+            }
             dim3 tg((unsigned)(nb < 65535 ? nb : 65535), (unsigned)c->trace_slabs);
             if (c->profile) cudaEventRecord(c->ev0, st);
             c->trace<<<tg, 256, c->trace_smem, st>>>(a, (int)nb);
