@@ -896,7 +896,7 @@ int tl_loglike_linear_batch(tl_ctx *c, const float *params, int64_t B, float *lo
     if (chunk > B) chunk = B;
     tl::RowC *rows = nullptr;
     float *ext = nullptr, *mimg = nullptr;
-    if (!pool_alloc(c, &rows, sizeof(tl::RowC) * (size_t)chunk, st)) return TL_ENOMEM;
+    if (!pool_alloc(c, &rows, (sizeof(tl::RowC) + sizeof(int)) * (size_t)chunk, st)) return TL_ENOMEM;   // + a tile-queue head per row
     if (!pool_alloc(c, &ext, ext_row * (size_t)chunk, st) ||
         !pool_alloc(c, &mimg, m_row * (size_t)chunk, st)) {
         cudaFreeAsync(rows, st);
@@ -915,6 +915,8 @@ int tl_loglike_linear_batch(tl_ctx *c, const float *params, int64_t B, float *lo
         a.rows = rows; a.B = nb; a.rows_per_lens = rows_per_lens; a.row0 = r0;
         a.logL = logL; a.amps = amps; a.ext = ext; a.mimg = mimg;
         a.tile_rows = c->lin_tile_rows; a.n_tiles = c->lin_n_tiles; a.rowtab = c->lin_rowtab;
+        a.tile_counters = reinterpret_cast<int *>(rows + chunk);          // the row's CTAs draw warp tiles from one queue (see run_batch)
+        cudaMemsetAsync(a.tile_counters, 0, sizeof(int) * (size_t)nb, st);
         dim3 tg((unsigned)nb, 8);
         if (c->profile) cudaEventRecord(c->ev0, st);
         c->trace_lin<<<tg, 256, c->lin_trace_smem, st>>>(a, (int)nb);
