@@ -179,6 +179,7 @@ def _small_problem(orc, **kw):
     dict(ny=5, nx=4, psf_size=9, supersample=2),    # PSF larger than the image
     dict(ny=40, nx=40, supersample=5, psf_size=3, n_source=1),
     dict(ny=16, nx=130, supersample=2, psf_size=11, edge_mode=W.EDGE_ZERO, n_lens_light=0),
+    dict(ny=40, nx=44, supersample=2, psf_size=21),  # S = 2, K <= 21: the three-CTAs-per-SM variant of the fused kernel, two sources
 ])
 def test_shapes_and_edge_modes(api, torch, orc, kw):
     w, prob = _small_problem(orc, **kw)

@@ -35,6 +35,10 @@ CASES = [
     W.Workload(index=7, name="odd", ny=37, nx=45, pix_scale=0.11, supersample=3, psf_size=15, psf_kind="moffat",
                psf_fwhm=0.3, psf_beta=2.5, n_lens_light=1, n_source=2, noise_bg=0.05, noise_exptime=150.0,
                source_amp=(1.0, 20.0), batch=16),
+    # S = 2 with two sources and a 21 x 21 PSF: the three-CTAs-per-SM variant of the fused kernel (no 31 / 41 blocks)
+    W.Workload(index=7, name="s2-two-sources", ny=48, nx=56, pix_scale=0.09, supersample=2, psf_size=21, psf_kind="gaussian",
+               psf_fwhm=0.25, psf_beta=0.0, n_lens_light=1, n_source=2, noise_bg=0.05, noise_exptime=300.0,
+               source_amp=(1.0, 20.0), batch=16),
     W.Workload(index=7, name="zero-edge", ny=20, nx=18, pix_scale=0.2, supersample=2, psf_size=5, psf_kind="gaussian",
                psf_fwhm=0.4, psf_beta=0.0, n_lens_light=0, n_source=1, noise_bg=0.05, noise_exptime=0.0,
                source_amp=(5.0, 5.0), batch=16, edge_mode=W.EDGE_ZERO),
