@@ -270,10 +270,10 @@ int tl_loglike_linear_batch(tl_ctx *ctx, const float *params, int64_t B, float *
  * TL_ENOMEM or TL_ECUDA.
  *
  * tl_mge_columns -- n_gauss + n_source (the width of `amps`), or < 0 when no set is defined.
- * tl_mge_chunk_rows -- a call with more rows is processed in chunks of this many (seven launches
- *   each, same stream; the component images of a chunk are staged in <= 8 GB of scratch from
- *   the stream-ordered allocator; a call halves its chunk when the device cannot give that much);
- *   < 0 when no set is defined.
+ * tl_mge_chunk_rows -- a call with more rows is processed in chunks of this many (six launches
+ *   each, same stream; the blurred component images of a chunk are staged in <= 2 GiB of scratch
+ *   from the context's stream-ordered pool; a call halves its chunk when the device cannot give
+ *   that much); < 0 when no set is defined.
  *
  * tl_loglike_mge_batch -- logL[r] = Eq. 5 at the NNLS-optimal amplitudes of row r.
  *   params   DEVICE pointer, float [B][P], the context's usual row layout; of the lens-light

@@ -16,7 +16,8 @@
 //                              unblurred Gaussians never touch global memory.  (Images too large
 //                              for that: mge_gauss_kernel -> ext, then conv_lin_kernel.)
 //   conv_lin_kernel            the source images blurred with the PSF
-//   gram_mge_kernel            G = M'WM, b = M'Wd, d'Wd in FP64 (fixed summation order) -> global
+//   gram_reg_kernel / gram_mge_kernel   G = M'WM, b = M'Wd, d'Wd in FP64 (fixed summation order) -> global
+//                              (up to 11 columns: every entry in registers; more: staged through shared memory)
 //   nnls_mge_kernel            NNLS by the Gram-matrix active-set iteration of Bro & De Jong (the
 //                              paper's solver), one warp per row -> amplitudes,
 //                              and chi^2 = d'Wd - 2 s'b + s'Gs -> logL.  All of it FP64 on exact
@@ -496,10 +497,9 @@ inline gram_reg_fn gram_reg_for(int n1)
     }
 }
 
-// NNLS: one warp per row (lane 0 iterates; the iteration is a chain of dependent FP64 operations
-// through shared memory, so what matters is how many rows are in flight per SM: 4 warps per CTA,
-// ~6 KB of shared memory each).  Writes the amplitudes (FP64, for resid_mge_kernel; float for the
-// caller) and reports invalid rows.
+// NNLS: one warp per row, the iteration run by the whole warp (nnls_gram_warp, tl_nnls.cuh); four warps per
+// CTA, a compact copy of G in dynamic shared memory (2 n^2 + 3 n doubles per row).  Writes the amplitudes and
+// logL from the Gram quantities, and reports invalid rows.
 __global__ void __launch_bounds__(32 * MGE_NNLS_WARPS) nnls_mge_kernel(const KArgs a, int chunk_rows)
 {
     // per warp (dynamic shared memory, sized by the actual column count n): G [n][n] | b [n] | L [n][n] | z [n] | s [n]
