@@ -203,6 +203,37 @@ int tl_loglike_batch(tl_ctx *ctx, const float *params, int64_t B, float *logL, v
 int tl_render_batch(tl_ctx *ctx, const float *params, int64_t B, float *images, void *cuda_stream);
 
 /*
+ * Serve mode -- a persistent kernel for a sampler that proposes a handful of rows at a time (SURVEY.md 8(f)
+ * NEXT-4; the CPU<->GPU round trips, not the likelihood, limit the pipeline).
+ * tl_serve_start launches ONE kernel that occupies every SM of the device and polls a request block in pinned,
+ * mapped host memory; tl_serve_eval writes the rows and a sequence number into that block and spins until the
+ * kernel has written logL back: no cudaMemcpy, no kernel launch and no stream synchronisation per request.
+ * The arithmetic is that of tl_loglike_batch (the same device functions in the same order): logL is bit for bit
+ * what tl_loglike_batch returns for the same rows.
+ *   tl_serve_start(ctx, max_rows, idle_timeout_s)
+ *       max_rows        1 .. 16: the most rows one request may hold
+ *       idle_timeout_s  (0, 300]: the kernel leaves by itself after this long without a request (and after 120 s
+ *                       in any case); the next tl_serve_eval starts it again (one launch).  Every wait inside the
+ *                       kernel is bounded in the same way, so a host that goes away cannot leave a spinning GPU.
+ *       Contexts: FP32 precision, n_lens = 1, SIE mass model, even supersampling factor, fused path with a
+ *       register-blocked PSF size (5, 15, 21, 31, 41); otherwise TL_EINVAL / TL_ESIZE.  Allocates the request
+ *       block, per-row scratch for 16 rows and a stream of its own.  TL_EINVAL when already serving.
+ *   tl_serve_eval(ctx, params_host, B, logL_host)
+ *       params_host  HOST pointer, float [B][P] (need not be pinned: it is copied into the request block)
+ *       B            1 .. max_rows
+ *       logL_host    HOST pointer, float [B], written (-INFINITY for invalid rows)
+ *       Blocking, one request at a time per context (not thread-safe).  TL_ECUDA when the kernel does not answer
+ *       within 20 s.
+ *   tl_serve_stop(ctx)  tells the kernel to leave, waits for it and frees what tl_serve_start allocated; also done
+ *       by tl_destroy.  TL_OK when the context is not serving.
+ * WHILE SERVING THE GPU IS TAKEN: kernels launched by anybody else on the device (tl_loglike_batch of this or another
+ * context included) only start once the serving kernel has left, i.e. after tl_serve_stop or the idle timeout.
+ */
+int tl_serve_start(tl_ctx *ctx, int32_t max_rows, double idle_timeout_s);
+int tl_serve_eval(tl_ctx *ctx, const float *params_host, int32_t B, float *logL_host);
+int tl_serve_stop(tl_ctx *ctx);
+
+/*
  * tl_loglike_batch_noalloc -- tl_loglike_batch (Eq. 5; same steps a0-a7, same kernels,
  * same bits) for callers that may not allocate: code under CUDA graph capture, serving loops,
  * harnesses that forbid cudaMalloc.  tl_loglike_batch takes its per-call scratch -- the array of

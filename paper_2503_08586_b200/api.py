@@ -83,6 +83,9 @@ def load(build_if_missing: bool = True):
     L.tl_get_info.restype = C.c_int; L.tl_get_info.argtypes = [vp, C.POINTER(tl_info)]
     L.tl_loglike_batch.restype = C.c_int; L.tl_loglike_batch.argtypes = [vp, vp, i64, vp, vp]
     L.tl_render_batch.restype = C.c_int; L.tl_render_batch.argtypes = [vp, vp, i64, vp, vp]
+    L.tl_serve_start.restype = C.c_int; L.tl_serve_start.argtypes = [vp, i32, C.c_double]
+    L.tl_serve_eval.restype = C.c_int; L.tl_serve_eval.argtypes = [vp, vp, i32, vp]
+    L.tl_serve_stop.restype = C.c_int; L.tl_serve_stop.argtypes = [vp]
     L.tl_loglike_batch_noalloc.restype = C.c_int; L.tl_loglike_batch_noalloc.argtypes = [vp, vp, i64, vp, vp]
     L.tl_loglike_batch_host.restype = C.c_int; L.tl_loglike_batch_host.argtypes = [vp, vp, i64, vp, vp]
     L.tl_loglike_batch_host_async.restype = C.c_int; L.tl_loglike_batch_host_async.argtypes = [vp, vp, i64, vp, vp]
@@ -217,6 +220,28 @@ def tl_loglike_batch(handle: int, params, out=None, stream=None):
 
 
 TL_NOALLOC_MAX_ROWS = 4096
+
+
+def tl_serve_start(handle: int, max_rows: int = 16, idle_timeout_s: float = 2.0):
+    """Launch the persistent serving kernel (include/tinylens.h): the GPU is taken until tl_serve_stop / the timeout."""
+    _check(load().tl_serve_start(handle, int(max_rows), float(idle_timeout_s)), "tl_serve_start")
+
+
+def tl_serve_eval(handle: int, params_host, out_host=None):
+    """params_host: numpy float32 [B,P] (B <= max_rows) -> logL numpy float32 [B], through the serving kernel."""
+    p = np.ascontiguousarray(params_host, dtype=np.float32)
+    if p.ndim != 2:
+        raise TinyLensError(TL_EINVAL, "params_host must be [B, P]")
+    if out_host is None:
+        out_host = np.empty(p.shape[0], np.float32)
+    if out_host.dtype != np.float32 or out_host.shape != (p.shape[0],) or not out_host.flags["C_CONTIGUOUS"]:
+        raise TinyLensError(TL_EINVAL, "out_host must be a contiguous float32 array of shape (B,)")
+    _check(load().tl_serve_eval(handle, p.ctypes.data, p.shape[0], out_host.ctypes.data), "tl_serve_eval")
+    return out_host
+
+
+def tl_serve_stop(handle: int):
+    _check(load().tl_serve_stop(handle), "tl_serve_stop")
 
 
 def tl_loglike_batch_noalloc(handle: int, params, out, stream=None):
@@ -409,6 +434,15 @@ class LensContext:
 
     def loglike(self, params, out=None, stream=None):
         return tl_loglike_batch(self.handle, params, out, stream)
+
+    def serve_start(self, max_rows=16, idle_timeout_s=2.0):
+        tl_serve_start(self.handle, max_rows, idle_timeout_s)
+
+    def serve_eval(self, params_host, out_host=None):
+        return tl_serve_eval(self.handle, params_host, out_host)
+
+    def serve_stop(self):
+        tl_serve_stop(self.handle)
 
     def loglike_noalloc(self, params, out, stream=None):
         return tl_loglike_batch_noalloc(self.handle, params, out, stream)

@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtinylens.so")
 SOURCES = [os.path.join(CSRC, f) for f in ("tinylens.cu", "tl_inst_fused.cu", "tl_inst_split.cu", "tl_inst_lin.cu",
-                                           "tl_inst_epl.cu", "tl_inst_epl_lin.cu", "tl_peaks.cu")]
+                                           "tl_inst_epl.cu", "tl_inst_epl_lin.cu", "tl_inst_serve.cu", "tl_peaks.cu")]
 HEADERS = sorted(os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cuh", ".h"))) + \
           [os.path.join(os.path.dirname(HERE), "include", "tinylens.h")]
 

@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <ctime>
 #include <mutex>
 #include <new>
 #include <vector>
@@ -19,6 +20,7 @@
 #include "tl_precise.cuh"
 #include "tl_dp.cuh"
 #include "tl_mge.cuh"
+#include "tl_serve.cuh"
 
 #define TL_VERSION_STRING "tinylens-b200 0.2 (sm_100a)"
 
@@ -101,6 +103,19 @@ struct tl_ctx {
     } slots[2];
     int next_slot = 0;
     cudaStream_t s_up = nullptr, s_down = nullptr;
+    // serve mode (tl_serve_start: the persistent kernel of tl_serve.cuh)
+    struct Serve {
+        serve_fn fn = nullptr;
+        tl::ServeCtl *ctl = nullptr, *ctl_dev = nullptr;     // pinned + mapped request block: host / device address
+        tl::ServeDev *dev = nullptr;
+        tl::RowC *rows = nullptr;
+        float *ext = nullptr, *cblk = nullptr, *params = nullptr;
+        int *counters = nullptr;
+        cudaStream_t stream = nullptr;
+        int grid = 0, max_rows = 0;
+        size_t smem = 0;
+        unsigned long long seq = 0, idle_ns = 0;
+    } sv;
     tl_options opt;               // create-time options (tl_create_ex); defaults = automatic
     cudaMemPool_t pool = nullptr; // library-owned stream-ordered pool: per-call scratch (never the device's default pool)
     // benchmark facility (tl_set_profiling): events around the dominant kernel of the last call
@@ -462,6 +477,158 @@ int run_batch(tl_ctx *c, const float *params, int64_t B, float *logL, float *ima
 }
 
 }  // namespace
+
+// ------------------------------------------------------------------ serve mode (tl_serve.cuh)
+namespace {
+
+// launch geometry of a B-row request on `grid` resident CTAs: run_small_batch's, with the CTAs of the persistent grid
+void serve_geometry(const tl_ctx *c, int B, int grid, int *per_row, int *bands_out, int *band_pairs_out, int *xseg_out, size_t *conv_smem)
+{
+    const int npair = (c->cfg.ny + 1) / 2, nsx = (c->cfg.nx + 3) / 4;
+    int want = grid / B;
+    if (want < 1) want = 1;
+    const int S = c->cfg.supersample, ppw = 32 / (S * S / 2), wpc = c->threads / 32;
+    const int n_wt = (c->He * c->We + ppw - 1) / ppw;
+    *per_row = want < (n_wt + wpc - 1) / wpc ? want : (n_wt + wpc - 1) / wpc;
+    int bands = want < npair ? want : npair;
+    const size_t fixed = sizeof(float) * ((size_t)c->K * c->Kp + c->pitch + c->Kp + 8);
+    int band_pairs = (npair + bands - 1) / bands;
+    const int max_pairs = (int)(((SMEM_LIMIT - 4096 - fixed) / (sizeof(float) * c->pitch) - (c->K - 1)) / 2);
+    if (band_pairs > max_pairs) band_pairs = max_pairs;
+    bands = (npair + band_pairs - 1) / band_pairs;
+    const int per_pass = c->threads / c->K;
+    int xseg = want / bands;
+    const int one_pass = (band_pairs * nsx + per_pass - 1) / per_pass;
+    if (xseg > one_pass) xseg = one_pass;
+    if (xseg > nsx) xseg = nsx;
+    if (xseg < 1) xseg = 1;
+    if ((band_pairs * ((nsx + xseg - 1) / xseg) + per_pass - 1) / per_pass > 2) xseg = 0;
+    *bands_out = bands; *band_pairs_out = band_pairs; *xseg_out = xseg;
+    *conv_smem = fixed + sizeof(float) * ((size_t)(2 * band_pairs + c->K - 1) * c->pitch + (xseg ? (size_t)per_pass * c->K * 8 : 0));
+}
+
+void serve_free(tl_ctx *c)
+{
+    tl_ctx::Serve &v = c->sv;
+    if (v.stream) cudaStreamDestroy(v.stream);
+    if (v.ctl) cudaFreeHost(v.ctl);
+    cudaFree(v.dev); cudaFree(v.rows); cudaFree(v.ext); cudaFree(v.cblk); cudaFree(v.params); cudaFree(v.counters);
+    v = tl_ctx::Serve();
+}
+
+// (re)start the persistent kernel; it takes up where the last one left (requests up to ctl->done are served)
+bool serve_launch(tl_ctx *c)
+{
+    tl_ctx::Serve &v = c->sv;
+    if (!cuda_ok(cudaStreamSynchronize(v.stream))) return false;               // the previous kernel, if any, has left
+    tl::ServeDev d0;
+    memset(&d0, 0, sizeof(d0));
+    d0.seq = v.ctl->done; d0.start = v.ctl->done;
+    if (!cuda_ok(cudaMemcpyAsync(v.dev, &d0, sizeof(d0), cudaMemcpyHostToDevice, v.stream))) return false;
+    if (!cuda_ok(cudaStreamSynchronize(v.stream))) return false;               // (d0 is on the stack)
+    tl::KArgs a = base_args(c);
+    a.rows = v.rows; a.B = tl::SERVE_MAX_ROWS; a.rows_per_lens = (int64_t)1 << 40; a.row0 = 0;
+    a.logL = v.ctl_dev->logL; a.ext = v.ext; a.rowtab = 0; a.tile_counters = v.counters;
+    tl::PrologueArgs pa;
+    fill_prologue_args(c, pa, v.params, v.rows, tl::SERVE_MAX_ROWS, 0, (int64_t)1 << 40, 0);
+    v.ctl->alive = 1; v.ctl->error = 0;
+    v.fn<<<v.grid, c->threads, v.smem, v.stream>>>(a, pa, v.ctl_dev, v.dev, v.cblk, v.idle_ns, (unsigned long long)120e9);   // (lifetime: 120 s, then restarted on demand)
+    return cuda_ok(cudaGetLastError());
+}
+
+}  // namespace
+
+extern "C" {
+
+int tl_serve_start(tl_ctx *c, int32_t max_rows, double idle_timeout_s)
+{
+    if (!c || max_rows < 1 || max_rows > tl::SERVE_MAX_ROWS || !(idle_timeout_s > 0.0) || idle_timeout_s > 300.0) return TL_EINVAL;
+    if (c->sv.fn) return TL_EINVAL;                                             // already serving
+    if (c->cfg.n_lens != 1 || c->cfg.n_lens_light > 1 || c->cfg.mass_model != TL_MASS_SIE || c->precision != TL_PRECISION_FP32) return TL_EINVAL;
+    const bool kblk = c->K == 5 || c->K == 15 || c->K == 21 || c->K == 31 || c->K == 41;
+    serve_fn fn = tl_serve_for(c->cfg.supersample, c->cfg.n_lens_light, c->cfg.n_source);
+    if (c->path != 0 || !kblk || !fn || c->P > tl::SERVE_MAX_P) return TL_ESIZE;
+    DeviceGuard guard(c->device);
+    if (!guard.ok) return TL_ECUDA;
+    tl_ctx::Serve &v = c->sv;
+    v.max_rows = max_rows; v.idle_ns = (unsigned long long)(idle_timeout_s * 1e9);
+    const size_t npair = (size_t)(c->cfg.ny + 1) / 2, nsx = (size_t)(c->cfg.nx + 3) / 4, ext_row = (size_t)c->He * c->pitch;
+    bool ok = cuda_ok(cudaHostAlloc(reinterpret_cast<void **>(&v.ctl), sizeof(tl::ServeCtl), cudaHostAllocMapped));
+    if (ok) memset(v.ctl, 0, sizeof(tl::ServeCtl));
+    ok = ok && cuda_ok(cudaHostGetDevicePointer(reinterpret_cast<void **>(&v.ctl_dev), v.ctl, 0));
+    ok = ok && cuda_ok(cudaMalloc(&v.dev, sizeof(tl::ServeDev))) && cuda_ok(cudaMalloc(&v.rows, sizeof(tl::RowC) * tl::SERVE_MAX_ROWS)) &&
+         cuda_ok(cudaMalloc(&v.ext, sizeof(float) * ext_row * tl::SERVE_MAX_ROWS)) &&
+         cuda_ok(cudaMalloc(&v.cblk, sizeof(float) * npair * nsx * tl::SERVE_MAX_ROWS)) &&
+         cuda_ok(cudaMalloc(&v.params, sizeof(float) * tl::SERVE_MAX_ROWS * tl::SERVE_MAX_P)) &&
+         cuda_ok(cudaMalloc(&v.counters, sizeof(int) * 2 * tl::SERVE_MAX_ROWS)) &&
+         cuda_ok(cudaMemset(v.ext, 0, sizeof(float) * ext_row * tl::SERVE_MAX_ROWS)) &&       // the pitch padding reads as zeros
+         cuda_ok(cudaStreamCreateWithFlags(&v.stream, cudaStreamNonBlocking));
+    if (ok) {
+        // the grid: every resident slot; shared memory: the largest band any request size needs on that grid
+        ok = cuda_ok(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(SMEM_LIMIT - 4096)));
+        int occ = 0;
+        size_t smem = 0;
+        for (int pass = 0; pass < 2 && ok; ++pass) {                             // the occupancy depends on the size, the size on the grid
+            ok = cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, c->threads, smem)) && occ >= 1;
+            v.grid = occ * c->n_sm;
+            smem = 0;
+            for (int B = 1; B <= max_rows && ok; ++B) {
+                int pr, bd, bp, xs;
+                size_t cs;
+                serve_geometry(c, B, v.grid, &pr, &bd, &bp, &xs, &cs);
+                if (cs > smem) smem = cs;
+            }
+        }
+        v.smem = smem;
+        ok = ok && cuda_ok(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, c->threads, smem)) && occ * c->n_sm >= v.grid;
+    }
+    if (ok) { v.fn = fn; ok = serve_launch(c); }
+    if (!ok) { cudaGetLastError(); serve_free(c); return TL_ECUDA; }
+    return TL_OK;
+}
+
+int tl_serve_eval(tl_ctx *c, const float *params_host, int32_t B, float *logL_host)
+{
+    if (!c || !c->sv.fn || !params_host || !logL_host || B < 1 || B > c->sv.max_rows) return TL_EINVAL;
+    tl_ctx::Serve &v = c->sv;
+    tl::ServeCtl *ctl = v.ctl;
+    int pr, bd, bp, xs;
+    size_t cs;
+    serve_geometry(c, B, v.grid, &pr, &bd, &bp, &xs, &cs);
+    ctl->B = B; ctl->per_row = pr; ctl->bands = bd; ctl->band_pairs = bp; ctl->xseg = xs;
+    memcpy(ctl->params, params_host, sizeof(float) * (size_t)B * c->P);
+    const unsigned long long n = ++v.seq;
+    __atomic_store_n(&ctl->seq, n, __ATOMIC_RELEASE);
+    struct timespec t0, t1;
+    clock_gettime(CLOCK_MONOTONIC, &t0);
+    for (unsigned spin = 0;; ++spin) {
+        if (__atomic_load_n(&ctl->done, __ATOMIC_ACQUIRE) == n) break;
+        if ((spin & 1023) == 1023) {
+            if (__atomic_load_n(&ctl->alive, __ATOMIC_ACQUIRE) == 0 && __atomic_load_n(&ctl->done, __ATOMIC_ACQUIRE) != n) {
+                // the kernel left (idle or lifetime limit) before it saw this request: start it again
+                DeviceGuard guard(c->device);
+                if (!guard.ok || ctl->error || !serve_launch(c)) return TL_ECUDA;
+            }
+            clock_gettime(CLOCK_MONOTONIC, &t1);
+            if ((t1.tv_sec - t0.tv_sec) + 1e-9 * (t1.tv_nsec - t0.tv_nsec) > 20.0) return TL_ECUDA;
+        }
+    }
+    memcpy(logL_host, const_cast<const float *>(ctl->logL), sizeof(float) * (size_t)B);
+    return TL_OK;
+}
+
+int tl_serve_stop(tl_ctx *c)
+{
+    if (!c) return TL_EINVAL;
+    if (!c->sv.fn) return TL_OK;
+    DeviceGuard guard(c->device);
+    __atomic_store_n(&c->sv.ctl->seq, tl::SERVE_EXIT, __ATOMIC_RELEASE);
+    const bool ok = guard.ok && cuda_ok(cudaStreamSynchronize(c->sv.stream));
+    serve_free(c);
+    return ok ? TL_OK : TL_ECUDA;
+}
+
+}  // extern "C"
 
 // ------------------------------------------------------------------ tl_loglike_batch_noalloc
 // The per-row constants of tl_loglike_batch's fused path (RowC[B], written by prologue_kernel, read by
@@ -1282,6 +1449,7 @@ int tl_last_kernel_ms(tl_ctx *c, float *ms)
 void tl_destroy(tl_ctx *c)
 {
     if (!c) return;
+    tl_serve_stop(c);
     if (c->ev0) cudaEventDestroy(c->ev0);
     if (c->ev1) cudaEventDestroy(c->ev1);
     for (auto &sl : c->slots) {

@@ -216,7 +216,6 @@ __device__ inline bool shape_from_e(double e1, double e2, double *q, double *c, 
     return true;
 }
 
-#ifdef TL_MAIN_TU
 // the constants of one slot of one row: slot 0 = lens, slot 1 + k = Sersic component k
 __device__ __forceinline__ void prologue_slot(const PrologueArgs &a, int64_t row, int slot)
 {
@@ -389,6 +388,7 @@ __device__ __forceinline__ void prologue_slot(const PrologueArgs &a, int64_t row
     rc->comp[a.mge ? (is_lens_light ? a.n_source + k : k - a.n_lens_light) : k] = C;
 }
 
+#ifdef TL_MAIN_TU
 // One block = 32 rows; warp w takes slot w, w + 4, ... of them, so that the lens branch and the Sersic
 // branch never share a warp (they are long FP64 chains: side by side in a warp they run one after the
 // other, which was half of a one-row call's prologue).  Grid: prologue_blocks(B).

@@ -876,24 +876,16 @@ __global__ void __launch_bounds__(256, 2) trace_kernel(const KArgs a, int chunk_
 // longest chain of the call -- the FP64 refinement of the samples next to the source centre, which
 // trace_tiles runs sixteen deep per lane at S = 4 -- becomes two deep, and one row fills the GPU.
 // Rows on the q < 0.5 branch go through trace_tiles.  Grid (rows, CTAs per row): as many as are resident at once.
+// (body: warp `warp` of the `n_warps` that share the row whose constants are rc_s; no CTA-wide barrier inside)
 template <int S_T, int NLL, int NSRC>
-__global__ void __launch_bounds__(256, 2) trace_pairs_kernel(const KArgs a, int chunk_rows)
+__device__ __forceinline__ void trace_pairs_row(const RowC &rc_s, const KArgs &a, float *dst, int warp, int n_warps)
 {
     static_assert(S_T == 2 || S_T == 4 || S_T == 8, "S^2 / 2 lanes per pixel must divide a warp");
     constexpr int NP = S_T / 2, LPP = S_T * NP, PPW = 32 / LPP;
-    __shared__ RowC rc_s;
-    pdl_launch();
-    pdl_wait();                                        // the row constants come from the prologue kernel
-    const int r = blockIdx.x;
-    if (r >= chunk_rows) return;
-    load_row_consts(&rc_s, a.rows + r);
-    __syncthreads();
-    if (!row_is_valid(rc_s, a.n_comp)) return;
-    float *dst = a.ext + (size_t)r * a.He * a.pitch;
-    const int warp = (blockIdx.y * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
+    const int lane = threadIdx.x & 31;
     const HotC<NLL, NSRC, MASS_SIE> h(rc_s);
     if (rc_s.lens.mode != 0) {                         // uniform over the row
-        const int n = a.tiles_x * a.tiles_y, n_warps = (gridDim.y * blockDim.x) >> 5;
+        const int n = a.tiles_x * a.tiles_y;
         int t = (int)((long long)n * warp / n_warps);
         const int t_end = (int)((long long)n * (warp + 1) / n_warps);
         trace_tiles<S_T, NLL, NSRC, false, false, MASS_SIE>(rc_s, h, a, nullptr, [&]() -> int { return t < t_end ? t++ : -1; },
@@ -901,7 +893,7 @@ __global__ void __launch_bounds__(256, 2) trace_pairs_kernel(const KArgs a, int 
         return;
     }
     const int sub = lane % LPP, sa = sub / NP, sp = sub - sa * NP, base = lane - sub;
-    const int npix = a.He * a.We, n_warps = (gridDim.y * blockDim.x) >> 5;
+    const int npix = a.He * a.We;
     // warp tiles of PPW pixels, dealt out round-robin: neighbouring tiles (the refined ones cluster
     // round the source centre) go to different warps
     for (int p0 = warp * PPW; p0 < npix; p0 += n_warps * PPW) {
@@ -951,6 +943,21 @@ __global__ void __launch_bounds__(256, 2) trace_pairs_kernel(const KArgs a, int 
         un2(acc2, a0, a1);
         if (live && sub == 0) dst[i * a.pitch + j] = edge ? 0.f : a0 + a1;
     }
+}
+
+template <int S_T, int NLL, int NSRC>
+__global__ void __launch_bounds__(256, 2) trace_pairs_kernel(const KArgs a, int chunk_rows)
+{
+    __shared__ RowC rc_s;
+    pdl_launch();
+    pdl_wait();                                        // the row constants come from the prologue kernel
+    const int r = blockIdx.x;
+    if (r >= chunk_rows) return;
+    load_row_consts(&rc_s, a.rows + r);
+    __syncthreads();
+    if (!row_is_valid(rc_s, a.n_comp)) return;
+    trace_pairs_row<S_T, NLL, NSRC>(rc_s, a, a.ext + (size_t)r * a.He * a.pitch, (blockIdx.y * blockDim.x + threadIdx.x) >> 5,
+                                    (gridDim.y * blockDim.x) >> 5);
 }
 
 #ifdef TL_MAIN_TU
@@ -1006,6 +1013,8 @@ __global__ void finalize_kernel(const KArgs a, int chunk_rows)
     const double ll = -0.5 * (s + a.lconst[row / a.rows_per_lens]);
     a.logL[row] = isfinite(s) ? (float)ll : -INFINITY;
 }
+
+#endif  // TL_MAIN_TU
 
 // ------------------------------------------------------------------------------ small batches
 // (NEXT-4: the sampler hands over small proposal batches.)  With fewer rows
@@ -1093,31 +1102,33 @@ __device__ __forceinline__ void conv_blocks_split(const KArgs &a, const float *i
 // one CTA per (row, band of `band_pairs` output row pairs x one of `xseg` runs of strips); cblk:
 // [chunk][npair * nsx] or null; a.tile_counters[chunk_rows + r] (zeroed) counts the finished CTAs of row r.
 // xseg = 0: whole bands, one thread per block (conv_blocks_store: more rows than the split form pays for)
-__global__ void __launch_bounds__(512) conv_small_kernel(const KArgs a, int chunk_rows, int band_pairs, int xseg, float *cblk)
+// (body: row r, virtual block `by` of `n_by` per row; every thread of the CTA calls; `wait`: the rows / images
+// come from kernels launched before this one with programmatic dependent launch)
+// Returns true (to every thread) when this call wrote the row's logL.
+__device__ __forceinline__ bool conv_small_body(const KArgs &a, int chunk_rows, int r, int by, int n_by, int band_pairs, int xseg,
+                                                float *cblk, unsigned char *smem_raw, bool wait)
 {
     __shared__ double red[32];
     __shared__ int is_last;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
     float *taps = reinterpret_cast<float *>(smem_raw);
     float *part = taps + a.K * a.Kp;                                // [blockDim.x / K][K][8]
     float *img = xseg ? part + (blockDim.x / a.K) * a.K * 8 : part;
-    const int r = blockIdx.x;
     const int npair = (a.ny + 1) / 2, nsx = (a.nx + 3) / 4;
     const int nseg = xseg ? xseg : 1;
-    const int band = blockIdx.y / nseg, seg = blockIdx.y - band * nseg;
+    const int band = by / nseg, seg = by - band * nseg;
     const int p0 = band * band_pairs, p1 = min(npair, p0 + band_pairs);
     const int xb0 = (int)((long long)nsx * seg / nseg), xb1 = (int)((long long)nsx * (seg + 1) / nseg);
     const int64_t row = a.row0 + r;
     const int64_t lens = row / a.rows_per_lens;
     const size_t npix = (size_t)a.ny * a.nx;
     load_psf(taps, a.psf + lens * a.K * a.Kp, a.K * a.Kp);          // context data: before the wait
-    pdl_wait();                                                   // rows / ext come from the preceding kernels
+    if (wait) pdl_wait();                                         // rows / ext come from the preceding kernels
     if (!row_is_valid(a.rows[r], a.n_comp)) {
         if (a.images && seg == 0)
             for (size_t i = (size_t)2 * p0 * a.nx + threadIdx.x; i < (size_t)min(a.ny, 2 * p1) * a.nx; i += blockDim.x)
                 a.images[row * npix + i] = NAN;
-        if (a.logL && blockIdx.y == 0 && threadIdx.x == 0) a.logL[row] = -INFINITY;
-        return;
+        if (a.logL && by == 0 && threadIdx.x == 0) a.logL[row] = -INFINITY;
+        return a.logL && by == 0;
     }
     // extended rows 2 p0 .. 2 (p1 - 1) + K of this row's binned image (the last one may lie past
     // the image when ny is odd: zeros), plus the slack the strips may touch
@@ -1145,20 +1156,28 @@ __global__ void __launch_bounds__(512) conv_small_kernel(const KArgs a, int chun
     default: break;
     }
 #undef TL_CONV_CASE
-    if (!cb) return;
+    if (!cb) return false;
     // the row's last band to finish reduces the stored terms: per-thread partials over
     // s = tid, tid + blockDim, ... and block_sum, exactly as fused_kernel does
     __threadfence();
     __syncthreads();
-    if (threadIdx.x == 0) is_last = atomicAdd(a.tile_counters + chunk_rows + r, 1) == (int)gridDim.y - 1;
+    if (threadIdx.x == 0) is_last = atomicAdd(a.tile_counters + chunk_rows + r, 1) == n_by - 1;
     __syncthreads();
-    if (!is_last) return;
+    if (!is_last) return false;
     __threadfence();
     const int total = npair * nsx;
     double psum = 0.0;
     for (int s = threadIdx.x; s < total; s += blockDim.x) psum += (double)__ldcg(cb + s);
     const double chi2 = block_sum(psum, red);
     if (threadIdx.x == 0) a.logL[row] = (float)(-0.5 * (chi2 + a.lconst[lens]));
+    return true;
+}
+
+#ifdef TL_MAIN_TU
+__global__ void __launch_bounds__(512) conv_small_kernel(const KArgs a, int chunk_rows, int band_pairs, int xseg, float *cblk)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    conv_small_body(a, chunk_rows, blockIdx.x, blockIdx.y, gridDim.y, band_pairs, xseg, cblk, smem_raw, true);
 }
 
 #endif  // TL_MAIN_TU
