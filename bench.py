@@ -684,6 +684,58 @@ def run_peaks(args):
                                             "rsqrt.approx.f64": err[2], "rsqrt + 1 Newton": err[3]}}))
 
 
+def run_serve(args):
+    """`--serve`: host-to-host latency of small requests through the persistent serving kernel (tl_serve_eval)
+    beside the ordinary host entry point (tl_loglike_batch_host), configs[`--config`], as one JSON line."""
+    import torch
+    from paper_2503_08586_b200 import api
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    torch.cuda.set_device(0)
+    w = W.workload(args.config)
+    dev = torch.device("cuda", 0)
+
+    def gpu_render(w1, psf, row):
+        ctx = api.LensContext(w1.ny, w1.nx, w1.pix_scale, w1.supersample, w1.n_lens_light, w1.n_source,
+                              psf[None], np.zeros((1, w1.ny, w1.nx), np.float32),
+                              np.ones((1, w1.ny, w1.nx), np.float32), w1.edge_mode, mass_model=w1.mass_model)
+        im = ctx.render(torch.from_numpy(np.ascontiguousarray(row[None])).to(dev)).cpu().numpy()[0]
+        ctx.close()
+        return im
+
+    prob = W.make_problem(w, gpu_render)
+    ctx = api.LensContext.from_problem(prob)
+    rows = W.batch_rows(w, 16)
+    res = []
+    with ClockSampler(0) as clk:
+        for B in (1, 2, 4, 8, 16):
+            r = np.ascontiguousarray(rows[:B])
+            out = np.empty(B, np.float32)
+            for _ in range(20):
+                ctx.loglike_host(r)
+            t0 = time.perf_counter()
+            for _ in range(200):
+                ctx.loglike_host(r)
+            t_host = (time.perf_counter() - t0) / 200
+            ref = ctx.loglike_host(r)
+            ctx.serve_start(max_rows=16, idle_timeout_s=1.0)
+            try:
+                for _ in range(50):
+                    ctx.serve_eval(r, out)
+                t0 = time.perf_counter()
+                for _ in range(1000):
+                    ctx.serve_eval(r, out)
+                t_serve = (time.perf_counter() - t0) / 1000
+            finally:
+                ctx.serve_stop()
+            res.append({"B": B, "served_us": 1e6 * t_serve, "host_entry_us": 1e6 * t_host,
+                        "served_per_s": B / t_serve, "host_entry_per_s": B / t_host,
+                        "bitwise_equal": bool(np.array_equal(np.asarray(ref), out))})
+    print(json.dumps({"metric": "host-to-host latency of a small request", "unit": "us", "higher_is_better": False,
+                      "config": config_dict(w, "n/a (one request at a time)"), "requests": res, "clocks": clk.summary(),
+                      "data": "synthetic", "dtype": "f32"}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -716,9 +768,14 @@ def main():
     ap.add_argument("--sub-batch", type=int, default=4096, help="rows per sub-batch when --streams > 1")
     ap.add_argument("--peaks", action="store_true",
                     help="run the pipe micro-benchmarks (tl_measure_peaks: FFMA, FFMA2, MUFU, DFMA and mixes) and exit")
+    ap.add_argument("--serve", action="store_true",
+                    help="latency of 1..16-row requests through the persistent serving kernel (tl_serve_eval) and exit")
     args = ap.parse_args()
     if args.peaks:
         run_peaks(args)
+        return
+    if args.serve:
+        run_serve(args)
         return
     w = W.workload(args.config)
     if args.mass == "epl":
