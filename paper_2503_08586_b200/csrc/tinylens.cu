@@ -1030,7 +1030,11 @@ int tl_loglike_linear_batch(tl_ctx *c, const float *params, int64_t B, float *lo
     // FP64 (and AUTO: with the amplitudes solved every row is near its best fit, so every row needs it)
     if (c->precision == TL_PRECISION_FP64 || c->precision == TL_PRECISION_AUTO)
         return run_dp(c, params, B, logL, nullptr, st, nullptr, nullptr, 1, amps);
-    if (c->fused_lin && !c->opt.linear_staged) {
+    // few rows (a sampler's small proposal batches): the fused pipeline gives a row to ONE CTA, so such
+    // a call costs a whole row-time of one SM (0.21 ms on configs[1]); the staged pipeline spreads a row over many
+    // CTAs -- and returns the same bits
+    const bool few = B <= c->n_sm / 2 && c->opt.small_batch_rows != 0;
+    if (c->fused_lin && !c->opt.linear_staged && !few) {
         const int64_t chunkf = CONST_CHUNK < B ? CONST_CHUNK : B;
         tl::RowC *rowsf = nullptr;
         float *mscr = nullptr;
@@ -1084,12 +1088,29 @@ int tl_loglike_linear_batch(tl_ctx *c, const float *params, int64_t B, float *lo
         a.tile_rows = c->lin_tile_rows; a.n_tiles = c->lin_n_tiles; a.rowtab = c->lin_rowtab;
         a.tile_counters = reinterpret_cast<int *>(rows + chunk);          // the row's CTAs draw warp tiles from one queue (see run_batch)
         cudaMemsetAsync(a.tile_counters, 0, sizeof(int) * (size_t)nb, st);
-        dim3 tg((unsigned)nb, 8);
+        int slabs = 8;
+        size_t conv_smem = c->lin_conv_smem;
+        if (few) {
+            // as many CTAs per row as are resident at once: more ray-trace slabs, thinner convolution tiles (pairs of rows)
+            const int want = 2 * c->n_sm / (int)nb, n_wtiles = a.tiles_x * a.tiles_y;
+            slabs = want < (n_wtiles + 7) / 8 ? want : (n_wtiles + 7) / 8;
+            if (slabs < 1) slabs = 1;
+            int nt = want / NC;
+            if (nt < 1) nt = 1;
+            int tr = (c->cfg.ny + nt - 1) / nt;
+            tr = (tr + 1) & ~1;
+            if (tr < 2) tr = 2;
+            if (tr < c->lin_tile_rows) {
+                a.tile_rows = tr; a.n_tiles = (c->cfg.ny + tr - 1) / tr;
+                conv_smem = conv_smem_bytes(c, tr);
+            }
+        }
+        dim3 tg((unsigned)nb, (unsigned)slabs);
         if (c->profile) cudaEventRecord(c->ev0, st);
         c->trace_lin<<<tg, 256, c->lin_trace_smem, st>>>(a, (int)nb);
         if (c->profile) { cudaEventRecord(c->ev1, st); c->prof_pending = 1; }
-        dim3 cg((unsigned)nb, (unsigned)c->lin_n_tiles, (unsigned)NC);
-        tl::conv_lin_kernel<<<cg, 256, c->lin_conv_smem, st>>>(a, (int)nb);
+        dim3 cg((unsigned)nb, (unsigned)a.n_tiles, (unsigned)NC);
+        tl::conv_lin_kernel<<<cg, 256, conv_smem, st>>>(a, (int)nb);
         tl::solve_lin_kernel<<<(unsigned)nb, 256, 0, st>>>(a, (int)nb);
         if (!cuda_ok(cudaGetLastError())) rc = TL_ECUDA;
     }

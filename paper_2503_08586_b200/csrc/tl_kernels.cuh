@@ -594,6 +594,30 @@ __device__ __forceinline__ double block_sum(double v, double *red)
     return s;
 }
 
+// N sums at once through one pair of barriers: value by value the operations of block_sum in the same order, so
+// the same bits; red: N * 32 doubles.
+template <int N>
+__device__ __forceinline__ void block_sum_n(double (&v)[N], double *red)
+{
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+#pragma unroll
+    for (int n = 0; n < N; ++n) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v[n] += __shfl_down_sync(0xffffffffu, v[n], o);
+        if (lane == 0) red[n * 32 + wid] = v[n];
+    }
+    __syncthreads();
+    if (threadIdx.x < N) {
+        double s = 0.0;
+        for (int w = 0; w < nw; ++w) s += red[threadIdx.x * 32 + w];
+        red[threadIdx.x * 32] = s;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int n = 0; n < N; ++n) v[n] = red[n * 32];
+    __syncthreads();
+}
+
 __device__ __forceinline__ void load_row_consts(RowC *dst, const RowC *src)
 {
     const int n16 = sizeof(RowC) / 16;
@@ -1232,50 +1256,60 @@ __global__ void __launch_bounds__(256, 2) conv_lin_kernel(const KArgs a, int chu
 
 #endif  // TL_MAIN_TU
 
-// G = M'WM, b = M'Wd (fixed-shape FP64 reductions), NNLS, chi^2 of the residual d - M s -> logL.
+// G = M'WM, b = M'Wd, d'Wd (fixed-shape FP64 reductions), NNLS, chi^2 = d'Wd - 2 s'b + s'G s -> logL.
 // All threads of the CTA; M = the row's blurred unit-amplitude component images [C][npix].
+// red: 32 doubles, or -- red_wide -- 10 * 32 (then the ten sums share one pair of barriers: calls with a few rows,
+// where the row's one CTA is what the caller waits for).
 __device__ __forceinline__ void solve_row(const KArgs &a, const float *M, int64_t row, int64_t lens,
-                                          double *red, double *s_sh)
+                                          double *red, double *s_sh, bool red_wide = false)
 {
+    (void)s_sh;
     const int NC = a.n_comp, npix = a.ny * a.nx;
     const float *d = a.data + lens * (size_t)npix, *w = a.wgt + lens * (size_t)npix;
     double g[6] = {0, 0, 0, 0, 0, 0}, bb[3] = {0, 0, 0};             // G00 G01 G02 G11 G12 G22
     double dd = 0.0;                                               // d'Wd: the scale of "zero" for the solver
+    const float *M1 = NC > 1 ? M + (size_t)npix : M, *M2 = NC > 2 ? M + 2 * (size_t)npix : M;
+    const double k1 = NC > 1 ? 1.0 : 0.0, k2 = NC > 2 ? 1.0 : 0.0;   // (absent components: exact zeros, as before)
+#pragma unroll 4
     for (int i = threadIdx.x; i < npix; i += blockDim.x) {
         const double wi = w[i], di = d[i];
-        double m[3] = {0.0, 0.0, 0.0};
-        for (int k = 0; k < NC; ++k) m[k] = M[(size_t)k * npix + i];
+        const double m[3] = {(double)M[i], k1 * (double)M1[i], k2 * (double)M2[i]};
         g[0] += wi * m[0] * m[0]; g[1] += wi * m[0] * m[1]; g[2] += wi * m[0] * m[2];
         g[3] += wi * m[1] * m[1]; g[4] += wi * m[1] * m[2]; g[5] += wi * m[2] * m[2];
         bb[0] += wi * m[0] * di; bb[1] += wi * m[1] * di; bb[2] += wi * m[2] * di;
         dd += wi * di * di;
     }
     double G[3][3], b[3];
-    const double g0 = block_sum(g[0], red), g1 = block_sum(g[1], red), g2 = block_sum(g[2], red),
-                 g3 = block_sum(g[3], red), g4 = block_sum(g[4], red), g5 = block_sum(g[5], red);
-    b[0] = block_sum(bb[0], red); b[1] = block_sum(bb[1], red); b[2] = block_sum(bb[2], red);
-    const double dwd = block_sum(dd, red);
+    double g0, g1, g2, g3, g4, g5, dwd;
+    if (red_wide) {
+        double v[10] = {g[0], g[1], g[2], g[3], g[4], g[5], bb[0], bb[1], bb[2], dd};
+        block_sum_n<10>(v, red);
+        g0 = v[0]; g1 = v[1]; g2 = v[2]; g3 = v[3]; g4 = v[4]; g5 = v[5]; b[0] = v[6]; b[1] = v[7]; b[2] = v[8]; dwd = v[9];
+    } else {
+        g0 = block_sum(g[0], red); g1 = block_sum(g[1], red); g2 = block_sum(g[2], red);
+        g3 = block_sum(g[3], red); g4 = block_sum(g[4], red); g5 = block_sum(g[5], red);
+        b[0] = block_sum(bb[0], red); b[1] = block_sum(bb[1], red); b[2] = block_sum(bb[2], red);
+        dwd = block_sum(dd, red);
+    }
     if (threadIdx.x == 0) {
         G[0][0] = g0; G[0][1] = G[1][0] = g1; G[0][2] = G[2][0] = g2; G[1][1] = g3; G[1][2] = G[2][1] = g4; G[2][2] = g5;
         // the paper's solver (Bro & De Jong's Gram-matrix active set), as in the MGE mode
         double s[3] = {0.0, 0.0, 0.0}, Lc[9], z[3];
         nnls_gram<3>(NC, &G[0][0], 3, b, dwd, s, Lc, z);
-        s_sh[0] = s[0]; s_sh[1] = s[1]; s_sh[2] = s[2];
-    }
-    __syncthreads();
-    const double s0 = s_sh[0], s1 = s_sh[1], s2 = s_sh[2];
-    double part = 0.0;
-    for (int i = threadIdx.x; i < npix; i += blockDim.x) {
-        double m = s0 * M[i];
-        if (NC > 1) m += s1 * M[(size_t)npix + i];
-        if (NC > 2) m += s2 * M[2 * (size_t)npix + i];
-        const double res = (double)d[i] - m;
-        part += res * res * (double)w[i];
-    }
-    const double chi2 = block_sum(part, red);
-    if (threadIdx.x == 0) {
+        // chi^2 = d'Wd - 2 s'b + s'G s at the solved amplitudes (Eq. 5), as in the MGE mode: the three
+        // terms are FP64 sums of exact products of the FP32 columns, ~1e9 against chi^2 ~1e4 -- 1e-7 absolute, so
+        // the second pass over the pixels that formed the residual is not needed
+        double sb = 0.0, sGs = 0.0;
+        for (int i = 0; i < NC; ++i) {
+            if (s[i] == 0.0) continue;
+            sb += s[i] * b[i];
+            double gi = 0.0;
+            for (int k = 0; k < NC; ++k) gi += G[i][k] * s[k];
+            sGs += s[i] * gi;
+        }
+        const double chi2 = (dwd - 2.0 * sb) + sGs;
         a.logL[row] = (float)(-0.5 * (chi2 + a.lconst[lens]));
-        if (a.amps) { a.amps[row * NC] = (float)s0; if (NC > 1) a.amps[row * NC + 1] = (float)s1; if (NC > 2) a.amps[row * NC + 2] = (float)s2; }
+        if (a.amps) { a.amps[row * NC] = (float)s[0]; if (NC > 1) a.amps[row * NC + 1] = (float)s[1]; if (NC > 2) a.amps[row * NC + 2] = (float)s[2]; }
     }
 }
 
@@ -1291,12 +1325,12 @@ __device__ __forceinline__ void invalid_row_lin(const KArgs &a, int64_t row)
 // staged pipeline: one CTA per row
 __global__ void __launch_bounds__(256) solve_lin_kernel(const KArgs a, int chunk_rows)
 {
-    __shared__ double red[32];
+    __shared__ double red[10 * 32];
     __shared__ double s_sh[3];
     const int r = blockIdx.x;
     const int64_t row = a.row0 + r;
     if (!row_is_valid(a.rows[r], a.n_comp)) { invalid_row_lin(a, row); return; }
-    solve_row(a, a.mimg + (size_t)r * a.n_comp * a.ny * a.nx, row, row / a.rows_per_lens, red, s_sh);
+    solve_row(a, a.mimg + (size_t)r * a.n_comp * a.ny * a.nx, row, row / a.rows_per_lens, red, s_sh, true);
 }
 
 #endif  // TL_MAIN_TU
