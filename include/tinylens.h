@@ -276,7 +276,9 @@ int tl_loglike_batch_noalloc(tl_ctx *ctx, const float *params, int64_t B, float 
  * Asynchronous on cuda_stream; bitwise reproducible.  Two pipelines with identical results
  * (bit for bit): fused (the component images of a row stay in shared memory; chosen when they
  * fit) and staged (component images through global memory; larger images, or
- * tl_options.linear_staged).  The NNLS problem is solved on the Gram matrix by the active-set
+ * tl_options.linear_staged; also calls of at most half the SM count of rows, whose rows it spreads over
+ * the whole GPU: 0.08 instead of 0.21 ms for one row of the CSST-like config).  chi^2 at the solved
+ * amplitudes is d'Wd - 2 s'b + s'G s from the FP64 Gram quantities.  The NNLS problem is solved on the Gram matrix by the active-set
  * iteration of Bro & De Jong.  Returns TL_OK, TL_EINVAL, TL_ENOMEM, TL_ECUDA,
  * or TL_ESIZE when the PSF tile does not fit in shared memory.
  */
