@@ -1343,17 +1343,42 @@ int tl_loglike_mge_batch(tl_ctx *c, const float *params, int64_t B, float *logL,
         at.rowtab = c->mge_rowtab; at.ext_nc = ext_nc; at.ext_k0 = fused ? 0 : NG;
         at.tile_counters = reinterpret_cast<int *>(rows + chunk);
         cudaMemsetAsync(at.tile_counters, 0, sizeof(int) * (size_t)nb, st);
-        c->mge_trace<<<dim3((unsigned)nb, 2), 256, c->mge_trace_smem, st>>>(at, (int)nb);       // (slabs per row: 1 .. 4 measured equal, 8 1 % slower)
+        // calls with a few rows (a sampler's small proposal batches): as many CTAs per row as are resident at once
+        const bool few = nb <= c->n_sm / 2 && c->opt.small_batch_rows != 0;
+        const int want = few ? 2 * c->n_sm / (int)nb : 0;
+        int tslabs = 2;                                        // (slabs per row: 1 .. 4 measured equal, 8 1 % slower)
+        if (few) {
+            const int n_wtiles = at.tiles_x * at.tiles_y;
+            tslabs = want < (n_wtiles + 7) / 8 ? want : (n_wtiles + 7) / 8;
+            if (tslabs < 1) tslabs = 1;
+        }
+        c->mge_trace<<<dim3((unsigned)nb, (unsigned)tslabs), 256, c->mge_trace_smem, st>>>(at, (int)nb);
         a.ext_nc = NC;                                         // from here on: the width of M
         if (fused) {
             // 2. every Gaussian evaluated into shared memory and blurred from there -> M[0 .. NG)
             if (c->profile) cudaEventRecord(c->ev0, st);
-            tl::gauss_conv_for(c->cfg.supersample, c->K)<<<dim3((unsigned)nb, (unsigned)NG), 256, c->mge_gc_smem, st>>>(a, (int)nb);
+            int gbands = 1;                                    // few rows: the output row pairs of a Gaussian over several CTAs
+            const bool kblk = c->K == 5 || c->K == 15 || c->K == 21 || c->K == 31 || c->K == 41;
+            if (few && kblk) {
+                gbands = want / NG;
+                const int npair = (c->cfg.ny + 1) / 2;
+                if (gbands > npair) gbands = npair;
+                if (gbands < 1) gbands = 1;
+            }
+            tl::gauss_conv_for(c->cfg.supersample, c->K)<<<dim3((unsigned)nb, (unsigned)NG, (unsigned)gbands), 256, c->mge_gc_smem, st>>>(a, (int)nb);
             if (c->profile) { cudaEventRecord(c->ev1, st); c->prof_pending = 1; }
             // 3. the sources blurred -> M[NG ..)
             tl::KArgs ac = a;
             ac.conv_ext_nc = NS; ac.conv_m_nc = NC; ac.conv_m_k0 = NG;
-            tl::conv_lin_kernel<<<dim3((unsigned)nb, (unsigned)c->lin_n_tiles, (unsigned)NS), 256, c->lin_conv_smem, st>>>(ac, (int)nb);
+            size_t lsmem = c->lin_conv_smem;
+            if (few) {                                         // thin tiles (pairs of rows): the source images over many CTAs too
+                int nt = want / NS;
+                if (nt < 1) nt = 1;
+                int tr = ((c->cfg.ny + nt - 1) / nt + 1) & ~1;
+                if (tr < 2) tr = 2;
+                if (tr < c->lin_tile_rows) { ac.tile_rows = tr; ac.n_tiles = (c->cfg.ny + tr - 1) / tr; lsmem = conv_smem_bytes(c, tr); }
+            }
+            tl::conv_lin_kernel<<<dim3((unsigned)nb, (unsigned)ac.n_tiles, (unsigned)NS), 256, lsmem, st>>>(ac, (int)nb);
         } else {
             for (int j = 0, k0 = 0; j < c->mge_n_sets; k0 += c->mge_per_set[j], ++j) {          // one launch per set
                 tl::KArgs ag = a;

@@ -98,13 +98,13 @@ __global__ void __launch_bounds__(256) mge_gauss_kernel(const KArgs a, int chunk
 }
 
 // The 2 x 4 blocks of output row pairs ip0 .. ip1 x strips xb0 .. xb1 (inclusive) of one blurred image
-// -> image_out; every other pixel of image_out is written as 0.  (gauss_conv_kernel: outside that
+// -> image_out; every other pixel of the row pairs zp0 .. zp1 of image_out is written as 0.  (gauss_conv_kernel: outside that
 // rectangle every window holds nothing but exact zeros, and ConvBlock's sums of +-0 products are +0.)
 template <int K>
 __device__ __forceinline__ void conv_blocks_rect(const KArgs &a, const float *img, const float *taps,
-                                                 int ip0, int ip1, int xb0, int xb1, float *image_out)
+                                                 int ip0, int ip1, int xb0, int xb1, float *image_out, int zp0, int zp1)
 {
-    const int nsx = (a.nx + 3) / 4, npair = (a.ny + 1) / 2;
+    const int nsx = (a.nx + 3) / 4;
     const int nbx = xb1 - xb0 + 1, nby = ip1 - ip0 + 1;
     const float zero[4] = {0.f, 0.f, 0.f, 0.f};
     if (nbx > 0 && nby > 0) {
@@ -116,8 +116,8 @@ __device__ __forceinline__ void conv_blocks_rect(const KArgs &a, const float *im
             if (i + 1 < a.ny) chi2_strip(a, a1, i + 1, x0, nullptr, nullptr, image_out);
         }
     }
-    for (int s = threadIdx.x; s < npair * nsx; s += blockDim.x) {
-        const int ip = s / nsx, xb = s - ip * nsx;
+    for (int s = threadIdx.x; s < (zp1 - zp0 + 1) * nsx; s += blockDim.x) {           // the pairs zp0 .. zp1 are this CTA's
+        const int ip = zp0 + s / nsx, xb = s - (ip - zp0) * nsx;
         if (ip >= ip0 && ip <= ip1 && xb >= xb0 && xb <= xb1) continue;
         chi2_strip(a, zero, 2 * ip, 4 * xb, nullptr, nullptr, image_out);
         if (2 * ip + 1 < a.ny) chi2_strip(a, zero, 2 * ip + 1, 4 * xb, nullptr, nullptr, image_out);
@@ -175,10 +175,17 @@ __global__ void __launch_bounds__(256, (K_T > 0 && K_T <= 21) ? 3 : 2) gauss_con
             i_hi = min(i_hi, (int)ceilf((cY + rho - 1.f + (float)(S * a.He)) * inv2s) + 1);
         }
     }
+    // calls with a few rows: the output row pairs are shared out over gridDim.z CTAs (bands), each evaluating only the
+    // extended rows its outputs read
+    const int npair = (a.ny + 1) / 2, per_band = (npair + gridDim.z - 1) / gridDim.z;
+    const int pb0 = blockIdx.z * per_band, pb1 = min(npair, pb0 + per_band) - 1;       // this CTA's pairs (inclusive)
+    if (pb0 > pb1) return;
+    const int e_lo = 2 * pb0, e_hi = min(a.He - 1, 2 * pb1 + 1 + a.K - 1);            // the extended rows they read
+    i_lo = max(i_lo, e_lo); i_hi = min(i_hi, e_hi);
     const int bw = j_hi - j_lo + 1, bh = i_hi - i_lo + 1;
     {   // everything outside the box, the pitch padding and the slack read as zero
-        float4 *z = reinterpret_cast<float4 *>(img);
-        const int n4 = (npx + a.pitch + a.Kp + 8 + 3) / 4;
+        float4 *z = reinterpret_cast<float4 *>(img) + (e_lo * a.pitch) / 4;           // (pitch is a multiple of 4)
+        const int n4 = (((gridDim.z == 1 ? npx : (e_hi + 1) * a.pitch) - e_lo * a.pitch) + a.pitch + a.Kp + 8 + 3) / 4;
         for (int p = threadIdx.x; p < n4; p += blockDim.x) z[p] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
     __syncthreads();
@@ -243,8 +250,9 @@ __global__ void __launch_bounds__(256, (K_T > 0 && K_T <= 21) ? 3 : 2) gauss_con
     // output (i, x) reads extended rows i .. i + K - 1 and columns x .. x + K - 1
     const int oi0 = max(0, i_lo - a.K + 1), oi1 = min(a.ny - 1, i_hi), ox0 = max(0, j_lo - a.K + 1), ox1 = min(a.nx - 1, j_hi);
     const bool none = bw <= 0 || bh <= 0 || oi0 > oi1 || ox0 > ox1;
-    const int ip0 = none ? 1 : oi0 / 2, ip1 = none ? 0 : oi1 / 2, xb0 = none ? 1 : ox0 / 4, xb1 = none ? 0 : ox1 / 4;
-    if constexpr (K_T > 0) { conv_blocks_rect<K_T>(a, img, taps, ip0, ip1, xb0, xb1, out); return; }
+    const int ip0 = none ? 1 : max(pb0, oi0 / 2), ip1 = none ? 0 : min(pb1, oi1 / 2), xb0 = none ? 1 : ox0 / 4, xb1 = none ? 0 : ox1 / 4;
+    if constexpr (K_T > 0) { conv_blocks_rect<K_T>(a, img, taps, ip0, ip1, xb0, xb1, out, pb0, pb1); return; }
+    if (gridDim.z != 1) return;                                               // (other PSF sizes are launched without bands)
     // other PSF sizes: the generic 1 x 4 strips over the whole image
     const int nsx = (a.nx + CONV_R - 1) / CONV_R;
     for (int s = threadIdx.x; s < a.ny * nsx; s += blockDim.x) {
