@@ -70,7 +70,9 @@ extern "C" {
 #define TL_PRECISION_FP64_LIBM 2 /* the same model with CUDA's double math library (csrc/tl_precise.cuh):   */
                                  /* slow; an independent check of the polynomial FP64 path                  */
 #define TL_PRECISION_AUTO      3 /* FP32 for every row, then the rows whose first-order FP32 error bound    */
-                                 /* exceeds the tolerance are re-evaluated in FP64 (rows near the best fit) */
+                                 /* exceeds the tolerance are re-evaluated in FP64 (rows near the best fit); */
+                                 /* calls of at most half the SM count of rows are evaluated in FP64 outright */
+                                 /* (faster there than the FP32 pass, which gives a row to one CTA)            */
 
 #define TL_EDGE_EXTEND 0 /* evaluate the analytic model on a border of h = (K-1)/2 pixels so   */
                          /* every output pixel sees its full PSF support (Eq. 3 with only the  */

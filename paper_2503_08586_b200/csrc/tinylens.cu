@@ -402,6 +402,10 @@ int run_batch(tl_ctx *c, const float *params, int64_t B, float *logL, float *ima
     // AUTO on the split path (large images): the conv tiles do not carry the error sums, so every row
     // is evaluated in FP64; AUTO renders are FP32 renders (the image has no 1e-8 requirement)
     if (autop && c->path == 1) return run_dp(c, params, B, logL, images, st, nullptr, nullptr);
+    // AUTO with a few rows: the FP32 pass would give each row to one CTA (a whole row-time of one SM), the FP64 path
+    // spreads a row over the GPU and is the faster of the two up to half the SM count of rows (71 against 166 us for one
+    // row of configs[1]) -- and meets the tolerance on every row by construction
+    if (autop && B <= c->n_sm / 2) return run_dp(c, params, B, logL, nullptr, st, nullptr, nullptr);
     if (c->path == 0 && B <= c->sb_max_rows && !autop) return run_small_batch(c, params, B, logL, images, st);
     int *flags = nullptr;                            // [0] = count, [1 .. B] = flagged rows
     if (autop) {
