@@ -1438,6 +1438,18 @@ int tl_loglike_batch_host_async(tl_ctx *c, const float *params, int64_t B, float
     }
     memcpy(sl.h_params, params, sizeof(float) * (size_t)B * c->P);       // the caller's buffer is free again on return
     int rc = TL_OK;
+    // up to 8 rows (measured: 56 -> 45 us host to host for one row, no gain from 16): the kernels read the rows from and write logL to the pinned staging buffers themselves (under 1 KB over
+    // PCIe inside the prologue / the last reduction) -- two copies, three events and two stream waits less per call
+    void *hp_dev = nullptr, *hl_dev = nullptr;
+    if (B <= 8 && cuda_ok(cudaHostGetDevicePointer(&hp_dev, sl.h_params, 0)) && cuda_ok(cudaHostGetDevicePointer(&hl_dev, sl.h_logl, 0))) {
+        rc = run_batch(c, static_cast<const float *>(hp_dev), B, static_cast<float *>(hl_dev), nullptr, st);
+        if (rc == TL_OK && !cuda_ok(cudaEventRecord(sl.fin, st))) rc = TL_ECUDA;
+        if (rc != TL_OK) return rc;
+        sl.B = B; sl.user_logl = logL; sl.busy = 1; sl.rc = TL_OK;
+        c->next_slot = id ^ 1;
+        return id;
+    }
+    cudaGetLastError();
     if (!cuda_ok(cudaMemcpyAsync(sl.d_params, sl.h_params, sizeof(float) * (size_t)B * c->P, cudaMemcpyHostToDevice, c->s_up)) ||
         !cuda_ok(cudaEventRecord(sl.up, c->s_up)) || !cuda_ok(cudaStreamWaitEvent(st, sl.up, 0))) rc = TL_ECUDA;
     if (rc == TL_OK) rc = run_batch(c, sl.d_params, B, sl.d_logl, nullptr, st);
