@@ -165,6 +165,11 @@ typedef struct {
                                 /*    keeps cached between calls                                */
     double  refine_tau;         /* 0 default, else the selective-FP64 threshold in units of     */
                                 /*    sigma_min                                  */
+    int32_t debug_canaries;     /* 1: every per-call scratch allocation carries 256 guard bytes */
+                                /*    on either side, checked when it is freed                  */
+                                /*    (tl_debug_canary_errors); a debugging aid, a few launches */
+                                /*    more per call                                             */
+    int32_t reserved;           /* 0                                                            */
 } tl_options;
 int tl_create_ex(tl_ctx **out, const tl_config *cfg,
                  const float *psf, int32_t psf_ny, int32_t psf_nx,
@@ -420,6 +425,18 @@ typedef struct {
     double ms;                 /* duration of the probe kernel                                  */
 } tl_peak;
 int tl_measure_peaks(tl_peak *out, int32_t n_max, double *seed_err4);
+
+/*
+ * Guard-word check of the library's scratch memory (compute-sanitizer is not available everywhere): a context
+ * created with tl_options.debug_canaries = 1 surrounds every per-call scratch allocation with 256 bytes of
+ * 0xA5 and, when the allocation is freed (stream-ordered, at the end of the call), counts the guard words that
+ * changed.  tl_debug_canary_errors synchronises the device and returns that count (0 = no kernel of any call so
+ * far wrote outside its scratch buffers); tl_debug_canary_selftest writes one word on either side of a test
+ * allocation on purpose and returns TL_OK when both hits are counted (the counter is reset afterwards).
+ * TL_EINVAL for a context without the option.
+ */
+int tl_debug_canary_errors(tl_ctx *ctx, int64_t *count);
+int tl_debug_canary_selftest(tl_ctx *ctx);
 
 /* Release a context and its device memory (NULL is allowed).                                  */
 void tl_destroy(tl_ctx *ctx);

@@ -48,7 +48,7 @@ class tl_info(C.Structure):
 class tl_options(C.Structure):
     _fields_ = [("small_batch_rows", C.c_int32), ("force_split", C.c_int32), ("block_threads", C.c_int32),
                 ("linear_staged", C.c_int32), ("mge_chunk_rows", C.c_int64), ("scratch_keep_bytes", C.c_int64),
-                ("refine_tau", C.c_double)]
+                ("refine_tau", C.c_double), ("debug_canaries", C.c_int32), ("reserved", C.c_int32)]
 
 
 class tl_peak(C.Structure):
@@ -83,6 +83,8 @@ def load(build_if_missing: bool = True):
     L.tl_get_info.restype = C.c_int; L.tl_get_info.argtypes = [vp, C.POINTER(tl_info)]
     L.tl_loglike_batch.restype = C.c_int; L.tl_loglike_batch.argtypes = [vp, vp, i64, vp, vp]
     L.tl_render_batch.restype = C.c_int; L.tl_render_batch.argtypes = [vp, vp, i64, vp, vp]
+    L.tl_debug_canary_errors.restype = C.c_int; L.tl_debug_canary_errors.argtypes = [vp, C.POINTER(i64)]
+    L.tl_debug_canary_selftest.restype = C.c_int; L.tl_debug_canary_selftest.argtypes = [vp]
     L.tl_serve_start.restype = C.c_int; L.tl_serve_start.argtypes = [vp, i32, C.c_double]
     L.tl_serve_eval.restype = C.c_int; L.tl_serve_eval.argtypes = [vp, vp, i32, vp]
     L.tl_serve_stop.restype = C.c_int; L.tl_serve_stop.argtypes = [vp]
@@ -434,6 +436,15 @@ class LensContext:
 
     def loglike(self, params, out=None, stream=None):
         return tl_loglike_batch(self.handle, params, out, stream)
+
+    def canary_errors(self) -> int:
+        """Guard words of the scratch allocations found changed so far (contexts created with options={"debug_canaries": 1})."""
+        n = C.c_int64(0)
+        _check(load().tl_debug_canary_errors(self.handle, C.byref(n)), "tl_debug_canary_errors")
+        return int(n.value)
+
+    def canary_selftest(self):
+        _check(load().tl_debug_canary_selftest(self.handle), "tl_debug_canary_selftest")
 
     def serve_start(self, max_rows=16, idle_timeout_s=2.0):
         tl_serve_start(self.handle, max_rows, idle_timeout_s)

@@ -8,6 +8,7 @@
 #include <cstring>
 #include <ctime>
 #include <mutex>
+#include <unordered_map>
 #include <new>
 #include <vector>
 
@@ -117,6 +118,10 @@ struct tl_ctx {
         unsigned long long seq = 0, idle_ns = 0;
     } sv;
     tl_options opt;               // create-time options (tl_create_ex); defaults = automatic
+    // tl_options.debug_canaries: every scratch allocation carries 256 guard bytes on either side, checked when it is freed
+    int *canary_errors = nullptr;                              // device counter of guard words found changed
+    mutable std::mutex canary_mu;
+    mutable std::unordered_map<void *, size_t> canary_size;    // user pointer -> bytes (rounded up to 256)
     cudaMemPool_t pool = nullptr; // library-owned stream-ordered pool: per-call scratch (never the device's default pool)
     // benchmark facility (tl_set_profiling): events around the dominant kernel of the last call
     int profile = 0;
@@ -159,15 +164,55 @@ struct DeviceGuard {
 };
 
 // per-call scratch: stream-ordered allocation from the context's own pool
+constexpr size_t CANARY_BYTES = 256;
+constexpr unsigned CANARY_WORD = 0xA5A5A5A5u;
+
+__global__ void canary_check_kernel(const unsigned *front, const unsigned *back, int *errors)
+{
+    if (front[threadIdx.x] != CANARY_WORD) atomicAdd(errors, 1);
+    if (back[threadIdx.x] != CANARY_WORD) atomicAdd(errors, 1);
+}
+
 template <class T>
 inline bool pool_alloc(const tl_ctx *c, T **p, size_t bytes, cudaStream_t st)
 {
     *p = nullptr;
     void *v = nullptr;
-    const cudaError_t e = c->pool ? cudaMallocFromPoolAsync(&v, bytes ? bytes : 1, c->pool, st) : cudaMallocAsync(&v, bytes ? bytes : 1, st);
+    const bool guard = c->canary_errors != nullptr;
+    const size_t body = guard ? ((bytes ? bytes : 1) + CANARY_BYTES - 1) / CANARY_BYTES * CANARY_BYTES : (bytes ? bytes : 1);
+    const size_t total = guard ? body + 2 * CANARY_BYTES : body;
+    const cudaError_t e = c->pool ? cudaMallocFromPoolAsync(&v, total, c->pool, st) : cudaMallocAsync(&v, total, st);
     if (e != cudaSuccess) { cudaGetLastError(); return false; }
+    if (guard) {
+        unsigned char *b = static_cast<unsigned char *>(v);
+        cudaMemsetAsync(b, 0xA5, CANARY_BYTES, st);
+        cudaMemsetAsync(b + CANARY_BYTES + body, 0xA5, CANARY_BYTES, st);
+        v = b + CANARY_BYTES;
+        std::lock_guard<std::mutex> lock(c->canary_mu);
+        c->canary_size[v] = body;
+    }
     *p = static_cast<T *>(v);
     return true;
+}
+
+inline void pool_free(const tl_ctx *c, void *p, cudaStream_t st)
+{
+    if (!p) return;
+    if (c->canary_errors) {
+        size_t body = 0;
+        {
+            std::lock_guard<std::mutex> lock(c->canary_mu);
+            auto it = c->canary_size.find(p);
+            if (it != c->canary_size.end()) { body = it->second; c->canary_size.erase(it); }
+        }
+        if (body) {
+            unsigned char *b = static_cast<unsigned char *>(p) - CANARY_BYTES;
+            canary_check_kernel<<<1, (unsigned)(CANARY_BYTES / sizeof(unsigned)), 0, st>>>(
+                reinterpret_cast<const unsigned *>(b), reinterpret_cast<const unsigned *>(b + CANARY_BYTES + body), c->canary_errors);
+            p = b;
+        }
+    }
+    cudaFreeAsync(p, st);
 }
 
 size_t fused_smem_bytes(const tl_ctx *c)
@@ -287,7 +332,7 @@ int run_small_batch(tl_ctx *c, const float *params, int64_t B, float *logL, floa
     lc.gridDim = dim3((unsigned)nb, (unsigned)(bands * (xseg ? xseg : 1))); lc.blockDim = dim3((unsigned)c->threads); lc.dynamicSmemBytes = conv_smem;
     okl = okl && cuda_ok(cudaLaunchKernelEx(&lc, tl::conv_small_kernel, (const tl::KArgs)a, nb, band_pairs, xseg, cblk));
     const int rc = (okl && cuda_ok(cudaGetLastError())) ? TL_OK : TL_ECUDA;
-    cudaFreeAsync(blob, st);
+    pool_free(c, blob, st);
     return rc;
 }
 
@@ -310,9 +355,9 @@ int run_dp(tl_ctx *c, const float *params, int64_t B, float *logL, float *images
     if (!pool_alloc(c, &ext, ext_row * (size_t)chunk, st) ||
         !pool_alloc(c, &partial, sizeof(double) * (size_t)chunk * c->dp_n_bands, st) ||
         (lin && !pool_alloc(c, &m64, m_row * (size_t)chunk, st))) {
-        cudaFreeAsync(rows, st);
-        if (ext) cudaFreeAsync(ext, st);
-        if (partial) cudaFreeAsync(partial, st);
+        pool_free(c, rows, st);
+        if (ext) pool_free(c, ext, st);
+        if (partial) pool_free(c, partial, st);
         return TL_ENOMEM;
     }
     // the pitch padding (Wp - We <= 1 column) is read by discarded strip lanes only, but must be finite
@@ -348,8 +393,8 @@ int run_dp(tl_ctx *c, const float *params, int64_t B, float *logL, float *images
         else if (logL) tl::finalize_dp_kernel<<<(unsigned)((nb + 127) / 128), 128, 0, st>>>(a);
         if (!cuda_ok(cudaGetLastError())) rc = TL_ECUDA;
     }
-    cudaFreeAsync(rows, st); cudaFreeAsync(ext, st); cudaFreeAsync(partial, st);
-    if (m64) cudaFreeAsync(m64, st);
+    pool_free(c, rows, st); pool_free(c, ext, st); pool_free(c, partial, st);
+    if (m64) pool_free(c, m64, st);
     return rc;
 }
 
@@ -395,7 +440,7 @@ int run_batch(tl_ctx *c, const float *params, int64_t B, float *logL, float *ima
             tl::precise_conv_kernel<<<(unsigned)nb, 256, 0, st>>>(pa);
             if (!cuda_ok(cudaGetLastError())) prc = TL_ECUDA;
         }
-        cudaFreeAsync(pext, st);
+        pool_free(c, pext, st);
         return prc;
     }
     const bool autop = c->precision == TL_PRECISION_AUTO && logL != nullptr;
@@ -423,8 +468,8 @@ int run_batch(tl_ctx *c, const float *params, int64_t B, float *logL, float *ima
         const size_t ext_bytes = sizeof(float) * (size_t)chunk * c->He * c->pitch;
         if (!pool_alloc(c, &ext, ext_bytes, st) ||
             !pool_alloc(c, &partial, sizeof(double) * (size_t)chunk * c->n_tiles, st)) {
-            cudaFreeAsync(rows, st);
-            if (ext) cudaFreeAsync(ext, st);
+            pool_free(c, rows, st);
+            if (ext) pool_free(c, ext, st);
             return TL_ENOMEM;
         }
         cudaMemsetAsync(ext, 0, ext_bytes, st);      // pitch padding must read as finite zeros
@@ -470,12 +515,12 @@ int run_batch(tl_ctx *c, const float *params, int64_t B, float *logL, float *ima
         }
         if (!cuda_ok(cudaGetLastError())) rc = TL_ECUDA;
     }
-    cudaFreeAsync(rows, st);
-    if (ext) cudaFreeAsync(ext, st);
-    if (partial) cudaFreeAsync(partial, st);
+    pool_free(c, rows, st);
+    if (ext) pool_free(c, ext, st);
+    if (partial) pool_free(c, partial, st);
     if (autop) {
         if (rc == TL_OK) rc = run_dp(c, params, B, logL, nullptr, st, flags + 1, flags);
-        cudaFreeAsync(flags, st);
+        pool_free(c, flags, st);
     }
     return rc;
 }
@@ -543,6 +588,37 @@ bool serve_launch(tl_ctx *c)
 }  // namespace
 
 extern "C" {
+
+int tl_debug_canary_errors(tl_ctx *c, int64_t *count)
+{
+    if (!c || !count) return TL_EINVAL;
+    *count = 0;
+    if (!c->canary_errors) return TL_EINVAL;                   // the context was not created with tl_options.debug_canaries
+    DeviceGuard guard(c->device);
+    int n = 0;
+    if (!guard.ok || !cuda_ok(cudaDeviceSynchronize()) || !cuda_ok(cudaMemcpy(&n, c->canary_errors, sizeof(int), cudaMemcpyDeviceToHost))) return TL_ECUDA;
+    *count = n;
+    return TL_OK;
+}
+
+namespace { __global__ void canary_poke_kernel(unsigned *p) { *p = 0u; } }
+
+int tl_debug_canary_selftest(tl_ctx *c)
+{
+    if (!c || !c->canary_errors) return TL_EINVAL;
+    DeviceGuard guard(c->device);
+    if (!guard.ok) return TL_ECUDA;
+    int64_t before = 0, after = 0;
+    if (tl_debug_canary_errors(c, &before) != TL_OK) return TL_ECUDA;
+    unsigned *buf = nullptr;
+    if (!pool_alloc(c, &buf, 1000, nullptr)) return TL_ENOMEM;        // 1000 bytes: the body is rounded up to 1024
+    canary_poke_kernel<<<1, 1>>>(buf + 1024 / sizeof(unsigned));      // the first guard word behind the body
+    canary_poke_kernel<<<1, 1>>>(buf - 1);                            // the last guard word in front of it
+    pool_free(c, buf, nullptr);
+    if (tl_debug_canary_errors(c, &after) != TL_OK) return TL_ECUDA;
+    if (!cuda_ok(cudaMemset(c->canary_errors, 0, sizeof(int)))) return TL_ECUDA;   // the two deliberate hits do not count
+    return after - before == 2 ? TL_OK : TL_ECUDA;
+}
 
 int tl_serve_start(tl_ctx *c, int32_t max_rows, double idle_timeout_s)
 {
@@ -727,6 +803,7 @@ int tl_create_ex(tl_ctx **out, const tl_config *cfg, const float *psf_in, int32_
         if (opt->small_batch_rows < -1 || opt->mge_chunk_rows < 0 || opt->scratch_keep_bytes < 0) return TL_EINVAL;
         if (opt->block_threads && (opt->block_threads < 32 || opt->block_threads > 512 || opt->block_threads % 32)) return TL_EINVAL;
         if (opt->refine_tau < 0.0 || !std::isfinite(opt->refine_tau)) return TL_EINVAL;
+        if (opt->debug_canaries < 0 || opt->debug_canaries > 1 || opt->reserved != 0) return TL_EINVAL;
     }
     if (cfg->ny < 1 || cfg->nx < 1 || !(cfg->pix_scale > 0.0) || !std::isfinite(cfg->pix_scale)) return TL_EINVAL;
     if (cfg->supersample < 1 || cfg->supersample > 16) return TL_EINVAL;
@@ -786,6 +863,9 @@ int tl_create_ex(tl_ctx **out, const tl_config *cfg, const float *psf_in, int32_
             cudaMemPoolSetAttribute(c->pool, cudaMemPoolAttrReleaseThreshold, &keep);
         } else c->pool = nullptr;                     // falls back to the default pool (untouched)
         cudaGetLastError();
+    }
+    if (c->opt.debug_canaries) {
+        if (!cuda_ok(cudaMalloc(&c->canary_errors, sizeof(int))) || !cuda_ok(cudaMemset(c->canary_errors, 0, sizeof(int)))) { tl_destroy(c); return TL_ECUDA; }
     }
     c->n_comp = cfg->n_lens_light + cfg->n_source;
     c->lens_np = 7 + (cfg->mass_model == TL_MASS_EPL ? 1 : 0);
@@ -1043,7 +1123,7 @@ int tl_loglike_linear_batch(tl_ctx *c, const float *params, int64_t B, float *lo
         tl::RowC *rowsf = nullptr;
         float *mscr = nullptr;
         if (!pool_alloc(c, &rowsf, sizeof(tl::RowC) * (size_t)chunkf, st)) return TL_ENOMEM;
-        if (!pool_alloc(c, &mscr, sizeof(float) * (size_t)c->lin_fused_grid * NC * npix, st)) { cudaFreeAsync(rowsf, st); return TL_ENOMEM; }
+        if (!pool_alloc(c, &mscr, sizeof(float) * (size_t)c->lin_fused_grid * NC * npix, st)) { pool_free(c, rowsf, st); return TL_ENOMEM; }
         const int64_t rpl = B / c->cfg.n_lens;
         int rcf = TL_OK;
         for (int64_t r0 = 0; r0 < B && rcf == TL_OK; r0 += chunkf) {
@@ -1061,7 +1141,7 @@ int tl_loglike_linear_batch(tl_ctx *c, const float *params, int64_t B, float *lo
             if (c->profile) { cudaEventRecord(c->ev1, st); c->prof_pending = 1; }
             if (!cuda_ok(cudaGetLastError())) rcf = TL_ECUDA;
         }
-        cudaFreeAsync(rowsf, st); cudaFreeAsync(mscr, st);
+        pool_free(c, rowsf, st); pool_free(c, mscr, st);
         return rcf;
     }
     const size_t ext_row = sizeof(float) * (size_t)NC * c->He * c->pitch, m_row = sizeof(float) * NC * npix;
@@ -1074,8 +1154,8 @@ int tl_loglike_linear_batch(tl_ctx *c, const float *params, int64_t B, float *lo
     if (!pool_alloc(c, &rows, (sizeof(tl::RowC) + sizeof(int)) * (size_t)chunk, st)) return TL_ENOMEM;   // + a tile-queue head per row
     if (!pool_alloc(c, &ext, ext_row * (size_t)chunk, st) ||
         !pool_alloc(c, &mimg, m_row * (size_t)chunk, st)) {
-        cudaFreeAsync(rows, st);
-        if (ext) cudaFreeAsync(ext, st);
+        pool_free(c, rows, st);
+        if (ext) pool_free(c, ext, st);
         return TL_ENOMEM;
     }
     cudaMemsetAsync(ext, 0, ext_row * (size_t)chunk, st);      // pitch padding must read as finite zeros
@@ -1118,7 +1198,7 @@ int tl_loglike_linear_batch(tl_ctx *c, const float *params, int64_t B, float *lo
         tl::solve_lin_kernel<<<(unsigned)nb, 256, 0, st>>>(a, (int)nb);
         if (!cuda_ok(cudaGetLastError())) rc = TL_ECUDA;
     }
-    cudaFreeAsync(rows, st); cudaFreeAsync(ext, st); cudaFreeAsync(mimg, st);
+    pool_free(c, rows, st); pool_free(c, ext, st); pool_free(c, mimg, st);
     return rc;
 }
 
@@ -1229,10 +1309,10 @@ int run_mge_dp(tl_ctx *c, const float *params, int64_t B, float *logL, float *am
     if (!pool_alloc(c, &rows, sizeof(tl::RowC) * (size_t)chunk, st) || !pool_alloc(c, &rowsd, sizeof(tl::RowD) * (size_t)chunk, st) ||
         !pool_alloc(c, &ext, ext_row * (size_t)chunk, st) || !pool_alloc(c, &m64, m_row * (size_t)chunk, st) ||
         !pool_alloc(c, &gram, g_row * (size_t)chunk, st)) {
-        if (rows) cudaFreeAsync(rows, st);
-        if (rowsd) cudaFreeAsync(rowsd, st);
-        if (ext) cudaFreeAsync(ext, st);
-        if (m64) cudaFreeAsync(m64, st);
+        if (rows) pool_free(c, rows, st);
+        if (rowsd) pool_free(c, rowsd, st);
+        if (ext) pool_free(c, ext, st);
+        if (m64) pool_free(c, m64, st);
         return TL_ENOMEM;
     }
     if (c->dp_Wp != c->We) cudaMemsetAsync(ext, 0, ext_row * (size_t)chunk, st);     // pitch padding must be finite
@@ -1277,7 +1357,7 @@ int run_mge_dp(tl_ctx *c, const float *params, int64_t B, float *logL, float *am
         tl::nnls_mge_kernel<<<(unsigned)((nb + tl::MGE_NNLS_WARPS - 1) / tl::MGE_NNLS_WARPS), 32 * tl::MGE_NNLS_WARPS, nnls_smem, st>>>(a, (int)nb);
         if (!cuda_ok(cudaGetLastError())) rc = TL_ECUDA;
     }
-    cudaFreeAsync(rows, st); cudaFreeAsync(rowsd, st); cudaFreeAsync(ext, st); cudaFreeAsync(m64, st); cudaFreeAsync(gram, st);
+    pool_free(c, rows, st); pool_free(c, rowsd, st); pool_free(c, ext, st); pool_free(c, m64, st); pool_free(c, gram, st);
     return rc;
 }
 }  // namespace
@@ -1315,10 +1395,10 @@ int tl_loglike_mge_batch(tl_ctx *c, const float *params, int64_t B, float *logL,
             pool_alloc(c, &mimg, m_row * (size_t)chunk, st) &&
             pool_alloc(c, &gram, g_row * (size_t)chunk, st)) break;
         cudaGetLastError();                                    // an allocation failure is not sticky
-        if (rows) cudaFreeAsync(rows, st);
-        if (ext) cudaFreeAsync(ext, st);
-        if (mimg) cudaFreeAsync(mimg, st);
-        if (gram) cudaFreeAsync(gram, st);
+        if (rows) pool_free(c, rows, st);
+        if (ext) pool_free(c, ext, st);
+        if (mimg) pool_free(c, mimg, st);
+        if (gram) pool_free(c, gram, st);
         if (chunk == 1) return TL_ENOMEM;
         chunk = (chunk + 1) / 2;
     }
@@ -1401,7 +1481,7 @@ int tl_loglike_mge_batch(tl_ctx *c, const float *params, int64_t B, float *logL,
         tl::nnls_mge_kernel<<<(unsigned)((nb + tl::MGE_NNLS_WARPS - 1) / tl::MGE_NNLS_WARPS), 32 * tl::MGE_NNLS_WARPS, nnls_smem, st>>>(a, (int)nb);
         if (!cuda_ok(cudaGetLastError())) rc = TL_ECUDA;
     }
-    cudaFreeAsync(rows, st); cudaFreeAsync(ext, st); cudaFreeAsync(mimg, st); cudaFreeAsync(gram, st);
+    pool_free(c, rows, st); pool_free(c, ext, st); pool_free(c, mimg, st); pool_free(c, gram, st);
     return rc;
 }
 
@@ -1523,7 +1603,7 @@ void tl_destroy(tl_ctx *c)
     }
     if (c->s_up) cudaStreamDestroy(c->s_up);
     if (c->s_down) cudaStreamDestroy(c->s_down);
-    cudaFree(c->mge_c); cudaFree(c->mge_set);
+    cudaFree(c->mge_c); cudaFree(c->mge_set); cudaFree(c->canary_errors);
     cudaFree(c->psf); cudaFree(c->data); cudaFree(c->wgt); cudaFree(c->wgt64); cudaFree(c->noise); cudaFree(c->sigma_min); cudaFree(c->lconst);
     if (c->pool) cudaMemPoolDestroy(c->pool);
     delete c;
