@@ -166,7 +166,9 @@ typedef struct {
     double  refine_tau;         /* 0 default, else the selective-FP64 threshold in units of     */
                                 /*    sigma_min                                  */
     int32_t debug_canaries;     /* 1: every per-call scratch allocation carries 256 guard bytes */
-                                /*    on either side, checked when it is freed                  */
+                                /*    on either side, checked when it is freed, and starts      */
+                                /*    filled with 0xFF (NaN / -1: a read of scratch that nobody */
+                                /*    wrote shows in the results)                               */
                                 /*    (tl_debug_canary_errors); a debugging aid, a few launches */
                                 /*    more per call                                             */
     int32_t reserved;           /* 0                                                            */

@@ -186,6 +186,7 @@ inline bool pool_alloc(const tl_ctx *c, T **p, size_t bytes, cudaStream_t st)
     if (guard) {
         unsigned char *b = static_cast<unsigned char *>(v);
         cudaMemsetAsync(b, 0xA5, CANARY_BYTES, st);
+        cudaMemsetAsync(b + CANARY_BYTES, 0xFF, body, st);           // the body starts as NaNs / -1: a read of scratch nobody wrote shows in the result
         cudaMemsetAsync(b + CANARY_BYTES + body, 0xA5, CANARY_BYTES, st);
         v = b + CANARY_BYTES;
         std::lock_guard<std::mutex> lock(c->canary_mu);

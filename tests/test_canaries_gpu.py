@@ -4,7 +4,9 @@ compute-sanitizer cannot be run on this GPU pool (profiles/r2_sanitizers.md), so
 its own for writes outside the per-call scratch buffers: 256 bytes of 0xA5 on either side of every
 allocation, compared when it is freed.  Every entry point and every path (fused, small-batch, split, staged,
 FP64, AUTO, libm, linear, MGE with one and two sets, host entries) is driven here on several shapes with the
-option on; the count must stay 0, and the self-test must see its two deliberate hits."""
+option on; the count must stay 0, and the self-test must see its two deliberate hits.  With the option the
+scratch also starts filled with 0xFF (NaN / -1), so a kernel that read scratch nobody wrote would change the
+results: they must equal those of a context without the option bit for bit."""
 import numpy as np
 import pytest
 
@@ -45,8 +47,12 @@ def test_no_kernel_writes_outside_its_scratch(api, w):
     import torch
     prob = W.make_problem(w, _flat_data)
     ctx = api.LensContext.from_problem(prob, options={"debug_canaries": 1})
+    plain = api.LensContext.from_problem(prob)                     # (the scratch of `ctx` starts as NaNs: same results all the same)
     ctx.canary_selftest()                                          # the check sees a word changed on either side
     assert ctx.canary_errors() == 0
+
+    def same(x, y):
+        return torch.equal(torch.nan_to_num(x, nan=-7.0), torch.nan_to_num(y, nan=-7.0))
     big = W.batch_rows(w, max(1, 200 // w.n_lens))                 # more rows than half the SMs: the large-batch paths
     small = W.batch_rows(w, 1 if w.n_lens > 1 else 3)              # a few rows: the small-batch routes
     big[1, 0] = -1.0                                               # an invalid row
@@ -55,17 +61,19 @@ def test_no_kernel_writes_outside_its_scratch(api, w):
         for prec in (api.TL_PRECISION_FP32, api.TL_PRECISION_FP64, api.TL_PRECISION_AUTO, api.TL_PRECISION_FP64_LIBM):
             if prec == api.TL_PRECISION_FP64_LIBM and (w.mass_model or rows is big and w.name == "large"):
                 continue
-            ctx.set_precision(prec)
-            ctx.loglike(d)
+            ctx.set_precision(prec); plain.set_precision(prec)
+            assert same(ctx.loglike(d), plain.loglike(d)), (w.name, prec)
             if prec in (api.TL_PRECISION_FP32, api.TL_PRECISION_FP64):
-                ctx.render(d[: 2 * w.n_lens].contiguous())
+                sub = d[: 2 * w.n_lens].contiguous()
+                assert same(ctx.render(sub), plain.render(sub)), (w.name, prec)
             if w.n_lens_light <= 1 and prec != api.TL_PRECISION_FP64_LIBM:
-                ctx.loglike_linear(d)
-        ctx.set_precision(api.TL_PRECISION_FP32)
-        ctx.loglike_host(np.ascontiguousarray(rows))
+                (la, aa), (lb, ab) = ctx.loglike_linear(d), plain.loglike_linear(d)
+                assert same(la, lb) and same(aa, ab), (w.name, prec)
+        ctx.set_precision(api.TL_PRECISION_FP32); plain.set_precision(api.TL_PRECISION_FP32)
+        assert np.array_equal(ctx.loglike_host(np.ascontiguousarray(rows)), plain.loglike_host(np.ascontiguousarray(rows)))
     torch.cuda.synchronize()
     assert ctx.canary_errors() == 0
-    ctx.close()
+    ctx.close(); plain.close()
     # the staged linear pipeline where the fused one would have been taken
     if w.n_lens_light <= 1:
         ctx = api.LensContext.from_problem(prob, options={"debug_canaries": 1, "linear_staged": 1})
@@ -80,18 +88,22 @@ def test_mge_kernels_stay_inside_their_scratch(api, idx):
     w = W.workload(idx).scaled(batch=64, n_lens=1) if idx == 3 else W.workload(idx)
     prob = W.make_problem(w, _flat_data)
     ctx = api.LensContext.from_problem(prob, options={"debug_canaries": 1})
-    ctx.set_mge(W.mge_sigmas(w, 10))
+    plain = api.LensContext.from_problem(prob)
+    ctx.set_mge(W.mge_sigmas(w, 10)); plain.set_mge(W.mge_sigmas(w, 10))
     for n in (160, 3):
         d = torch.from_numpy(np.ascontiguousarray(W.batch_rows(w, n))).cuda()
         for prec in (api.TL_PRECISION_FP32, api.TL_PRECISION_FP64):
-            ctx.set_precision(prec)
-            ctx.loglike_mge(d)
-    ctx.set_precision(api.TL_PRECISION_FP32)
-    ctx.set_mge(W.mge_sigmas(w, 14))                               # more than 11 columns: the shared-memory Gram kernel
-    ctx.loglike_mge(torch.from_numpy(np.ascontiguousarray(W.batch_rows(w, 100))).cuda())
+            ctx.set_precision(prec); plain.set_precision(prec)
+            (la, aa), (lb, ab) = ctx.loglike_mge(d), plain.loglike_mge(d)
+            assert torch.equal(la, lb) and torch.equal(aa, ab), (n, prec)
+    ctx.set_precision(api.TL_PRECISION_FP32); plain.set_precision(api.TL_PRECISION_FP32)
+    ctx.set_mge(W.mge_sigmas(w, 14)); plain.set_mge(W.mge_sigmas(w, 14))   # more than 11 columns: the shared-memory Gram kernel
+    d = torch.from_numpy(np.ascontiguousarray(W.batch_rows(w, 100))).cuda()
+    (la, aa), (lb, ab) = ctx.loglike_mge(d), plain.loglike_mge(d)
+    assert torch.equal(la, lb) and torch.equal(aa, ab)
     torch.cuda.synchronize()
     assert ctx.canary_errors() == 0
-    ctx.close()
+    ctx.close(); plain.close()
 
 
 def test_canary_calls_need_the_option(api):
