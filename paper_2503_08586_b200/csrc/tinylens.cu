@@ -1475,7 +1475,7 @@ int tl_loglike_mge_batch(tl_ctx *c, const float *params, int64_t B, float *logL,
             if (c->profile) { cudaEventRecord(c->ev1, st); c->prof_pending = 1; }
         }
         // 4. Gram matrix, 5. NNLS + logL
-        if (NC <= tl::MGE_GRAM_REG_COLS && ((c->cfg.ny * c->cfg.nx) & 1) == 0) tl::gram_reg_for(NC + 1)<<<(unsigned)nb, 128, 0, st>>>(a, (int)nb);
+        if (NC <= tl::MGE_GRAM_REG_COLS && ((c->cfg.ny * c->cfg.nx) & 1) == 0) tl::gram_reg_for(NC + 1, c->cfg.ny * c->cfg.nx)<<<(unsigned)nb, 128, 0, st>>>(a, (int)nb);
         else if (NC + 1 <= 20) tl::gram_mge_kernel<128><<<(unsigned)nb, 128, 0, st>>>(a, (int)nb);
         else tl::gram_mge_kernel<512><<<(unsigned)nb, 512, 0, st>>>(a, (int)nb);
         const size_t nnls_smem = sizeof(double) * tl::MGE_NNLS_WARPS * (size_t)(2 * NC * NC + 3 * NC);

@@ -416,7 +416,9 @@ __global__ void __launch_bounds__(THREADS) gram_mge_kernel(const KArgs a, int ch
 // N1 (N1 + 1) / 2 entries from registers.  Fixed order: a thread's pixels in sequence, then a butterfly
 // over the warp and the four warps in order.  Needs an even pixel count.
 constexpr int MGE_GRAM_REG_COLS = 11;          // (13 columns + data would spill)
-template <int N1>
+// W = 4: four neighbouring pixels per step (16-byte loads, no explicit prefetch: 13 x 16 bytes per thread in flight);
+// needs a pixel count that is a multiple of 4.  W = 2: two pixels per step, the next step's loads in flight meanwhile.
+template <int N1, int W>
 __global__ void __launch_bounds__(128) gram_reg_kernel(const KArgs a, int chunk_rows)
 {
     constexpr int NE = N1 * (N1 + 1) / 2;
@@ -427,26 +429,10 @@ __global__ void __launch_bounds__(128) gram_reg_kernel(const KArgs a, int chunk_
     constexpr int n = N1 - 1;
     if (!row_is_valid(a.rows[r], a.n_comp)) return;   // nnls_mge_kernel reports the row
     const int64_t lens = row / a.rows_per_lens;
-    const int npix = a.ny * a.nx, np2 = npix >> 1;
-    const float2 *M2 = reinterpret_cast<const float2 *>(a.mimg + (size_t)r * n * npix);
-    const float2 *d2 = reinterpret_cast<const float2 *>(a.data + lens * (size_t)npix);
-    const float2 *w2 = reinterpret_cast<const float2 *>(a.wgt + lens * (size_t)npix);
+    const int npix = a.ny * a.nx;
     double acc[NE];
 #pragma unroll
     for (int e = 0; e < NE; ++e) acc[e] = 0.0;
-    float2 cur[N1], nxt[N1], wc, wn;
-    auto fetch = [&](int p, float2 (&v)[N1], float2 &wv) {
-        if (p < np2) {
-#pragma unroll
-            for (int k = 0; k < n; ++k) v[k] = __ldg(M2 + (size_t)k * np2 + p);
-            v[n] = __ldg(d2 + p);
-            wv = __ldg(w2 + p);
-        } else {
-#pragma unroll
-            for (int k = 0; k < N1; ++k) v[k] = make_float2(0.f, 0.f);
-            wv = make_float2(0.f, 0.f);
-        }
-    };
     auto pixel = [&](const double (&v)[N1], double wd) {
         int e = 0;
 #pragma unroll
@@ -456,20 +442,65 @@ __global__ void __launch_bounds__(128) gram_reg_kernel(const KArgs a, int chunk_
             for (int l = k; l < N1; ++l, ++e) acc[e] = fma(wk, v[l], acc[e]);
         }
     };
-    fetch(threadIdx.x, cur, wc);
+    if constexpr (W == 4) {
+        const int np4 = npix >> 2;
+        const float4 *M4 = reinterpret_cast<const float4 *>(a.mimg + (size_t)r * n * npix);
+        const float4 *d4 = reinterpret_cast<const float4 *>(a.data + lens * (size_t)npix);
+        const float4 *w4 = reinterpret_cast<const float4 *>(a.wgt + lens * (size_t)npix);
 #pragma unroll 1
-    for (int p = threadIdx.x; p < np2; p += 128) {
-        fetch(p + 128, nxt, wn);
-        double v[N1];
+        for (int p = threadIdx.x; p < np4; p += 128) {
+            float4 c[N1];
 #pragma unroll
-        for (int k = 0; k < N1; ++k) v[k] = (double)cur[k].x;
-        pixel(v, (double)wc.x);
+            for (int k = 0; k < n; ++k) c[k] = __ldg(M4 + (size_t)k * np4 + p);
+            c[n] = __ldg(d4 + p);
+            const float4 wv = __ldg(w4 + p);
+            double v[N1];
 #pragma unroll
-        for (int k = 0; k < N1; ++k) v[k] = (double)cur[k].y;
-        pixel(v, (double)wc.y);
+            for (int k = 0; k < N1; ++k) v[k] = (double)c[k].x;
+            pixel(v, (double)wv.x);
 #pragma unroll
-        for (int k = 0; k < N1; ++k) cur[k] = nxt[k];
-        wc = wn;
+            for (int k = 0; k < N1; ++k) v[k] = (double)c[k].y;
+            pixel(v, (double)wv.y);
+#pragma unroll
+            for (int k = 0; k < N1; ++k) v[k] = (double)c[k].z;
+            pixel(v, (double)wv.z);
+#pragma unroll
+            for (int k = 0; k < N1; ++k) v[k] = (double)c[k].w;
+            pixel(v, (double)wv.w);
+        }
+    } else {
+        const int np2 = npix >> 1;
+        const float2 *M2 = reinterpret_cast<const float2 *>(a.mimg + (size_t)r * n * npix);
+        const float2 *d2 = reinterpret_cast<const float2 *>(a.data + lens * (size_t)npix);
+        const float2 *w2 = reinterpret_cast<const float2 *>(a.wgt + lens * (size_t)npix);
+        float2 cur[N1], nxt[N1], wc, wn;
+        auto fetch = [&](int p, float2 (&v)[N1], float2 &wv) {
+            if (p < np2) {
+#pragma unroll
+                for (int k = 0; k < n; ++k) v[k] = __ldg(M2 + (size_t)k * np2 + p);
+                v[n] = __ldg(d2 + p);
+                wv = __ldg(w2 + p);
+            } else {
+#pragma unroll
+                for (int k = 0; k < N1; ++k) v[k] = make_float2(0.f, 0.f);
+                wv = make_float2(0.f, 0.f);
+            }
+        };
+        fetch(threadIdx.x, cur, wc);
+#pragma unroll 1
+        for (int p = threadIdx.x; p < np2; p += 128) {
+            fetch(p + 128, nxt, wn);
+            double v[N1];
+#pragma unroll
+            for (int k = 0; k < N1; ++k) v[k] = (double)cur[k].x;
+            pixel(v, (double)wc.x);
+#pragma unroll
+            for (int k = 0; k < N1; ++k) v[k] = (double)cur[k].y;
+            pixel(v, (double)wc.y);
+#pragma unroll
+            for (int k = 0; k < N1; ++k) cur[k] = nxt[k];
+            wc = wn;
+        }
     }
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 #pragma unroll
@@ -494,16 +525,19 @@ __global__ void __launch_bounds__(128) gram_reg_kernel(const KArgs a, int chunk_
 }
 
 typedef void (*gram_reg_fn)(const KArgs, int);
-inline gram_reg_fn gram_reg_for(int n1)
+template <int W>
+inline gram_reg_fn gram_reg_for_w(int n1)
 {
     switch (n1) {
-    case 2: return gram_reg_kernel<2>;   case 3: return gram_reg_kernel<3>;   case 4: return gram_reg_kernel<4>;
-    case 5: return gram_reg_kernel<5>;   case 6: return gram_reg_kernel<6>;   case 7: return gram_reg_kernel<7>;
-    case 8: return gram_reg_kernel<8>;   case 9: return gram_reg_kernel<9>;   case 10: return gram_reg_kernel<10>;
-    case 11: return gram_reg_kernel<11>; case 12: return gram_reg_kernel<12>;
+    case 2: return gram_reg_kernel<2, W>;   case 3: return gram_reg_kernel<3, W>;   case 4: return gram_reg_kernel<4, W>;
+    case 5: return gram_reg_kernel<5, W>;   case 6: return gram_reg_kernel<6, W>;   case 7: return gram_reg_kernel<7, W>;
+    case 8: return gram_reg_kernel<8, W>;   case 9: return gram_reg_kernel<9, W>;   case 10: return gram_reg_kernel<10, W>;
+    case 11: return gram_reg_kernel<11, W>; case 12: return gram_reg_kernel<12, W>;
     default: return nullptr;
     }
 }
+// npix: a multiple of 4 takes the 16-byte loads, else (even) the 8-byte ones
+inline gram_reg_fn gram_reg_for(int n1, int npix) { return (npix & 3) == 0 ? gram_reg_for_w<4>(n1) : gram_reg_for_w<2>(n1); }
 
 // NNLS: one warp per row, the iteration run by the whole warp (nnls_gram_warp, tl_nnls.cuh); four warps per
 // CTA, a compact copy of G in dynamic shared memory (2 n^2 + 3 n doubles per row).  Writes the amplitudes and
