@@ -200,7 +200,8 @@ int tl_get_info(const tl_ctx *ctx, tl_info *info);
  * row does not depend on the batch it is evaluated in: calls with few rows (at most
  * tl_info.small_batch_rows = half the SM count, "CPU<->GPU" round trips of a sampler
  * that proposes small batches) spread each row over many CTAs instead of one, 3 launches instead
- * of 2, and return the same bits as a large batch does.
+ * of 2, and return the same bits as a large batch does; so do the rows of the last, mostly empty
+ * wave of a larger batch (at most that many rows beyond a multiple of the persistent grid).
  */
 int tl_loglike_batch(tl_ctx *ctx, const float *params, int64_t B, float *logL, void *cuda_stream);
 
