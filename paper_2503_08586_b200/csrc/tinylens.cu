@@ -1134,14 +1134,23 @@ int tl_loglike_linear_batch(tl_ctx *c, const float *params, int64_t B, float *lo
     // few rows (a sampler's small proposal batches): the fused pipeline gives a row to ONE CTA, so such
     // a call costs a whole row-time of one SM (0.21 ms on configs[1]); the staged pipeline spreads a row over many
     // CTAs -- and returns the same bits
-    const bool few = B <= c->n_sm / 2 && c->opt.small_batch_rows != 0;
+    bool few = B <= c->n_sm / 2 && c->opt.small_batch_rows != 0;
+    int64_t r_begin = 0;                                       // the staged pipeline serves rows r_begin .. B - 1
     if (c->fused_lin && !c->opt.linear_staged && !few) {
+        // the rows of a last, mostly empty wave of the persistent grid go through the staged pipeline (as in run_batch)
+        int64_t B_tail = 0;
+        if (c->opt.small_batch_rows != 0 && B <= CONST_CHUNK && B > c->lin_fused_grid) {
+            const int64_t rem = B % c->lin_fused_grid;
+            if (rem > 0 && rem <= c->n_sm / 2) B_tail = rem;
+        }
+        const int64_t B_all = B;
+        B -= B_tail;
         const int64_t chunkf = CONST_CHUNK < B ? CONST_CHUNK : B;
         tl::RowC *rowsf = nullptr;
         float *mscr = nullptr;
         if (!pool_alloc(c, &rowsf, sizeof(tl::RowC) * (size_t)chunkf, st)) return TL_ENOMEM;
         if (!pool_alloc(c, &mscr, sizeof(float) * (size_t)c->lin_fused_grid * NC * npix, st)) { pool_free(c, rowsf, st); return TL_ENOMEM; }
-        const int64_t rpl = B / c->cfg.n_lens;
+        const int64_t rpl = B_all / c->cfg.n_lens;
         int rcf = TL_OK;
         for (int64_t r0 = 0; r0 < B && rcf == TL_OK; r0 += chunkf) {
             const int64_t nb = (B - r0 < chunkf) ? (B - r0) : chunkf;
@@ -1159,13 +1168,16 @@ int tl_loglike_linear_batch(tl_ctx *c, const float *params, int64_t B, float *lo
             if (!cuda_ok(cudaGetLastError())) rcf = TL_ECUDA;
         }
         pool_free(c, rowsf, st); pool_free(c, mscr, st);
-        return rcf;
+        r_begin = B;
+        B = B_all;
+        if (rcf != TL_OK || B_tail == 0) return rcf;
+        few = true;
     }
     const size_t ext_row = sizeof(float) * (size_t)NC * c->He * c->pitch, m_row = sizeof(float) * NC * npix;
     int64_t chunk = (int64_t)(EXT_SCRATCH_BYTES / (ext_row + m_row));
     if (chunk < 1) chunk = 1;
     if (chunk > 65535) chunk = 65535;
-    if (chunk > B) chunk = B;
+    if (chunk > B - r_begin) chunk = B - r_begin;
     tl::RowC *rows = nullptr;
     float *ext = nullptr, *mimg = nullptr;
     if (!pool_alloc(c, &rows, (sizeof(tl::RowC) + sizeof(int)) * (size_t)chunk, st)) return TL_ENOMEM;   // + a tile-queue head per row
@@ -1178,7 +1190,7 @@ int tl_loglike_linear_batch(tl_ctx *c, const float *params, int64_t B, float *lo
     cudaMemsetAsync(ext, 0, ext_row * (size_t)chunk, st);      // pitch padding must read as finite zeros
     const int64_t rows_per_lens = B / c->cfg.n_lens;
     int rc = TL_OK;
-    for (int64_t r0 = 0; r0 < B && rc == TL_OK; r0 += chunk) {
+    for (int64_t r0 = r_begin; r0 < B && rc == TL_OK; r0 += chunk) {
         const int64_t nb = (B - r0 < chunk) ? (B - r0) : chunk;
         tl::PrologueArgs pa;
         fill_prologue_args(c, pa, params, rows, nb, r0, rows_per_lens, 1);
