@@ -768,6 +768,9 @@ def main():
     ap.add_argument("--sub-batch", type=int, default=4096, help="rows per sub-batch when --streams > 1")
     ap.add_argument("--peaks", action="store_true",
                     help="run the pipe micro-benchmarks (tl_measure_peaks: FFMA, FFMA2, MUFU, DFMA and mixes) and exit")
+    ap.add_argument("--all-configs", action="store_true",
+                    help="one JSON line per BASELINE.json config (0..4), each from a run of this script with --config i "
+                         "(config 4: 2 steps); the other options are passed on")
     ap.add_argument("--serve", action="store_true",
                     help="latency of 1..16-row requests through the persistent serving kernel (tl_serve_eval) and exit")
     args = ap.parse_args()
@@ -776,6 +779,14 @@ def main():
         return
     if args.serve:
         run_serve(args)
+        return
+    if args.all_configs:
+        import subprocess
+        rest = [x for x in sys.argv[1:] if x != "--all-configs"]
+        for i in range(5):
+            cmd = [sys.executable, os.path.abspath(__file__), "--config", str(i), "--no-cpu-baseline"] + rest + (["--steps", "2"] if i == 4 else [])
+            out = subprocess.run(cmd, stdout=subprocess.PIPE, text=True).stdout.strip().splitlines()
+            print(out[-1] if out else json.dumps({"config": i, "error": "no output"}), flush=True)
         return
     w = W.workload(args.config)
     if args.mass == "epl":
