@@ -86,6 +86,7 @@ struct tl_ctx {
     int sb_rowtab = 0, sb_max_rows = 0;
     // MGE mode (tl_set_mge / tl_loglike_mge_batch)
     float *mge_c = nullptr;       // device [n_gauss]: log2(e) / (2 sigma_k^2)
+    double *mge_c64 = nullptr;    // the same in FP64, for the FP64 pipeline (a float coefficient is 6e-8 off: 3e-7 in the profile at 3 sigma)
     int *mge_set = nullptr;       // device [n_gauss]: the set each Gaussian belongs to
     int n_gauss = 0, mge_n_sets = 0, mge_per_set[tl::MGE_MAX_SETS] = {0, 0};
     void (*mge_trace)(const tl::KArgs, int) = nullptr;   // sources only: trace_kernel<S,0,1> or trace_lin_kernel<S,0,2>
@@ -1247,19 +1248,23 @@ int tl_set_mge_sets(tl_ctx *c, const float *sigmas, const int32_t *n_per_set, in
     if (n_gauss > tl::MGE_MAX_GAUSS) return TL_EINVAL;
     if (!c->trace_lin) return TL_ESIZE;
     float ck[tl::MGE_MAX_GAUSS];
+    double ck64[tl::MGE_MAX_GAUSS];
     int set_of[tl::MGE_MAX_GAUSS];
     for (int k = 0, j = 0, left = n_per_set[0]; k < n_gauss; ++k, --left) {
         while (left == 0) left = n_per_set[++j];
         set_of[k] = j;
         if (!std::isfinite(sigmas[k]) || !(sigmas[k] > 0.f)) return TL_EINVAL;
-        ck[k] = (float)(1.4426950408889634074 / (2.0 * (double)sigmas[k] * (double)sigmas[k]));
+        ck64[k] = 1.4426950408889634074 / (2.0 * (double)sigmas[k] * (double)sigmas[k]);
+        ck[k] = (float)ck64[k];
         if (!std::isfinite(ck[k])) return TL_EINVAL;
     }
     DeviceGuard guard(c->device);
     if (!guard.ok) return TL_ECUDA;
     if (!c->mge_c && (!cuda_ok(cudaMalloc(&c->mge_c, sizeof(float) * tl::MGE_MAX_GAUSS)) ||
+                      !cuda_ok(cudaMalloc(&c->mge_c64, sizeof(double) * tl::MGE_MAX_GAUSS)) ||
                       !cuda_ok(cudaMalloc(&c->mge_set, sizeof(int) * tl::MGE_MAX_GAUSS)))) return TL_ENOMEM;
     if (!cuda_ok(cudaMemcpy(c->mge_c, ck, sizeof(float) * n_gauss, cudaMemcpyHostToDevice)) ||
+        !cuda_ok(cudaMemcpy(c->mge_c64, ck64, sizeof(double) * n_gauss, cudaMemcpyHostToDevice)) ||
         !cuda_ok(cudaMemcpy(c->mge_set, set_of, sizeof(int) * n_gauss, cudaMemcpyHostToDevice))) return TL_ECUDA;
     c->mge_n_sets = n_sets;
     for (int j = 0; j < tl::MGE_MAX_SETS; ++j) c->mge_per_set[j] = j < n_sets ? n_per_set[j] : 0;
@@ -1358,7 +1363,7 @@ int run_mge_dp(tl_ctx *c, const float *params, int64_t B, float *logL, float *am
         d.params = params; d.rows = rowsd; d.n_rows = (int)nb; d.row0 = r0; d.rows_per_lens = rows_per_lens;
         d.psf = c->psf; d.data = c->data; d.wgt64 = c->wgt64; d.lconst = c->lconst;
         d.ext = ext; d.m64 = m64; d.logL = logL; d.amps = amps; d.lin = 1; d.mge = 1;
-        d.ext_nc = NC; d.ext_k0 = NG; d.n_gauss = NG; d.n_source = NS; d.mge_c = c->mge_c; d.mge_set = c->mge_set;
+        d.ext_nc = NC; d.ext_k0 = NG; d.n_gauss = NG; d.n_source = NS; d.mge_c = c->mge_c64; d.mge_set = c->mge_set;
         d.P = c->P; d.ny = c->cfg.ny; d.nx = c->cfg.nx; d.K = c->K; d.Kp = c->Kp; d.h = c->h;
         d.He = c->He; d.We = c->We; d.Wp = c->dp_Wp; d.S = c->cfg.supersample;
         d.n_lens_light = c->cfg.n_lens_light; d.n_comp = c->n_comp;
@@ -1632,7 +1637,7 @@ void tl_destroy(tl_ctx *c)
     }
     if (c->s_up) cudaStreamDestroy(c->s_up);
     if (c->s_down) cudaStreamDestroy(c->s_down);
-    cudaFree(c->mge_c); cudaFree(c->mge_set); cudaFree(c->canary_errors);
+    cudaFree(c->mge_c); cudaFree(c->mge_c64); cudaFree(c->mge_set); cudaFree(c->canary_errors);
     cudaFree(c->psf); cudaFree(c->data); cudaFree(c->wgt); cudaFree(c->wgt64); cudaFree(c->noise); cudaFree(c->sigma_min); cudaFree(c->lconst);
     if (c->pool) cudaMemPoolDestroy(c->pool);
     delete c;

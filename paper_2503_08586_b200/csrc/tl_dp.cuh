@@ -80,7 +80,7 @@ struct DpArgs {
     // shapes of the Gaussian sets (r_e := 1: t = R_p^2 in arcsec^2); ext / m64 have ext_nc = n_gauss + n_source
     // components per row, the ray-traced sources from slot ext_k0 = n_gauss on
     int mge, ext_nc, ext_k0, n_gauss, n_source;
-    const float *mge_c;          // [n_gauss] log2(e) / (2 sigma_k^2)
+    const double *mge_c;         // [n_gauss] log2(e) / (2 sigma_k^2), FP64
     const int *mge_set;          // [n_gauss] set of Gaussian k
     int P, ny, nx, K, Kp, h, He, We, Wp, S, n_lens_light, n_comp, edge_zero, mass_model, lens_np;
     int band_rows, n_bands;
@@ -440,7 +440,7 @@ __global__ void __launch_bounds__(256) gauss_dp_kernel(const DpArgs a)
     for (int w = blockIdx.y * blockDim.x + threadIdx.x; w < npx * a.n_gauss; w += gridDim.y * blockDim.x) {
         const int k = w / npx, pix = w - k * npx, i = pix / a.We, j = pix - i * a.We;
         const CompD &C = R.comp[a.n_source + a.mge_set[k]];
-        const double ck = -(double)a.mge_c[k];
+        const double ck = -a.mge_c[k];
         double acc = 0.0;
         const bool edge = a.edge_zero && (j < a.h || j >= a.We - a.h || i < a.h || i >= a.He - a.h);
         if (!edge) {

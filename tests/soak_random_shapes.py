@@ -1,7 +1,8 @@
 """Soak run (not collected by pytest): `python tests/soak_random_shapes.py FIRST LAST` drives seeds FIRST .. LAST-1 of a
 seeded random geometry (3..69 pixels a side, S = 1..8, PSF 1..31, one or two sources, with / without lens light,
 both edge modes, a quarter of them EPL) through tl_loglike_batch and tl_render_batch in the FP32, FP64 and AUTO modes
-and through tl_loglike_linear_batch, with tl_options.debug_canaries on: every result against the oracle (pixels to
+and through tl_loglike_linear_batch and (with a lens-light block) tl_loglike_mge_batch in FP32 and FP64, with
+tl_options.debug_canaries on: every result against the oracle (pixels to
 1e-5 of the peak; logL to north_star in FP64 / AUTO, to 60 x north_star in FP32 -- the FP32 floor of small images,
 DESIGN.md 6), one row alone against the same row in the batch (same bits), the finite / -inf pattern, 0 guard words
 changed.  Prints the seeds that fail.  tests/test_parity_gpu.py::test_random_shapes is the 12-seed version of it."""
@@ -56,6 +57,20 @@ for seed in range(s0, s1):
             fl = np.isfinite(ol)
             rl = np.abs(l1.cpu().numpy().astype(np.float64)[fl] - ol[fl]) / PT.logl_tol(ol)[fl]
             assert (rl.max() if rl.size else 0.0) <= 60.0, ("linear", rl.max())
+        if w.n_lens_light == 1 and min(ny, nx) >= 8:
+            # MGE lens light: 2..8 Gaussians + the sources by NNLS, FP32 and FP64 pipelines
+            sig = W.mge_sigmas(w, int(rng.integers(2, 9)))
+            ctx.set_mge(sig)
+            om, _ = O.loglike_mge_batch(O.config_of(w), prob.psf, prob.data, prob.noise, rows, sig)
+            fm = np.isfinite(om)
+            for prec, lim in ((api.TL_PRECISION_FP32, 60.0), (api.TL_PRECISION_FP64, 1.0)):
+                ctx.set_precision(prec)
+                lm, _ = ctx.loglike_mge(d)
+                lm = lm.cpu().numpy().astype(np.float64)
+                assert np.array_equal(np.isfinite(lm), fm), ("mge finite pattern", prec)
+                rm = np.abs(lm[fm] - om[fm]) / PT.logl_tol(om)[fm]
+                assert (rm.max() if rm.size else 0.0) <= lim, ("mge", prec, rm.max())
+            ctx.set_precision(api.TL_PRECISION_FP32)
         assert ctx.canary_errors() == 0, "canary"
         ctx.close()
     except Exception as e:
