@@ -1,6 +1,6 @@
 """Soak run (not collected by pytest): `python tests/soak_random_shapes.py FIRST LAST` drives seeds FIRST .. LAST-1 of a
 seeded random geometry (3..69 pixels a side, S = 1..8, PSF 1..31, one or two sources, with / without lens light,
-both edge modes, a quarter of them EPL) through tl_loglike_batch and tl_render_batch in the FP32, FP64 and AUTO modes
+both edge modes, a quarter of them EPL, one to three lenses per call, a third forced onto the split path) through tl_loglike_batch and tl_render_batch in the FP32, FP64 and AUTO modes
 and through tl_loglike_linear_batch and (with a lens-light block) tl_loglike_mge_batch in FP32 and FP64, with
 tl_options.debug_canaries on: every result against the oracle (pixels to
 1e-5 of the peak; logL to north_star in FP64 / AUTO, to 60 x north_star in FP32 -- the FP32 floor of small images,
@@ -28,10 +28,14 @@ for seed in range(s0, s1):
     try:
         w = W.Workload(**kw)
         if rng.integers(0, 4) == 0: w = w.with_epl()
+        n_lens = int(rng.choice([1, 1, 2, 3]))                     # several lenses share a call (own PSF / data / noise each)
+        if n_lens > 1: w = w.scaled(batch=8 * n_lens, n_lens=n_lens)
+        opts = {"debug_canaries": 1}
+        if rng.integers(0, 3) == 0: opts["force_split"] = 1        # the split path (large images) on a small one
         prob = W.make_problem(w, O.render_for_workloads)
         rows, isnear = PT.rows_with_near(W, w, prob, 6, 2)
         oll, oim = PT.oracle_reference(O, w, prob, rows)
-        ctx = api.LensContext.from_problem(prob, options={"debug_canaries": 1})
+        ctx = api.LensContext.from_problem(prob, options=opts)
         d = torch.from_numpy(np.ascontiguousarray(rows)).cuda()
         tol = PT.logl_tol(oll)
         fin = np.isfinite(oll)
@@ -47,13 +51,13 @@ for seed in range(s0, s1):
             lim = 1.0 if prec != api.TL_PRECISION_FP32 else 60.0
             assert (r.max() if r.size else 0.0) <= lim, ("logL", prec, r.max())
             # one row alone = the same bits (FP32: small-batch / fused; the others: same path)
-            if prec == api.TL_PRECISION_FP32:
+            if prec == api.TL_PRECISION_FP32 and w.n_lens == 1:
                 one = ctx.loglike(d[:1].contiguous()).cpu().numpy().astype(np.float64)
                 assert np.array_equal(one, ll[:1], equal_nan=True), ("batch independence", one, ll[:1])
         ctx.set_precision(api.TL_PRECISION_FP32)
         if w.n_lens_light <= 1:
             l1, a1 = ctx.loglike_linear(d)
-            ol, oa = O.loglike_linear_batch(O.config_of(w), prob.psf, prob.data, prob.noise, rows)
+            ol, oa = O.loglike_linear_batch(O.config_of(w), prob.psf, prob.data, prob.noise, rows, n_lens=w.n_lens)
             fl = np.isfinite(ol)
             rl = np.abs(l1.cpu().numpy().astype(np.float64)[fl] - ol[fl]) / PT.logl_tol(ol)[fl]
             assert (rl.max() if rl.size else 0.0) <= 60.0, ("linear", rl.max())
@@ -61,7 +65,7 @@ for seed in range(s0, s1):
             # MGE lens light: 2..8 Gaussians + the sources by NNLS, FP32 and FP64 pipelines
             sig = W.mge_sigmas(w, int(rng.integers(2, 9)))
             ctx.set_mge(sig)
-            om, _ = O.loglike_mge_batch(O.config_of(w), prob.psf, prob.data, prob.noise, rows, sig)
+            om, _ = O.loglike_mge_batch(O.config_of(w), prob.psf, prob.data, prob.noise, rows, sig, n_lens=w.n_lens)
             fm = np.isfinite(om)
             for prec, lim in ((api.TL_PRECISION_FP32, 60.0), (api.TL_PRECISION_FP64, 1.0)):
                 ctx.set_precision(prec)
