@@ -1,7 +1,7 @@
 """Soak run (not collected by pytest): `python tests/soak_random_shapes.py FIRST LAST` drives seeds FIRST .. LAST-1 of a
 seeded random geometry (3..69 pixels a side, S = 1..8, PSF 1..31, one or two sources, with / without lens light,
 both edge modes, a quarter of them EPL, one to three lenses per call, a third forced onto the split path) through tl_loglike_batch and tl_render_batch in the FP32, FP64 and AUTO modes
-and through tl_loglike_linear_batch and (with a lens-light block) tl_loglike_mge_batch in FP32 and FP64, with
+and through tl_loglike_linear_batch and (with a lens-light block) tl_loglike_mge_batch (one set, and on a third of those shapes two sets) in FP32 and FP64, with
 tl_options.debug_canaries on: every result against the oracle (pixels to
 1e-5 of the peak; logL to north_star in FP64 / AUTO, to 60 x north_star in FP32 -- the FP32 floor of small images,
 DESIGN.md 6), one row alone against the same row in the batch (same bits), the finite / -inf pattern, 0 guard words
@@ -79,6 +79,25 @@ for seed in range(s0, s1):
             ctx.set_precision(api.TL_PRECISION_FP32)
         assert ctx.canary_errors() == 0, "canary"
         ctx.close()
+        if w.n_lens_light == 1 and w.n_lens == 1 and min(ny, nx) >= 8 and rng.integers(0, 3) == 0:
+            # two Gaussian sets on ellipses of their own (two lens-light blocks in the row), the data of the one-set problem
+            w2 = W.Workload(**{**w.__dict__, "n_lens_light": 2})
+            rows2 = W.batch_rows(w2, 6)
+            sets = [W.mge_sigmas(w2, int(rng.integers(2, 7))), (W.mge_sigmas(w2, int(rng.integers(2, 7))) * 1.3).astype(np.float32)]
+            prob2 = type(prob)(w2, prob.psf, prob.data, prob.noise, rows2[:1].copy())
+            ctx2 = api.LensContext.from_problem(prob2, options=opts)
+            ctx2.set_mge_sets(sets)
+            d2 = torch.from_numpy(np.ascontiguousarray(rows2)).cuda()
+            o2 = np.array([O.loglike_mge_sets(O.config_of(w2), prob.psf[0], prob.data[0], prob.noise[0], rows2[r], sets)[0] for r in range(len(rows2))])
+            f2 = np.isfinite(o2)
+            for prec, lim in ((api.TL_PRECISION_FP32, 60.0), (api.TL_PRECISION_FP64, 1.0)):
+                ctx2.set_precision(prec)
+                l2 = ctx2.loglike_mge(d2)[0].cpu().numpy().astype(np.float64)
+                assert np.array_equal(np.isfinite(l2), f2), ("mge sets finite pattern", prec)
+                r2 = np.abs(l2[f2] - o2[f2]) / PT.logl_tol(o2)[f2]
+                assert (r2.max() if r2.size else 0.0) <= lim, ("mge sets", prec, r2.max())
+            assert ctx2.canary_errors() == 0, "canary (sets)"
+            ctx2.close()
     except Exception as e:
         bad += 1
         print("SEED %d FAILED: %r  kw=%r" % (seed, e, kw), flush=True)
