@@ -3,7 +3,7 @@ shapes (40..120 pixels a side, S = 2 / 4, PSF 5 / 15 / 21, SIE, one lens: the sh
 tail routing of the last wave, tl_loglike_batch_noalloc and the serving kernel are all available) the value of a row
 must not depend on how it is asked for: a 310-row call is the reference, and calls of 1, 5, 17, 74, 75, 149 and 200 of
 its rows, the allocation-free entry point and served requests of 1, 3 and 16 rows must return the same bits; the
-linear-amplitude mode likewise for 1, 17, 149 and 200 rows.  With tl_options.debug_canaries on; prints the seeds that fail."""
+linear-amplitude mode likewise for 1, 17, 149 and 200 rows, the MGE mode for 1, 7 and 74 rows against 200.  With tl_options.debug_canaries on; prints the seeds that fail."""
 import os
 import sys
 import traceback
@@ -40,6 +40,12 @@ for seed in range(s0, s1):
         for B in (1, 17, 149, 200):
             gl, ga = ctx.loglike_linear(d[:B].contiguous())
             assert torch.equal(gl, refl[:B]) and torch.equal(torch.nan_to_num(ga, nan=-7.0), torch.nan_to_num(refa[:B], nan=-7.0)), ("linear", B)
+        if w.n_lens_light == 1:                                   # MGE: a few rows (bands of gauss_conv_kernel, thin tiles) against many
+            ctx.set_mge(W.mge_sigmas(w, int(rng.integers(3, 11))))
+            rm, ra = ctx.loglike_mge(d[:200].contiguous())
+            for B in (1, 7, 74):
+                gm, ga = ctx.loglike_mge(d[:B].contiguous())
+                assert torch.equal(gm, rm[:B]) and torch.equal(torch.nan_to_num(ga, nan=-7.0), torch.nan_to_num(ra[:B], nan=-7.0)), ("mge", B)
         torch.cuda.synchronize()
         refh = ref.cpu().numpy()
         ctx.serve_start(16, 0.5)
